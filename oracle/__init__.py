@@ -1,0 +1,224 @@
+"""ctypes wrapper of the CPU oracle (oracle/oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference`
+legs may import this package.  It imports nothing from paper_2507_08578_b200 and the
+product never imports it.  All arithmetic is in oracle.c; this file marshals numpy arrays.
+
+`cfg` arguments are the dicts of synth.make_config (input data only).
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+BUILD_CMD = ["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+             _SRC, "-o", _LIB, "-lm"]
+
+
+def build(force=False):
+    """Compile oracle.c -> liboracle.so (in-tree, git-ignored) if missing or stale."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        cmd = list(BUILD_CMD)
+        cmd[cmd.index(_LIB)] = tmp
+        subprocess.check_call(cmd)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_sphere.restype = C.c_int64
+        _lib.orc_kin.restype = C.c_double
+        _lib.orc_spline.restype = C.c_double
+        _lib.orc_ylm.restype = C.c_double
+        _lib.orc_max_q.restype = C.c_double
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _d(a):
+    return a.ctypes.data_as(_dp) if a is not None else None
+
+
+def _i(a):
+    return a.ctypes.data_as(_ip) if a is not None else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def num_threads():
+    return lib().orc_num_threads()
+
+
+def set_num_threads(n):
+    lib().orc_set_num_threads(int(n))
+
+
+# ---------------------------------------------------------------- lattice / sphere
+def lattice(rprimd):
+    bm = np.zeros(9); gm = np.zeros(9)
+    lib().orc_lattice(_d(_f64(rprimd).ravel()), _d(bm), _d(gm))
+    return bm.reshape(3, 3), gm.reshape(3, 3)
+
+
+def kin_of(rprimd, k, m):
+    _, gm = lattice(rprimd)
+    return lib().orc_kin(_d(gm.ravel()), _d(_f64(k)), C.c_int(int(m[0])), C.c_int(int(m[1])), C.c_int(int(m[2])))
+
+
+def sphere(rprimd, k, ecut, ngfft):
+    """Brute-force sphere: returns (kg[npw,3] int32, igfft[npw] int32, kin[npw] float64)."""
+    r = _f64(rprimd).ravel(); kk = _f64(k); n = _i32(ngfft)
+    npw = lib().orc_sphere(_d(r), _d(kk), C.c_double(ecut), _i(n), None, None, None, C.c_int64(0))
+    kg = np.zeros((npw, 3), np.int32); ig = np.zeros(npw, np.int32); kin = np.zeros(npw)
+    lib().orc_sphere(_d(r), _d(kk), C.c_double(ecut), _i(n), _i(kg), _i(ig), _d(kin), C.c_int64(npw))
+    return kg, ig, kin
+
+
+def sphere_extent(rprimd, k, ecut, ngfft):
+    mn = np.zeros(3, np.int32); mx = np.zeros(3, np.int32)
+    fits = lib().orc_sphere_extent(_d(_f64(rprimd).ravel()), _d(_f64(k)), C.c_double(ecut), _i(_i32(ngfft)), _i(mn), _i(mx))
+    return bool(fits), mn, mx
+
+
+# ---------------------------------------------------------------- transforms
+def dft1d(x, sign, method):
+    x = np.ascontiguousarray(x, np.complex128); out = np.zeros_like(x)
+    lib().orc_dft1d(C.c_int(len(x)), C.c_int(sign), C.c_int(method), _d(x.view(np.float64)), _d(out.view(np.float64)))
+    return out
+
+
+def dft3d(box, sign, method):
+    """box[n3][n2][n1] complex -> transformed copy (no scaling)."""
+    b = np.array(box, dtype=np.complex128, order="C")
+    n = _i32(b.shape[::-1])
+    lib().orc_dft3d(_i(n), C.c_int(sign), C.c_int(method), _d(b.view(np.float64)))
+    return b
+
+
+def g2r(ngfft, igfft, c, method=2):
+    n = _i32(ngfft); c = np.ascontiguousarray(c, np.complex128)
+    box = np.zeros((n[2], n[1], n[0]), np.complex128)
+    lib().orc_g2r(_i(n), C.c_int64(len(igfft)), _i(_i32(igfft)), _d(c.view(np.float64)), C.c_int(method), _d(box.view(np.float64)))
+    return box
+
+
+def vtilde(V):
+    V = _f64(V); n = _i32(V.shape[::-1]); out = np.zeros(V.shape, np.complex128)
+    lib().orc_vtilde(_i(n), _d(V), _d(out.view(np.float64)))
+    return out
+
+
+# ---------------------------------------------------------------- projectors
+def spline(f, f2, dq, q):
+    f = _f64(f); f2 = _f64(f2)
+    return lib().orc_spline(C.c_int(len(f)), C.c_double(dq), _d(f), _d(f2), C.c_double(q))
+
+
+def ylm(l, m, v):
+    return lib().orc_ylm(C.c_int(l), C.c_int(m), C.c_double(v[0]), C.c_double(v[1]), C.c_double(v[2]))
+
+
+class _Proj:
+    """Flattened per-type projector metadata in the padded layout oracle.c expects."""
+
+    def __init__(self, cfg, ik):
+        ty = cfg["types"]
+        self.keep = []
+        self.lmax = cfg["nlmn_max"]; self.ntypat = len(ty)
+        self.nrad_max = max(t["nrad"] for t in ty); self.nq_max = max(t["nq"] for t in ty)
+        self.nlmn = _i32([t["nlmn"] for t in ty])
+        self.l = np.zeros((self.ntypat, self.lmax), np.int32); self.m = self.l.copy(); self.ir = self.l.copy()
+        self.f = np.zeros((self.ntypat, self.nrad_max, self.nq_max)); self.f2 = self.f.copy()
+        for t, T in enumerate(ty):
+            self.l[t, :T["nlmn"]] = T["l"]; self.m[t, :T["nlmn"]] = T["m"]; self.ir[t, :T["nlmn"]] = T["irad"]
+            self.f[t, :T["nrad"], :T["nq"]] = T["f"]; self.f2[t, :T["nrad"], :T["nq"]] = T["f2"]
+        self.nq = _i32([t["nq"] for t in ty]); self.dq = _f64([t["dq"] for t in ty])
+        self.rprimd = _f64(cfg["rprimd"]).ravel(); self.k = _f64(cfg["kpt"][ik])
+        self.typat = _i32(cfg["typat"]); self.xred = _f64(cfg["xred"]).ravel()
+        self.natom = cfg["natom"]
+
+    def args(self):
+        return (_d(self.rprimd), _d(self.k), C.c_int(self.natom), _i(self.typat), _d(self.xred),
+                C.c_int(self.ntypat), C.c_int(self.lmax), _i(self.nlmn), _i(self.l), _i(self.m), _i(self.ir),
+                C.c_int(self.nrad_max), C.c_int(self.nq_max), _i(self.nq), _d(self.dq), _d(self.f), _d(self.f2))
+
+
+def projector_table(cfg, ik, kg):
+    """P[nproj][npw] complex128 (materialised; small cases only)."""
+    P = _Proj(cfg, ik); kg = _i32(kg)
+    out = np.zeros((cfg["nproj"], len(kg)), np.complex128)
+    lib().orc_projector_table(*P.args(), C.c_int64(len(kg)), _i(kg), _d(out.view(np.float64)))
+    return out
+
+
+def max_q(cfg, ik, kg):
+    kg = _i32(kg)
+    return lib().orc_max_q(_d(_f64(cfg["rprimd"]).ravel()), _d(_f64(cfg["kpt"][ik])), C.c_int64(len(kg)), _i(kg))
+
+
+def nonlocal_apply(cfg, ik, kg, psi, dij=None, want_cprj=False):
+    """V_nl psi for psi[nband][npw]; returns out (and cprj[nproj][nband] if asked)."""
+    P = _Proj(cfg, ik); kg = _i32(kg)
+    psi = np.ascontiguousarray(psi, np.complex128); nb, ld = psi.shape
+    out = np.zeros_like(psi)
+    dij = _f64(cfg["dij"] if dij is None else dij)
+    cp = np.zeros((cfg["nproj"], nb), np.complex128) if want_cprj else None
+    lib().orc_nonlocal_apply(*P.args(), _d(dij), C.c_int64(len(kg)), _i(kg), C.c_int(nb), C.c_int64(ld),
+                             _d(psi.view(np.float64)), _d(out.view(np.float64)),
+                             _d(cp.view(np.float64)) if want_cprj else None)
+    return (out, cp) if want_cprj else out
+
+
+# ---------------------------------------------------------------- whole operator
+KIN, LOC, NL, ALL = 1, 2, 4, 7
+
+
+def apply_h(cfg, ik, kg, igfft, kin, psi, method=2, terms=ALL, vloc=None, dij=None):
+    """H psi for psi[nband][ld] (ld >= npw; columns >= npw ignored and returned as 0)."""
+    P = _Proj(cfg, ik); kg = _i32(kg); igfft = _i32(igfft); kin = _f64(kin)
+    psi = np.ascontiguousarray(psi, np.complex128); nb, ld = psi.shape
+    V = _f64(cfg["vloc"] if vloc is None else vloc)
+    dij = _f64(cfg["dij"] if dij is None else dij)
+    n = _i32(cfg["ngfft"]); out = np.zeros_like(psi)
+    lib().orc_apply_h(*P.args(), _d(dij), _i(n), _d(V), C.c_int64(len(kg)), _i(kg), _i(igfft), _d(kin),
+                      C.c_int(nb), C.c_int64(ld), _d(psi.view(np.float64)), _d(out.view(np.float64)),
+                      C.c_int(method), C.c_int(terms))
+    return out
+
+
+def dense_h(cfg, ik, kg, kin, terms=ALL, vloc=None, dij=None):
+    """T0: explicit H[npw][npw] complex128 in the plane-wave basis."""
+    P = _Proj(cfg, ik); kg = _i32(kg); kin = _f64(kin)
+    V = _f64(cfg["vloc"] if vloc is None else vloc)
+    dij = _f64(cfg["dij"] if dij is None else dij)
+    n = _i32(cfg["ngfft"]); npw = len(kg)
+    H = np.zeros((npw, npw), np.complex128)
+    lib().orc_dense_h(*P.args(), _d(dij), _i(n), _d(V), C.c_int64(npw), _i(kg), _d(kin), C.c_int(terms),
+                      _d(H.view(np.float64)))
+    return H
+
+
+def dense_matvec(H, x):
+    H = np.ascontiguousarray(H, np.complex128); x = np.ascontiguousarray(x, np.complex128)
+    y = np.zeros_like(x)
+    lib().orc_dense_matvec(C.c_int64(len(x)), _d(H.view(np.float64)), _d(x.view(np.float64)), _d(y.view(np.float64)))
+    return y

@@ -1,0 +1,67 @@
+"""Whole-operator pins of the oracle (SURVEY.md 8(c) "Whole operator" row)."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from util import config, sphere, rel_err, rand_c
+
+
+@pytest.mark.parametrize("name,ik", [("c0", 0), ("aniso", 0), ("c3k2", 1), ("c1m", 0), ("c2m", 0), ("c4m", 0)])
+def test_dense_h_equals_fft_path_and_is_hermitian(name, ik):
+    c = config(name); kg, ig, kin = sphere(name, ik)
+    psi = synth.gen_psi(c, [sphere(name, j)[2] for j in range(c["nkpt"])])[ik]
+    H = oracle.dense_h(c, ik, kg, kin)
+    assert abs(H - H.conj().T).max() < 1e-13 * abs(H).max()
+    ref = np.array([oracle.dense_matvec(H, p[:len(kg)]) for p in psi])
+    for method in (1, 2):
+        got = oracle.apply_h(c, ik, kg, ig, kin, psi, method=method)
+        assert rel_err(got[:, :len(kg)], ref) < 1e-12
+        assert np.all(got[:, len(kg):] == 0)
+
+
+def test_hermiticity_linearity_permutation_batching():
+    c = config("c1m"); kg, ig, kin = sphere("c1m")
+    x = rand_c((4, len(kg)), 11)
+    h = oracle.apply_h(c, 0, kg, ig, kin, x)
+    # <phi|H psi> = <H phi|psi> = conj(<psi|H phi>)
+    a = np.vdot(x[0], h[1]); b = np.vdot(h[0], x[1]); d = np.conj(np.vdot(x[1], h[0]))
+    assert abs(a - b) < 1e-12 * abs(a) and abs(a - d) < 1e-12 * abs(a)
+    lin = oracle.apply_h(c, 0, kg, ig, kin, (2.5 * x[0] - 1j * x[2])[None])[0]
+    assert rel_err(lin, 2.5 * h[0] - 1j * h[2]) < 1e-13
+    perm = [2, 0, 3, 1]
+    assert rel_err(oracle.apply_h(c, 0, kg, ig, kin, x[perm]), h[perm]) < 1e-14
+    assert rel_err(oracle.apply_h(c, 0, kg, ig, kin, x[1:2]), h[1:2]) < 1e-14
+
+
+def test_translation_covariance():
+    """Shift atoms and V by a grid vector tau, multiply c(m) by exp(-2 pi i (k+m).tau):
+    (H psi)(m) picks up the same phase.  Exercises sphere, wrap, structure factors and D_ij at once."""
+    c = dict(config("aniso")); kg, ig, kin = sphere("aniso")
+    n1, n2, n3 = c["ngfft"]
+    s = np.array([3, -5, 7]); tau = s / np.array([n1, n2, n3])
+    psi = rand_c((2, len(kg)), 13)
+    h = oracle.apply_h(c, 0, kg, ig, kin, psi)
+    c2 = dict(c)
+    c2["xred"] = c["xred"] + tau
+    c2["vloc"] = np.roll(c["vloc"], shift=(s[2], s[1], s[0]), axis=(0, 1, 2))
+    ph = np.exp(-2j * np.pi * ((kg + c["kpt"][0]) @ tau))
+    h2 = oracle.apply_h(c2, 0, kg, ig, kin, psi * ph)
+    assert rel_err(h2, h * ph) < 1e-13
+
+
+def test_term_isolation_adds_up():
+    c = config("c0"); kg, ig, kin = sphere("c0")
+    x = rand_c((2, len(kg)), 17)
+    parts = sum(oracle.apply_h(c, 0, kg, ig, kin, x, terms=t) for t in (oracle.KIN, oracle.LOC, oracle.NL))
+    assert rel_err(parts, oracle.apply_h(c, 0, kg, ig, kin, x)) < 1e-14
+
+
+def test_generator_is_chunk_independent():
+    c = config("c0"); kg, ig, kin = sphere("c0")
+    full = synth.gen_psi(c, [kin])
+    some = synth.gen_psi(c, [kin], bands=[5, 2])
+    assert np.array_equal(some[0, 0], full[0, 5]) and np.array_equal(some[0, 1], full[0, 2])
+    assert abs(np.std(full.real * (1 + 2 * kin)) - 1) < 0.1
+    d = c["dij"]
+    assert np.array_equal(d, d.transpose(0, 2, 1))

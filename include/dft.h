@@ -1,0 +1,142 @@
+/* dft.h -- C ABI of libdftb200: the plane-wave Kohn-Sham Hamiltonian applied to a block of bands
+ *
+ *      H|psi> = 1/2|k+G|^2 psi + FFT^-1[ V_loc(r) . FFT[psi] ] + sum_a sum_ij |p_a,i> D^a_ij <p_a,j|psi>
+ *
+ * on one NVIDIA B200 (sm_100a), FP64.  The operator is the one the ABINIT 2025 paper offloads in
+ * its SCF loop (Sec. V: ":456 applying the Hamiltonian to a set of vectors"; the three
+ * terms and their cost at :475; the non-local operator is Eq. 26 at :470; "multiple concurrent
+ * Fourier transforms using an array of wave functions" at :436).  The paper prints no interface;
+ * the entry points follow BASELINE.json `north_star` (dft_plan_create / dft_set_vloc /
+ * dft_apply_h) in the concrete form of SURVEY.md section 8(b).  Conventions the paper is silent
+ * on are the numbered "readings" of DESIGN.md section 3.
+ *
+ * General rules
+ *   - every call returns a status code (0 = DFT_OK, negative = error); nothing throws or aborts
+ *     across the boundary; on error, output arguments are left untouched and dft_last_error()
+ *     holds a message (thread-local).
+ *   - reals are double; complex numbers are interleaved (re, im) doubles; sizes are int32/int64.
+ *   - "host" / "device" is stated for every pointer.  Host arrays are copied during the call and
+ *     may be freed afterwards.  Device arrays stay owned by the caller.
+ *   - no CPU fallback exists: without a CUDA device every call that needs one returns DFT_ERR_CUDA.
+ *   - a plan may be used from one host thread and one stream at a time.
+ */
+#ifndef DFT_B200_H
+#define DFT_B200_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dft_plan dft_plan; /* opaque; owns its device buffers */
+
+enum {
+  DFT_OK = 0,
+  DFT_ERR_INVALID_ARG = -1,    /* null pointer, non-positive size, bad l/m/irad, singular lattice ... */
+  DFT_ERR_GRID_TOO_SMALL = -2, /* some sphere point violates -floor(n/2) <= m <= floor((n-1)/2)     */
+  DFT_ERR_TABLE_RANGE = -3,    /* max |k+G| exceeds (nq-1)*dq of a radial table                    */
+  DFT_ERR_ALLOC = -4,          /* host or device allocation failed / workspace too small           */
+  DFT_ERR_CUDA = -5,           /* CUDA runtime / driver error (message in dft_last_error)          */
+  DFT_ERR_NOT_READY = -6,      /* dft_apply_h before dft_set_vloc                                  */
+  DFT_ERR_UNSUPPORTED = -7     /* FFT length with a prime factor > 5, l > 2, ...                   */
+};
+
+/* One atom type's non-local projectors (Eq. 26, PAPER.md :470; readings 6-9).  All
+ * pointers are HOST memory, copied by dft_plan_create.
+ *   projector i (0 <= i < nlmn) has angular momentum l[i] in 0..2, real-harmonic index m[i] in
+ *   -l..l and radial function irad[i] in 0..nrad-1.
+ *   radial function r is tabulated on the uniform grid q_j = j*dq, j = 0..nq-1 as the cubic-
+ *   spline pair f[r*nq + j] (values) and f2[r*nq + j] (second derivatives).                       */
+typedef struct {
+  int32_t nlmn;
+  const int32_t *l, *m, *irad; /* [nlmn]      */
+  int32_t nrad, nq;
+  double dq;
+  const double *f, *f2;        /* [nrad][nq]  */
+} dft_proj_table;
+
+/* Build a plan: the G-sphere of every k-point (S_k = {m : 1/2|k+G|^2 <= ecut}, ascending FFT-box
+ * index; readings 1-3), the pruned-FFT schedules, and the materialised projector table
+ * P[a,i](G) = F(|q|) Y_lm(q^) exp(-2 pi i (k+m).x_a) in device memory ("computed and stored in
+ * memory", PAPER.md :479).  All pointer arguments are HOST memory.
+ *   rprimd[9]   row i = lattice vector a_i in bohr (row-major)
+ *   kpt         [nkpt][3] reduced coordinates; nkpt >= 1 (all k-points are applied in one batch)
+ *   ecut        Hartree
+ *   ngfft[3]    FFT box n1,n2,n3; each must factor into 2,3,5 and be <= 1024
+ *   typat       [natom] type index 0..ntypat-1;   xred [natom][3] reduced positions
+ *   tables      [ntypat]
+ *   dij         [natom][nlmn_max][nlmn_max] real symmetric, row-major, nlmn_max = max_t nlmn;
+ *               entries outside an atom's nlmn are ignored
+ * natom may be 0 (no non-local term; tables/dij may then be NULL).
+ * On success *out receives the plan.  Synchronises the device.                                   */
+int dft_plan_create(dft_plan **out, const double rprimd[9], int32_t nkpt, const double *kpt,
+                    double ecut, const int32_t ngfft[3], int32_t natom, const int32_t *typat,
+                    const double *xred, int32_t ntypat, const dft_proj_table *tables,
+                    const double *dij);
+
+/* Sizes.  Any output pointer may be NULL.  npw: HOST [nkpt].  mpw = max_k npw_k is the leading
+ * dimension of psi/hpsi.  workspace_bytes_per_band: device scratch dft_apply_h needs per band of
+ * a band chunk (see dft_set_workspace).                                                          */
+int dft_plan_get_info(const dft_plan *p, int32_t *nkpt, int32_t *npw, int32_t *mpw,
+                      int32_t *nproj, int64_t *workspace_bytes_per_band);
+
+/* Copy the index maps of k-point ik to HOST arrays (any may be NULL): kg [npw][3] (integer
+ * m1,m2,m3 of each plane wave), igfft [npw] (box index i1 + n1*(i2 + n2*i3), strictly increasing)
+ * and kin [npw] = 1/2|k+G|^2.                                                                    */
+int dft_plan_get_kg(const dft_plan *p, int32_t ik, int32_t *kg, int32_t *igfft, double *kin);
+
+/* Copy the materialised projector table of k-point ik to a HOST array ptab [nproj][npw] complex
+ * (test / inspection aid; the table of the largest cell is 19.4 GB).                             */
+int dft_plan_get_projectors(const dft_plan *p, int32_t ik, double *ptab);
+
+/* Replace D_ij (PAW: "from self-consistent terms", PAPER.md :473).  HOST [natom][nlmn_max]^2.    */
+int dft_set_dij(dft_plan *p, const double *dij);
+
+/* Set the local potential: V_r is DEVICE memory, [n3][n2][n1] doubles, i1 fastest.  It is copied
+ * (pre-scaled by 1/N) on `stream` (a cudaStream_t passed as void*; NULL = default stream); V_r
+ * may be reused once that stream has passed the call.                                            */
+int dft_set_vloc(dft_plan *p, const double *V_r, void *stream);
+
+/* Optional caller-owned DEVICE scratch (e.g. a torch tensor).  bytes must cover at least one band
+ * chunk of one band; dft_apply_h then never allocates.  dev_ptr = NULL returns to plan-owned
+ * scratch (allocated lazily, grown on demand).  256-byte alignment required.                     */
+int dft_set_workspace(dft_plan *p, void *dev_ptr, int64_t bytes);
+
+/* Options: "band_chunk" (bands per FFT pass launch, > 0), "terms" (bit 0 kinetic, bit 1 local,
+ * bit 2 non-local; default 7), "splitk" (GEMM-1 K splits, 0 = automatic).  Unknown key or bad
+ * value -> DFT_ERR_INVALID_ARG.                                                                  */
+int dft_plan_set_option(dft_plan *p, const char *key, int64_t value);
+
+/* hpsi = H psi for nband bands per k-point.  psi and hpsi are DEVICE memory, layout
+ * [nkpt][nband][mpw] complex128 (16-byte aligned); entries ipw >= npw_k of psi must be finite and
+ * do not influence the result; the same entries of hpsi are written as 0.  hpsi is overwritten;
+ * psi is not modified; they must not overlap.  The call only ENQUEUES work on `stream`
+ * (cudaStream_t as void*, NULL = default stream) and returns; it performs no host
+ * synchronisation and no device->host traffic.  DFT_ERR_NOT_READY if dft_set_vloc was never
+ * called (unless the local term is switched off with "terms").                                   */
+int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);
+
+/* Same, with HOST psi/hpsi (pageable or pinned): copies psi to the device in band blocks, applies
+ * H, copies the result back, and returns after the last copy has completed.                      */
+int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int32_t nband);
+
+/* Number of kernel launches the last dft_apply_h / dft_apply_h_host of this plan enqueued.       */
+int64_t dft_plan_last_launches(const dft_plan *p);
+
+/* Device time of one named kernel group summed over the last apply is not tracked here; use CUDA
+ * events around dft_apply_h, or the bench-only hook below: when `on` != 0 every kernel group of
+ * later applies is bracketed by CUDA events on the launching stream; dft_plan_phase_ms then
+ * returns (after synchronising) the accumulated milliseconds of phase i and resets it.
+ * Phases: 0 fft_A(scatter) 1 fft_B 2 fft_C*V*C^-1 3 fft_B^-1 4 fft_A^-1(gather) 5 gemm1 6 dij
+ * 7 gemm2(+kinetic).                                                                             */
+int dft_plan_set_timing(dft_plan *p, int32_t on);
+int dft_plan_phase_ms(dft_plan *p, int32_t phase, double *ms, int64_t *launches);
+
+int dft_plan_destroy(dft_plan *p);
+
+const char *dft_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DFT_B200_H */

@@ -1,0 +1,293 @@
+"""paper_2507_08578_b200 -- thin ctypes binding of libdftb200.so (C ABI in include/dft.h).
+
+The library applies the plane-wave Kohn-Sham Hamiltonian to a block of bands on one B200
+(Sec. V, :456, Eq. 26 :470-:475).  This module only marshals arguments: every step of
+the path (G-sphere builder, pruned FFT passes, projector GEMMs) runs in the CUDA kernels of
+csrc/.  PyTorch is used for device memory and streams only.  There is no CPU fallback: if the
+shared library cannot be loaded, importing `lib()` raises.
+
+Function names mirror the C ABI (dft_plan_create, dft_set_vloc, dft_apply_h, ...); `Plan` is a
+small convenience wrapper around them.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdftb200.so")
+
+DFT_OK = 0
+DFT_ERR_INVALID_ARG = -1
+DFT_ERR_GRID_TOO_SMALL = -2
+DFT_ERR_TABLE_RANGE = -3
+DFT_ERR_ALLOC = -4
+DFT_ERR_CUDA = -5
+DFT_ERR_NOT_READY = -6
+DFT_ERR_UNSUPPORTED = -7
+
+PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather", "gemm1", "dij", "gemm2_kinetic")
+
+# every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
+SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_set_dij",
+           "dft_set_vloc", "dft_set_workspace", "dft_plan_set_option", "dft_apply_h", "dft_apply_h_host",
+           "dft_plan_last_launches", "dft_plan_set_timing", "dft_plan_phase_ms", "dft_plan_destroy", "dft_last_error")
+
+
+class DftError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libdftb200 error %d: %s" % (code, msg))
+        self.code = code
+
+
+class dft_proj_table(C.Structure):
+    _fields_ = [("nlmn", C.c_int32), ("l", C.POINTER(C.c_int32)), ("m", C.POINTER(C.c_int32)),
+                ("irad", C.POINTER(C.c_int32)), ("nrad", C.c_int32), ("nq", C.c_int32), ("dq", C.c_double),
+                ("f", C.POINTER(C.c_double)), ("f2", C.POINTER(C.c_double))]
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+
+
+def lib():
+    """Load (building first if the sources are newer and nvcc is present) the shared library."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if os.path.exists(_build.NVCC):
+        _build.build()
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("libdftb200.so is missing and nvcc is not available to build it; "
+                           "run `python -m paper_2507_08578_b200._build` (there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    L.dft_last_error.restype = C.c_char_p
+    L.dft_plan_last_launches.restype = C.c_int64
+    L.dft_plan_last_launches.argtypes = [C.c_void_p]
+    L.dft_plan_create.argtypes = [C.POINTER(C.c_void_p), _dp, C.c_int32, _dp, C.c_double, _ip, C.c_int32, _ip, _dp,
+                                  C.c_int32, C.POINTER(dft_proj_table), _dp]
+    L.dft_plan_get_info.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip, C.POINTER(C.c_int64)]
+    L.dft_plan_get_kg.argtypes = [C.c_void_p, C.c_int32, _ip, _ip, _dp]
+    L.dft_plan_get_projectors.argtypes = [C.c_void_p, C.c_int32, _dp]
+    L.dft_set_dij.argtypes = [C.c_void_p, _dp]
+    L.dft_set_vloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.dft_set_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
+    L.dft_plan_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
+    L.dft_apply_h.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    L.dft_apply_h_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
+    L.dft_plan_set_timing.argtypes = [C.c_void_p, C.c_int32]
+    L.dft_plan_phase_ms.argtypes = [C.c_void_p, C.c_int32, _dp, C.POINTER(C.c_int64)]
+    L.dft_plan_destroy.argtypes = [C.c_void_p]
+    _lib = L
+    return L
+
+
+def dft_last_error():
+    return lib().dft_last_error().decode()
+
+
+def _check(rc):
+    if rc != DFT_OK:
+        raise DftError(rc, dft_last_error())
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _d(a):
+    return a.ctypes.data_as(_dp) if a is not None else None
+
+
+def _i(a):
+    return a.ctypes.data_as(_ip) if a is not None else None
+
+
+# ------------------------------------------------------------------------------------- C-ABI mirrors
+def dft_plan_create(rprimd, kpt, ecut, ngfft, typat, xred, types, dij):
+    """types: list of dicts with keys nlmn, l, m, irad, nrad, nq, dq, f[nrad][nq], f2[nrad][nq] (host).
+    Returns the opaque plan handle (int)."""
+    rp = _f64(rprimd).reshape(9)
+    kp = _f64(kpt).reshape(-1, 3)
+    ng = _i32(ngfft).reshape(3)
+    ty = _i32(typat).reshape(-1)
+    xr = _f64(xred).reshape(-1, 3)
+    natom = len(ty)
+    keep = []
+    tabs = (dft_proj_table * max(1, len(types)))()
+    for t, T in enumerate(types):
+        l, m, ir = _i32(T["l"]), _i32(T["m"]), _i32(T["irad"])
+        f, f2 = _f64(T["f"]), _f64(T["f2"])
+        keep += [l, m, ir, f, f2]
+        tabs[t].nlmn = int(T["nlmn"]); tabs[t].l = _i(l); tabs[t].m = _i(m); tabs[t].irad = _i(ir)
+        tabs[t].nrad = int(T["nrad"]); tabs[t].nq = int(T["nq"]); tabs[t].dq = float(T["dq"])
+        tabs[t].f = _d(f); tabs[t].f2 = _d(f2)
+    dj = _f64(dij) if dij is not None else None
+    out = C.c_void_p()
+    rc = lib().dft_plan_create(C.byref(out), _d(rp), len(kp), _d(kp), float(ecut), _i(ng), natom,
+                               _i(ty) if natom else None, _d(xr) if natom else None, len(types), tabs, _d(dj))
+    _check(rc)
+    return out.value
+
+
+def dft_plan_get_info(plan):
+    nk = C.c_int32()
+    _check(lib().dft_plan_get_info(plan, C.byref(nk), None, None, None, None))
+    npw = np.zeros(nk.value, np.int32)
+    mpw, nproj, ws = C.c_int32(), C.c_int32(), C.c_int64()
+    _check(lib().dft_plan_get_info(plan, C.byref(nk), _i(npw), C.byref(mpw), C.byref(nproj), C.byref(ws)))
+    return dict(nkpt=nk.value, npw=npw, mpw=mpw.value, nproj=nproj.value, workspace_bytes_per_band=ws.value)
+
+
+def dft_plan_get_kg(plan, ik, npw):
+    kg = np.zeros((npw, 3), np.int32); ig = np.zeros(npw, np.int32); kin = np.zeros(npw)
+    _check(lib().dft_plan_get_kg(plan, ik, _i(kg), _i(ig), _d(kin)))
+    return kg, ig, kin
+
+
+def dft_plan_get_projectors(plan, ik, nproj, npw):
+    out = np.zeros((nproj, npw), np.complex128)
+    _check(lib().dft_plan_get_projectors(plan, ik, _d(out.view(np.float64))))
+    return out
+
+
+def dft_set_dij(plan, dij):
+    _check(lib().dft_set_dij(plan, _d(_f64(dij))))
+
+
+def dft_set_vloc(plan, v_dev_ptr, stream=0):
+    _check(lib().dft_set_vloc(plan, v_dev_ptr, stream))
+
+
+def dft_set_workspace(plan, dev_ptr, nbytes):
+    _check(lib().dft_set_workspace(plan, dev_ptr, nbytes))
+
+
+def dft_plan_set_option(plan, key, value):
+    _check(lib().dft_plan_set_option(plan, key.encode(), int(value)))
+
+
+def dft_apply_h(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream=0):
+    _check(lib().dft_apply_h(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream))
+
+
+def dft_apply_h_host(plan, psi_host_ptr, hpsi_host_ptr, nband):
+    _check(lib().dft_apply_h_host(plan, psi_host_ptr, hpsi_host_ptr, nband))
+
+
+def dft_plan_last_launches(plan):
+    return int(lib().dft_plan_last_launches(plan))
+
+
+def dft_plan_set_timing(plan, on):
+    _check(lib().dft_plan_set_timing(plan, 1 if on else 0))
+
+
+def dft_plan_phase_ms(plan, phase):
+    ms = C.c_double(); n = C.c_int64()
+    _check(lib().dft_plan_phase_ms(plan, phase, C.byref(ms), C.byref(n)))
+    return ms.value, n.value
+
+
+def dft_plan_destroy(plan):
+    _check(lib().dft_plan_destroy(plan))
+
+
+# ------------------------------------------------------------------------------------- convenience
+class Plan:
+    """Owns one dft_plan.  `cfg` is a dict with rprimd, kpt, ecut, ngfft, typat, xred, types, dij
+    (the layout synth.make_config produces); tensors are torch CUDA tensors."""
+
+    def __init__(self, cfg):
+        self.h = dft_plan_create(cfg["rprimd"], cfg["kpt"], cfg["ecut"], cfg["ngfft"], cfg["typat"], cfg["xred"],
+                                 cfg["types"], cfg["dij"])
+        info = dft_plan_get_info(self.h)
+        self.nkpt, self.npw, self.mpw, self.nproj = info["nkpt"], info["npw"], info["mpw"], info["nproj"]
+        self.workspace_bytes_per_band = info["workspace_bytes_per_band"]
+        self.ngfft = tuple(int(v) for v in cfg["ngfft"])
+        self._keep = []
+
+    def get_kg(self, ik=0):
+        return dft_plan_get_kg(self.h, ik, int(self.npw[ik]))
+
+    def get_projectors(self, ik=0):
+        return dft_plan_get_projectors(self.h, ik, self.nproj, int(self.npw[ik]))
+
+    def set_dij(self, dij):
+        dft_set_dij(self.h, dij)
+
+    def set_vloc(self, v):
+        """v: torch float64 CUDA tensor [n3][n2][n1] (or anything with that many elements)."""
+        import torch
+        assert v.is_cuda and v.dtype == torch.float64 and v.is_contiguous()
+        assert v.numel() == self.ngfft[0] * self.ngfft[1] * self.ngfft[2]
+        dft_set_vloc(self.h, v.data_ptr(), torch.cuda.current_stream().cuda_stream)
+
+    def set_workspace(self, t):
+        if t is None:
+            dft_set_workspace(self.h, None, 0)
+        else:
+            assert t.is_cuda and t.is_contiguous()
+            self._keep = [t]
+            dft_set_workspace(self.h, t.data_ptr(), t.numel() * t.element_size())
+
+    def set_option(self, key, value):
+        dft_plan_set_option(self.h, key, value)
+
+    def apply_h(self, psi, hpsi=None):
+        """psi: torch complex128 CUDA tensor [nkpt][nband][mpw] (or [nband][mpw] when nkpt = 1)."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous()
+        assert psi.shape[-1] == self.mpw and psi.numel() % (self.nkpt * self.mpw) == 0
+        nband = psi.numel() // (self.nkpt * self.mpw) if self.mpw else 0
+        if hpsi is None:
+            hpsi = torch.empty_like(psi)
+        assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.is_contiguous() and hpsi.shape == psi.shape
+        dft_apply_h(self.h, psi.data_ptr(), hpsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
+        return hpsi
+
+    def apply_h_host(self, psi, hpsi=None):
+        """psi: numpy complex128 array or CPU torch tensor (pinned or not); returns the same kind."""
+        is_np = isinstance(psi, np.ndarray)
+        if is_np:
+            psi = np.ascontiguousarray(psi, np.complex128)
+            if hpsi is None:
+                hpsi = np.empty_like(psi)
+            pin, pout, numel = psi.ctypes.data, hpsi.ctypes.data, psi.size
+        else:
+            import torch
+            assert not psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous()
+            if hpsi is None:
+                hpsi = torch.empty_like(psi, pin_memory=psi.is_pinned())
+            pin, pout, numel = psi.data_ptr(), hpsi.data_ptr(), psi.numel()
+        nband = numel // (self.nkpt * self.mpw) if self.mpw else 0
+        dft_apply_h_host(self.h, pin, pout, nband)
+        return hpsi
+
+    def last_launches(self):
+        return dft_plan_last_launches(self.h)
+
+    def set_timing(self, on):
+        dft_plan_set_timing(self.h, on)
+
+    def phase_ms(self):
+        """{phase name: (milliseconds, launches)} accumulated since the last call; synchronises."""
+        return {name: dft_plan_phase_ms(self.h, i) for i, name in enumerate(PHASES)}
+
+    def destroy(self):
+        if self.h:
+            dft_plan_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

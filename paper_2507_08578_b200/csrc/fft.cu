@@ -1,0 +1,430 @@
+// fft.cu -- K2: the local term  V_loc psi = FFT^-1[ V_loc(r) . FFT[psi] ]  (PAPER.md :475 "local part
+// using fast Fourier transforms", :436 "multiple concurrent Fourier transforms using an array of
+// wave functions"), as a sphere-pruned, batched complex128 3-D transform in five passes
+// (SURVEY.md 8(a) steps S3-S7):
+//
+//   A    scatter sphere -> zero-padded x-lines, transform along x, only the ncol non-empty (i2,i3) columns
+//   B    transform along y for every x, only the s3 non-empty i3 planes
+//   C    per (x,y) line: pad s3 -> n3, transform along z, multiply by V(r)/N, inverse transform, keep s3
+//   B^-1 inverse along y, keep only the non-empty columns
+//   A^-1 inverse along x, gather the sphere entries -> hpsi
+//
+// Reading 4: G->r uses exp(+2 pi i m.j/n) unscaled, r->G uses exp(-...) and 1/N; the
+// 1/N is folded into the stored potential by dft_set_vloc.  The pruned sequence is an exact
+// re-arrangement of the full-box transform (skipped lines are identically zero on the way in and
+// are never read on the way out).
+//
+// Every pass stages its lines in shared memory and runs Stockham autosort radix passes
+// (radices 2,3,4,5,8,9) with one butterfly per thread; strided passes (B, C) keep x fastest so
+// that global accesses are contiguous runs of XT complex numbers and shared accesses are
+// conflict-free.
+#include <math.h>
+
+#include "internal.h"
+
+namespace dftb200 {
+
+// ------------------------------------------------------------------------------------------
+// factorisation of a 1-D length into the radices the butterflies below implement
+// ------------------------------------------------------------------------------------------
+bool factorize(int n, FftFactors *f) {
+  f->n = n; f->nfac = 0;
+  if (n < 1) return false;
+  int e2 = 0, e3 = 0, e5 = 0, m = n;
+  while (m % 2 == 0) { m /= 2; e2++; }
+  while (m % 3 == 0) { m /= 3; e3++; }
+  while (m % 5 == 0) { m /= 5; e5++; }
+  if (m != 1) return false;
+  auto push = [&](int r) { f->radix[f->nfac++] = r; };
+  while (e3 >= 2) { push(9); e3 -= 2; }
+  if (e3) push(3);
+  for (int i = 0; i < e5; i++) push(5);
+  if (e2 == 1) push(2);
+  else if (e2 % 3 == 1) { push(4); push(4); e2 -= 4; }
+  else if (e2 % 3 == 2) { push(4); e2 -= 2; }
+  if (e2 >= 3) while (e2 > 0) { push(8); e2 -= 3; }
+  return f->nfac <= 12;
+}
+
+// ------------------------------------------------------------------------------------------
+// complex helpers and radix butterflies:  X[q] = sum_r v[r] w^(q r),  w = exp(S 2 pi i / R)
+// ------------------------------------------------------------------------------------------
+typedef double2 cplx;
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a.x * s, a.y * s); }
+// multiply by S*i
+template <int S> __device__ __forceinline__ cplx mul_si(cplx a) {
+  return S > 0 ? make_double2(-a.y, a.x) : make_double2(a.y, -a.x);
+}
+
+template <int S> __device__ __forceinline__ void bfly2(cplx &a, cplx &b) {
+  cplx t = csub(a, b); a = cadd(a, b); b = t;
+}
+template <int S> __device__ __forceinline__ void bfly3(cplx &v0, cplx &v1, cplx &v2) {
+  const double H = 0.86602540378443864676;  // sqrt(3)/2
+  cplx t = cadd(v1, v2), u = mul_si<S>(cscale(csub(v1, v2), H));
+  cplx m = make_double2(v0.x - 0.5 * t.x, v0.y - 0.5 * t.y);
+  v0 = cadd(v0, t); v1 = cadd(m, u); v2 = csub(m, u);
+}
+template <int S> __device__ __forceinline__ void bfly4(cplx &v0, cplx &v1, cplx &v2, cplx &v3) {
+  cplx t0 = cadd(v0, v2), t1 = csub(v0, v2), t2 = cadd(v1, v3), t3 = mul_si<S>(csub(v1, v3));
+  v0 = cadd(t0, t2); v2 = csub(t0, t2); v1 = cadd(t1, t3); v3 = csub(t1, t3);
+}
+template <int S> __device__ __forceinline__ void bfly5(cplx &v0, cplx &v1, cplx &v2, cplx &v3, cplx &v4) {
+  const double C1 = 0.30901699437494742410, C2 = -0.80901699437494742410;  // cos(2pi/5), cos(4pi/5)
+  const double S1 = 0.95105651629515357212, S2 = 0.58778525229247312917;   // sin(2pi/5), sin(4pi/5)
+  cplx a1 = cadd(v1, v4), a2 = cadd(v2, v3), b1 = csub(v1, v4), b2 = csub(v2, v3);
+  cplx m1 = make_double2(v0.x + C1 * a1.x + C2 * a2.x, v0.y + C1 * a1.y + C2 * a2.y);
+  cplx m2 = make_double2(v0.x + C2 * a1.x + C1 * a2.x, v0.y + C2 * a1.y + C1 * a2.y);
+  cplx u1 = mul_si<S>(make_double2(S1 * b1.x + S2 * b2.x, S1 * b1.y + S2 * b2.y));
+  cplx u2 = mul_si<S>(make_double2(S2 * b1.x - S1 * b2.x, S2 * b1.y - S1 * b2.y));
+  v0 = cadd(v0, cadd(a1, a2));
+  v1 = cadd(m1, u1); v4 = csub(m1, u1);
+  v2 = cadd(m2, u2); v3 = csub(m2, u2);
+}
+
+template <int R, int S> struct Bfly;
+template <int S> struct Bfly<2, S> { static __device__ __forceinline__ void run(cplx *v) { bfly2<S>(v[0], v[1]); } };
+template <int S> struct Bfly<3, S> { static __device__ __forceinline__ void run(cplx *v) { bfly3<S>(v[0], v[1], v[2]); } };
+template <int S> struct Bfly<4, S> { static __device__ __forceinline__ void run(cplx *v) { bfly4<S>(v[0], v[1], v[2], v[3]); } };
+template <int S> struct Bfly<5, S> { static __device__ __forceinline__ void run(cplx *v) { bfly5<S>(v[0], v[1], v[2], v[3], v[4]); } };
+// 8 = 2 x 4 (decimation in time: even/odd halves, then X[q] = E[q] + w8^q O[q], X[q+4] = E[q] - w8^q O[q])
+template <int S> struct Bfly<8, S> {
+  static __device__ __forceinline__ void run(cplx *v) {
+    const double Q = 0.70710678118654752440;
+    bfly4<S>(v[0], v[2], v[4], v[6]);   // E[0..3] in v0,v2,v4,v6
+    bfly4<S>(v[1], v[3], v[5], v[7]);   // O[0..3] in v1,v3,v5,v7
+    cplx o1 = make_double2(Q * (v[3].x - S * v[3].y), Q * (v[3].y + S * v[3].x));       // w8^1 = (1 + S i)/sqrt2
+    cplx o2 = mul_si<S>(v[5]);                                                           // w8^2 = S i
+    cplx o3 = make_double2(Q * (-v[7].x - S * v[7].y), Q * (-v[7].y + S * v[7].x));     // w8^3 = (-1 + S i)/sqrt2
+    cplx e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
+    v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+    v[1] = cadd(e1, o1); v[5] = csub(e1, o1);
+    v[2] = cadd(e2, o2); v[6] = csub(e2, o2);
+    v[3] = cadd(e3, o3); v[7] = csub(e3, o3);
+  }
+};
+// 9 = 3 x 3:  r = 3a + b, q = q1 + 3 q2;  Y_b[q1] = DFT3_a v[3a+b];  X[q1+3q2] = DFT3_b (w9^(b q1) Y_b[q1])
+template <int S> struct Bfly<9, S> {
+  static __device__ __forceinline__ void run(cplx *v) {
+    const double C1 = 0.76604444311897803520, S1 = 0.64278760968653932632;   // cos/sin(2pi/9)
+    const double C2 = 0.17364817766693034885, S2 = 0.98480775301220805937;   // cos/sin(4pi/9)
+    const double C4 = -0.93969262078590838405, S4 = 0.34202014332566873304;  // cos/sin(8pi/9)
+    bfly3<S>(v[0], v[3], v[6]);   // b = 0: Y_0[q1] in v0,v3,v6
+    bfly3<S>(v[1], v[4], v[7]);   // b = 1
+    bfly3<S>(v[2], v[5], v[8]);   // b = 2
+    // twiddles w9^(b q1): (b,q1) = (1,1)->w, (1,2)->w^2, (2,1)->w^2, (2,2)->w^4
+    v[4] = cmul(v[4], make_double2(C1, S * S1));
+    v[7] = cmul(v[7], make_double2(C2, S * S2));
+    v[5] = cmul(v[5], make_double2(C2, S * S2));
+    v[8] = cmul(v[8], make_double2(C4, S * S4));
+    bfly3<S>(v[0], v[1], v[2]);   // q1 = 0: X[0], X[3], X[6]
+    bfly3<S>(v[3], v[4], v[5]);   // q1 = 1: X[1], X[4], X[7]
+    bfly3<S>(v[6], v[7], v[8]);   // q1 = 2: X[2], X[5], X[8]
+    cplx x1 = v[3], x2 = v[6], x3 = v[1], x4 = v[4], x5 = v[7], x6 = v[2], x7 = v[5];
+    v[1] = x1; v[2] = x2; v[3] = x3; v[4] = x4; v[5] = x5; v[6] = x6; v[7] = x7;
+  }
+};
+
+struct FacDev { int nfac; int radix[12]; };
+
+// One Stockham pass of radix R over `nlines` lines held in shared memory.
+// element j of line l sits at buf[l*ls + j*es]; tw[j] = exp(+2 pi i j/n).
+template <int R, int S>
+__device__ __forceinline__ void stockham_pass(const cplx *__restrict__ in, cplx *__restrict__ out, const cplx *__restrict__ tw,
+                                              int n, int Ns, int nlines, int es, int ls) {
+  const int nb = n / R;             // butterflies per line
+  const int tstep = n / (Ns * R);   // twiddle exp(S 2 pi i r k/(Ns R)) = tw[r k tstep]
+  for (int w = threadIdx.x; w < nb * nlines; w += blockDim.x) {
+    int l = w % nlines, j = w / nlines;
+    int k = j % Ns;
+    cplx v[R];
+    const cplx *src = in + l * ls + j * es;
+#pragma unroll
+    for (int r = 0; r < R; r++) v[r] = src[r * nb * es];
+    if (Ns > 1) {
+#pragma unroll
+      for (int r = 1; r < R; r++) {
+        cplx t = tw[r * k * tstep];
+        if (S < 0) t.y = -t.y;
+        v[r] = cmul(v[r], t);
+      }
+    }
+    Bfly<R, S>::run(v);
+    int j0 = (j / Ns) * Ns * R + k;
+    cplx *dst = out + l * ls + j0 * es;
+#pragma unroll
+    for (int r = 0; r < R; r++) dst[r * Ns * es] = v[r];
+  }
+}
+
+// Full 1-D transform of all lines; ping-pongs between a and b, returns the buffer holding the result.
+template <int S>
+__device__ __forceinline__ cplx *fft_lines(cplx *a, cplx *b, const cplx *tw, int n, const FacDev &F, int nlines, int es, int ls) {
+  int Ns = 1;
+  for (int f = 0; f < F.nfac; f++) {
+    int R = F.radix[f];
+    __syncthreads();
+    switch (R) {
+      case 2: stockham_pass<2, S>(a, b, tw, n, Ns, nlines, es, ls); break;
+      case 3: stockham_pass<3, S>(a, b, tw, n, Ns, nlines, es, ls); break;
+      case 4: stockham_pass<4, S>(a, b, tw, n, Ns, nlines, es, ls); break;
+      case 5: stockham_pass<5, S>(a, b, tw, n, Ns, nlines, es, ls); break;
+      case 8: stockham_pass<8, S>(a, b, tw, n, Ns, nlines, es, ls); break;
+      default: stockham_pass<9, S>(a, b, tw, n, Ns, nlines, es, ls); break;
+    }
+    Ns *= R;
+    cplx *t = a; a = b; b = t;
+  }
+  __syncthreads();
+  return a;
+}
+
+__device__ __forceinline__ void load_twiddles(cplx *tws, const double *tw, int n) {
+  const cplx *g = reinterpret_cast<const cplx *>(tw);
+  for (int j = threadIdx.x; j < n; j += blockDim.x) tws[j] = g[j];
+}
+
+struct FftGeom {
+  int n1, n2, n3, n1p;         // n1p: odd line stride used by the x passes
+  int npw, mpw, ncol, nplane;
+  int XT, nxt;                 // x-tile width of the strided passes, number of tiles
+  int CL;                      // columns per CTA in the x passes
+  const int32_t *col_start, *col_i2, *col_plane, *pw_i1, *plane_i3, *plane_col0;
+  const double *tw1, *tw2, *tw3;
+  FacDev f1, f2, f3;
+  int64_t t1_band, t2_band;    // complex elements per band of T1 [ncol][n1] and T2 [nplane][n2][n1]
+};
+
+constexpr int FFT_THREADS = 256;
+
+// ---- pass A: scatter + transform along x.  grid (ceil(ncol/CL), nb) -------------------------------
+__global__ void __launch_bounds__(FFT_THREADS) fft_pass_a_kernel(FftGeom G, const cplx *__restrict__ psi, cplx *__restrict__ T1) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *tws = reinterpret_cast<cplx *>(smem_raw);
+  cplx *bufa = tws + G.n1, *bufb = bufa + G.CL * G.n1p;
+  int c0 = blockIdx.x * G.CL, nc = min(G.CL, G.ncol - c0), b = blockIdx.y;
+  load_twiddles(tws, G.tw1, G.n1);
+  for (int i = threadIdx.x; i < G.CL * G.n1p; i += blockDim.x) bufa[i] = make_double2(0.0, 0.0);
+  __syncthreads();
+  const cplx *src = psi + (size_t)b * G.mpw;
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+  for (int lc = warp; lc < nc; lc += nwarp) {
+    int g0 = G.col_start[c0 + lc], g1 = G.col_start[c0 + lc + 1];
+    for (int g = g0 + lane; g < g1; g += 32) bufa[lc * G.n1p + G.pw_i1[g]] = src[g];
+  }
+  cplx *res = fft_lines<+1>(bufa, bufb, tws, G.n1, G.f1, G.CL, 1, G.n1p);
+  cplx *dst = T1 + (size_t)b * G.t1_band + (size_t)c0 * G.n1;
+  for (int i = threadIdx.x; i < nc * G.n1; i += blockDim.x) dst[i] = res[(i / G.n1) * G.n1p + (i % G.n1)];
+}
+
+// ---- pass A^-1: inverse along x + gather.  grid (ceil(ncol/CL), nb) ---------------------------------
+__global__ void __launch_bounds__(FFT_THREADS) fft_pass_ainv_kernel(FftGeom G, const cplx *__restrict__ T1, cplx *__restrict__ hpsi) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *tws = reinterpret_cast<cplx *>(smem_raw);
+  cplx *bufa = tws + G.n1, *bufb = bufa + G.CL * G.n1p;
+  int c0 = blockIdx.x * G.CL, nc = min(G.CL, G.ncol - c0), b = blockIdx.y;
+  load_twiddles(tws, G.tw1, G.n1);
+  const cplx *src = T1 + (size_t)b * G.t1_band + (size_t)c0 * G.n1;
+  for (int i = threadIdx.x; i < G.CL * G.n1; i += blockDim.x) {
+    int lc = i / G.n1, x = i % G.n1;
+    bufa[lc * G.n1p + x] = (lc < nc) ? src[i] : make_double2(0.0, 0.0);
+  }
+  cplx *res = fft_lines<-1>(bufa, bufb, tws, G.n1, G.f1, G.CL, 1, G.n1p);
+  cplx *dst = hpsi + (size_t)b * G.mpw;
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+  for (int lc = warp; lc < nc; lc += nwarp) {
+    int g0 = G.col_start[c0 + lc], g1 = G.col_start[c0 + lc + 1];
+    for (int g = g0 + lane; g < g1; g += 32) dst[g] = res[lc * G.n1p + G.pw_i1[g]];
+  }
+  // entries ipw >= npw of the band are defined to be 0 on output
+  if (blockIdx.x == gridDim.x - 1)
+    for (int g = G.npw + threadIdx.x; g < G.mpw; g += blockDim.x) dst[g] = make_double2(0.0, 0.0);
+}
+
+// ---- pass B: transform along y.  grid (nxt, nplane, nb) -------------------------------------------
+template <int S>
+__global__ void __launch_bounds__(FFT_THREADS) fft_pass_b_kernel(FftGeom G, cplx *__restrict__ T1, cplx *__restrict__ T2) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *tws = reinterpret_cast<cplx *>(smem_raw);
+  cplx *bufa = tws + G.n2, *bufb = bufa + G.n2 * G.XT;
+  int x0 = blockIdx.x * G.XT, nx = min(G.XT, G.n1 - x0), p = blockIdx.y, b = blockIdx.z;
+  int ca = G.plane_col0[p], cb = G.plane_col0[p + 1];
+  load_twiddles(tws, G.tw2, G.n2);
+  cplx *t1 = T1 + (size_t)b * G.t1_band;
+  cplx *t2 = T2 + (size_t)b * G.t2_band + (size_t)p * G.n2 * G.n1;
+  if (S > 0) {
+    for (int i = threadIdx.x; i < G.n2 * G.XT; i += blockDim.x) bufa[i] = make_double2(0.0, 0.0);
+    __syncthreads();
+    for (int i = threadIdx.x; i < (cb - ca) * G.XT; i += blockDim.x) {
+      int c = ca + i / G.XT, xt = i % G.XT;
+      if (xt < nx) bufa[G.col_i2[c] * G.XT + xt] = t1[(size_t)c * G.n1 + x0 + xt];
+    }
+  } else {
+    for (int i = threadIdx.x; i < G.n2 * G.XT; i += blockDim.x) {
+      int y = i / G.XT, xt = i % G.XT;
+      bufa[i] = (xt < nx) ? t2[(size_t)y * G.n1 + x0 + xt] : make_double2(0.0, 0.0);
+    }
+  }
+  cplx *res = fft_lines<S>(bufa, bufb, tws, G.n2, G.f2, G.XT, G.XT, 1);
+  if (S > 0) {
+    for (int i = threadIdx.x; i < G.n2 * G.XT; i += blockDim.x) {
+      int y = i / G.XT, xt = i % G.XT;
+      if (xt < nx) t2[(size_t)y * G.n1 + x0 + xt] = res[i];
+    }
+  } else {
+    for (int i = threadIdx.x; i < (cb - ca) * G.XT; i += blockDim.x) {
+      int c = ca + i / G.XT, xt = i % G.XT;
+      if (xt < nx) t1[(size_t)c * G.n1 + x0 + xt] = res[G.col_i2[c] * G.XT + xt];
+    }
+  }
+}
+
+// ---- pass C: along z, times V/N, inverse along z.  grid (nxt, n2, nb) ------------------------------
+__global__ void __launch_bounds__(FFT_THREADS) fft_pass_c_kernel(FftGeom G, cplx *__restrict__ T2, const double *__restrict__ vloc) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *tws = reinterpret_cast<cplx *>(smem_raw);
+  cplx *bufa = tws + G.n3, *bufb = bufa + G.n3 * G.XT;
+  int x0 = blockIdx.x * G.XT, nx = min(G.XT, G.n1 - x0), y = blockIdx.y, b = blockIdx.z;
+  load_twiddles(tws, G.tw3, G.n3);
+  cplx *t2 = T2 + (size_t)b * G.t2_band + (size_t)y * G.n1 + x0;
+  size_t pstride = (size_t)G.n2 * G.n1;
+  for (int i = threadIdx.x; i < G.n3 * G.XT; i += blockDim.x) bufa[i] = make_double2(0.0, 0.0);
+  __syncthreads();
+  for (int i = threadIdx.x; i < G.nplane * G.XT; i += blockDim.x) {
+    int p = i / G.XT, xt = i % G.XT;
+    if (xt < nx) bufa[G.plane_i3[p] * G.XT + xt] = t2[p * pstride + xt];
+  }
+  cplx *res = fft_lines<+1>(bufa, bufb, tws, G.n3, G.f3, G.XT, G.XT, 1);
+  cplx *other = (res == bufa) ? bufb : bufa;
+  const double *v = vloc + (size_t)y * G.n1 + x0;
+  for (int i = threadIdx.x; i < G.n3 * G.XT; i += blockDim.x) {
+    int z = i / G.XT, xt = i % G.XT;
+    double s = (xt < nx) ? v[z * pstride + xt] : 0.0;
+    res[i] = make_double2(res[i].x * s, res[i].y * s);
+  }
+  res = fft_lines<-1>(res, other, tws, G.n3, G.f3, G.XT, G.XT, 1);
+  for (int i = threadIdx.x; i < G.nplane * G.XT; i += blockDim.x) {
+    int p = i / G.XT, xt = i % G.XT;
+    if (xt < nx) t2[p * pstride + xt] = res[G.plane_i3[p] * G.XT + xt];
+  }
+}
+
+__global__ void zero_kernel(double *p, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = 0.0;
+}
+
+int zero_fill(double *hpsi, int64_t ndouble, cudaStream_t st) {
+  if (ndouble <= 0) return DFT_OK;
+  int grid = (int)((ndouble + 255) / 256 < 148 * 8 ? (ndouble + 255) / 256 : 148 * 8);
+  zero_kernel<<<grid, 256, 0, st>>>(hpsi, ndouble);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------
+static const size_t SMEM_BUDGET = 200 * 1024;
+
+static int choose_xt(int n1, int nmax) {
+  int cap = (int)(SMEM_BUDGET / (32 * (size_t)nmax));   // two buffers of n*XT complex
+  if (cap < 1) cap = 1;
+  int xt = 0;
+  for (int d = 16; d <= 40; d += 2)
+    if (n1 % d == 0) { xt = d; break; }
+  if (!xt) xt = n1 <= 40 ? n1 : 16;
+  return xt < cap ? xt : cap;
+}
+static int choose_cl(int n1p) {
+  int cap = (int)(SMEM_BUDGET / (32 * (size_t)n1p));
+  return cap < 16 ? (cap < 1 ? 1 : cap) : 16;
+}
+
+static FftGeom make_geom(const dft_plan *p, int ik) {
+  const KPoint &kp = p->kp[ik];
+  FftGeom G;
+  G.n1 = p->n[0]; G.n2 = p->n[1]; G.n3 = p->n[2]; G.n1p = G.n1 | 1;
+  G.npw = kp.npw; G.mpw = p->mpw; G.ncol = kp.ncol; G.nplane = kp.nplane;
+  int nmax = G.n2 > G.n3 ? G.n2 : G.n3;
+  G.XT = choose_xt(G.n1, nmax); G.nxt = (G.n1 + G.XT - 1) / G.XT;
+  G.CL = choose_cl(G.n1p);
+  G.col_start = kp.col_start; G.col_i2 = kp.col_i2; G.col_plane = kp.col_plane; G.pw_i1 = kp.pw_i1;
+  G.plane_i3 = kp.plane_i3; G.plane_col0 = kp.plane_col0;
+  G.tw1 = p->d_tw[0]; G.tw2 = p->d_tw[1]; G.tw3 = p->d_tw[2];
+  const FftFactors *f[3] = {&p->fac[0], &p->fac[1], &p->fac[2]};
+  FacDev *d[3] = {&G.f1, &G.f2, &G.f3};
+  for (int c = 0; c < 3; c++) {
+    d[c]->nfac = f[c]->nfac;
+    for (int i = 0; i < 12; i++) d[c]->radix[i] = f[c]->radix[i];
+  }
+  G.t1_band = (int64_t)kp.ncol * G.n1;
+  G.t2_band = (int64_t)kp.nplane * G.n2 * G.n1;
+  return G;
+}
+
+// scratch per band: T1 [ncol][n1] + T2 [nplane][n2][n1] complex (max over k-points), 256-byte rounded
+int64_t fft_ws_bytes_per_band(const dft_plan *p) {
+  int64_t mx = 0;
+  for (int ik = 0; ik < p->nkpt; ik++) {
+    const KPoint &kp = p->kp[ik];
+    int64_t t1 = ((int64_t)kp.ncol * p->n[0] * 16 + 255) / 256 * 256;
+    int64_t t2 = ((int64_t)kp.nplane * p->n[1] * p->n[0] * 16 + 255) / 256 * 256;
+    if (t1 + t2 > mx) mx = t1 + t2;
+  }
+  return mx;
+}
+
+static bool g_attr_done = false;
+static int set_attrs() {
+  if (g_attr_done) return DFT_OK;
+  int mx = (int)(SMEM_BUDGET + 24 * 1024);
+  DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_a_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+  DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_ainv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+  DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_b_kernel<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+  DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_b_kernel<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+  DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_c_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
+  g_attr_done = true;
+  return DFT_OK;
+}
+
+int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb, void *ws, cudaStream_t st) {
+  int rc = set_attrs();
+  if (rc) return rc;
+  const KPoint &kp = p->kp[ik];
+  if (kp.npw == 0 || nb == 0) return zero_fill(hpsi, (int64_t)nb * p->mpw * 2, st);
+  FftGeom G = make_geom(p, ik);
+  int64_t t1b = ((int64_t)G.t1_band * 16 + 255) / 256 * 256;
+  cplx *T1 = reinterpret_cast<cplx *>(ws);
+  cplx *T2 = reinterpret_cast<cplx *>(reinterpret_cast<char *>(ws) + t1b * nb);
+  // T1 is addressed with the rounded per-band stride
+  G.t1_band = t1b / 16;
+  G.t2_band = (((int64_t)G.t2_band * 16 + 255) / 256 * 256) / 16;
+  const cplx *cpsi = reinterpret_cast<const cplx *>(psi);
+  cplx *chpsi = reinterpret_cast<cplx *>(hpsi);
+  size_t sm_a = sizeof(cplx) * ((size_t)G.n1 + 2 * (size_t)G.CL * G.n1p);
+  size_t sm_b = sizeof(cplx) * ((size_t)G.n2 + 2 * (size_t)G.n2 * G.XT);
+  size_t sm_c = sizeof(cplx) * ((size_t)G.n3 + 2 * (size_t)G.n3 * G.XT);
+  dim3 ga((G.ncol + G.CL - 1) / G.CL, nb), gb(G.nxt, G.nplane, nb), gc(G.nxt, G.n2, nb);
+  phase_begin(p, 0, st);
+  fft_pass_a_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, cpsi, T1);
+  phase_end(p, 0, st, 1);
+  phase_begin(p, 1, st);
+  fft_pass_b_kernel<+1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
+  phase_end(p, 1, st, 1);
+  phase_begin(p, 2, st);
+  fft_pass_c_kernel<<<gc, FFT_THREADS, sm_c, st>>>(G, T2, p->d_vloc);
+  phase_end(p, 2, st, 1);
+  phase_begin(p, 3, st);
+  fft_pass_b_kernel<-1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
+  phase_end(p, 3, st, 1);
+  phase_begin(p, 4, st);
+  fft_pass_ainv_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, T1, chpsi);
+  phase_end(p, 4, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+}  // namespace dftb200

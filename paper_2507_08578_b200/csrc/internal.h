@@ -1,0 +1,142 @@
+// internal.h -- plan structure and the launchers shared by the translation units of libdftb200.
+// Nothing here is shared with oracle/ (the CPU checker): every rule is restated from DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/dft.h"
+
+namespace dftb200 {
+
+// ------------------------------------------------------------------------------------------
+// error plumbing
+// ------------------------------------------------------------------------------------------
+void set_error(const char *fmt, ...);
+#define DFT_CUDA_CHECK(expr)                                                              \
+  do {                                                                                    \
+    cudaError_t e__ = (expr);                                                             \
+    if (e__ != cudaSuccess) {                                                             \
+      ::dftb200::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+      return DFT_ERR_CUDA;                                                                \
+    }                                                                                     \
+  } while (0)
+
+// ------------------------------------------------------------------------------------------
+// FFT schedule of one 1-D length: radices (each in {2,3,4,5,8,9}), product = n
+// ------------------------------------------------------------------------------------------
+struct FftFactors {
+  int n = 0;
+  int nfac = 0;
+  int radix[12] = {0};
+};
+bool factorize(int n, FftFactors *f);
+
+// Per-k-point geometry of the sphere and of the pruned passes (device pointers unless noted)
+struct KPoint {
+  double k[3];
+  int npw = 0;
+  // sphere (K1)
+  int32_t *kg = nullptr;      // [npw][3]
+  int32_t *igfft = nullptr;   // [npw]
+  double *kin = nullptr;      // [npw]
+  // pruned-FFT geometry derived from kg on the host
+  int ncol = 0;               // non-empty (i2,i3) columns, sorted by (i3,i2) = order of first plane wave
+  int nplane = 0;             // non-empty i3 planes (s_3)
+  int32_t *col_start = nullptr;  // [ncol+1] first plane wave of column c (columns are contiguous runs of the kg list)
+  int32_t *col_i2 = nullptr;     // [ncol]
+  int32_t *col_plane = nullptr;  // [ncol]  plane ordinal p (0..nplane-1) of the column
+  int32_t *pw_i1 = nullptr;      // [npw]   box index along axis 1 of each plane wave
+  int32_t *plane_i3 = nullptr;   // [nplane] box index i3 of plane p
+  int32_t *plane_col0 = nullptr; // [nplane+1] first column of plane p
+  // host copies for getters
+  std::vector<int32_t> h_kg, h_igfft;
+  std::vector<double> h_kin;
+};
+
+struct PhaseTimer {
+  bool on = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[8];
+  int64_t launches[8] = {0};
+};
+
+}  // namespace dftb200
+
+struct dft_plan {
+  // lattice
+  double rprimd[9], bm[9], gmet[9];
+  double ecut;
+  int n[3];
+  int64_t nbox;
+  int nkpt = 0, mpw = 0;
+  std::vector<dftb200::KPoint> kp;
+  // atoms / projectors
+  int natom = 0, ntypat = 0, lmax = 0, nproj = 0;
+  std::vector<int32_t> typat, nlmn, lmn_l, lmn_m, lmn_irad, atom_first;  // lmn_*: [ntypat][lmax]
+  std::vector<double> xred;
+  std::vector<int32_t> nq; std::vector<double> dq;   // per type
+  int nrad_max = 0, nq_max = 0;
+  double *d_f = nullptr, *d_f2 = nullptr;            // [ntypat][nrad_max][nq_max]
+  int32_t *d_typat = nullptr, *d_nlmn = nullptr, *d_lmn_l = nullptr, *d_lmn_m = nullptr, *d_lmn_irad = nullptr;
+  int32_t *d_atom_first = nullptr, *d_nq = nullptr;
+  double *d_dq = nullptr, *d_xred = nullptr;
+  double *d_dij = nullptr;                           // [natom][lmax][lmax]
+  double *d_ptab = nullptr;                          // [nkpt][nproj][mpw] complex, zero padded beyond npw_k
+  int32_t *d_npw = nullptr;                          // [nkpt]
+  const double **d_kinptr = nullptr;                 // [nkpt] device pointers to kin of each k-point
+  // local potential
+  double *d_vloc = nullptr;                          // [n3][n2][n1], pre-scaled by 1/N
+  bool vloc_set = false;
+  // FFT
+  dftb200::FftFactors fac[3];
+  double *d_tw[3] = {nullptr, nullptr, nullptr};     // twiddles exp(+2 pi i j/n_c), [n_c] complex
+  // options
+  int band_chunk = 0;      // 0 = automatic
+  int terms = 7;
+  int splitk = 0;
+  // workspace
+  void *ws_user = nullptr; int64_t ws_user_bytes = 0;
+  void *ws_own = nullptr;  int64_t ws_own_bytes = 0;
+  // GEMM scratch (plan-owned, sized at first use)
+  double *d_part = nullptr; int64_t part_bytes = 0;  // split-K partials
+  double *d_cprj = nullptr; int64_t cprj_bytes = 0;  // c' [nkpt][nband][nproj] complex
+  // host staging for dft_apply_h_host
+  double *d_stage_in = nullptr, *d_stage_out = nullptr; int64_t stage_bytes = 0;
+  cudaStream_t host_stream = nullptr;
+  // TMA
+  void *encode_fn = nullptr;   // cuTensorMapEncodeTiled
+  int sm_count = 148;
+  int64_t last_launches = 0;
+  dftb200::PhaseTimer timer;
+};
+
+namespace dftb200 {
+
+// --- sphere.cu (K1) -----------------------------------------------------------------------
+void lattice_algebra(const double *a, double *bm, double *gmet, double *det);
+// Extents of the sphere over the integer cube |m_j| <= bound_j; returns status.
+int sphere_extent(const double *gmet, const double *k, double ecut, const int bound[3], int mmin[3], int mmax[3]);
+// Build kg/igfft/kin of one k-point on the device (ascending box index); fills kp.npw and device arrays.
+int sphere_build(const double *gmet, const int n[3], double ecut, KPoint *kp);
+
+// --- projtab.cu (S1) ----------------------------------------------------------------------
+int build_projector_table(dft_plan *p, int ik, double *maxq_out);
+
+// --- fft.cu (K2) --------------------------------------------------------------------------
+int64_t fft_ws_bytes_per_band(const dft_plan *p);
+// V_loc psi for `nb` bands of k-point ik: psi/hpsi point at the first band ([nb][mpw] complex)
+int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb, void *ws, cudaStream_t st);
+int zero_fill(double *hpsi, int64_t ndouble, cudaStream_t st);
+
+// --- nonlocal.cu (K3) ---------------------------------------------------------------------
+// hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi
+int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin,
+                   bool with_nl, cudaStream_t st);
+
+// --- timing hooks ------------------------------------------------------------------------------
+void phase_begin(dft_plan *p, int phase, cudaStream_t st);
+void phase_end(dft_plan *p, int phase, cudaStream_t st, int launches);
+
+}  // namespace dftb200

@@ -1,0 +1,451 @@
+// nonlocal.cu -- K3: the non-local operator of Eq. 26 (PAPER.md :470) plus the kinetic diagonal,
+//
+//   (H_nl psi_b)(G) = sum_a sum_ij p_{a,i}(G) D^a_ij sum_G' conj(p_{a,j}(G')) psi_b(G'),
+//
+// in the BLAS-3 formulation the paper describes for stored projectors (:479 "matrix-matrix
+// multiplications"), SURVEY.md 8(a) steps S8-S10:
+//
+//   GEMM-1  cprj[p][b]  = sum_G conj(P[p][G]) psi[b][G]          M = nproj, N = nband, K = npw   (split-K)
+//   D_ij    c'[b][a,i]  = sum_j D^a_ij cprj[a,j][b]              (also reduces the split-K partials, fixed order)
+//   GEMM-2  hpsi[b][G]  = (V_loc psi)[b][G] + kin[G] psi[b][G] + sum_p P[p][G] c'[b][p]
+//                                                                M = npw, N = nband, K = nproj   (kinetic epilogue)
+//
+// Both GEMMs run on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> DMMA.8x8x4; sm_100a has no
+// tcgen05 FP64 kind) with operands staged by TMA (cp.async.bulk.tensor, 128-byte swizzle) through an
+// mbarrier ring filled by one elected thread.  Complex arithmetic is 4 real DMMAs per
+// 8x8x4 complex block: the (re, im) halves of a 16-byte element are the A/B fragments of two
+// different k-groups, so there is no operand re-packing and no wasted tensor work.
+//
+// Shared-memory layout of every operand tile: rows of 128 bytes (8 complex numbers), TMA
+// SWIZZLE_128B (16-byte chunk c of row r stored at chunk c ^ (r & 7)).  A DMMA k-group takes the
+// complex numbers {kg, kg+2, kg+4, kg+6} of a row (kg = 0, 1), which makes every LDS.128 of a
+// quarter-warp hit eight distinct chunks (conflict-free).
+#include <stdio.h>
+
+#include "internal.h"
+
+namespace dftb200 {
+
+constexpr int NL_BM = 128;        // rows of the M operand per CTA tile
+constexpr int NL_BN = 64;         // bands per CTA tile
+constexpr int NL_STAGES = 6;
+constexpr int NL_PREFETCH = NL_STAGES - 2;   // TMA runs this many slabs ahead of the MMA
+constexpr int NL_CONSUMERS = 8;   // warps: 4 (M) x 2 (N), 32 x 32 complex outputs each
+// 8 warps = 2 per SM sub-partition, so each thread may hold up to 255 registers (the 64 complex
+// accumulators alone are 128); a ninth (producer) warp would put 3 warps on one sub-partition and cap
+// the kernel at 168.  Lane 0 of warp 0 therefore also issues the TMA loads, NL_PREFETCH slabs ahead,
+// into a stage every warp released two iterations earlier (so it practically never waits).
+constexpr int NL_THREADS = NL_CONSUMERS * 32;
+constexpr int NL_STAGE_A = NL_BM * 128;   // 16 KB
+constexpr int NL_STAGE_B = NL_BN * 128;   // 8 KB
+constexpr int NL_STAGE_BYTES = NL_STAGE_A + NL_STAGE_B;
+constexpr int NL_SMEM = NL_STAGES * NL_STAGE_BYTES + 1024 + 256;
+
+// ---------------------------------------------------------------- PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ uint32_t mbar_try_wait(uint64_t *bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return ok;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {}
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+struct Gemm1Params {
+  int nproj, nband, nslab, nsplit, slabs_per_split, tiles_m, tiles_n;
+  double2 *part;   // [nkpt][nsplit][nproj][nband]
+};
+struct Gemm2Params {
+  int nproj, nband, mpw, nslab, tiles_n, accumulate, with_kin, with_nl;
+  const int32_t *npw;     // [nkpt] device
+  const double *const *kin;   // [nkpt] device pointers
+  const double2 *psi; double2 *hpsi;   // [nkpt][nband][mpw]
+};
+
+// The MMA main loop shared by both GEMMs.  MODE 1: acc += conj(A) B (GEMM-1); MODE 2: acc += A B.
+// As/Bs: one stage; A rows are addressed as a_row0 + mb*a_mb_stride bytes (+ row-in-block handled
+// by the caller-provided offsets).
+template <int MODE>
+__device__ __forceinline__ void mma_stage(const unsigned char *As, const unsigned char *Bs, int wm, int wn, int lane,
+                                          double (&cre)[4][4][2], double (&cim)[4][4][2]) {
+  const int i = lane >> 2, j = lane & 3;
+#pragma unroll
+  for (int kg = 0; kg < 2; kg++) {
+    double ar[4], ai[4], br[4], bi[4];
+    if (MODE == 1) {
+      // A tile [128 rows p][8 complex g]: row = wm*32 + mb*8 + i, chunk (2j+kg) ^ i
+      const unsigned char *a0 = As + (wm * 32 + i) * 128 + (((2 * j + kg) ^ i) << 4);
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++) {
+        double2 v = *reinterpret_cast<const double2 *>(a0 + mb * 8 * 128);
+        ar[mb] = v.x; ai[mb] = v.y;
+      }
+    } else {
+      // A tile [16 g-blocks][8 rows p][8 complex g]: block t = wm*4 + mb, row p = 2j+kg, chunk i ^ p
+      const int pr = 2 * j + kg;
+      const unsigned char *a0 = As + (wm * 4) * 1024 + pr * 128 + ((i ^ pr) << 4);
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++) {
+        double2 v = *reinterpret_cast<const double2 *>(a0 + mb * 1024);
+        ar[mb] = v.x; ai[mb] = v.y;
+      }
+    }
+    const unsigned char *b0 = Bs + (wn * 32 + i) * 128 + (((2 * j + kg) ^ i) << 4);
+#pragma unroll
+    for (int nb = 0; nb < 4; nb++) {
+      double2 v = *reinterpret_cast<const double2 *>(b0 + nb * 8 * 128);
+      br[nb] = v.x; bi[nb] = v.y;
+    }
+#pragma unroll
+    for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+      for (int nb = 0; nb < 4; nb++) dmma(cre[mb][nb][0], cre[mb][nb][1], ar[mb], br[nb]);
+#pragma unroll
+    for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+      for (int nb = 0; nb < 4; nb++) dmma(cim[mb][nb][0], cim[mb][nb][1], ar[mb], bi[nb]);
+    if (MODE == 1) {
+      // conj(p) psi: re += p_i psi_i, im -= p_i psi_r
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+        for (int nb = 0; nb < 4; nb++) dmma(cre[mb][nb][0], cre[mb][nb][1], ai[mb], bi[nb]);
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++) ai[mb] = -ai[mb];
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+        for (int nb = 0; nb < 4; nb++) dmma(cim[mb][nb][0], cim[mb][nb][1], ai[mb], br[nb]);
+    } else {
+      // p c: im += p_i c_r, re -= p_i c_i
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+        for (int nb = 0; nb < 4; nb++) dmma(cim[mb][nb][0], cim[mb][nb][1], ai[mb], br[nb]);
+#pragma unroll
+      for (int nb = 0; nb < 4; nb++) bi[nb] = -bi[nb];
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+        for (int nb = 0; nb < 4; nb++) dmma(cre[mb][nb][0], cre[mb][nb][1], ai[mb], bi[nb]);
+    }
+  }
+}
+
+struct Pipe {
+  unsigned char *tiles;
+  uint64_t *full, *empty;
+};
+__device__ __forceinline__ Pipe pipe_setup(unsigned char *smem_raw) {
+  Pipe P;
+  uintptr_t base = (reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023;
+  P.tiles = reinterpret_cast<unsigned char *>(base);
+  P.full = reinterpret_cast<uint64_t *>(P.tiles + NL_STAGES * NL_STAGE_BYTES);
+  P.empty = P.full + NL_STAGES;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < NL_STAGES; s++) { mbar_init(&P.full[s], 1); mbar_init(&P.empty[s], NL_CONSUMERS); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  return P;
+}
+
+// ---------------------------------------------------------------- GEMM-1: projection (split-K partials)
+// grid: (tiles_m*tiles_n, nsplit, nkpt)
+__global__ void __launch_bounds__(NL_THREADS, 1)
+gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapPsi, Gemm1Params Q) {
+  extern __shared__ unsigned char smem_raw[];
+  Pipe P = pipe_setup(smem_raw);
+  const int tile = blockIdx.x, tn = tile % Q.tiles_n, tm = tile / Q.tiles_n;
+  const int split = blockIdx.y, ik = blockIdx.z;
+  const int s0 = split * Q.slabs_per_split;
+  int ns = Q.nslab - s0; if (ns > Q.slabs_per_split) ns = Q.slabs_per_split; if (ns < 0) ns = 0;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  auto issue = [&](int j) {
+    int s = j % NL_STAGES;
+    if (j >= NL_STAGES) mbar_wait(&P.empty[s], ((j / NL_STAGES) - 1) & 1);
+    unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mbar_expect_tx(&P.full[s], NL_STAGE_BYTES);
+    tma_load_3d(st, &mapP, &P.full[s], (s0 + j) * 16, tm * NL_BM, ik);
+    tma_load_3d(st + NL_STAGE_A, &mapPsi, &P.full[s], (s0 + j) * 16, tn * NL_BN, ik);
+  };
+  const bool producer = (threadIdx.x == 0);
+  if (producer)
+    for (int j = 0; j < NL_PREFETCH && j < ns; j++) issue(j);
+  const int wm = warp >> 1, wn = warp & 1;
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
+  for (int it = 0; it < ns; it++) {
+    if (producer && it + NL_PREFETCH < ns) issue(it + NL_PREFETCH);
+    __syncwarp();
+    int s = it % NL_STAGES;
+    mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
+    const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mma_stage<1>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&P.empty[s]);
+  }
+  // partial[ik][split][p][b] complex; thread holds rows p = lane/4, bands 2*(lane%4)+{0,1} of each 8x8 block
+  double2 *out = Q.part + ((size_t)(ik * Q.nsplit + split) * Q.nproj) * Q.nband;
+  const int i = lane >> 2, j = lane & 3;
+#pragma unroll
+  for (int mb = 0; mb < 4; mb++) {
+    int pr = tm * NL_BM + wm * 32 + mb * 8 + i;
+    if (pr >= Q.nproj) continue;
+#pragma unroll
+    for (int nb = 0; nb < 4; nb++) {
+      int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j;
+      double2 *d = out + (size_t)pr * Q.nband + b;
+      if (b < Q.nband) d[0] = make_double2(cre[mb][nb][0], cim[mb][nb][0]);
+      if (b + 1 < Q.nband) d[1] = make_double2(cre[mb][nb][1], cim[mb][nb][1]);
+    }
+  }
+}
+
+// ---------------------------------------------------------------- D_ij + split-K reduction
+// c'[ik][b][first_a + i] = sum_j D^a_ij sum_s part[ik][s][first_a + j][b];  one thread per (b, a, ik), b fastest
+constexpr int DIJ_MAXL = 16;
+__global__ void dij_kernel(const double2 *__restrict__ part, double2 *__restrict__ cpr, const double *__restrict__ dij,
+                           const int32_t *__restrict__ typat, const int32_t *__restrict__ nlmn,
+                           const int32_t *__restrict__ atom_first, int natom, int lmax, int nproj, int nband, int nsplit) {
+  int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y, ik = blockIdx.z;
+  if (b >= nband) return;
+  int nl = nlmn[typat[a]], first = atom_first[a];
+  double2 c[DIJ_MAXL];
+  for (int jj = 0; jj < nl; jj++) {
+    double sr = 0.0, si = 0.0;
+    for (int s = 0; s < nsplit; s++) {
+      double2 v = part[((size_t)(ik * nsplit + s) * nproj + first + jj) * nband + b];
+      sr += v.x; si += v.y;
+    }
+    c[jj] = make_double2(sr, si);
+  }
+  const double *D = dij + (size_t)a * lmax * lmax;
+  double2 *dst = cpr + ((size_t)ik * nband + b) * nproj + first;
+  for (int ii = 0; ii < nl; ii++) {
+    double sr = 0.0, si = 0.0;
+    for (int jj = 0; jj < nl; jj++) { double d = D[ii * lmax + jj]; sr += d * c[jj].x; si += d * c[jj].y; }
+    dst[ii] = make_double2(sr, si);
+  }
+}
+
+// ---------------------------------------------------------------- GEMM-2: back-projection + kinetic epilogue
+// grid: (tiles_n * tiles_m, 1, nkpt), band tiles fastest so that concurrent CTAs share a slab of P in L2
+__global__ void __launch_bounds__(NL_THREADS, 1)
+gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapC, Gemm2Params Q) {
+  extern __shared__ unsigned char smem_raw[];
+  Pipe P = pipe_setup(smem_raw);
+  const int tn = blockIdx.x % Q.tiles_n, tm = blockIdx.x / Q.tiles_n, ik = blockIdx.z;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int ns = Q.with_nl ? Q.nslab : 0;
+  auto issue = [&](int j) {
+    int s = j % NL_STAGES;
+    if (j >= NL_STAGES) mbar_wait(&P.empty[s], ((j / NL_STAGES) - 1) & 1);
+    unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mbar_expect_tx(&P.full[s], NL_STAGE_BYTES);
+#pragma unroll 1
+    for (int t = 0; t < 16; t++) tma_load_3d(st + t * 1024, &mapP, &P.full[s], (tm * NL_BM + t * 8) * 2, j * 8, ik);
+    tma_load_3d(st + NL_STAGE_A, &mapC, &P.full[s], j * 16, tn * NL_BN, ik);
+  };
+  const bool producer = (threadIdx.x == 0);
+  if (producer)
+    for (int j = 0; j < NL_PREFETCH && j < ns; j++) issue(j);
+  const int wm = warp >> 1, wn = warp & 1;
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
+  for (int it = 0; it < ns; it++) {
+    if (producer && it + NL_PREFETCH < ns) issue(it + NL_PREFETCH);
+    __syncwarp();
+    int s = it % NL_STAGES;
+    mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
+    const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mma_stage<2>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&P.empty[s]);
+  }
+  // epilogue: hpsi[b][g] = (V_loc psi)[b][g] + kin[g] psi[b][g] + acc;  rows g = lane/4, bands 2*(lane%4)+{0,1}
+  const int npw = Q.npw[ik];
+  const double *kin = Q.kin[ik];
+  const double2 *psi = Q.psi + (size_t)ik * Q.nband * Q.mpw;
+  double2 *hpsi = Q.hpsi + (size_t)ik * Q.nband * Q.mpw;
+  const int i = lane >> 2, j = lane & 3;
+#pragma unroll
+  for (int mb = 0; mb < 4; mb++) {
+    int g = tm * NL_BM + wm * 32 + mb * 8 + i;
+    if (g >= npw) continue;
+    double kg = Q.with_kin ? kin[g] : 0.0;
+#pragma unroll
+    for (int nb = 0; nb < 4; nb++) {
+#pragma unroll
+      for (int e = 0; e < 2; e++) {
+        int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j + e;
+        if (b >= Q.nband) continue;
+        size_t off = (size_t)b * Q.mpw + g;
+        double2 r = make_double2(cre[mb][nb][e], cim[mb][nb][e]);
+        if (Q.with_kin) { double2 x = psi[off]; r.x += kg * x.x; r.y += kg * x.y; }
+        if (Q.accumulate) { double2 h = hpsi[off]; r.x += h.x; r.y += h.y; }
+        hpsi[off] = r;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- host side
+typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                             const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                             CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 3-D FP64 tensor map over a [d2][d1][d0] array (d0 contiguous doubles), box {16, box1, 1}, 128-byte swizzle
+static int make_map(dft_plan *p, CUtensorMap *m, const void *base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t stride1_bytes,
+                    uint64_t stride2_bytes, uint32_t box1) {
+  cuuint64_t dims[3] = {d0, d1, d2};
+  cuuint64_t strides[2] = {stride1_bytes, stride2_bytes};
+  cuuint32_t box[3] = {16, box1, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = ((EncodeFn)p->encode_fn)(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void *>(base), dims, strides, box, estr,
+                                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    set_error("cuTensorMapEncodeTiled failed (%d): dims %llu %llu %llu strides %llu %llu box1 %u", (int)r,
+              (unsigned long long)d0, (unsigned long long)d1, (unsigned long long)d2, (unsigned long long)stride1_bytes,
+              (unsigned long long)stride2_bytes, box1);
+    return DFT_ERR_CUDA;
+  }
+  return DFT_OK;
+}
+
+__global__ void kin_only_kernel(const double2 *__restrict__ psi, double2 *__restrict__ hpsi, const double *const *kin,
+                                const int32_t *npw, int nband, int mpw, int accumulate, int with_kin) {
+  int ik = blockIdx.z, b = blockIdx.y;
+  const double *k = kin[ik];
+  int n = npw[ik];
+  size_t row = ((size_t)ik * nband + b) * mpw;
+  for (int g = blockIdx.x * blockDim.x + threadIdx.x; g < n; g += gridDim.x * blockDim.x) {
+    double2 r = make_double2(0.0, 0.0);
+    if (with_kin) { double2 x = psi[row + g]; double kg = k[g]; r.x = kg * x.x; r.y = kg * x.y; }
+    if (accumulate) { double2 h = hpsi[row + g]; r.x += h.x; r.y += h.y; }
+    hpsi[row + g] = r;
+  }
+}
+
+static bool g_nl_attr = false;
+
+// choose the number of K splits of GEMM-1: fill the SMs in whole waves, keep >= 32 slabs per split
+static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
+  int best = 1; double best_eff = 0.0;
+  for (int s = 1; s <= 64; s++) {
+    if (s > 1 && nslab / s < 32) break;
+    double units = (double)tiles * s * nkpt;
+    double waves = units / sm_count;
+    double eff = waves / (double)(int64_t)(waves + 0.999999);
+    if (eff > best_eff + 0.01) { best_eff = eff; best = s; }
+  }
+  return best;
+}
+
+int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
+                   cudaStream_t st) {
+  if (p->mpw == 0 || nband == 0) return DFT_OK;
+  if (p->nproj == 0) with_nl = false;
+  if (!with_nl && !with_kin && accumulate) return DFT_OK;
+  if (!g_nl_attr) {
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    g_nl_attr = true;
+  }
+  const int32_t *d_npw = p->d_npw;
+  const double *const *d_kin = p->d_kinptr;
+  int rc;
+  const double2 *cpsi = reinterpret_cast<const double2 *>(psi);
+  double2 *chpsi = reinterpret_cast<double2 *>(hpsi);
+  if (!with_nl) {
+    dim3 grid((p->mpw + 255) / 256 < 64 ? (p->mpw + 255) / 256 : 64, nband, p->nkpt);
+    phase_begin(p, 7, st);
+    kin_only_kernel<<<grid, 256, 0, st>>>(cpsi, chpsi, d_kin, d_npw, nband, p->mpw, accumulate, with_kin);
+    phase_end(p, 7, st, 1);
+    DFT_CUDA_CHECK(cudaGetLastError());
+    return DFT_OK;
+  }
+  const int nproj = p->nproj, mpw = p->mpw, nkpt = p->nkpt;
+  // ---- GEMM-1
+  Gemm1Params q1;
+  q1.nproj = nproj; q1.nband = nband;
+  q1.nslab = (mpw + 7) / 8;
+  q1.tiles_m = (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
+  int ns = p->splitk > 0 ? p->splitk : choose_splitk(q1.tiles_m * q1.tiles_n, q1.nslab, p->sm_count, nkpt);
+  if (ns > q1.nslab) ns = q1.nslab;
+  q1.slabs_per_split = (q1.nslab + ns - 1) / ns;
+  ns = (q1.nslab + q1.slabs_per_split - 1) / q1.slabs_per_split;
+  q1.nsplit = ns;
+  int64_t need_part = (int64_t)nkpt * ns * nproj * nband * 16, need_cprj = (int64_t)nkpt * nband * nproj * 16;
+  if (need_part > p->part_bytes || !p->d_part) {
+    if (p->d_part) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_part); p->d_part = nullptr; }
+    if (cudaMalloc(&p->d_part, need_part) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes of split-K scratch", (long long)need_part); p->part_bytes = 0; return DFT_ERR_ALLOC; }
+    p->part_bytes = need_part;
+  }
+  if (need_cprj > p->cprj_bytes || !p->d_cprj) {
+    if (p->d_cprj) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_cprj); p->d_cprj = nullptr; }
+    if (cudaMalloc(&p->d_cprj, need_cprj) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes for cprj", (long long)need_cprj); p->cprj_bytes = 0; return DFT_ERR_ALLOC; }
+    p->cprj_bytes = need_cprj;
+  }
+  q1.part = reinterpret_cast<double2 *>(p->d_part);
+  CUtensorMap mapP1, mapPsi, mapP2, mapC;
+  uint64_t rowb = (uint64_t)mpw * 16;
+  if ((rc = make_map(p, &mapP1, p->d_ptab, 2 * (uint64_t)mpw, nproj, nkpt, rowb, rowb * nproj, NL_BM))) return rc;
+  if ((rc = make_map(p, &mapPsi, psi, 2 * (uint64_t)mpw, nband, nkpt, rowb, rowb * nband, NL_BN))) return rc;
+  if ((rc = make_map(p, &mapP2, p->d_ptab, 2 * (uint64_t)mpw, nproj, nkpt, rowb, rowb * nproj, 8))) return rc;
+  if ((rc = make_map(p, &mapC, p->d_cprj, 2 * (uint64_t)nproj, nband, nkpt, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * nband, NL_BN))) return rc;
+  phase_begin(p, 5, st);
+  gemm1_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  phase_end(p, 5, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  // ---- D_ij
+  phase_begin(p, 6, st);
+  dij_kernel<<<dim3((nband + 127) / 128, p->natom, nkpt), 128, 0, st>>>(q1.part, reinterpret_cast<double2 *>(p->d_cprj), p->d_dij,
+                                                                        p->d_typat, p->d_nlmn, p->d_atom_first, p->natom, p->lmax,
+                                                                        nproj, nband, ns);
+  phase_end(p, 6, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  // ---- GEMM-2
+  Gemm2Params q2;
+  q2.nproj = nproj; q2.nband = nband; q2.mpw = mpw; q2.nslab = (nproj + 7) / 8;
+  q2.tiles_n = q1.tiles_n; q2.accumulate = accumulate; q2.with_kin = with_kin; q2.with_nl = 1;
+  q2.npw = d_npw; q2.kin = d_kin; q2.psi = cpsi; q2.hpsi = chpsi;
+  int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
+  phase_begin(p, 7, st);
+  gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  phase_end(p, 7, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+}  // namespace dftb200

@@ -1,0 +1,478 @@
+// plan.cu -- the C ABI of include/dft.h: plan construction, setters, and dft_apply_h, which enqueues
+//
+//   fft_A(scatter) -> fft_B -> fft_C.V.C^-1 -> fft_B^-1 -> fft_A^-1(gather)      (fft.cu,  V_loc psi)
+//   gemm1 (cprj = P^H psi) -> dij -> gemm2 (+ kinetic epilogue, accumulates)     (nonlocal.cu)
+//
+// on the caller's stream without any host synchronisation (PAPER.md :438 "minimize host-device and
+// device-host transfers"; :456 the operation itself).
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "internal.h"
+
+namespace dftb200 {
+
+static thread_local char g_err[512] = "";
+void set_error(const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+void phase_begin(dft_plan *p, int phase, cudaStream_t st) {
+  if (!p->timer.on) return;
+  cudaEvent_t a, b;
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  cudaEventRecord(a, st);
+  p->timer.ev[phase].push_back({a, b});
+}
+void phase_end(dft_plan *p, int phase, cudaStream_t st, int launches) {
+  p->last_launches += launches;
+  if (!p->timer.on) return;
+  cudaEventRecord(p->timer.ev[phase].back().second, st);
+  p->timer.launches[phase] += launches;
+}
+
+template <typename T>
+static int to_device(T **dst, const T *src, size_t count) {
+  DFT_CUDA_CHECK(cudaMalloc((void **)dst, (count ? count : 1) * sizeof(T)));
+  if (count) DFT_CUDA_CHECK(cudaMemcpy(*dst, src, count * sizeof(T), cudaMemcpyHostToDevice));
+  return DFT_OK;
+}
+
+__global__ void scale_copy_kernel(const double *__restrict__ src, double *__restrict__ dst, int64_t n, double s) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) dst[i] = src[i] * s;
+}
+
+static void free_kpoint(KPoint &k) {
+  cudaFree(k.kg); cudaFree(k.igfft); cudaFree(k.kin); cudaFree(k.col_start); cudaFree(k.col_i2); cudaFree(k.col_plane);
+  cudaFree(k.pw_i1); cudaFree(k.plane_i3); cudaFree(k.plane_col0);
+}
+
+static void destroy_plan(dft_plan *p) {
+  if (!p) return;
+  for (auto &k : p->kp) free_kpoint(k);
+  cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
+  cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
+  cudaFree(p->d_dij); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
+  cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
+  if (p->host_stream) cudaStreamDestroy(p->host_stream);
+  for (int ph = 0; ph < 8; ph++)
+    for (auto &e : p->timer.ev[ph]) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
+  cudaGetLastError();
+  delete p;
+}
+
+static int create_impl(dft_plan *p, const double rprimd[9], int32_t nkpt, const double *kpt, double ecut, const int32_t ngfft[3],
+                       int32_t natom, const int32_t *typat, const double *xred, int32_t ntypat, const dft_proj_table *tables,
+                       const double *dij) {
+  int dev_count = 0;
+  if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) {
+    cudaGetLastError();
+    set_error("no CUDA device available (this library has no CPU path)");
+    return DFT_ERR_CUDA;
+  }
+  int dev = 0;
+  DFT_CUDA_CHECK(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  DFT_CUDA_CHECK(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major < 10) { set_error("device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor); return DFT_ERR_CUDA; }
+  p->sm_count = prop.multiProcessorCount;
+
+  // ---- lattice (reading 1)
+  for (int i = 0; i < 9; i++) {
+    if (!isfinite(rprimd[i])) { set_error("rprimd has a non-finite entry"); return DFT_ERR_INVALID_ARG; }
+    p->rprimd[i] = rprimd[i];
+  }
+  double det;
+  lattice_algebra(p->rprimd, p->bm, p->gmet, &det);
+  if (!(fabs(det) > 0.0) || !isfinite(det)) { set_error("lattice vectors are coplanar (det = %g)", det); return DFT_ERR_INVALID_ARG; }
+  p->ecut = ecut;
+  for (int c = 0; c < 3; c++) {
+    p->n[c] = ngfft[c];
+    if (ngfft[c] < 1 || ngfft[c] > 1024) { set_error("ngfft[%d] = %d outside 1..1024", c, ngfft[c]); return DFT_ERR_INVALID_ARG; }
+    if (!factorize(ngfft[c], &p->fac[c])) { set_error("ngfft[%d] = %d has a prime factor > 5", c, ngfft[c]); return DFT_ERR_UNSUPPORTED; }
+  }
+  p->nbox = (int64_t)p->n[0] * p->n[1] * p->n[2];
+  if (p->nbox >= ((int64_t)1 << 31)) { set_error("FFT box too large"); return DFT_ERR_UNSUPPORTED; }
+
+  // ---- atoms / projector metadata
+  p->natom = natom; p->ntypat = natom > 0 ? ntypat : 0;
+  p->lmax = 0; p->nrad_max = 0; p->nq_max = 0;
+  for (int t = 0; t < p->ntypat; t++) {
+    const dft_proj_table &T = tables[t];
+    if (T.nlmn < 0 || T.nlmn > 16) { set_error("type %d: nlmn = %d outside 0..16", t, T.nlmn); return DFT_ERR_INVALID_ARG; }
+    if (T.nlmn > 0 && (!T.l || !T.m || !T.irad || !T.f || !T.f2 || T.nrad < 1 || T.nq < 2 || !(T.dq > 0.0))) {
+      set_error("type %d: incomplete projector table", t); return DFT_ERR_INVALID_ARG;
+    }
+    for (int i = 0; i < T.nlmn; i++) {
+      if (T.l[i] < 0 || T.l[i] > 2) { set_error("type %d projector %d: l = %d unsupported (0..2)", t, i, T.l[i]); return DFT_ERR_UNSUPPORTED; }
+      if (T.m[i] < -T.l[i] || T.m[i] > T.l[i]) { set_error("type %d projector %d: m = %d outside -l..l", t, i, T.m[i]); return DFT_ERR_INVALID_ARG; }
+      if (T.irad[i] < 0 || T.irad[i] >= T.nrad) { set_error("type %d projector %d: irad = %d outside 0..nrad-1", t, i, T.irad[i]); return DFT_ERR_INVALID_ARG; }
+    }
+    if (T.nlmn > p->lmax) p->lmax = T.nlmn;
+    if (T.nlmn > 0) { if (T.nrad > p->nrad_max) p->nrad_max = T.nrad; if (T.nq > p->nq_max) p->nq_max = T.nq; }
+  }
+  p->typat.assign(typat, typat + natom);
+  p->xred.assign(xred, xred + 3 * (size_t)natom);
+  p->nlmn.resize(p->ntypat); p->nq.resize(p->ntypat); p->dq.resize(p->ntypat);
+  size_t lm = (size_t)p->ntypat * (p->lmax ? p->lmax : 1);
+  p->lmn_l.assign(lm, 0); p->lmn_m.assign(lm, 0); p->lmn_irad.assign(lm, 0);
+  std::vector<double> hf((size_t)p->ntypat * p->nrad_max * p->nq_max, 0.0), hf2(hf.size(), 0.0);
+  for (int t = 0; t < p->ntypat; t++) {
+    const dft_proj_table &T = tables[t];
+    p->nlmn[t] = T.nlmn; p->nq[t] = T.nlmn ? T.nq : 2; p->dq[t] = T.nlmn ? T.dq : 1e300;
+    for (int i = 0; i < T.nlmn; i++) { p->lmn_l[t * p->lmax + i] = T.l[i]; p->lmn_m[t * p->lmax + i] = T.m[i]; p->lmn_irad[t * p->lmax + i] = T.irad[i]; }
+    if (T.nlmn)
+      for (int r = 0; r < T.nrad; r++)
+        for (int j = 0; j < T.nq; j++) {
+          hf[((size_t)t * p->nrad_max + r) * p->nq_max + j] = T.f[(size_t)r * T.nq + j];
+          hf2[((size_t)t * p->nrad_max + r) * p->nq_max + j] = T.f2[(size_t)r * T.nq + j];
+        }
+  }
+  p->atom_first.resize(natom + 1);
+  p->nproj = 0;
+  for (int a = 0; a < natom; a++) {
+    if (typat[a] < 0 || typat[a] >= ntypat) { set_error("typat[%d] = %d outside 0..ntypat-1", a, typat[a]); return DFT_ERR_INVALID_ARG; }
+    for (int c = 0; c < 3; c++) if (!isfinite(xred[3 * a + c])) { set_error("xred of atom %d is not finite", a); return DFT_ERR_INVALID_ARG; }
+    p->atom_first[a] = p->nproj; p->nproj += p->nlmn[typat[a]];
+  }
+  p->atom_first[natom] = p->nproj;
+  if (natom > 65535) { set_error("natom > 65535 unsupported"); return DFT_ERR_UNSUPPORTED; }
+
+  // ---- K1: spheres
+  p->nkpt = nkpt;
+  p->kp.resize(nkpt);
+  p->mpw = 0;
+  const double TWO_PI = 6.283185307179586;
+  for (int ik = 0; ik < nkpt; ik++) {
+    KPoint &K = p->kp[ik];
+    for (int c = 0; c < 3; c++) {
+      K.k[c] = kpt[3 * ik + c];
+      if (!isfinite(K.k[c])) { set_error("k-point %d is not finite", ik); return DFT_ERR_INVALID_ARG; }
+    }
+    // |(k+m)_j| = |a_j . q|/(2 pi) <= |a_j| sqrt(2 ecut)/(2 pi): integer cube that surely contains the sphere
+    int bound[3], mmin[3], mmax[3];
+    for (int j = 0; j < 3; j++) {
+      const double *a = p->rprimd + 3 * j;
+      double len = sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+      double b = ceil(len * sqrt(2.0 * ecut) / TWO_PI + fabs(K.k[j])) + 1.0;
+      if (!(b < 4096.0)) { set_error("sphere extent along axis %d is too large", j); return DFT_ERR_UNSUPPORTED; }
+      bound[j] = (int)b;
+    }
+    int rc = sphere_extent(p->gmet, K.k, ecut, bound, mmin, mmax);
+    if (rc) return rc;
+    for (int j = 0; j < 3; j++)
+      if (mmin[j] <= mmax[j] && (mmin[j] < -(p->n[j] / 2) || mmax[j] > (p->n[j] - 1) / 2)) {
+        set_error("k-point %d: sphere spans m_%d in [%d, %d], FFT box n = %d holds [%d, %d]", ik, j + 1, mmin[j], mmax[j], p->n[j],
+                  -(p->n[j] / 2), (p->n[j] - 1) / 2);
+        return DFT_ERR_GRID_TOO_SMALL;
+      }
+    rc = sphere_build(p->gmet, p->n, ecut, &K);
+    if (rc) return rc;
+    if (K.npw > p->mpw) p->mpw = K.npw;
+  }
+  {
+    std::vector<int32_t> npw(nkpt);
+    std::vector<const double *> kin(nkpt);
+    for (int ik = 0; ik < nkpt; ik++) { npw[ik] = p->kp[ik].npw; kin[ik] = p->kp[ik].kin; }
+    int rc;
+    if ((rc = to_device(&p->d_npw, npw.data(), nkpt))) return rc;
+    if ((rc = to_device((const double ***)&p->d_kinptr, kin.data(), nkpt))) return rc;
+  }
+
+  // ---- device copies of the atom data, D_ij, projector table (S1)
+  int rc;
+  if ((rc = to_device(&p->d_typat, p->typat.data(), natom))) return rc;
+  if ((rc = to_device(&p->d_nlmn, p->nlmn.data(), p->ntypat))) return rc;
+  if ((rc = to_device(&p->d_lmn_l, p->lmn_l.data(), p->lmn_l.size()))) return rc;
+  if ((rc = to_device(&p->d_lmn_m, p->lmn_m.data(), p->lmn_m.size()))) return rc;
+  if ((rc = to_device(&p->d_lmn_irad, p->lmn_irad.data(), p->lmn_irad.size()))) return rc;
+  if ((rc = to_device(&p->d_atom_first, p->atom_first.data(), p->atom_first.size()))) return rc;
+  if ((rc = to_device(&p->d_nq, p->nq.data(), p->ntypat))) return rc;
+  if ((rc = to_device(&p->d_dq, p->dq.data(), p->ntypat))) return rc;
+  if ((rc = to_device(&p->d_xred, p->xred.data(), p->xred.size()))) return rc;
+  if ((rc = to_device(&p->d_f, hf.data(), hf.size()))) return rc;
+  if ((rc = to_device(&p->d_f2, hf2.data(), hf2.size()))) return rc;
+  size_t ndij = (size_t)natom * p->lmax * p->lmax;
+  if (ndij) {
+    if (!dij) { set_error("dij is NULL"); return DFT_ERR_INVALID_ARG; }
+    if ((rc = to_device(&p->d_dij, dij, ndij))) return rc;
+  }
+  size_t tab = (size_t)nkpt * p->nproj * p->mpw * 16;
+  if (tab) {
+    if (cudaMalloc(&p->d_ptab, tab + 256) != cudaSuccess) {
+      cudaGetLastError();
+      set_error("cannot allocate the projector table (%zu bytes)", tab);
+      return DFT_ERR_ALLOC;
+    }
+  }
+  for (int ik = 0; ik < nkpt; ik++) {
+    double maxq;
+    if ((rc = build_projector_table(p, ik, &maxq))) return rc;
+  }
+
+  // ---- twiddles exp(+2 pi i j/n) from long double
+  for (int c = 0; c < 3; c++) {
+    int n = p->n[c];
+    std::vector<double> tw(2 * (size_t)n);
+    const long double PI_L = 3.14159265358979323846264338327950288L;
+    for (int j = 0; j < n; j++) {
+      long double ang = 2.0L * PI_L * (long double)j / (long double)n;
+      tw[2 * j] = (double)cosl(ang); tw[2 * j + 1] = (double)sinl(ang);
+    }
+    if ((rc = to_device(&p->d_tw[c], tw.data(), tw.size()))) return rc;
+  }
+  DFT_CUDA_CHECK(cudaMalloc(&p->d_vloc, sizeof(double) * (size_t)p->nbox));
+
+  // ---- TMA descriptor encoder (driver entry point; no link against libcuda)
+  cudaDriverEntryPointQueryResult qres;
+  void *fn = nullptr;
+  DFT_CUDA_CHECK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+  if (!fn || qres != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled not available in this driver"); return DFT_ERR_CUDA; }
+  p->encode_fn = fn;
+  DFT_CUDA_CHECK(cudaDeviceSynchronize());
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+static int ensure_workspace(dft_plan *p, int64_t per_band, int nband, int *chunk_out, void **ws_out, cudaStream_t st) {
+  int chunk = p->band_chunk > 0 ? p->band_chunk : 0;
+  if (p->ws_user) {
+    int64_t fit = per_band > 0 ? p->ws_user_bytes / per_band : nband;
+    if (fit < 1) { set_error("workspace of %lld bytes is smaller than one band (%lld bytes)", (long long)p->ws_user_bytes, (long long)per_band); return DFT_ERR_ALLOC; }
+    if (chunk == 0 || chunk > fit) chunk = (int)(fit < 65535 ? fit : 65535);
+    if (chunk > nband) chunk = nband;
+    *chunk_out = chunk; *ws_out = p->ws_user;
+    return DFT_OK;
+  }
+  if (chunk == 0) {
+    int64_t target = (int64_t)2 << 30;   // about 2 GiB of pass-to-pass scratch
+    int64_t fit = per_band > 0 ? target / per_band : nband;
+    chunk = (int)(fit < 1 ? 1 : (fit > 4096 ? 4096 : fit));
+  }
+  if (chunk > nband) chunk = nband;
+  if (chunk > 65535) chunk = 65535;
+  int64_t need = per_band * chunk;
+  if (need > p->ws_own_bytes) {
+    if (p->ws_own) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->ws_own); p->ws_own = nullptr; p->ws_own_bytes = 0; }
+    if (cudaMalloc(&p->ws_own, need) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes of FFT scratch", (long long)need); return DFT_ERR_ALLOC; }
+    p->ws_own_bytes = need;
+  }
+  *chunk_out = chunk; *ws_out = p->ws_own;
+  return DFT_OK;
+}
+
+static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nband, cudaStream_t st) {
+  p->last_launches = 0;
+  if (nband == 0 || p->mpw == 0 || p->nkpt == 0) return DFT_OK;
+  const bool loc = (p->terms & 2) != 0, kin = (p->terms & 1) != 0, nl = (p->terms & 4) != 0 && p->nproj > 0;
+  if (loc && !p->vloc_set) { set_error("dft_apply_h called before dft_set_vloc"); return DFT_ERR_NOT_READY; }
+  int rc;
+  const size_t band_stride = (size_t)p->mpw * 2;
+  if (loc) {
+    int chunk; void *ws;
+    if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
+    for (int ik = 0; ik < p->nkpt; ik++)
+      for (int b0 = 0; b0 < nband; b0 += chunk) {
+        int nb = nband - b0 < chunk ? nband - b0 : chunk;
+        size_t off = ((size_t)ik * nband + b0) * band_stride;
+        if ((rc = fft_apply_vloc(p, ik, psi + off, hpsi + off, nb, ws, st))) return rc;
+      }
+  } else {
+    phase_begin(p, 4, st);
+    if ((rc = zero_fill(hpsi, (int64_t)p->nkpt * nband * band_stride, st))) return rc;
+    phase_end(p, 4, st, 1);
+  }
+  if (kin || nl)
+    if ((rc = nonlocal_apply(p, psi, hpsi, nband, true, kin, nl, st))) return rc;
+  return DFT_OK;
+}
+
+}  // namespace dftb200
+
+using namespace dftb200;
+
+#define DFT_GUARD_BEGIN try {
+#define DFT_GUARD_END                                          \
+  } catch (const std::bad_alloc &) {                           \
+    set_error("host allocation failed");                       \
+    return DFT_ERR_ALLOC;                                      \
+  } catch (...) {                                              \
+    set_error("unexpected internal error");                    \
+    return DFT_ERR_INVALID_ARG;                                \
+  }
+
+extern "C" {
+
+const char *dft_last_error(void) { return g_err; }
+
+int dft_plan_create(dft_plan **out, const double rprimd[9], int32_t nkpt, const double *kpt, double ecut, const int32_t ngfft[3],
+                    int32_t natom, const int32_t *typat, const double *xred, int32_t ntypat, const dft_proj_table *tables,
+                    const double *dij) {
+  DFT_GUARD_BEGIN
+  if (!out || !rprimd || !kpt || !ngfft) { set_error("null argument"); return DFT_ERR_INVALID_ARG; }
+  if (nkpt < 1) { set_error("nkpt = %d must be >= 1", nkpt); return DFT_ERR_INVALID_ARG; }
+  if (!(ecut > 0.0) || !isfinite(ecut)) { set_error("ecut = %g must be positive and finite", ecut); return DFT_ERR_INVALID_ARG; }
+  if (natom < 0 || ntypat < 0) { set_error("negative natom/ntypat"); return DFT_ERR_INVALID_ARG; }
+  if (natom > 0 && (!typat || !xred || !tables || ntypat < 1)) { set_error("atoms given without typat/xred/tables"); return DFT_ERR_INVALID_ARG; }
+  dft_plan *p = new dft_plan();
+  int rc = create_impl(p, rprimd, nkpt, kpt, ecut, ngfft, natom, typat, xred, ntypat, tables, dij);
+  if (rc != DFT_OK) { destroy_plan(p); return rc; }
+  *out = p;
+  return DFT_OK;
+  DFT_GUARD_END
+}
+
+int dft_plan_get_info(const dft_plan *p, int32_t *nkpt, int32_t *npw, int32_t *mpw, int32_t *nproj, int64_t *ws_per_band) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nkpt) *nkpt = p->nkpt;
+  if (npw) for (int ik = 0; ik < p->nkpt; ik++) npw[ik] = p->kp[ik].npw;
+  if (mpw) *mpw = p->mpw;
+  if (nproj) *nproj = p->nproj;
+  if (ws_per_band) *ws_per_band = fft_ws_bytes_per_band(p);
+  return DFT_OK;
+}
+
+int dft_plan_get_kg(const dft_plan *p, int32_t ik, int32_t *kg, int32_t *igfft, double *kin) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (ik < 0 || ik >= p->nkpt) { set_error("ik = %d outside 0..%d", ik, p->nkpt - 1); return DFT_ERR_INVALID_ARG; }
+  const KPoint &K = p->kp[ik];
+  if (kg && K.npw) memcpy(kg, K.h_kg.data(), sizeof(int32_t) * 3 * (size_t)K.npw);
+  if (igfft && K.npw) memcpy(igfft, K.h_igfft.data(), sizeof(int32_t) * (size_t)K.npw);
+  if (kin && K.npw) memcpy(kin, K.h_kin.data(), sizeof(double) * (size_t)K.npw);
+  return DFT_OK;
+}
+
+int dft_plan_get_projectors(const dft_plan *p, int32_t ik, double *ptab) {
+  if (!p || !ptab) { set_error("null argument"); return DFT_ERR_INVALID_ARG; }
+  if (ik < 0 || ik >= p->nkpt) { set_error("ik = %d outside 0..%d", ik, p->nkpt - 1); return DFT_ERR_INVALID_ARG; }
+  int npw = p->kp[ik].npw;
+  if (p->nproj == 0 || npw == 0) return DFT_OK;
+  const double *src = p->d_ptab + (size_t)ik * p->nproj * p->mpw * 2;
+  DFT_CUDA_CHECK(cudaMemcpy2D(ptab, (size_t)npw * 16, src, (size_t)p->mpw * 16, (size_t)npw * 16, p->nproj, cudaMemcpyDeviceToHost));
+  return DFT_OK;
+}
+
+int dft_set_dij(dft_plan *p, const double *dij) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  size_t n = (size_t)p->natom * p->lmax * p->lmax;
+  if (n == 0) return DFT_OK;
+  if (!dij) { set_error("dij is NULL"); return DFT_ERR_INVALID_ARG; }
+  DFT_CUDA_CHECK(cudaMemcpy(p->d_dij, dij, n * sizeof(double), cudaMemcpyHostToDevice));
+  return DFT_OK;
+}
+
+int dft_set_vloc(dft_plan *p, const double *V_r, void *stream) {
+  if (!p || !V_r) { set_error("null argument"); return DFT_ERR_INVALID_ARG; }
+  cudaStream_t st = (cudaStream_t)stream;
+  int64_t n = p->nbox;
+  int grid = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
+  scale_copy_kernel<<<grid, 256, 0, st>>>(V_r, p->d_vloc, n, 1.0 / (double)n);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  p->vloc_set = true;
+  return DFT_OK;
+}
+
+int dft_set_workspace(dft_plan *p, void *dev_ptr, int64_t bytes) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (dev_ptr && (bytes <= 0 || ((uintptr_t)dev_ptr & 255))) { set_error("workspace must be 256-byte aligned with bytes > 0"); return DFT_ERR_INVALID_ARG; }
+  if (dev_ptr && bytes < fft_ws_bytes_per_band(p)) { set_error("workspace smaller than one band (%lld bytes needed)", (long long)fft_ws_bytes_per_band(p)); return DFT_ERR_ALLOC; }
+  p->ws_user = dev_ptr; p->ws_user_bytes = dev_ptr ? bytes : 0;
+  return DFT_OK;
+}
+
+int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
+  if (!p || !key) { set_error("null argument"); return DFT_ERR_INVALID_ARG; }
+  if (!strcmp(key, "band_chunk")) {
+    if (value < 0 || value > 65535) { set_error("band_chunk = %lld outside 0..65535", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->band_chunk = (int)value; return DFT_OK;
+  }
+  if (!strcmp(key, "terms")) {
+    if (value < 0 || value > 7) { set_error("terms = %lld outside 0..7", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->terms = (int)value; return DFT_OK;
+  }
+  if (!strcmp(key, "splitk")) {
+    if (value < 0 || value > 4096) { set_error("splitk = %lld outside 0..4096", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->splitk = (int)value; return DFT_OK;
+  }
+  set_error("unknown option '%s'", key);
+  return DFT_ERR_INVALID_ARG;
+}
+
+int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  if (nband > 0 && p->mpw > 0 && (!psi || !hpsi)) { set_error("null psi/hpsi"); return DFT_ERR_INVALID_ARG; }
+  if (((uintptr_t)psi & 15) || ((uintptr_t)hpsi & 15)) { set_error("psi/hpsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  return apply_impl(p, psi, hpsi, nband, (cudaStream_t)stream);
+  DFT_GUARD_END
+}
+
+int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int32_t nband) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  int64_t bytes = (int64_t)p->nkpt * nband * p->mpw * 16;
+  if (bytes == 0) return DFT_OK;
+  if (!psi_host || !hpsi_host) { set_error("null psi/hpsi"); return DFT_ERR_INVALID_ARG; }
+  if (!p->host_stream) DFT_CUDA_CHECK(cudaStreamCreateWithFlags(&p->host_stream, cudaStreamNonBlocking));
+  if (bytes > p->stage_bytes) {
+    cudaFree(p->d_stage_in); cudaFree(p->d_stage_out); p->d_stage_in = p->d_stage_out = nullptr; p->stage_bytes = 0;
+    if (cudaMalloc(&p->d_stage_in, bytes) != cudaSuccess || cudaMalloc(&p->d_stage_out, bytes) != cudaSuccess) {
+      cudaGetLastError(); cudaFree(p->d_stage_in); p->d_stage_in = nullptr;
+      set_error("cannot allocate 2 x %lld bytes of device staging", (long long)bytes);
+      return DFT_ERR_ALLOC;
+    }
+    p->stage_bytes = bytes;
+  }
+  cudaStream_t st = p->host_stream;
+  DFT_CUDA_CHECK(cudaMemcpyAsync(p->d_stage_in, psi_host, bytes, cudaMemcpyHostToDevice, st));
+  int rc = apply_impl(p, p->d_stage_in, p->d_stage_out, nband, st);
+  if (rc) return rc;
+  DFT_CUDA_CHECK(cudaMemcpyAsync(hpsi_host, p->d_stage_out, bytes, cudaMemcpyDeviceToHost, st));
+  DFT_CUDA_CHECK(cudaStreamSynchronize(st));
+  return DFT_OK;
+  DFT_GUARD_END
+}
+
+int64_t dft_plan_last_launches(const dft_plan *p) { return p ? p->last_launches : 0; }
+
+int dft_plan_set_timing(dft_plan *p, int32_t on) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  p->timer.on = on != 0;
+  return DFT_OK;
+}
+
+int dft_plan_phase_ms(dft_plan *p, int32_t phase, double *ms, int64_t *launches) {
+  if (!p || phase < 0 || phase >= 8) { set_error("bad phase"); return DFT_ERR_INVALID_ARG; }
+  double tot = 0.0;
+  for (auto &e : p->timer.ev[phase]) {
+    DFT_CUDA_CHECK(cudaEventSynchronize(e.second));
+    float t = 0.f;
+    DFT_CUDA_CHECK(cudaEventElapsedTime(&t, e.first, e.second));
+    tot += t;
+    cudaEventDestroy(e.first); cudaEventDestroy(e.second);
+  }
+  p->timer.ev[phase].clear();
+  if (ms) *ms = tot;
+  if (launches) *launches = p->timer.launches[phase];
+  p->timer.launches[phase] = 0;
+  return DFT_OK;
+}
+
+int dft_plan_destroy(dft_plan *p) {
+  if (!p) return DFT_OK;
+  cudaDeviceSynchronize();
+  destroy_plan(p);
+  return DFT_OK;
+}
+
+}  // extern "C"

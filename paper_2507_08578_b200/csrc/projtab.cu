@@ -1,0 +1,138 @@
+// projtab.cu -- S1: materialise the non-local projectors of Eq. 26 (PAPER.md :470) in device memory,
+// the "projectors ... computed and stored in memory" variant of :479.
+//
+//   p_{a,i}(m) = F_{t(a),irad_i}(|q|) . Y_{l_i m_i}(q^) . exp(-2 pi i (k+m).x_a),   q = 2 pi (k+m)^T Bm
+//
+// Readings: 6 form of the projector, 7 cubic-spline evaluation of the radial
+// table, 8 real spherical harmonics without Condon-Shortley sign, m = -l..l, 11 phase argument
+// reduced mod 1.  Layout: P[ik][row][mpw] complex128, row = atom_first[a] + i, zero for ipw >= npw_k,
+// i.e. K-contiguous for GEMM-1 and M-contiguous for GEMM-2 (nonlocal.cu).
+#include <math.h>
+
+#include "internal.h"
+
+namespace dftb200 {
+
+struct ProjParams {
+  double bm[9];
+  double k[3];
+  int npw, mpw, natom, lmax, nrad_max, nq_max;
+  const int32_t *kg;
+  const int32_t *typat, *nlmn, *lmn_l, *lmn_m, *lmn_irad, *atom_first, *nq;
+  const double *dq, *xred, *f, *f2;
+  double *ptab;   // this k-point's [nproj][mpw] complex
+};
+
+// reading 7
+__device__ __forceinline__ double spline_eval(int nq, double dq, const double *f, const double *f2, double q) {
+  int j = (int)floor(q / dq);
+  if (j > nq - 2) j = nq - 2;
+  if (j < 0) j = 0;
+  double A = ((double)(j + 1) * dq - q) / dq, B = 1.0 - A;
+  return A * f[j] + B * f[j + 1] + ((A * A * A - A) * f2[j] + (B * B * B - B) * f2[j + 1]) * (dq * dq) / 6.0;
+}
+
+// reading 8: orthonormal real harmonics; (x,y,z) = q vector, qn = |q|.  l > 0 at q = 0 gives 0.
+__device__ __forceinline__ double real_ylm(int l, int m, double x, double y, double z, double qn) {
+  const double PI = 3.14159265358979323846;
+  if (l == 0) return 0.5 / sqrt(PI);
+  if (qn == 0.0) return 0.0;
+  if (l == 1) {
+    double c = sqrt(3.0 / (4.0 * PI));
+    double v = (m == -1) ? y : ((m == 0) ? z : x);
+    return c * v / qn;
+  }
+  double q2 = qn * qn;
+  double c1 = 0.5 * sqrt(15.0 / PI), c0 = 0.25 * sqrt(5.0 / PI), c2 = 0.25 * sqrt(15.0 / PI);
+  switch (m) {
+    case -2: return c1 * x * y / q2;
+    case -1: return c1 * y * z / q2;
+    case 0:  return c0 * (3.0 * z * z - q2) / q2;
+    case 1:  return c1 * x * z / q2;
+    default: return c2 * (x * x - y * y) / q2;
+  }
+}
+
+constexpr int PT_THREADS = 128;
+constexpr int PT_MAXRAD = 8;
+
+// grid: (ceil(mpw / PT_THREADS), natom); one thread = one plane wave of one atom, writes nlmn rows
+__global__ void __launch_bounds__(PT_THREADS) projtab_kernel(ProjParams P) {
+  int g = blockIdx.x * PT_THREADS + threadIdx.x;
+  int a = blockIdx.y;
+  if (g >= P.mpw) return;
+  int t = P.typat[a], nl = P.nlmn[t];
+  double2 *dst = reinterpret_cast<double2 *>(P.ptab) + (size_t)P.atom_first[a] * P.mpw + g;
+  if (g >= P.npw) {
+    for (int i = 0; i < nl; i++) dst[(size_t)i * P.mpw] = make_double2(0.0, 0.0);
+    return;
+  }
+  const double TWO_PI = 6.283185307179586;
+  double t0 = P.k[0] + (double)P.kg[3 * g], t1 = P.k[1] + (double)P.kg[3 * g + 1], t2 = P.k[2] + (double)P.kg[3 * g + 2];
+  double qx = TWO_PI * (t0 * P.bm[0] + t1 * P.bm[3] + t2 * P.bm[6]);
+  double qy = TWO_PI * (t0 * P.bm[1] + t1 * P.bm[4] + t2 * P.bm[7]);
+  double qz = TWO_PI * (t0 * P.bm[2] + t1 * P.bm[5] + t2 * P.bm[8]);
+  double qn = sqrt(qx * qx + qy * qy + qz * qz);
+  // reading 11: exp(-2 pi i frac((k+m).x_a))
+  const double *x = P.xred + 3 * a;
+  double arg = t0 * x[0] + t1 * x[1] + t2 * x[2];
+  arg -= floor(arg);
+  double sn, cs;
+  sincospi(2.0 * arg, &sn, &cs);
+  sn = -sn;
+  double frad[PT_MAXRAD];
+  bool have[PT_MAXRAD];
+#pragma unroll
+  for (int r = 0; r < PT_MAXRAD; r++) have[r] = false;
+  for (int i = 0; i < nl; i++) {
+    int ir = P.lmn_irad[t * P.lmax + i];
+    double F;
+    if (ir < PT_MAXRAD && have[ir]) {
+      F = frad[ir];
+    } else {
+      size_t off = ((size_t)t * P.nrad_max + ir) * P.nq_max;
+      F = spline_eval(P.nq[t], P.dq[t], P.f + off, P.f2 + off, qn);
+      if (ir < PT_MAXRAD) { frad[ir] = F; have[ir] = true; }
+    }
+    double fy = F * real_ylm(P.lmn_l[t * P.lmax + i], P.lmn_m[t * P.lmax + i], qx, qy, qz, qn);
+    dst[(size_t)i * P.mpw] = make_double2(fy * cs, fy * sn);
+  }
+}
+
+int build_projector_table(dft_plan *p, int ik, double *maxq_out) {
+  KPoint &kp = p->kp[ik];
+  // max |k+G| (host, O(npw)) for the table-range check of the boundary
+  double mx = 0.0;
+  const double TWO_PI = 6.283185307179586;
+  for (int g = 0; g < kp.npw; g++) {
+    double t0 = kp.k[0] + kp.h_kg[3 * g], t1 = kp.k[1] + kp.h_kg[3 * g + 1], t2 = kp.k[2] + kp.h_kg[3 * g + 2];
+    double q2 = 0.0;
+    for (int c = 0; c < 3; c++) {
+      double q = TWO_PI * (t0 * p->bm[c] + t1 * p->bm[3 + c] + t2 * p->bm[6 + c]);
+      q2 += q * q;
+    }
+    if (q2 > mx) mx = q2;
+  }
+  *maxq_out = sqrt(mx);
+  if (p->natom == 0 || p->nproj == 0 || p->mpw == 0) return DFT_OK;
+  for (int t = 0; t < p->ntypat; t++)
+    if (*maxq_out > (p->nq[t] - 1) * p->dq[t]) {
+      set_error("k-point %d: max|k+G| = %.6f exceeds the radial table range (nq-1)*dq = %.6f of type %d", ik,
+                *maxq_out, (p->nq[t] - 1) * p->dq[t], t);
+      return DFT_ERR_TABLE_RANGE;
+    }
+  ProjParams P;
+  for (int i = 0; i < 9; i++) P.bm[i] = p->bm[i];
+  for (int i = 0; i < 3; i++) P.k[i] = kp.k[i];
+  P.npw = kp.npw; P.mpw = p->mpw; P.natom = p->natom; P.lmax = p->lmax; P.nrad_max = p->nrad_max; P.nq_max = p->nq_max;
+  P.kg = kp.kg; P.typat = p->d_typat; P.nlmn = p->d_nlmn; P.lmn_l = p->d_lmn_l; P.lmn_m = p->d_lmn_m;
+  P.lmn_irad = p->d_lmn_irad; P.atom_first = p->d_atom_first; P.nq = p->d_nq; P.dq = p->d_dq; P.xred = p->d_xred;
+  P.f = p->d_f; P.f2 = p->d_f2;
+  P.ptab = p->d_ptab + (size_t)ik * p->nproj * p->mpw * 2;
+  dim3 grid((p->mpw + PT_THREADS - 1) / PT_THREADS, p->natom);
+  projtab_kernel<<<grid, PT_THREADS>>>(P);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+}  // namespace dftb200

@@ -244,3 +244,23 @@ def gen_psi(cfg, kin_list, nband=None, bands=None, threads=8):
         for t in jobs:
             work(t)
     return psi
+
+
+def gen_psi_torch(cfg, kin_list, device, nband=None):
+    """Same block as gen_psi, drawn on a torch device: tensor [nkpt][nband][mpw] complex128."""
+    import torch
+    nband = cfg["nband"] if nband is None else nband
+    mpw = max(len(k) for k in kin_list)
+    nk = len(kin_list)
+    psi = torch.zeros((nk, nband, mpw), dtype=torch.complex128, device=device)
+    for ik, kin in enumerate(kin_list):
+        npw = len(kin)
+        env = 1.0 / (1.0 + 2.0 * torch.as_tensor(np.asarray(kin), device=device))
+        step = max(1, (1 << 24) // max(npw, 1))
+        for b0 in range(0, nband, step):
+            b1 = min(nband, b0 + step)
+            flat = torch.arange(ik * cfg["nband"] + b0, ik * cfg["nband"] + b1, device=device, dtype=torch.int64)
+            idx = flat[:, None] * mpw + torch.arange(npw, device=device, dtype=torch.int64)[None, :]
+            n0, n1 = rng.torch_normals_pair(cfg["seed"], STREAM_PSI, idx)
+            psi[ik, b0:b1, :npw] = torch.complex(n0 * env, n1 * env)
+    return psi

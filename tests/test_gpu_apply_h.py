@@ -1,0 +1,143 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle: H psi to <= 1e-10 relative per band
+(BASELINE.json north_star), on the five configs and the extra cases of SURVEY.md 8(c)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from gpu_util import (make_plan, lib_spheres, oracle_spheres, assert_spheres_equal, gpu_apply, oracle_apply,
+                      band_rel_err)
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10     # north_star: "relative error <= 1e-10 per band in FP64"
+
+
+def _setup(name, **over):
+    cfg = synth.make_config(name, **over)
+    plan = make_plan(cfg)
+    sph = lib_spheres(plan)
+    assert_spheres_equal(sph, oracle_spheres(cfg))
+    return cfg, plan, sph
+
+
+@pytest.mark.parametrize("name", ["c0", "c1m", "c2m", "c4m", "aniso", "c3k2"])
+def test_small_cells_all_terms_and_isolations(name):
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    for terms in (7, 1, 2, 4, 3, 6):
+        plan.set_option("terms", terms)
+        got = gpu_apply(plan, psi)
+        ref = oracle_apply(cfg, sph, psi, terms=terms, method=1 if name in ("c0", "aniso") else 2)
+        err = band_rel_err(got, ref)
+        assert err <= TOL, "%s terms=%d: rel err %.3e" % (name, terms, err)
+        for ik in range(plan.nkpt):                      # pad entries are written as 0
+            assert np.all(got[ik][:, plan.npw[ik]:] == 0)
+    plan.destroy()
+
+
+def test_c0_against_dense_h():
+    """tier T0: explicit dense H_{GG'} on the tiny cell (north_star: 'brute-force dense H on the tiny cell')."""
+    cfg, plan, sph = _setup("c0")
+    kg, ig, kin = sph[0]
+    psi = synth.gen_psi(cfg, [kin])
+    H = oracle.dense_h(cfg, 0, kg, kin)
+    ref = np.stack([oracle.dense_matvec(H, psi[0, b]) for b in range(psi.shape[1])])[None]
+    err = band_rel_err(gpu_apply(plan, psi), ref)
+    assert err <= TOL, err
+    plan.destroy()
+
+
+@pytest.mark.parametrize("nband", [1, 3, 64, 65])
+def test_band_counts_and_chunking(nband):
+    cfg, plan, sph = _setup("c1m")
+    psi = synth.gen_psi(cfg, [s[2] for s in sph], nband=nband)
+    ref = oracle_apply(cfg, sph, psi)
+    for chunk in (0, 1, 7):
+        plan.set_option("band_chunk", chunk)
+        err = band_rel_err(gpu_apply(plan, psi), ref)
+        assert err <= TOL, "nband=%d chunk=%d: %.3e" % (nband, chunk, err)
+    plan.destroy()
+
+
+def test_projector_table_matches_oracle():
+    for name in ("c0", "aniso", "c3k2"):
+        cfg, plan, sph = _setup(name)
+        for ik in range(plan.nkpt):
+            ref = oracle.projector_table(cfg, ik, sph[ik][0])
+            got = plan.get_projectors(ik)
+            assert np.max(np.abs(got - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
+        plan.destroy()
+
+
+def test_tight_box_wraparound():
+    """SURVEY.md 8(c) case (iii): a box that just holds the sphere (n_j = 2 m_max + 1 -> heavy aliasing wrap)."""
+    cfg, plan, sph = _setup("c0", ngfft=(9, 9, 9))
+    psi = synth.gen_psi(cfg, [sph[0][2]])
+    err = band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, method=1))
+    assert err <= TOL, err
+    plan.destroy()
+
+
+def test_set_dij_and_user_workspace_and_host_api():
+    cfg, plan, sph = _setup("c1m")
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    d2 = cfg["dij"] * 0.5 + 0.1 * np.eye(cfg["nlmn_max"])[None]
+    plan.set_dij(d2)
+    ws = torch.empty(plan.workspace_bytes_per_band * 2 + 256, dtype=torch.uint8, device="cuda")
+    off = (-ws.data_ptr()) % 256
+    plan.set_workspace(ws[off:off + plan.workspace_bytes_per_band * 2])
+    ref = oracle_apply(cfg, sph, psi, dij=d2)
+    assert band_rel_err(gpu_apply(plan, psi), ref) <= TOL
+    got_host = plan.apply_h_host(psi)
+    assert band_rel_err(got_host, ref) <= TOL
+    plan.set_workspace(None)
+    assert band_rel_err(gpu_apply(plan, psi), ref) <= TOL
+    assert plan.last_launches() == 8
+    plan.destroy()
+
+
+def test_c1_full():
+    cfg, plan, sph = _setup("c1")
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    err = band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi))
+    assert err <= TOL, err
+    plan.destroy()
+
+
+def test_c3_full_multik_batch():
+    cfg, plan, sph = _setup("c3")
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    err = band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi))
+    assert err <= TOL, err
+    plan.destroy()
+
+
+def _sampled_full_size(name, sample):
+    """Full-size run in bench.py's launch configuration; the oracle computes a seeded sample of bands
+    one by one (bands are independent, PAPER.md :436)."""
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi_torch(cfg, [s[2] for s in sph], "cuda")
+    out = plan.apply_h(psi)
+    torch.cuda.synchronize()
+    psi_s = psi[:, sample].cpu().numpy()
+    got = out[:, sample].cpu().numpy()
+    ref = oracle_apply(cfg, sph, psi_s)
+    err = band_rel_err(got, ref)
+    assert err <= TOL, "%s sampled bands %s: %.3e" % (name, sample, err)
+    # property at full size: Hermiticity <phi|H psi> = <H phi|psi> on two other bands
+    a, b = 1, cfg["nband"] - 2
+    lhs = torch.vdot(psi[0, a], out[0, b]); rhs = torch.vdot(out[0, a], psi[0, b])
+    scale = torch.linalg.norm(psi[0, a]) * torch.linalg.norm(out[0, b])
+    assert abs(lhs - rhs) <= 1e-11 * scale
+    plan.destroy()
+    del psi, out
+    torch.cuda.empty_cache()
+
+
+def test_c2_full_size_sampled():
+    _sampled_full_size("c2", [0, 217, 431])
+
+
+def test_c4_full_size_sampled():
+    _sampled_full_size("c4", [5, 1023])

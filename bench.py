@@ -1,0 +1,292 @@
+#!/usr/bin/env python
+"""bench.py -- H|psi> bands/s (FP64) on B200, with roofline and CPU-oracle context.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c4] [--impl reference]
+
+A "step" is one pass of the whole hot path (dft_apply_h: five pruned-FFT passes, GEMM-1, D_ij, GEMM-2 with
+kinetic epilogue) over one batch of synthetic bands.  Default workload: BASELINE.json configs[4] (Si512, 180^3,
+1024 bands, 4096 projectors), the cell north_star's >= 60 %-of-roofline target is quoted on; it fits one GPU.
+Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for the definition of every field.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "H|psi> bands/s (FP64)"
+UNIT = "bands/s"
+FP64_PEAK_TFLOPS = 37.2      # 148 SM x 4 sub-partitions x one DMMA.8x8x4 (512 flop) per 16 clk x 1.965 GHz
+WORKLOADS = {
+    "c0": "c0: Si2 FCC, Gamma, ecut 8 Ha, box 20^3, 8 bands, 16 projectors",
+    "c1": "c1: Si64, k=(1/4,1/4,1/4), ecut 15 Ha, box 72^3, 128 bands, 512 projectors",
+    "c2": "c2: Si216, Gamma, ecut 20 Ha, box 128^3, 432 bands, 1728 projectors",
+    "c3": "c3: Al4 x 32 k-points (4x4x2 MP), ecut 20 Ha, box 32^3, 64 bands per k, 36 projectors",
+    "c4": "c4: Si512, Gamma, ecut 20 Ha, box 180^3, 1024 bands, 4096 projectors (BASELINE.json configs[4])",
+}
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz, self._stop, self._t = [], set(), None, threading.Event(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20,
+                 "hw_power_brake": 0x80, "sync_boost": 0x10, "display_clock_setting": 0x100}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        if self.nv:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._t:
+            self._t.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+
+
+def geometry(plan):
+    """Sizes the byte/flop model needs, from the library's own index maps (ik = 0 .. nkpt-1)."""
+    n1, n2, n3 = plan.ngfft
+    out = []
+    for ik in range(plan.nkpt):
+        _, ig, _ = plan.get_kg(ik)
+        col = np.unique(ig // n1)
+        out.append(dict(npw=len(ig), ncol=len(col), nplane=len(np.unique(col // n2))))
+    return out
+
+
+def byte_flop_model(plan, geo, nband):
+    """Algorithmic bytes of the five pruned FFT passes and flops of the two GEMMs for ONE step."""
+    n1, n2, n3 = plan.ngfft
+    fft = dict(A=0.0, B=0.0, C=0.0, Binv=0.0, Ainv=0.0)
+    g1 = g2 = 0.0
+    for g in geo:
+        a = 16.0 * g["npw"]; b = 16.0 * g["ncol"] * n1; c = 16.0 * n1 * n2 * g["nplane"]
+        fft["A"] += nband * (a + b); fft["B"] += nband * (b + c); fft["C"] += nband * 2 * c
+        fft["Binv"] += nband * (c + b); fft["Ainv"] += nband * (b + a)
+        g1 += 8.0 * plan.nproj * g["npw"] * nband
+        g2 += 8.0 * plan.nproj * g["npw"] * nband
+    return fft, g1, g2
+
+
+def oracle_sample(cfg, nsample, steps, warmup):
+    """Times the CPU oracle, as it stands, on `nsample` bands of the workload per step."""
+    import oracle
+    import synth
+    sph = [oracle.sphere(cfg["rprimd"], cfg["kpt"][ik], cfg["ecut"], cfg["ngfft"]) for ik in range(cfg["nkpt"])]
+    bands = list(range(nsample))
+    psi = synth.gen_psi(cfg, [s[2] for s in sph], bands=bands)
+    ts = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        for ik, (kg, ig, kin) in enumerate(sph):
+            oracle.apply_h(cfg, ik, kg, ig, kin, psi[ik], method=2)
+        if it >= warmup:
+            ts.append(time.perf_counter() - t0)
+    per_step = sum(ts) / len(ts)
+    return cfg["nkpt"] * nsample / per_step, per_step, oracle.num_threads()
+
+
+def run_reference(args, cfg, rank):
+    if rank != 0:
+        return
+    nsample = args.ref_bands if args.ref_bands else {"c4": 4, "c2": 8, "c1": 64, "c3": 16, "c0": 8}[args.config]
+    nsample = min(nsample, cfg["nband"])
+    value, per_step, cores = oracle_sample(cfg, nsample, args.steps, min(args.warmup, 1))
+    sample = "%d bands x %d k-point(s) of %s per step, oracle tier T2 (own mixed-radix FFT) + direct-loop non-local" % (
+        nsample, cfg["nkpt"], args.config)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.config], "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--nband", type=int, default=0, help="override the band count (experiments only)")
+    ap.add_argument("--band-chunk", type=int, default=0)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (experiments only)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the e2e leg (experiments only)")
+    ap.add_argument("--ref-bands", type=int, default=0)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    import synth
+    cfg = synth.make_config(args.config, with_vloc=(args.impl == "ours" or True))
+    if args.nband:
+        cfg["nband"] = args.nband
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+
+    import torch
+    import paper_2507_08578_b200 as dft
+    from paper_2507_08578_b200 import sharding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        sharding.init("nccl")
+    W = max(3, args.warmup); K = max(1, args.steps)
+
+    plan = dft.Plan(cfg)
+    if args.band_chunk:
+        plan.set_option("band_chunk", args.band_chunk)
+    plan.set_vloc(torch.as_tensor(cfg["vloc"], device="cuda"))
+    kin_list = [plan.get_kg(ik)[2] for ik in range(plan.nkpt)]
+    nband = cfg["nband"]
+    # weak scaling: every rank owns its own block of nband bands (rank r draws bands r*nband ..), no collective
+    cfg_r = dict(cfg, seed=cfg["seed"] + 1000 * rank)
+    psi = synth.gen_psi_torch(cfg_r, kin_list, "cuda")
+    hpsi = torch.empty_like(psi)
+    geo = geometry(plan)
+    fft_bytes, g1_flops, g2_flops = byte_flop_model(plan, geo, nband)
+    hbm_gbs, hbm_src = measured_peaks()
+
+    for _ in range(W):
+        plan.apply_h(psi, hpsi)
+    torch.cuda.synchronize()
+    plan.set_timing(True)
+    sampler = ClockSampler(local); sampler.start()
+    sharding.barrier(); torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        plan.apply_h(psi, hpsi)
+    e1.record()
+    torch.cuda.synchronize(); sharding.barrier()
+    clocks = sampler.stop()
+    ms_total = sharding.max_over_ranks(e0.elapsed_time(e1))
+    launches = plan.last_launches() * K
+    phases = plan.phase_ms()
+    plan.set_timing(False)
+    ms_step = ms_total / K
+    units = plan.nkpt * nband * world
+    value = units / (ms_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (largest share of the step), per launch
+    ph_ms = {k: v[0] / K for k, v in phases.items()}
+    ph_n = {k: max(1, v[1] // K) for k, v in phases.items()}
+    fft_names = {"fft_A_scatter": "A", "fft_B": "B", "fft_C_V_Cinv": "C", "fft_Binv": "Binv", "fft_Ainv_gather": "Ainv"}
+    per_kernel = {}
+    for name, key in fft_names.items():
+        if ph_ms[name] > 0:
+            per_kernel[name] = {"bound": "hbm", "ms_per_step": ph_ms[name], "launches_per_step": ph_n[name],
+                                "achieved": fft_bytes[key] / (ph_ms[name] * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
+    for name, fl in (("gemm1", g1_flops), ("gemm2_kinetic", g2_flops)):
+        if ph_ms[name] > 0 and fl > 0:
+            per_kernel[name] = {"bound": "tensor", "ms_per_step": ph_ms[name], "launches_per_step": ph_n[name],
+                                "achieved": fl / (ph_ms[name] * 1e-3) / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s"}
+    for v in per_kernel.values():
+        v["frac"] = v["achieved"] / v["peak"]
+    dom = max(per_kernel, key=lambda k: per_kernel[k]["ms_per_step"])
+    d = per_kernel[dom]
+    roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],
+                "frac": d["frac"], "traffic": None,
+                "peak_source": ("FP64 DMMA: 148 SM x 4 x 512 flop / 16 clk x 1.965 GHz (microbenchmark 37.06), "
+                                "DESIGN.md 8" if d["bound"] == "tensor" else hbm_src),
+                "share_of_step": d["ms_per_step"] / ms_step}
+    t_roof = sum(fft_bytes.values()) / (hbm_gbs * 1e9) + (g1_flops + g2_flops) / (FP64_PEAK_TFLOPS * 1e12)
+    path = {"t_roof_ms": t_roof * 1e3, "frac": t_roof * 1e3 / ms_step,
+            "definition": "sum_phases max(bytes/HBM_measured, flops/FP64_peak) / measured step time",
+            "kernels": per_kernel}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.config], "nband_per_gpu": nband, "nkpt": plan.nkpt,
+                       "npw": [int(v) for v in plan.npw][:4], "fft_box": list(plan.ngfft), "nproj": plan.nproj,
+                       "parallelism": "bands sharded over %d GPU(s), no collective" % world,
+                       "l2": "inputs larger than L2 between iterations (psi+hpsi %.2f GB, projector table %.2f GB)" % (
+                           2 * psi.numel() * 16 / 1e9, plan.nkpt * plan.nproj * plan.mpw * 16 / 1e9)},
+            "clocks": clocks, "gpu_launches": launches, "roofline": roofline, "roofline_path": path}
+
+    # ---- e2e: same metric through dft_apply_h_host, host<->device copies inside the timed region
+    if not args.no_e2e:
+        psi_h = torch.empty(psi.shape, dtype=psi.dtype, pin_memory=True)
+        psi_h.copy_(psi)
+        hpsi_h = torch.empty(psi.shape, dtype=psi.dtype, pin_memory=True)
+        del hpsi
+        torch.cuda.empty_cache()
+        plan.apply_h_host(psi_h, hpsi_h)
+        ke = min(K, 3)
+        sharding.barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            plan.apply_h_host(psi_h, hpsi_h)
+        dt = sharding.max_over_ranks((time.perf_counter() - t0) * 1e3) / ke
+        nbytes = psi_h.numel() * 16
+        line["e2e"] = {"value": units / (dt * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+                       "d2h_bytes_per_step": nbytes, "ms_per_step": dt, "steps": ke,
+                       "api": "dft_apply_h_host (pinned host psi -> device, H, device -> pinned host hpsi)"}
+    plan.destroy()
+
+    # ---- cpu_baseline: the oracle as it stands, bounded sample, rank 0 at N=1 only
+    if rank == 0 and world == 1 and not args.no_cpu:
+        nsample = min(cfg["nband"], {"c4": 8, "c2": 16, "c1": 128, "c3": 64, "c0": 8}[args.config])
+        v, per_step, cores = oracle_sample(cfg, nsample, 1, 0)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": "%d bands x %d k-point(s) of %s, one pass (%.1f s), tier T2 FFT + direct-loop "
+                                          "non-local" % (nsample, cfg["nkpt"], args.config, per_step)}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    sharding.shutdown()
+
+
+if __name__ == "__main__":
+    main()

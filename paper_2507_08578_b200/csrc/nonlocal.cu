@@ -70,6 +70,11 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, u
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
       ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
 __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
@@ -269,8 +274,8 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
     if (j >= NL_STAGES) mbar_wait(&P.empty[s], ((j / NL_STAGES) - 1) & 1);
     unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
     mbar_expect_tx(&P.full[s], NL_STAGE_BYTES);
-#pragma unroll 1
-    for (int t = 0; t < 16; t++) tma_load_3d(st + t * 1024, &mapP, &P.full[s], (tm * NL_BM + t * 8) * 2, j * 8, ik);
+    // one box {16 doubles, 8 projector rows, 16 g-blocks}: lands as [g-block][p][8 complex], 128-byte swizzled
+    tma_load_4d(st, &mapP, &P.full[s], 0, j * 8, tm * (NL_BM / 8), ik);
     tma_load_3d(st + NL_STAGE_A, &mapC, &P.full[s], j * 16, tn * NL_BN, ik);
   };
   const bool producer = (threadIdx.x == 0);
@@ -422,7 +427,21 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   uint64_t rowb = (uint64_t)mpw * 16;
   if ((rc = make_map(p, &mapP1, p->d_ptab, 2 * (uint64_t)mpw, nproj, nkpt, rowb, rowb * nproj, NL_BM))) return rc;
   if ((rc = make_map(p, &mapPsi, psi, 2 * (uint64_t)mpw, nband, nkpt, rowb, rowb * nband, NL_BN))) return rc;
-  if ((rc = make_map(p, &mapP2, p->d_ptab, 2 * (uint64_t)mpw, nproj, nkpt, rowb, rowb * nproj, 8))) return rc;
+  {
+    // GEMM-2 reads P "M-major": view each table row as [g-block][16 doubles] and put the projector
+    // index between them, so ONE box {16, 8 rows, 16 g-blocks} brings a 128 g x 8 p tile in the
+    // [g-block][p][8 complex] order the fragments want (16 separate 1 KB boxes starved the MMA loop:
+    // profiles/r1_gemm2_tma.md).  The last g-block of a row may run into the next row (or the 256-byte
+    // pad after the table); those values only reach output rows g >= npw, which are never stored.
+    cuuint64_t dims[4] = {16, (cuuint64_t)nproj, ((cuuint64_t)mpw + 7) / 8, (cuuint64_t)nkpt};
+    cuuint64_t strides[3] = {rowb, 128, rowb * nproj};
+    cuuint32_t box[4] = {16, 8, NL_BM / 8, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = ((EncodeFn)p->encode_fn)(&mapP2, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, p->d_ptab, dims, strides, box, estr,
+                                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (GEMM-2 P map) failed (%d)", (int)r); return DFT_ERR_CUDA; }
+  }
   if ((rc = make_map(p, &mapC, p->d_cprj, 2 * (uint64_t)nproj, nband, nkpt, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * nband, NL_BN))) return rc;
   phase_begin(p, 5, st);
   gemm1_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);

@@ -20,6 +20,7 @@
 // conflict-free.
 #include <math.h>
 
+#include "fft_codelets.cuh"
 #include "internal.h"
 
 namespace dftb200 {
@@ -46,88 +47,6 @@ bool factorize(int n, FftFactors *f) {
   return f->nfac <= 12;
 }
 
-// ------------------------------------------------------------------------------------------
-// complex helpers and radix butterflies:  X[q] = sum_r v[r] w^(q r),  w = exp(S 2 pi i / R)
-// ------------------------------------------------------------------------------------------
-typedef double2 cplx;
-__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-__device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a.x * s, a.y * s); }
-// multiply by S*i
-template <int S> __device__ __forceinline__ cplx mul_si(cplx a) {
-  return S > 0 ? make_double2(-a.y, a.x) : make_double2(a.y, -a.x);
-}
-
-template <int S> __device__ __forceinline__ void bfly2(cplx &a, cplx &b) {
-  cplx t = csub(a, b); a = cadd(a, b); b = t;
-}
-template <int S> __device__ __forceinline__ void bfly3(cplx &v0, cplx &v1, cplx &v2) {
-  const double H = 0.86602540378443864676;  // sqrt(3)/2
-  cplx t = cadd(v1, v2), u = mul_si<S>(cscale(csub(v1, v2), H));
-  cplx m = make_double2(v0.x - 0.5 * t.x, v0.y - 0.5 * t.y);
-  v0 = cadd(v0, t); v1 = cadd(m, u); v2 = csub(m, u);
-}
-template <int S> __device__ __forceinline__ void bfly4(cplx &v0, cplx &v1, cplx &v2, cplx &v3) {
-  cplx t0 = cadd(v0, v2), t1 = csub(v0, v2), t2 = cadd(v1, v3), t3 = mul_si<S>(csub(v1, v3));
-  v0 = cadd(t0, t2); v2 = csub(t0, t2); v1 = cadd(t1, t3); v3 = csub(t1, t3);
-}
-template <int S> __device__ __forceinline__ void bfly5(cplx &v0, cplx &v1, cplx &v2, cplx &v3, cplx &v4) {
-  const double C1 = 0.30901699437494742410, C2 = -0.80901699437494742410;  // cos(2pi/5), cos(4pi/5)
-  const double S1 = 0.95105651629515357212, S2 = 0.58778525229247312917;   // sin(2pi/5), sin(4pi/5)
-  cplx a1 = cadd(v1, v4), a2 = cadd(v2, v3), b1 = csub(v1, v4), b2 = csub(v2, v3);
-  cplx m1 = make_double2(v0.x + C1 * a1.x + C2 * a2.x, v0.y + C1 * a1.y + C2 * a2.y);
-  cplx m2 = make_double2(v0.x + C2 * a1.x + C1 * a2.x, v0.y + C2 * a1.y + C1 * a2.y);
-  cplx u1 = mul_si<S>(make_double2(S1 * b1.x + S2 * b2.x, S1 * b1.y + S2 * b2.y));
-  cplx u2 = mul_si<S>(make_double2(S2 * b1.x - S1 * b2.x, S2 * b1.y - S1 * b2.y));
-  v0 = cadd(v0, cadd(a1, a2));
-  v1 = cadd(m1, u1); v4 = csub(m1, u1);
-  v2 = cadd(m2, u2); v3 = csub(m2, u2);
-}
-
-template <int R, int S> struct Bfly;
-template <int S> struct Bfly<2, S> { static __device__ __forceinline__ void run(cplx *v) { bfly2<S>(v[0], v[1]); } };
-template <int S> struct Bfly<3, S> { static __device__ __forceinline__ void run(cplx *v) { bfly3<S>(v[0], v[1], v[2]); } };
-template <int S> struct Bfly<4, S> { static __device__ __forceinline__ void run(cplx *v) { bfly4<S>(v[0], v[1], v[2], v[3]); } };
-template <int S> struct Bfly<5, S> { static __device__ __forceinline__ void run(cplx *v) { bfly5<S>(v[0], v[1], v[2], v[3], v[4]); } };
-// 8 = 2 x 4 (decimation in time: even/odd halves, then X[q] = E[q] + w8^q O[q], X[q+4] = E[q] - w8^q O[q])
-template <int S> struct Bfly<8, S> {
-  static __device__ __forceinline__ void run(cplx *v) {
-    const double Q = 0.70710678118654752440;
-    bfly4<S>(v[0], v[2], v[4], v[6]);   // E[0..3] in v0,v2,v4,v6
-    bfly4<S>(v[1], v[3], v[5], v[7]);   // O[0..3] in v1,v3,v5,v7
-    cplx o1 = make_double2(Q * (v[3].x - S * v[3].y), Q * (v[3].y + S * v[3].x));       // w8^1 = (1 + S i)/sqrt2
-    cplx o2 = mul_si<S>(v[5]);                                                           // w8^2 = S i
-    cplx o3 = make_double2(Q * (-v[7].x - S * v[7].y), Q * (-v[7].y + S * v[7].x));     // w8^3 = (-1 + S i)/sqrt2
-    cplx e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
-    v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
-    v[1] = cadd(e1, o1); v[5] = csub(e1, o1);
-    v[2] = cadd(e2, o2); v[6] = csub(e2, o2);
-    v[3] = cadd(e3, o3); v[7] = csub(e3, o3);
-  }
-};
-// 9 = 3 x 3:  r = 3a + b, q = q1 + 3 q2;  Y_b[q1] = DFT3_a v[3a+b];  X[q1+3q2] = DFT3_b (w9^(b q1) Y_b[q1])
-template <int S> struct Bfly<9, S> {
-  static __device__ __forceinline__ void run(cplx *v) {
-    const double C1 = 0.76604444311897803520, S1 = 0.64278760968653932632;   // cos/sin(2pi/9)
-    const double C2 = 0.17364817766693034885, S2 = 0.98480775301220805937;   // cos/sin(4pi/9)
-    const double C4 = -0.93969262078590838405, S4 = 0.34202014332566873304;  // cos/sin(8pi/9)
-    bfly3<S>(v[0], v[3], v[6]);   // b = 0: Y_0[q1] in v0,v3,v6
-    bfly3<S>(v[1], v[4], v[7]);   // b = 1
-    bfly3<S>(v[2], v[5], v[8]);   // b = 2
-    // twiddles w9^(b q1): (b,q1) = (1,1)->w, (1,2)->w^2, (2,1)->w^2, (2,2)->w^4
-    v[4] = cmul(v[4], make_double2(C1, S * S1));
-    v[7] = cmul(v[7], make_double2(C2, S * S2));
-    v[5] = cmul(v[5], make_double2(C2, S * S2));
-    v[8] = cmul(v[8], make_double2(C4, S * S4));
-    bfly3<S>(v[0], v[1], v[2]);   // q1 = 0: X[0], X[3], X[6]
-    bfly3<S>(v[3], v[4], v[5]);   // q1 = 1: X[1], X[4], X[7]
-    bfly3<S>(v[6], v[7], v[8]);   // q1 = 2: X[2], X[5], X[8]
-    cplx x1 = v[3], x2 = v[6], x3 = v[1], x4 = v[4], x5 = v[7], x6 = v[2], x7 = v[5];
-    v[1] = x1; v[2] = x2; v[3] = x3; v[4] = x4; v[5] = x5; v[6] = x6; v[7] = x7;
-  }
-};
-
 struct FacDev { int nfac; int radix[12]; };
 
 // One Stockham pass of radix R over `nlines` lines held in shared memory.
@@ -152,7 +71,7 @@ __device__ __forceinline__ void stockham_pass(const cplx *__restrict__ in, cplx 
         v[r] = cmul(v[r], t);
       }
     }
-    Bfly<R, S>::run(v);
+    Dft<R, S>::run(v);
     int j0 = (j / Ns) * Ns * R + k;
     cplx *dst = out + l * ls + j0 * es;
 #pragma unroll
@@ -408,21 +327,22 @@ int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb,
   size_t sm_b = sizeof(cplx) * ((size_t)G.n2 + 2 * (size_t)G.n2 * G.XT);
   size_t sm_c = sizeof(cplx) * ((size_t)G.n3 + 2 * (size_t)G.n3 * G.XT);
   dim3 ga((G.ncol + G.CL - 1) / G.CL, nb), gb(G.nxt, G.nplane, nb), gc(G.nxt, G.n2, nb);
-  phase_begin(p, 0, st);
-  fft_pass_a_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, cpsi, T1);
-  phase_end(p, 0, st, 1);
-  phase_begin(p, 1, st);
-  fft_pass_b_kernel<+1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
-  phase_end(p, 1, st, 1);
-  phase_begin(p, 2, st);
-  fft_pass_c_kernel<<<gc, FFT_THREADS, sm_c, st>>>(G, T2, p->d_vloc);
-  phase_end(p, 2, st, 1);
-  phase_begin(p, 3, st);
-  fft_pass_b_kernel<-1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
-  phase_end(p, 3, st, 1);
-  phase_begin(p, 4, st);
-  fft_pass_ainv_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, T1, chpsi);
-  phase_end(p, 4, st, 1);
+  // per pass: the register-resident two-stage kernel (fft2.cu) when the axis length factorises into two
+  // codelet radices and the sphere's occupied sets are runs; otherwise the generic Stockham kernel
+  bool fast[3];
+  for (int c = 0; c < 3; c++) fast[c] = p->fft_path == 0 && kp.runs_ok && fft2_pair(p->n[c], nullptr, nullptr);
+  const int axis_of[5] = {0, 1, 2, 1, 0};
+  for (int pass = 0; pass < 5; pass++) {
+    phase_begin(p, pass, st);
+    if (fast[axis_of[pass]]) {
+      if ((rc = fft2_launch(p, ik, pass, psi, hpsi, T1, T2, G.t1_band, G.t2_band, nb, st))) return rc;
+    } else if (pass == 0) fft_pass_a_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, cpsi, T1);
+    else if (pass == 1) fft_pass_b_kernel<+1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
+    else if (pass == 2) fft_pass_c_kernel<<<gc, FFT_THREADS, sm_c, st>>>(G, T2, p->d_vloc);
+    else if (pass == 3) fft_pass_b_kernel<-1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
+    else fft_pass_ainv_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, T1, chpsi);
+    phase_end(p, pass, st, 1);
+  }
   DFT_CUDA_CHECK(cudaGetLastError());
   return DFT_OK;
 }

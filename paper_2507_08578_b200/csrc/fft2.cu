@@ -1,0 +1,378 @@
+// fft2.cu -- K2, register-resident path: every 1-D transform of the five pruned passes (fft.cu header,
+// SURVEY.md 8(a) S3-S7; PAPER.md :475 "local part using fast Fourier transforms", :436 batched over bands)
+// is ONE two-stage decomposition n = R1 * R2 done in registers with a single shared-memory exchange:
+//
+//   type I  (G -> r, w = exp(+2 pi i/n)):  j = j2 + R2 j1,  k = k1 + R1 k2
+//       thread j2:  Y[k1] = sum_j1 x[j2 + R2 j1] w_R1^(j1 k1);   Z[k1] = Y[k1] w_n^(j2 k1)      (radix R1, R2 threads)
+//       exchange;   thread k1:  X[k1 + R1 k2] = sum_j2 Z_j2[k1] w_R2^(j2 k2)                    (radix R2, R1 threads)
+//   type II (r -> G, w = exp(-2 pi i/n)):  j = a + R1 b,    k = c + R2 d
+//       thread a:   Y[c] = sum_b x[a + R1 b] w_R2^(b c);         Z[c] = Y[c] w_n^(a c)          (radix R2, R1 threads)
+//       exchange;   thread c:   X[c + R2 d] = sum_a Z_a[c] w_R1^(a d)                           (radix R1, R2 threads)
+//
+// Type II consumes exactly the register layout type I produces (thread k1 holds k1 + R1 k2) and returns
+// the layout type I reads (thread j2 holds j2 + R2 j1), so pass C (forward along z, times V(r)/N,
+// inverse along z) touches shared memory twice per line instead of twelve times, and every global
+// access goes straight from/to registers: along y and z a warp's lanes are consecutive x (contiguous runs
+// of XT complex numbers); along x the lanes are the consecutive slots j2 / k1 / a / c of one line.
+// Pruning: the occupied x of a column, y of a plane and z of the box are (at most) two runs of
+// consecutive box indices each (the sphere is convex), so "is this input non-zero / is this output
+// kept" is two range checks (struct Run) and the sphere <-> box maps need no index list.
+#include "fft_codelets.cuh"
+#include "internal.h"
+
+namespace dftb200 {
+
+__device__ __forceinline__ int run_map(const Run &r, int x) {
+  unsigned d = (unsigned)(x - r.lo);
+  if (d < (unsigned)r.nlo) return r.base + (int)d;
+  d = (unsigned)(x - r.hi);
+  if (d < (unsigned)r.nhi) return r.base + r.nlo + (int)d;
+  return -1;
+}
+__device__ __forceinline__ Run load_run(const Run *p) {
+  const int4 *q = reinterpret_cast<const int4 *>(p);
+  int4 a = __ldg(q), b = __ldg(q + 1);
+  Run r; r.base = a.x; r.lo = a.y; r.nlo = a.z; r.hi = a.w; r.nhi = b.x; r.aux0 = b.y; r.aux1 = b.z; r.pad = b.w;
+  return r;
+}
+__device__ __forceinline__ cplx ldtw(const cplx *tw, int i) {
+  return __ldg(tw + i);
+}
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b) {   // a * conj(b)
+  return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+constexpr int F2_THREADS = 256;
+__host__ __device__ constexpr int imax(int a, int b) { return a > b ? a : b; }
+__host__ __device__ constexpr int pad8(int len, int want) { return len + (((want - len) % 8) + 8) % 8; }   // smallest >= len congruent to want mod 8
+
+struct Fft2Geom {
+  int n1, n2, n3, npw, mpw, ncol, nplane;
+  const Run *col_run, *plane_run;
+  Run zrun;
+  const cplx *tw1, *tw2, *tw3;
+  int64_t t1_band, t2_band;   // complex elements per band of T1 [ncol][n1] and T2 [nplane][n2][n1]
+};
+
+// ---- pass A: sphere -> x-lines (type I).  block = lpc lines x NS slots, slot fastest; grid = nb * ntile
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_a_fwd_kernel(Fft2Geom G, const cplx *__restrict__ psi, cplx *__restrict__ T1, int lpc, int ntile) {
+  constexpr int NS = imax(R1, R2), KS = R2 | 1, LS = pad8(R1 * KS, NS);
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *sm = reinterpret_cast<cplx *>(smem_raw);
+  const int t = threadIdx.x, s = t % NS, l = t / NS;
+  const int tile = blockIdx.x % ntile, b = blockIdx.x / ntile;
+  const int c = tile * lpc + l;
+  const bool ok = c < G.ncol;
+  Run r = load_run(G.col_run + (ok ? c : 0));
+  cplx v[NS];
+  if (s < R2) {
+    const cplx *src = psi + (size_t)b * G.mpw;
+#pragma unroll
+    for (int j1 = 0; j1 < R1; j1++) {
+      int g = ok ? run_map(r, s + R2 * j1) : -1;
+      v[j1] = g >= 0 ? src[g] : make_double2(0.0, 0.0);
+    }
+    Dft<R1, +1>::run(v);
+#pragma unroll
+    for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw1, s * k1));
+#pragma unroll
+    for (int k1 = 0; k1 < R1; k1++) sm[l * LS + k1 * KS + s] = v[k1];
+  }
+  __syncthreads();
+  if (s < R1) {
+#pragma unroll
+    for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[l * LS + s * KS + j2];
+    Dft<R2, +1>::run(v);
+    if (ok) {
+      cplx *dst = T1 + (size_t)b * G.t1_band + (size_t)c * G.n1 + s;
+#pragma unroll
+      for (int k2 = 0; k2 < R2; k2++) dst[R1 * k2] = v[k2];
+    }
+  }
+}
+
+// ---- pass A^-1: x-lines -> sphere (type II) + zero the pad entries ipw >= npw of the band
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_a_inv_kernel(Fft2Geom G, const cplx *__restrict__ T1, cplx *__restrict__ hpsi, int lpc, int ntile) {
+  constexpr int NS = imax(R1, R2), KS = R1 | 1, LS = pad8(R2 * KS, NS);
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *sm = reinterpret_cast<cplx *>(smem_raw);
+  const int t = threadIdx.x, s = t % NS, l = t / NS;
+  const int tile = blockIdx.x % ntile, b = blockIdx.x / ntile;
+  const int c = tile * lpc + l;
+  const bool ok = c < G.ncol;
+  Run r = load_run(G.col_run + (ok ? c : 0));
+  cplx v[NS];
+  if (s < R1) {
+    const cplx *src = T1 + (size_t)b * G.t1_band + (size_t)(ok ? c : 0) * G.n1 + s;
+#pragma unroll
+    for (int b2 = 0; b2 < R2; b2++) v[b2] = ok ? src[R1 * b2] : make_double2(0.0, 0.0);
+    Dft<R2, -1>::run(v);
+#pragma unroll
+    for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw1, s * cc));
+#pragma unroll
+    for (int cc = 0; cc < R2; cc++) sm[l * LS + cc * KS + s] = v[cc];
+  }
+  __syncthreads();
+  cplx *dst = hpsi + (size_t)b * G.mpw;
+  if (s < R2) {
+#pragma unroll
+    for (int a = 0; a < R1; a++) v[a] = sm[l * LS + s * KS + a];
+    Dft<R1, -1>::run(v);
+#pragma unroll
+    for (int d = 0; d < R1; d++) {
+      int g = ok ? run_map(r, s + R2 * d) : -1;
+      if (g >= 0) dst[g] = v[d];
+    }
+  }
+  if (tile == ntile - 1)
+    for (int g = G.npw + t; g < G.mpw; g += blockDim.x) dst[g] = make_double2(0.0, 0.0);
+}
+
+// ---- pass B: along y on the occupied planes (type I).  block = NS slots x XT consecutive x, x fastest;
+//      grid = nb * nplane * nxt.  Shared exchange element (k1, j2, px) at k1*KS + j2*XT + px.
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_b_fwd_kernel(Fft2Geom G, const cplx *__restrict__ T1, cplx *__restrict__ T2, int XT, int nxt) {
+  constexpr int NS = imax(R1, R2);
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *sm = reinterpret_cast<cplx *>(smem_raw);
+  const int t = threadIdx.x, px = t % XT, s = t / XT;
+  const int xt = blockIdx.x % nxt, p = (blockIdx.x / nxt) % G.nplane, b = blockIdx.x / (nxt * G.nplane);
+  const int x = xt * XT + px;
+  const bool xok = x < G.n1;
+  const int KS = pad8(R2 * XT, XT);
+  Run r = load_run(G.plane_run + p);
+  cplx v[NS];
+  if (s < R2) {
+    const cplx *src = T1 + (size_t)b * G.t1_band + x;
+#pragma unroll
+    for (int j1 = 0; j1 < R1; j1++) {
+      int c = xok ? run_map(r, s + R2 * j1) : -1;
+      v[j1] = c >= 0 ? src[(size_t)c * G.n1] : make_double2(0.0, 0.0);
+    }
+    Dft<R1, +1>::run(v);
+#pragma unroll
+    for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw2, s * k1));
+#pragma unroll
+    for (int k1 = 0; k1 < R1; k1++) sm[k1 * KS + s * XT + px] = v[k1];
+  }
+  __syncthreads();
+  if (s < R1) {
+#pragma unroll
+    for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KS + j2 * XT + px];
+    Dft<R2, +1>::run(v);
+    if (xok) {
+      cplx *dst = T2 + (size_t)b * G.t2_band + ((size_t)p * G.n2 + s) * G.n1 + x;
+#pragma unroll
+      for (int k2 = 0; k2 < R2; k2++) dst[(size_t)(R1 * k2) * G.n1] = v[k2];
+    }
+  }
+}
+
+// ---- pass B^-1: inverse along y, keep the non-empty columns (type II)
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_b_inv_kernel(Fft2Geom G, cplx *__restrict__ T1, const cplx *__restrict__ T2, int XT, int nxt) {
+  constexpr int NS = imax(R1, R2);
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *sm = reinterpret_cast<cplx *>(smem_raw);
+  const int t = threadIdx.x, px = t % XT, s = t / XT;
+  const int xt = blockIdx.x % nxt, p = (blockIdx.x / nxt) % G.nplane, b = blockIdx.x / (nxt * G.nplane);
+  const int x = xt * XT + px;
+  const bool xok = x < G.n1;
+  const int KS = pad8(R1 * XT, XT);
+  Run r = load_run(G.plane_run + p);
+  cplx v[NS];
+  if (s < R1) {
+    const cplx *src = T2 + (size_t)b * G.t2_band + ((size_t)p * G.n2 + s) * G.n1 + (xok ? x : 0);
+#pragma unroll
+    for (int b2 = 0; b2 < R2; b2++) v[b2] = xok ? src[(size_t)(R1 * b2) * G.n1] : make_double2(0.0, 0.0);
+    Dft<R2, -1>::run(v);
+#pragma unroll
+    for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw2, s * cc));
+#pragma unroll
+    for (int cc = 0; cc < R2; cc++) sm[cc * KS + s * XT + px] = v[cc];
+  }
+  __syncthreads();
+  if (s < R2) {
+#pragma unroll
+    for (int a = 0; a < R1; a++) v[a] = sm[s * KS + a * XT + px];
+    Dft<R1, -1>::run(v);
+    cplx *dst = T1 + (size_t)b * G.t1_band + x;
+#pragma unroll
+    for (int d = 0; d < R1; d++) {
+      int c = xok ? run_map(r, s + R2 * d) : -1;
+      if (c >= 0) dst[(size_t)c * G.n1] = v[d];
+    }
+  }
+}
+
+// ---- pass C: along z (type I), times V(r)/N, inverse along z (type II), in place on the occupied planes.
+//      grid = ntile * nb with the BAND fastest, so the nb CTAs that need the same V tile run together
+//      and V is fetched from DRAM once per band chunk.
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_c_kernel(Fft2Geom G, cplx *__restrict__ T2, const double *__restrict__ vloc, int XT, int nxt, int nb) {
+  constexpr int NS = imax(R1, R2);
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *sm = reinterpret_cast<cplx *>(smem_raw);
+  const int t = threadIdx.x, px = t % XT, s = t / XT;
+  const int b = blockIdx.x % nb, tile = blockIdx.x / nb, xt = tile % nxt, y = tile / nxt;
+  const int x = xt * XT + px;
+  const bool xok = x < G.n1;
+  const int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
+  const size_t pstride = (size_t)G.n2 * G.n1;
+  cplx *base = T2 + (size_t)b * G.t2_band + (size_t)y * G.n1 + (xok ? x : 0);
+  cplx v[NS];
+  if (s < R2) {
+#pragma unroll
+    for (int j1 = 0; j1 < R1; j1++) {
+      int p = xok ? run_map(G.zrun, s + R2 * j1) : -1;
+      v[j1] = p >= 0 ? base[(size_t)p * pstride] : make_double2(0.0, 0.0);
+    }
+    Dft<R1, +1>::run(v);
+#pragma unroll
+    for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw3, s * k1));
+#pragma unroll
+    for (int k1 = 0; k1 < R1; k1++) sm[k1 * KSa + s * XT + px] = v[k1];
+  }
+  __syncthreads();
+  if (s < R1) {
+#pragma unroll
+    for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KSa + j2 * XT + px];
+  }
+  __syncthreads();   // every read of the forward exchange is done before the buffer is reused
+  if (s < R1) {
+    Dft<R2, +1>::run(v);
+    // thread s now holds psi(r) at z = s + R1 k2
+    const double *vp = vloc + (size_t)s * pstride + (size_t)y * G.n1 + (xok ? x : 0);
+#pragma unroll
+    for (int k2 = 0; k2 < R2; k2++) {
+      double w = xok ? __ldg(vp + (size_t)(R1 * k2) * pstride) : 0.0;
+      v[k2] = cscale(v[k2], w);
+    }
+    Dft<R2, -1>::run(v);
+#pragma unroll
+    for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw3, s * cc));
+#pragma unroll
+    for (int cc = 0; cc < R2; cc++) sm[cc * KSb + s * XT + px] = v[cc];
+  }
+  __syncthreads();
+  if (s < R2) {
+#pragma unroll
+    for (int a = 0; a < R1; a++) v[a] = sm[s * KSb + a * XT + px];
+    Dft<R1, -1>::run(v);
+#pragma unroll
+    for (int d = 0; d < R1; d++) {
+      int p = xok ? run_map(G.zrun, s + R2 * d) : -1;
+      if (p >= 0) base[(size_t)p * pstride] = v[d];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// host side: pair table, launch geometry
+// ------------------------------------------------------------------------------------------
+// (R1, R2) with R1 <= R2, both radices available as register codelets
+#define FFT2_PAIRS(X) \
+  X(3, 3) X(4, 4) X(4, 5) X(4, 6) X(5, 5) X(5, 6) X(4, 8) X(6, 6) X(5, 8) X(6, 8) X(5, 10) X(6, 10) X(8, 8) X(8, 9) \
+  X(8, 10) X(9, 9) X(9, 10) X(8, 12) X(10, 10) X(9, 12) X(10, 12) X(8, 16) X(12, 12) X(10, 15) X(10, 16) X(12, 15) \
+  X(12, 16) X(15, 15) X(15, 16) X(16, 16)
+
+bool fft2_pair(int n, int *r1, int *r2) {
+  int best1 = 0, best2 = 0;
+#define X(a, b) if ((a) * (b) == n && (best2 == 0 || (b) < best2)) { best1 = (a); best2 = (b); }
+  FFT2_PAIRS(X)
+#undef X
+  if (!best2) return false;
+  if (r1) *r1 = best1;
+  if (r2) *r2 = best2;
+  return true;
+}
+
+static int choose_xt2(int n1, int ns) {
+  int cap = F2_THREADS / ns;
+  if (cap > n1) cap = n1;
+  for (int d = cap; d >= 4; d--)
+    if (n1 % d == 0 && d % 2 == 0) return d;
+  return cap < 1 ? 1 : cap;
+}
+
+static Fft2Geom make_geom2(const dft_plan *p, int ik, int64_t t1_band, int64_t t2_band) {
+  const KPoint &kp = p->kp[ik];
+  Fft2Geom G;
+  G.n1 = p->n[0]; G.n2 = p->n[1]; G.n3 = p->n[2];
+  G.npw = kp.npw; G.mpw = p->mpw; G.ncol = kp.ncol; G.nplane = kp.nplane;
+  G.col_run = kp.col_run; G.plane_run = kp.plane_run; G.zrun = kp.zrun;
+  G.tw1 = reinterpret_cast<const cplx *>(p->d_tw[0]);
+  G.tw2 = reinterpret_cast<const cplx *>(p->d_tw[1]);
+  G.tw3 = reinterpret_cast<const cplx *>(p->d_tw[2]);
+  G.t1_band = t1_band; G.t2_band = t2_band;
+  return G;
+}
+
+template <typename K>
+static int set_smem(K kernel, size_t bytes) {
+  if (bytes > 48 * 1024) DFT_CUDA_CHECK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  return DFT_OK;
+}
+
+template <int R1, int R2>
+static int launch_pass(const Fft2Geom &G, int pass, const cplx *psi, cplx *hpsi, cplx *T1, cplx *T2, const double *vloc, int nb,
+                       cudaStream_t st) {
+  constexpr int NS = imax(R1, R2);
+  int rc;
+  if (pass == 0 || pass == 4) {
+    int lpc = F2_THREADS / NS;
+    if (lpc > G.ncol) lpc = G.ncol;
+    int ntile = (G.ncol + lpc - 1) / lpc;
+    constexpr int LSf = pad8(R1 * (R2 | 1), NS), LSi = pad8(R2 * (R1 | 1), NS);
+    size_t sm = sizeof(cplx) * (size_t)lpc * (pass == 0 ? LSf : LSi);
+    int64_t grid = (int64_t)nb * ntile;
+    if (grid > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
+    if (pass == 0) {
+      if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2>, sm))) return rc;
+      fft2_a_fwd_kernel<R1, R2><<<(unsigned)grid, lpc * NS, sm, st>>>(G, psi, T1, lpc, ntile);
+    } else {
+      if ((rc = set_smem(fft2_a_inv_kernel<R1, R2>, sm))) return rc;
+      fft2_a_inv_kernel<R1, R2><<<(unsigned)grid, lpc * NS, sm, st>>>(G, T1, hpsi, lpc, ntile);
+    }
+  } else {
+    int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
+    size_t sm = sizeof(cplx) * (size_t)(pad8(R2 * XT, XT) * R1 > pad8(R1 * XT, XT) * R2 ? pad8(R2 * XT, XT) * R1 : pad8(R1 * XT, XT) * R2);
+    int64_t grid = (int64_t)nb * nxt * (pass == 2 ? G.n2 : G.nplane);
+    if (grid > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
+    if (pass == 1) {
+      if ((rc = set_smem(fft2_b_fwd_kernel<R1, R2>, sm))) return rc;
+      fft2_b_fwd_kernel<R1, R2><<<(unsigned)grid, XT * NS, sm, st>>>(G, T1, T2, XT, nxt);
+    } else if (pass == 3) {
+      if ((rc = set_smem(fft2_b_inv_kernel<R1, R2>, sm))) return rc;
+      fft2_b_inv_kernel<R1, R2><<<(unsigned)grid, XT * NS, sm, st>>>(G, T1, T2, XT, nxt);
+    } else {
+      if ((rc = set_smem(fft2_c_kernel<R1, R2>, sm))) return rc;
+      fft2_c_kernel<R1, R2><<<(unsigned)grid, XT * NS, sm, st>>>(G, T2, vloc, XT, nxt, nb);
+    }
+  }
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+// pass: 0 A, 1 B, 2 C, 3 B^-1, 4 A^-1.  The pair is that of the axis the pass transforms.
+int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, void *T1, void *T2, int64_t t1_band,
+                int64_t t2_band, int nb, cudaStream_t st) {
+  int axis = (pass == 0 || pass == 4) ? 0 : (pass == 2 ? 2 : 1);
+  int r1, r2;
+  if (!fft2_pair(p->n[axis], &r1, &r2)) { set_error("no two-stage factorisation of %d", p->n[axis]); return DFT_ERR_UNSUPPORTED; }
+  Fft2Geom G = make_geom2(p, ik, t1_band, t2_band);
+  const cplx *cpsi = reinterpret_cast<const cplx *>(psi);
+  cplx *chpsi = reinterpret_cast<cplx *>(hpsi), *t1 = reinterpret_cast<cplx *>(T1), *t2 = reinterpret_cast<cplx *>(T2);
+#define X(a, b) if (r1 == (a) && r2 == (b)) return launch_pass<a, b>(G, pass, cpsi, chpsi, t1, t2, p->d_vloc, nb, st);
+  FFT2_PAIRS(X)
+#undef X
+  return DFT_ERR_UNSUPPORTED;
+}
+
+}  // namespace dftb200

@@ -34,6 +34,13 @@ struct FftFactors {
 };
 bool factorize(int n, FftFactors *f);
 
+// Up to two runs of consecutive box indices along one axis: [lo, lo+nlo) -> base + (x - lo),
+// [hi, hi+nhi) -> base + nlo + (x - hi).  The sphere is convex, so the occupied x of a column, the
+// occupied y of a plane and the occupied z of the box each have this form (K2).
+struct Run {
+  int32_t base, lo, nlo, hi, nhi, aux0, aux1, pad;
+};
+
 // Per-k-point geometry of the sphere and of the pruned passes (device pointers unless noted)
 struct KPoint {
   double k[3];
@@ -51,6 +58,11 @@ struct KPoint {
   int32_t *pw_i1 = nullptr;      // [npw]   box index along axis 1 of each plane wave
   int32_t *plane_i3 = nullptr;   // [nplane] box index i3 of plane p
   int32_t *plane_col0 = nullptr; // [nplane+1] first column of plane p
+  // the same geometry as runs (register-resident FFT path, fft2.cu)
+  Run *col_run = nullptr;        // [ncol]   base = first plane wave, runs along x; aux0 = i2, aux1 = plane
+  Run *plane_run = nullptr;      // [nplane] base = first column, runs along y; aux0 = i3
+  Run zrun = {0, 0, 0, 0, 0, 0, 0, 0};   // base = 0, runs along z (plane ordinals)
+  bool runs_ok = false;          // every occupied set really is <= 2 runs (else the generic path is used)
   // host copies for getters
   std::vector<int32_t> h_kg, h_igfft;
   std::vector<double> h_kin;
@@ -95,6 +107,7 @@ struct dft_plan {
   // options
   int band_chunk = 0;      // 0 = automatic
   int terms = 7;
+  int fft_path = 0;        // 0 = automatic (register path where available), 1 = generic Stockham path only
   int splitk = 0;
   // workspace
   void *ws_user = nullptr; int64_t ws_user_bytes = 0;
@@ -129,6 +142,11 @@ int64_t fft_ws_bytes_per_band(const dft_plan *p);
 // V_loc psi for `nb` bands of k-point ik: psi/hpsi point at the first band ([nb][mpw] complex)
 int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb, void *ws, cudaStream_t st);
 int zero_fill(double *hpsi, int64_t ndouble, cudaStream_t st);
+// fft2.cu: two-stage register path.  fft2_pair: is n = R1*R2 with both radices available as codelets?
+bool fft2_pair(int n, int *r1, int *r2);
+// pass: 0 A, 1 B, 2 C, 3 B^-1, 4 A^-1; T1/T2 strides in complex elements per band
+int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, void *T1, void *T2, int64_t t1_band,
+                int64_t t2_band, int nb, cudaStream_t st);
 
 // --- nonlocal.cu (K3) ---------------------------------------------------------------------
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi

@@ -51,7 +51,7 @@ __global__ void scale_copy_kernel(const double *__restrict__ src, double *__rest
 
 static void free_kpoint(KPoint &k) {
   cudaFree(k.kg); cudaFree(k.igfft); cudaFree(k.kin); cudaFree(k.col_start); cudaFree(k.col_i2); cudaFree(k.col_plane);
-  cudaFree(k.pw_i1); cudaFree(k.plane_i3); cudaFree(k.plane_col0);
+  cudaFree(k.pw_i1); cudaFree(k.plane_i3); cudaFree(k.plane_col0); cudaFree(k.col_run); cudaFree(k.plane_run);
 }
 
 static void destroy_plan(dft_plan *p) {
@@ -397,6 +397,10 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
   if (!strcmp(key, "terms")) {
     if (value < 0 || value > 7) { set_error("terms = %lld outside 0..7", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->terms = (int)value; return DFT_OK;
+  }
+  if (!strcmp(key, "fft_path")) {
+    if (value < 0 || value > 1) { set_error("fft_path = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->fft_path = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "splitk")) {
     if (value < 0 || value > 4096) { set_error("splitk = %lld outside 0..4096", (long long)value); return DFT_ERR_INVALID_ARG; }

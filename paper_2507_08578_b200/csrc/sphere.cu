@@ -206,7 +206,36 @@ int sphere_build(const double *gmet, const int n[3], double ecut, KPoint *kp) {
   kp->nplane = (int)plane_i3.size();
   col_start.push_back((int32_t)tot);
   plane_col0.push_back(kp->ncol);
+  // the same geometry as runs of consecutive box indices
+  auto make_run = [](const int32_t *idx, int cnt, int base, Run *r) -> bool {
+    r->base = base; r->lo = cnt ? idx[0] : 0; r->nlo = 0; r->hi = 0; r->nhi = 0; r->aux0 = r->aux1 = r->pad = 0;
+    int i = 0;
+    while (i < cnt && idx[i] == r->lo + i) i++;
+    r->nlo = i;
+    if (i < cnt) {
+      r->hi = idx[i];
+      int j = i;
+      while (j < cnt && idx[j] == r->hi + (j - i)) j++;
+      r->nhi = j - i;
+      if (j < cnt) return false;
+    }
+    return true;
+  };
+  std::vector<Run> col_run(kp->ncol), plane_run(kp->nplane);
+  bool runs_ok = true;
+  for (int c = 0; c < kp->ncol; c++) {
+    runs_ok &= make_run(pw_i1.data() + col_start[c], col_start[c + 1] - col_start[c], col_start[c], &col_run[c]);
+    col_run[c].aux0 = col_i2[c]; col_run[c].aux1 = col_plane[c];
+  }
+  for (int p = 0; p < kp->nplane; p++) {
+    runs_ok &= make_run(col_i2.data() + plane_col0[p], plane_col0[p + 1] - plane_col0[p], plane_col0[p], &plane_run[p]);
+    plane_run[p].aux0 = plane_i3[p];
+  }
+  runs_ok &= make_run(plane_i3.data(), kp->nplane, 0, &kp->zrun);
+  kp->runs_ok = runs_ok;
   int rc;
+  if ((rc = upload(&kp->col_run, col_run))) return rc;
+  if ((rc = upload(&kp->plane_run, plane_run))) return rc;
   if ((rc = upload(&kp->col_start, col_start))) return rc;
   if ((rc = upload(&kp->col_i2, col_i2))) return rc;
   if ((rc = upload(&kp->col_plane, col_plane))) return rc;

@@ -36,6 +36,30 @@ def test_small_cells_all_terms_and_isolations(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c0", "c1m", "c4m", "aniso", "c3k2"])
+def test_generic_fft_path_agrees(name):
+    """Option fft_path=1 forces the generic shared-memory Stockham kernels (used for box lengths with no
+    two-stage factorisation); both paths must match the oracle."""
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    ref = oracle_apply(cfg, sph, psi, method=1 if name in ("c0", "aniso") else 2)
+    for path in (1, 0):
+        plan.set_option("fft_path", path)
+        err = band_rel_err(gpu_apply(plan, psi), ref)
+        assert err <= TOL, "%s fft_path=%d: rel err %.3e" % (name, path, err)
+    plan.destroy()
+
+
+def test_box_without_two_stage_factorisation():
+    """Box 10 x 20 x 27: 10 and 27 have no two-stage factorisation (generic kernels), 20 = 4 x 5 has, so the
+    passes of one transform mix both kernel families."""
+    cfg, plan, sph = _setup("c0", ngfft=(10, 20, 27))
+    psi = synth.gen_psi(cfg, [sph[0][2]])
+    err = band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, method=1))
+    assert err <= TOL, err
+    plan.destroy()
+
+
 def test_c0_against_dense_h():
     """tier T0: explicit dense H_{GG'} on the tiny cell (north_star: 'brute-force dense H on the tiny cell')."""
     cfg, plan, sph = _setup("c0")

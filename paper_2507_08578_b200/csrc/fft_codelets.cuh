@@ -4,7 +4,7 @@
 // constants after unrolling).  Small radices are written out; composite ones are built from them with the
 // prime-factor map (coprime factors, no internal twiddles) or one Cooley-Tukey step (constant twiddles).
 // Shared by the generic Stockham path and the two-stage register path of fft.cu.  Nothing here is shared
-// with oracle/.
+// with the CPU checker.
 #pragma once
 #include <cuda_runtime.h>
 

@@ -159,6 +159,7 @@ def main():
     ap.add_argument("--config", default="c4", choices=sorted(WORKLOADS))
     ap.add_argument("--nband", type=int, default=0, help="override the band count (experiments only)")
     ap.add_argument("--band-chunk", type=int, default=0)
+    ap.add_argument("--fft-path", type=int, default=0, help="dft_plan_set_option fft_path (experiments only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (experiments only)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the e2e leg (experiments only)")
     ap.add_argument("--ref-bands", type=int, default=0)
@@ -187,6 +188,8 @@ def main():
     plan = dft.Plan(cfg)
     if args.band_chunk:
         plan.set_option("band_chunk", args.band_chunk)
+    if args.fft_path:
+        plan.set_option("fft_path", args.fft_path)
     plan.set_vloc(torch.as_tensor(cfg["vloc"], device="cuda"))
     kin_list = [plan.get_kg(ik)[2] for ik in range(plan.nkpt)]
     nband = cfg["nband"]

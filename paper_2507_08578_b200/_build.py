@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdftb200.so")
 SOURCES = ["plan.cu", "sphere.cu", "projtab.cu", "fft.cu", "fft2.cu", "nonlocal.cu"]
-HEADERS = [os.path.join(CSRC, "internal.h"), os.path.join(CSRC, "fft_codelets.cuh"), os.path.join(HERE, "..", "include", "dft.h")]
+HEADERS = [os.path.join(CSRC, "internal.h"), os.path.join(CSRC, "fft_codelets.cuh"), os.path.join(CSRC, "ptx.cuh"), os.path.join(HERE, "..", "include", "dft.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC,-ffp-contract=off", "-Xptxas", "-v"]

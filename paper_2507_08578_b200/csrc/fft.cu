@@ -330,7 +330,7 @@ int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb,
   // per pass: the register-resident two-stage kernel (fft2.cu) when the axis length factorises into two
   // codelet radices and the sphere's occupied sets are runs; otherwise the generic Stockham kernel
   bool fast[3];
-  for (int c = 0; c < 3; c++) fast[c] = p->fft_path == 0 && kp.runs_ok && fft2_pair(p->n[c], nullptr, nullptr);
+  for (int c = 0; c < 3; c++) fast[c] = p->fft_path != 1 && kp.runs_ok && fft2_pair(p->n[c], nullptr, nullptr);
   const int axis_of[5] = {0, 1, 2, 1, 0};
   for (int pass = 0; pass < 5; pass++) {
     phase_begin(p, pass, st);

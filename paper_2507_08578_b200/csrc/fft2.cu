@@ -19,6 +19,7 @@
 // kept" is two range checks (struct Run) and the sphere <-> box maps need no index list.
 #include "fft_codelets.cuh"
 #include "internal.h"
+#include "ptx.cuh"
 
 namespace dftb200 {
 
@@ -58,7 +59,7 @@ template <int R1, int R2>
 __global__ void __launch_bounds__(F2_THREADS, 2)
 fft2_a_fwd_kernel(Fft2Geom G, const cplx *__restrict__ psi, cplx *__restrict__ T1, int lpc, int ntile) {
   constexpr int NS = imax(R1, R2), KS = R2 | 1, LS = pad8(R1 * KS, NS);
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
   const int t = threadIdx.x, s = t % NS, l = t / NS;
   const int tile = blockIdx.x % ntile, b = blockIdx.x / ntile;
@@ -97,7 +98,7 @@ template <int R1, int R2>
 __global__ void __launch_bounds__(F2_THREADS, 2)
 fft2_a_inv_kernel(Fft2Geom G, const cplx *__restrict__ T1, cplx *__restrict__ hpsi, int lpc, int ntile) {
   constexpr int NS = imax(R1, R2), KS = R1 | 1, LS = pad8(R2 * KS, NS);
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
   const int t = threadIdx.x, s = t % NS, l = t / NS;
   const int tile = blockIdx.x % ntile, b = blockIdx.x / ntile;
@@ -137,7 +138,7 @@ template <int R1, int R2>
 __global__ void __launch_bounds__(F2_THREADS, 2)
 fft2_b_fwd_kernel(Fft2Geom G, const cplx *__restrict__ T1, cplx *__restrict__ T2, int XT, int nxt) {
   constexpr int NS = imax(R1, R2);
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
   const int t = threadIdx.x, px = t % XT, s = t / XT;
   const int xt = blockIdx.x % nxt, p = (blockIdx.x / nxt) % G.nplane, b = blockIdx.x / (nxt * G.nplane);
@@ -177,7 +178,7 @@ template <int R1, int R2>
 __global__ void __launch_bounds__(F2_THREADS, 2)
 fft2_b_inv_kernel(Fft2Geom G, cplx *__restrict__ T1, const cplx *__restrict__ T2, int XT, int nxt) {
   constexpr int NS = imax(R1, R2);
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
   const int t = threadIdx.x, px = t % XT, s = t / XT;
   const int xt = blockIdx.x % nxt, p = (blockIdx.x / nxt) % G.nplane, b = blockIdx.x / (nxt * G.nplane);
@@ -217,7 +218,7 @@ template <int R1, int R2>
 __global__ void __launch_bounds__(F2_THREADS, 2)
 fft2_c_kernel(Fft2Geom G, cplx *__restrict__ T2, const double *__restrict__ vloc, int XT, int nxt, int nb) {
   constexpr int NS = imax(R1, R2);
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
   const int t = threadIdx.x, px = t % XT, s = t / XT;
   const int b = blockIdx.x % nb, tile = blockIdx.x / nb, xt = tile % nxt, y = tile / nxt;
@@ -274,6 +275,264 @@ fft2_c_kernel(Fft2Geom G, cplx *__restrict__ T2, const double *__restrict__ vloc
 }
 
 // ------------------------------------------------------------------------------------------
+// TMA-ring variants of the three strided passes (B, C, B^-1).  Same arithmetic, same register
+// layout; what changes is how a tile's INPUT reaches the registers.  Above, every thread issues its own
+// R loads and then waits for them, so with 2 CTAs of ~6 warps per SM the kernel is exposed to DRAM
+// latency for a large part of each tile (ncu r1: 17 % warps active, long-scoreboard stalls, 25-50 % of
+// HBM peak).  Here a CTA is persistent, walks a list of tiles, and lane 0 keeps S-1 tiles in flight with
+// cp.async.bulk.tensor (one box = all occupied rows of the tile x XT consecutive x) into a
+// shared-memory ring guarded by mbarriers; the threads read their strided inputs from the ring
+// (consecutive lanes -> consecutive 16-byte words, conflict-free) and DRAM latency is off the critical
+// path.  Outputs still go from registers straight to global memory (stores do not stall).
+// ------------------------------------------------------------------------------------------
+struct RingParams {
+  int XT, nxt, ntiles, S, nb;
+  uint32_t stage_stride, box_bytes;   // bytes; stage_stride is box_bytes rounded up to 128
+};
+__device__ __forceinline__ int run_local(const Run &r, int x) {   // row inside the tile's box (box row 0 = r.base)
+  unsigned d = (unsigned)(x - r.lo);
+  if (d < (unsigned)r.nlo) return (int)d;
+  d = (unsigned)(x - r.hi);
+  if (d < (unsigned)r.nhi) return r.nlo + (int)d;
+  return -1;
+}
+
+// ---- pass B (type I along y): box {XT x, HB columns starting at the plane's first column} of T1
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_b_fwd_ring_kernel(const __grid_constant__ CUtensorMap mapT1, Fft2Geom G, cplx *__restrict__ T2, RingParams Q) {
+  constexpr int NS = imax(R1, R2);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int XT = Q.XT, KS = pad8(R2 * XT, XT);
+  unsigned char *stages = smem_raw;
+  cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
+  Run *runs = reinterpret_cast<Run *>(sm + R1 * KS);
+  uint64_t *full = reinterpret_cast<uint64_t *>(runs + G.nplane);
+  const int t = threadIdx.x, px = t % XT, s = t / XT;
+  for (int i = t; i < G.nplane * 2; i += blockDim.x)
+    reinterpret_cast<int4 *>(runs)[i] = __ldg(reinterpret_cast<const int4 *>(G.plane_run) + i);
+  if (t == 0) {
+    for (int i = 0; i < Q.S; i++) mbar_init(&full[i], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  // contiguous range of tiles (x-tile fastest, then plane, then band), decoded incrementally
+  const int first = (int)(((int64_t)Q.ntiles * blockIdx.x) / gridDim.x);
+  const int nmine = (int)(((int64_t)Q.ntiles * (blockIdx.x + 1)) / gridDim.x) - first;
+  int xt = first % Q.nxt, p = (first / Q.nxt) % G.nplane, b = first / (Q.nxt * G.nplane);
+  int ixt = xt, ip = p, ib = b, ist = 0;      // producer's copy (lane 0 only), runs S-1 tiles ahead
+  auto issue = [&]() {
+    mbar_expect_tx(&full[ist], Q.box_bytes);
+    tma_load_3d(stages + (size_t)ist * Q.stage_stride, &mapT1, &full[ist], 2 * ixt * XT, runs[ip].base, ib);
+    if (++ist == Q.S) ist = 0;
+    if (++ixt == Q.nxt) { ixt = 0; if (++ip == G.nplane) { ip = 0; ib++; } }
+  };
+  if (t == 0)
+    for (int j = 0; j < Q.S - 1 && j < nmine; j++) issue();
+  int st = 0; uint32_t ph = 0;
+  for (int it = 0; it < nmine; it++) {
+    if (t == 0 && it + Q.S - 1 < nmine) issue();
+    const int x = xt * XT + px;
+    const bool xok = x < G.n1;
+    const Run r = runs[p];
+    const cplx *in = reinterpret_cast<const cplx *>(stages + (size_t)st * Q.stage_stride) + px;
+    mbar_wait(&full[st], ph);
+    cplx v[NS];
+    if (s < R2) {
+#pragma unroll
+      for (int j1 = 0; j1 < R1; j1++) {
+        int c = run_local(r, s + R2 * j1);
+        v[j1] = c >= 0 ? in[c * XT] : make_double2(0.0, 0.0);
+      }
+      Dft<R1, +1>::run(v);
+#pragma unroll
+      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw2, s * k1));
+#pragma unroll
+      for (int k1 = 0; k1 < R1; k1++) sm[k1 * KS + s * XT + px] = v[k1];
+    }
+    __syncthreads();
+    if (s < R1) {
+#pragma unroll
+      for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KS + j2 * XT + px];
+      Dft<R2, +1>::run(v);
+      if (xok) {
+        cplx *dst = T2 + (size_t)b * G.t2_band + ((size_t)p * G.n2 + s) * G.n1 + x;
+#pragma unroll
+        for (int k2 = 0; k2 < R2; k2++) dst[(size_t)(R1 * k2) * G.n1] = v[k2];
+      }
+    }
+    __syncthreads();   // the exchange buffer is rewritten by the next tile
+    if (++st == Q.S) { st = 0; ph ^= 1; }
+    if (++xt == Q.nxt) { xt = 0; if (++p == G.nplane) { p = 0; b++; } }
+  }
+}
+
+// ---- pass B^-1 (type II along y): box {XT x, n2 y} of one plane of T2
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_b_inv_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *__restrict__ T1, RingParams Q) {
+  constexpr int NS = imax(R1, R2);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int XT = Q.XT, KS = pad8(R1 * XT, XT);
+  unsigned char *stages = smem_raw;
+  cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
+  Run *runs = reinterpret_cast<Run *>(sm + R2 * KS);
+  uint64_t *full = reinterpret_cast<uint64_t *>(runs + G.nplane);
+  const int t = threadIdx.x, px = t % XT, s = t / XT;
+  for (int i = t; i < G.nplane * 2; i += blockDim.x)
+    reinterpret_cast<int4 *>(runs)[i] = __ldg(reinterpret_cast<const int4 *>(G.plane_run) + i);
+  if (t == 0) {
+    for (int i = 0; i < Q.S; i++) mbar_init(&full[i], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  // contiguous range of tiles (x-tile fastest, then plane, then band), decoded incrementally
+  const int first = (int)(((int64_t)Q.ntiles * blockIdx.x) / gridDim.x);
+  const int nmine = (int)(((int64_t)Q.ntiles * (blockIdx.x + 1)) / gridDim.x) - first;
+  int xt = first % Q.nxt, p = (first / Q.nxt) % G.nplane, b = first / (Q.nxt * G.nplane);
+  int ixt = xt, ip = p, ib = b, ist = 0;      // producer's copy (lane 0 only), runs S-1 tiles ahead
+  auto issue = [&]() {
+    mbar_expect_tx(&full[ist], Q.box_bytes);
+    tma_load_4d(stages + (size_t)ist * Q.stage_stride, &mapT2, &full[ist], 2 * ixt * XT, 0, ip, ib);
+    if (++ist == Q.S) ist = 0;
+    if (++ixt == Q.nxt) { ixt = 0; if (++ip == G.nplane) { ip = 0; ib++; } }
+  };
+  if (t == 0)
+    for (int j = 0; j < Q.S - 1 && j < nmine; j++) issue();
+  int st = 0; uint32_t ph = 0;
+  for (int it = 0; it < nmine; it++) {
+    if (t == 0 && it + Q.S - 1 < nmine) issue();
+    const int x = xt * XT + px;
+    const bool xok = x < G.n1;
+    const Run r = runs[p];
+    const cplx *in = reinterpret_cast<const cplx *>(stages + (size_t)st * Q.stage_stride) + px;
+    mbar_wait(&full[st], ph);
+    cplx v[NS];
+    if (s < R1) {
+#pragma unroll
+      for (int b2 = 0; b2 < R2; b2++) v[b2] = in[(s + R1 * b2) * XT];
+      Dft<R2, -1>::run(v);
+#pragma unroll
+      for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw2, s * cc));
+#pragma unroll
+      for (int cc = 0; cc < R2; cc++) sm[cc * KS + s * XT + px] = v[cc];
+    }
+    __syncthreads();
+    if (s < R2) {
+#pragma unroll
+      for (int a = 0; a < R1; a++) v[a] = sm[s * KS + a * XT + px];
+      Dft<R1, -1>::run(v);
+      cplx *dst = T1 + (size_t)b * G.t1_band + x;
+#pragma unroll
+      for (int d = 0; d < R1; d++) {
+        int c = xok ? run_map(r, s + R2 * d) : -1;
+        if (c >= 0) dst[(size_t)c * G.n1] = v[d];
+      }
+    }
+    __syncthreads();
+    if (++st == Q.S) { st = 0; ph ^= 1; }
+    if (++xt == Q.nxt) { xt = 0; if (++p == G.nplane) { p = 0; b++; } }
+  }
+}
+
+// ---- pass C: box {XT x, one y, all occupied planes} of T2; a CTA owns a contiguous range of tiles with the
+//      band fastest, so its V(r)/N tile [n3][XT] is staged in shared memory once per (y, x-tile) group.
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *__restrict__ T2,
+                   const double *__restrict__ vloc, RingParams Q) {
+  constexpr int NS = imax(R1, R2);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int XT = Q.XT, KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
+  const int exn = imax(R1 * KSa, R2 * KSb);
+  unsigned char *stages = smem_raw;
+  cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
+  double *vs = reinterpret_cast<double *>(sm + exn);
+  uint64_t *full = reinterpret_cast<uint64_t *>(vs + ((G.n3 * XT + 1) & ~1));
+  const int t = threadIdx.x, px = t % XT, s = t / XT;
+  if (t == 0) {
+    for (int i = 0; i < Q.S; i++) mbar_init(&full[i], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int first = (int)(((int64_t)Q.ntiles * blockIdx.x) / gridDim.x);
+  const int nmine = (int)(((int64_t)Q.ntiles * (blockIdx.x + 1)) / gridDim.x) - first;
+  const size_t pstride = (size_t)G.n2 * G.n1;
+  int b = first % Q.nb, xt = (first / Q.nb) % Q.nxt, y = first / (Q.nb * Q.nxt);
+  int ib = b, ixt = xt, iy = y, ist = 0;      // producer's copy (lane 0 only), runs S-1 tiles ahead
+  auto issue = [&]() {
+    mbar_expect_tx(&full[ist], Q.box_bytes);
+    tma_load_4d(stages + (size_t)ist * Q.stage_stride, &mapT2, &full[ist], 2 * ixt * XT, iy, 0, ib);
+    if (++ist == Q.S) ist = 0;
+    if (++ib == Q.nb) { ib = 0; if (++ixt == Q.nxt) { ixt = 0; iy++; } }
+  };
+  if (t == 0)
+    for (int j = 0; j < Q.S - 1 && j < nmine; j++) issue();
+  int st = 0; uint32_t ph = 0;
+  bool newgroup = true;
+  for (int it = 0; it < nmine; it++) {
+    if (t == 0 && it + Q.S - 1 < nmine) issue();
+    const int x = xt * XT + px;
+    const bool xok = x < G.n1;
+    if (newgroup) {
+      // every read of the previous V tile happened before the barrier that ended the last iteration
+      const double *vp = vloc + (size_t)y * G.n1 + xt * XT;
+      for (int i = t; i < G.n3 * XT; i += blockDim.x) {
+        int z = i / XT, xx = i - z * XT;
+        vs[i] = (xt * XT + xx < G.n1) ? __ldg(vp + (size_t)z * pstride + xx) : 0.0;
+      }
+      newgroup = false;
+    }
+    const cplx *in = reinterpret_cast<const cplx *>(stages + (size_t)st * Q.stage_stride) + px;
+    mbar_wait(&full[st], ph);
+    cplx v[NS];
+    if (s < R2) {
+#pragma unroll
+      for (int j1 = 0; j1 < R1; j1++) {
+        int p = run_map(G.zrun, s + R2 * j1);
+        v[j1] = p >= 0 ? in[p * XT] : make_double2(0.0, 0.0);
+      }
+      Dft<R1, +1>::run(v);
+#pragma unroll
+      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw3, s * k1));
+#pragma unroll
+      for (int k1 = 0; k1 < R1; k1++) sm[k1 * KSa + s * XT + px] = v[k1];
+    }
+    __syncthreads();
+    if (s < R1) {
+#pragma unroll
+      for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KSa + j2 * XT + px];
+    }
+    __syncthreads();
+    if (s < R1) {
+      Dft<R2, +1>::run(v);
+#pragma unroll
+      for (int k2 = 0; k2 < R2; k2++) v[k2] = cscale(v[k2], vs[(s + R1 * k2) * XT + px]);
+      Dft<R2, -1>::run(v);
+#pragma unroll
+      for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw3, s * cc));
+#pragma unroll
+      for (int cc = 0; cc < R2; cc++) sm[cc * KSb + s * XT + px] = v[cc];
+    }
+    __syncthreads();
+    if (s < R2) {
+#pragma unroll
+      for (int a = 0; a < R1; a++) v[a] = sm[s * KSb + a * XT + px];
+      Dft<R1, -1>::run(v);
+      cplx *base = T2 + (size_t)b * G.t2_band + (size_t)y * G.n1 + x;
+#pragma unroll
+      for (int d = 0; d < R1; d++) {
+        int p = xok ? run_map(G.zrun, s + R2 * d) : -1;
+        if (p >= 0) base[(size_t)p * pstride] = v[d];
+      }
+    }
+    __syncthreads();
+    if (++st == Q.S) { st = 0; ph ^= 1; }
+    if (++b == Q.nb) { b = 0; newgroup = true; if (++xt == Q.nxt) { xt = 0; y++; } }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // host side: pair table, launch geometry
 // ------------------------------------------------------------------------------------------
 // (R1, R2) with R1 <= R2, both radices available as register codelets
@@ -320,11 +579,93 @@ static int set_smem(K kernel, size_t bytes) {
   return DFT_OK;
 }
 
+typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                             const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                             CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// FP64 tensor map of rank `rank` (dims/strides innermost first, strides in bytes for dims 1..), no swizzle, OOB = 0
+static int encode_map(dft_plan *p, CUtensorMap *m, void *base, int rank, const cuuint64_t *dims, const cuuint64_t *strides,
+                      const cuuint32_t *box) {
+  cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  for (int i = 0; i < rank; i++)
+    if (box[i] == 0 || box[i] > 256) return DFT_ERR_UNSUPPORTED;
+  CUresult r = ((EncodeFn)p->encode_fn)(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, rank, base, dims, strides, box, estr,
+                                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? DFT_OK : DFT_ERR_UNSUPPORTED;
+}
+
+// Ring launch of pass 1 (B), 2 (C) or 3 (B^-1).  Returns DFT_ERR_UNSUPPORTED (without setting the error text)
+// when the tile does not fit a TMA box or two CTAs' shared memory; the caller then uses the plain kernels.
 template <int R1, int R2>
-static int launch_pass(const Fft2Geom &G, int pass, const cplx *psi, cplx *hpsi, cplx *T1, cplx *T2, const double *vloc, int nb,
+static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx *T2, const double *vloc, int nb, int hb,
                        cudaStream_t st) {
   constexpr int NS = imax(R1, R2);
+  if (!p->encode_fn) return DFT_ERR_UNSUPPORTED;
+  const int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
+  if (XT * NS > F2_THREADS || (XT * 16) % 16) return DFT_ERR_UNSUPPORTED;
+  const int rows = pass == 1 ? hb : (pass == 2 ? G.nplane : G.n2);
+  const int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
+  size_t ex = sizeof(cplx) * (size_t)(pass == 1 ? R1 * KSa : (pass == 3 ? R2 * KSb : imax(R1 * KSa, R2 * KSb)));
+  size_t extra = pass == 2 ? sizeof(double) * (size_t)((G.n3 * XT + 1) & ~1) : sizeof(Run) * (size_t)G.nplane;
+  RingParams Q;
+  Q.XT = XT; Q.nxt = nxt; Q.nb = nb;
+  Q.box_bytes = (uint32_t)((size_t)rows * XT * 16);
+  Q.stage_stride = (Q.box_bytes + 127u) & ~127u;
+  int64_t ntiles = (int64_t)nb * nxt * (pass == 2 ? G.n2 : G.nplane);
+  if (ntiles > 0x7fffffffLL) return DFT_ERR_UNSUPPORTED;
+  Q.ntiles = (int)ntiles;
+  const size_t fixed = ex + extra + 8 * 8;
+  const size_t budget2 = (size_t)(p->smem_per_sm / 2) - 1024, budget1 = (size_t)p->smem_optin;
+  int S = 0, per_sm = 2;
+  for (int s = 4; s >= 2 && !S; s--)
+    if (fixed + (size_t)s * Q.stage_stride <= budget2) S = s;
+  if (!S) {
+    per_sm = 1;
+    for (int s = 4; s >= 2 && !S; s--)
+      if (fixed + (size_t)s * Q.stage_stride <= budget1) S = s;
+  }
+  if (!S) return DFT_ERR_UNSUPPORTED;
+  Q.S = S;
+  const size_t smem = fixed + (size_t)S * Q.stage_stride;
+  CUtensorMap map;
   int rc;
+  if (pass == 1) {
+    cuuint64_t dims[3] = {2 * (cuuint64_t)G.n1, (cuuint64_t)G.ncol, (cuuint64_t)nb};
+    cuuint64_t strides[2] = {(cuuint64_t)G.n1 * 16, (cuuint64_t)G.t1_band * 16};
+    cuuint32_t box[3] = {2 * (cuuint32_t)XT, (cuuint32_t)rows, 1};
+    if ((rc = encode_map(p, &map, T1, 3, dims, strides, box))) return rc;
+  } else {
+    cuuint64_t dims[4] = {2 * (cuuint64_t)G.n1, (cuuint64_t)G.n2, (cuuint64_t)G.nplane, (cuuint64_t)nb};
+    cuuint64_t strides[3] = {(cuuint64_t)G.n1 * 16, (cuuint64_t)G.n1 * G.n2 * 16, (cuuint64_t)G.t2_band * 16};
+    cuuint32_t box[4] = {2 * (cuuint32_t)XT, pass == 2 ? 1u : (cuuint32_t)rows, pass == 2 ? (cuuint32_t)rows : 1u, 1};
+    if ((rc = encode_map(p, &map, T2, 4, dims, strides, box))) return rc;
+  }
+  int grid = per_sm * p->sm_count;
+  if (grid > Q.ntiles) grid = Q.ntiles;
+  if (pass == 1) {
+    if ((rc = set_smem(fft2_b_fwd_ring_kernel<R1, R2>, smem))) return rc;
+    fft2_b_fwd_ring_kernel<R1, R2><<<grid, XT * NS, smem, st>>>(map, G, T2, Q);
+  } else if (pass == 3) {
+    if ((rc = set_smem(fft2_b_inv_ring_kernel<R1, R2>, smem))) return rc;
+    fft2_b_inv_ring_kernel<R1, R2><<<grid, XT * NS, smem, st>>>(map, G, T1, Q);
+  } else {
+    if ((rc = set_smem(fft2_c_ring_kernel<R1, R2>, smem))) return rc;
+    fft2_c_ring_kernel<R1, R2><<<grid, XT * NS, smem, st>>>(map, G, T2, vloc, Q);
+  }
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+template <int R1, int R2>
+static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi, cplx *hpsi, cplx *T1, cplx *T2, const double *vloc,
+                       int nb, int hb, cudaStream_t st) {
+  constexpr int NS = imax(R1, R2);
+  int rc;
+  if (pass >= 1 && pass <= 3 && p->fft_path == 0) {
+    rc = launch_ring<R1, R2>(p, G, pass, T1, T2, vloc, nb, hb, st);
+    if (rc != DFT_ERR_UNSUPPORTED) return rc;
+  }
   if (pass == 0 || pass == 4) {
     int lpc = F2_THREADS / NS;
     if (lpc > G.ncol) lpc = G.ncol;
@@ -369,7 +710,8 @@ int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, 
   Fft2Geom G = make_geom2(p, ik, t1_band, t2_band);
   const cplx *cpsi = reinterpret_cast<const cplx *>(psi);
   cplx *chpsi = reinterpret_cast<cplx *>(hpsi), *t1 = reinterpret_cast<cplx *>(T1), *t2 = reinterpret_cast<cplx *>(T2);
-#define X(a, b) if (r1 == (a) && r2 == (b)) return launch_pass<a, b>(G, pass, cpsi, chpsi, t1, t2, p->d_vloc, nb, st);
+  const int hb = p->kp[ik].max_cols_per_plane;
+#define X(a, b) if (r1 == (a) && r2 == (b)) return launch_pass<a, b>(p, G, pass, cpsi, chpsi, t1, t2, p->d_vloc, nb, hb, st);
   FFT2_PAIRS(X)
 #undef X
   return DFT_ERR_UNSUPPORTED;

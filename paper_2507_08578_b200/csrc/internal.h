@@ -62,6 +62,7 @@ struct KPoint {
   Run *col_run = nullptr;        // [ncol]   base = first plane wave, runs along x; aux0 = i2, aux1 = plane
   Run *plane_run = nullptr;      // [nplane] base = first column, runs along y; aux0 = i3
   Run zrun = {0, 0, 0, 0, 0, 0, 0, 0};   // base = 0, runs along z (plane ordinals)
+  int max_cols_per_plane = 0;    // largest number of non-empty columns in one plane (TMA box height of pass B)
   bool runs_ok = false;          // every occupied set really is <= 2 runs (else the generic path is used)
   // host copies for getters
   std::vector<int32_t> h_kg, h_igfft;
@@ -107,7 +108,8 @@ struct dft_plan {
   // options
   int band_chunk = 0;      // 0 = automatic
   int terms = 7;
-  int fft_path = 0;        // 0 = automatic (register path where available), 1 = generic Stockham path only
+  int fft_path = 0;        // 0 = automatic (register path, TMA ring for the strided passes), 1 = generic Stockham path only,
+                           // 2 = register path without the TMA ring
   int splitk = 0;
   // workspace
   void *ws_user = nullptr; int64_t ws_user_bytes = 0;
@@ -121,6 +123,7 @@ struct dft_plan {
   // TMA
   void *encode_fn = nullptr;   // cuTensorMapEncodeTiled
   int sm_count = 148;
+  int smem_per_sm = 233472, smem_optin = 232448;   // bytes of shared memory per SM / per CTA (opt-in), from the device
   int64_t last_launches = 0;
   dftb200::PhaseTimer timer;
 };

@@ -84,6 +84,8 @@ static int create_impl(dft_plan *p, const double rprimd[9], int32_t nkpt, const 
   DFT_CUDA_CHECK(cudaGetDeviceProperties(&prop, dev));
   if (prop.major < 10) { set_error("device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor); return DFT_ERR_CUDA; }
   p->sm_count = prop.multiProcessorCount;
+  p->smem_per_sm = (int)prop.sharedMemPerMultiprocessor;
+  p->smem_optin = (int)prop.sharedMemPerBlockOptin;
 
   // ---- lattice (reading 1)
   for (int i = 0; i < 9; i++) {
@@ -399,7 +401,7 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     p->terms = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "fft_path")) {
-    if (value < 0 || value > 1) { set_error("fft_path = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if (value < 0 || value > 2) { set_error("fft_path = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->fft_path = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "splitk")) {

@@ -233,6 +233,9 @@ int sphere_build(const double *gmet, const int n[3], double ecut, KPoint *kp) {
   }
   runs_ok &= make_run(plane_i3.data(), kp->nplane, 0, &kp->zrun);
   kp->runs_ok = runs_ok;
+  kp->max_cols_per_plane = 0;
+  for (int p = 0; p < kp->nplane; p++)
+    if (plane_col0[p + 1] - plane_col0[p] > kp->max_cols_per_plane) kp->max_cols_per_plane = plane_col0[p + 1] - plane_col0[p];
   int rc;
   if ((rc = upload(&kp->col_run, col_run))) return rc;
   if ((rc = upload(&kp->plane_run, plane_run))) return rc;

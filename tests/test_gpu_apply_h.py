@@ -39,11 +39,11 @@ def test_small_cells_all_terms_and_isolations(name):
 @pytest.mark.parametrize("name", ["c0", "c1m", "c4m", "aniso", "c3k2"])
 def test_generic_fft_path_agrees(name):
     """Option fft_path=1 forces the generic shared-memory Stockham kernels (used for box lengths with no
-    two-stage factorisation); both paths must match the oracle."""
+    two-stage factorisation), 2 the register path without the TMA ring; all paths must match the oracle."""
     cfg, plan, sph = _setup(name)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     ref = oracle_apply(cfg, sph, psi, method=1 if name in ("c0", "aniso") else 2)
-    for path in (1, 0):
+    for path in (1, 2, 0):
         plan.set_option("fft_path", path)
         err = band_rel_err(gpu_apply(plan, psi), ref)
         assert err <= TOL, "%s fft_path=%d: rel err %.3e" % (name, path, err)

@@ -111,6 +111,7 @@ struct dft_plan {
   int fft_path = 0;        // 0 = automatic (register path, TMA ring for the strided passes), 1 = generic Stockham path only,
                            // 2 = register path without the TMA ring
   int splitk = 0;
+  int gemm_3m = 1;         // 1 = three real products per complex multiply-add (6 flops), 0 = four (8 flops)
   // workspace
   void *ws_user = nullptr; int64_t ws_user_bytes = 0;
   void *ws_own = nullptr;  int64_t ws_own_bytes = 0;

@@ -133,8 +133,9 @@ struct Pipe {
 };
 __device__ __forceinline__ Pipe pipe_setup(unsigned char *smem_raw) {
   Pipe P;
-  uintptr_t base = (reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023;
-  P.tiles = reinterpret_cast<unsigned char *>(base);
+  // 1024-byte alignment (128-byte swizzle atom) by an offset on the __shared__ array itself, so the
+  // compiler keeps the shared address space (LDS/STS, not generic LD/ST)
+  P.tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   P.full = reinterpret_cast<uint64_t *>(P.tiles + NL_STAGES * NL_STAGE_BYTES);
   P.empty = P.full + NL_STAGES;
   if (threadIdx.x == 0) {
@@ -291,6 +292,197 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
   }
 }
 
+// ---------------------------------------------------------------- 3M variant of both GEMMs
+// A complex product needs only three real products (the "3M" scheme, exact up to rounding order):
+//   (a_r + i a_i)(b_r + i b_i):  T1 = a_r b_r,  T2 = a_i b_i,  T3 = (a_r + a_i)(b_r + b_i);  Re = T1 - T2,  Im = T3 - T1 - T2
+//   conj(a) b (GEMM-1):          T1, T2 as above, T3 = (a_r - a_i)(b_r + b_i);              Re = T1 + T2,  Im = T3 - T1 + T2
+// i.e. three real GEMMs over the same K instead of four: 6 instead of 8 flops per complex multiply-add
+// on the FP64 tensor pipe, which is what bounds K3.  The three products need three accumulator sets
+// (3 x 128 x 64 doubles per CTA tile = 75 % of the register file), so the CTA has 12 warps in three groups
+// of four: group g accumulates T_{g+1} for the whole 128 x 64 tile (warp tile 32 x 64, 128 accumulator
+// registers per thread, 3 warps per SM sub-partition, one of each group).  Groups 0/1 read only the
+// re/im half of each 16-byte shared-memory element; group 2 adds the halves in registers (one DADD per
+// fragment: 12 per 32 DMMAs).  The epilogue stages T1 and T2 through the (drained) tile ring and
+// group 2 combines.  TMA ring, tile shapes, swizzle and fragment addressing are those of the kernels above.
+constexpr int NL3_CONSUMERS = 12;
+constexpr int NL3_THREADS = NL3_CONSUMERS * 32;
+
+template <int MODE, int GRP>
+__device__ __forceinline__ void mma3_stage(const unsigned char *As, const unsigned char *Bs, int wq, int lane,
+                                           double (&acc)[4][8][2]) {
+  const int i = lane >> 2, j = lane & 3;
+#pragma unroll
+  for (int kg = 0; kg < 2; kg++) {
+    double a[4];
+    const unsigned char *a0;
+    int astride;
+    if (MODE == 1) { a0 = As + (wq * 32 + i) * 128 + (((2 * j + kg) ^ i) << 4); astride = 8 * 128; }
+    else { const int pr = 2 * j + kg; a0 = As + (wq * 4) * 1024 + pr * 128 + ((i ^ pr) << 4); astride = 1024; }
+#pragma unroll
+    for (int mb = 0; mb < 4; mb++) {
+      if (GRP == 0) a[mb] = *reinterpret_cast<const double *>(a0 + mb * astride);
+      else if (GRP == 1) a[mb] = *reinterpret_cast<const double *>(a0 + mb * astride + 8);
+      else {
+        double2 v = *reinterpret_cast<const double2 *>(a0 + mb * astride);
+        a[mb] = MODE == 1 ? v.x - v.y : v.x + v.y;
+      }
+    }
+    const unsigned char *b0 = Bs + i * 128 + (((2 * j + kg) ^ i) << 4);
+#pragma unroll
+    for (int nb = 0; nb < 8; nb++) {
+      double b;
+      if (GRP == 0) b = *reinterpret_cast<const double *>(b0 + nb * 8 * 128);
+      else if (GRP == 1) b = *reinterpret_cast<const double *>(b0 + nb * 8 * 128 + 8);
+      else {
+        double2 v = *reinterpret_cast<const double2 *>(b0 + nb * 8 * 128);
+        b = v.x + v.y;
+      }
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++) dmma(acc[mb][nb][0], acc[mb][nb][1], a[mb], b);
+    }
+  }
+}
+
+__device__ __forceinline__ Pipe pipe_setup3(unsigned char *smem_raw) {
+  Pipe P;
+  // 1024-byte alignment (128-byte swizzle atom) by an offset on the __shared__ array itself, so the
+  // compiler keeps the shared address space (LDS/STS, not generic LD/ST)
+  P.tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  P.full = reinterpret_cast<uint64_t *>(P.tiles + NL_STAGES * NL_STAGE_BYTES);
+  P.empty = P.full + NL_STAGES;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < NL_STAGES; s++) { mbar_init(&P.full[s], 1); mbar_init(&P.empty[s], NL3_CONSUMERS); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  return P;
+}
+
+// main loop of one warp of group GRP: waits for slabs, multiplies, releases; the producer lane also issues
+template <int MODE, int GRP, typename Issue>
+__device__ __forceinline__ void mainloop3(const Pipe &P, int ns, bool producer, int wq, int lane, double (&acc)[4][8][2],
+                                          Issue &issue) {
+  for (int it = 0; it < ns; it++) {
+    if (producer && it + NL_PREFETCH < ns) issue(it + NL_PREFETCH);
+    __syncwarp();
+    int s = it % NL_STAGES;
+    mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
+    const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mma3_stage<MODE, GRP>(st, st + NL_STAGE_A, wq, lane, acc);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&P.empty[s]);
+  }
+}
+
+// T1 (group 0) and T2 (group 1) go through shared memory; group 2 combines and hands every output
+// (mb, nb, e, re, im) of its 32 x 64 warp tile to `emit`
+template <int MODE, typename Emit>
+__device__ __forceinline__ void combine3(const Pipe &P, int grp, int wq, int lane, double (&acc)[4][8][2], Emit &emit) {
+  __syncthreads();   // every warp is done with the tile ring (all issued slabs were consumed)
+  double *X = reinterpret_cast<double *>(P.tiles);
+  if (grp < 2) {
+    double *dst = X + (size_t)grp * (NL_BM * NL_BN) + (size_t)wq * 64 * 32 + lane;
+#pragma unroll
+    for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+      for (int nb = 0; nb < 8; nb++)
+#pragma unroll
+        for (int e = 0; e < 2; e++) dst[((mb * 8 + nb) * 2 + e) * 32] = acc[mb][nb][e];
+  }
+  __syncthreads();
+  if (grp == 2) {
+    const double *s1 = X + (size_t)wq * 64 * 32 + lane, *s2 = s1 + NL_BM * NL_BN;
+#pragma unroll
+    for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+      for (int nb = 0; nb < 8; nb++)
+#pragma unroll
+        for (int e = 0; e < 2; e++) {
+          double t1 = s1[((mb * 8 + nb) * 2 + e) * 32], t2 = s2[((mb * 8 + nb) * 2 + e) * 32];
+          if (MODE == 1) emit(mb, nb, e, t1 + t2, (acc[mb][nb][e] - t1) + t2);
+          else emit(mb, nb, e, t1 - t2, (acc[mb][nb][e] - t1) - t2);
+        }
+  }
+}
+
+#define NL3_ZERO_ACC(acc)                                   \
+  _Pragma("unroll") for (int a_ = 0; a_ < 4; a_++)          \
+  _Pragma("unroll") for (int b_ = 0; b_ < 8; b_++) { acc[a_][b_][0] = 0.0; acc[a_][b_][1] = 0.0; }
+
+__global__ void __launch_bounds__(NL3_THREADS, 1)
+gemm1_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapPsi, Gemm1Params Q) {
+  extern __shared__ unsigned char smem_raw[];
+  Pipe P = pipe_setup3(smem_raw);
+  const int tile = blockIdx.x, tn = tile % Q.tiles_n, tm = tile / Q.tiles_n;
+  const int split = blockIdx.y, ik = blockIdx.z;
+  const int s0 = split * Q.slabs_per_split;
+  int ns = Q.nslab - s0; if (ns > Q.slabs_per_split) ns = Q.slabs_per_split; if (ns < 0) ns = 0;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, grp = warp >> 2, wq = warp & 3;
+  auto issue = [&](int j) {
+    int s = j % NL_STAGES;
+    if (j >= NL_STAGES) mbar_wait(&P.empty[s], ((j / NL_STAGES) - 1) & 1);
+    unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mbar_expect_tx(&P.full[s], NL_STAGE_BYTES);
+    tma_load_3d(st, &mapP, &P.full[s], (s0 + j) * 16, tm * NL_BM, ik);
+    tma_load_3d(st + NL_STAGE_A, &mapPsi, &P.full[s], (s0 + j) * 16, tn * NL_BN, ik);
+  };
+  const bool producer = (threadIdx.x == 0);
+  if (producer)
+    for (int j = 0; j < NL_PREFETCH && j < ns; j++) issue(j);
+  double acc[4][8][2];
+  NL3_ZERO_ACC(acc)
+  if (grp == 0) mainloop3<1, 0>(P, ns, producer, wq, lane, acc, issue);
+  else if (grp == 1) mainloop3<1, 1>(P, ns, false, wq, lane, acc, issue);
+  else mainloop3<1, 2>(P, ns, false, wq, lane, acc, issue);
+  double2 *out = Q.part + ((size_t)(ik * Q.nsplit + split) * Q.nproj) * Q.nband;
+  const int i = lane >> 2, j = lane & 3;
+  auto emit = [&](int mb, int nb, int e, double re, double im) {
+    int pr = tm * NL_BM + wq * 32 + mb * 8 + i, b = tn * NL_BN + nb * 8 + 2 * j + e;
+    if (pr < Q.nproj && b < Q.nband) out[(size_t)pr * Q.nband + b] = make_double2(re, im);
+  };
+  combine3<1>(P, grp, wq, lane, acc, emit);
+}
+
+__global__ void __launch_bounds__(NL3_THREADS, 1)
+gemm2_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapC, Gemm2Params Q) {
+  extern __shared__ unsigned char smem_raw[];
+  Pipe P = pipe_setup3(smem_raw);
+  const int tn = blockIdx.x % Q.tiles_n, tm = blockIdx.x / Q.tiles_n, ik = blockIdx.z;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, grp = warp >> 2, wq = warp & 3;
+  const int ns = Q.with_nl ? Q.nslab : 0;
+  auto issue = [&](int j) {
+    int s = j % NL_STAGES;
+    if (j >= NL_STAGES) mbar_wait(&P.empty[s], ((j / NL_STAGES) - 1) & 1);
+    unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mbar_expect_tx(&P.full[s], NL_STAGE_BYTES);
+    tma_load_4d(st, &mapP, &P.full[s], 0, j * 8, tm * (NL_BM / 8), ik);
+    tma_load_3d(st + NL_STAGE_A, &mapC, &P.full[s], j * 16, tn * NL_BN, ik);
+  };
+  const bool producer = (threadIdx.x == 0);
+  if (producer)
+    for (int j = 0; j < NL_PREFETCH && j < ns; j++) issue(j);
+  double acc[4][8][2];
+  NL3_ZERO_ACC(acc)
+  if (grp == 0) mainloop3<2, 0>(P, ns, producer, wq, lane, acc, issue);
+  else if (grp == 1) mainloop3<2, 1>(P, ns, false, wq, lane, acc, issue);
+  else mainloop3<2, 2>(P, ns, false, wq, lane, acc, issue);
+  const int npw = Q.npw[ik];
+  const double *kin = Q.kin[ik];
+  const double2 *psi = Q.psi + (size_t)ik * Q.nband * Q.mpw;
+  double2 *hpsi = Q.hpsi + (size_t)ik * Q.nband * Q.mpw;
+  const int i = lane >> 2, j = lane & 3;
+  auto emit = [&](int mb, int nb, int e, double re, double im) {
+    int g = tm * NL_BM + wq * 32 + mb * 8 + i, b = tn * NL_BN + nb * 8 + 2 * j + e;
+    if (g >= npw || b >= Q.nband) return;
+    size_t off = (size_t)b * Q.mpw + g;
+    double2 r = make_double2(re, im);
+    if (Q.with_kin) { double kg = kin[g]; double2 x = psi[off]; r.x += kg * x.x; r.y += kg * x.y; }
+    if (Q.accumulate) { double2 h = hpsi[off]; r.x += h.x; r.y += h.y; }
+    hpsi[off] = r;
+  };
+  combine3<2>(P, grp, wq, lane, acc, emit);
+}
+
 // ---------------------------------------------------------------- host side
 typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                              const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -352,6 +544,8 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   if (!g_nl_attr) {
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     g_nl_attr = true;
   }
   const int32_t *d_npw = p->d_npw;
@@ -411,7 +605,8 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   }
   if ((rc = make_map(p, &mapC, p->d_cprj, 2 * (uint64_t)nproj, nband, nkpt, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * nband, NL_BN))) return rc;
   phase_begin(p, 5, st);
-  gemm1_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  else gemm1_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   phase_end(p, 5, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   // ---- D_ij
@@ -428,7 +623,8 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   q2.npw = d_npw; q2.kin = d_kin; q2.psi = cpsi; q2.hpsi = chpsi;
   int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
   phase_begin(p, 7, st);
-  gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  else gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   phase_end(p, 7, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   return DFT_OK;

@@ -404,6 +404,10 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     if (value < 0 || value > 2) { set_error("fft_path = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->fft_path = (int)value; return DFT_OK;
   }
+  if (!strcmp(key, "gemm_3m")) {
+    if (value < 0 || value > 1) { set_error("gemm_3m = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->gemm_3m = (int)value; return DFT_OK;
+  }
   if (!strcmp(key, "splitk")) {
     if (value < 0 || value > 4096) { set_error("splitk = %lld outside 0..4096", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->splitk = (int)value; return DFT_OK;

@@ -293,60 +293,63 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
 }
 
 // ---------------------------------------------------------------- 3M variant of both GEMMs
-// A complex product needs only three real products (the "3M" scheme, exact up to rounding order):
-//   (a_r + i a_i)(b_r + i b_i):  T1 = a_r b_r,  T2 = a_i b_i,  T3 = (a_r + a_i)(b_r + b_i);  Re = T1 - T2,  Im = T3 - T1 - T2
-//   conj(a) b (GEMM-1):          T1, T2 as above, T3 = (a_r - a_i)(b_r + b_i);              Re = T1 + T2,  Im = T3 - T1 + T2
-// i.e. three real GEMMs over the same K instead of four: 6 instead of 8 flops per complex multiply-add
-// on the FP64 tensor pipe, which is what bounds K3.  The three products need three accumulator sets
+// A complex product needs only three real products (Gauss / "3M", exact up to rounding order):
+//   a b       (GEMM-2):  k1 = (a_r + a_i) b_r,  k2 = a_r (b_i - b_r),  k3 = a_i (b_r + b_i);  Re = k1 - k3,  Im = k1 + k2
+//   conj(a) b (GEMM-1):  k1 = (a_r - a_i) b_r,  k2, k3 as above;                              Re = k1 + k3,  Im = k1 + k2
+// i.e. three real GEMMs over the same K instead of four: 6 instead of 8 flops per complex multiply-add on
+// the FP64 tensor pipe, which is what bounds K3.  The three products need three accumulator sets
 // (3 x 128 x 64 doubles per CTA tile = 75 % of the register file), so the CTA has 12 warps in three groups
-// of four: group g accumulates T_{g+1} for the whole 128 x 64 tile (warp tile 32 x 64, 128 accumulator
-// registers per thread, 3 warps per SM sub-partition, one of each group).  Groups 0/1 read only the
-// re/im half of each 16-byte shared-memory element; group 2 adds the halves in registers (one DADD per
-// fragment: 12 per 32 DMMAs).  The epilogue stages T1 and T2 through the (drained) tile ring and
-// group 2 combines.  TMA ring, tile shapes, swizzle and fragment addressing are those of the kernels above.
+// of four (one warp of each group per SM sub-partition, 128 accumulator registers per thread):
+//   group 0: k1, warp tile 32 (M) x 64 (N): 4 A fragments summed in registers, 8 plain B fragments
+//   group 1: k2, warp tile 64 x 32: 8 plain A fragments (re), 4 B fragments (b_i - b_r)
+//   group 2: k3, warp tile 64 x 32: 8 plain A fragments (im), 4 B fragments (b_r + b_i)
+// so every warp does 12 shared-memory loads, 4 DADDs and 32 DMMAs per k-group: the groups run at the same
+// pace (with all the sums in one group that group lagged and the others idled at the ring: 88 % DMMA
+// utilisation, profiles/).  The epilogue stages k2 and k3 through the drained tile ring; group 0 combines.
+// TMA ring, tile shapes, swizzle and fragment addressing are those of the kernels above.
 constexpr int NL3_CONSUMERS = 12;
 constexpr int NL3_THREADS = NL3_CONSUMERS * 32;
+constexpr int NL3_XS = NL_BN + 2;   // padded row stride (doubles) of the staged k2 / k3 tiles
 
+// GRP 0: acc[mb 0..3][nb 0..7]; GRP 1, 2: acc[mb 0..7][nb 0..3]; flat index (mb * NB + nb) * 2 + e
 template <int MODE, int GRP>
-__device__ __forceinline__ void mma3_stage(const unsigned char *As, const unsigned char *Bs, int wq, int lane,
-                                           double (&acc)[4][8][2]) {
+__device__ __forceinline__ void mma3_stage(const unsigned char *As, const unsigned char *Bs, int wq, int lane, double (&acc)[64]) {
+  constexpr int MB = GRP == 0 ? 4 : 8, NB = GRP == 0 ? 8 : 4;
   const int i = lane >> 2, j = lane & 3;
+  const int row0 = GRP == 0 ? wq * 32 : (wq >> 1) * 64, col0 = GRP == 0 ? 0 : (wq & 1) * 32;
 #pragma unroll
   for (int kg = 0; kg < 2; kg++) {
-    double a[4];
+    double a[MB], b[NB];
     const unsigned char *a0;
     int astride;
-    if (MODE == 1) { a0 = As + (wq * 32 + i) * 128 + (((2 * j + kg) ^ i) << 4); astride = 8 * 128; }
-    else { const int pr = 2 * j + kg; a0 = As + (wq * 4) * 1024 + pr * 128 + ((i ^ pr) << 4); astride = 1024; }
+    if (MODE == 1) { a0 = As + (row0 + i) * 128 + (((2 * j + kg) ^ i) << 4); astride = 8 * 128; }
+    else { const int pr = 2 * j + kg; a0 = As + (row0 >> 3) * 1024 + pr * 128 + ((i ^ pr) << 4); astride = 1024; }
 #pragma unroll
-    for (int mb = 0; mb < 4; mb++) {
-      if (GRP == 0) a[mb] = *reinterpret_cast<const double *>(a0 + mb * astride);
-      else if (GRP == 1) a[mb] = *reinterpret_cast<const double *>(a0 + mb * astride + 8);
-      else {
+    for (int mb = 0; mb < MB; mb++) {
+      if (GRP == 0) {
         double2 v = *reinterpret_cast<const double2 *>(a0 + mb * astride);
         a[mb] = MODE == 1 ? v.x - v.y : v.x + v.y;
-      }
+      } else if (GRP == 1) a[mb] = *reinterpret_cast<const double *>(a0 + mb * astride);
+      else a[mb] = *reinterpret_cast<const double *>(a0 + mb * astride + 8);
     }
-    const unsigned char *b0 = Bs + i * 128 + (((2 * j + kg) ^ i) << 4);
+    const unsigned char *b0 = Bs + (col0 + i) * 128 + (((2 * j + kg) ^ i) << 4);
 #pragma unroll
-    for (int nb = 0; nb < 8; nb++) {
-      double b;
-      if (GRP == 0) b = *reinterpret_cast<const double *>(b0 + nb * 8 * 128);
-      else if (GRP == 1) b = *reinterpret_cast<const double *>(b0 + nb * 8 * 128 + 8);
+    for (int nb = 0; nb < NB; nb++) {
+      if (GRP == 0) b[nb] = *reinterpret_cast<const double *>(b0 + nb * 8 * 128);
       else {
         double2 v = *reinterpret_cast<const double2 *>(b0 + nb * 8 * 128);
-        b = v.x + v.y;
+        b[nb] = GRP == 1 ? v.y - v.x : v.x + v.y;
       }
-#pragma unroll
-      for (int mb = 0; mb < 4; mb++) dmma(acc[mb][nb][0], acc[mb][nb][1], a[mb], b);
     }
+#pragma unroll
+    for (int mb = 0; mb < MB; mb++)
+#pragma unroll
+      for (int nb = 0; nb < NB; nb++) dmma(acc[(mb * NB + nb) * 2], acc[(mb * NB + nb) * 2 + 1], a[mb], b[nb]);
   }
 }
 
 __device__ __forceinline__ Pipe pipe_setup3(unsigned char *smem_raw) {
   Pipe P;
-  // 1024-byte alignment (128-byte swizzle atom) by an offset on the __shared__ array itself, so the
-  // compiler keeps the shared address space (LDS/STS, not generic LD/ST)
   P.tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   P.full = reinterpret_cast<uint64_t *>(P.tiles + NL_STAGES * NL_STAGE_BYTES);
   P.empty = P.full + NL_STAGES;
@@ -360,8 +363,7 @@ __device__ __forceinline__ Pipe pipe_setup3(unsigned char *smem_raw) {
 
 // main loop of one warp of group GRP: waits for slabs, multiplies, releases; the producer lane also issues
 template <int MODE, int GRP, typename Issue>
-__device__ __forceinline__ void mainloop3(const Pipe &P, int ns, bool producer, int wq, int lane, double (&acc)[4][8][2],
-                                          Issue &issue) {
+__device__ __forceinline__ void mainloop3(const Pipe &P, int ns, bool producer, int wq, int lane, double (&acc)[64], Issue &issue) {
   for (int it = 0; it < ns; it++) {
     if (producer && it + NL_PREFETCH < ns) issue(it + NL_PREFETCH);
     __syncwarp();
@@ -374,40 +376,37 @@ __device__ __forceinline__ void mainloop3(const Pipe &P, int ns, bool producer, 
   }
 }
 
-// T1 (group 0) and T2 (group 1) go through shared memory; group 2 combines and hands every output
-// (mb, nb, e, re, im) of its 32 x 64 warp tile to `emit`
+// k2 (group 1) and k3 (group 2) go through shared memory as [128][NL3_XS] tiles; group 0 combines and hands
+// every output (row in tile, column in tile, re, im) of its 32 x 64 warp tile to `emit`
 template <int MODE, typename Emit>
-__device__ __forceinline__ void combine3(const Pipe &P, int grp, int wq, int lane, double (&acc)[4][8][2], Emit &emit) {
+__device__ __forceinline__ void combine3(const Pipe &P, int grp, int wq, int lane, double (&acc)[64], Emit &emit) {
   __syncthreads();   // every warp is done with the tile ring (all issued slabs were consumed)
   double *X = reinterpret_cast<double *>(P.tiles);
-  if (grp < 2) {
-    double *dst = X + (size_t)grp * (NL_BM * NL_BN) + (size_t)wq * 64 * 32 + lane;
+  const int i = lane >> 2, j = lane & 3;
+  if (grp > 0) {
+    double *dst = X + (size_t)(grp - 1) * (NL_BM * NL3_XS) + (size_t)((wq >> 1) * 64 + i) * NL3_XS + (wq & 1) * 32 + 2 * j;
 #pragma unroll
-    for (int mb = 0; mb < 4; mb++)
+    for (int mb = 0; mb < 8; mb++)
 #pragma unroll
-      for (int nb = 0; nb < 8; nb++)
-#pragma unroll
-        for (int e = 0; e < 2; e++) dst[((mb * 8 + nb) * 2 + e) * 32] = acc[mb][nb][e];
+      for (int nb = 0; nb < 4; nb++)
+        *reinterpret_cast<double2 *>(dst + (size_t)mb * 8 * NL3_XS + nb * 8) = make_double2(acc[(mb * 4 + nb) * 2], acc[(mb * 4 + nb) * 2 + 1]);
   }
   __syncthreads();
-  if (grp == 2) {
-    const double *s1 = X + (size_t)wq * 64 * 32 + lane, *s2 = s1 + NL_BM * NL_BN;
+  if (grp == 0) {
+    const double *s2 = X + (size_t)(wq * 32 + i) * NL3_XS + 2 * j, *s3 = s2 + NL_BM * NL3_XS;
 #pragma unroll
     for (int mb = 0; mb < 4; mb++)
 #pragma unroll
-      for (int nb = 0; nb < 8; nb++)
-#pragma unroll
-        for (int e = 0; e < 2; e++) {
-          double t1 = s1[((mb * 8 + nb) * 2 + e) * 32], t2 = s2[((mb * 8 + nb) * 2 + e) * 32];
-          if (MODE == 1) emit(mb, nb, e, t1 + t2, (acc[mb][nb][e] - t1) + t2);
-          else emit(mb, nb, e, t1 - t2, (acc[mb][nb][e] - t1) - t2);
-        }
+      for (int nb = 0; nb < 8; nb++) {
+        double2 k2 = *reinterpret_cast<const double2 *>(s2 + (size_t)mb * 8 * NL3_XS + nb * 8);
+        double2 k3 = *reinterpret_cast<const double2 *>(s3 + (size_t)mb * 8 * NL3_XS + nb * 8);
+        double k1a = acc[(mb * 8 + nb) * 2], k1b = acc[(mb * 8 + nb) * 2 + 1];
+        const int r = wq * 32 + mb * 8 + i, c = nb * 8 + 2 * j;
+        if (MODE == 1) { emit(r, c, k1a + k3.x, k1a + k2.x); emit(r, c + 1, k1b + k3.y, k1b + k2.y); }
+        else { emit(r, c, k1a - k3.x, k1a + k2.x); emit(r, c + 1, k1b - k3.y, k1b + k2.y); }
+      }
   }
 }
-
-#define NL3_ZERO_ACC(acc)                                   \
-  _Pragma("unroll") for (int a_ = 0; a_ < 4; a_++)          \
-  _Pragma("unroll") for (int b_ = 0; b_ < 8; b_++) { acc[a_][b_][0] = 0.0; acc[a_][b_][1] = 0.0; }
 
 __global__ void __launch_bounds__(NL3_THREADS, 1)
 gemm1_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapPsi, Gemm1Params Q) {
@@ -429,15 +428,15 @@ gemm1_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant_
   const bool producer = (threadIdx.x == 0);
   if (producer)
     for (int j = 0; j < NL_PREFETCH && j < ns; j++) issue(j);
-  double acc[4][8][2];
-  NL3_ZERO_ACC(acc)
+  double acc[64];
+#pragma unroll
+  for (int q = 0; q < 64; q++) acc[q] = 0.0;
   if (grp == 0) mainloop3<1, 0>(P, ns, producer, wq, lane, acc, issue);
   else if (grp == 1) mainloop3<1, 1>(P, ns, false, wq, lane, acc, issue);
   else mainloop3<1, 2>(P, ns, false, wq, lane, acc, issue);
   double2 *out = Q.part + ((size_t)(ik * Q.nsplit + split) * Q.nproj) * Q.nband;
-  const int i = lane >> 2, j = lane & 3;
-  auto emit = [&](int mb, int nb, int e, double re, double im) {
-    int pr = tm * NL_BM + wq * 32 + mb * 8 + i, b = tn * NL_BN + nb * 8 + 2 * j + e;
+  auto emit = [&](int r, int c, double re, double im) {
+    int pr = tm * NL_BM + r, b = tn * NL_BN + c;
     if (pr < Q.nproj && b < Q.nband) out[(size_t)pr * Q.nband + b] = make_double2(re, im);
   };
   combine3<1>(P, grp, wq, lane, acc, emit);
@@ -461,24 +460,20 @@ gemm2_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant_
   const bool producer = (threadIdx.x == 0);
   if (producer)
     for (int j = 0; j < NL_PREFETCH && j < ns; j++) issue(j);
-  double acc[4][8][2];
-  NL3_ZERO_ACC(acc)
+  double acc[64];
+#pragma unroll
+  for (int q = 0; q < 64; q++) acc[q] = 0.0;
   if (grp == 0) mainloop3<2, 0>(P, ns, producer, wq, lane, acc, issue);
   else if (grp == 1) mainloop3<2, 1>(P, ns, false, wq, lane, acc, issue);
   else mainloop3<2, 2>(P, ns, false, wq, lane, acc, issue);
-  const int npw = Q.npw[ik];
-  const double *kin = Q.kin[ik];
-  const double2 *psi = Q.psi + (size_t)ik * Q.nband * Q.mpw;
-  double2 *hpsi = Q.hpsi + (size_t)ik * Q.nband * Q.mpw;
-  const int i = lane >> 2, j = lane & 3;
-  auto emit = [&](int mb, int nb, int e, double re, double im) {
-    int g = tm * NL_BM + wq * 32 + mb * 8 + i, b = tn * NL_BN + nb * 8 + 2 * j + e;
-    if (g >= npw || b >= Q.nband) return;
-    size_t off = (size_t)b * Q.mpw + g;
-    double2 r = make_double2(re, im);
-    if (Q.with_kin) { double kg = kin[g]; double2 x = psi[off]; r.x += kg * x.x; r.y += kg * x.y; }
-    if (Q.accumulate) { double2 h = hpsi[off]; r.x += h.x; r.y += h.y; }
-    hpsi[off] = r;
+  auto emit = [&](int r, int c, double re, double im) {
+    const int g = tm * NL_BM + r, b = tn * NL_BN + c;
+    if (g >= Q.npw[ik] || b >= Q.nband) return;
+    size_t off = ((size_t)ik * Q.nband + b) * Q.mpw + g;
+    double2 v = make_double2(re, im);
+    if (Q.with_kin) { double kg = Q.kin[ik][g]; double2 x = Q.psi[off]; v.x += kg * x.x; v.y += kg * x.y; }
+    if (Q.accumulate) { double2 h = Q.hpsi[off]; v.x += h.x; v.y += h.y; }
+    Q.hpsi[off] = v;
   };
   combine3<2>(P, grp, wq, lane, acc, emit);
 }

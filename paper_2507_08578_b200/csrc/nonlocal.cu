@@ -466,16 +466,43 @@ gemm2_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant_
   if (grp == 0) mainloop3<2, 0>(P, ns, producer, wq, lane, acc, issue);
   else if (grp == 1) mainloop3<2, 1>(P, ns, false, wq, lane, acc, issue);
   else mainloop3<2, 2>(P, ns, false, wq, lane, acc, issue);
-  auto emit = [&](int r, int c, double re, double im) {
-    const int g = tm * NL_BM + r, b = tn * NL_BN + c;
-    if (g >= Q.npw[ik] || b >= Q.nband) return;
-    size_t off = ((size_t)ik * Q.nband + b) * Q.mpw + g;
-    double2 v = make_double2(re, im);
-    if (Q.with_kin) { double kg = Q.kin[ik][g]; double2 x = Q.psi[off]; v.x += kg * x.x; v.y += kg * x.y; }
-    if (Q.accumulate) { double2 h = Q.hpsi[off]; v.x += h.x; v.y += h.y; }
-    Q.hpsi[off] = v;
+  // group 0 leaves (re, im) of the whole 128 x 64 tile in the k2 / k3 staging tiles; then all 12 warps run the
+  // epilogue with g (contiguous in psi / hpsi) along the lanes and their loads batched U at a time
+  auto keep = [&](int r, int c, double re, double im) {
+    double *X = reinterpret_cast<double *>(P.tiles);
+    X[(size_t)r * NL3_XS + c] = re;
+    X[(size_t)NL_BM * NL3_XS + (size_t)r * NL3_XS + c] = im;
   };
-  combine3<2>(P, grp, wq, lane, acc, emit);
+  combine3<2>(P, grp, wq, lane, acc, keep);
+  __syncthreads();
+  const double *Xre = reinterpret_cast<const double *>(P.tiles), *Xim = Xre + NL_BM * NL3_XS;
+  const int r = threadIdx.x & (NL_BM - 1), c0 = threadIdx.x >> 7;   // 384 threads = 3 columns of 128 rows
+  const int g = tm * NL_BM + r;
+  const bool gok = g < Q.npw[ik];
+  const double kg = (Q.with_kin && gok) ? Q.kin[ik][g] : 0.0;
+  const size_t base = (size_t)ik * Q.nband * Q.mpw + g;
+  constexpr int U = 6, NQ = (NL_BN + 2) / 3;
+#pragma unroll 1
+  for (int q0 = 0; q0 < NQ; q0 += U) {
+    double2 x[U], h[U];
+    bool ok[U];
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+      const int c = c0 + 3 * (q0 + u), b = tn * NL_BN + c;
+      ok[u] = gok && c < NL_BN && b < Q.nband;
+      const size_t off = base + (size_t)b * Q.mpw;
+      x[u] = (ok[u] && Q.with_kin) ? Q.psi[off] : make_double2(0.0, 0.0);
+      h[u] = (ok[u] && Q.accumulate) ? Q.hpsi[off] : make_double2(0.0, 0.0);
+    }
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+      const int c = c0 + 3 * (q0 + u), b = tn * NL_BN + c;
+      if (ok[u]) {
+        double2 v = make_double2(Xre[(size_t)r * NL3_XS + c] + kg * x[u].x + h[u].x, Xim[(size_t)r * NL3_XS + c] + kg * x[u].y + h[u].y);
+        Q.hpsi[base + (size_t)b * Q.mpw] = v;
+      }
+    }
+  }
 }
 
 // ---------------------------------------------------------------- host side

@@ -457,14 +457,15 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
   __syncthreads();
   const int first = (int)(((int64_t)Q.ntiles * blockIdx.x) / gridDim.x);
   const int nmine = (int)(((int64_t)Q.ntiles * (blockIdx.x + 1)) / gridDim.x) - first;
+  // the (x, y) plane is one flat index xy = x + n1 y (x-lines are contiguous in T2 and V), tiled XT at a time
   const size_t pstride = (size_t)G.n2 * G.n1;
-  int b = first % Q.nb, xt = (first / Q.nb) % Q.nxt, y = first / (Q.nb * Q.nxt);
-  int ib = b, ixt = xt, iy = y, ist = 0;      // producer's copy (lane 0 only), runs S-1 tiles ahead
+  int b = first % Q.nb, g = first / Q.nb;
+  int ib = b, ig = g, ist = 0;      // producer's copy (lane 0 only), runs S-1 tiles ahead
   auto issue = [&]() {
     mbar_expect_tx(&full[ist], Q.box_bytes);
-    tma_load_4d(stages + (size_t)ist * Q.stage_stride, &mapT2, &full[ist], 2 * ixt * XT, iy, 0, ib);
+    tma_load_3d(stages + (size_t)ist * Q.stage_stride, &mapT2, &full[ist], 2 * ig * XT, 0, ib);
     if (++ist == Q.S) ist = 0;
-    if (++ib == Q.nb) { ib = 0; if (++ixt == Q.nxt) { ixt = 0; iy++; } }
+    if (++ib == Q.nb) { ib = 0; ig++; }
   };
   if (t == 0)
     for (int j = 0; j < Q.S - 1 && j < nmine; j++) issue();
@@ -472,14 +473,14 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
   bool newgroup = true;
   for (int it = 0; it < nmine; it++) {
     if (t == 0 && it + Q.S - 1 < nmine) issue();
-    const int x = xt * XT + px;
-    const bool xok = x < G.n1;
+    const size_t xy = (size_t)g * XT + px;
+    const bool xok = xy < pstride;
     if (newgroup) {
       // every read of the previous V tile happened before the barrier that ended the last iteration
-      const double *vp = vloc + (size_t)y * G.n1 + xt * XT;
+      const double *vp = vloc + (size_t)g * XT;
       for (int i = t; i < G.n3 * XT; i += blockDim.x) {
         int z = i / XT, xx = i - z * XT;
-        vs[i] = (xt * XT + xx < G.n1) ? __ldg(vp + (size_t)z * pstride + xx) : 0.0;
+        vs[i] = ((size_t)g * XT + xx < pstride) ? __ldg(vp + (size_t)z * pstride + xx) : 0.0;
       }
       newgroup = false;
     }
@@ -519,7 +520,7 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
 #pragma unroll
       for (int a = 0; a < R1; a++) v[a] = sm[s * KSb + a * XT + px];
       Dft<R1, -1>::run(v);
-      cplx *base = T2 + (size_t)b * G.t2_band + (size_t)y * G.n1 + x;
+      cplx *base = T2 + (size_t)b * G.t2_band + xy;
 #pragma unroll
       for (int d = 0; d < R1; d++) {
         int p = xok ? run_map(G.zrun, s + R2 * d) : -1;
@@ -528,7 +529,7 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
     }
     __syncthreads();
     if (++st == Q.S) { st = 0; ph ^= 1; }
-    if (++b == Q.nb) { b = 0; newgroup = true; if (++xt == Q.nxt) { xt = 0; y++; } }
+    if (++b == Q.nb) { b = 0; newgroup = true; g++; }
   }
 }
 
@@ -602,8 +603,17 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
                        cudaStream_t st) {
   constexpr int NS = imax(R1, R2);
   if (!p->encode_fn) return DFT_ERR_UNSUPPORTED;
-  const int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
-  if (XT * NS > F2_THREADS || (XT * 16) % 16) return DFT_ERR_UNSUPPORTED;
+  // passes B / B^-1 tile x; pass C tiles the flat (x, y) plane, so its XT need not divide n1: the largest multiple of 8
+  // (128-byte runs, 8 full warps for NS = 15, 16) that fits the block
+  int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
+  if (pass == 2) {
+    XT = (F2_THREADS / NS) & ~7;
+    if (XT < 8) return DFT_ERR_UNSUPPORTED;
+    int64_t nxy = (int64_t)G.n1 * G.n2;
+    if (XT > nxy) XT = (int)((nxy + 1) & ~1LL);
+    nxt = (int)((nxy + XT - 1) / XT);
+  }
+  if (XT * NS > F2_THREADS) return DFT_ERR_UNSUPPORTED;
   const int rows = pass == 1 ? hb : (pass == 2 ? G.nplane : G.n2);
   const int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
   size_t ex = sizeof(cplx) * (size_t)(pass == 1 ? R1 * KSa : (pass == 3 ? R2 * KSb : imax(R1 * KSa, R2 * KSb)));
@@ -612,7 +622,7 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
   Q.XT = XT; Q.nxt = nxt; Q.nb = nb;
   Q.box_bytes = (uint32_t)((size_t)rows * XT * 16);
   Q.stage_stride = (Q.box_bytes + 127u) & ~127u;
-  int64_t ntiles = (int64_t)nb * nxt * (pass == 2 ? G.n2 : G.nplane);
+  int64_t ntiles = (int64_t)nb * nxt * (pass == 2 ? 1 : G.nplane);
   if (ntiles > 0x7fffffffLL) return DFT_ERR_UNSUPPORTED;
   Q.ntiles = (int)ntiles;
   const size_t fixed = ex + extra + 8 * 8;
@@ -635,10 +645,15 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
     cuuint64_t strides[2] = {(cuuint64_t)G.n1 * 16, (cuuint64_t)G.t1_band * 16};
     cuuint32_t box[3] = {2 * (cuuint32_t)XT, (cuuint32_t)rows, 1};
     if ((rc = encode_map(p, &map, T1, 3, dims, strides, box))) return rc;
+  } else if (pass == 2) {
+    cuuint64_t dims[3] = {2 * (cuuint64_t)G.n1 * G.n2, (cuuint64_t)G.nplane, (cuuint64_t)nb};
+    cuuint64_t strides[2] = {(cuuint64_t)G.n1 * G.n2 * 16, (cuuint64_t)G.t2_band * 16};
+    cuuint32_t box[3] = {2 * (cuuint32_t)XT, (cuuint32_t)rows, 1};
+    if ((rc = encode_map(p, &map, T2, 3, dims, strides, box))) return rc;
   } else {
     cuuint64_t dims[4] = {2 * (cuuint64_t)G.n1, (cuuint64_t)G.n2, (cuuint64_t)G.nplane, (cuuint64_t)nb};
     cuuint64_t strides[3] = {(cuuint64_t)G.n1 * 16, (cuuint64_t)G.n1 * G.n2 * 16, (cuuint64_t)G.t2_band * 16};
-    cuuint32_t box[4] = {2 * (cuuint32_t)XT, pass == 2 ? 1u : (cuuint32_t)rows, pass == 2 ? (cuuint32_t)rows : 1u, 1};
+    cuuint32_t box[4] = {2 * (cuuint32_t)XT, (cuuint32_t)rows, 1, 1};
     if ((rc = encode_map(p, &map, T2, 4, dims, strides, box))) return rc;
   }
   int grid = per_sm * p->sm_count;

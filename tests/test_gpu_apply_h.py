@@ -50,6 +50,22 @@ def test_generic_fft_path_agrees(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c1m", "c4m", "aniso", "c3k2"])
+def test_both_gemm_variants_agree(name):
+    """Option gemm_3m: 1 (default) = three real DMMA products per complex multiply-add (Gauss), 0 = four;
+    both must match the oracle, with and without the non-local term's neighbours."""
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    for terms in (7, 4):
+        ref = oracle_apply(cfg, sph, psi, terms=terms, method=1 if name == "aniso" else 2)
+        plan.set_option("terms", terms)
+        for g3 in (0, 1):
+            plan.set_option("gemm_3m", g3)
+            err = band_rel_err(gpu_apply(plan, psi), ref)
+            assert err <= TOL, "%s gemm_3m=%d terms=%d: rel err %.3e" % (name, g3, terms, err)
+    plan.destroy()
+
+
 def test_box_without_two_stage_factorisation():
     """Box 10 x 20 x 27: 10 and 27 have no two-stage factorisation (generic kernels), 20 = 4 x 5 has, so the
     passes of one transform mix both kernel families."""

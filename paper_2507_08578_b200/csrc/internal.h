@@ -120,7 +120,8 @@ struct dft_plan {
   double *d_cprj = nullptr; int64_t cprj_bytes = 0;  // c' [nkpt][nband][nproj] complex
   // host staging for dft_apply_h_host
   double *d_stage_in = nullptr, *d_stage_out = nullptr; int64_t stage_bytes = 0;
-  cudaStream_t host_stream = nullptr;
+  cudaStream_t host_stream = nullptr, h2d_stream = nullptr, d2h_stream = nullptr;
+  int host_groups = 4;     // dft_apply_h_host: band groups whose copies overlap the kernels of their neighbours
   // TMA
   void *encode_fn = nullptr;   // cuTensorMapEncodeTiled
   int sm_count = 148;

@@ -63,6 +63,8 @@ static void destroy_plan(dft_plan *p) {
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
+  if (p->h2d_stream) cudaStreamDestroy(p->h2d_stream);
+  if (p->d2h_stream) cudaStreamDestroy(p->d2h_stream);
   for (int ph = 0; ph < 8; ph++)
     for (auto &e : p->timer.ev[ph]) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
   cudaGetLastError();
@@ -404,6 +406,10 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     if (value < 0 || value > 2) { set_error("fft_path = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->fft_path = (int)value; return DFT_OK;
   }
+  if (!strcmp(key, "host_groups")) {
+    if (value < 1 || value > 64) { set_error("host_groups = %lld outside 1..64", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->host_groups = (int)value; return DFT_OK;
+  }
   if (!strcmp(key, "gemm_3m")) {
     if (value < 0 || value > 1) { set_error("gemm_3m = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->gemm_3m = (int)value; return DFT_OK;
@@ -444,11 +450,51 @@ int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int
     p->stage_bytes = bytes;
   }
   cudaStream_t st = p->host_stream;
-  DFT_CUDA_CHECK(cudaMemcpyAsync(p->d_stage_in, psi_host, bytes, cudaMemcpyHostToDevice, st));
-  int rc = apply_impl(p, p->d_stage_in, p->d_stage_out, nband, st);
+  // One k-point: the band block is cut into groups that go through the whole path one after the other, so
+  // that the host->device copy of group g+1 and the device->host copy of group g-1 overlap the kernels of
+  // group g (three streams, events between them).  Several k-points: one copy in, one pass, one copy out.
+  int ngroup = 1;
+  if (p->nkpt == 1 && p->host_groups > 1 && nband >= 2 * 64) {
+    ngroup = p->host_groups;
+    if (nband / ngroup < 64) ngroup = nband / 64;
+  }
+  if (ngroup <= 1) {
+    DFT_CUDA_CHECK(cudaMemcpyAsync(p->d_stage_in, psi_host, bytes, cudaMemcpyHostToDevice, st));
+    int rc = apply_impl(p, p->d_stage_in, p->d_stage_out, nband, st);
+    if (rc) return rc;
+    DFT_CUDA_CHECK(cudaMemcpyAsync(hpsi_host, p->d_stage_out, bytes, cudaMemcpyDeviceToHost, st));
+    DFT_CUDA_CHECK(cudaStreamSynchronize(st));
+    return DFT_OK;
+  }
+  if (!p->h2d_stream) DFT_CUDA_CHECK(cudaStreamCreateWithFlags(&p->h2d_stream, cudaStreamNonBlocking));
+  if (!p->d2h_stream) DFT_CUDA_CHECK(cudaStreamCreateWithFlags(&p->d2h_stream, cudaStreamNonBlocking));
+  const int per = ((nband + ngroup - 1) / ngroup + 63) / 64 * 64;   // whole GEMM band tiles per group
+  std::vector<cudaEvent_t> ev;
+  int64_t launches = 0;
+  int rc = DFT_OK;
+  for (int b0 = 0; b0 < nband && rc == DFT_OK; b0 += per) {
+    const int nb = nband - b0 < per ? nband - b0 : per;
+    const size_t off = (size_t)b0 * p->mpw * 2, gbytes = (size_t)nb * p->mpw * 16;
+    cudaEvent_t in_done, k_done;
+    if (cudaEventCreateWithFlags(&in_done, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&k_done, cudaEventDisableTiming) != cudaSuccess) { set_error("cudaEventCreate failed"); rc = DFT_ERR_CUDA; break; }
+    ev.push_back(in_done); ev.push_back(k_done);
+    if (cudaMemcpyAsync(p->d_stage_in + off, psi_host + off, gbytes, cudaMemcpyHostToDevice, p->h2d_stream) != cudaSuccess ||
+        cudaEventRecord(in_done, p->h2d_stream) != cudaSuccess || cudaStreamWaitEvent(st, in_done, 0) != cudaSuccess) {
+      set_error("host->device copy of bands %d.. failed: %s", b0, cudaGetErrorString(cudaGetLastError())); rc = DFT_ERR_CUDA; break;
+    }
+    if ((rc = apply_impl(p, p->d_stage_in + off, p->d_stage_out + off, nb, st))) break;
+    launches += p->last_launches;
+    if (cudaEventRecord(k_done, st) != cudaSuccess || cudaStreamWaitEvent(p->d2h_stream, k_done, 0) != cudaSuccess ||
+        cudaMemcpyAsync(hpsi_host + off, p->d_stage_out + off, gbytes, cudaMemcpyDeviceToHost, p->d2h_stream) != cudaSuccess) {
+      set_error("device->host copy of bands %d.. failed: %s", b0, cudaGetErrorString(cudaGetLastError())); rc = DFT_ERR_CUDA; break;
+    }
+  }
+  cudaError_t e1 = cudaStreamSynchronize(p->h2d_stream), e2 = cudaStreamSynchronize(st), e3 = cudaStreamSynchronize(p->d2h_stream);
+  for (cudaEvent_t e : ev) cudaEventDestroy(e);
+  p->last_launches = launches;
   if (rc) return rc;
-  DFT_CUDA_CHECK(cudaMemcpyAsync(hpsi_host, p->d_stage_out, bytes, cudaMemcpyDeviceToHost, st));
-  DFT_CUDA_CHECK(cudaStreamSynchronize(st));
+  if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) { set_error("dft_apply_h_host: stream synchronisation failed"); return DFT_ERR_CUDA; }
   return DFT_OK;
   DFT_GUARD_END
 }

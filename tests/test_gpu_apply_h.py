@@ -137,6 +137,20 @@ def test_set_dij_and_user_workspace_and_host_api():
     plan.destroy()
 
 
+def test_host_api_band_groups():
+    """dft_apply_h_host cuts one k-point's bands into groups whose copies overlap the neighbours' kernels;
+    the result must not depend on the grouping."""
+    cfg, plan, sph = _setup("c1m", nband=200)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    ref = oracle_apply(cfg, sph, psi)
+    for groups in (3, 1, 4):
+        plan.set_option("host_groups", groups)
+        got = plan.apply_h_host(psi)
+        assert band_rel_err(got, ref) <= TOL, groups
+        assert plan.last_launches() == 8 * (2 if groups > 1 else 1)   # 200 bands -> groups of 128 and 72
+    plan.destroy()
+
+
 def test_c1_full():
     cfg, plan, sph = _setup("c1")
     psi = synth.gen_psi(cfg, [s[2] for s in sph])

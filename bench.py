@@ -245,8 +245,15 @@ def main():
         v["frac"] = v["achieved"] / v["peak"]
     dom = max(per_kernel, key=lambda k: per_kernel[k]["ms_per_step"])
     d = per_kernel[dom]
+    traffic = None      # ncu dram bytes per launch of that kernel, from the committed capture summary (full-size runs only)
+    try:
+        if not args.nband and world == 1:
+            with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as f:
+                traffic = json.load(f).get(args.config, {}).get(dom)
+    except Exception:
+        traffic = None
     roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],
-                "frac": d["frac"], "traffic": None,
+                "frac": d["frac"], "traffic": traffic,
                 "peak_source": ("FP64 DMMA: 148 SM x 4 x 512 flop / 16 clk x 1.965 GHz (microbenchmark 37.06), "
                                 "DESIGN.md 8" if d["bound"] == "tensor" else hbm_src),
                 "share_of_step": d["ms_per_step"] / ms_step}

@@ -121,6 +121,19 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value);
  * called (unless the local term is switched off with "terms").                                   */
 int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);
 
+/* PAW overlap coefficients s^a_ij, HOST [natom][nlmn_max][nlmn_max] real symmetric (zero after
+ * dft_plan_create): "the overlap operator S ... has the same structure" as Eq. 26 (PAPER.md :473).  */
+int dft_set_sij(dft_plan *p, const double *sij);
+
+/* spsi = S psi = psi + sum_a sum_ij |p_a,i> s^a_ij <p_a,j|psi> (PAPER.md :473), same layouts, stream and
+ * pad-entry rules as dft_apply_h: GEMM-1, s_ij, GEMM-2 with a unit diagonal in its epilogue.        */
+int dft_apply_s(dft_plan *p, const double *psi, double *spsi, int32_t nband, void *stream);
+
+/* cprj = <p_a,i|psi_n> (PAPER.md :477 "coefficients c_a,i,n,k ... cprj"): DEVICE output
+ * [nkpt][nband][nproj] complex128, projector index fastest, atoms in order, i = 0..nlmn-1 inside an
+ * atom.  GEMM-1 and the fixed-order split-K reduction only; enqueues on `stream`.                 */
+int dft_get_cprj(dft_plan *p, const double *psi, double *cprj, int32_t nband, void *stream);
+
 /* Same, with HOST psi/hpsi (pageable or pinned): copies psi to the device in band blocks, applies
  * H, copies the result back, and returns after the last copy has completed.                      */
 int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int32_t nband);

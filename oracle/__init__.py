@@ -188,6 +188,23 @@ def nonlocal_apply(cfg, ik, kg, psi, dij=None, want_cprj=False):
     return (out, cp) if want_cprj else out
 
 
+def cprj(cfg, ik, kg, psi):
+    """<p_a,i|psi_b> (PAPER.md :477 "coefficients c_a,i,n,k"), [nproj][nband] complex: step 1 of Eq. 26 (:470),
+    as the streamed loops of orc_nonlocal_apply compute it."""
+    return nonlocal_apply(cfg, ik, kg, psi, dij=np.zeros_like(_f64(cfg["dij"])), want_cprj=True)[1]
+
+
+def apply_s(cfg, ik, kg, psi, sij):
+    """S psi = psi + sum_a sum_ij |p_a,i> s^a_ij <p_a,j|psi>: PAPER.md :473, "the overlap operator S ... has the same
+    structure" as the non-local operator of Eq. 26, so it is the definition's unit term plus orc_nonlocal_apply with
+    s_ij in the place of D_ij.  psi [nband][ld >= npw]; columns >= npw are returned as 0."""
+    psi = np.ascontiguousarray(psi, np.complex128)
+    out = nonlocal_apply(cfg, ik, kg, psi, dij=sij)
+    npw = len(kg)
+    out[:, :npw] += psi[:, :npw]
+    return out
+
+
 # ---------------------------------------------------------------- whole operator
 KIN, LOC, NL, ALL = 1, 2, 4, 7
 

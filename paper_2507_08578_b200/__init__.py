@@ -32,6 +32,7 @@ PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather
 
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_set_dij",
+           "dft_set_sij", "dft_apply_s", "dft_get_cprj",
            "dft_set_vloc", "dft_set_workspace", "dft_plan_set_option", "dft_apply_h", "dft_apply_h_host",
            "dft_plan_last_launches", "dft_plan_set_timing", "dft_plan_phase_ms", "dft_plan_destroy", "dft_last_error")
 
@@ -78,6 +79,9 @@ def lib():
     L.dft_plan_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
     L.dft_apply_h.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_apply_h_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
+    L.dft_set_sij.argtypes = [C.c_void_p, _dp]
+    L.dft_apply_s.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    L.dft_get_cprj.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_plan_set_timing.argtypes = [C.c_void_p, C.c_int32]
     L.dft_plan_phase_ms.argtypes = [C.c_void_p, C.c_int32, _dp, C.POINTER(C.c_int64)]
     L.dft_plan_destroy.argtypes = [C.c_void_p]
@@ -178,6 +182,18 @@ def dft_apply_h(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream=0):
     _check(lib().dft_apply_h(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream))
 
 
+def dft_set_sij(plan, sij):
+    _check(lib().dft_set_sij(plan, _d(_f64(sij))))
+
+
+def dft_apply_s(plan, psi_dev_ptr, spsi_dev_ptr, nband, stream=0):
+    _check(lib().dft_apply_s(plan, psi_dev_ptr, spsi_dev_ptr, nband, stream))
+
+
+def dft_get_cprj(plan, psi_dev_ptr, cprj_dev_ptr, nband, stream=0):
+    _check(lib().dft_get_cprj(plan, psi_dev_ptr, cprj_dev_ptr, nband, stream))
+
+
 def dft_apply_h_host(plan, psi_host_ptr, hpsi_host_ptr, nband):
     _check(lib().dft_apply_h_host(plan, psi_host_ptr, hpsi_host_ptr, nband))
 
@@ -252,6 +268,29 @@ class Plan:
         assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.is_contiguous() and hpsi.shape == psi.shape
         dft_apply_h(self.h, psi.data_ptr(), hpsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
         return hpsi
+
+    def set_sij(self, sij):
+        dft_set_sij(self.h, sij)
+
+    def apply_s(self, psi, spsi=None):
+        """S psi (PAW overlap); same tensors as apply_h."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.shape[-1] == self.mpw
+        nband = psi.numel() // (self.nkpt * self.mpw) if self.mpw else 0
+        if spsi is None:
+            spsi = torch.empty_like(psi)
+        assert spsi.is_cuda and spsi.dtype == torch.complex128 and spsi.is_contiguous() and spsi.shape == psi.shape
+        dft_apply_s(self.h, psi.data_ptr(), spsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
+        return spsi
+
+    def get_cprj(self, psi):
+        """<p|psi> as a torch complex128 CUDA tensor [nkpt][nband][nproj]."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.shape[-1] == self.mpw
+        nband = psi.numel() // (self.nkpt * self.mpw) if self.mpw else 0
+        out = torch.zeros((self.nkpt, nband, self.nproj), dtype=torch.complex128, device=psi.device)
+        dft_get_cprj(self.h, psi.data_ptr(), out.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
+        return out
 
     def apply_h_host(self, psi, hpsi=None):
         """psi: numpy complex128 array or CPU torch tensor (pinned or not); returns the same kind."""

@@ -96,6 +96,9 @@ struct dft_plan {
   int32_t *d_atom_first = nullptr, *d_nq = nullptr;
   double *d_dq = nullptr, *d_xred = nullptr;
   double *d_dij = nullptr;                           // [natom][lmax][lmax]
+  double *d_sij = nullptr;                           // [natom][lmax][lmax] overlap coefficients s_ij (zero until dft_set_sij)
+  double *d_ones = nullptr;                          // [mpw] of 1.0: the unit diagonal of S in GEMM-2's epilogue
+  const double **d_oneptr = nullptr;                 // [nkpt] device pointers to d_ones
   double *d_ptab = nullptr;                          // [nkpt][nproj][mpw] complex, zero padded beyond npw_k
   int32_t *d_npw = nullptr;                          // [nkpt]
   const double **d_kinptr = nullptr;                 // [nkpt] device pointers to kin of each k-point
@@ -156,7 +159,8 @@ int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, 
 // --- nonlocal.cu (K3) ---------------------------------------------------------------------
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi
 int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin,
-                   bool with_nl, cudaStream_t st);
+                   bool with_nl, cudaStream_t st, const double *dmat = nullptr, const double *const *diag = nullptr,
+                   double *cprj_out = nullptr);
 
 // --- timing hooks ------------------------------------------------------------------------------
 void phase_begin(dft_plan *p, int phase, cudaStream_t st);

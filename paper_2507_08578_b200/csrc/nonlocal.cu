@@ -219,8 +219,12 @@ __global__ void dij_kernel(const double2 *__restrict__ part, double2 *__restrict
     }
     c[jj] = make_double2(sr, si);
   }
-  const double *D = dij + (size_t)a * lmax * lmax;
   double2 *dst = cpr + ((size_t)ik * nband + b) * nproj + first;
+  if (!dij) {   // no D: the reduced projections <p|psi> themselves (dft_get_cprj)
+    for (int ii = 0; ii < nl; ii++) dst[ii] = c[ii];
+    return;
+  }
+  const double *D = dij + (size_t)a * lmax * lmax;
   for (int ii = 0; ii < nl; ii++) {
     double sr = 0.0, si = 0.0;
     for (int jj = 0; jj < nl; jj++) { double d = D[ii * lmax + jj]; sr += d * c[jj].x; si += d * c[jj].y; }
@@ -558,9 +562,13 @@ static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
   return best;
 }
 
+// dmat: per-atom matrices applied between the GEMMs (null = the plan's D_ij); diag: per-k-point device pointers to the
+// diagonal multiplying psi in the epilogue (null = the kinetic energies); cprj_out (device, [nkpt][nband][nproj]
+// complex): if given, only GEMM-1 and the split-K reduction run and <p|psi> is written there.
 int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
-                   cudaStream_t st) {
+                   cudaStream_t st, const double *dmat, const double *const *diag, double *cprj_out) {
   if (p->mpw == 0 || nband == 0) return DFT_OK;
+  if (cprj_out && p->nproj == 0) return DFT_OK;
   if (p->nproj == 0) with_nl = false;
   if (!with_nl && !with_kin && accumulate) return DFT_OK;
   if (!g_nl_attr) {
@@ -571,7 +579,8 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     g_nl_attr = true;
   }
   const int32_t *d_npw = p->d_npw;
-  const double *const *d_kin = p->d_kinptr;
+  const double *const *d_kin = diag ? diag : p->d_kinptr;
+  if (!dmat) dmat = p->d_dij;
   int rc;
   const double2 *cpsi = reinterpret_cast<const double2 *>(psi);
   double2 *chpsi = reinterpret_cast<double2 *>(hpsi);
@@ -633,11 +642,12 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   DFT_CUDA_CHECK(cudaGetLastError());
   // ---- D_ij
   phase_begin(p, 6, st);
-  dij_kernel<<<dim3((nband + 127) / 128, p->natom, nkpt), 128, 0, st>>>(q1.part, reinterpret_cast<double2 *>(p->d_cprj), p->d_dij,
-                                                                        p->d_typat, p->d_nlmn, p->d_atom_first, p->natom, p->lmax,
-                                                                        nproj, nband, ns);
+  dij_kernel<<<dim3((nband + 127) / 128, p->natom, nkpt), 128, 0, st>>>(
+      q1.part, reinterpret_cast<double2 *>(cprj_out ? cprj_out : p->d_cprj), cprj_out ? nullptr : dmat, p->d_typat, p->d_nlmn,
+      p->d_atom_first, p->natom, p->lmax, nproj, nband, ns);
   phase_end(p, 6, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
+  if (cprj_out) return DFT_OK;
   // ---- GEMM-2
   Gemm2Params q2;
   q2.nproj = nproj; q2.nband = nband; q2.mpw = mpw; q2.nslab = (nproj + 7) / 8;

@@ -59,7 +59,7 @@ static void destroy_plan(dft_plan *p) {
   for (auto &k : p->kp) free_kpoint(k);
   cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
   cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
-  cudaFree(p->d_dij); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
@@ -208,6 +208,14 @@ static int create_impl(dft_plan *p, const double rprimd[9], int32_t nkpt, const 
   if (ndij) {
     if (!dij) { set_error("dij is NULL"); return DFT_ERR_INVALID_ARG; }
     if ((rc = to_device(&p->d_dij, dij, ndij))) return rc;
+    std::vector<double> zero(ndij, 0.0);
+    if ((rc = to_device(&p->d_sij, zero.data(), ndij))) return rc;
+  }
+  if (p->mpw > 0) {   // unit diagonal of the overlap operator, addressed like the kinetic energies
+    std::vector<double> ones((size_t)p->mpw, 1.0);
+    if ((rc = to_device(&p->d_ones, ones.data(), ones.size()))) return rc;
+    std::vector<const double *> optr((size_t)nkpt, p->d_ones);
+    if ((rc = to_device((const double ***)&p->d_oneptr, optr.data(), nkpt))) return rc;
   }
   size_t tab = (size_t)nkpt * p->nproj * p->mpw * 16;
   if (tab) {
@@ -429,6 +437,43 @@ int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, voi
   if (nband > 0 && p->mpw > 0 && (!psi || !hpsi)) { set_error("null psi/hpsi"); return DFT_ERR_INVALID_ARG; }
   if (((uintptr_t)psi & 15) || ((uintptr_t)hpsi & 15)) { set_error("psi/hpsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
   return apply_impl(p, psi, hpsi, nband, (cudaStream_t)stream);
+  DFT_GUARD_END
+}
+
+int dft_set_sij(dft_plan *p, const double *sij) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  size_t n = (size_t)p->natom * p->lmax * p->lmax;
+  if (n == 0) return DFT_OK;
+  if (!sij) { set_error("sij is NULL"); return DFT_ERR_INVALID_ARG; }
+  DFT_CUDA_CHECK(cudaMemcpy(p->d_sij, sij, n * sizeof(double), cudaMemcpyHostToDevice));
+  return DFT_OK;
+}
+
+int dft_apply_s(dft_plan *p, const double *psi, double *spsi, int32_t nband, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  if (nband > 0 && p->mpw > 0 && (!psi || !spsi)) { set_error("null psi/spsi"); return DFT_ERR_INVALID_ARG; }
+  if (((uintptr_t)psi & 15) || ((uintptr_t)spsi & 15)) { set_error("psi/spsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  p->last_launches = 0;
+  if (nband == 0 || p->mpw == 0 || p->nkpt == 0) return DFT_OK;
+  // S psi = psi + sum_a sum_ij |p_a,i> s^a_ij <p_a,j|psi>: the non-local path with s_ij for D_ij and a unit diagonal
+  bool ragged = false;
+  for (int ik = 0; ik < p->nkpt; ik++) ragged |= p->kp[ik].npw < p->mpw;
+  if (ragged) DFT_CUDA_CHECK(cudaMemsetAsync(spsi, 0, (size_t)p->nkpt * nband * p->mpw * 16, (cudaStream_t)stream));   // pad entries = 0
+  return nonlocal_apply(p, psi, spsi, nband, false, true, p->nproj > 0, (cudaStream_t)stream, p->d_sij, p->d_oneptr, nullptr);
+  DFT_GUARD_END
+}
+
+int dft_get_cprj(dft_plan *p, const double *psi, double *cprj, int32_t nband, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  p->last_launches = 0;
+  if (nband == 0 || p->mpw == 0 || p->nkpt == 0 || p->nproj == 0) return DFT_OK;
+  if (!psi || !cprj) { set_error("null psi/cprj"); return DFT_ERR_INVALID_ARG; }
+  if (((uintptr_t)psi & 15) || ((uintptr_t)cprj & 15)) { set_error("psi/cprj must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  return nonlocal_apply(p, psi, nullptr, nband, false, false, true, (cudaStream_t)stream, nullptr, nullptr, cprj);
   DFT_GUARD_END
 }
 

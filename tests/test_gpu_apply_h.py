@@ -137,6 +137,35 @@ def test_set_dij_and_user_workspace_and_host_api():
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c1m", "c4m", "aniso", "c3k2"])
+def test_overlap_operator_and_cprj(name):
+    """dft_apply_s (S psi, PAPER.md :473) and dft_get_cprj (<p|psi>, :477) against the oracle, both GEMM variants."""
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    rng = np.random.default_rng(3)
+    sij = rng.standard_normal(cfg["dij"].shape) * 0.3
+    sij = 0.5 * (sij + sij.transpose(0, 2, 1))
+    tpsi = torch.as_tensor(psi, device="cuda")
+    ident = plan.apply_s(tpsi).cpu().numpy()                  # s_ij = 0 after plan creation: S = 1 on the sphere
+    for ik, (kg, ig, kin) in enumerate(sph):
+        assert np.array_equal(ident[ik][:, :len(ig)], psi[ik][:, :len(ig)]) and np.all(ident[ik][:, len(ig):] == 0)
+    plan.set_sij(sij)
+    for g3 in (1, 0):
+        plan.set_option("gemm_3m", g3)
+        got = plan.apply_s(tpsi).cpu().numpy()
+        cp = plan.get_cprj(tpsi).cpu().numpy()
+        for ik, (kg, ig, kin) in enumerate(sph):
+            ref = oracle.apply_s(cfg, ik, kg, psi[ik], sij)
+            err = float(np.max(np.linalg.norm(got[ik] - ref, axis=1) / np.linalg.norm(ref, axis=1)))
+            assert err <= TOL, "%s S psi gemm_3m=%d k=%d: %.3e" % (name, g3, ik, err)
+            assert np.all(got[ik][:, len(ig):] == 0)
+            cref = oracle.cprj(cfg, ik, kg, psi[ik][:, :len(ig)]).T          # [nband][nproj]
+            cerr = float(np.max(np.linalg.norm(cp[ik] - cref, axis=1) / np.linalg.norm(cref, axis=1)))
+            assert cerr <= TOL, "%s cprj gemm_3m=%d k=%d: %.3e" % (name, g3, ik, cerr)
+    assert plan.last_launches() == 2
+    plan.destroy()
+
+
 def test_host_api_band_groups():
     """dft_apply_h_host cuts one k-point's bands into groups whose copies overlap the neighbours' kernels;
     the result must not depend on the grouping."""

@@ -114,3 +114,37 @@ def test_single_s_projector_rank_and_zero_d():
     assert np.linalg.norm(out) < 1e-12 * np.linalg.norm(x)                     # rank(V_nl) <= nproj
     assert np.linalg.matrix_rank(oracle.dense_h(c, 0, kg, kin, terms=oracle.NL), tol=1e-10) <= c["nproj"]
     assert np.all(oracle.nonlocal_apply(c, 0, kg, rand_c((2, len(kg)), 3), dij=np.zeros_like(c["dij"])) == 0)
+
+
+def test_overlap_operator_pins():
+    """S = 1 + sum |p> s <p| (PAPER.md :473): numpy reduction I + P^T s conj(P), closed form on one projector,
+    Hermiticity, s = 0 -> identity, and pad columns returned as zero."""
+    for name in ("c0", "aniso"):
+        c = config(name); kg, ig, kin = sphere(name)
+        npw = len(kg)
+        rng = np.random.default_rng(5)
+        sij = rng.standard_normal(c["dij"].shape) * 0.3
+        sij = 0.5 * (sij + sij.transpose(0, 2, 1))
+        psi = rand_c((3, npw + 2), 11)
+        out = oracle.apply_s(c, 0, kg, psi, sij)
+        P = oracle.projector_table(c, 0, kg)
+        Sm = np.zeros((c["nproj"], c["nproj"]))
+        r = 0
+        for a in range(c["natom"]):
+            nl = c["types"][c["typat"][a]]["nlmn"]
+            Sm[r:r + nl, r:r + nl] = sij[a, :nl, :nl]; r += nl
+        x = psi[:, :npw]
+        ref = x + (P.T @ (Sm @ (P.conj() @ x.T))).T
+        assert rel_err(out[:, :npw], ref) < 1e-13
+        assert np.all(out[:, npw:] == 0)
+        phi = rand_c((1, npw), 12)
+        sphi = oracle.apply_s(c, 0, kg, phi, sij)
+        lhs = np.vdot(phi[0], out[0, :npw]); rhs = np.vdot(sphi[0], x[0])
+        assert abs(lhs - rhs) < 1e-12 * abs(lhs)                              # <phi|S psi> = <S phi|psi>
+        assert rel_err(oracle.apply_s(c, 0, kg, x, np.zeros_like(sij)), x) == 0.0
+        assert rel_err(oracle.cprj(c, 0, kg, x).T, (P.conj() @ x.T).T) < 1e-13
+    c = dict(config("c0")); kg, ig, kin = sphere("c0")
+    c["natom"] = 1; c["xred"] = np.zeros((1, 3)); c["typat"] = np.zeros(1, np.int32); c["nproj"] = 8
+    s1 = np.zeros((1, 8, 8)); s1[0, 0, 0] = 0.4
+    p = oracle.projector_table(c, 0, kg)[0]
+    np.testing.assert_allclose(oracle.apply_s(c, 0, kg, p[None], s1)[0], (1 + 0.4 * np.vdot(p, p).real) * p, rtol=1e-13)

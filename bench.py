@@ -165,6 +165,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (experiments only)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the e2e leg (experiments only)")
     ap.add_argument("--ref-bands", type=int, default=0)
+    ap.add_argument("--cheb-degree", type=int, default=10, help="degree of the Chebyshev-filter context figure (0 = skip)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -275,6 +276,25 @@ def main():
                        "l2": "inputs larger than L2 between iterations (psi+hpsi %.2f GB, projector table %.2f GB)" % (
                            2 * psi.numel() * 16 / 1e9, plan.nkpt * plan.nproj * plan.mpw * 16 / 1e9)},
             "clocks": clocks, "gpu_launches": launches, "roofline": roofline, "roofline_path": path}
+
+    # ---- context figure: Chebyshev filter of degree mdeg_filter = 10 (PAPER.md :489), i.e. 10
+    #      chained H applications with the recurrence fused into GEMM-2's epilogue; not part of `value`
+    if args.cheb_degree > 0 and world == 1:
+        work = torch.empty(2 * psi.numel(), dtype=psi.dtype, device="cuda")
+        tmp = psi.clone()
+        kmax = max(float(k.max()) for k in kin_list)
+        cen, half = 0.5 * kmax + 1.0, 0.5 * kmax + 0.5
+        plan.chebyshev_filter(tmp, 1, cen, half, work)
+        torch.cuda.synchronize()
+        c0 = torch.cuda.Event(enable_timing=True); c1 = torch.cuda.Event(enable_timing=True)
+        c0.record(); plan.chebyshev_filter(tmp, args.cheb_degree, cen, half, work); c1.record()
+        torch.cuda.synchronize()
+        cms = c0.elapsed_time(c1)
+        line["chebyshev_filter"] = {"degree": args.cheb_degree, "ms": cms, "ms_per_h_application": cms / args.cheb_degree,
+                                    "bands_per_s_per_h_application": units / (cms / args.cheb_degree * 1e-3),
+                                    "api": "dft_chebyshev_filter (in place, 2 psi-sized work arrays)"}
+        del work, tmp
+        torch.cuda.empty_cache()
 
     # ---- e2e: same metric through dft_apply_h_host, host<->device copies inside the timed region
     if not args.no_e2e:

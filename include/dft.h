@@ -134,6 +134,18 @@ int dft_apply_s(dft_plan *p, const double *psi, double *spsi, int32_t nband, voi
  * atom.  GEMM-1 and the fixed-order split-K reduction only; enqueues on `stream`.                 */
 int dft_get_cprj(dft_plan *p, const double *psi, double *cprj, int32_t nband, void *stream);
 
+/* Chebyshev filter (PAPER.md :458 "Chebyshev filtering algorithm ... filters the spectrum of the Hamiltonian",
+ * :489 "mdeg_filter 10"; the paper prints no formula, this is the textbook three-term recurrence):
+ *   T_0 = psi,  T_1 = (H - center) T_0 / halfwidth,  T_{j+1} = 2 (H - center) T_j / halfwidth - T_{j-1},
+ * psi := T_degree, i.e. the Chebyshev polynomial of the first kind of (H - center)/halfwidth applied to psi
+ * (center, halfwidth: centre and half-width of the part of the spectrum to damp, Hartree; halfwidth > 0).
+ * psi: DEVICE in/out, layout of dft_apply_h; work: DEVICE scratch of TWO psi-sized arrays
+ * (2 * nkpt*nband*mpw complex128, 16-byte aligned), contents undefined afterwards.  `degree` applications
+ * of H; the recurrence combination is done where GEMM-2's epilogue stores H T_j (no extra passes).
+ * Pad entries ipw >= npw_k of the result are 0.  Enqueues on `stream`, no host synchronisation.     */
+int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, int32_t degree, double center,
+                         double halfwidth, void *stream);
+
 /* Same, with HOST psi/hpsi (pageable or pinned): copies psi to the device in band blocks, applies
  * H, copies the result back, and returns after the last copy has completed.                      */
 int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int32_t nband);

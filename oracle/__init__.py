@@ -222,6 +222,23 @@ def apply_h(cfg, ik, kg, igfft, kin, psi, method=2, terms=ALL, vloc=None, dij=No
     return out
 
 
+def chebyshev_filter(cfg, ik, kg, igfft, kin, psi, degree, center, halfwidth, method=2, terms=ALL, vloc=None, dij=None):
+    """T_degree((H - center)/halfwidth) psi by the three-term recurrence, one apply_h per degree (PAPER.md :458
+    "Chebyshev filtering algorithm", :489 mdeg_filter; the paper prints no formula -- DESIGN.md reading 21):
+    T_0 = psi, T_1 = (H - c) T_0 / e, T_{j+1} = 2 (H - c) T_j / e - T_{j-1}."""
+    psi = np.ascontiguousarray(psi, np.complex128)
+    H = lambda x: apply_h(cfg, ik, kg, igfft, kin, x, method=method, terms=terms, vloc=vloc, dij=dij)
+    npw = len(kg)
+    t_prev = psi.copy(); t_prev[:, npw:] = 0
+    if degree == 0:
+        return psi.copy()
+    t_cur = (H(t_prev) - center * t_prev) / halfwidth
+    for _ in range(1, degree):
+        t_next = 2.0 * (H(t_cur) - center * t_cur) / halfwidth - t_prev
+        t_prev, t_cur = t_cur, t_next
+    return t_cur
+
+
 def dense_h(cfg, ik, kg, kin, terms=ALL, vloc=None, dij=None):
     """T0: explicit H[npw][npw] complex128 in the plane-wave basis."""
     P = _Proj(cfg, ik); kg = _i32(kg); kin = _f64(kin)

@@ -156,11 +156,18 @@ bool fft2_pair(int n, int *r1, int *r2);
 int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, void *T1, void *T2, int64_t t1_band,
                 int64_t t2_band, int nb, cudaStream_t st);
 
+// Optional combination applied where H psi is stored (GEMM-2 epilogue): out = sh * (H psi) + sy * psi + sx * xprev.
+// One step of a three-term recurrence in H (Chebyshev filter, PAPER.md :458) without extra passes over psi-sized arrays.
+struct Recurrence {
+  double sh, sy, sx;
+  const double *xprev;   // device [nkpt][nband][mpw] complex; read only where sx != 0
+};
+
 // --- nonlocal.cu (K3) ---------------------------------------------------------------------
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi
 int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin,
                    bool with_nl, cudaStream_t st, const double *dmat = nullptr, const double *const *diag = nullptr,
-                   double *cprj_out = nullptr);
+                   double *cprj_out = nullptr, const Recurrence *rec = nullptr);
 
 // --- timing hooks ------------------------------------------------------------------------------
 void phase_begin(dft_plan *p, int phase, cudaStream_t st);

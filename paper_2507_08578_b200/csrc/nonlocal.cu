@@ -55,6 +55,10 @@ struct Gemm2Params {
   const int32_t *npw;     // [nkpt] device
   const double *const *kin;   // [nkpt] device pointers
   const double2 *psi; double2 *hpsi;   // [nkpt][nband][mpw]
+  // optional recurrence combination of the epilogue (Chebyshev filter): out = sh * (H psi) + sy * psi + sx * xprev
+  int cheb;
+  double sh, sy, sx;
+  const double2 *xprev;                // [nkpt][nband][mpw], read only where sx != 0
 };
 
 // The MMA main loop shared by both GEMMs.  MODE 1: acc += conj(A) B (GEMM-1); MODE 2: acc += A B.
@@ -290,6 +294,10 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
         double2 r = make_double2(cre[mb][nb][e], cim[mb][nb][e]);
         if (Q.with_kin) { double2 x = psi[off]; r.x += kg * x.x; r.y += kg * x.y; }
         if (Q.accumulate) { double2 h = hpsi[off]; r.x += h.x; r.y += h.y; }
+        if (Q.cheb) {
+          double2 y = psi[off], xp = Q.sx != 0.0 ? Q.xprev[(size_t)ik * Q.nband * Q.mpw + off] : make_double2(0.0, 0.0);
+          r.x = Q.sh * r.x + Q.sy * y.x + Q.sx * xp.x; r.y = Q.sh * r.y + Q.sy * y.y + Q.sx * xp.y;
+        }
         hpsi[off] = r;
       }
     }
@@ -488,21 +496,25 @@ gemm2_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant_
   constexpr int U = 6, NQ = (NL_BN + 2) / 3;
 #pragma unroll 1
   for (int q0 = 0; q0 < NQ; q0 += U) {
-    double2 x[U], h[U];
+    double2 x[U], h[U], xp[U];
     bool ok[U];
 #pragma unroll
     for (int u = 0; u < U; u++) {
       const int c = c0 + 3 * (q0 + u), b = tn * NL_BN + c;
       ok[u] = gok && c < NL_BN && b < Q.nband;
       const size_t off = base + (size_t)b * Q.mpw;
-      x[u] = (ok[u] && Q.with_kin) ? Q.psi[off] : make_double2(0.0, 0.0);
+      x[u] = (ok[u] && (Q.with_kin || Q.cheb)) ? Q.psi[off] : make_double2(0.0, 0.0);
       h[u] = (ok[u] && Q.accumulate) ? Q.hpsi[off] : make_double2(0.0, 0.0);
+      xp[u] = (ok[u] && Q.cheb && Q.sx != 0.0) ? Q.xprev[off] : make_double2(0.0, 0.0);
     }
 #pragma unroll
     for (int u = 0; u < U; u++) {
       const int c = c0 + 3 * (q0 + u), b = tn * NL_BN + c;
       if (ok[u]) {
         double2 v = make_double2(Xre[(size_t)r * NL3_XS + c] + kg * x[u].x + h[u].x, Xim[(size_t)r * NL3_XS + c] + kg * x[u].y + h[u].y);
+        if (Q.cheb) {
+          v.x = Q.sh * v.x + Q.sy * x[u].x + Q.sx * xp[u].x; v.y = Q.sh * v.y + Q.sy * x[u].y + Q.sx * xp[u].y;
+        }
         Q.hpsi[base + (size_t)b * Q.mpw] = v;
       }
     }
@@ -534,7 +546,8 @@ static int make_map(dft_plan *p, CUtensorMap *m, const void *base, uint64_t d0, 
 }
 
 __global__ void kin_only_kernel(const double2 *__restrict__ psi, double2 *__restrict__ hpsi, const double *const *kin,
-                                const int32_t *npw, int nband, int mpw, int accumulate, int with_kin) {
+                                const int32_t *npw, int nband, int mpw, int accumulate, int with_kin, int cheb, double sh,
+                                double sy, double sx, const double2 *__restrict__ xprev) {
   int ik = blockIdx.z, b = blockIdx.y;
   const double *k = kin[ik];
   int n = npw[ik];
@@ -543,6 +556,10 @@ __global__ void kin_only_kernel(const double2 *__restrict__ psi, double2 *__rest
     double2 r = make_double2(0.0, 0.0);
     if (with_kin) { double2 x = psi[row + g]; double kg = k[g]; r.x = kg * x.x; r.y = kg * x.y; }
     if (accumulate) { double2 h = hpsi[row + g]; r.x += h.x; r.y += h.y; }
+    if (cheb) {
+      double2 y = psi[row + g], xp = sx != 0.0 ? xprev[row + g] : make_double2(0.0, 0.0);
+      r.x = sh * r.x + sy * y.x + sx * xp.x; r.y = sh * r.y + sy * y.y + sx * xp.y;
+    }
     hpsi[row + g] = r;
   }
 }
@@ -566,11 +583,11 @@ static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
 // diagonal multiplying psi in the epilogue (null = the kinetic energies); cprj_out (device, [nkpt][nband][nproj]
 // complex): if given, only GEMM-1 and the split-K reduction run and <p|psi> is written there.
 int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
-                   cudaStream_t st, const double *dmat, const double *const *diag, double *cprj_out) {
+                   cudaStream_t st, const double *dmat, const double *const *diag, double *cprj_out, const Recurrence *rec) {
   if (p->mpw == 0 || nband == 0) return DFT_OK;
   if (cprj_out && p->nproj == 0) return DFT_OK;
   if (p->nproj == 0) with_nl = false;
-  if (!with_nl && !with_kin && accumulate) return DFT_OK;
+  if (!with_nl && !with_kin && accumulate && !rec) return DFT_OK;
   if (!g_nl_attr) {
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
@@ -587,7 +604,9 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   if (!with_nl) {
     dim3 grid((p->mpw + 255) / 256 < 64 ? (p->mpw + 255) / 256 : 64, nband, p->nkpt);
     phase_begin(p, 7, st);
-    kin_only_kernel<<<grid, 256, 0, st>>>(cpsi, chpsi, d_kin, d_npw, nband, p->mpw, accumulate, with_kin);
+    kin_only_kernel<<<grid, 256, 0, st>>>(cpsi, chpsi, d_kin, d_npw, nband, p->mpw, accumulate, with_kin, rec != nullptr,
+                                          rec ? rec->sh : 1.0, rec ? rec->sy : 0.0, rec ? rec->sx : 0.0,
+                                          rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr);
     phase_end(p, 7, st, 1);
     DFT_CUDA_CHECK(cudaGetLastError());
     return DFT_OK;
@@ -653,6 +672,8 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   q2.nproj = nproj; q2.nband = nband; q2.mpw = mpw; q2.nslab = (nproj + 7) / 8;
   q2.tiles_n = q1.tiles_n; q2.accumulate = accumulate; q2.with_kin = with_kin; q2.with_nl = 1;
   q2.npw = d_npw; q2.kin = d_kin; q2.psi = cpsi; q2.hpsi = chpsi;
+  q2.cheb = rec != nullptr; q2.sh = rec ? rec->sh : 1.0; q2.sy = rec ? rec->sy : 0.0; q2.sx = rec ? rec->sx : 0.0;
+  q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr;
   int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
   phase_begin(p, 7, st);
   if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);

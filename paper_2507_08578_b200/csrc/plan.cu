@@ -281,7 +281,7 @@ static int ensure_workspace(dft_plan *p, int64_t per_band, int nband, int *chunk
   return DFT_OK;
 }
 
-static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nband, cudaStream_t st) {
+static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nband, cudaStream_t st, const Recurrence *rec = nullptr) {
   p->last_launches = 0;
   if (nband == 0 || p->mpw == 0 || p->nkpt == 0) return DFT_OK;
   const bool loc = (p->terms & 2) != 0, kin = (p->terms & 1) != 0, nl = (p->terms & 4) != 0 && p->nproj > 0;
@@ -302,8 +302,8 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
     if ((rc = zero_fill(hpsi, (int64_t)p->nkpt * nband * band_stride, st))) return rc;
     phase_end(p, 4, st, 1);
   }
-  if (kin || nl)
-    if ((rc = nonlocal_apply(p, psi, hpsi, nband, true, kin, nl, st))) return rc;
+  if (kin || nl || rec)
+    if ((rc = nonlocal_apply(p, psi, hpsi, nband, true, kin, nl, st, nullptr, nullptr, nullptr, rec))) return rc;
   return DFT_OK;
 }
 
@@ -437,6 +437,38 @@ int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, voi
   if (nband > 0 && p->mpw > 0 && (!psi || !hpsi)) { set_error("null psi/hpsi"); return DFT_ERR_INVALID_ARG; }
   if (((uintptr_t)psi & 15) || ((uintptr_t)hpsi & 15)) { set_error("psi/hpsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
   return apply_impl(p, psi, hpsi, nband, (cudaStream_t)stream);
+  DFT_GUARD_END
+}
+
+int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, int32_t degree, double center,
+                         double halfwidth, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0 || degree < 0) { set_error("nband = %d, degree = %d: negative", nband, degree); return DFT_ERR_INVALID_ARG; }
+  if (!(halfwidth > 0.0) || !(center == center)) { set_error("halfwidth must be > 0 and center finite"); return DFT_ERR_INVALID_ARG; }
+  p->last_launches = 0;
+  const size_t n = (size_t)p->nkpt * nband * p->mpw * 2;   // doubles per psi-sized array
+  if (n == 0 || degree == 0) return DFT_OK;
+  if (!psi || !work) { set_error("null psi/work"); return DFT_ERR_INVALID_ARG; }
+  if (((uintptr_t)psi & 15) || ((uintptr_t)work & 15)) { set_error("psi/work must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  cudaStream_t st = (cudaStream_t)stream;
+  // three psi-sized arrays rotate: x = T_{j-1}, y = T_j, w receives T_{j+1} from the GEMM-2 epilogue
+  double *buf[3] = {psi, work, work + n};
+  int ix = 2, iy = 0, iw = 1;
+  int64_t launches = 0;
+  for (int j = 0; j < degree; j++) {
+    Recurrence rec;
+    if (j == 0) { rec.sh = 1.0 / halfwidth; rec.sy = -center / halfwidth; rec.sx = 0.0; rec.xprev = nullptr; }
+    else { rec.sh = 2.0 / halfwidth; rec.sy = -2.0 * center / halfwidth; rec.sx = -1.0; rec.xprev = buf[ix]; }
+    // T_{j+1} goes to the third array: the FFT passes store V_loc T_j there before the epilogue reads T_{j-1}
+    int rc = apply_impl(p, buf[iy], buf[iw], nband, st, &rec);
+    if (rc) return rc;
+    launches += p->last_launches;
+    int t = ix; ix = iy; iy = iw; iw = t;
+  }
+  p->last_launches = launches;
+  if (buf[iy] != psi) DFT_CUDA_CHECK(cudaMemcpyAsync(psi, buf[iy], n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  return DFT_OK;
   DFT_GUARD_END
 }
 

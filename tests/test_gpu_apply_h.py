@@ -166,6 +166,31 @@ def test_overlap_operator_and_cprj(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c1m", "aniso", "c3k2"])
+def test_chebyshev_filter(name):
+    """dft_chebyshev_filter (PAPER.md :458, :489) against the oracle's recurrence; T_n grows like cosh(n acosh x) outside
+    [-1, 1], so the per-band relative error is what is bounded."""
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    kmax = max(float(s[2].max()) for s in sph)
+    cen, e = 0.5 * kmax + 1.0, 0.5 * kmax + 0.5           # damp roughly [0.5, kmax + 1.5] Ha
+    for g3 in (1, 0):
+        plan.set_option("gemm_3m", g3)
+        for deg in (0, 1, 4, 7):
+            t = torch.as_tensor(psi, device="cuda").clone()
+            got = plan.chebyshev_filter(t, deg, cen, e).cpu().numpy()
+            if plan.nkpt == 1:
+                assert plan.last_launches() == 8 * deg
+            for ik, (kg, ig, kin) in enumerate(sph):
+                ref = oracle.chebyshev_filter(cfg, ik, kg, ig, kin, psi[ik], deg, cen, e, method=1 if name == "aniso" else 2)
+                npw = len(ig)
+                err = float(np.max(np.linalg.norm(got[ik][:, :npw] - ref[:, :npw], axis=1) / np.linalg.norm(ref[:, :npw], axis=1)))
+                assert err <= TOL, "%s deg=%d gemm_3m=%d k=%d: %.3e" % (name, deg, g3, ik, err)
+                if deg > 0:
+                    assert np.all(got[ik][:, npw:] == 0)
+    plan.destroy()
+
+
 def test_host_api_band_groups():
     """dft_apply_h_host cuts one k-point's bands into groups whose copies overlap the neighbours' kernels;
     the result must not depend on the grouping."""

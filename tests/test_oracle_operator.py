@@ -65,3 +65,30 @@ def test_generator_is_chunk_independent():
     assert abs(np.std(full.real * (1 + 2 * kin)) - 1) < 0.1
     d = c["dij"]
     assert np.array_equal(d, d.transpose(0, 2, 1))
+
+
+def test_chebyshev_filter_pins():
+    """The recurrence reproduces the Chebyshev polynomial of H: (i) free electron (V = 0, D = 0), H diagonal, so the
+    result is numpy's chebval of (kin - c)/e times psi; (ii) c0 with every term, through the eigen-decomposition of the
+    dense H (numpy eigh): V T_n((lambda - c)/e) V^H psi; (iii) degrees 0 and 1 by hand."""
+    from numpy.polynomial import chebyshev as C
+    import oracle
+    from util import config, sphere, rand_c, rel_err
+    c = config("c0"); kg, ig, kin = sphere("c0")
+    psi = rand_c((2, len(kg)), 21)
+    cen, e = 6.0, 5.0
+    for deg in (2, 5, 10):
+        coef = np.zeros(deg + 1); coef[deg] = 1.0
+        got = oracle.chebyshev_filter(c, 0, kg, ig, kin, psi, deg, cen, e, terms=oracle.KIN)
+        assert rel_err(got, C.chebval((kin - cen) / e, coef)[None, :] * psi) < 1e-12
+    H = oracle.dense_h(c, 0, kg, kin)
+    lam, V = np.linalg.eigh(H)
+    cen, e = 0.5 * (lam[-1] + lam[4]), 0.5 * (lam[-1] - lam[4])          # damp everything above the 4 lowest states
+    for deg in (3, 8):
+        coef = np.zeros(deg + 1); coef[deg] = 1.0
+        ref = (V @ (C.chebval((lam - cen) / e, coef)[:, None] * (V.conj().T @ psi.T))).T
+        got = oracle.chebyshev_filter(c, 0, kg, ig, kin, psi, deg, cen, e, method=1)
+        assert rel_err(got, ref) < 1e-11
+    assert np.array_equal(oracle.chebyshev_filter(c, 0, kg, ig, kin, psi, 0, cen, e), psi)
+    h1 = oracle.apply_h(c, 0, kg, ig, kin, psi)
+    assert rel_err(oracle.chebyshev_filter(c, 0, kg, ig, kin, psi, 1, cen, e), (h1 - cen * psi) / e) < 1e-15

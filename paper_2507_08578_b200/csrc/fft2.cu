@@ -54,10 +54,19 @@ struct Fft2Geom {
   int64_t t1_band, t2_band;   // complex elements per band of T1 [ncol][n1] and T2 [nplane][n2][n1]
 };
 
+// Several k-points in one launch (BATCH): blockIdx.y = k-point, geometry read from a device array, per-k strides of
+// the caller's arrays and of the scratch; grid.x is sized for the k-point with the most columns / planes.
+struct Fft2Batch {
+  const Fft2Geom *Gs;
+  int64_t ks_psi, ks_t1, ks_t2;   // complex elements between consecutive k-points
+};
+
 // ---- pass A: sphere -> x-lines (type I).  block = lpc lines x NS slots, slot fastest; grid = nb * ntile
-template <int R1, int R2>
+template <int R1, int R2, bool BATCH>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-fft2_a_fwd_kernel(Fft2Geom G, const cplx *__restrict__ psi, cplx *__restrict__ T1, int lpc, int ntile) {
+fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *__restrict__ T1, int lpc, int ntile) {
+  const Fft2Geom G = BATCH ? B.Gs[blockIdx.y] : G0;
+  if (BATCH) { psi += (size_t)blockIdx.y * B.ks_psi; T1 += (size_t)blockIdx.y * B.ks_t1; }
   constexpr int NS = imax(R1, R2), KS = R2 | 1, LS = pad8(R1 * KS, NS);
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
@@ -94,9 +103,11 @@ fft2_a_fwd_kernel(Fft2Geom G, const cplx *__restrict__ psi, cplx *__restrict__ T
 }
 
 // ---- pass A^-1: x-lines -> sphere (type II) + zero the pad entries ipw >= npw of the band
-template <int R1, int R2>
+template <int R1, int R2, bool BATCH>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-fft2_a_inv_kernel(Fft2Geom G, const cplx *__restrict__ T1, cplx *__restrict__ hpsi, int lpc, int ntile) {
+fft2_a_inv_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ T1, cplx *__restrict__ hpsi, int lpc, int ntile) {
+  const Fft2Geom G = BATCH ? B.Gs[blockIdx.y] : G0;
+  if (BATCH) { hpsi += (size_t)blockIdx.y * B.ks_psi; T1 += (size_t)blockIdx.y * B.ks_t1; }
   constexpr int NS = imax(R1, R2), KS = R1 | 1, LS = pad8(R2 * KS, NS);
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
@@ -134,9 +145,12 @@ fft2_a_inv_kernel(Fft2Geom G, const cplx *__restrict__ T1, cplx *__restrict__ hp
 
 // ---- pass B: along y on the occupied planes (type I).  block = NS slots x XT consecutive x, x fastest;
 //      grid = nb * nplane * nxt.  Shared exchange element (k1, j2, px) at k1*KS + j2*XT + px.
-template <int R1, int R2>
+template <int R1, int R2, bool BATCH>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-fft2_b_fwd_kernel(Fft2Geom G, const cplx *__restrict__ T1, cplx *__restrict__ T2, int XT, int nxt) {
+fft2_b_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ T1, cplx *__restrict__ T2, int XT, int nxt, int nb) {
+  const Fft2Geom G = BATCH ? B.Gs[blockIdx.y] : G0;
+  if (BATCH) { T1 += (size_t)blockIdx.y * B.ks_t1; T2 += (size_t)blockIdx.y * B.ks_t2; }
+  if (BATCH && (int)(blockIdx.x / (nxt * G.nplane)) >= nb) return;   // grid sized for the k-point with most planes
   constexpr int NS = imax(R1, R2);
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
@@ -174,9 +188,12 @@ fft2_b_fwd_kernel(Fft2Geom G, const cplx *__restrict__ T1, cplx *__restrict__ T2
 }
 
 // ---- pass B^-1: inverse along y, keep the non-empty columns (type II)
-template <int R1, int R2>
+template <int R1, int R2, bool BATCH>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-fft2_b_inv_kernel(Fft2Geom G, cplx *__restrict__ T1, const cplx *__restrict__ T2, int XT, int nxt) {
+fft2_b_inv_kernel(Fft2Geom G0, Fft2Batch B, cplx *__restrict__ T1, const cplx *__restrict__ T2, int XT, int nxt, int nb) {
+  const Fft2Geom G = BATCH ? B.Gs[blockIdx.y] : G0;
+  if (BATCH) { T1 += (size_t)blockIdx.y * B.ks_t1; T2 += (size_t)blockIdx.y * B.ks_t2; }
+  if (BATCH && (int)(blockIdx.x / (nxt * G.nplane)) >= nb) return;
   constexpr int NS = imax(R1, R2);
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
@@ -214,9 +231,11 @@ fft2_b_inv_kernel(Fft2Geom G, cplx *__restrict__ T1, const cplx *__restrict__ T2
 // ---- pass C: along z (type I), times V(r)/N, inverse along z (type II), in place on the occupied planes.
 //      grid = ntile * nb with the BAND fastest, so the nb CTAs that need the same V tile run together
 //      and V is fetched from DRAM once per band chunk.
-template <int R1, int R2>
+template <int R1, int R2, bool BATCH>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-fft2_c_kernel(Fft2Geom G, cplx *__restrict__ T2, const double *__restrict__ vloc, int XT, int nxt, int nb) {
+fft2_c_kernel(Fft2Geom G0, Fft2Batch B, cplx *__restrict__ T2, const double *__restrict__ vloc, int XT, int nxt, int nb) {
+  const Fft2Geom G = BATCH ? B.Gs[blockIdx.y] : G0;
+  if (BATCH) T2 += (size_t)blockIdx.y * B.ks_t2;
   constexpr int NS = imax(R1, R2);
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
@@ -690,11 +709,11 @@ static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi
     int64_t grid = (int64_t)nb * ntile;
     if (grid > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
     if (pass == 0) {
-      if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2>, sm))) return rc;
-      fft2_a_fwd_kernel<R1, R2><<<(unsigned)grid, lpc * NS, sm, st>>>(G, psi, T1, lpc, ntile);
+      if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, false>, sm))) return rc;
+      fft2_a_fwd_kernel<R1, R2, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), psi, T1, lpc, ntile);
     } else {
-      if ((rc = set_smem(fft2_a_inv_kernel<R1, R2>, sm))) return rc;
-      fft2_a_inv_kernel<R1, R2><<<(unsigned)grid, lpc * NS, sm, st>>>(G, T1, hpsi, lpc, ntile);
+      if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, false>, sm))) return rc;
+      fft2_a_inv_kernel<R1, R2, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), T1, hpsi, lpc, ntile);
     }
   } else {
     int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
@@ -702,17 +721,110 @@ static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi
     int64_t grid = (int64_t)nb * nxt * (pass == 2 ? G.n2 : G.nplane);
     if (grid > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
     if (pass == 1) {
-      if ((rc = set_smem(fft2_b_fwd_kernel<R1, R2>, sm))) return rc;
-      fft2_b_fwd_kernel<R1, R2><<<(unsigned)grid, XT * NS, sm, st>>>(G, T1, T2, XT, nxt);
+      if ((rc = set_smem(fft2_b_fwd_kernel<R1, R2, false>, sm))) return rc;
+      fft2_b_fwd_kernel<R1, R2, false><<<(unsigned)grid, XT * NS, sm, st>>>(G, Fft2Batch(), T1, T2, XT, nxt, nb);
     } else if (pass == 3) {
-      if ((rc = set_smem(fft2_b_inv_kernel<R1, R2>, sm))) return rc;
-      fft2_b_inv_kernel<R1, R2><<<(unsigned)grid, XT * NS, sm, st>>>(G, T1, T2, XT, nxt);
+      if ((rc = set_smem(fft2_b_inv_kernel<R1, R2, false>, sm))) return rc;
+      fft2_b_inv_kernel<R1, R2, false><<<(unsigned)grid, XT * NS, sm, st>>>(G, Fft2Batch(), T1, T2, XT, nxt, nb);
     } else {
-      if ((rc = set_smem(fft2_c_kernel<R1, R2>, sm))) return rc;
-      fft2_c_kernel<R1, R2><<<(unsigned)grid, XT * NS, sm, st>>>(G, T2, vloc, XT, nxt, nb);
+      if ((rc = set_smem(fft2_c_kernel<R1, R2, false>, sm))) return rc;
+      fft2_c_kernel<R1, R2, false><<<(unsigned)grid, XT * NS, sm, st>>>(G, Fft2Batch(), T2, vloc, XT, nxt, nb);
     }
   }
   DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+// ---- several k-points per launch (small boxes, e.g. 32 k-points of a 32^3 box: one launch per pass instead of 32)
+template <int R1, int R2>
+static int launch_pass_batched(const Fft2Geom &G, const Fft2Batch &B, int nk, int pass, const cplx *psi, cplx *hpsi, cplx *T1,
+                               cplx *T2, const double *vloc, int nb, int max_ncol, int max_nplane, cudaStream_t st) {
+  constexpr int NS = imax(R1, R2);
+  int rc;
+  if (pass == 0 || pass == 4) {
+    int lpc = F2_THREADS / NS;
+    if (lpc > max_ncol) lpc = max_ncol;
+    int ntile = (max_ncol + lpc - 1) / lpc;
+    constexpr int LSf = pad8(R1 * (R2 | 1), NS), LSi = pad8(R2 * (R1 | 1), NS);
+    size_t sm = sizeof(cplx) * (size_t)lpc * (pass == 0 ? LSf : LSi);
+    int64_t grid = (int64_t)nb * ntile;
+    if (grid > 0x7fffffffLL) return DFT_ERR_UNSUPPORTED;
+    if (pass == 0) {
+      if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, true>, sm))) return rc;
+      fft2_a_fwd_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, psi, T1, lpc, ntile);
+    } else {
+      if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, true>, sm))) return rc;
+      fft2_a_inv_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, T1, hpsi, lpc, ntile);
+    }
+  } else {
+    int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
+    size_t sm = sizeof(cplx) * (size_t)(pad8(R2 * XT, XT) * R1 > pad8(R1 * XT, XT) * R2 ? pad8(R2 * XT, XT) * R1 : pad8(R1 * XT, XT) * R2);
+    int64_t grid = (int64_t)nb * nxt * (pass == 2 ? G.n2 : max_nplane);
+    if (grid > 0x7fffffffLL) return DFT_ERR_UNSUPPORTED;
+    if (pass == 1) {
+      if ((rc = set_smem(fft2_b_fwd_kernel<R1, R2, true>, sm))) return rc;
+      fft2_b_fwd_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), XT * NS, sm, st>>>(G, B, T1, T2, XT, nxt, nb);
+    } else if (pass == 3) {
+      if ((rc = set_smem(fft2_b_inv_kernel<R1, R2, true>, sm))) return rc;
+      fft2_b_inv_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), XT * NS, sm, st>>>(G, B, T1, T2, XT, nxt, nb);
+    } else {
+      if ((rc = set_smem(fft2_c_kernel<R1, R2, true>, sm))) return rc;
+      fft2_c_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), XT * NS, sm, st>>>(G, B, T2, vloc, XT, nxt, nb);
+    }
+  }
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+bool fft2_batch_ok(const dft_plan *p) {
+  if (p->nkpt < 2 || p->nkpt > 65535 || p->fft_path == 1) return false;
+  for (int c = 0; c < 3; c++)
+    if (!fft2_pair(p->n[c], nullptr, nullptr)) return false;
+  for (int ik = 0; ik < p->nkpt; ik++)
+    if (!p->kp[ik].runs_ok || p->kp[ik].npw == 0) return false;
+  return true;
+}
+
+// V_loc psi for `nb` bands of EVERY k-point: psi/hpsi point at the first of those bands of k-point 0, consecutive
+// k-points are nband_total bands apart; ws holds T1 [nkpt][nb] then T2 [nkpt][nb] with the per-band strides of
+// fft_ws_bytes_per_band's maxima.
+int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int nband_total, void *ws, cudaStream_t st) {
+  const int nk = p->nkpt;
+  int64_t t1b = 0, t2b = 0;
+  int max_ncol = 0, max_nplane = 0;
+  for (int ik = 0; ik < nk; ik++) {
+    const KPoint &kp = p->kp[ik];
+    int64_t a = ((int64_t)kp.ncol * p->n[0] * 16 + 255) / 256 * 256, b = ((int64_t)kp.nplane * p->n[1] * p->n[0] * 16 + 255) / 256 * 256;
+    if (a > t1b) t1b = a;
+    if (b > t2b) t2b = b;
+    if (kp.ncol > max_ncol) max_ncol = kp.ncol;
+    if (kp.nplane > max_nplane) max_nplane = kp.nplane;
+  }
+  t1b /= 16; t2b /= 16;
+  if (!p->d_geom2) {
+    std::vector<Fft2Geom> g(nk);
+    for (int ik = 0; ik < nk; ik++) g[ik] = make_geom2(p, ik, t1b, t2b);
+    if (cudaMalloc(&p->d_geom2, sizeof(Fft2Geom) * nk) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the k-point geometry array"); return DFT_ERR_ALLOC; }
+    DFT_CUDA_CHECK(cudaMemcpy(p->d_geom2, g.data(), sizeof(Fft2Geom) * nk, cudaMemcpyHostToDevice));
+  }
+  Fft2Geom G = make_geom2(p, 0, t1b, t2b);
+  Fft2Batch B;
+  B.Gs = reinterpret_cast<const Fft2Geom *>(p->d_geom2);
+  B.ks_psi = (int64_t)nband_total * p->mpw; B.ks_t1 = (int64_t)nb * t1b; B.ks_t2 = (int64_t)nb * t2b;
+  cplx *T1 = reinterpret_cast<cplx *>(ws), *T2 = T1 + (size_t)nk * nb * t1b;
+  const cplx *cpsi = reinterpret_cast<const cplx *>(psi);
+  cplx *chpsi = reinterpret_cast<cplx *>(hpsi);
+  const int axis_of[5] = {0, 1, 2, 1, 0};
+  for (int pass = 0; pass < 5; pass++) {
+    int r1, r2, rc = DFT_ERR_UNSUPPORTED;
+    fft2_pair(p->n[axis_of[pass]], &r1, &r2);
+    phase_begin(p, pass, st);
+#define X(a, b) if (r1 == (a) && r2 == (b)) rc = launch_pass_batched<a, b>(G, B, nk, pass, cpsi, chpsi, T1, T2, p->d_vloc, nb, max_ncol, max_nplane, st);
+    FFT2_PAIRS(X)
+#undef X
+    phase_end(p, pass, st, 1);
+    if (rc) { if (rc == DFT_ERR_UNSUPPORTED) set_error("batched FFT pass %d cannot be launched", pass); return rc; }
+  }
   return DFT_OK;
 }
 

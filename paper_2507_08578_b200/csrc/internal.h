@@ -127,6 +127,7 @@ struct dft_plan {
   int host_groups = 4;     // dft_apply_h_host: band groups whose copies overlap the kernels of their neighbours
   // TMA
   void *encode_fn = nullptr;   // cuTensorMapEncodeTiled
+  void *d_geom2 = nullptr;    // device array of per-k-point FFT geometry (fft2.cu, built at first batched call)
   int sm_count = 148;
   int smem_per_sm = 233472, smem_optin = 232448;   // bytes of shared memory per SM / per CTA (opt-in), from the device
   int64_t last_launches = 0;
@@ -162,6 +163,10 @@ struct Recurrence {
   double sh, sy, sx;
   const double *xprev;   // device [nkpt][nband][mpw] complex; read only where sx != 0
 };
+
+// several k-points per launch (plain register kernels with blockIdx.y = k-point)
+bool fft2_batch_ok(const dft_plan *p);
+int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int nband_total, void *ws, cudaStream_t st);
 
 // --- nonlocal.cu (K3) ---------------------------------------------------------------------
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi

@@ -59,7 +59,7 @@ static void destroy_plan(dft_plan *p) {
   for (auto &k : p->kp) free_kpoint(k);
   cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
   cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
-  cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  cudaFree(p->d_geom2); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
@@ -290,6 +290,14 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
   const size_t band_stride = (size_t)p->mpw * 2;
   if (loc) {
     int chunk; void *ws;
+    if (fft2_batch_ok(p) && (!p->ws_user || p->ws_user_bytes >= fft_ws_bytes_per_band(p) * p->nkpt)) {
+      // small boxes, many k-points: every pass is one launch over all k-points (blockIdx.y = k-point)
+      if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p) * p->nkpt, nband, &chunk, &ws, st))) return rc;
+      for (int b0 = 0; b0 < nband; b0 += chunk) {
+        int nb = nband - b0 < chunk ? nband - b0 : chunk;
+        if ((rc = fft2_apply_batched(p, psi + (size_t)b0 * band_stride, hpsi + (size_t)b0 * band_stride, nb, nband, ws, st))) return rc;
+      }
+    } else {
     if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
     for (int ik = 0; ik < p->nkpt; ik++)
       for (int b0 = 0; b0 < nband; b0 += chunk) {
@@ -297,6 +305,7 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
         size_t off = ((size_t)ik * nband + b0) * band_stride;
         if ((rc = fft_apply_vloc(p, ik, psi + off, hpsi + off, nb, ws, st))) return rc;
       }
+    }
   } else {
     phase_begin(p, 4, st);
     if ((rc = zero_fill(hpsi, (int64_t)p->nkpt * nband * band_stride, st))) return rc;

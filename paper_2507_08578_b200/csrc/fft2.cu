@@ -467,8 +467,10 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
   unsigned char *stages = smem_raw;
   cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
   double *vs = reinterpret_cast<double *>(sm + exn);
-  uint64_t *full = reinterpret_cast<uint64_t *>(vs + ((G.n3 * XT + 1) & ~1));
+  cplx *tws = reinterpret_cast<cplx *>(vs + ((G.n3 * XT + 1) & ~1));   // twiddles exp(+2 pi i j / n3), j < n3
+  uint64_t *full = reinterpret_cast<uint64_t *>(tws + G.n3);
   const int t = threadIdx.x, px = t % XT, s = t / XT;
+  for (int i = t; i < G.n3; i += blockDim.x) tws[i] = __ldg(G.tw3 + i);
   if (t == 0) {
     for (int i = 0; i < Q.S; i++) mbar_init(&full[i], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -514,7 +516,7 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
       }
       Dft<R1, +1>::run(v);
 #pragma unroll
-      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw3, s * k1));
+      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], tws[s * k1]);
 #pragma unroll
       for (int k1 = 0; k1 < R1; k1++) sm[k1 * KSa + s * XT + px] = v[k1];
     }
@@ -530,7 +532,7 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
       for (int k2 = 0; k2 < R2; k2++) v[k2] = cscale(v[k2], vs[(s + R1 * k2) * XT + px]);
       Dft<R2, -1>::run(v);
 #pragma unroll
-      for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw3, s * cc));
+      for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], tws[s * cc]);
 #pragma unroll
       for (int cc = 0; cc < R2; cc++) sm[cc * KSb + s * XT + px] = v[cc];
     }
@@ -636,7 +638,7 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
   const int rows = pass == 1 ? hb : (pass == 2 ? G.nplane : G.n2);
   const int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
   size_t ex = sizeof(cplx) * (size_t)(pass == 1 ? R1 * KSa : (pass == 3 ? R2 * KSb : imax(R1 * KSa, R2 * KSb)));
-  size_t extra = pass == 2 ? sizeof(double) * (size_t)((G.n3 * XT + 1) & ~1) : sizeof(Run) * (size_t)G.nplane;
+  size_t extra = pass == 2 ? sizeof(double) * (size_t)((G.n3 * XT + 1) & ~1) + sizeof(cplx) * (size_t)G.n3 : sizeof(Run) * (size_t)G.nplane;
   RingParams Q;
   Q.XT = XT; Q.nxt = nxt; Q.nb = nb;
   Q.box_bytes = (uint32_t)((size_t)rows * XT * 16);

@@ -134,6 +134,12 @@ int dft_apply_s(dft_plan *p, const double *psi, double *spsi, int32_t nband, voi
  * atom.  GEMM-1 and the fixed-order split-K reduction only; enqueues on `stream`.                 */
 int dft_get_cprj(dft_plan *p, const double *psi, double *cprj, int32_t nband, void *stream);
 
+/* Velocity-gauge vector potential (PAPER.md :340: in RT-TDDFT "the velocity gauge changes only the kinetic
+ * term", -i grad -> -i grad + A(t)): while set, the kinetic diagonal of dft_apply_h / dft_chebyshev_filter is
+ * 1/2 |k + G + A|^2 with A = a_cart[3] (HOST, Cartesian, atomic units).  The sphere (defined at A = 0) and
+ * every other term are unchanged.  NULL or (0,0,0) switches it off.  Synchronises the device.        */
+int dft_set_vector_potential(dft_plan *p, const double *a_cart);
+
 /* Chebyshev filter (PAPER.md :458 "Chebyshev filtering algorithm ... filters the spectrum of the Hamiltonian",
  * :489 "mdeg_filter 10"; the paper prints no formula, this is the textbook three-term recurrence):
  *   T_0 = psi,  T_1 = (H - center) T_0 / halfwidth,  T_{j+1} = 2 (H - center) T_j / halfwidth - T_{j-1},

@@ -188,6 +188,15 @@ def nonlocal_apply(cfg, ik, kg, psi, dij=None, want_cprj=False):
     return (out, cp) if want_cprj else out
 
 
+def kin_vecpot(rprimd, k, kg, a_cart):
+    """1/2 |k + G + A|^2 per plane wave (PAPER.md :340, velocity gauge: -i grad -> -i grad + A): q = 2 pi (k + m) Bm
+    Cartesian (reading 1), A Cartesian in atomic units.  Plain numpy; pass the result to apply_h as `kin`."""
+    bm, _ = lattice(rprimd)
+    q = 2.0 * np.pi * (np.asarray(kg, float) + np.asarray(k, float)[None, :]) @ np.asarray(bm, float).reshape(3, 3)
+    q = q + np.asarray(a_cart, float)[None, :]
+    return 0.5 * np.sum(q * q, axis=1)
+
+
 def cprj(cfg, ik, kg, psi):
     """<p_a,i|psi_b> (PAPER.md :477 "coefficients c_a,i,n,k"), [nproj][nband] complex: step 1 of Eq. 26 (:470),
     as the streamed loops of orc_nonlocal_apply compute it."""

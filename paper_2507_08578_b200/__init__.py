@@ -33,6 +33,7 @@ PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_get_cprj", "dft_chebyshev_filter",
+           "dft_set_vector_potential",
            "dft_set_vloc", "dft_set_workspace", "dft_plan_set_option", "dft_apply_h", "dft_apply_h_host",
            "dft_plan_last_launches", "dft_plan_set_timing", "dft_plan_phase_ms", "dft_plan_destroy", "dft_last_error")
 
@@ -80,6 +81,7 @@ def lib():
     L.dft_apply_h.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_apply_h_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
     L.dft_set_sij.argtypes = [C.c_void_p, _dp]
+    L.dft_set_vector_potential.argtypes = [C.c_void_p, _dp]
     L.dft_chebyshev_filter.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                        C.c_void_p]
     L.dft_apply_s.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
@@ -196,6 +198,10 @@ def dft_get_cprj(plan, psi_dev_ptr, cprj_dev_ptr, nband, stream=0):
     _check(lib().dft_get_cprj(plan, psi_dev_ptr, cprj_dev_ptr, nband, stream))
 
 
+def dft_set_vector_potential(plan, a_cart):
+    _check(lib().dft_set_vector_potential(plan, None if a_cart is None else _d(_f64(a_cart))))
+
+
 def dft_chebyshev_filter(plan, psi_dev_ptr, work_dev_ptr, nband, degree, center, halfwidth, stream=0):
     _check(lib().dft_chebyshev_filter(plan, psi_dev_ptr, work_dev_ptr, nband, degree, center, halfwidth, stream))
 
@@ -297,6 +303,10 @@ class Plan:
         out = torch.zeros((self.nkpt, nband, self.nproj), dtype=torch.complex128, device=psi.device)
         dft_get_cprj(self.h, psi.data_ptr(), out.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
         return out
+
+    def set_vector_potential(self, a_cart):
+        """Velocity gauge: kinetic term 1/2|k+G+A|^2 (A Cartesian, a.u.); None switches it off."""
+        dft_set_vector_potential(self.h, a_cart)
 
     def chebyshev_filter(self, psi, degree, center, halfwidth, work=None):
         """In place: psi := T_degree((H - center)/halfwidth) psi.  work: optional complex128 CUDA tensor, 2 x psi.numel()."""

@@ -97,6 +97,9 @@ struct dft_plan {
   double *d_dq = nullptr, *d_xred = nullptr;
   double *d_dij = nullptr;                           // [natom][lmax][lmax]
   double *d_sij = nullptr;                           // [natom][lmax][lmax] overlap coefficients s_ij (zero until dft_set_sij)
+  double *d_kina = nullptr;                          // [nkpt][mpw] 1/2|k+G+A|^2 while a vector potential is set
+  const double **d_kinaptr = nullptr;                // [nkpt] device pointers into d_kina
+  bool vecpot_on = false;
   double *d_ones = nullptr;                          // [mpw] of 1.0: the unit diagonal of S in GEMM-2's epilogue
   const double **d_oneptr = nullptr;                 // [nkpt] device pointers to d_ones
   double *d_ptab = nullptr;                          // [nkpt][nproj][mpw] complex, zero padded beyond npw_k

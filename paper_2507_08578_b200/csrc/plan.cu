@@ -59,7 +59,7 @@ static void destroy_plan(dft_plan *p) {
   for (auto &k : p->kp) free_kpoint(k);
   cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
   cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
-  cudaFree(p->d_geom2); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  cudaFree(p->d_geom2); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
@@ -312,7 +312,7 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
     phase_end(p, 4, st, 1);
   }
   if (kin || nl || rec)
-    if ((rc = nonlocal_apply(p, psi, hpsi, nband, true, kin, nl, st, nullptr, nullptr, nullptr, rec))) return rc;
+    if ((rc = nonlocal_apply(p, psi, hpsi, nband, true, kin, nl, st, nullptr, p->vecpot_on ? p->d_kinaptr : nullptr, nullptr, rec))) return rc;
   return DFT_OK;
 }
 
@@ -446,6 +446,54 @@ int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, voi
   if (nband > 0 && p->mpw > 0 && (!psi || !hpsi)) { set_error("null psi/hpsi"); return DFT_ERR_INVALID_ARG; }
   if (((uintptr_t)psi & 15) || ((uintptr_t)hpsi & 15)) { set_error("psi/hpsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
   return apply_impl(p, psi, hpsi, nband, (cudaStream_t)stream);
+  DFT_GUARD_END
+}
+
+}  // extern "C"
+namespace dftb200 {
+// 1/2 |k + G + A|^2 for the plane waves of one k-point: q = 2 pi (k + m) Bm (Cartesian), A Cartesian, atomic units
+__global__ void kin_vecpot_kernel(const int32_t *__restrict__ kg, int npw, double k1, double k2, double k3, const double *__restrict__ bm9,
+                                  double a1, double a2, double a3, double *__restrict__ out) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= npw) return;
+  const double twopi = 6.283185307179586476925286766559;
+  double t1 = k1 + (double)kg[3 * g], t2 = k2 + (double)kg[3 * g + 1], t3 = k3 + (double)kg[3 * g + 2];
+  double q1 = twopi * (t1 * bm9[0] + t2 * bm9[3] + t3 * bm9[6]) + a1;
+  double q2 = twopi * (t1 * bm9[1] + t2 * bm9[4] + t3 * bm9[7]) + a2;
+  double q3 = twopi * (t1 * bm9[2] + t2 * bm9[5] + t3 * bm9[8]) + a3;
+  out[g] = 0.5 * (q1 * q1 + q2 * q2 + q3 * q3);
+}
+}  // namespace dftb200
+extern "C" {
+
+int dft_set_vector_potential(dft_plan *p, const double *a_cart) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (!a_cart || (a_cart[0] == 0.0 && a_cart[1] == 0.0 && a_cart[2] == 0.0)) { p->vecpot_on = false; return DFT_OK; }
+  for (int c = 0; c < 3; c++)
+    if (!(a_cart[c] == a_cart[c]) || a_cart[c] - a_cart[c] != 0.0) { set_error("vector potential is not finite"); return DFT_ERR_INVALID_ARG; }
+  if (p->mpw == 0 || p->nkpt == 0) return DFT_OK;
+  int rc;
+  if (!p->d_kina) {
+    if (cudaMalloc(&p->d_kina, sizeof(double) * (size_t)p->nkpt * p->mpw) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the kinetic array"); return DFT_ERR_ALLOC; }
+    std::vector<const double *> ptr(p->nkpt);
+    for (int ik = 0; ik < p->nkpt; ik++) ptr[ik] = p->d_kina + (size_t)ik * p->mpw;
+    if ((rc = to_device((const double ***)&p->d_kinaptr, ptr.data(), p->nkpt))) return rc;
+  }
+  double *d_bm = nullptr;
+  if ((rc = to_device(&d_bm, p->bm, 9))) return rc;
+  DFT_CUDA_CHECK(cudaMemset(p->d_kina, 0, sizeof(double) * (size_t)p->nkpt * p->mpw));
+  for (int ik = 0; ik < p->nkpt; ik++) {
+    const KPoint &K = p->kp[ik];
+    if (K.npw == 0) continue;
+    kin_vecpot_kernel<<<(K.npw + 255) / 256, 256>>>(K.kg, K.npw, K.k[0], K.k[1], K.k[2], d_bm, a_cart[0], a_cart[1], a_cart[2],
+                                                   p->d_kina + (size_t)ik * p->mpw);
+  }
+  cudaError_t e = cudaDeviceSynchronize();
+  cudaFree(d_bm);
+  if (e != cudaSuccess) { set_error("kin_vecpot_kernel failed: %s", cudaGetErrorString(e)); return DFT_ERR_CUDA; }
+  p->vecpot_on = true;
+  return DFT_OK;
   DFT_GUARD_END
 }
 

@@ -191,6 +191,30 @@ def test_chebyshev_filter(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c1m", "aniso", "c3k2"])
+def test_velocity_gauge_kinetic(name):
+    """dft_set_vector_potential (PAPER.md :340): kinetic term 1/2|k+G+A|^2, everything else unchanged; switching it off
+    restores the plain operator."""
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    a = np.array([0.35, -0.2, 0.15])
+    plain = gpu_apply(plan, psi)
+    plan.set_vector_potential(a)
+    for terms in (7, 1):
+        plan.set_option("terms", terms)
+        got = gpu_apply(plan, psi)
+        for ik, (kg, ig, kin) in enumerate(sph):
+            ka = oracle.kin_vecpot(cfg["rprimd"], cfg["kpt"][ik], kg, a)
+            ref = oracle.apply_h(cfg, ik, kg, ig, ka, psi[ik], method=1 if name == "aniso" else 2, terms=terms)
+            npw = len(ig)
+            err = float(np.max(np.linalg.norm(got[ik][:, :npw] - ref[:, :npw], axis=1) / np.linalg.norm(ref[:, :npw], axis=1)))
+            assert err <= TOL, "%s terms=%d k=%d: %.3e" % (name, terms, ik, err)
+    plan.set_option("terms", 7)
+    plan.set_vector_potential(None)
+    assert np.array_equal(gpu_apply(plan, psi), plain)
+    plan.destroy()
+
+
 def test_host_api_band_groups():
     """dft_apply_h_host cuts one k-point's bands into groups whose copies overlap the neighbours' kernels;
     the result must not depend on the grouping."""

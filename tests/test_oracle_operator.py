@@ -92,3 +92,28 @@ def test_chebyshev_filter_pins():
     assert np.array_equal(oracle.chebyshev_filter(c, 0, kg, ig, kin, psi, 0, cen, e), psi)
     h1 = oracle.apply_h(c, 0, kg, ig, kin, psi)
     assert rel_err(oracle.chebyshev_filter(c, 0, kg, ig, kin, psi, 1, cen, e), (h1 - cen * psi) / e) < 1e-15
+
+
+def test_velocity_gauge_kinetic_pins():
+    """1/2|k+G+A|^2 (PAPER.md :340): A = 0 gives the sphere's kin; A = 2 pi Bm^T d for an integer triple d is the
+    kinetic energy of the plane wave m + d (k shifted by a reciprocal vector); cubic closed form; and with V = 0,
+    D = 0 the operator is that diagonal."""
+    import oracle
+    from util import config, sphere, rand_c, rel_err
+    for name in ("c0", "aniso"):
+        c = config(name); kg, ig, kin = sphere(name)
+        k = np.asarray(c["kpt"][0], float)
+        assert np.max(np.abs(oracle.kin_vecpot(c["rprimd"], k, kg, [0, 0, 0]) - kin)) < 1e-13 * kin.max()
+        bm, _ = oracle.lattice(c["rprimd"])
+        d = np.array([1, -2, 3])
+        a = 2 * np.pi * d @ bm
+        ref = np.array([oracle.kin_of(c["rprimd"], k, m + d) for m in kg])
+        assert np.max(np.abs(oracle.kin_vecpot(c["rprimd"], k, kg, a) - ref)) < 1e-12 * ref.max()
+    c = config("c1m"); kg, ig, kin = sphere("c1m")
+    L = c["rprimd"][0][0]; a = np.array([0.3, -0.1, 0.25])
+    q = 2 * np.pi / L * (kg + np.asarray(c["kpt"][0])[None, :]) + a[None, :]
+    ka = oracle.kin_vecpot(c["rprimd"], c["kpt"][0], kg, a)
+    assert np.max(np.abs(ka - 0.5 * np.sum(q * q, axis=1))) < 1e-13 * ka.max()
+    psi = rand_c((2, len(kg)), 4)
+    out = oracle.apply_h(c, 0, kg, ig, ka, psi, terms=oracle.KIN)
+    assert rel_err(out, ka[None, :] * psi) < 1e-15

@@ -296,6 +296,22 @@ def main():
         del work, tmp
         torch.cuda.empty_cache()
 
+    # ---- context figure: density accumulation n(r) = sum w |psi(r)|^2 (Eq. 6) over all bands
+    if args.cheb_degree > 0 and world == 1:
+        wts = np.ones((plan.nkpt, nband))
+        rho = plan.accumulate_density(psi, wts)
+        torch.cuda.synchronize()
+        d0 = torch.cuda.Event(enable_timing=True); d1 = torch.cuda.Event(enable_timing=True)
+        d0.record(); plan.accumulate_density(psi, wts, rho); d1.record()
+        torch.cuda.synchronize()
+        dms = d0.elapsed_time(d1)
+        n1_, n2_, n3_ = plan.ngfft
+        dbytes = sum(nband * (16.0 * g_["npw"] + 2 * 16.0 * g_["ncol"] * n1_ + 2 * 16.0 * n1_ * n2_ * g_["nplane"]) for g_ in geo)
+        line["density"] = {"ms": dms, "bands_per_s": units / (dms * 1e-3), "hbm_frac": dbytes / (dms * 1e-3) / 1e9 / hbm_gbs,
+                           "bytes_model": "per band a + 2b + 2c (scatter read, T1 write+read, T2 write+read), DESIGN.md 7",
+                           "api": "dft_accumulate_density"}
+        del rho
+
     # ---- e2e: same metric through dft_apply_h_host, host<->device copies inside the timed region
     if not args.no_e2e:
         psi_h = torch.empty(psi.shape, dtype=psi.dtype, pin_memory=True)

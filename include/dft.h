@@ -134,6 +134,15 @@ int dft_apply_s(dft_plan *p, const double *psi, double *spsi, int32_t nband, voi
  * atom.  GEMM-1 and the fixed-order split-K reduction only; enqueues on `stream`.                 */
 int dft_get_cprj(dft_plan *p, const double *psi, double *cprj, int32_t nband, void *stream);
 
+/* Density accumulation (Eq. 6, :140: n(r) = sum_nk w_nk |psi_nk(r)|^2; Eq. 3, :110 with
+ * w_nk = 2 w_k f_nk):  rho[j] += sum_k sum_n weights[k][n] |psi_nk(r_j)|^2  on the FFT box, with
+ * psi_nk(r_j) = sum_G c_nk(G) exp(+2 pi i G.r_j) (the unnormalised G->r transform of dft_apply_h; fold 1/Omega
+ * and occupations into the weights).  psi: DEVICE [nkpt][nband][mpw]; weights: HOST [nkpt][nband], copied before
+ * the call returns (one synchronisation of `stream`); rho: DEVICE [n3][n2][n1] doubles, i1 fastest, ACCUMULATED into (zero it first).  Runs the
+ * scatter + x and y passes of dft_apply_h and the forward half of its z pass, summing over bands in registers
+ * (no atomics, fixed order).  DFT_ERR_UNSUPPORTED for box lengths without a two-radix factorisation.  */
+int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights, double *rho, int32_t nband, void *stream);
+
 /* Velocity-gauge vector potential (PAPER.md :340: in RT-TDDFT "the velocity gauge changes only the kinetic
  * term", -i grad -> -i grad + A(t)): while set, the kinetic diagonal of dft_apply_h / dft_chebyshev_filter is
  * 1/2 |k + G + A|^2 with A = a_cart[3] (HOST, Cartesian, atomic units).  The sphere (defined at A = 0) and

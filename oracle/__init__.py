@@ -197,6 +197,18 @@ def kin_vecpot(rprimd, k, kg, a_cart):
     return 0.5 * np.sum(q * q, axis=1)
 
 
+def density(ngfft, igfft, psi, weights, method=2):
+    """sum_b weights[b] |psi_b(r_j)|^2 on the FFT box, [n3][n2][n1] (Eq. 6, :140), with
+    psi_b(r_j) = sum_G c_b(G) exp(+2 pi i G.r_j) by the oracle's own G->r transform (orc_g2r: scatter + T1/T2 DFT)."""
+    n1, n2, n3 = [int(v) for v in ngfft]
+    rho = np.zeros((n3, n2, n1))
+    npw = len(igfft)
+    for c, w in zip(np.asarray(psi, np.complex128), np.asarray(weights, float)):
+        box = g2r(ngfft, igfft, c[:npw], method)
+        rho += w * (box.real ** 2 + box.imag ** 2)
+    return rho
+
+
 def cprj(cfg, ik, kg, psi):
     """<p_a,i|psi_b> (PAPER.md :477 "coefficients c_a,i,n,k"), [nproj][nband] complex: step 1 of Eq. 26 (:470),
     as the streamed loops of orc_nonlocal_apply compute it."""

@@ -554,6 +554,84 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
   }
 }
 
+// ---- density (Eq. 6, :140: n(r) = sum_nk w_nk |psi_nk(r)|^2): the forward half of pass C, then
+//      rho(r) += sum_b w_b |psi_b(r)|^2.  A CTA owns WHOLE groups (one flat-xy tile, all bands of the launch), keeps the
+//      running sum over the bands in registers and adds it to rho once per group: no atomics, fixed summation order.
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_density_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, const double *__restrict__ wgt,
+                    double *__restrict__ rho, RingParams Q) {
+  constexpr int NS = imax(R1, R2);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int XT = Q.XT, KSa = pad8(R2 * XT, XT);
+  unsigned char *stages = smem_raw;
+  cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
+  cplx *tws = sm + R1 * KSa;
+  uint64_t *full = reinterpret_cast<uint64_t *>(tws + G.n3);
+  const int t = threadIdx.x, px = t % XT, s = t / XT;
+  for (int i = t; i < G.n3; i += blockDim.x) tws[i] = __ldg(G.tw3 + i);
+  if (t == 0) {
+    for (int i = 0; i < Q.S; i++) mbar_init(&full[i], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int g0 = (int)(((int64_t)Q.nxt * blockIdx.x) / gridDim.x), g1 = (int)(((int64_t)Q.nxt * (blockIdx.x + 1)) / gridDim.x);
+  const int nmine = (g1 - g0) * Q.nb;
+  const size_t pstride = (size_t)G.n2 * G.n1;
+  int b = 0, g = g0;
+  int ib = 0, ig = g0, ist = 0;
+  auto issue = [&]() {
+    mbar_expect_tx(&full[ist], Q.box_bytes);
+    tma_load_3d(stages + (size_t)ist * Q.stage_stride, &mapT2, &full[ist], 2 * ig * XT, 0, ib);
+    if (++ist == Q.S) ist = 0;
+    if (++ib == Q.nb) { ib = 0; ig++; }
+  };
+  if (t == 0)
+    for (int j = 0; j < Q.S - 1 && j < nmine; j++) issue();
+  int st = 0; uint32_t ph = 0;
+  double acc[R2];
+#pragma unroll
+  for (int k2 = 0; k2 < R2; k2++) acc[k2] = 0.0;
+  for (int it = 0; it < nmine; it++) {
+    if (t == 0 && it + Q.S - 1 < nmine) issue();
+    const cplx *in = reinterpret_cast<const cplx *>(stages + (size_t)st * Q.stage_stride) + px;
+    mbar_wait(&full[st], ph);
+    cplx v[NS];
+    if (s < R2) {
+#pragma unroll
+      for (int j1 = 0; j1 < R1; j1++) {
+        int p = run_map(G.zrun, s + R2 * j1);
+        v[j1] = p >= 0 ? in[p * XT] : make_double2(0.0, 0.0);
+      }
+      Dft<R1, +1>::run(v);
+#pragma unroll
+      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], tws[s * k1]);
+#pragma unroll
+      for (int k1 = 0; k1 < R1; k1++) sm[k1 * KSa + s * XT + px] = v[k1];
+    }
+    __syncthreads();
+    if (s < R1) {
+#pragma unroll
+      for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KSa + j2 * XT + px];
+      Dft<R2, +1>::run(v);
+      const double wb = __ldg(wgt + b);
+#pragma unroll
+      for (int k2 = 0; k2 < R2; k2++) acc[k2] += wb * (v[k2].x * v[k2].x + v[k2].y * v[k2].y);   // psi(r) at z = s + R1 k2
+    }
+    __syncthreads();   // the exchange buffer is rewritten by the next tile
+    if (++st == Q.S) { st = 0; ph ^= 1; }
+    if (++b == Q.nb) {
+      const size_t xy = (size_t)g * XT + px;
+      if (s < R1 && xy < pstride) {
+        double *dst = rho + (size_t)s * pstride + xy;
+#pragma unroll
+        for (int k2 = 0; k2 < R2; k2++) { dst[(size_t)(R1 * k2) * pstride] += acc[k2]; acc[k2] = 0.0; }
+      }
+      b = 0; g++;
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // host side: pair table, launch geometry
 // ------------------------------------------------------------------------------------------
@@ -828,6 +906,81 @@ int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int
     if (rc) { if (rc == DFT_ERR_UNSUPPORTED) set_error("batched FFT pass %d cannot be launched", pass); return rc; }
   }
   return DFT_OK;
+}
+
+int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, void *T1, void *T2, int64_t t1_band,
+                int64_t t2_band, int nb, cudaStream_t st);
+
+template <int R1, int R2>
+static int launch_density(dft_plan *p, const Fft2Geom &G, cplx *T2, const double *wgt, double *rho, int nb, cudaStream_t st) {
+  constexpr int NS = imax(R1, R2);
+  if (!p->encode_fn || G.nplane > 256) return DFT_ERR_UNSUPPORTED;
+  int XT = (F2_THREADS / NS) & ~7;
+  if (XT < 8) return DFT_ERR_UNSUPPORTED;
+  const int64_t nxy = (int64_t)G.n1 * G.n2;
+  if (XT > nxy) XT = (int)((nxy + 1) & ~1LL);
+  RingParams Q;
+  Q.XT = XT; Q.nxt = (int)((nxy + XT - 1) / XT); Q.nb = nb; Q.ntiles = 0;
+  Q.box_bytes = (uint32_t)((size_t)G.nplane * XT * 16);
+  Q.stage_stride = (Q.box_bytes + 127u) & ~127u;
+  const size_t fixed = sizeof(cplx) * (size_t)R1 * pad8(R2 * XT, XT) + sizeof(cplx) * (size_t)G.n3 + 8 * 8;
+  const size_t budget2 = (size_t)(p->smem_per_sm / 2) - 1024, budget1 = (size_t)p->smem_optin;
+  int S = 0, per_sm = 2;
+  for (int sg = 4; sg >= 2 && !S; sg--)
+    if (fixed + (size_t)sg * Q.stage_stride <= budget2) S = sg;
+  if (!S) {
+    per_sm = 1;
+    for (int sg = 4; sg >= 2 && !S; sg--)
+      if (fixed + (size_t)sg * Q.stage_stride <= budget1) S = sg;
+  }
+  if (!S) return DFT_ERR_UNSUPPORTED;
+  Q.S = S;
+  const size_t smem = fixed + (size_t)S * Q.stage_stride;
+  CUtensorMap map;
+  cuuint64_t dims[3] = {2 * (cuuint64_t)nxy, (cuuint64_t)G.nplane, (cuuint64_t)nb};
+  cuuint64_t strides[2] = {(cuuint64_t)nxy * 16, (cuuint64_t)G.t2_band * 16};
+  cuuint32_t box[3] = {2 * (cuuint32_t)XT, (cuuint32_t)G.nplane, 1};
+  int rc;
+  if ((rc = encode_map(p, &map, T2, 3, dims, strides, box))) return rc;
+  if ((rc = set_smem(fft2_density_kernel<R1, R2>, smem))) return rc;
+  int grid = per_sm * p->sm_count;
+  if (grid > Q.nxt) grid = Q.nxt;
+  fft2_density_kernel<R1, R2><<<grid, XT * NS, smem, st>>>(map, G, wgt, rho, Q);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+// rho(r) += sum_b wgt[b] |psi_b(r)|^2 for nb bands of k-point ik: passes A and B as in H psi, then the density kernel.
+// Only the register path has it: DFT_ERR_UNSUPPORTED for box lengths without a two-radix factorisation.
+int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st) {
+  const KPoint &kp = p->kp[ik];
+  if (kp.npw == 0 || nb == 0) return DFT_OK;
+  int r1, r2;
+  for (int c = 0; c < 3; c++)
+    if (!fft2_pair(p->n[c], &r1, &r2) || !kp.runs_ok) {
+      set_error("dft_accumulate_density needs box lengths with a two-radix factorisation (got %d)", p->n[c]);
+      return DFT_ERR_UNSUPPORTED;
+    }
+  int64_t t1b = ((int64_t)kp.ncol * p->n[0] * 16 + 255) / 256 * 256, t2b = ((int64_t)kp.nplane * p->n[1] * p->n[0] * 16 + 255) / 256 * 256;
+  cplx *T1 = reinterpret_cast<cplx *>(ws);
+  cplx *T2 = reinterpret_cast<cplx *>(reinterpret_cast<char *>(ws) + t1b * nb);
+  int rc;
+  for (int pass = 0; pass < 2; pass++) {
+    phase_begin(p, pass, st);
+    rc = fft2_launch(p, ik, pass, psi, nullptr, T1, T2, t1b / 16, t2b / 16, nb, st);
+    phase_end(p, pass, st, 1);
+    if (rc) return rc;
+  }
+  Fft2Geom G = make_geom2(p, ik, t1b / 16, t2b / 16);
+  fft2_pair(p->n[2], &r1, &r2);
+  rc = DFT_ERR_UNSUPPORTED;
+  phase_begin(p, 2, st);
+#define X(a, b) if (r1 == (a) && r2 == (b)) rc = launch_density<a, b>(p, G, T2, wgt_dev, rho, nb, st);
+  FFT2_PAIRS(X)
+#undef X
+  phase_end(p, 2, st, 1);
+  if (rc == DFT_ERR_UNSUPPORTED) set_error("density kernel: tile does not fit (nplane = %d)", kp.nplane);
+  return rc;
 }
 
 // pass: 0 A, 1 B, 2 C, 3 B^-1, 4 A^-1.  The pair is that of the axis the pass transforms.

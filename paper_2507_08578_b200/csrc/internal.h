@@ -130,6 +130,7 @@ struct dft_plan {
   int host_groups = 4;     // dft_apply_h_host: band groups whose copies overlap the kernels of their neighbours
   // TMA
   void *encode_fn = nullptr;   // cuTensorMapEncodeTiled
+  double *d_wgt = nullptr; int64_t wgt_count = 0;    // device copy of the band weights of dft_accumulate_density
   void *d_geom2 = nullptr;    // device array of per-k-point FFT geometry (fft2.cu, built at first batched call)
   int sm_count = 148;
   int smem_per_sm = 233472, smem_optin = 232448;   // bytes of shared memory per SM / per CTA (opt-in), from the device
@@ -170,6 +171,9 @@ struct Recurrence {
 // several k-points per launch (plain register kernels with blockIdx.y = k-point)
 bool fft2_batch_ok(const dft_plan *p);
 int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int nband_total, void *ws, cudaStream_t st);
+
+// rho(r) += sum_b wgt[b] |psi_b(r)|^2 (device wgt [nb]); forward passes A, B and the density kernel
+int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st);
 
 // --- nonlocal.cu (K3) ---------------------------------------------------------------------
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi

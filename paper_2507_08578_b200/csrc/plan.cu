@@ -59,7 +59,7 @@ static void destroy_plan(dft_plan *p) {
   for (auto &k : p->kp) free_kpoint(k);
   cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
   cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
-  cudaFree(p->d_geom2); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
@@ -525,6 +525,37 @@ int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, 
   }
   p->last_launches = launches;
   if (buf[iy] != psi) DFT_CUDA_CHECK(cudaMemcpyAsync(psi, buf[iy], n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  return DFT_OK;
+  DFT_GUARD_END
+}
+
+int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights, double *rho, int32_t nband, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  p->last_launches = 0;
+  if (nband == 0 || p->mpw == 0 || p->nkpt == 0) return DFT_OK;
+  if (!psi || !weights || !rho) { set_error("null psi/weights/rho"); return DFT_ERR_INVALID_ARG; }
+  if ((uintptr_t)psi & 15) { set_error("psi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t nw = (int64_t)p->nkpt * nband;
+  if (nw > p->wgt_count) {
+    if (p->d_wgt) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_wgt); p->d_wgt = nullptr; p->wgt_count = 0; }
+    if (cudaMalloc(&p->d_wgt, sizeof(double) * nw) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the weight array"); return DFT_ERR_ALLOC; }
+    p->wgt_count = nw;
+  }
+  // weights are HOST memory and must be consumed before the call returns: copy on the stream, then wait for it
+  DFT_CUDA_CHECK(cudaMemcpyAsync(p->d_wgt, weights, sizeof(double) * nw, cudaMemcpyHostToDevice, st));
+  DFT_CUDA_CHECK(cudaStreamSynchronize(st));
+  int chunk; void *ws; int rc;
+  if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
+  const size_t band_stride = (size_t)p->mpw * 2;
+  for (int ik = 0; ik < p->nkpt; ik++)
+    for (int b0 = 0; b0 < nband; b0 += chunk) {
+      int nb = nband - b0 < chunk ? nband - b0 : chunk;
+      size_t off = ((size_t)ik * nband + b0) * band_stride;
+      if ((rc = fft2_density(p, ik, psi + off, p->d_wgt + (size_t)ik * nband + b0, rho, nb, ws, st))) return rc;
+    }
   return DFT_OK;
   DFT_GUARD_END
 }

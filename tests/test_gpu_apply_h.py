@@ -215,6 +215,27 @@ def test_velocity_gauge_kinetic(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c0", "c1m", "aniso", "c3k2"])
+def test_density_accumulation(name):
+    """dft_accumulate_density (Eq. 6, :140) against the oracle, accumulating over k-points, in two calls
+    (rho is added to), with a band chunk that leaves a ragged tail."""
+    cfg, plan, sph = _setup(name, nband=7)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    rng = np.random.default_rng(9)
+    w = rng.uniform(0.1, 2.0, size=(plan.nkpt, 7))
+    plan.set_option("band_chunk", 3)
+    tpsi = torch.as_tensor(psi, device="cuda")
+    rho = plan.accumulate_density(tpsi, w)
+    rho = plan.accumulate_density(tpsi, 0.5 * w, rho)
+    torch.cuda.synchronize()
+    ref = np.zeros(rho.shape)
+    for ik, (kg, ig, kin) in enumerate(sph):
+        ref += 1.5 * oracle.density(cfg["ngfft"], ig, psi[ik], w[ik], method=1 if name in ("c0", "aniso") else 2)
+    got = rho.cpu().numpy()
+    assert np.max(np.abs(got - ref)) <= 1e-12 * ref.max(), np.max(np.abs(got - ref)) / ref.max()
+    plan.destroy()
+
+
 def test_host_api_band_groups():
     """dft_apply_h_host cuts one k-point's bands into groups whose copies overlap the neighbours' kernels;
     the result must not depend on the grouping."""

@@ -113,3 +113,34 @@ def test_tight_box_heavy_wraparound():
     t0 = psi @ oracle.dense_h(c, 0, kg, kin, terms=oracle.LOC).T
     t2 = oracle.apply_h(c, 0, kg, ig, kin, psi, terms=oracle.LOC)
     assert rel_err(t2, t0) < 1e-13
+
+
+def test_density_pins():
+    """n(r) = sum_b w_b |psi_b(r)|^2 (Eq. 6, :140): Parseval (mean over the box = sum_b w_b <psi_b|psi_b>),
+    one plane wave -> constant w, two plane waves -> w (|a|^2 + |b|^2 + 2 Re(conj(a) b e^{2 pi i (m_b - m_a).j/n})),
+    and the numpy ifftn reduction."""
+    import oracle
+    from util import config, sphere, rand_c
+    for name in ("c0", "aniso"):
+        c = config(name); kg, ig, kin = sphere(name)
+        n = c["ngfft"]; N = int(np.prod(n)); npw = len(ig)
+        psi = rand_c((3, npw), 31); w = np.array([0.7, 1.3, 2.0])
+        rho = oracle.density(n, ig, psi, w, method=1)
+        assert rho.shape == (n[2], n[1], n[0]) and rho.min() >= 0
+        assert abs(rho.sum() / N - np.sum(w * np.sum(np.abs(psi) ** 2, axis=1))) < 1e-12 * rho.sum() / N
+        ref = np.zeros_like(rho)
+        for cb, wb in zip(psi, w):
+            box = np.zeros(N, complex); box[ig] = cb
+            r = np.fft.ifftn(box.reshape(n[2], n[1], n[0])) * N
+            ref += wb * np.abs(r) ** 2
+        assert np.max(np.abs(rho - ref)) < 1e-12 * ref.max()
+        assert np.max(np.abs(oracle.density(n, ig, psi, w, method=2) - rho)) < 1e-12 * rho.max()
+        one = np.zeros((1, npw), complex); one[0, 5] = 0.6 - 0.8j
+        assert np.max(np.abs(oracle.density(n, ig, one, [2.5]) - 2.5)) < 1e-13
+        two = np.zeros((1, npw), complex); a, b = 0.5 + 0.2j, -0.3 + 0.9j
+        two[0, 3] = a; two[0, 11] = b
+        dm = kg[11] - kg[3]
+        j3, j2, j1 = np.meshgrid(np.arange(n[2]), np.arange(n[1]), np.arange(n[0]), indexing="ij")
+        ph = np.exp(2j * np.pi * (dm[0] * j1 / n[0] + dm[1] * j2 / n[1] + dm[2] * j3 / n[2]))
+        ref2 = 1.5 * (abs(a) ** 2 + abs(b) ** 2 + 2 * np.real(np.conj(a) * b * ph))
+        assert np.max(np.abs(oracle.density(n, ig, two, [1.5]) - ref2)) < 1e-13

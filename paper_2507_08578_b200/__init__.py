@@ -278,7 +278,7 @@ class Plan:
         """psi: torch complex128 CUDA tensor [nkpt][nband][mpw] (or [nband][mpw] when nkpt = 1)."""
         import torch
         assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous()
-        assert psi.shape[-1] == self.mpw and psi.numel() % (self.nkpt * self.mpw) == 0
+        assert psi.shape[-1] == self.mpw and (self.mpw == 0 or psi.numel() % (self.nkpt * self.mpw) == 0)
         nband = psi.numel() // (self.nkpt * self.mpw) if self.mpw else 0
         if hpsi is None:
             hpsi = torch.empty_like(psi)

@@ -236,6 +236,38 @@ def test_density_accumulation(name):
     plan.destroy()
 
 
+def test_degenerate_inputs():
+    """Edge cases of the method: no bands, one plane wave (ecut below the first shell), a k-point whose sphere is empty,
+    and error codes for bad arguments."""
+    import paper_2507_08578_b200 as dft
+    cfg, plan, sph = _setup("c0")
+    empty = torch.zeros((1, 0, plan.mpw), dtype=torch.complex128, device="cuda")
+    assert plan.apply_h(empty).shape == (1, 0, plan.mpw) and plan.last_launches() == 0
+    assert plan.apply_s(empty).numel() == 0 and plan.get_cprj(empty).numel() == 0
+    plan.chebyshev_filter(empty, 3, 1.0, 2.0)
+    with pytest.raises(dft.DftError) as ei:
+        plan.set_option("no_such_option", 1)
+    assert ei.value.code == dft.DFT_ERR_INVALID_ARG
+    with pytest.raises(dft.DftError):
+        plan.chebyshev_filter(torch.zeros((1, 2, plan.mpw), dtype=torch.complex128, device="cuda"), 2, 0.0, 0.0)   # halfwidth must be > 0
+    plan.destroy()
+    # one plane wave at Gamma: H is the 1x1 matrix kin(0) + mean(V) + sum |p(0)|^2-terms; compare with the oracle
+    cfg, plan, sph = _setup("c0", ecut=0.05)
+    assert plan.npw[0] == 1
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    assert band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, method=1)) <= TOL
+    plan.destroy()
+    # k = (1/2,1/2,1/2) of the FCC cell with a cutoff below its lowest |k+G|^2/2: the sphere is empty, nothing to do
+    cfg = synth.make_config("c0", ecut=0.05, kpt=[[0.5, 0.5, 0.5]])
+    okg, oig, okin = oracle.sphere(cfg["rprimd"], cfg["kpt"][0], cfg["ecut"], cfg["ngfft"])
+    assert len(oig) == 0
+    plan = make_plan(cfg)
+    assert plan.npw[0] == 0 and plan.mpw == 0
+    out = plan.apply_h(torch.zeros((1, 4, 0), dtype=torch.complex128, device="cuda"))
+    assert out.numel() == 0
+    plan.destroy()
+
+
 def test_host_api_band_groups():
     """dft_apply_h_host cuts one k-point's bands into groups whose copies overlap the neighbours' kernels;
     the result must not depend on the grouping."""

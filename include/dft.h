@@ -103,7 +103,7 @@ int dft_set_vloc(dft_plan *p, const double *V_r, void *stream);
 int dft_set_workspace(dft_plan *p, void *dev_ptr, int64_t bytes);
 
 /* Options: "band_chunk" (bands per FFT pass launch, > 0), "terms" (bit 0 kinetic, bit 1 local,
- * bit 2 non-local; default 7), "splitk" (GEMM-1 K splits, 0 = automatic), "host_groups" (dft_apply_h_host only: band groups, default 4,
+ * bit 2 non-local, bit 3 meta-GGA term; default 15), "splitk" (GEMM-1 K splits, 0 = automatic), "host_groups" (dft_apply_h_host only: band groups, default 4,
  * whose host<->device copies overlap the kernels of the neighbouring groups), "gemm_3m" (1 = default: three real
  * products per complex multiply-add in the projector GEMMs, 0 = four; same result up to rounding), "fft_path" (0 = automatic:
  * register-resident two-stage transforms where the box length factorises, their strided passes fed by a
@@ -142,6 +142,14 @@ int dft_get_cprj(dft_plan *p, const double *psi, double *cprj, int32_t nband, vo
  * scatter + x and y passes of dft_apply_h and the forward half of its z pass, summing over bands in registers
  * (no atomics, fixed order).  DFT_ERR_UNSUPPORTED for box lengths without a two-radix factorisation.  */
 int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights, double *rho, int32_t nband, void *stream);
+
+/* Meta-GGA term of the Hamiltonian (Eq. 8, :152: "- 1/2 div( v_tau(r) grad )", v_tau = d f_xc / d tau, Eq. 9):
+ * once set, dft_apply_h adds  1/2 sum_{d=x,y,z} (k+G)_d FFT^-1[ v_tau(r) FFT[ (k+G')_d psi ] ]  (three more local
+ * applications whose diagonal factors are fused into the scatter and gather passes).  vtau_r: DEVICE
+ * [n3][n2][n1] doubles like V_r of dft_set_vloc, copied on `stream`; NULL switches the term off.  Option "terms"
+ * bit 3 (value 8) gates it.  Needs box lengths with a two-radix factorisation (else dft_apply_h returns
+ * DFT_ERR_UNSUPPORTED while the term is on).                                                       */
+int dft_set_vtau(dft_plan *p, const double *vtau_r, void *stream);
 
 /* Velocity-gauge vector potential (PAPER.md :340: in RT-TDDFT "the velocity gauge changes only the kinetic
  * term", -i grad -> -i grad + A(t)): while set, the kinetic diagonal of dft_apply_h / dft_chebyshev_filter is

@@ -209,6 +209,24 @@ def density(ngfft, igfft, psi, weights, method=2):
     return rho
 
 
+def apply_mgga(cfg, ik, kg, igfft, psi, vtau, method=2):
+    """Meta-GGA term of Eq. 8 (PAPER.md :152), -1/2 div(v_tau grad psi), on the plane-wave coefficients of
+    psi(r) = sum_G c(G) e^{i(k+G).r}: grad -> i q with q = k + G Cartesian (2 pi (k + m) Bm, reading 1), so
+    (H_tau c)(G) = 1/2 sum_d q_d(G) [Loc_{v_tau} (q_d c)](G), Loc_v = the local operator of reading 4 with V := v_tau
+    (the oracle's own scatter / DFT / multiply / DFT / gather, orc_apply_h with terms = LOC)."""
+    psi = np.ascontiguousarray(psi, np.complex128)
+    npw = len(kg)
+    bm, _ = lattice(cfg["rprimd"])
+    q = 2.0 * np.pi * (np.asarray(kg, float) + np.asarray(cfg["kpt"][ik], float)[None, :]) @ np.asarray(bm, float).reshape(3, 3)
+    out = np.zeros_like(psi)
+    zero = np.zeros(npw)
+    for d in range(3):
+        x = psi.copy(); x[:, :npw] *= q[None, :, d]
+        y = apply_h(cfg, ik, kg, igfft, zero, x, method=method, terms=LOC, vloc=vtau)
+        out[:, :npw] += 0.5 * q[None, :, d] * y[:, :npw]
+    return out
+
+
 def cprj(cfg, ik, kg, psi):
     """<p_a,i|psi_b> (PAPER.md :477 "coefficients c_a,i,n,k"), [nproj][nband] complex: step 1 of Eq. 26 (:470),
     as the streamed loops of orc_nonlocal_apply compute it."""

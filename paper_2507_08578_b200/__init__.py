@@ -34,6 +34,7 @@ PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather
 SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_get_cprj", "dft_chebyshev_filter",
            "dft_set_vector_potential", "dft_accumulate_density",
+           "dft_set_vtau",
            "dft_set_vloc", "dft_set_workspace", "dft_plan_set_option", "dft_apply_h", "dft_apply_h_host",
            "dft_plan_last_launches", "dft_plan_set_timing", "dft_plan_phase_ms", "dft_plan_destroy", "dft_last_error")
 
@@ -82,6 +83,7 @@ def lib():
     L.dft_apply_h_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
     L.dft_set_sij.argtypes = [C.c_void_p, _dp]
     L.dft_set_vector_potential.argtypes = [C.c_void_p, _dp]
+    L.dft_set_vtau.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.dft_accumulate_density.argtypes = [C.c_void_p, C.c_void_p, _dp, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_chebyshev_filter.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                        C.c_void_p]
@@ -203,6 +205,10 @@ def dft_accumulate_density(plan, psi_dev_ptr, weights, rho_dev_ptr, nband, strea
     _check(lib().dft_accumulate_density(plan, psi_dev_ptr, _d(_f64(weights)), rho_dev_ptr, nband, stream))
 
 
+def dft_set_vtau(plan, vtau_dev_ptr, stream=0):
+    _check(lib().dft_set_vtau(plan, vtau_dev_ptr, stream))
+
+
 def dft_set_vector_potential(plan, a_cart):
     _check(lib().dft_set_vector_potential(plan, None if a_cart is None else _d(_f64(a_cart))))
 
@@ -322,6 +328,15 @@ class Plan:
         assert w.size == self.nkpt * nband
         dft_accumulate_density(self.h, psi.data_ptr(), w, rho.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
         return rho
+
+    def set_vtau(self, v):
+        """Meta-GGA v_tau(r): torch float64 CUDA tensor with n1*n2*n3 elements ([n3][n2][n1]); None switches the term off."""
+        import torch
+        if v is None:
+            dft_set_vtau(self.h, None)
+            return
+        assert v.is_cuda and v.dtype == torch.float64 and v.is_contiguous() and v.numel() == int(np.prod(self.ngfft))
+        dft_set_vtau(self.h, v.data_ptr(), torch.cuda.current_stream().cuda_stream)
 
     def set_vector_potential(self, a_cart):
         """Velocity gauge: kinetic term 1/2|k+G+A|^2 (A Cartesian, a.u.); None switches it off."""

@@ -309,11 +309,12 @@ static int set_attrs() {
   return DFT_OK;
 }
 
-int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb, void *ws, cudaStream_t st) {
+int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb, void *ws, cudaStream_t st,
+                   const FftExtra *extra) {
   int rc = set_attrs();
   if (rc) return rc;
   const KPoint &kp = p->kp[ik];
-  if (kp.npw == 0 || nb == 0) return zero_fill(hpsi, (int64_t)nb * p->mpw * 2, st);
+  if (kp.npw == 0 || nb == 0) return (extra && extra->accumulate) ? DFT_OK : zero_fill(hpsi, (int64_t)nb * p->mpw * 2, st);
   FftGeom G = make_geom(p, ik);
   int64_t t1b = ((int64_t)G.t1_band * 16 + 255) / 256 * 256;
   cplx *T1 = reinterpret_cast<cplx *>(ws);
@@ -331,11 +332,15 @@ int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb,
   // codelet radices and the sphere's occupied sets are runs; otherwise the generic Stockham kernel
   bool fast[3];
   for (int c = 0; c < 3; c++) fast[c] = p->fft_path != 1 && kp.runs_ok && fft2_pair(p->n[c], nullptr, nullptr);
+  if (extra && !(fast[0] && fast[1] && fast[2])) {
+    set_error("this term needs box lengths with a two-radix factorisation (register FFT path)");
+    return DFT_ERR_UNSUPPORTED;
+  }
   const int axis_of[5] = {0, 1, 2, 1, 0};
   for (int pass = 0; pass < 5; pass++) {
     phase_begin(p, pass, st);
     if (fast[axis_of[pass]]) {
-      if ((rc = fft2_launch(p, ik, pass, psi, hpsi, T1, T2, G.t1_band, G.t2_band, nb, st))) return rc;
+      if ((rc = fft2_launch(p, ik, pass, psi, hpsi, T1, T2, G.t1_band, G.t2_band, nb, st, extra))) return rc;
     } else if (pass == 0) fft_pass_a_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, cpsi, T1);
     else if (pass == 1) fft_pass_b_kernel<+1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
     else if (pass == 2) fft_pass_c_kernel<<<gc, FFT_THREADS, sm_c, st>>>(G, T2, p->d_vloc);

@@ -64,7 +64,8 @@ struct Fft2Batch {
 // ---- pass A: sphere -> x-lines (type I).  block = lpc lines x NS slots, slot fastest; grid = nb * ntile
 template <int R1, int R2, bool BATCH>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *__restrict__ T1, int lpc, int ntile) {
+fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *__restrict__ T1, int lpc, int ntile,
+                  const double *__restrict__ pre) {
   const Fft2Geom G = BATCH ? B.Gs[blockIdx.y] : G0;
   if (BATCH) { psi += (size_t)blockIdx.y * B.ks_psi; T1 += (size_t)blockIdx.y * B.ks_t1; }
   constexpr int NS = imax(R1, R2), KS = R2 | 1, LS = pad8(R1 * KS, NS);
@@ -82,6 +83,7 @@ fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *
     for (int j1 = 0; j1 < R1; j1++) {
       int g = ok ? run_map(r, s + R2 * j1) : -1;
       v[j1] = g >= 0 ? src[g] : make_double2(0.0, 0.0);
+      if (pre && g >= 0) v[j1] = cscale(v[j1], __ldg(pre + g));     // diagonal factor in G space before the transform
     }
     Dft<R1, +1>::run(v);
 #pragma unroll
@@ -105,7 +107,8 @@ fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *
 // ---- pass A^-1: x-lines -> sphere (type II) + zero the pad entries ipw >= npw of the band
 template <int R1, int R2, bool BATCH>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-fft2_a_inv_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ T1, cplx *__restrict__ hpsi, int lpc, int ntile) {
+fft2_a_inv_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ T1, cplx *__restrict__ hpsi, int lpc, int ntile,
+                  const double *__restrict__ post, int accumulate) {
   const Fft2Geom G = BATCH ? B.Gs[blockIdx.y] : G0;
   if (BATCH) { hpsi += (size_t)blockIdx.y * B.ks_psi; T1 += (size_t)blockIdx.y * B.ks_t1; }
   constexpr int NS = imax(R1, R2), KS = R1 | 1, LS = pad8(R2 * KS, NS);
@@ -136,10 +139,14 @@ fft2_a_inv_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ T1, cplx *_
 #pragma unroll
     for (int d = 0; d < R1; d++) {
       int g = ok ? run_map(r, s + R2 * d) : -1;
-      if (g >= 0) dst[g] = v[d];
+      if (g >= 0) {
+        cplx o = post ? cscale(v[d], __ldg(post + g)) : v[d];        // diagonal factor in G space after the transform
+        if (accumulate) { cplx h = dst[g]; o.x += h.x; o.y += h.y; }
+        dst[g] = o;
+      }
     }
   }
-  if (tile == ntile - 1)
+  if (tile == ntile - 1 && !accumulate)
     for (int g = G.npw + t; g < G.mpw; g += blockDim.x) dst[g] = make_double2(0.0, 0.0);
 }
 
@@ -773,7 +780,7 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
 
 template <int R1, int R2>
 static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi, cplx *hpsi, cplx *T1, cplx *T2, const double *vloc,
-                       int nb, int hb, cudaStream_t st) {
+                       int nb, int hb, cudaStream_t st, const FftExtra &X) {
   constexpr int NS = imax(R1, R2);
   int rc;
   if (pass >= 1 && pass <= 3 && p->fft_path == 0) {
@@ -790,10 +797,10 @@ static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi
     if (grid > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
     if (pass == 0) {
       if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, false>, sm))) return rc;
-      fft2_a_fwd_kernel<R1, R2, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), psi, T1, lpc, ntile);
+      fft2_a_fwd_kernel<R1, R2, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), psi, T1, lpc, ntile, X.pre);
     } else {
       if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, false>, sm))) return rc;
-      fft2_a_inv_kernel<R1, R2, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), T1, hpsi, lpc, ntile);
+      fft2_a_inv_kernel<R1, R2, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), T1, hpsi, lpc, ntile, X.post, X.accumulate);
     }
   } else {
     int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
@@ -831,10 +838,10 @@ static int launch_pass_batched(const Fft2Geom &G, const Fft2Batch &B, int nk, in
     if (grid > 0x7fffffffLL) return DFT_ERR_UNSUPPORTED;
     if (pass == 0) {
       if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, true>, sm))) return rc;
-      fft2_a_fwd_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, psi, T1, lpc, ntile);
+      fft2_a_fwd_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, psi, T1, lpc, ntile, nullptr);
     } else {
       if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, true>, sm))) return rc;
-      fft2_a_inv_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, T1, hpsi, lpc, ntile);
+      fft2_a_inv_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, T1, hpsi, lpc, ntile, nullptr, 0);
     }
   } else {
     int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
@@ -908,9 +915,6 @@ int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int
   return DFT_OK;
 }
 
-int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, void *T1, void *T2, int64_t t1_band,
-                int64_t t2_band, int nb, cudaStream_t st);
-
 template <int R1, int R2>
 static int launch_density(dft_plan *p, const Fft2Geom &G, cplx *T2, const double *wgt, double *rho, int nb, cudaStream_t st) {
   constexpr int NS = imax(R1, R2);
@@ -967,7 +971,7 @@ int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, 
   int rc;
   for (int pass = 0; pass < 2; pass++) {
     phase_begin(p, pass, st);
-    rc = fft2_launch(p, ik, pass, psi, nullptr, T1, T2, t1b / 16, t2b / 16, nb, st);
+    rc = fft2_launch(p, ik, pass, psi, nullptr, T1, T2, t1b / 16, t2b / 16, nb, st, nullptr);
     phase_end(p, pass, st, 1);
     if (rc) return rc;
   }
@@ -985,7 +989,10 @@ int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, 
 
 // pass: 0 A, 1 B, 2 C, 3 B^-1, 4 A^-1.  The pair is that of the axis the pass transforms.
 int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, void *T1, void *T2, int64_t t1_band,
-                int64_t t2_band, int nb, cudaStream_t st) {
+                int64_t t2_band, int nb, cudaStream_t st, const FftExtra *extra) {
+  FftExtra X;
+  if (extra) X = *extra;
+  const double *vpot = X.vpot ? X.vpot : p->d_vloc;
   int axis = (pass == 0 || pass == 4) ? 0 : (pass == 2 ? 2 : 1);
   int r1, r2;
   if (!fft2_pair(p->n[axis], &r1, &r2)) { set_error("no two-stage factorisation of %d", p->n[axis]); return DFT_ERR_UNSUPPORTED; }
@@ -993,7 +1000,7 @@ int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, 
   const cplx *cpsi = reinterpret_cast<const cplx *>(psi);
   cplx *chpsi = reinterpret_cast<cplx *>(hpsi), *t1 = reinterpret_cast<cplx *>(T1), *t2 = reinterpret_cast<cplx *>(T2);
   const int hb = p->kp[ik].max_cols_per_plane;
-#define X(a, b) if (r1 == (a) && r2 == (b)) return launch_pass<a, b>(p, G, pass, cpsi, chpsi, t1, t2, p->d_vloc, nb, hb, st);
+#define X(a, b) if (r1 == (a) && r2 == (b)) return launch_pass<a, b>(p, G, pass, cpsi, chpsi, t1, t2, vpot, nb, hb, st, X);
   FFT2_PAIRS(X)
 #undef X
   return DFT_ERR_UNSUPPORTED;

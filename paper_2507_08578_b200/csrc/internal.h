@@ -108,12 +108,15 @@ struct dft_plan {
   // local potential
   double *d_vloc = nullptr;                          // [n3][n2][n1], pre-scaled by 1/N
   bool vloc_set = false;
+  double *d_vtau = nullptr;                          // [n3][n2][n1] v_tau(r)/N (meta-GGA), set by dft_set_vtau
+  double *d_qcart = nullptr, *d_qhalf = nullptr;     // [nkpt][3][mpw] Cartesian k+G and half of it
+  bool vtau_set = false;
   // FFT
   dftb200::FftFactors fac[3];
   double *d_tw[3] = {nullptr, nullptr, nullptr};     // twiddles exp(+2 pi i j/n_c), [n_c] complex
   // options
   int band_chunk = 0;      // 0 = automatic
-  int terms = 7;
+  int terms = 15;          // bit 0 kinetic, bit 1 local, bit 2 non-local, bit 3 meta-GGA term (active once dft_set_vtau was called)
   int fft_path = 0;        // 0 = automatic (register path, TMA ring for the strided passes), 1 = generic Stockham path only,
                            // 2 = register path without the TMA ring
   int splitk = 0;
@@ -150,16 +153,25 @@ int sphere_build(const double *gmet, const int n[3], double ecut, KPoint *kp);
 // --- projtab.cu (S1) ----------------------------------------------------------------------
 int build_projector_table(dft_plan *p, int ik, double *maxq_out);
 
+// Optional variations of the local application (meta-GGA term): another potential in pass C, a real diagonal factor
+// applied to psi in G space while scattering (pass A), another one while gathering (pass A^-1), accumulation onto hpsi.
+struct FftExtra {
+  const double *vpot = nullptr;   // device [n3][n2][n1], pre-scaled by 1/N; null = the plan's V_loc
+  const double *pre = nullptr;    // device [npw]; null = 1
+  const double *post = nullptr;   // device [npw]; null = 1
+  int accumulate = 0;             // 1: hpsi += result (pad entries untouched) instead of hpsi = result
+};
 // --- fft.cu (K2) --------------------------------------------------------------------------
 int64_t fft_ws_bytes_per_band(const dft_plan *p);
 // V_loc psi for `nb` bands of k-point ik: psi/hpsi point at the first band ([nb][mpw] complex)
-int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb, void *ws, cudaStream_t st);
+int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb, void *ws, cudaStream_t st,
+                   const FftExtra *extra = nullptr);
 int zero_fill(double *hpsi, int64_t ndouble, cudaStream_t st);
 // fft2.cu: two-stage register path.  fft2_pair: is n = R1*R2 with both radices available as codelets?
 bool fft2_pair(int n, int *r1, int *r2);
 // pass: 0 A, 1 B, 2 C, 3 B^-1, 4 A^-1; T1/T2 strides in complex elements per band
 int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, void *T1, void *T2, int64_t t1_band,
-                int64_t t2_band, int nb, cudaStream_t st);
+                int64_t t2_band, int nb, cudaStream_t st, const FftExtra *extra = nullptr);
 
 // Optional combination applied where H psi is stored (GEMM-2 epilogue): out = sh * (H psi) + sy * psi + sx * xprev.
 // One step of a three-term recurrence in H (Chebyshev filter, PAPER.md :458) without extra passes over psi-sized arrays.

@@ -59,7 +59,7 @@ static void destroy_plan(dft_plan *p) {
   for (auto &k : p->kp) free_kpoint(k);
   cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
   cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
-  cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  cudaFree(p->d_vtau); cudaFree(p->d_qcart); cudaFree(p->d_qhalf); cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
@@ -311,6 +311,25 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
     if ((rc = zero_fill(hpsi, (int64_t)p->nkpt * nband * band_stride, st))) return rc;
     phase_end(p, 4, st, 1);
   }
+  if ((p->terms & 8) && p->vtau_set) {
+    // meta-GGA term (Eq. 8): hpsi += 1/2 sum_d q_d . FFT^-1[ v_tau(r) FFT[ q_d psi ] ], q = k + G Cartesian;
+    // three more local applications with diagonal factors fused into the scatter and gather passes
+    int chunk; void *ws;
+    if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
+    for (int ik = 0; ik < p->nkpt; ik++)
+      for (int b0 = 0; b0 < nband; b0 += chunk) {
+        int nb = nband - b0 < chunk ? nband - b0 : chunk;
+        size_t off = ((size_t)ik * nband + b0) * band_stride;
+        for (int d = 0; d < 3; d++) {
+          FftExtra X;
+          X.vpot = p->d_vtau;
+          X.pre = p->d_qcart + ((size_t)ik * 3 + d) * p->mpw;
+          X.post = p->d_qhalf + ((size_t)ik * 3 + d) * p->mpw;
+          X.accumulate = 1;
+          if ((rc = fft_apply_vloc(p, ik, psi + off, hpsi + off, nb, ws, st, &X))) return rc;
+        }
+      }
+  }
   if (kin || nl || rec)
     if ((rc = nonlocal_apply(p, psi, hpsi, nband, true, kin, nl, st, nullptr, p->vecpot_on ? p->d_kinaptr : nullptr, nullptr, rec))) return rc;
   return DFT_OK;
@@ -401,6 +420,58 @@ int dft_set_vloc(dft_plan *p, const double *V_r, void *stream) {
   return DFT_OK;
 }
 
+}  // extern "C"
+namespace dftb200 {
+// Cartesian q = 2 pi (k + m) Bm per plane wave: out[d][g] = q_d, half[d][g] = q_d / 2 (rows mpw apart)
+__global__ void qcart_kernel(const int32_t *__restrict__ kg, int npw, int mpw, double k1, double k2, double k3,
+                             const double *__restrict__ bm9, double *__restrict__ out, double *__restrict__ half) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= npw) return;
+  const double twopi = 6.283185307179586476925286766559;
+  double t1 = k1 + (double)kg[3 * g], t2 = k2 + (double)kg[3 * g + 1], t3 = k3 + (double)kg[3 * g + 2];
+  for (int d = 0; d < 3; d++) {
+    double q = twopi * (t1 * bm9[d] + t2 * bm9[3 + d] + t3 * bm9[6 + d]);
+    out[(size_t)d * mpw + g] = q; half[(size_t)d * mpw + g] = 0.5 * q;
+  }
+}
+}  // namespace dftb200
+extern "C" {
+
+int dft_set_vtau(dft_plan *p, const double *vtau_r, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (!vtau_r) { p->vtau_set = false; return DFT_OK; }
+  cudaStream_t st = (cudaStream_t)stream;
+  int64_t n = p->nbox;
+  if (!p->d_vtau && cudaMalloc(&p->d_vtau, sizeof(double) * n) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate v_tau"); return DFT_ERR_ALLOC; }
+  if (!p->d_qcart && p->mpw > 0) {
+    size_t cnt = (size_t)p->nkpt * 3 * p->mpw;
+    if (cudaMalloc(&p->d_qcart, sizeof(double) * cnt) != cudaSuccess || cudaMalloc(&p->d_qhalf, sizeof(double) * cnt) != cudaSuccess) {
+      cudaGetLastError(); set_error("cannot allocate the k+G arrays"); return DFT_ERR_ALLOC;
+    }
+    DFT_CUDA_CHECK(cudaMemset(p->d_qcart, 0, sizeof(double) * cnt));
+    DFT_CUDA_CHECK(cudaMemset(p->d_qhalf, 0, sizeof(double) * cnt));
+    double *d_bm = nullptr;
+    int rc;
+    if ((rc = to_device(&d_bm, p->bm, 9))) return rc;
+    for (int ik = 0; ik < p->nkpt; ik++) {
+      const KPoint &K = p->kp[ik];
+      if (K.npw == 0) continue;
+      qcart_kernel<<<(K.npw + 255) / 256, 256>>>(K.kg, K.npw, p->mpw, K.k[0], K.k[1], K.k[2], d_bm,
+                                                p->d_qcart + (size_t)ik * 3 * p->mpw, p->d_qhalf + (size_t)ik * 3 * p->mpw);
+    }
+    cudaError_t e = cudaDeviceSynchronize();
+    cudaFree(d_bm);
+    if (e != cudaSuccess) { set_error("qcart_kernel failed: %s", cudaGetErrorString(e)); return DFT_ERR_CUDA; }
+  }
+  int grid = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
+  scale_copy_kernel<<<grid, 256, 0, st>>>(vtau_r, p->d_vtau, n, 1.0 / (double)n);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  p->vtau_set = true;
+  return DFT_OK;
+  DFT_GUARD_END
+}
+
 int dft_set_workspace(dft_plan *p, void *dev_ptr, int64_t bytes) {
   if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
   if (dev_ptr && (bytes <= 0 || ((uintptr_t)dev_ptr & 255))) { set_error("workspace must be 256-byte aligned with bytes > 0"); return DFT_ERR_INVALID_ARG; }
@@ -416,7 +487,7 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     p->band_chunk = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "terms")) {
-    if (value < 0 || value > 7) { set_error("terms = %lld outside 0..7", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if (value < 0 || value > 15) { set_error("terms = %lld outside 0..15", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->terms = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "fft_path")) {

@@ -236,6 +236,30 @@ def test_density_accumulation(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c1m", "aniso", "c3k2"])
+def test_meta_gga_term(name):
+    """dft_set_vtau (Eq. 8): the term alone (terms = 8), with everything else (15), and switched off again."""
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    n = cfg["ngfft"]
+    rng = np.random.default_rng(6)
+    vt = 0.4 + 0.15 * rng.standard_normal((n[2], n[1], n[0]))
+    plain = gpu_apply(plan, psi)
+    plan.set_vtau(torch.as_tensor(vt, device="cuda"))
+    m = 1 if name == "aniso" else 2
+    tau = np.zeros_like(psi)
+    for ik, (kg, ig, kin) in enumerate(sph):
+        tau[ik] = oracle.apply_mgga(cfg, ik, kg, ig, psi[ik], vt, method=m)
+    plan.set_option("terms", 8)
+    assert band_rel_err(gpu_apply(plan, psi), tau) <= TOL
+    plan.set_option("terms", 15)
+    ref = oracle_apply(cfg, sph, psi, method=m) + tau
+    assert band_rel_err(gpu_apply(plan, psi), ref) <= TOL
+    plan.set_vtau(None)
+    assert np.array_equal(gpu_apply(plan, psi), plain)
+    plan.destroy()
+
+
 def test_degenerate_inputs():
     """Edge cases of the method: no bands, one plane wave (ecut below the first shell), a k-point whose sphere is empty,
     and error codes for bad arguments."""

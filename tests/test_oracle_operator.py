@@ -117,3 +117,27 @@ def test_velocity_gauge_kinetic_pins():
     psi = rand_c((2, len(kg)), 4)
     out = oracle.apply_h(c, 0, kg, ig, ka, psi, terms=oracle.KIN)
     assert rel_err(out, ka[None, :] * psi) < 1e-15
+
+
+def test_meta_gga_term_pins():
+    """-1/2 div(v_tau grad) (Eq. 8): constant v_tau = c gives c * 1/2|k+G|^2 psi; the dense definition
+    H_tau[m, m'] = 1/2 q(m).q(m') vt~[(m - m') mod n] built from the oracle's Fourier coefficients of v_tau;
+    Hermiticity."""
+    import oracle
+    from util import config, sphere, rand_c, rel_err
+    for name in ("c0", "aniso"):
+        c = config(name); kg, ig, kin = sphere(name)
+        n = c["ngfft"]; npw = len(kg)
+        psi = rand_c((2, npw), 17)
+        const = np.full((n[2], n[1], n[0]), 0.37)
+        assert rel_err(oracle.apply_mgga(c, 0, kg, ig, psi, const, method=1), 0.37 * kin[None, :] * psi) < 1e-12
+        rng = np.random.default_rng(2)
+        vt = 0.5 + 0.2 * rng.standard_normal((n[2], n[1], n[0]))
+        got = oracle.apply_mgga(c, 0, kg, ig, psi, vt, method=1)
+        vtil = oracle.vtilde(vt).reshape(-1)                       # [(d3*n2 + d2)*n1 + d1]
+        bm, _ = oracle.lattice(c["rprimd"])
+        q = 2 * np.pi * (kg + np.asarray(c["kpt"][0])[None, :]) @ bm
+        d = (kg[:, None, :] - kg[None, :, :]) % np.array(n)[None, None, :]
+        H = 0.5 * (q @ q.T) * vtil[(d[..., 2] * n[1] + d[..., 1]) * n[0] + d[..., 0]]
+        assert rel_err(got, psi @ H.T) < 1e-12
+        assert np.max(np.abs(H - H.conj().T)) < 1e-13 * np.max(np.abs(H))

@@ -143,6 +143,11 @@ int dft_get_cprj(dft_plan *p, const double *psi, double *cprj, int32_t nband, vo
  * (no atomics, fixed order).  DFT_ERR_UNSUPPORTED for box lengths without a two-radix factorisation.  */
 int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights, double *rho, int32_t nband, void *stream);
 
+/* Kinetic-energy density of the same equation (Eq. 6: tau(r) = 1/2 sum_nk w_nk |grad psi_nk(r)|^2):
+ * tau[j] += 1/2 sum_k sum_n weights[k][n] sum_d |FFT[(k+G)_d c_nk](r_j)|^2, (k+G) Cartesian.  Same arguments,
+ * layouts and rules as dft_accumulate_density (three density passes with the gradient factor fused into the scatter). */
+int dft_accumulate_tau(dft_plan *p, const double *psi, const double *weights, double *tau, int32_t nband, void *stream);
+
 /* Meta-GGA term of the Hamiltonian (Eq. 8, :152: "- 1/2 div( v_tau(r) grad )", v_tau = d f_xc / d tau, Eq. 9):
  * once set, dft_apply_h adds  1/2 sum_{d=x,y,z} (k+G)_d FFT^-1[ v_tau(r) FFT[ (k+G')_d psi ] ]  (three more local
  * applications whose diagonal factors are fused into the scatter and gather passes).  vtau_r: DEVICE

@@ -227,6 +227,20 @@ def apply_mgga(cfg, ik, kg, igfft, psi, vtau, method=2):
     return out
 
 
+def tau_density(cfg, ik, kg, igfft, psi, weights, method=2):
+    """Kinetic-energy density of PAPER.md Eq. 6 (:140): tau(r_j) = 1/2 sum_b w_b sum_d |d_d psi_b(r_j)|^2 with
+    d_d psi(r) = sum_G i q_d(G) c(G) e^{i(k+G).r}, q = k + G Cartesian; |.|^2 drops the factor i and the Bloch phase, so
+    each gradient component is a density() of the coefficients q_d c with weight w/2."""
+    bm, _ = lattice(cfg["rprimd"])
+    npw = len(kg)
+    q = 2.0 * np.pi * (np.asarray(kg, float) + np.asarray(cfg["kpt"][ik], float)[None, :]) @ np.asarray(bm, float).reshape(3, 3)
+    psi = np.asarray(psi, np.complex128)[:, :npw]
+    out = 0.0
+    for d in range(3):
+        out = out + density(cfg["ngfft"], igfft, psi * q[None, :, d], 0.5 * np.asarray(weights, float), method)
+    return out
+
+
 def cprj(cfg, ik, kg, psi):
     """<p_a,i|psi_b> (PAPER.md :477 "coefficients c_a,i,n,k"), [nproj][nband] complex: step 1 of Eq. 26 (:470),
     as the streamed loops of orc_nonlocal_apply compute it."""

@@ -33,7 +33,7 @@ PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_get_cprj", "dft_chebyshev_filter",
-           "dft_set_vector_potential", "dft_accumulate_density",
+           "dft_set_vector_potential", "dft_accumulate_density", "dft_accumulate_tau",
            "dft_set_vtau",
            "dft_set_vloc", "dft_set_workspace", "dft_plan_set_option", "dft_apply_h", "dft_apply_h_host",
            "dft_plan_last_launches", "dft_plan_set_timing", "dft_plan_phase_ms", "dft_plan_destroy", "dft_last_error")
@@ -85,6 +85,7 @@ def lib():
     L.dft_set_vector_potential.argtypes = [C.c_void_p, _dp]
     L.dft_set_vtau.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.dft_accumulate_density.argtypes = [C.c_void_p, C.c_void_p, _dp, C.c_void_p, C.c_int32, C.c_void_p]
+    L.dft_accumulate_tau.argtypes = [C.c_void_p, C.c_void_p, _dp, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_chebyshev_filter.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                        C.c_void_p]
     L.dft_apply_s.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
@@ -205,6 +206,10 @@ def dft_accumulate_density(plan, psi_dev_ptr, weights, rho_dev_ptr, nband, strea
     _check(lib().dft_accumulate_density(plan, psi_dev_ptr, _d(_f64(weights)), rho_dev_ptr, nband, stream))
 
 
+def dft_accumulate_tau(plan, psi_dev_ptr, weights, tau_dev_ptr, nband, stream=0):
+    _check(lib().dft_accumulate_tau(plan, psi_dev_ptr, _d(_f64(weights)), tau_dev_ptr, nband, stream))
+
+
 def dft_set_vtau(plan, vtau_dev_ptr, stream=0):
     _check(lib().dft_set_vtau(plan, vtau_dev_ptr, stream))
 
@@ -315,8 +320,9 @@ class Plan:
         dft_get_cprj(self.h, psi.data_ptr(), out.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
         return out
 
-    def accumulate_density(self, psi, weights, rho=None):
-        """rho[n3][n2][n1] += sum_kn weights[k][n] |psi_kn(r)|^2; rho: torch float64 CUDA tensor (created as zeros if None)."""
+    def accumulate_density(self, psi, weights, rho=None, tau=False):
+        """rho[n3][n2][n1] += sum_kn weights[k][n] |psi_kn(r)|^2; rho: torch float64 CUDA tensor (created as zeros if None).
+        tau=True accumulates the kinetic-energy density 1/2 sum w |grad psi|^2 instead."""
         import torch
         assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.shape[-1] == self.mpw
         nband = psi.numel() // (self.nkpt * self.mpw) if self.mpw else 0
@@ -326,7 +332,8 @@ class Plan:
         assert rho.is_cuda and rho.dtype == torch.float64 and rho.is_contiguous() and rho.numel() == n1 * n2 * n3
         w = np.ascontiguousarray(weights, np.float64)
         assert w.size == self.nkpt * nband
-        dft_accumulate_density(self.h, psi.data_ptr(), w, rho.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
+        fn = dft_accumulate_tau if tau else dft_accumulate_density
+        fn(self.h, psi.data_ptr(), w, rho.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
         return rho
 
     def set_vtau(self, v):

@@ -956,7 +956,8 @@ static int launch_density(dft_plan *p, const Fft2Geom &G, cplx *T2, const double
 
 // rho(r) += sum_b wgt[b] |psi_b(r)|^2 for nb bands of k-point ik: passes A and B as in H psi, then the density kernel.
 // Only the register path has it: DFT_ERR_UNSUPPORTED for box lengths without a two-radix factorisation.
-int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st) {
+int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st,
+                 const double *pre) {
   const KPoint &kp = p->kp[ik];
   if (kp.npw == 0 || nb == 0) return DFT_OK;
   int r1, r2;
@@ -971,7 +972,9 @@ int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, 
   int rc;
   for (int pass = 0; pass < 2; pass++) {
     phase_begin(p, pass, st);
-    rc = fft2_launch(p, ik, pass, psi, nullptr, T1, T2, t1b / 16, t2b / 16, nb, st, nullptr);
+    FftExtra X;
+    X.pre = pre;      // optional diagonal factor in G space (gradient component for the kinetic-energy density)
+    rc = fft2_launch(p, ik, pass, psi, nullptr, T1, T2, t1b / 16, t2b / 16, nb, st, &X);
     phase_end(p, pass, st, 1);
     if (rc) return rc;
   }

@@ -185,7 +185,8 @@ bool fft2_batch_ok(const dft_plan *p);
 int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int nband_total, void *ws, cudaStream_t st);
 
 // rho(r) += sum_b wgt[b] |psi_b(r)|^2 (device wgt [nb]); forward passes A, B and the density kernel
-int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st);
+int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st,
+                 const double *pre = nullptr);
 
 // --- nonlocal.cu (K3) ---------------------------------------------------------------------
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi

@@ -437,13 +437,7 @@ __global__ void qcart_kernel(const int32_t *__restrict__ kg, int npw, int mpw, d
 }  // namespace dftb200
 extern "C" {
 
-int dft_set_vtau(dft_plan *p, const double *vtau_r, void *stream) {
-  DFT_GUARD_BEGIN
-  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
-  if (!vtau_r) { p->vtau_set = false; return DFT_OK; }
-  cudaStream_t st = (cudaStream_t)stream;
-  int64_t n = p->nbox;
-  if (!p->d_vtau && cudaMalloc(&p->d_vtau, sizeof(double) * n) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate v_tau"); return DFT_ERR_ALLOC; }
+static int ensure_qcart(dft_plan *p) {
   if (!p->d_qcart && p->mpw > 0) {
     size_t cnt = (size_t)p->nkpt * 3 * p->mpw;
     if (cudaMalloc(&p->d_qcart, sizeof(double) * cnt) != cudaSuccess || cudaMalloc(&p->d_qhalf, sizeof(double) * cnt) != cudaSuccess) {
@@ -464,6 +458,17 @@ int dft_set_vtau(dft_plan *p, const double *vtau_r, void *stream) {
     cudaFree(d_bm);
     if (e != cudaSuccess) { set_error("qcart_kernel failed: %s", cudaGetErrorString(e)); return DFT_ERR_CUDA; }
   }
+  return DFT_OK;
+}
+
+int dft_set_vtau(dft_plan *p, const double *vtau_r, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (!vtau_r) { p->vtau_set = false; return DFT_OK; }
+  cudaStream_t st = (cudaStream_t)stream;
+  int64_t n = p->nbox;
+  if (!p->d_vtau && cudaMalloc(&p->d_vtau, sizeof(double) * n) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate v_tau"); return DFT_ERR_ALLOC; }
+  { int rcq = ensure_qcart(p); if (rcq) return rcq; }
   int grid = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
   scale_copy_kernel<<<grid, 256, 0, st>>>(vtau_r, p->d_vtau, n, 1.0 / (double)n);
   DFT_CUDA_CHECK(cudaGetLastError());
@@ -600,7 +605,7 @@ int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, 
   DFT_GUARD_END
 }
 
-int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights, double *rho, int32_t nband, void *stream) {
+static int accumulate_impl(dft_plan *p, const double *psi, const double *weights, double *rho, int32_t nband, void *stream, bool tau) {
   DFT_GUARD_BEGIN
   if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
   if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
@@ -616,7 +621,13 @@ int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights
     p->wgt_count = nw;
   }
   // weights are HOST memory and must be consumed before the call returns: copy on the stream, then wait for it
-  DFT_CUDA_CHECK(cudaMemcpyAsync(p->d_wgt, weights, sizeof(double) * nw, cudaMemcpyHostToDevice, st));
+  std::vector<double> wh(weights, weights + nw);
+  if (tau) {   // tau(r) = 1/2 sum w |grad psi|^2: three gradient components, each a density with half the weight
+    for (auto &v : wh) v *= 0.5;
+    int rcq = ensure_qcart(p);
+    if (rcq) return rcq;
+  }
+  DFT_CUDA_CHECK(cudaMemcpyAsync(p->d_wgt, wh.data(), sizeof(double) * nw, cudaMemcpyHostToDevice, st));
   DFT_CUDA_CHECK(cudaStreamSynchronize(st));
   int chunk; void *ws; int rc;
   if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
@@ -625,10 +636,20 @@ int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights
     for (int b0 = 0; b0 < nband; b0 += chunk) {
       int nb = nband - b0 < chunk ? nband - b0 : chunk;
       size_t off = ((size_t)ik * nband + b0) * band_stride;
-      if ((rc = fft2_density(p, ik, psi + off, p->d_wgt + (size_t)ik * nband + b0, rho, nb, ws, st))) return rc;
+      for (int d = 0; d < (tau ? 3 : 1); d++)
+        if ((rc = fft2_density(p, ik, psi + off, p->d_wgt + (size_t)ik * nband + b0, rho, nb, ws, st,
+                               tau ? p->d_qcart + ((size_t)ik * 3 + d) * p->mpw : nullptr))) return rc;
     }
   return DFT_OK;
   DFT_GUARD_END
+}
+
+int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights, double *rho, int32_t nband, void *stream) {
+  return accumulate_impl(p, psi, weights, rho, nband, stream, false);
+}
+
+int dft_accumulate_tau(dft_plan *p, const double *psi, const double *weights, double *tau, int32_t nband, void *stream) {
+  return accumulate_impl(p, psi, weights, tau, nband, stream, true);
 }
 
 int dft_set_sij(dft_plan *p, const double *sij) {

@@ -233,6 +233,11 @@ def test_density_accumulation(name):
         ref += 1.5 * oracle.density(cfg["ngfft"], ig, psi[ik], w[ik], method=1 if name in ("c0", "aniso") else 2)
     got = rho.cpu().numpy()
     assert np.max(np.abs(got - ref)) <= 1e-12 * ref.max(), np.max(np.abs(got - ref)) / ref.max()
+    tau = plan.accumulate_density(tpsi, w, tau=True).cpu().numpy()          # kinetic-energy density of the same equation
+    tref = np.zeros(tau.shape)
+    for ik, (kg, ig, kin) in enumerate(sph):
+        tref += oracle.tau_density(cfg, ik, kg, ig, psi[ik], w[ik], method=1 if name in ("c0", "aniso") else 2)
+    assert np.max(np.abs(tau - tref)) <= 1e-12 * tref.max(), np.max(np.abs(tau - tref)) / tref.max()
     plan.destroy()
 
 

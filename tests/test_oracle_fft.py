@@ -144,3 +144,19 @@ def test_density_pins():
         ph = np.exp(2j * np.pi * (dm[0] * j1 / n[0] + dm[1] * j2 / n[1] + dm[2] * j3 / n[2]))
         ref2 = 1.5 * (abs(a) ** 2 + abs(b) ** 2 + 2 * np.real(np.conj(a) * b * ph))
         assert np.max(np.abs(oracle.density(n, ig, two, [1.5]) - ref2)) < 1e-13
+
+
+def test_tau_density_pins():
+    """tau(r) = 1/2 sum w |grad psi|^2 (Eq. 6): one plane wave -> the constant w * 1/2|k+G|^2; the box mean is
+    sum_b w_b sum_G 1/2|k+G|^2 |c_b(G)|^2 (Parseval per gradient component)."""
+    import oracle
+    from util import config, sphere, rand_c
+    for name in ("c0", "aniso"):
+        c = config(name); kg, ig, kin = sphere(name)
+        npw = len(ig); N = int(np.prod(c["ngfft"]))
+        one = np.zeros((1, npw), complex); one[0, 7] = 0.6 - 0.8j
+        assert np.max(np.abs(oracle.tau_density(c, 0, kg, ig, one, [2.0], method=1) - 2.0 * kin[7])) < 1e-12 * (1 + kin[7])
+        psi = rand_c((3, npw), 41); w = np.array([0.4, 1.1, 0.9])
+        tau = oracle.tau_density(c, 0, kg, ig, psi, w, method=1)
+        ref = np.sum(w * np.sum(kin[None, :] * np.abs(psi) ** 2, axis=1))
+        assert tau.min() >= 0 and abs(tau.sum() / N - ref) < 1e-12 * ref

@@ -265,6 +265,34 @@ def test_meta_gga_term(name):
     plan.destroy()
 
 
+def test_apply_h_is_cuda_graph_capturable():
+    """dft_apply_h only enqueues (no allocation or synchronisation once scratch exists), so a launch-bound small cell
+    can be captured into a CUDA graph and replayed."""
+    cfg, plan, sph = _setup("c0")
+    psi = torch.as_tensor(synth.gen_psi(cfg, [s[2] for s in sph]), device="cuda")
+    out = torch.empty_like(psi)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        plan.apply_h(psi, out)                                  # warm-up: scratch allocation, kernel attributes
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    ref = out.clone()
+    graph = torch.cuda.CUDAGraph()
+    out.zero_()
+    with torch.cuda.graph(graph):
+        plan.apply_h(psi, out)
+    out.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    psi.mul_(2.0)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.allclose(out, 2.0 * ref, rtol=1e-13, atol=0)
+    plan.destroy()
+
+
 def test_degenerate_inputs():
     """Edge cases of the method: no bands, one plane wave (ecut below the first shell), a k-point whose sphere is empty,
     and error codes for bad arguments."""

@@ -161,6 +161,7 @@ def main():
     ap.add_argument("--nband", type=int, default=0, help="override the band count (experiments only)")
     ap.add_argument("--band-chunk", type=int, default=0)
     ap.add_argument("--fft-path", type=int, default=0, help="dft_plan_set_option fft_path (experiments only)")
+    ap.add_argument("--proj-mode", type=int, default=0, help="1 = factorised projectors FY.S (experiments only)")
     ap.add_argument("--gemm-3m", type=int, default=1, help="0 = 4-product complex GEMMs (experiments only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (experiments only)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the e2e leg (experiments only)")
@@ -195,6 +196,8 @@ def main():
     if args.fft_path:
         plan.set_option("fft_path", args.fft_path)
     plan.set_option("gemm_3m", args.gemm_3m)
+    if args.proj_mode:
+        plan.set_option("proj_mode", args.proj_mode)
     plan.set_vloc(torch.as_tensor(cfg["vloc"], device="cuda"))
     kin_list = [plan.get_kg(ik)[2] for ik in range(plan.nkpt)]
     nband = cfg["nband"]

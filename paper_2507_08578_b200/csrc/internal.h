@@ -102,6 +102,9 @@ struct dft_plan {
   bool vecpot_on = false;
   double *d_ones = nullptr;                          // [mpw] of 1.0: the unit diagonal of S in GEMM-2's epilogue
   const double **d_oneptr = nullptr;                 // [nkpt] device pointers to d_ones
+  double *d_stab = nullptr, *d_fytab = nullptr;      // factorised projectors: structure factors / form factors (proj_mode = 1)
+  int ldf = 0;                                       // row length of d_fytab (mpw rounded up to 8)
+  int proj_mode = 0;                                 // 0 = materialised table (GEMMs on P), 1 = factorised P = FY . S
   double *d_ptab = nullptr;                          // [nkpt][nproj][mpw] complex, zero padded beyond npw_k
   int32_t *d_npw = nullptr;                          // [nkpt]
   const double **d_kinptr = nullptr;                 // [nkpt] device pointers to kin of each k-point
@@ -152,6 +155,7 @@ int sphere_build(const double *gmet, const int n[3], double ecut, KPoint *kp);
 
 // --- projtab.cu (S1) ----------------------------------------------------------------------
 int build_projector_table(dft_plan *p, int ik, double *maxq_out);
+int build_factor_tables(dft_plan *p);   // S [nkpt][natom][mpw] complex and FY [nkpt][ntypat*8][ldf] real (factorised projectors)
 
 // Optional variations of the local application (meta-GGA term): another potential in pass C, a real diagonal factor
 // applied to psi in G space while scattering (pass A), another one while gathering (pass A^-1), accumulation onto hpsi.

@@ -521,6 +521,241 @@ gemm2_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant_
   }
 }
 
+// ---------------------------------------------------------------- factorised projectors (proj_mode = 1)
+// p_{a,i}(G) = FY_{t(a),i}(G) . S_a(G) with FY real and S_a a phase (projtab.cu), the paper's "computed on-the-fly"
+// variant (:477).  Neither GEMM then needs the [nproj][npw] table, and because FY is real the contraction over G is a
+// REAL x complex product after one complex multiplication per (atom, band, G):
+//   GEMM-1:  z_{a,b}(G) = conj(S_a(G)) psi_b(G)                (4 FP64 instructions per thread, shared by the 8 projectors)
+//            cprj[a,i,b] = sum_G FY[i,G] z_{a,b}(G)            (2 DMMA per 8 x 8 x 4 block: re and im columns)
+// 2 DMMAs + 4 FP64 instructions where the 4-product form needs 4 DMMAs and the Gauss form 3 (+ sums): 40 against 64 /
+// 49 pipe clocks per block.  M = 8 of the m8n8k4 shape is the 8 projectors of one atom, so the CTA tile is
+// 16 atoms x 64 bands (8 warps, 4 atoms x 32 bands each, the accumulator layout of the 4-product kernel).
+constexpr int FC_BA = 16;                  // atoms per CTA tile
+constexpr int FC_OFF_S = NL_BN * 128;      // stage layout: psi tile 8 KB | S tile 2 KB | FY tile <= 1 KB
+constexpr int FC_OFF_F = FC_OFF_S + FC_BA * 128;
+constexpr int FC_STAGE_BYTES = 11 * 1024;
+constexpr int FC_STAGES = 8;
+constexpr int FC_PREFETCH = FC_STAGES - 2;
+constexpr int FC_SMEM = FC_STAGES * FC_STAGE_BYTES + 1024 + 256;
+
+struct Fac1Params {
+  int natom, nband, nproj, nslab, nsplit, slabs_per_split, tiles_n, ntypat;
+  const int32_t *typat, *nlmn, *atom_first;
+  double2 *part;   // [nkpt][nsplit][nproj][nband]
+};
+
+// grid: (tiles_a * tiles_n, nsplit, nkpt)
+__global__ void __launch_bounds__(NL_THREADS, 1)
+gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_constant__ CUtensorMap mapS,
+                 const __grid_constant__ CUtensorMap mapF, Fac1Params Q) {
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char *tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  uint64_t *full = reinterpret_cast<uint64_t *>(tiles + FC_STAGES * FC_STAGE_BYTES), *empty = full + FC_STAGES;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < FC_STAGES; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], NL_CONSUMERS); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int tn = blockIdx.x % Q.tiles_n, ta = blockIdx.x / Q.tiles_n, split = blockIdx.y, ik = blockIdx.z;
+  const int s0 = split * Q.slabs_per_split;
+  int ns = Q.nslab - s0; if (ns > Q.slabs_per_split) ns = Q.slabs_per_split; if (ns < 0) ns = 0;
+  const uint32_t tx = NL_BN * 128 + FC_BA * 128 + 64 * 8 * Q.ntypat;
+  auto issue = [&](int j) {
+    int s = j % FC_STAGES;
+    if (j >= FC_STAGES) mbar_wait(&empty[s], ((j / FC_STAGES) - 1) & 1);
+    unsigned char *st = tiles + s * FC_STAGE_BYTES;
+    mbar_expect_tx(&full[s], tx);
+    tma_load_3d(st, &mapPsi, &full[s], (s0 + j) * 16, tn * NL_BN, ik);
+    tma_load_3d(st + FC_OFF_S, &mapS, &full[s], (s0 + j) * 16, ta * FC_BA, ik);
+    tma_load_3d(st + FC_OFF_F, &mapF, &full[s], (s0 + j) * 8, 0, ik);
+  };
+  const bool producer = (threadIdx.x == 0);
+  if (producer)
+    for (int j = 0; j < FC_PREFETCH && j < ns; j++) issue(j);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wm = warp >> 1, wn = warp & 1;
+  const int i = lane >> 2, j = lane & 3;
+  int frow[4];   // byte offset of this lane's FY row (its atom's type, projector i) inside the FY tile
+#pragma unroll
+  for (int q = 0; q < 4; q++) {
+    int atom = ta * FC_BA + wm * 4 + q;
+    frow[q] = ((atom < Q.natom ? Q.typat[atom] : 0) * 8 + i) * 64;
+  }
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
+  for (int it = 0; it < ns; it++) {
+    if (producer && it + FC_PREFETCH < ns) issue(it + FC_PREFETCH);
+    __syncwarp();
+    int s = it % FC_STAGES;
+    mbar_wait(&full[s], (it / FC_STAGES) & 1);
+    const unsigned char *Ps = tiles + s * FC_STAGE_BYTES, *Ss = Ps + FC_OFF_S, *Fs = Ps + FC_OFF_F;
+#pragma unroll
+    for (int kg = 0; kg < 2; kg++) {
+      const int e = 2 * j + kg;   // this lane's G inside the slab (k index of the 8x8x4 block)
+      double pr[4], pi[4];
+      const unsigned char *b0 = Ps + (wn * 32 + i) * 128 + ((e ^ i) << 4);
+#pragma unroll
+      for (int nb = 0; nb < 4; nb++) {
+        double2 v = *reinterpret_cast<const double2 *>(b0 + nb * 8 * 128);
+        pr[nb] = v.x; pi[nb] = v.y;
+      }
+#pragma unroll
+      for (int q = 0; q < 4; q++) {
+        const int arow = wm * 4 + q;
+        const double2 sg = *reinterpret_cast<const double2 *>(Ss + arow * 128 + ((e ^ (arow & 7)) << 4));
+        const double fa = *reinterpret_cast<const double *>(Fs + frow[q] + e * 8);
+#pragma unroll
+        for (int nb = 0; nb < 4; nb++) {
+          double zr = sg.x * pr[nb] + sg.y * pi[nb], zi = sg.x * pi[nb] - sg.y * pr[nb];   // conj(S) psi
+          dmma(cre[q][nb][0], cre[q][nb][1], fa, zr);
+          dmma(cim[q][nb][0], cim[q][nb][1], fa, zi);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[s]);
+  }
+  // partial[ik][split][first_a + i][b]; thread holds projector i of its 4 atoms, bands 2j, 2j+1 of each 8-band block
+  double2 *out = Q.part + ((size_t)(ik * Q.nsplit + split) * Q.nproj) * Q.nband;
+#pragma unroll
+  for (int q = 0; q < 4; q++) {
+    int atom = ta * FC_BA + wm * 4 + q;
+    if (atom >= Q.natom) continue;
+    if (i >= Q.nlmn[Q.typat[atom]]) continue;
+    double2 *row = out + (size_t)(Q.atom_first[atom] + i) * Q.nband;
+#pragma unroll
+    for (int nb = 0; nb < 4; nb++) {
+      int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j;
+      if (b < Q.nband) row[b] = make_double2(cre[q][nb][0], cim[q][nb][0]);
+      if (b + 1 < Q.nband) row[b + 1] = make_double2(cre[q][nb][1], cim[q][nb][1]);
+    }
+  }
+}
+
+//   GEMM-2:  w_{a,b}(G) = sum_i FY[i,G] c'[a,i,b]               (4 DMMA per 8 x 8 block: 2 k-groups of projectors x re/im)
+//            hpsi_b(G) += S_a(G) w_{a,b}(G)                     (8 FP64 instructions per thread and block)
+// One K-slab = one atom: its c' tile [64 bands][8 projectors] (TMA, swizzled) and its phases for the tile's 128 G.
+// The FY rows of the tile's 128 G (8 per atom type, row stride 132 doubles against bank conflicts) are loaded once.
+constexpr int FD_OFF_S = NL_BN * 128;                 // stage: c' tile 8 KB | S_a(G) 2 KB
+constexpr int FD_STAGE_BYTES = 10 * 1024;
+constexpr int FD_STAGES = 8;
+constexpr int FD_PREFETCH = FD_STAGES - 2;
+constexpr int FD_FLD = NL_BM + 4;                     // FY row stride in shared memory (doubles)
+constexpr int FD_FBYTES = 2 * 8 * FD_FLD * 8;         // up to two atom types
+constexpr int FD_SMEM = FD_STAGES * FD_STAGE_BYTES + FD_FBYTES + 1024 + 256;
+
+// grid: (tiles_n * tiles_m, 1, nkpt); Q as in gemm2_kernel, nslab = natom
+__global__ void __launch_bounds__(NL_THREADS, 1)
+gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant__ CUtensorMap mapS,
+                 const __grid_constant__ CUtensorMap mapF, Gemm2Params Q, const int32_t *__restrict__ typat,
+                 const int32_t *__restrict__ atom_first, int ntypat) {
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char *tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  unsigned char *Fs = tiles + FD_STAGES * FD_STAGE_BYTES;
+  uint64_t *full = reinterpret_cast<uint64_t *>(Fs + FD_FBYTES), *empty = full + FD_STAGES, *fbar = empty + FD_STAGES;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < FD_STAGES; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], NL_CONSUMERS); }
+    mbar_init(fbar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int tn = blockIdx.x % Q.tiles_n, tm = blockIdx.x / Q.tiles_n, ik = blockIdx.z;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wm = warp >> 1, wn = warp & 1;
+  const int i = lane >> 2, j = lane & 3;
+  const int ns = Q.with_nl ? Q.nslab : 0;
+  auto issue = [&](int a) {
+    int s = a % FD_STAGES;
+    if (a >= FD_STAGES) mbar_wait(&empty[s], ((a / FD_STAGES) - 1) & 1);
+    unsigned char *st = tiles + s * FD_STAGE_BYTES;
+    mbar_expect_tx(&full[s], NL_BN * 128 + NL_BM * 16);
+    tma_load_3d(st, &mapC, &full[s], 2 * __ldg(atom_first + a), tn * NL_BN, ik);
+    tma_load_3d(st + FD_OFF_S, &mapS, &full[s], tm * NL_BM * 2, a, ik);
+  };
+  const bool producer = (threadIdx.x == 0);
+  if (producer && ns > 0) {
+    mbar_expect_tx(fbar, (uint32_t)(ntypat * 8 * FD_FLD * 8));
+    tma_load_3d(Fs, &mapF, fbar, tm * NL_BM, 0, ik);
+    for (int a = 0; a < FD_PREFETCH && a < ns; a++) issue(a);
+  }
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
+  if (ns > 0) mbar_wait(fbar, 0);
+  for (int a = 0; a < ns; a++) {
+    if (producer && a + FD_PREFETCH < ns) issue(a + FD_PREFETCH);
+    __syncwarp();
+    int s = a % FD_STAGES;
+    const int t = __ldg(typat + a);
+    mbar_wait(&full[s], (a / FD_STAGES) & 1);
+    const unsigned char *Cs = tiles + s * FD_STAGE_BYTES, *Ss = Cs + FD_OFF_S;
+    double2 sg[4];
+    double fa[4][2];
+#pragma unroll
+    for (int mb = 0; mb < 4; mb++) {
+      const int g = wm * 32 + mb * 8 + i;                                   // G row of this lane inside the tile
+      sg[mb] = *reinterpret_cast<const double2 *>(Ss + g * 16);
+#pragma unroll
+      for (int kgp = 0; kgp < 2; kgp++)                                      // projector 2j + kgp of the atom's type
+        fa[mb][kgp] = *reinterpret_cast<const double *>(Fs + ((size_t)((t * 8 + 2 * j + kgp) * FD_FLD + g)) * 8);
+    }
+#pragma unroll
+    for (int nb = 0; nb < 4; nb++) {
+      double cr[2], ci[2];
+      const unsigned char *b0 = Cs + (wn * 32 + nb * 8 + i) * 128;
+#pragma unroll
+      for (int kgp = 0; kgp < 2; kgp++) {
+        double2 v = *reinterpret_cast<const double2 *>(b0 + (((2 * j + kgp) ^ i) << 4));
+        cr[kgp] = v.x; ci[kgp] = v.y;
+      }
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++) {
+        double wr0 = 0.0, wr1 = 0.0, wi0 = 0.0, wi1 = 0.0;
+#pragma unroll
+        for (int kgp = 0; kgp < 2; kgp++) {
+          dmma(wr0, wr1, fa[mb][kgp], cr[kgp]);
+          dmma(wi0, wi1, fa[mb][kgp], ci[kgp]);
+        }
+        cre[mb][nb][0] += sg[mb].x * wr0 - sg[mb].y * wi0; cim[mb][nb][0] += sg[mb].x * wi0 + sg[mb].y * wr0;
+        cre[mb][nb][1] += sg[mb].x * wr1 - sg[mb].y * wi1; cim[mb][nb][1] += sg[mb].x * wi1 + sg[mb].y * wr1;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[s]);
+  }
+  // epilogue as in gemm2_kernel: rows g = lane/4, bands 2*(lane%4)+{0,1}
+  const int npw = Q.npw[ik];
+  const double *kin = Q.kin[ik];
+  const double2 *psi = Q.psi + (size_t)ik * Q.nband * Q.mpw;
+  double2 *hpsi = Q.hpsi + (size_t)ik * Q.nband * Q.mpw;
+#pragma unroll
+  for (int mb = 0; mb < 4; mb++) {
+    int g = tm * NL_BM + wm * 32 + mb * 8 + i;
+    if (g >= npw) continue;
+    double kg = Q.with_kin ? kin[g] : 0.0;
+#pragma unroll
+    for (int nb = 0; nb < 4; nb++) {
+#pragma unroll
+      for (int e = 0; e < 2; e++) {
+        int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j + e;
+        if (b >= Q.nband) continue;
+        size_t off = (size_t)b * Q.mpw + g;
+        double2 r = make_double2(cre[mb][nb][e], cim[mb][nb][e]);
+        if (Q.with_kin) { double2 x = psi[off]; r.x += kg * x.x; r.y += kg * x.y; }
+        if (Q.accumulate) { double2 h = hpsi[off]; r.x += h.x; r.y += h.y; }
+        if (Q.cheb) {
+          double2 y = psi[off], xp = Q.sx != 0.0 ? Q.xprev[(size_t)ik * Q.nband * Q.mpw + off] : make_double2(0.0, 0.0);
+          r.x = Q.sh * r.x + Q.sy * y.x + Q.sx * xp.x; r.y = Q.sh * r.y + Q.sy * y.y + Q.sx * xp.y;
+        }
+        hpsi[off] = r;
+      }
+    }
+  }
+}
+
 // ---------------------------------------------------------------- host side
 typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                              const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -542,6 +777,20 @@ static int make_map(dft_plan *p, CUtensorMap *m, const void *base, uint64_t d0, 
               (unsigned long long)stride2_bytes, box1);
     return DFT_ERR_CUDA;
   }
+  return DFT_OK;
+}
+
+// 3-D FP64 tensor map without swizzle (rows longer than 128 bytes or narrower than a swizzle atom)
+static int make_map_plain(dft_plan *p, CUtensorMap *m, const void *base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t stride1_bytes,
+                          uint64_t stride2_bytes, uint32_t box0, uint32_t box1) {
+  cuuint64_t dims[3] = {d0, d1, d2};
+  cuuint64_t strides[2] = {stride1_bytes, stride2_bytes};
+  cuuint32_t box[3] = {box0, box1, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = ((EncodeFn)p->encode_fn)(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void *>(base), dims, strides, box, estr,
+                                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (plain map, box %u x %u) failed (%d)", box0, box1, (int)r); return DFT_ERR_CUDA; }
   return DFT_OK;
 }
 
@@ -593,6 +842,8 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_fac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FC_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_fac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FD_SMEM));
     g_nl_attr = true;
   }
   const int32_t *d_npw = p->d_npw;
@@ -616,7 +867,8 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   Gemm1Params q1;
   q1.nproj = nproj; q1.nband = nband;
   q1.nslab = (mpw + 7) / 8;
-  q1.tiles_m = (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
+  const bool fac = p->proj_mode == 1;     // factorised projectors: tiles of 16 atoms instead of 128 table rows
+  q1.tiles_m = fac ? (p->natom + FC_BA - 1) / FC_BA : (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
   int ns = p->splitk > 0 ? p->splitk : choose_splitk(q1.tiles_m * q1.tiles_n, q1.nslab, p->sm_count, nkpt);
   if (ns > q1.nslab) ns = q1.nslab;
   q1.slabs_per_split = (q1.nslab + ns - 1) / ns;
@@ -636,9 +888,18 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   q1.part = reinterpret_cast<double2 *>(p->d_part);
   CUtensorMap mapP1, mapPsi, mapP2, mapC;
   uint64_t rowb = (uint64_t)mpw * 16;
-  if ((rc = make_map(p, &mapP1, p->d_ptab, 2 * (uint64_t)mpw, nproj, nkpt, rowb, rowb * nproj, NL_BM))) return rc;
+  if (!fac && (rc = make_map(p, &mapP1, p->d_ptab, 2 * (uint64_t)mpw, nproj, nkpt, rowb, rowb * nproj, NL_BM))) return rc;
   if ((rc = make_map(p, &mapPsi, psi, 2 * (uint64_t)mpw, nband, nkpt, rowb, rowb * nband, NL_BN))) return rc;
-  {
+  CUtensorMap mapS1, mapF1, mapS2, mapF2;
+  if (fac) {
+    if (!p->d_stab || !p->d_fytab) { set_error("factor tables missing"); return DFT_ERR_NOT_READY; }
+    const uint64_t frow = (uint64_t)p->ldf * 8, nfr = (uint64_t)p->ntypat * 8;
+    if ((rc = make_map(p, &mapS1, p->d_stab, 2 * (uint64_t)mpw, p->natom, nkpt, rowb, rowb * p->natom, FC_BA))) return rc;
+    if ((rc = make_map_plain(p, &mapF1, p->d_fytab, p->ldf, nfr, nkpt, frow, frow * nfr, 8, (uint32_t)nfr))) return rc;
+    if ((rc = make_map_plain(p, &mapS2, p->d_stab, 2 * (uint64_t)mpw, p->natom, nkpt, rowb, rowb * p->natom, 2 * NL_BM, 1))) return rc;
+    if ((rc = make_map_plain(p, &mapF2, p->d_fytab, p->ldf, nfr, nkpt, frow, frow * nfr, FD_FLD, (uint32_t)nfr))) return rc;
+  }
+  if (!fac) {
     // GEMM-2 reads P "M-major": view each table row as [g-block][16 doubles] and put the projector
     // index between them, so ONE box {16, 8 rows, 16 g-blocks} brings a 128 g x 8 p tile in the
     // [g-block][p][8 complex] order the fragments want (16 separate 1 KB boxes starved the MMA loop:
@@ -655,7 +916,13 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   }
   if ((rc = make_map(p, &mapC, p->d_cprj, 2 * (uint64_t)nproj, nband, nkpt, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * nband, NL_BN))) return rc;
   phase_begin(p, 5, st);
-  if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  if (fac) {
+    Fac1Params f1;
+    f1.natom = p->natom; f1.nband = nband; f1.nproj = nproj; f1.nslab = q1.nslab; f1.nsplit = q1.nsplit;
+    f1.slabs_per_split = q1.slabs_per_split; f1.tiles_n = q1.tiles_n; f1.ntypat = p->ntypat;
+    f1.typat = p->d_typat; f1.nlmn = p->d_nlmn; f1.atom_first = p->d_atom_first; f1.part = q1.part;
+    gemm1_fac_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1, f1);
+  } else if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   else gemm1_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   phase_end(p, 5, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
@@ -676,7 +943,11 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr;
   int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
   phase_begin(p, 7, st);
-  if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  if (fac) {
+    q2.nslab = p->natom;
+    gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_typat,
+                                                                                      p->d_atom_first, p->ntypat);
+  } else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   else gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   phase_end(p, 7, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());

@@ -59,7 +59,7 @@ static void destroy_plan(dft_plan *p) {
   for (auto &k : p->kp) free_kpoint(k);
   cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
   cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
-  cudaFree(p->d_vtau); cudaFree(p->d_qcart); cudaFree(p->d_qhalf); cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  cudaFree(p->d_stab); cudaFree(p->d_fytab); cudaFree(p->d_vtau); cudaFree(p->d_qcart); cudaFree(p->d_qhalf); cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
@@ -498,6 +498,14 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
   if (!strcmp(key, "fft_path")) {
     if (value < 0 || value > 2) { set_error("fft_path = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->fft_path = (int)value; return DFT_OK;
+  }
+  if (!strcmp(key, "proj_mode")) {
+    if (value < 0 || value > 1) { set_error("proj_mode = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if (value == 1 && p->nproj > 0 && (!p->d_stab || !p->d_fytab)) {
+      int rc = build_factor_tables(p);
+      if (rc) return rc;
+    }
+    p->proj_mode = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "host_groups")) {
     if (value < 1 || value > 64) { set_error("host_groups = %lld outside 1..64", (long long)value); return DFT_ERR_INVALID_ARG; }

@@ -135,4 +135,82 @@ int build_projector_table(dft_plan *p, int ik, double *maxq_out) {
   return DFT_OK;
 }
 
+
+// ------------------------------------------------------------------------------------------
+// Factorised projectors (PAPER.md :477 "computed on-the-fly"): p_{a,i}(m) = FY_{t(a),i}(m) . S_a(m)
+// with FY = F.Y real (one row per projector of an atom TYPE) and S_a(m) = exp(-2 pi i (k+m).x_a) (one row per ATOM).
+// The two small tables replace the [nproj][mpw] complex one: S [natom][mpw] complex, FY [ntypat*8][ldf] real
+// (8 rows per type, rows >= nlmn zero; needs nlmn <= 8), zero for ipw >= npw_k.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(PT_THREADS) stab_kernel(ProjParams P, double2 *__restrict__ stab) {
+  int g = blockIdx.x * PT_THREADS + threadIdx.x, a = blockIdx.y;
+  if (g >= P.mpw) return;
+  double2 v = make_double2(0.0, 0.0);
+  if (g < P.npw) {
+    double t0 = P.k[0] + (double)P.kg[3 * g], t1 = P.k[1] + (double)P.kg[3 * g + 1], t2 = P.k[2] + (double)P.kg[3 * g + 2];
+    const double *x = P.xred + 3 * a;
+    double arg = t0 * x[0] + t1 * x[1] + t2 * x[2];
+    arg -= floor(arg);
+    double sn, cs;
+    sincospi(2.0 * arg, &sn, &cs);
+    v = make_double2(cs, -sn);
+  }
+  stab[(size_t)a * P.mpw + g] = v;
+}
+
+__global__ void __launch_bounds__(PT_THREADS) fytab_kernel(ProjParams P, double *__restrict__ fy, int ldf) {
+  int g = blockIdx.x * PT_THREADS + threadIdx.x, t = blockIdx.y;
+  if (g >= ldf) return;
+  int nl = P.nlmn[t];
+  double *dst = fy + (size_t)t * 8 * ldf + g;
+  if (g >= P.npw) {
+    for (int i = 0; i < 8; i++) dst[(size_t)i * ldf] = 0.0;
+    return;
+  }
+  const double TWO_PI = 6.283185307179586;
+  double t0 = P.k[0] + (double)P.kg[3 * g], t1 = P.k[1] + (double)P.kg[3 * g + 1], t2 = P.k[2] + (double)P.kg[3 * g + 2];
+  double qx = TWO_PI * (t0 * P.bm[0] + t1 * P.bm[3] + t2 * P.bm[6]);
+  double qy = TWO_PI * (t0 * P.bm[1] + t1 * P.bm[4] + t2 * P.bm[7]);
+  double qz = TWO_PI * (t0 * P.bm[2] + t1 * P.bm[5] + t2 * P.bm[8]);
+  double qn = sqrt(qx * qx + qy * qy + qz * qz);
+  for (int i = 0; i < 8; i++) {
+    double v = 0.0;
+    if (i < nl) {
+      int ir = P.lmn_irad[t * P.lmax + i];
+      size_t off = ((size_t)t * P.nrad_max + ir) * P.nq_max;
+      double F = spline_eval(P.nq[t], P.dq[t], P.f + off, P.f2 + off, qn);
+      v = F * real_ylm(P.lmn_l[t * P.lmax + i], P.lmn_m[t * P.lmax + i], qx, qy, qz, qn);
+    }
+    dst[(size_t)i * ldf] = v;
+  }
+}
+
+// Builds (or rebuilds) both tables for every k-point.  DFT_ERR_UNSUPPORTED if some type has more than 8 projectors.
+int build_factor_tables(dft_plan *p) {
+  if (p->natom == 0 || p->nproj == 0 || p->mpw == 0) return DFT_OK;
+  for (int t = 0; t < p->ntypat; t++)
+    if (p->nlmn[t] > 8) { set_error("factorised projectors need nlmn <= 8 per atom type (type %d has %d)", t, p->nlmn[t]); return DFT_ERR_UNSUPPORTED; }
+  if (p->ntypat > 2) { set_error("factorised projectors support at most 2 atom types (got %d)", p->ntypat); return DFT_ERR_UNSUPPORTED; }
+  p->ldf = (p->mpw + 7) / 8 * 8;
+  size_t sbytes = (size_t)p->nkpt * p->natom * p->mpw * 16 + 256, fbytes = (size_t)p->nkpt * p->ntypat * 8 * p->ldf * 8 + 256;
+  if (!p->d_stab && cudaMalloc(&p->d_stab, sbytes) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the structure-factor table (%zu bytes)", sbytes); return DFT_ERR_ALLOC; }
+  if (!p->d_fytab && cudaMalloc(&p->d_fytab, fbytes) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the form-factor table (%zu bytes)", fbytes); return DFT_ERR_ALLOC; }
+  for (int ik = 0; ik < p->nkpt; ik++) {
+    KPoint &kp = p->kp[ik];
+    ProjParams P;
+    for (int i = 0; i < 9; i++) P.bm[i] = p->bm[i];
+    for (int i = 0; i < 3; i++) P.k[i] = kp.k[i];
+    P.npw = kp.npw; P.mpw = p->mpw; P.natom = p->natom; P.lmax = p->lmax; P.nrad_max = p->nrad_max; P.nq_max = p->nq_max;
+    P.kg = kp.kg; P.typat = p->d_typat; P.nlmn = p->d_nlmn; P.lmn_l = p->d_lmn_l; P.lmn_m = p->d_lmn_m;
+    P.lmn_irad = p->d_lmn_irad; P.atom_first = p->d_atom_first; P.nq = p->d_nq; P.dq = p->d_dq; P.xred = p->d_xred;
+    P.f = p->d_f; P.f2 = p->d_f2; P.ptab = nullptr;
+    stab_kernel<<<dim3((p->mpw + PT_THREADS - 1) / PT_THREADS, p->natom), PT_THREADS>>>(
+        P, reinterpret_cast<double2 *>(p->d_stab) + (size_t)ik * p->natom * p->mpw);
+    fytab_kernel<<<dim3((p->ldf + PT_THREADS - 1) / PT_THREADS, p->ntypat), PT_THREADS>>>(
+        P, p->d_fytab + (size_t)ik * p->ntypat * 8 * p->ldf, p->ldf);
+  }
+  DFT_CUDA_CHECK(cudaDeviceSynchronize());
+  return DFT_OK;
+}
+
 }  // namespace dftb200

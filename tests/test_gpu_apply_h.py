@@ -265,6 +265,44 @@ def test_meta_gga_term(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c1m", "c4m", "c2m", "aniso", "c3k2"])
+def test_factorised_projectors(name):
+    """Option proj_mode = 1 (PAPER.md :477 "computed on-the-fly"): p = FY . S evaluated inside both GEMMs instead of the
+    materialised table; H psi, S psi and cprj must match the oracle as before.  Types with more than 8 projectors are refused."""
+    import paper_2507_08578_b200 as dft
+    cfg, plan, sph = _setup(name)
+    if max(t["nlmn"] for t in cfg["types"]) > 8:
+        with pytest.raises(dft.DftError) as ei:
+            plan.set_option("proj_mode", 1)
+        assert ei.value.code == dft.DFT_ERR_UNSUPPORTED
+        plan.destroy()
+        return
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    tpsi = torch.as_tensor(psi, device="cuda")
+    plan.set_option("proj_mode", 1)
+    m = 1 if name == "aniso" else 2
+    for terms in (15, 4):
+        plan.set_option("terms", terms)
+        ref = oracle_apply(cfg, sph, psi, terms=terms & 7, method=m)
+        err = band_rel_err(gpu_apply(plan, psi), ref)
+        assert err <= TOL, "%s terms=%d: %.3e" % (name, terms, err)
+    cp = plan.get_cprj(tpsi).cpu().numpy()
+    rng = np.random.default_rng(3)
+    sij = rng.standard_normal(cfg["dij"].shape) * 0.3
+    sij = 0.5 * (sij + sij.transpose(0, 2, 1))
+    plan.set_sij(sij)
+    got = plan.apply_s(tpsi).cpu().numpy()
+    for ik, (kg, ig, kin) in enumerate(sph):
+        cref = oracle.cprj(cfg, ik, kg, psi[ik][:, :len(ig)]).T
+        assert float(np.max(np.linalg.norm(cp[ik] - cref, axis=1) / np.linalg.norm(cref, axis=1))) <= TOL
+        sref = oracle.apply_s(cfg, ik, kg, psi[ik], sij)
+        assert float(np.max(np.linalg.norm(got[ik] - sref, axis=1) / np.linalg.norm(sref, axis=1))) <= TOL
+    plan.set_option("proj_mode", 0)
+    plan.set_option("terms", 15)
+    assert band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, method=m)) <= TOL
+    plan.destroy()
+
+
 def test_apply_h_is_cuda_graph_capturable():
     """dft_apply_h only enqueues (no allocation or synchronisation once scratch exists), so a launch-bound small cell
     can be captured into a CUDA graph and replayed."""

@@ -62,7 +62,7 @@ struct Fft2Batch {
 };
 
 // ---- pass A: sphere -> x-lines (type I).  block = lpc lines x NS slots, slot fastest; grid = nb * ntile
-template <int R1, int R2, bool BATCH>
+template <int R1, int R2, bool BATCH, bool EXTRA>
 __global__ void __launch_bounds__(F2_THREADS, 2)
 fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *__restrict__ T1, int lpc, int ntile,
                   const double *__restrict__ pre) {
@@ -83,7 +83,7 @@ fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *
     for (int j1 = 0; j1 < R1; j1++) {
       int g = ok ? run_map(r, s + R2 * j1) : -1;
       v[j1] = g >= 0 ? src[g] : make_double2(0.0, 0.0);
-      if (pre && g >= 0) v[j1] = cscale(v[j1], __ldg(pre + g));     // diagonal factor in G space before the transform
+      if (EXTRA && pre && g >= 0) v[j1] = cscale(v[j1], __ldg(pre + g));     // diagonal factor in G space before the transform
     }
     Dft<R1, +1>::run(v);
 #pragma unroll
@@ -105,7 +105,7 @@ fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *
 }
 
 // ---- pass A^-1: x-lines -> sphere (type II) + zero the pad entries ipw >= npw of the band
-template <int R1, int R2, bool BATCH>
+template <int R1, int R2, bool BATCH, bool EXTRA>
 __global__ void __launch_bounds__(F2_THREADS, 2)
 fft2_a_inv_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ T1, cplx *__restrict__ hpsi, int lpc, int ntile,
                   const double *__restrict__ post, int accumulate) {
@@ -140,13 +140,16 @@ fft2_a_inv_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ T1, cplx *_
     for (int d = 0; d < R1; d++) {
       int g = ok ? run_map(r, s + R2 * d) : -1;
       if (g >= 0) {
-        cplx o = post ? cscale(v[d], __ldg(post + g)) : v[d];        // diagonal factor in G space after the transform
-        if (accumulate) { cplx h = dst[g]; o.x += h.x; o.y += h.y; }
+        cplx o = v[d];
+        if (EXTRA) {
+          if (post) o = cscale(o, __ldg(post + g));                  // diagonal factor in G space after the transform
+          if (accumulate) { cplx h = dst[g]; o.x += h.x; o.y += h.y; }
+        }
         dst[g] = o;
       }
     }
   }
-  if (tile == ntile - 1 && !accumulate)
+  if (tile == ntile - 1 && !(EXTRA && accumulate))
     for (int g = G.npw + t; g < G.mpw; g += blockDim.x) dst[g] = make_double2(0.0, 0.0);
 }
 
@@ -796,11 +799,21 @@ static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi
     int64_t grid = (int64_t)nb * ntile;
     if (grid > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
     if (pass == 0) {
-      if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, false>, sm))) return rc;
-      fft2_a_fwd_kernel<R1, R2, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), psi, T1, lpc, ntile, X.pre);
+      if (X.pre) {
+        if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, false, true>, sm))) return rc;
+        fft2_a_fwd_kernel<R1, R2, false, true><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), psi, T1, lpc, ntile, X.pre);
+      } else {
+        if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, false, false>, sm))) return rc;
+        fft2_a_fwd_kernel<R1, R2, false, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), psi, T1, lpc, ntile, nullptr);
+      }
     } else {
-      if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, false>, sm))) return rc;
-      fft2_a_inv_kernel<R1, R2, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), T1, hpsi, lpc, ntile, X.post, X.accumulate);
+      if (X.post || X.accumulate) {
+        if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, false, true>, sm))) return rc;
+        fft2_a_inv_kernel<R1, R2, false, true><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), T1, hpsi, lpc, ntile, X.post, X.accumulate);
+      } else {
+        if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, false, false>, sm))) return rc;
+        fft2_a_inv_kernel<R1, R2, false, false><<<(unsigned)grid, lpc * NS, sm, st>>>(G, Fft2Batch(), T1, hpsi, lpc, ntile, nullptr, 0);
+      }
     }
   } else {
     int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
@@ -837,11 +850,11 @@ static int launch_pass_batched(const Fft2Geom &G, const Fft2Batch &B, int nk, in
     int64_t grid = (int64_t)nb * ntile;
     if (grid > 0x7fffffffLL) return DFT_ERR_UNSUPPORTED;
     if (pass == 0) {
-      if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, true>, sm))) return rc;
-      fft2_a_fwd_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, psi, T1, lpc, ntile, nullptr);
+      if ((rc = set_smem(fft2_a_fwd_kernel<R1, R2, true, false>, sm))) return rc;
+      fft2_a_fwd_kernel<R1, R2, true, false><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, psi, T1, lpc, ntile, nullptr);
     } else {
-      if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, true>, sm))) return rc;
-      fft2_a_inv_kernel<R1, R2, true><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, T1, hpsi, lpc, ntile, nullptr, 0);
+      if ((rc = set_smem(fft2_a_inv_kernel<R1, R2, true, false>, sm))) return rc;
+      fft2_a_inv_kernel<R1, R2, true, false><<<dim3((unsigned)grid, nk), lpc * NS, sm, st>>>(G, B, T1, hpsi, lpc, ntile, nullptr, 0);
     }
   } else {
     int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;

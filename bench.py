@@ -330,6 +330,25 @@ def main():
                            "api": "dft_accumulate_density"}
         del rho
 
+    # ---- context figure: the same step with factorised projectors (option proj_mode = 1)
+    if args.cheb_degree > 0 and world == 1 and not args.proj_mode:
+        try:
+            plan.set_option("proj_mode", 1)
+            plan.apply_h(psi, hpsi)
+            torch.cuda.synchronize()
+            f0 = torch.cuda.Event(enable_timing=True); f1 = torch.cuda.Event(enable_timing=True)
+            f0.record()
+            for _ in range(2):
+                plan.apply_h(psi, hpsi)
+            f1.record()
+            torch.cuda.synchronize()
+            fms = f0.elapsed_time(f1) / 2
+            line["factorised_projectors"] = {"value": units / (fms * 1e-3), "unit": UNIT, "ms_per_step": fms,
+                                             "option": "proj_mode = 1 (FY.S tables instead of the materialised projector table)"}
+        except dft.DftError as e:
+            line["factorised_projectors"] = {"unavailable": str(e)}
+        plan.set_option("proj_mode", 0)
+
     # ---- e2e: same metric through dft_apply_h_host, host<->device copies inside the timed region
     if not args.no_e2e:
         psi_h = torch.empty(psi.shape, dtype=psi.dtype, pin_memory=True)

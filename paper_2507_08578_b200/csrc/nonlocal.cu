@@ -529,7 +529,7 @@ gemm2_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant_
 //            cprj[a,i,b] = sum_G FY[i,G] z_{a,b}(G)            (2 DMMA per 8 x 8 x 4 block: re and im columns)
 // 2 DMMAs + 4 FP64 instructions where the 4-product form needs 4 DMMAs and the Gauss form 3 (+ sums): 40 against 64 /
 // 49 pipe clocks per block.  M = 8 of the m8n8k4 shape is the 8 projectors of one atom, so the CTA tile is
-// 16 atoms x 64 bands (8 warps, 4 atoms x 32 bands each, the accumulator layout of the 4-product kernel).
+// 16 atoms x 64 bands (16 warps, 4 atoms x 16 bands each).
 constexpr int FC_BA = 16;                  // atoms per CTA tile
 constexpr int FC_OFF_S = NL_BN * 128;      // stage layout: psi tile 8 KB | S tile 2 KB | FY tile <= 1 KB
 constexpr int FC_OFF_F = FC_OFF_S + FC_BA * 128;
@@ -537,6 +537,8 @@ constexpr int FC_STAGE_BYTES = 11 * 1024;
 constexpr int FC_STAGES = 8;
 constexpr int FC_PREFETCH = FC_STAGES - 2;
 constexpr int FC_SMEM = FC_STAGES * FC_STAGE_BYTES + 1024 + 256;
+constexpr int FC_WARPS = 16;               // 4 (atom groups) x 4 (band groups): four warps per SM sub-partition hide the
+constexpr int FC_THREADS = FC_WARPS * 32;  // DMUL -> DFMA -> DMMA chains of the z = conj(S) psi products
 
 struct Fac1Params {
   int natom, nband, nproj, nslab, nsplit, slabs_per_split, tiles_n, ntypat;
@@ -545,14 +547,14 @@ struct Fac1Params {
 };
 
 // grid: (tiles_a * tiles_n, nsplit, nkpt)
-__global__ void __launch_bounds__(NL_THREADS, 1)
+__global__ void __launch_bounds__(FC_THREADS, 1)
 gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_constant__ CUtensorMap mapS,
                  const __grid_constant__ CUtensorMap mapF, Fac1Params Q) {
   extern __shared__ unsigned char smem_raw[];
   unsigned char *tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   uint64_t *full = reinterpret_cast<uint64_t *>(tiles + FC_STAGES * FC_STAGE_BYTES), *empty = full + FC_STAGES;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < FC_STAGES; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], NL_CONSUMERS); }
+    for (int s = 0; s < FC_STAGES; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], FC_WARPS); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -572,7 +574,7 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
   const bool producer = (threadIdx.x == 0);
   if (producer)
     for (int j = 0; j < FC_PREFETCH && j < ns; j++) issue(j);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wm = warp >> 1, wn = warp & 1;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wm = warp >> 2, wn = warp & 3;   // 4 atoms x 16 bands per warp
   const int i = lane >> 2, j = lane & 3;
   int frow[4];   // byte offset of this lane's FY row (its atom's type, projector i) inside the FY tile
 #pragma unroll
@@ -580,11 +582,11 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
     int atom = ta * FC_BA + wm * 4 + q;
     frow[q] = ((atom < Q.natom ? Q.typat[atom] : 0) * 8 + i) * 64;
   }
-  double cre[4][4][2], cim[4][4][2];
+  double cre[4][2][2], cim[4][2][2];
 #pragma unroll
   for (int a = 0; a < 4; a++)
 #pragma unroll
-    for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
+    for (int b = 0; b < 2; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
   for (int it = 0; it < ns; it++) {
     if (producer && it + FC_PREFETCH < ns) issue(it + FC_PREFETCH);
     __syncwarp();
@@ -594,10 +596,10 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
 #pragma unroll
     for (int kg = 0; kg < 2; kg++) {
       const int e = 2 * j + kg;   // this lane's G inside the slab (k index of the 8x8x4 block)
-      double pr[4], pi[4];
-      const unsigned char *b0 = Ps + (wn * 32 + i) * 128 + ((e ^ i) << 4);
+      double pr[2], pi[2];
+      const unsigned char *b0 = Ps + (wn * 16 + i) * 128 + ((e ^ i) << 4);
 #pragma unroll
-      for (int nb = 0; nb < 4; nb++) {
+      for (int nb = 0; nb < 2; nb++) {
         double2 v = *reinterpret_cast<const double2 *>(b0 + nb * 8 * 128);
         pr[nb] = v.x; pi[nb] = v.y;
       }
@@ -607,7 +609,7 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
         const double2 sg = *reinterpret_cast<const double2 *>(Ss + arow * 128 + ((e ^ (arow & 7)) << 4));
         const double fa = *reinterpret_cast<const double *>(Fs + frow[q] + e * 8);
 #pragma unroll
-        for (int nb = 0; nb < 4; nb++) {
+        for (int nb = 0; nb < 2; nb++) {
           double zr = sg.x * pr[nb] + sg.y * pi[nb], zi = sg.x * pi[nb] - sg.y * pr[nb];   // conj(S) psi
           dmma(cre[q][nb][0], cre[q][nb][1], fa, zr);
           dmma(cim[q][nb][0], cim[q][nb][1], fa, zi);
@@ -626,8 +628,8 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
     if (i >= Q.nlmn[Q.typat[atom]]) continue;
     double2 *row = out + (size_t)(Q.atom_first[atom] + i) * Q.nband;
 #pragma unroll
-    for (int nb = 0; nb < 4; nb++) {
-      int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j;
+    for (int nb = 0; nb < 2; nb++) {
+      int b = tn * NL_BN + wn * 16 + nb * 8 + 2 * j;
       if (b < Q.nband) row[b] = make_double2(cre[q][nb][0], cim[q][nb][0]);
       if (b + 1 < Q.nband) row[b + 1] = make_double2(cre[q][nb][1], cim[q][nb][1]);
     }
@@ -647,7 +649,7 @@ constexpr int FD_FBYTES = 2 * 8 * FD_FLD * 8;         // up to two atom types
 constexpr int FD_SMEM = FD_STAGES * FD_STAGE_BYTES + FD_FBYTES + 1024 + 256;
 
 // grid: (tiles_n * tiles_m, 1, nkpt); Q as in gemm2_kernel, nslab = natom
-__global__ void __launch_bounds__(NL_THREADS, 1)
+__global__ void __launch_bounds__(FC_THREADS, 1)
 gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant__ CUtensorMap mapS,
                  const __grid_constant__ CUtensorMap mapF, Gemm2Params Q, const int32_t *__restrict__ typat,
                  const int32_t *__restrict__ atom_first, int ntypat) {
@@ -656,13 +658,13 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
   unsigned char *Fs = tiles + FD_STAGES * FD_STAGE_BYTES;
   uint64_t *full = reinterpret_cast<uint64_t *>(Fs + FD_FBYTES), *empty = full + FD_STAGES, *fbar = empty + FD_STAGES;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < FD_STAGES; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], NL_CONSUMERS); }
+    for (int s = 0; s < FD_STAGES; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], FC_WARPS); }
     mbar_init(fbar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
   const int tn = blockIdx.x % Q.tiles_n, tm = blockIdx.x / Q.tiles_n, ik = blockIdx.z;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wm = warp >> 1, wn = warp & 1;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wm = warp >> 2, wn = warp & 3;   // 32 G x 16 bands per warp
   const int i = lane >> 2, j = lane & 3;
   const int ns = Q.with_nl ? Q.nslab : 0;
   auto issue = [&](int a) {
@@ -679,11 +681,11 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
     tma_load_3d(Fs, &mapF, fbar, tm * NL_BM, 0, ik);
     for (int a = 0; a < FD_PREFETCH && a < ns; a++) issue(a);
   }
-  double cre[4][4][2], cim[4][4][2];
+  double cre[4][2][2], cim[4][2][2];
 #pragma unroll
   for (int a = 0; a < 4; a++)
 #pragma unroll
-    for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
+    for (int b = 0; b < 2; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
   if (ns > 0) mbar_wait(fbar, 0);
   for (int a = 0; a < ns; a++) {
     if (producer && a + FD_PREFETCH < ns) issue(a + FD_PREFETCH);
@@ -703,9 +705,9 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
         fa[mb][kgp] = *reinterpret_cast<const double *>(Fs + ((size_t)((t * 8 + 2 * j + kgp) * FD_FLD + g)) * 8);
     }
 #pragma unroll
-    for (int nb = 0; nb < 4; nb++) {
+    for (int nb = 0; nb < 2; nb++) {
       double cr[2], ci[2];
-      const unsigned char *b0 = Cs + (wn * 32 + nb * 8 + i) * 128;
+      const unsigned char *b0 = Cs + (wn * 16 + nb * 8 + i) * 128;
 #pragma unroll
       for (int kgp = 0; kgp < 2; kgp++) {
         double2 v = *reinterpret_cast<const double2 *>(b0 + (((2 * j + kgp) ^ i) << 4));
@@ -737,10 +739,10 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
     if (g >= npw) continue;
     double kg = Q.with_kin ? kin[g] : 0.0;
 #pragma unroll
-    for (int nb = 0; nb < 4; nb++) {
+    for (int nb = 0; nb < 2; nb++) {
 #pragma unroll
       for (int e = 0; e < 2; e++) {
-        int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j + e;
+        int b = tn * NL_BN + wn * 16 + nb * 8 + 2 * j + e;
         if (b >= Q.nband) continue;
         size_t off = (size_t)b * Q.mpw + g;
         double2 r = make_double2(cre[mb][nb][e], cim[mb][nb][e]);
@@ -921,7 +923,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     f1.natom = p->natom; f1.nband = nband; f1.nproj = nproj; f1.nslab = q1.nslab; f1.nsplit = q1.nsplit;
     f1.slabs_per_split = q1.slabs_per_split; f1.tiles_n = q1.tiles_n; f1.ntypat = p->ntypat;
     f1.typat = p->d_typat; f1.nlmn = p->d_nlmn; f1.atom_first = p->d_atom_first; f1.part = q1.part;
-    gemm1_fac_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1, f1);
+    gemm1_fac_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), FC_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1, f1);
   } else if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   else gemm1_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   phase_end(p, 5, st, 1);
@@ -945,7 +947,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   phase_begin(p, 7, st);
   if (fac) {
     q2.nslab = p->natom;
-    gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_typat,
+    gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_typat,
                                                                                       p->d_atom_first, p->ntypat);
   } else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   else gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);

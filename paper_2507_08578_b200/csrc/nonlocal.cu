@@ -721,8 +721,11 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
           dmma(wr0, wr1, fa[mb][kgp], cr[kgp]);
           dmma(wi0, wi1, fa[mb][kgp], ci[kgp]);
         }
-        cre[mb][nb][0] += sg[mb].x * wr0 - sg[mb].y * wi0; cim[mb][nb][0] += sg[mb].x * wi0 + sg[mb].y * wr0;
-        cre[mb][nb][1] += sg[mb].x * wr1 - sg[mb].y * wi1; cim[mb][nb][1] += sg[mb].x * wi1 + sg[mb].y * wr1;
+        // acc += S_a(G) w: two fused multiply-adds per component (written out so that no separate add is generated)
+        cre[mb][nb][0] = fma(-sg[mb].y, wi0, fma(sg[mb].x, wr0, cre[mb][nb][0]));
+        cim[mb][nb][0] = fma(sg[mb].y, wr0, fma(sg[mb].x, wi0, cim[mb][nb][0]));
+        cre[mb][nb][1] = fma(-sg[mb].y, wi1, fma(sg[mb].x, wr1, cre[mb][nb][1]));
+        cim[mb][nb][1] = fma(sg[mb].y, wr1, fma(sg[mb].x, wi1, cim[mb][nb][1]));
       }
     }
     __syncwarp();

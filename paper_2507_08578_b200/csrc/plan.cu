@@ -395,6 +395,7 @@ int dft_plan_get_projectors(const dft_plan *p, int32_t ik, double *ptab) {
   if (ik < 0 || ik >= p->nkpt) { set_error("ik = %d outside 0..%d", ik, p->nkpt - 1); return DFT_ERR_INVALID_ARG; }
   int npw = p->kp[ik].npw;
   if (p->nproj == 0 || npw == 0) return DFT_OK;
+  if (!p->d_ptab) { set_error("the projector table is not materialised while proj_mode = 1"); return DFT_ERR_NOT_READY; }
   const double *src = p->d_ptab + (size_t)ik * p->nproj * p->mpw * 2;
   DFT_CUDA_CHECK(cudaMemcpy2D(ptab, (size_t)npw * 16, src, (size_t)p->mpw * 16, (size_t)npw * 16, p->nproj, cudaMemcpyDeviceToHost));
   return DFT_OK;
@@ -501,9 +502,24 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
   }
   if (!strcmp(key, "proj_mode")) {
     if (value < 0 || value > 1) { set_error("proj_mode = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
-    if (value == 1 && p->nproj > 0 && (!p->d_stab || !p->d_fytab)) {
-      int rc = build_factor_tables(p);
-      if (rc) return rc;
+    if (value == 1 && p->nproj > 0) {
+      if (!p->d_stab || !p->d_fytab) {
+        int rc = build_factor_tables(p);
+        if (rc) return rc;
+      }
+      // the materialised table is not needed in this mode: give its memory back (19.4 GB at c4)
+      DFT_CUDA_CHECK(cudaDeviceSynchronize());
+      cudaFree(p->d_ptab); p->d_ptab = nullptr;
+    }
+    if (value == 0 && p->nproj > 0 && p->mpw > 0 && !p->d_ptab) {
+      size_t tab = (size_t)p->nkpt * p->nproj * p->mpw * 16;
+      if (cudaMalloc(&p->d_ptab, tab + 256) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the projector table (%zu bytes)", tab); return DFT_ERR_ALLOC; }
+      for (int ik = 0; ik < p->nkpt; ik++) {
+        double maxq;
+        int rc = build_projector_table(p, ik, &maxq);
+        if (rc) return rc;
+      }
+      DFT_CUDA_CHECK(cudaDeviceSynchronize());
     }
     p->proj_mode = (int)value; return DFT_OK;
   }

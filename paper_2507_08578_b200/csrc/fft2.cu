@@ -472,8 +472,9 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
                    const double *__restrict__ vloc, RingParams Q) {
   constexpr int NS = imax(R1, R2);
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int XT = Q.XT, KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
-  const int exn = imax(R1 * KSa, R2 * KSb);
+  constexpr int XT = (F2_THREADS / NS) & ~7;     // a function of the radices only: all tile addressing is immediate
+  constexpr int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
+  constexpr int exn = imax(R1 * KSa, R2 * KSb);
   unsigned char *stages = smem_raw;
   cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
   double *vs = reinterpret_cast<double *>(sm + exn);
@@ -573,7 +574,8 @@ fft2_density_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, const
                     double *__restrict__ rho, RingParams Q) {
   constexpr int NS = imax(R1, R2);
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int XT = Q.XT, KSa = pad8(R2 * XT, XT);
+  constexpr int XT = (F2_THREADS / NS) & ~7;
+  constexpr int KSa = pad8(R2 * XT, XT);
   unsigned char *stages = smem_raw;
   cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
   cplx *tws = sm + R1 * KSa;
@@ -719,7 +721,7 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
     XT = (F2_THREADS / NS) & ~7;
     if (XT < 8) return DFT_ERR_UNSUPPORTED;
     int64_t nxy = (int64_t)G.n1 * G.n2;
-    if (XT > nxy) XT = (int)((nxy + 1) & ~1LL);
+    if (XT > nxy) return DFT_ERR_UNSUPPORTED;    // tiny planes: the plain kernel
     nxt = (int)((nxy + XT - 1) / XT);
   }
   if (XT * NS > F2_THREADS) return DFT_ERR_UNSUPPORTED;
@@ -935,7 +937,7 @@ static int launch_density(dft_plan *p, const Fft2Geom &G, cplx *T2, const double
   int XT = (F2_THREADS / NS) & ~7;
   if (XT < 8) return DFT_ERR_UNSUPPORTED;
   const int64_t nxy = (int64_t)G.n1 * G.n2;
-  if (XT > nxy) XT = (int)((nxy + 1) & ~1LL);
+  if (XT > nxy) return DFT_ERR_UNSUPPORTED;
   RingParams Q;
   Q.XT = XT; Q.nxt = (int)((nxy + XT - 1) / XT); Q.nb = nb; Q.ntiles = 0;
   Q.box_bytes = (uint32_t)((size_t)G.nplane * XT * 16);

@@ -749,12 +749,26 @@ int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int
   }
   if (!p->h2d_stream) DFT_CUDA_CHECK(cudaStreamCreateWithFlags(&p->h2d_stream, cudaStreamNonBlocking));
   if (!p->d2h_stream) DFT_CUDA_CHECK(cudaStreamCreateWithFlags(&p->d2h_stream, cudaStreamNonBlocking));
-  const int per = ((nband + ngroup - 1) / ngroup + 63) / 64 * 64;   // whole GEMM band tiles per group
+  // group sizes in whole GEMM band tiles of 64.  Only the copy-in of the first group and the copy-out of the last one
+  // are exposed, so with enough bands those two groups are one tile each and the rest is split evenly.
+  std::vector<int> sizes;
+  {
+    const int per = ((nband + ngroup - 1) / ngroup + 63) / 64 * 64;
+    if (ngroup >= 4 && nband >= 64 * 2 * ngroup) {
+      const int mid = ngroup - 2, rest = nband - 128, permid = ((rest + mid - 1) / mid + 63) / 64 * 64;
+      sizes.push_back(64);
+      for (int left = rest; left > 0; left -= permid) sizes.push_back(left < permid ? left : permid);
+      sizes.push_back(64);
+    } else {
+      for (int left = nband; left > 0; left -= per) sizes.push_back(left < per ? left : per);
+    }
+  }
   std::vector<cudaEvent_t> ev;
   int64_t launches = 0;
   int rc = DFT_OK;
-  for (int b0 = 0; b0 < nband && rc == DFT_OK; b0 += per) {
-    const int nb = nband - b0 < per ? nband - b0 : per;
+  int b0 = 0;
+  for (size_t gi = 0; gi < sizes.size() && rc == DFT_OK; b0 += sizes[gi], gi++) {
+    const int nb = sizes[gi];
     const size_t off = (size_t)b0 * p->mpw * 2, gbytes = (size_t)nb * p->mpw * 16;
     cudaEvent_t in_done, k_done;
     if (cudaEventCreateWithFlags(&in_done, cudaEventDisableTiming) != cudaSuccess ||

@@ -377,6 +377,22 @@ def test_host_api_band_groups():
     plan.destroy()
 
 
+def test_host_api_uneven_groups():
+    """With enough bands the first and last groups of dft_apply_h_host are one 64-band tile each (their copies are the
+    only exposed ones): 520 bands, 4 groups -> 64, 256, 136, 64."""
+    cfg, plan, sph = _setup("c1m", nband=520)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    plan.set_option("host_groups", 4)
+    got = plan.apply_h_host(psi)
+    assert plan.last_launches() == 8 * 4
+    ref = gpu_apply(plan, psi)
+    assert band_rel_err(got, ref) <= 1e-13
+    sample = [0, 63, 64, 319, 320, 455, 456, 519]
+    oref = oracle_apply(cfg, sph, psi[:, sample])
+    assert band_rel_err(got[:, sample], oref) <= TOL
+    plan.destroy()
+
+
 def test_c1_full():
     cfg, plan, sph = _setup("c1")
     psi = synth.gen_psi(cfg, [s[2] for s in sph])

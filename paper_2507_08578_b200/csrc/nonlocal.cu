@@ -823,8 +823,10 @@ static bool g_nl_attr = false;
 // choose the number of K splits of GEMM-1: fill the SMs in whole waves, keep >= 32 slabs per split
 static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
   int best = 1; double best_eff = 0.0;
+  // at least 32 slabs per split when the tiles alone fill the SMs; small problems (latency-bound) may go down to 8
+  const int min_slabs = (int64_t)tiles * nkpt >= sm_count ? 32 : 8;
   for (int s = 1; s <= 64; s++) {
-    if (s > 1 && nslab / s < 32) break;
+    if (s > 1 && nslab / s < min_slabs) break;
     double units = (double)tiles * s * nkpt;
     double waves = units / sm_count;
     double eff = waves / (double)(int64_t)(waves + 0.999999);

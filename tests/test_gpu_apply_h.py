@@ -377,6 +377,24 @@ def test_host_api_band_groups():
     plan.destroy()
 
 
+def test_multik_host_api_and_small_user_workspace():
+    """Several k-points: the host API takes its single-copy path, and a caller-owned workspace too small for the
+    all-k-points-per-launch FFT path makes the library fall back to one k-point per launch; same result either way."""
+    cfg, plan, sph = _setup("c3k2")
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    ref = oracle_apply(cfg, sph, psi)
+    assert band_rel_err(gpu_apply(plan, psi), ref) <= TOL
+    batched_launches = plan.last_launches()
+    assert band_rel_err(plan.apply_h_host(psi), ref) <= TOL
+    ws = torch.empty(plan.workspace_bytes_per_band + 256, dtype=torch.uint8, device="cuda")
+    off = (-ws.data_ptr()) % 256
+    plan.set_workspace(ws[off:off + plan.workspace_bytes_per_band])
+    assert band_rel_err(gpu_apply(plan, psi), ref) <= TOL
+    assert plan.last_launches() > batched_launches            # one band and one k-point per launch now
+    plan.set_workspace(None)
+    plan.destroy()
+
+
 def test_host_api_uneven_groups():
     """With enough bands the first and last groups of dft_apply_h_host are one 64-band tile each (their copies are the
     only exposed ones): 520 bands, 4 groups -> 64, 256, 136, 64."""

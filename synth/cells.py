@@ -23,7 +23,7 @@ BASE_SEED = 20250708
 STREAM_PSI, STREAM_VNOISE, STREAM_DIJ = 1, 2, 3
 
 CONFIG_NAMES = ("c0", "c1", "c2", "c3", "c4",
-                "c1m", "c2m", "c4m", "aniso", "c3k2")
+                "c1m", "c2m", "c4m", "aniso", "c3k2", "aniso8")
 
 _DIAMOND_SITES = np.array([[0, 0, 0], [0, .5, .5], [.5, 0, .5], [.5, .5, 0],
                            [.25, .25, .25], [.25, .75, .75], [.75, .25, .75], [.75, .75, .25]])
@@ -61,6 +61,9 @@ def _proj_type(kind, qmax, dq=0.01):
     elif kind == "Al":        # l=0,1,2 x 1 radial (rc 1.2) -> 9 projectors
         rads = [(0, 1.2), (1, 1.2), (2, 1.2)]
         lmn = [(0, 0, 0)] + [(1, m, 1) for m in (-1, 0, 1)] + [(2, m, 2) for m in (-2, -1, 0, 1, 2)]
+    elif kind == "Sip":       # test-only second light type: l=0 (rc 0.9), l=1 (rc 0.8) -> 4 projectors
+        rads = [(0, 0.9), (1, 0.8)]
+        lmn = [(0, 0, 0)] + [(1, m, 1) for m in (-1, 0, 1)]
     else:
         raise ValueError(kind)
     nq = int(np.ceil(1.05 * qmax / dq)) + 2
@@ -167,6 +170,13 @@ def make_config(name, with_vloc=True, **over):
         kinds = ["Si", "Al"]; typat = np.array([0, 1, 0], np.int32)
         kpt = [[0.1, -0.2, 0.05]]
         ecut, ngfft, nband = 2.5, (20, 24, 30), 4
+    elif name == "aniso8":    # aniso with two types of at most 8 projectors (8 and 4): rows of one atom are not 8-aligned
+        rprimd = np.array([[9.0, 0.4, -0.3], [0.7, 10.5, 0.5], [-0.6, 0.8, 13.0]])
+        xred = np.array([[0.0, 0.0, 0.0], [0.3183098861837907, 0.7071067811865476, 0.5772156649015329],
+                         [0.55, 0.25, 0.8], [0.12, 0.61, 0.33]])
+        kinds = ["Si", "Sip"]; typat = np.array([1, 0, 1, 0], np.int32)
+        kpt = [[0.1, -0.2, 0.05]]
+        ecut, ngfft, nband = 2.5, (20, 24, 30), 5
     else:
         raise ValueError(name)
     ecut = float(over.get("ecut", ecut))

@@ -21,14 +21,14 @@ def _setup(name, **over):
     return cfg, plan, sph
 
 
-@pytest.mark.parametrize("name", ["c0", "c1m", "c2m", "c4m", "aniso", "c3k2"])
+@pytest.mark.parametrize("name", ["c0", "c1m", "c2m", "c4m", "aniso", "aniso8", "c3k2"])
 def test_small_cells_all_terms_and_isolations(name):
     cfg, plan, sph = _setup(name)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     for terms in (7, 1, 2, 4, 3, 6):
         plan.set_option("terms", terms)
         got = gpu_apply(plan, psi)
-        ref = oracle_apply(cfg, sph, psi, terms=terms, method=1 if name in ("c0", "aniso") else 2)
+        ref = oracle_apply(cfg, sph, psi, terms=terms, method=1 if name in ("c0", "aniso", "aniso8") else 2)
         err = band_rel_err(got, ref)
         assert err <= TOL, "%s terms=%d: rel err %.3e" % (name, terms, err)
         for ik in range(plan.nkpt):                      # pad entries are written as 0
@@ -265,7 +265,7 @@ def test_meta_gga_term(name):
     plan.destroy()
 
 
-@pytest.mark.parametrize("name", ["c1m", "c4m", "c2m", "aniso", "c3k2"])
+@pytest.mark.parametrize("name", ["c1m", "c4m", "c2m", "aniso", "aniso8", "c3k2"])
 def test_factorised_projectors(name):
     """Option proj_mode = 1 (PAPER.md :477 "computed on-the-fly"): p = FY . S evaluated inside both GEMMs instead of the
     materialised table; H psi, S psi and cprj must match the oracle as before.  Types with more than 8 projectors are refused."""
@@ -280,7 +280,7 @@ def test_factorised_projectors(name):
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     tpsi = torch.as_tensor(psi, device="cuda")
     plan.set_option("proj_mode", 1)
-    m = 1 if name == "aniso" else 2
+    m = 1 if name.startswith("aniso") else 2
     for terms in (15, 4):
         plan.set_option("terms", terms)
         ref = oracle_apply(cfg, sph, psi, terms=terms & 7, method=m)

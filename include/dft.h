@@ -89,6 +89,11 @@ int dft_plan_get_kg(const dft_plan *p, int32_t ik, int32_t *kg, int32_t *igfft, 
  * (test / inspection aid; the table of the largest cell is 19.4 GB).                             */
 int dft_plan_get_projectors(const dft_plan *p, int32_t ik, double *ptab);
 
+/* The same table copied to DEVICE memory ptab_dev [nproj][mpw] complex (rows padded with zeros beyond npw_k),
+ * enqueued on `stream`: lets a caller run its own contraction on the identical projectors (bench.py's
+ * vendor-library context figure).                                                                  */
+int dft_plan_copy_projectors_device(const dft_plan *p, int32_t ik, double *ptab_dev, void *stream);
+
 /* Replace D_ij (PAW: "from self-consistent terms", PAPER.md :473).  HOST [natom][nlmn_max]^2.    */
 int dft_set_dij(dft_plan *p, const double *dij);
 

@@ -31,7 +31,7 @@ DFT_ERR_UNSUPPORTED = -7
 PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather", "gemm1", "dij", "gemm2_kinetic")
 
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
-SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_set_dij",
+SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_get_cprj", "dft_chebyshev_filter",
            "dft_set_vector_potential", "dft_accumulate_density", "dft_accumulate_tau",
            "dft_set_vtau",
@@ -76,6 +76,7 @@ def lib():
     L.dft_plan_get_kg.argtypes = [C.c_void_p, C.c_int32, _ip, _ip, _dp]
     L.dft_plan_get_projectors.argtypes = [C.c_void_p, C.c_int32, _dp]
     L.dft_set_dij.argtypes = [C.c_void_p, _dp]
+    L.dft_plan_copy_projectors_device.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.dft_set_vloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.dft_set_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
     L.dft_plan_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
@@ -168,6 +169,10 @@ def dft_plan_get_projectors(plan, ik, nproj, npw):
     out = np.zeros((nproj, npw), np.complex128)
     _check(lib().dft_plan_get_projectors(plan, ik, _d(out.view(np.float64))))
     return out
+
+
+def dft_plan_copy_projectors_device(plan, ik, ptab_dev_ptr, stream=0):
+    _check(lib().dft_plan_copy_projectors_device(plan, ik, ptab_dev_ptr, stream))
 
 
 def dft_set_dij(plan, dij):
@@ -263,6 +268,13 @@ class Plan:
 
     def get_projectors(self, ik=0):
         return dft_plan_get_projectors(self.h, ik, self.nproj, int(self.npw[ik]))
+
+    def projectors_device(self, ik=0):
+        """The materialised table of k-point ik as a torch complex128 CUDA tensor [nproj][mpw] (a copy)."""
+        import torch
+        out = torch.empty((self.nproj, self.mpw), dtype=torch.complex128, device="cuda")
+        dft_plan_copy_projectors_device(self.h, ik, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        return out
 
     def set_dij(self, dij):
         dft_set_dij(self.h, dij)

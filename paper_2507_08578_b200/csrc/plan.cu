@@ -401,6 +401,16 @@ int dft_plan_get_projectors(const dft_plan *p, int32_t ik, double *ptab) {
   return DFT_OK;
 }
 
+int dft_plan_copy_projectors_device(const dft_plan *p, int32_t ik, double *ptab_dev, void *stream) {
+  if (!p || !ptab_dev) { set_error("null argument"); return DFT_ERR_INVALID_ARG; }
+  if (ik < 0 || ik >= p->nkpt) { set_error("ik = %d outside 0..%d", ik, p->nkpt - 1); return DFT_ERR_INVALID_ARG; }
+  if (p->nproj == 0 || p->mpw == 0) return DFT_OK;
+  if (!p->d_ptab) { set_error("the projector table is not materialised while proj_mode = 1"); return DFT_ERR_NOT_READY; }
+  const double *src = p->d_ptab + (size_t)ik * p->nproj * p->mpw * 2;
+  DFT_CUDA_CHECK(cudaMemcpyAsync(ptab_dev, src, (size_t)p->nproj * p->mpw * 16, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return DFT_OK;
+}
+
 int dft_set_dij(dft_plan *p, const double *dij) {
   if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
   size_t n = (size_t)p->natom * p->lmax * p->lmax;

@@ -107,6 +107,8 @@ def test_projector_table_matches_oracle():
             ref = oracle.projector_table(cfg, ik, sph[ik][0])
             got = plan.get_projectors(ik)
             assert np.max(np.abs(got - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
+            dev = plan.projectors_device(ik).cpu().numpy()            # device-to-device copy of the same table
+            assert np.array_equal(dev[:, :got.shape[1]], got) and np.all(dev[:, got.shape[1]:] == 0)
         plan.destroy()
 
 

@@ -61,9 +61,10 @@ struct Fft2Batch {
   int64_t ks_psi, ks_t1, ks_t2;   // complex elements between consecutive k-points
 };
 
-// ---- pass A: sphere -> x-lines (type I).  block = lpc lines x NS slots, slot fastest; grid = nb * ntile
+// ---- pass A: sphere -> x-lines (type I).  block = lpc lines x NS slots, slot fastest; grid = nb * ntile.
+//      Three CTAs per SM (80 registers): the gather from psi is latency-bound, a third CTA buys 42 -> 53 % of HBM peak.
 template <int R1, int R2, bool BATCH, bool EXTRA>
-__global__ void __launch_bounds__(F2_THREADS, 2)
+__global__ void __launch_bounds__(F2_THREADS, 3)
 fft2_a_fwd_kernel(Fft2Geom G0, Fft2Batch B, const cplx *__restrict__ psi, cplx *__restrict__ T1, int lpc, int ntile,
                   const double *__restrict__ pre) {
   const Fft2Geom G = BATCH ? B.Gs[blockIdx.y] : G0;

@@ -446,6 +446,14 @@ def _sampled_full_size(name, sample):
     lhs = torch.vdot(psi[0, a], out[0, b]); rhs = torch.vdot(out[0, a], psi[0, b])
     scale = torch.linalg.norm(psi[0, a]) * torch.linalg.norm(out[0, b])
     assert abs(lhs - rhs) <= 1e-11 * scale
+    # the other GEMM variants at full size: 4-product table kernels and factorised projectors, same sampled bands
+    for key, val in (("gemm_3m", 0), ("proj_mode", 1)):
+        plan.set_option(key, val)
+        out2 = plan.apply_h(psi)
+        torch.cuda.synchronize()
+        err = band_rel_err(out2[:, sample].cpu().numpy(), ref)
+        assert err <= TOL, "%s %s=%d sampled bands: %.3e" % (name, key, val, err)
+        del out2
     plan.destroy()
     del psi, out
     torch.cuda.empty_cache()

@@ -265,7 +265,7 @@ static int ensure_workspace(dft_plan *p, int64_t per_band, int nband, int *chunk
     return DFT_OK;
   }
   if (chunk == 0) {
-    int64_t target = (int64_t)2 << 30;   // about 2 GiB of pass-to-pass scratch
+    int64_t target = (int64_t)8 << 30;   // about 8 GiB of pass-to-pass scratch (c4: 139 bands per chunk; fewer, longer launches)
     int64_t fit = per_band > 0 ? target / per_band : nband;
     chunk = (int)(fit < 1 ? 1 : (fit > 4096 ? 4096 : fit));
   }

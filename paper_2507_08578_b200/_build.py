@@ -7,7 +7,10 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdftb200.so")
-SOURCES = ["plan.cu", "sphere.cu", "projtab.cu", "fft.cu", "fft2.cu", "nonlocal.cu"]
+# (source, object, extra flags): fft2.cu is compiled in three parts, each instantiating a third of the radix pairs
+SOURCES = [("plan.cu", "plan.o", []), ("sphere.cu", "sphere.o", []), ("projtab.cu", "projtab.o", []), ("fft.cu", "fft.o", []),
+           ("fft2.cu", "fft2_p0.o", ["-DFFT2_PART=0"]), ("fft2.cu", "fft2_p1.o", ["-DFFT2_PART=1"]),
+           ("fft2.cu", "fft2_p2.o", ["-DFFT2_PART=2"]), ("nonlocal.cu", "nonlocal.o", [])]
 HEADERS = [os.path.join(CSRC, "internal.h"), os.path.join(CSRC, "fft_codelets.cuh"), os.path.join(CSRC, "ptx.cuh"), os.path.join(HERE, "..", "include", "dft.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -24,12 +27,12 @@ def _stale(target, deps):
 def build(force=False, verbose=False):
     """Compile every CUDA source and link the shared library; returns its path."""
     objs, jobs = [], []
-    for s in SOURCES:
+    for s, o, extra in SOURCES:
         src = os.path.join(CSRC, s)
-        obj = os.path.join(CSRC, s[:-3] + ".o")
+        obj = os.path.join(CSRC, o)
         objs.append(obj)
         if force or _stale(obj, [src] + HEADERS):
-            jobs.append([NVCC] + FLAGS + ["-c", src, "-o", obj])
+            jobs.append([NVCC] + FLAGS + extra + ["-c", src, "-o", obj])
 
     def run(cmd):
         r = subprocess.run(cmd, capture_output=True, text=True)

@@ -649,21 +649,50 @@ fft2_density_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, const
 // host side: pair table, launch geometry
 // ------------------------------------------------------------------------------------------
 // (R1, R2) with R1 <= R2, both radices available as register codelets
-#define FFT2_PAIRS(X) \
-  X(3, 3) X(4, 4) X(4, 5) X(4, 6) X(5, 5) X(5, 6) X(4, 8) X(6, 6) X(5, 8) X(6, 8) X(5, 10) X(6, 10) X(8, 8) X(8, 9) \
-  X(8, 10) X(9, 9) X(9, 10) X(8, 12) X(10, 10) X(9, 12) X(10, 12) X(8, 16) X(12, 12) X(10, 15) X(10, 16) X(12, 15) \
-  X(12, 16) X(15, 15) X(15, 16) X(16, 16)
+// The file is compiled three times (-DFFT2_PART=0,1,2, see _build.py): each translation unit instantiates the kernels of
+// a third of the pairs and exports the three dispatch functions below under a part-specific name; part 0 also holds the
+// entry points, which try the parts in turn.
+#ifndef FFT2_PART
+#define FFT2_PART 0
+#endif
+#define FFT2_PAIRS_0(X) X(3, 3) X(4, 4) X(4, 5) X(4, 6) X(5, 5) X(5, 6) X(4, 8) X(6, 6) X(5, 8) X(12, 15)
+#define FFT2_PAIRS_1(X) X(6, 8) X(5, 10) X(6, 10) X(8, 8) X(8, 9) X(8, 10) X(9, 9) X(9, 10) X(8, 12) X(8, 16)
+#define FFT2_PAIRS_2(X) X(10, 10) X(9, 12) X(10, 12) X(12, 12) X(10, 15) X(10, 16) X(12, 16) X(15, 15) X(15, 16) X(16, 16)
+#define FFT2_PAIRS_ALL(X) FFT2_PAIRS_0(X) FFT2_PAIRS_1(X) FFT2_PAIRS_2(X)
+#if FFT2_PART == 0
+#define FFT2_PAIRS(X) FFT2_PAIRS_0(X)
+#define FFT2_PARTFN(name) name##_p0
+#elif FFT2_PART == 1
+#define FFT2_PAIRS(X) FFT2_PAIRS_1(X)
+#define FFT2_PARTFN(name) name##_p1
+#else
+#define FFT2_PAIRS(X) FFT2_PAIRS_2(X)
+#define FFT2_PARTFN(name) name##_p2
+#endif
+constexpr int FFT2_NOT_MINE = 0x7f000001;   // "this pair is instantiated in another part"
+struct Fft2PassArgs {      // arguments of one pass launch, the same for every part
+  dft_plan *p; const Fft2Geom *G; const Fft2Batch *B; int nk, pass;
+  const cplx *psi; cplx *hpsi, *T1, *T2; const double *vpot; int nb, hb, max_ncol, max_nplane; cudaStream_t st;
+  const FftExtra *X; const double *wgt; double *rho;
+};
+#define FFT2_DECL(part) \
+  int fft2_pass_##part(const Fft2PassArgs &a, int r1, int r2); \
+  int fft2_batched_pass_##part(const Fft2PassArgs &a, int r1, int r2); \
+  int fft2_density_pass_##part(const Fft2PassArgs &a, int r1, int r2);
+FFT2_DECL(p0) FFT2_DECL(p1) FFT2_DECL(p2)
 
+#if FFT2_PART == 0
 bool fft2_pair(int n, int *r1, int *r2) {
   int best1 = 0, best2 = 0;
 #define X(a, b) if ((a) * (b) == n && (best2 == 0 || (b) < best2)) { best1 = (a); best2 = (b); }
-  FFT2_PAIRS(X)
+  FFT2_PAIRS_ALL(X)
 #undef X
   if (!best2) return false;
   if (r1) *r1 = best1;
   if (r2) *r2 = best2;
   return true;
 }
+#endif
 
 static int choose_xt2(int n1, int ns) {
   int cap = F2_THREADS / ns;
@@ -879,6 +908,23 @@ static int launch_pass_batched(const Fft2Geom &G, const Fft2Batch &B, int nk, in
   return DFT_OK;
 }
 
+// ---- the three dispatch functions of this part
+int FFT2_PARTFN(fft2_batched_pass)(const Fft2PassArgs &a, int r1, int r2) {
+#define X(q, r) if (r1 == (q) && r2 == (r)) return launch_pass_batched<q, r>(*a.G, *a.B, a.nk, a.pass, a.psi, a.hpsi, a.T1, a.T2, a.vpot, a.nb, a.max_ncol, a.max_nplane, a.st);
+  FFT2_PAIRS(X)
+#undef X
+  return FFT2_NOT_MINE;
+}
+
+#if FFT2_PART == 0
+static int try_parts(int (*f0)(const Fft2PassArgs &, int, int), int (*f1)(const Fft2PassArgs &, int, int),
+                     int (*f2)(const Fft2PassArgs &, int, int), const Fft2PassArgs &a, int r1, int r2) {
+  int rc = f0(a, r1, r2);
+  if (rc == FFT2_NOT_MINE) rc = f1(a, r1, r2);
+  if (rc == FFT2_NOT_MINE) rc = f2(a, r1, r2);
+  return rc == FFT2_NOT_MINE ? DFT_ERR_UNSUPPORTED : rc;
+}
+
 bool fft2_batch_ok(const dft_plan *p) {
   if (p->nkpt < 2 || p->nkpt > 65535 || p->fft_path == 1) return false;
   for (int c = 0; c < 3; c++)
@@ -922,14 +968,14 @@ int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int
     int r1, r2, rc = DFT_ERR_UNSUPPORTED;
     fft2_pair(p->n[axis_of[pass]], &r1, &r2);
     phase_begin(p, pass, st);
-#define X(a, b) if (r1 == (a) && r2 == (b)) rc = launch_pass_batched<a, b>(G, B, nk, pass, cpsi, chpsi, T1, T2, p->d_vloc, nb, max_ncol, max_nplane, st);
-    FFT2_PAIRS(X)
-#undef X
+    Fft2PassArgs a = {p, &G, &B, nk, pass, cpsi, chpsi, T1, T2, p->d_vloc, nb, 0, max_ncol, max_nplane, st, nullptr, nullptr, nullptr};
+    rc = try_parts(fft2_batched_pass_p0, fft2_batched_pass_p1, fft2_batched_pass_p2, a, r1, r2);
     phase_end(p, pass, st, 1);
     if (rc) { if (rc == DFT_ERR_UNSUPPORTED) set_error("batched FFT pass %d cannot be launched", pass); return rc; }
   }
   return DFT_OK;
 }
+#endif   // FFT2_PART == 0
 
 template <int R1, int R2>
 static int launch_density(dft_plan *p, const Fft2Geom &G, cplx *T2, const double *wgt, double *rho, int nb, cudaStream_t st) {
@@ -970,6 +1016,21 @@ static int launch_density(dft_plan *p, const Fft2Geom &G, cplx *T2, const double
   return DFT_OK;
 }
 
+int FFT2_PARTFN(fft2_density_pass)(const Fft2PassArgs &a, int r1, int r2) {
+#define X(q, r) if (r1 == (q) && r2 == (r)) return launch_density<q, r>(a.p, *a.G, a.T2, a.wgt, a.rho, a.nb, a.st);
+  FFT2_PAIRS(X)
+#undef X
+  return FFT2_NOT_MINE;
+}
+
+int FFT2_PARTFN(fft2_pass)(const Fft2PassArgs &a, int r1, int r2) {
+#define X(q, r) if (r1 == (q) && r2 == (r)) return launch_pass<q, r>(a.p, *a.G, a.pass, a.psi, a.hpsi, a.T1, a.T2, a.vpot, a.nb, a.hb, a.st, *a.X);
+  FFT2_PAIRS(X)
+#undef X
+  return FFT2_NOT_MINE;
+}
+
+#if FFT2_PART == 0
 // rho(r) += sum_b wgt[b] |psi_b(r)|^2 for nb bands of k-point ik: passes A and B as in H psi, then the density kernel.
 // Only the register path has it: DFT_ERR_UNSUPPORTED for box lengths without a two-radix factorisation.
 int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st,
@@ -998,9 +1059,10 @@ int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, 
   fft2_pair(p->n[2], &r1, &r2);
   rc = DFT_ERR_UNSUPPORTED;
   phase_begin(p, 2, st);
-#define X(a, b) if (r1 == (a) && r2 == (b)) rc = launch_density<a, b>(p, G, T2, wgt_dev, rho, nb, st);
-  FFT2_PAIRS(X)
-#undef X
+  {
+    Fft2PassArgs a = {p, &G, nullptr, 1, 2, nullptr, nullptr, T1, T2, nullptr, nb, 0, 0, 0, st, nullptr, wgt_dev, rho};
+    rc = try_parts(fft2_density_pass_p0, fft2_density_pass_p1, fft2_density_pass_p2, a, r1, r2);
+  }
   phase_end(p, 2, st, 1);
   if (rc == DFT_ERR_UNSUPPORTED) set_error("density kernel: tile does not fit (nplane = %d)", kp.nplane);
   return rc;
@@ -1019,10 +1081,9 @@ int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, 
   const cplx *cpsi = reinterpret_cast<const cplx *>(psi);
   cplx *chpsi = reinterpret_cast<cplx *>(hpsi), *t1 = reinterpret_cast<cplx *>(T1), *t2 = reinterpret_cast<cplx *>(T2);
   const int hb = p->kp[ik].max_cols_per_plane;
-#define X(a, b) if (r1 == (a) && r2 == (b)) return launch_pass<a, b>(p, G, pass, cpsi, chpsi, t1, t2, vpot, nb, hb, st, X);
-  FFT2_PAIRS(X)
-#undef X
-  return DFT_ERR_UNSUPPORTED;
+  Fft2PassArgs a = {p, &G, nullptr, 1, pass, cpsi, chpsi, t1, t2, vpot, nb, hb, 0, 0, st, &X, nullptr, nullptr};
+  return try_parts(fft2_pass_p0, fft2_pass_p1, fft2_pass_p2, a, r1, r2);
 }
+#endif   // FFT2_PART == 0
 
 }  // namespace dftb200

@@ -110,8 +110,8 @@ int dft_set_workspace(dft_plan *p, void *dev_ptr, int64_t bytes);
 /* Options: "band_chunk" (bands per FFT pass launch, > 0), "terms" (bit 0 kinetic, bit 1 local,
  * bit 2 non-local, bit 3 meta-GGA term; default 15), "splitk" (GEMM-1 K splits, 0 = automatic), "proj_mode" (0 = default: projector table materialised in
  * device memory; 1 = factorised projectors FY.S evaluated inside both GEMMs; the table is freed (and rebuilt when the option
- * returns to 0; dft_plan_get_projectors gives DFT_ERR_NOT_READY meanwhile); needs nlmn <= 8 per type and at most 2
- * types, else DFT_ERR_UNSUPPORTED), "host_groups" (dft_apply_h_host only: band groups, default 5,
+ * returns to 0; dft_plan_get_projectors gives DFT_ERR_NOT_READY meanwhile); an atom's projectors are taken in blocks of 8 and the form-factor rows of all types (8
+ * per block) must not exceed 32, else DFT_ERR_UNSUPPORTED), "host_groups" (dft_apply_h_host only: band groups, default 5,
  * whose host<->device copies overlap the kernels of the neighbouring groups), "gemm_3m" (1 = default: three real
  * products per complex multiply-add in the projector GEMMs, 0 = four; same result up to rounding), "fft_path" (0 = automatic:
  * register-resident two-stage transforms where the box length factorises, their strided passes fed by a

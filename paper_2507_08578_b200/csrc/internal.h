@@ -103,6 +103,8 @@ struct dft_plan {
   double *d_ones = nullptr;                          // [mpw] of 1.0: the unit diagonal of S in GEMM-2's epilogue
   const double **d_oneptr = nullptr;                 // [nkpt] device pointers to d_ones
   double *d_stab = nullptr, *d_fytab = nullptr;      // factorised projectors: structure factors / form factors (proj_mode = 1)
+  int32_t *d_blk_atom = nullptr, *d_blk_frow = nullptr, *d_blk_first = nullptr, *d_blk_nl = nullptr;   // projector blocks (<= 8 rows)
+  int nblk = 0, nfrow = 0;                           // number of blocks; FY rows of all types
   int ldf = 0;                                       // row length of d_fytab (mpw rounded up to 8)
   int proj_mode = 0;                                 // 0 = materialised table (GEMMs on P), 1 = factorised P = FY . S
   double *d_ptab = nullptr;                          // [nkpt][nproj][mpw] complex, zero padded beyond npw_k
@@ -155,6 +157,7 @@ int sphere_build(const double *gmet, const int n[3], double ecut, KPoint *kp);
 
 // --- projtab.cu (S1) ----------------------------------------------------------------------
 int build_projector_table(dft_plan *p, int ik, double *maxq_out);
+constexpr int FAC_MAX_FROWS = 32;        // FY rows (8 per projector block, summed over atom types) the kernels keep in shared memory
 int build_factor_tables(dft_plan *p);   // S [nkpt][natom][mpw] complex and FY [nkpt][ntypat*8][ldf] real (factorised projectors)
 
 // Optional variations of the local application (meta-GGA term): another potential in pass C, a real diagonal factor

@@ -533,7 +533,7 @@ gemm2_3m_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant_
 constexpr int FC_BA = 16;                  // atoms per CTA tile
 constexpr int FC_OFF_S = NL_BN * 128;      // stage layout: psi tile 8 KB | S tile 2 KB | FY tile <= 1 KB
 constexpr int FC_OFF_F = FC_OFF_S + FC_BA * 128;
-constexpr int FC_STAGE_BYTES = 11 * 1024;
+constexpr int FC_STAGE_BYTES = 12 * 1024;      // FY tile: FAC_MAX_FROWS rows x 8 doubles = 2 KB
 constexpr int FC_STAGES = 8;
 constexpr int FC_PREFETCH = FC_STAGES - 2;
 constexpr int FC_SMEM = FC_STAGES * FC_STAGE_BYTES + 1024 + 256;
@@ -541,8 +541,8 @@ constexpr int FC_WARPS = 16;               // 4 (atom groups) x 4 (band groups):
 constexpr int FC_THREADS = FC_WARPS * 32;  // DMUL -> DFMA -> DMMA chains of the z = conj(S) psi products
 
 struct Fac1Params {
-  int natom, nband, nproj, nslab, nsplit, slabs_per_split, tiles_n, ntypat;
-  const int32_t *typat, *nlmn, *atom_first;
+  int nblk, nfrow, nband, nproj, nslab, nsplit, slabs_per_split, tiles_n;
+  const int32_t *blk_atom, *blk_frow, *blk_first, *blk_nl;   // projector blocks of <= 8 rows (projtab.cu)
   double2 *part;   // [nkpt][nsplit][nproj][nband]
 };
 
@@ -561,14 +561,15 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
   const int tn = blockIdx.x % Q.tiles_n, ta = blockIdx.x / Q.tiles_n, split = blockIdx.y, ik = blockIdx.z;
   const int s0 = split * Q.slabs_per_split;
   int ns = Q.nslab - s0; if (ns > Q.slabs_per_split) ns = Q.slabs_per_split; if (ns < 0) ns = 0;
-  const uint32_t tx = NL_BN * 128 + FC_BA * 128 + 64 * 8 * Q.ntypat;
+  const uint32_t tx = NL_BN * 128 + FC_BA * 128 + 64 * Q.nfrow;
+  const int atom0 = __ldg(Q.blk_atom + ta * FC_BA);      // S rows of the tile: 16 atoms from the first block's atom
   auto issue = [&](int j) {
     int s = j % FC_STAGES;
     if (j >= FC_STAGES) mbar_wait(&empty[s], ((j / FC_STAGES) - 1) & 1);
     unsigned char *st = tiles + s * FC_STAGE_BYTES;
     mbar_expect_tx(&full[s], tx);
     tma_load_3d(st, &mapPsi, &full[s], (s0 + j) * 16, tn * NL_BN, ik);
-    tma_load_3d(st + FC_OFF_S, &mapS, &full[s], (s0 + j) * 16, ta * FC_BA, ik);
+    tma_load_3d(st + FC_OFF_S, &mapS, &full[s], (s0 + j) * 16, atom0, ik);
     tma_load_3d(st + FC_OFF_F, &mapF, &full[s], (s0 + j) * 8, 0, ik);
   };
   const bool producer = (threadIdx.x == 0);
@@ -576,11 +577,12 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
     for (int j = 0; j < FC_PREFETCH && j < ns; j++) issue(j);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wm = warp >> 2, wn = warp & 3;   // 4 atoms x 16 bands per warp
   const int i = lane >> 2, j = lane & 3;
-  int frow[4];   // byte offset of this lane's FY row (its atom's type, projector i) inside the FY tile
+  int frow[4], arow[4];   // this lane's FY row (byte offset in the FY tile) and its block's S row, per block of the warp
 #pragma unroll
   for (int q = 0; q < 4; q++) {
-    int atom = ta * FC_BA + wm * 4 + q;
-    frow[q] = ((atom < Q.natom ? Q.typat[atom] : 0) * 8 + i) * 64;
+    const int blk = ta * FC_BA + wm * 4 + q, ok = blk < Q.nblk;
+    frow[q] = ((ok ? Q.blk_frow[blk] : 0) + i) * 64;
+    arow[q] = ok ? Q.blk_atom[blk] - atom0 : 0;
   }
   double cre[4][2][2], cim[4][2][2];
 #pragma unroll
@@ -605,8 +607,7 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
       }
 #pragma unroll
       for (int q = 0; q < 4; q++) {
-        const int arow = wm * 4 + q;
-        const double2 sg = *reinterpret_cast<const double2 *>(Ss + arow * 128 + ((e ^ (arow & 7)) << 4));
+        const double2 sg = *reinterpret_cast<const double2 *>(Ss + arow[q] * 128 + ((e ^ (arow[q] & 7)) << 4));
         const double fa = *reinterpret_cast<const double *>(Fs + frow[q] + e * 8);
 #pragma unroll
         for (int nb = 0; nb < 2; nb++) {
@@ -619,14 +620,14 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[s]);
   }
-  // partial[ik][split][first_a + i][b]; thread holds projector i of its 4 atoms, bands 2j, 2j+1 of each 8-band block
+  // partial[ik][split][first_blk + i][b]; thread holds projector i of its 4 blocks, bands 2j, 2j+1 of each 8-band block
   double2 *out = Q.part + ((size_t)(ik * Q.nsplit + split) * Q.nproj) * Q.nband;
 #pragma unroll
   for (int q = 0; q < 4; q++) {
-    int atom = ta * FC_BA + wm * 4 + q;
-    if (atom >= Q.natom) continue;
-    if (i >= Q.nlmn[Q.typat[atom]]) continue;
-    double2 *row = out + (size_t)(Q.atom_first[atom] + i) * Q.nband;
+    const int blk = ta * FC_BA + wm * 4 + q;
+    if (blk >= Q.nblk) continue;
+    if (i >= Q.blk_nl[blk]) continue;
+    double2 *row = out + (size_t)(Q.blk_first[blk] + i) * Q.nband;
 #pragma unroll
     for (int nb = 0; nb < 2; nb++) {
       int b = tn * NL_BN + wn * 16 + nb * 8 + 2 * j;
@@ -638,21 +639,21 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
 
 //   GEMM-2:  w_{a,b}(G) = sum_i FY[i,G] c'[a,i,b]               (4 DMMA per 8 x 8 block: 2 k-groups of projectors x re/im)
 //            hpsi_b(G) += S_a(G) w_{a,b}(G)                     (8 FP64 instructions per thread and block)
-// One K-slab = one atom: its c' tile [64 bands][8 projectors] (TMA, swizzled) and its phases for the tile's 128 G.
+// One K-slab = one projector block (an atom's <= 8 rows): its c' tile [64 bands][8 projectors] (TMA, swizzled) and its phases for the tile's 128 G.
 // The FY rows of the tile's 128 G (8 per atom type, row stride 132 doubles against bank conflicts) are loaded once.
 constexpr int FD_OFF_S = NL_BN * 128;                 // stage: c' tile 8 KB | S_a(G) 2 KB
 constexpr int FD_STAGE_BYTES = 10 * 1024;
 constexpr int FD_STAGES = 8;
 constexpr int FD_PREFETCH = FD_STAGES - 2;
 constexpr int FD_FLD = NL_BM + 4;                     // FY row stride in shared memory (doubles)
-constexpr int FD_FBYTES = 2 * 8 * FD_FLD * 8;         // up to two atom types
+constexpr int FD_FBYTES = FAC_MAX_FROWS * FD_FLD * 8;  // FY rows of every type for the tile's 128 G
 constexpr int FD_SMEM = FD_STAGES * FD_STAGE_BYTES + FD_FBYTES + 1024 + 256;
 
 // grid: (tiles_n * tiles_m, 1, nkpt); Q as in gemm2_kernel, nslab = natom
 __global__ void __launch_bounds__(FC_THREADS, 1)
 gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant__ CUtensorMap mapS,
-                 const __grid_constant__ CUtensorMap mapF, Gemm2Params Q, const int32_t *__restrict__ typat,
-                 const int32_t *__restrict__ atom_first, int ntypat) {
+                 const __grid_constant__ CUtensorMap mapF, Gemm2Params Q, const int32_t *__restrict__ blk_atom,
+                 const int32_t *__restrict__ blk_frow, const int32_t *__restrict__ blk_first, int nfrow) {
   extern __shared__ unsigned char smem_raw[];
   unsigned char *tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   unsigned char *Fs = tiles + FD_STAGES * FD_STAGE_BYTES;
@@ -672,12 +673,12 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
     if (a >= FD_STAGES) mbar_wait(&empty[s], ((a / FD_STAGES) - 1) & 1);
     unsigned char *st = tiles + s * FD_STAGE_BYTES;
     mbar_expect_tx(&full[s], NL_BN * 128 + NL_BM * 16);
-    tma_load_3d(st, &mapC, &full[s], 2 * __ldg(atom_first + a), tn * NL_BN, ik);
-    tma_load_3d(st + FD_OFF_S, &mapS, &full[s], tm * NL_BM * 2, a, ik);
+    tma_load_3d(st, &mapC, &full[s], 2 * __ldg(blk_first + a), tn * NL_BN, ik);
+    tma_load_3d(st + FD_OFF_S, &mapS, &full[s], tm * NL_BM * 2, __ldg(blk_atom + a), ik);
   };
   const bool producer = (threadIdx.x == 0);
   if (producer && ns > 0) {
-    mbar_expect_tx(fbar, (uint32_t)(ntypat * 8 * FD_FLD * 8));
+    mbar_expect_tx(fbar, (uint32_t)(nfrow * FD_FLD * 8));
     tma_load_3d(Fs, &mapF, fbar, tm * NL_BM, 0, ik);
     for (int a = 0; a < FD_PREFETCH && a < ns; a++) issue(a);
   }
@@ -691,7 +692,7 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
     if (producer && a + FD_PREFETCH < ns) issue(a + FD_PREFETCH);
     __syncwarp();
     int s = a % FD_STAGES;
-    const int t = __ldg(typat + a);
+    const int fr0 = __ldg(blk_frow + a);      // first FY row of this block
     mbar_wait(&full[s], (a / FD_STAGES) & 1);
     const unsigned char *Cs = tiles + s * FD_STAGE_BYTES, *Ss = Cs + FD_OFF_S;
     double2 sg[4];
@@ -702,7 +703,7 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
       sg[mb] = *reinterpret_cast<const double2 *>(Ss + g * 16);
 #pragma unroll
       for (int kgp = 0; kgp < 2; kgp++)                                      // projector 2j + kgp of the atom's type
-        fa[mb][kgp] = *reinterpret_cast<const double *>(Fs + ((size_t)((t * 8 + 2 * j + kgp) * FD_FLD + g)) * 8);
+        fa[mb][kgp] = *reinterpret_cast<const double *>(Fs + ((size_t)((fr0 + 2 * j + kgp) * FD_FLD + g)) * 8);
     }
 #pragma unroll
     for (int nb = 0; nb < 2; nb++) {
@@ -875,7 +876,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   q1.nproj = nproj; q1.nband = nband;
   q1.nslab = (mpw + 7) / 8;
   const bool fac = p->proj_mode == 1;     // factorised projectors: tiles of 16 atoms instead of 128 table rows
-  q1.tiles_m = fac ? (p->natom + FC_BA - 1) / FC_BA : (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
+  q1.tiles_m = fac ? (p->nblk + FC_BA - 1) / FC_BA : (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
   int ns = p->splitk > 0 ? p->splitk : choose_splitk(q1.tiles_m * q1.tiles_n, q1.nslab, p->sm_count, nkpt);
   if (ns > q1.nslab) ns = q1.nslab;
   q1.slabs_per_split = (q1.nslab + ns - 1) / ns;
@@ -900,7 +901,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   CUtensorMap mapS1, mapF1, mapS2, mapF2;
   if (fac) {
     if (!p->d_stab || !p->d_fytab) { set_error("factor tables missing"); return DFT_ERR_NOT_READY; }
-    const uint64_t frow = (uint64_t)p->ldf * 8, nfr = (uint64_t)p->ntypat * 8;
+    const uint64_t frow = (uint64_t)p->ldf * 8, nfr = (uint64_t)p->nfrow;
     if ((rc = make_map(p, &mapS1, p->d_stab, 2 * (uint64_t)mpw, p->natom, nkpt, rowb, rowb * p->natom, FC_BA))) return rc;
     if ((rc = make_map_plain(p, &mapF1, p->d_fytab, p->ldf, nfr, nkpt, frow, frow * nfr, 8, (uint32_t)nfr))) return rc;
     if ((rc = make_map_plain(p, &mapS2, p->d_stab, 2 * (uint64_t)mpw, p->natom, nkpt, rowb, rowb * p->natom, 2 * NL_BM, 1))) return rc;
@@ -925,9 +926,9 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   phase_begin(p, 5, st);
   if (fac) {
     Fac1Params f1;
-    f1.natom = p->natom; f1.nband = nband; f1.nproj = nproj; f1.nslab = q1.nslab; f1.nsplit = q1.nsplit;
-    f1.slabs_per_split = q1.slabs_per_split; f1.tiles_n = q1.tiles_n; f1.ntypat = p->ntypat;
-    f1.typat = p->d_typat; f1.nlmn = p->d_nlmn; f1.atom_first = p->d_atom_first; f1.part = q1.part;
+    f1.nblk = p->nblk; f1.nfrow = p->nfrow; f1.nband = nband; f1.nproj = nproj; f1.nslab = q1.nslab; f1.nsplit = q1.nsplit;
+    f1.slabs_per_split = q1.slabs_per_split; f1.tiles_n = q1.tiles_n;
+    f1.blk_atom = p->d_blk_atom; f1.blk_frow = p->d_blk_frow; f1.blk_first = p->d_blk_first; f1.blk_nl = p->d_blk_nl; f1.part = q1.part;
     gemm1_fac_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), FC_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1, f1);
   } else if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   else gemm1_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
@@ -951,9 +952,9 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
   phase_begin(p, 7, st);
   if (fac) {
-    q2.nslab = p->natom;
-    gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_typat,
-                                                                                      p->d_atom_first, p->ntypat);
+    q2.nslab = p->nblk;
+    gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_blk_atom,
+                                                                                      p->d_blk_frow, p->d_blk_first, p->nfrow);
   } else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   else gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   phase_end(p, 7, st, 1);

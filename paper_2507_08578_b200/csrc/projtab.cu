@@ -9,6 +9,8 @@
 // i.e. K-contiguous for GEMM-1 and M-contiguous for GEMM-2 (nonlocal.cu).
 #include <math.h>
 
+#include <vector>
+
 #include "internal.h"
 
 namespace dftb200 {
@@ -140,7 +142,7 @@ int build_projector_table(dft_plan *p, int ik, double *maxq_out) {
 // Factorised projectors (PAPER.md :477 "computed on-the-fly"): p_{a,i}(m) = FY_{t(a),i}(m) . S_a(m)
 // with FY = F.Y real (one row per projector of an atom TYPE) and S_a(m) = exp(-2 pi i (k+m).x_a) (one row per ATOM).
 // The two small tables replace the [nproj][mpw] complex one: S [natom][mpw] complex, FY [ntypat*8][ldf] real
-// (8 rows per type, rows >= nlmn zero; needs nlmn <= 8), zero for ipw >= npw_k.
+// (whole 8-row blocks per type, rows >= nlmn zero), zero for ipw >= npw_k.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(PT_THREADS) stab_kernel(ProjParams P, double2 *__restrict__ stab) {
   int g = blockIdx.x * PT_THREADS + threadIdx.x, a = blockIdx.y;
@@ -158,13 +160,15 @@ __global__ void __launch_bounds__(PT_THREADS) stab_kernel(ProjParams P, double2 
   stab[(size_t)a * P.mpw + g] = v;
 }
 
-__global__ void __launch_bounds__(PT_THREADS) fytab_kernel(ProjParams P, double *__restrict__ fy, int ldf) {
+__global__ void __launch_bounds__(PT_THREADS) fytab_kernel(ProjParams P, double *__restrict__ fy, int ldf,
+                                                           const int32_t *__restrict__ type_row0, const int32_t *__restrict__ type_rows) {
   int g = blockIdx.x * PT_THREADS + threadIdx.x, t = blockIdx.y;
   if (g >= ldf) return;
   int nl = P.nlmn[t];
-  double *dst = fy + (size_t)t * 8 * ldf + g;
+  const int nrows = type_rows[t];                 // 8 * ceil(nlmn / 8): whole 8-row blocks, rows >= nlmn are zero
+  double *dst = fy + (size_t)type_row0[t] * ldf + g;
   if (g >= P.npw) {
-    for (int i = 0; i < 8; i++) dst[(size_t)i * ldf] = 0.0;
+    for (int i = 0; i < nrows; i++) dst[(size_t)i * ldf] = 0.0;
     return;
   }
   const double TWO_PI = 6.283185307179586;
@@ -173,7 +177,7 @@ __global__ void __launch_bounds__(PT_THREADS) fytab_kernel(ProjParams P, double 
   double qy = TWO_PI * (t0 * P.bm[1] + t1 * P.bm[4] + t2 * P.bm[7]);
   double qz = TWO_PI * (t0 * P.bm[2] + t1 * P.bm[5] + t2 * P.bm[8]);
   double qn = sqrt(qx * qx + qy * qy + qz * qz);
-  for (int i = 0; i < 8; i++) {
+  for (int i = 0; i < nrows; i++) {
     double v = 0.0;
     if (i < nl) {
       int ir = P.lmn_irad[t * P.lmax + i];
@@ -185,14 +189,43 @@ __global__ void __launch_bounds__(PT_THREADS) fytab_kernel(ProjParams P, double 
   }
 }
 
-// Builds (or rebuilds) both tables for every k-point.  DFT_ERR_UNSUPPORTED if some type has more than 8 projectors.
+// Builds (or rebuilds) both tables for every k-point, and the list of projector BLOCKS the factorised GEMMs walk: an atom
+// with nlmn projectors contributes ceil(nlmn / 8) blocks of up to 8 rows (M = 8 of the DMMA shape).  DFT_ERR_UNSUPPORTED
+// if the FY rows of all types (8 per block) exceed FAC_MAX_FROWS.
+template <typename T>
+static int upload_vec(T **dst, const std::vector<T> &v) {
+  cudaFree(*dst); *dst = nullptr;
+  if (v.empty()) return DFT_OK;
+  DFT_CUDA_CHECK(cudaMalloc(dst, v.size() * sizeof(T)));
+  DFT_CUDA_CHECK(cudaMemcpy(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return DFT_OK;
+}
+
 int build_factor_tables(dft_plan *p) {
   if (p->natom == 0 || p->nproj == 0 || p->mpw == 0) return DFT_OK;
-  for (int t = 0; t < p->ntypat; t++)
-    if (p->nlmn[t] > 8) { set_error("factorised projectors need nlmn <= 8 per atom type (type %d has %d)", t, p->nlmn[t]); return DFT_ERR_UNSUPPORTED; }
-  if (p->ntypat > 2) { set_error("factorised projectors support at most 2 atom types (got %d)", p->ntypat); return DFT_ERR_UNSUPPORTED; }
+  std::vector<int32_t> row0(p->ntypat), rows(p->ntypat);
+  int nfrow = 0;
+  for (int t = 0; t < p->ntypat; t++) { row0[t] = nfrow; rows[t] = (p->nlmn[t] + 7) / 8 * 8; nfrow += rows[t]; }
+  if (nfrow > FAC_MAX_FROWS) {
+    set_error("factorised projectors: %d form-factor rows (8 per block of projectors, all types) exceed %d", nfrow, FAC_MAX_FROWS);
+    return DFT_ERR_UNSUPPORTED;
+  }
+  std::vector<int32_t> b_atom, b_frow, b_first, b_nl;
+  for (int a = 0; a < p->natom; a++) {
+    int t = p->typat[a], nl = p->nlmn[t];
+    for (int mb = 0; mb * 8 < nl; mb++) {
+      b_atom.push_back(a); b_frow.push_back(row0[t] + 8 * mb); b_first.push_back(p->atom_first[a] + 8 * mb);
+      b_nl.push_back(nl - 8 * mb < 8 ? nl - 8 * mb : 8);
+    }
+  }
+  p->nblk = (int)b_atom.size(); p->nfrow = nfrow;
+  int rc;
+  int32_t *d_row0 = nullptr, *d_rows = nullptr;
+  if ((rc = upload_vec(&p->d_blk_atom, b_atom)) || (rc = upload_vec(&p->d_blk_frow, b_frow)) ||
+      (rc = upload_vec(&p->d_blk_first, b_first)) || (rc = upload_vec(&p->d_blk_nl, b_nl)) ||
+      (rc = upload_vec(&d_row0, row0)) || (rc = upload_vec(&d_rows, rows))) return rc;
   p->ldf = (p->mpw + 7) / 8 * 8;
-  size_t sbytes = (size_t)p->nkpt * p->natom * p->mpw * 16 + 256, fbytes = (size_t)p->nkpt * p->ntypat * 8 * p->ldf * 8 + 256;
+  size_t sbytes = (size_t)p->nkpt * p->natom * p->mpw * 16 + 256, fbytes = (size_t)p->nkpt * nfrow * p->ldf * 8 + 256;
   if (!p->d_stab && cudaMalloc(&p->d_stab, sbytes) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the structure-factor table (%zu bytes)", sbytes); return DFT_ERR_ALLOC; }
   if (!p->d_fytab && cudaMalloc(&p->d_fytab, fbytes) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the form-factor table (%zu bytes)", fbytes); return DFT_ERR_ALLOC; }
   for (int ik = 0; ik < p->nkpt; ik++) {
@@ -207,9 +240,11 @@ int build_factor_tables(dft_plan *p) {
     stab_kernel<<<dim3((p->mpw + PT_THREADS - 1) / PT_THREADS, p->natom), PT_THREADS>>>(
         P, reinterpret_cast<double2 *>(p->d_stab) + (size_t)ik * p->natom * p->mpw);
     fytab_kernel<<<dim3((p->ldf + PT_THREADS - 1) / PT_THREADS, p->ntypat), PT_THREADS>>>(
-        P, p->d_fytab + (size_t)ik * p->ntypat * 8 * p->ldf, p->ldf);
+        P, p->d_fytab + (size_t)ik * nfrow * p->ldf, p->ldf, d_row0, d_rows);
   }
-  DFT_CUDA_CHECK(cudaDeviceSynchronize());
+  cudaError_t e = cudaDeviceSynchronize();
+  cudaFree(d_row0); cudaFree(d_rows);
+  if (e != cudaSuccess) { set_error("factor-table kernels failed: %s", cudaGetErrorString(e)); return DFT_ERR_CUDA; }
   return DFT_OK;
 }
 

@@ -270,15 +270,9 @@ def test_meta_gga_term(name):
 @pytest.mark.parametrize("name", ["c1m", "c4m", "c2m", "aniso", "aniso8", "c3k2"])
 def test_factorised_projectors(name):
     """Option proj_mode = 1 (PAPER.md :477 "computed on-the-fly"): p = FY . S evaluated inside both GEMMs instead of the
-    materialised table; H psi, S psi and cprj must match the oracle as before.  Types with more than 8 projectors are refused."""
-    import paper_2507_08578_b200 as dft
+    materialised table; H psi, S psi and cprj must match the oracle as before.  Atoms with more than 8 projectors (Al: 9)
+    are walked as two blocks of 8 rows."""
     cfg, plan, sph = _setup(name)
-    if max(t["nlmn"] for t in cfg["types"]) > 8:
-        with pytest.raises(dft.DftError) as ei:
-            plan.set_option("proj_mode", 1)
-        assert ei.value.code == dft.DFT_ERR_UNSUPPORTED
-        plan.destroy()
-        return
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     tpsi = torch.as_tensor(psi, device="cuda")
     plan.set_option("proj_mode", 1)

@@ -304,8 +304,11 @@ def main():
     traffic = None      # ncu dram bytes per launch of that kernel, from the committed capture summary (full-size runs only)
     try:
         if not args.nband and world == 1:
-            with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as f:
-                traffic = json.load(f).get(args.config, {}).get(dom)
+            with open(os.path.join(ROOT, "profiles", "r1_traffic.csv")) as f:
+                for row in f.read().splitlines()[1:]:
+                    c_, k_, b_ = row.split(",")
+                    if c_ == args.config and k_ == dom and b_:
+                        traffic = int(b_)
     except Exception:
         traffic = None
     roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],

@@ -354,6 +354,21 @@ def main():
         del work, tmp
         torch.cuda.empty_cache()
 
+    # ---- context figure: H psi and S psi from one set of projections (three GEMMs instead of four)
+    if args.cheb_degree > 0 and world == 1:
+        plan.apply_hs(psi)
+        torch.cuda.synchronize()
+        h0 = torch.cuda.Event(enable_timing=True); h1 = torch.cuda.Event(enable_timing=True)
+        h0.record(); hs = plan.apply_hs(psi); h1.record()
+        torch.cuda.synchronize()
+        s0 = torch.cuda.Event(enable_timing=True); s1 = torch.cuda.Event(enable_timing=True)
+        s0.record(); sp = plan.apply_s(psi); s1.record()
+        torch.cuda.synchronize()
+        line["apply_hs"] = {"ms": h0.elapsed_time(h1), "ms_apply_s_alone": s0.elapsed_time(s1),
+                            "api": "dft_apply_hs (H psi and S psi, one GEMM-1) / dft_apply_s"}
+        del hs, sp
+        torch.cuda.empty_cache()
+
     # ---- context figure: density accumulation n(r) = sum w |psi(r)|^2 (Eq. 6) over all bands
     if args.cheb_degree > 0 and world == 1:
         wts = np.ones((plan.nkpt, nband))

@@ -137,6 +137,12 @@ int dft_set_sij(dft_plan *p, const double *sij);
  * pad-entry rules as dft_apply_h: GEMM-1, s_ij, GEMM-2 with a unit diagonal in its epilogue.        */
 int dft_apply_s(dft_plan *p, const double *psi, double *spsi, int32_t nband, void *stream);
 
+/* hpsi = H psi and spsi = S psi in one call, from ONE set of projections <p|psi> (PAPER.md :479-:485: keeping the
+ * cprj and reusing them saves non-local operations): the five FFT passes, GEMM-1, then D_ij + GEMM-2 into hpsi and
+ * s_ij + GEMM-2 (unit diagonal) into spsi -- three GEMMs instead of the four of dft_apply_h + dft_apply_s.  Arguments
+ * and rules of dft_apply_h; spsi like hpsi; the non-local term must be on.                              */
+int dft_apply_hs(dft_plan *p, const double *psi, double *hpsi, double *spsi, int32_t nband, void *stream);
+
 /* cprj = <p_a,i|psi_n> (PAPER.md :477 "coefficients c_a,i,n,k ... cprj"): DEVICE output
  * [nkpt][nband][nproj] complex128, projector index fastest, atoms in order, i = 0..nlmn-1 inside an
  * atom.  GEMM-1 and the fixed-order split-K reduction only; enqueues on `stream`.                 */

@@ -32,7 +32,7 @@ PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather
 
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
-           "dft_set_sij", "dft_apply_s", "dft_get_cprj", "dft_chebyshev_filter",
+           "dft_set_sij", "dft_apply_s", "dft_apply_hs", "dft_get_cprj", "dft_chebyshev_filter",
            "dft_set_vector_potential", "dft_accumulate_density", "dft_accumulate_tau",
            "dft_set_vtau",
            "dft_set_vloc", "dft_set_workspace", "dft_plan_set_option", "dft_apply_h", "dft_apply_h_host",
@@ -90,6 +90,7 @@ def lib():
     L.dft_chebyshev_filter.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                        C.c_void_p]
     L.dft_apply_s.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    L.dft_apply_hs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_get_cprj.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_plan_set_timing.argtypes = [C.c_void_p, C.c_int32]
     L.dft_plan_phase_ms.argtypes = [C.c_void_p, C.c_int32, _dp, C.POINTER(C.c_int64)]
@@ -201,6 +202,10 @@ def dft_set_sij(plan, sij):
 
 def dft_apply_s(plan, psi_dev_ptr, spsi_dev_ptr, nband, stream=0):
     _check(lib().dft_apply_s(plan, psi_dev_ptr, spsi_dev_ptr, nband, stream))
+
+
+def dft_apply_hs(plan, psi_dev_ptr, hpsi_dev_ptr, spsi_dev_ptr, nband, stream=0):
+    _check(lib().dft_apply_hs(plan, psi_dev_ptr, hpsi_dev_ptr, spsi_dev_ptr, nband, stream))
 
 
 def dft_get_cprj(plan, psi_dev_ptr, cprj_dev_ptr, nband, stream=0):
@@ -322,6 +327,15 @@ class Plan:
         assert spsi.is_cuda and spsi.dtype == torch.complex128 and spsi.is_contiguous() and spsi.shape == psi.shape
         dft_apply_s(self.h, psi.data_ptr(), spsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
         return spsi
+
+    def apply_hs(self, psi):
+        """(H psi, S psi) from one set of projections; same tensors as apply_h."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.shape[-1] == self.mpw
+        nband = psi.numel() // (self.nkpt * self.mpw) if self.mpw else 0
+        hpsi = torch.empty_like(psi); spsi = torch.empty_like(psi)
+        dft_apply_hs(self.h, psi.data_ptr(), hpsi.data_ptr(), spsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
+        return hpsi, spsi
 
     def get_cprj(self, psi):
         """<p|psi> as a torch complex128 CUDA tensor [nkpt][nband][nproj]."""

@@ -199,7 +199,7 @@ int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, 
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi
 int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin,
                    bool with_nl, cudaStream_t st, const double *dmat = nullptr, const double *const *diag = nullptr,
-                   double *cprj_out = nullptr, const Recurrence *rec = nullptr);
+                   double *cprj_out = nullptr, const Recurrence *rec = nullptr, double *spsi = nullptr);
 
 // --- timing hooks ------------------------------------------------------------------------------
 void phase_begin(dft_plan *p, int phase, cudaStream_t st);

@@ -840,7 +840,8 @@ static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
 // diagonal multiplying psi in the epilogue (null = the kinetic energies); cprj_out (device, [nkpt][nband][nproj]
 // complex): if given, only GEMM-1 and the split-K reduction run and <p|psi> is written there.
 int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
-                   cudaStream_t st, const double *dmat, const double *const *diag, double *cprj_out, const Recurrence *rec) {
+                   cudaStream_t st, const double *dmat, const double *const *diag, double *cprj_out, const Recurrence *rec,
+                   double *spsi) {
   if (p->mpw == 0 || nband == 0) return DFT_OK;
   if (cprj_out && p->nproj == 0) return DFT_OK;
   if (p->nproj == 0) with_nl = false;
@@ -867,6 +868,12 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
                                           rec ? rec->sh : 1.0, rec ? rec->sy : 0.0, rec ? rec->sx : 0.0,
                                           rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr);
     phase_end(p, 7, st, 1);
+    if (spsi) {   // no projectors: S = 1
+      phase_begin(p, 7, st);
+      kin_only_kernel<<<grid, 256, 0, st>>>(cpsi, reinterpret_cast<double2 *>(spsi), p->d_oneptr, d_npw, nband, p->mpw, 0, 1, 0, 1.0, 0.0,
+                                            0.0, nullptr);
+      phase_end(p, 7, st, 1);
+    }
     DFT_CUDA_CHECK(cudaGetLastError());
     return DFT_OK;
   }
@@ -959,6 +966,23 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   else gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   phase_end(p, 7, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
+  if (spsi) {
+    // second output from the SAME projections (dft_apply_hs): S psi = psi + sum |p> s <p|psi>.  The split-K partials of
+    // GEMM-1 are still there; reduce them again with s_ij into c' and back-project with a unit diagonal.
+    phase_begin(p, 6, st);
+    dij_kernel<<<dim3((nband + 127) / 128, p->natom, nkpt), 128, 0, st>>>(q1.part, reinterpret_cast<double2 *>(p->d_cprj), p->d_sij, p->d_typat,
+                                                                          p->d_nlmn, p->d_atom_first, p->natom, p->lmax, nproj, nband, ns);
+    phase_end(p, 6, st, 1);
+    q2.accumulate = 0; q2.with_kin = 1; q2.kin = p->d_oneptr; q2.hpsi = reinterpret_cast<double2 *>(spsi);
+    q2.cheb = 0; q2.sh = 1.0; q2.sy = 0.0; q2.sx = 0.0; q2.xprev = nullptr;
+    phase_begin(p, 7, st);
+    if (fac) gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_blk_atom,
+                                                                                               p->d_blk_frow, p->d_blk_first, p->nfrow);
+    else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+    else gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+    phase_end(p, 7, st, 1);
+    DFT_CUDA_CHECK(cudaGetLastError());
+  }
   return DFT_OK;
 }
 

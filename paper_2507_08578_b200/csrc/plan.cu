@@ -282,7 +282,8 @@ static int ensure_workspace(dft_plan *p, int64_t per_band, int nband, int *chunk
   return DFT_OK;
 }
 
-static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nband, cudaStream_t st, const Recurrence *rec = nullptr) {
+static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nband, cudaStream_t st, const Recurrence *rec = nullptr,
+                      double *spsi = nullptr) {
   p->last_launches = 0;
   if (nband == 0 || p->mpw == 0 || p->nkpt == 0) return DFT_OK;
   const bool loc = (p->terms & 2) != 0, kin = (p->terms & 1) != 0, nl = (p->terms & 4) != 0 && p->nproj > 0;
@@ -331,8 +332,9 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
         }
       }
   }
-  if (kin || nl || rec)
-    if ((rc = nonlocal_apply(p, psi, hpsi, nband, true, kin, nl, st, nullptr, p->vecpot_on ? p->d_kinaptr : nullptr, nullptr, rec))) return rc;
+  if (kin || nl || rec || spsi)
+    if ((rc = nonlocal_apply(p, psi, hpsi, nband, true, kin, nl, st, nullptr, p->vecpot_on ? p->d_kinaptr : nullptr, nullptr, rec,
+                             spsi))) return rc;
   return DFT_OK;
 }
 
@@ -709,6 +711,22 @@ int dft_apply_s(dft_plan *p, const double *psi, double *spsi, int32_t nband, voi
   for (int ik = 0; ik < p->nkpt; ik++) ragged |= p->kp[ik].npw < p->mpw;
   if (ragged) DFT_CUDA_CHECK(cudaMemsetAsync(spsi, 0, (size_t)p->nkpt * nband * p->mpw * 16, (cudaStream_t)stream));   // pad entries = 0
   return nonlocal_apply(p, psi, spsi, nband, false, true, p->nproj > 0, (cudaStream_t)stream, p->d_sij, p->d_oneptr, nullptr);
+  DFT_GUARD_END
+}
+
+int dft_apply_hs(dft_plan *p, const double *psi, double *hpsi, double *spsi, int32_t nband, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  if (nband > 0 && p->mpw > 0 && (!psi || !hpsi || !spsi)) { set_error("null psi/hpsi/spsi"); return DFT_ERR_INVALID_ARG; }
+  if (((uintptr_t)psi & 15) || ((uintptr_t)hpsi & 15) || ((uintptr_t)spsi & 15)) { set_error("psi/hpsi/spsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  if (nband > 0 && p->mpw > 0) {
+    if ((p->terms & 4) == 0) { set_error("dft_apply_hs needs the non-local term switched on (terms bit 2)"); return DFT_ERR_INVALID_ARG; }
+    bool ragged = false;
+    for (int ik = 0; ik < p->nkpt; ik++) ragged |= p->kp[ik].npw < p->mpw;
+    if (ragged) DFT_CUDA_CHECK(cudaMemsetAsync(spsi, 0, (size_t)p->nkpt * nband * p->mpw * 16, (cudaStream_t)stream));
+  }
+  return apply_impl(p, psi, hpsi, nband, (cudaStream_t)stream, nullptr, spsi);
   DFT_GUARD_END
 }
 

@@ -504,6 +504,15 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
     for (int j = 0; j < Q.S - 1 && j < nmine; j++) issue();
   int st = 0; uint32_t ph = 0;
   bool newgroup = true;
+  // which of this thread's z = s + R2 j are occupied planes, and in which of the two runs: fixed for the whole kernel
+  unsigned vmask = 0, hmask = 0;
+#pragma unroll
+  for (int j1 = 0; j1 < R1; j1++) {
+    const int z = s + R2 * j1;
+    if (run_map(G.zrun, z) >= 0) vmask |= 1u << j1;
+    if ((unsigned)(z - G.zrun.hi) < (unsigned)G.zrun.nhi) hmask |= 1u << j1;
+  }
+  const int off1 = (s - G.zrun.lo) * XT, off2 = (s - G.zrun.hi + G.zrun.nlo) * XT;   // plane ordinal * XT minus R2 j XT
   for (int it = 0; it < nmine; it++) {
     if (t == 0 && it + Q.S - 1 < nmine) issue();
     const size_t xy = (size_t)g * XT + px;
@@ -523,8 +532,8 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
     if (s < R2) {
 #pragma unroll
       for (int j1 = 0; j1 < R1; j1++) {
-        int p = run_map(G.zrun, s + R2 * j1);
-        v[j1] = p >= 0 ? in[p * XT] : make_double2(0.0, 0.0);
+        const cplx *src = in + ((hmask >> j1) & 1 ? off2 : off1) + R2 * j1 * XT;
+        v[j1] = (vmask >> j1) & 1 ? *src : make_double2(0.0, 0.0);
       }
       Dft<R1, +1>::run(v);
 #pragma unroll
@@ -555,10 +564,11 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
       Dft<R1, -1>::run(v);
       cplx *base = T2 + (size_t)b * G.t2_band + xy;
 #pragma unroll
-      for (int d = 0; d < R1; d++) {
-        int p = xok ? run_map(G.zrun, s + R2 * d) : -1;
-        if (p >= 0) base[(size_t)p * pstride] = v[d];
-      }
+      const unsigned smask = xok ? vmask : 0u;
+      cplx *base1 = base + (ptrdiff_t)(s - G.zrun.lo) * (ptrdiff_t)pstride, *base2 = base + (ptrdiff_t)(s - G.zrun.hi + G.zrun.nlo) * (ptrdiff_t)pstride;
+#pragma unroll
+      for (int d = 0; d < R1; d++)
+        if ((smask >> d) & 1) ((hmask >> d) & 1 ? base2 : base1)[(size_t)(R2 * d) * pstride] = v[d];
     }
     __syncthreads();
     if (++st == Q.S) { st = 0; ph ^= 1; }

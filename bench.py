@@ -89,6 +89,20 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
 
 
+def read_traffic(config, kernel):
+    """ncu dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed capture summaries."""
+    for name in ("r2_traffic.csv", "r1_traffic.csv"):
+        try:
+            with open(os.path.join(ROOT, "profiles", name)) as f:
+                for row in f.read().splitlines()[1:]:
+                    c_, k_, b_ = row.split(",")[:3]
+                    if c_ == config and k_ == kernel and b_:
+                        return int(b_)
+        except Exception:
+            pass
+    return None
+
+
 def geometry(plan):
     """Sizes the byte/flop model needs, from the library's own index maps (ik = 0 .. nkpt-1)."""
     n1, n2, n3 = plan.ngfft
@@ -169,6 +183,67 @@ def vendor_library_step(plan, cfg, psi, vloc_dev, dij_np, band_chunk=32):
     return step, out
 
 
+def measure_config(name, hbm_gbs, steps=20, warmup=3):
+    """One of the other BASELINE.json cells (c0..c3) in the default launch configuration: ms per dft_apply_h with the L2
+    flushed between steps (a 512 MB write; these cells' inputs do not all exceed the 126 MB L2) and back to back,
+    the fraction of SURVEY.md 8(d)'s five-pass + GEMM roofline, the fraction of the compulsory model (2a bytes + GEMM
+    flops: what 8(d) prescribes for the boxes that fit on chip, c0 and c3), and the kernel group with the largest share."""
+    import torch
+    import synth
+    import paper_2507_08578_b200 as dft
+    cfg = synth.make_config(name)
+    plan = dft.Plan(cfg)
+    plan.set_vloc(torch.as_tensor(cfg["vloc"], device="cuda"))
+    kin_list = [plan.get_kg(ik)[2] for ik in range(plan.nkpt)]
+    nband = cfg["nband"]
+    psi = synth.gen_psi_torch(cfg, kin_list, "cuda")
+    hpsi = torch.empty_like(psi)
+    geo = geometry(plan)
+    fft_bytes, g1, g2 = byte_flop_model(plan, geo, nband, 6.0)
+    for _ in range(warmup):
+        plan.apply_h(psi, hpsi)
+    torch.cuda.synchronize()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    cold = []
+    for _ in range(steps):
+        flush.zero_()
+        a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+        a.record(); plan.apply_h(psi, hpsi); b.record()
+        torch.cuda.synchronize()
+        cold.append(a.elapsed_time(b))
+    a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(steps):
+        plan.apply_h(psi, hpsi)
+    b.record()
+    torch.cuda.synchronize()
+    warm = a.elapsed_time(b) / steps
+    launches = plan.last_launches()
+    plan.set_timing(True); plan.phase_ms()
+    for _ in range(steps):
+        flush.zero_()
+        plan.apply_h(psi, hpsi)
+    torch.cuda.synchronize()
+    ph = {k: v[0] / steps for k, v in plan.phase_ms().items()}
+    plan.set_timing(False)
+    ms = statistics.median(cold)
+    units = plan.nkpt * nband
+    gemm_s = (g1 + g2) / (FP64_PEAK_TFLOPS * 1e12)
+    t_roof = sum(fft_bytes.values()) / (hbm_gbs * 1e9) + gemm_s
+    t_comp = sum(2 * 16.0 * g["npw"] * nband for g in geo) / (hbm_gbs * 1e9) + gemm_s
+    dom = max(ph, key=lambda k: ph[k])
+    out = {"workload": WORKLOADS[name], "ms_per_step": ms, "ms_per_step_back_to_back": warm, "bands_per_s": units / (ms * 1e-3),
+           "launches_per_step": launches, "t_roof_ms": t_roof * 1e3, "frac": t_roof * 1e3 / ms,
+           "frac_vs_F_nl_8flop": (t_roof + gemm_s / 3.0) * 1e3 / ms,
+           "t_compulsory_ms": t_comp * 1e3, "frac_compulsory": t_comp * 1e3 / ms,
+           "dominant_kernel": dom, "dominant_share": ph[dom] / max(sum(ph.values()), 1e-30),
+           "phase_ms": {k: round(v, 5) for k, v in ph.items()}, "l2": "flushed between steps (512 MB write)", "steps": steps}
+    plan.destroy()
+    del psi, hpsi, flush
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_reference(args, cfg, rank):
     if rank != 0:
         return
@@ -204,8 +279,14 @@ def main():
     ap.add_argument("--ref-bands", type=int, default=0)
     ap.add_argument("--vendor", type=int, default=1, help="0 = skip the cuFFT + cuBLAS context figure")
     ap.add_argument("--cuda-graph", action="store_true", help="replay the step from a captured CUDA graph (small cells)")
+    ap.add_argument("--other-configs", type=int, default=1, help="0 = skip the c0..c3 figures of the default c4 run")
     ap.add_argument("--cheb-degree", type=int, default=10, help="degree of the Chebyshev-filter context figure (0 = skip)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU), same arguments
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--local-addr", "127.0.0.1", os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
 
@@ -257,7 +338,7 @@ def main():
             plan.apply_h(psi, hpsi)
         graph.replay()
         torch.cuda.synchronize()
-    plan.set_timing(graph is None)
+    plan.set_timing(False)       # `value` is measured without the per-phase events; they get their own pass below
     sampler = ClockSampler(local); sampler.start()
     sharding.barrier(); torch.cuda.synchronize()
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
@@ -272,9 +353,16 @@ def main():
     clocks = sampler.stop()
     ms_total = sharding.max_over_ranks(e0.elapsed_time(e1))
     launches = plan.last_launches() * K
+    ms_step = ms_total / K
+    # per-phase breakdown: a separate instrumented pass of K steps (CUDA events around every kernel group, on the launching stream)
+    if graph is None:
+        plan.set_timing(True)
+        plan.phase_ms()
+        for _ in range(K):
+            plan.apply_h(psi, hpsi)
+        torch.cuda.synchronize()
     phases = plan.phase_ms()
     plan.set_timing(False)
-    ms_step = ms_total / K
     units = plan.nkpt * nband * world
     value = units / (ms_step * 1e-3)
 
@@ -304,11 +392,7 @@ def main():
     traffic = None      # ncu dram bytes per launch of that kernel, from the committed capture summary (full-size runs only)
     try:
         if not args.nband and world == 1:
-            with open(os.path.join(ROOT, "profiles", "r1_traffic.csv")) as f:
-                for row in f.read().splitlines()[1:]:
-                    c_, k_, b_ = row.split(",")
-                    if c_ == args.config and k_ == dom and b_:
-                        traffic = int(b_)
+            traffic = read_traffic(args.config, dom)
     except Exception:
         traffic = None
     roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],
@@ -446,6 +530,18 @@ def main():
                        "d2h_bytes_per_step": nbytes, "ms_per_step": dt, "steps": ke,
                        "api": "dft_apply_h_host (pinned host psi -> device, H, device -> pinned host hpsi)"}
     plan.destroy()
+
+    # ---- the other four BASELINE.json cells (north_star: "throughput is reported on the seeded synthetic cells"); each is
+    #      its own plan; none enters `value`
+    if args.config == "c4" and world == 1 and not args.nband and args.other_configs:
+        del psi
+        torch.cuda.empty_cache()
+        line["configs"] = {}
+        for name in ("c0", "c1", "c2", "c3"):
+            try:
+                line["configs"][name] = measure_config(name, hbm_gbs)
+            except Exception as e:       # never fail the headline over a context figure
+                line["configs"][name] = {"unavailable": repr(e)[:200]}
 
     # ---- cpu_baseline: the oracle as it stands, bounded sample, rank 0 at N=1 only
     if rank == 0 and world == 1 and not args.no_cpu:

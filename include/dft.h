@@ -94,7 +94,9 @@ int dft_plan_get_projectors(const dft_plan *p, int32_t ik, double *ptab);
  * vendor-library context figure).                                                                  */
 int dft_plan_copy_projectors_device(const dft_plan *p, int32_t ik, double *ptab_dev, void *stream);
 
-/* Replace D_ij (PAW: "from self-consistent terms", PAPER.md :473).  HOST [natom][nlmn_max]^2.    */
+/* Replace D_ij (PAW: "from self-consistent terms", PAPER.md :473).  HOST [natom][nlmn_max]^2.
+ * Synchronises the device first (work enqueued earlier by dft_apply_h on any stream still sees the old values),
+ * then copies; later calls see the new ones.                                                     */
 int dft_set_dij(dft_plan *p, const double *dij);
 
 /* Set the local potential: V_r is DEVICE memory, [n3][n2][n1] doubles, i1 fastest.  It is copied
@@ -106,6 +108,13 @@ int dft_set_vloc(dft_plan *p, const double *V_r, void *stream);
  * chunk of one band; dft_apply_h then never allocates.  dev_ptr = NULL returns to plan-owned
  * scratch (allocated lazily, grown on demand).  256-byte alignment required.                     */
 int dft_set_workspace(dft_plan *p, void *dev_ptr, int64_t bytes);
+
+/* Scratch sizes for dft_set_workspace (either output may be NULL): *min_bytes = the smallest workspace dft_apply_h can
+ * run with (one band of one k-point per launch); *full_bytes = the workspace with which `nband` bands per k-point go
+ * through the FFT passes in ONE chunk on the fastest path (for several k-points that is the all-k-points-per-launch
+ * path, whose layout is T1 [nkpt][nband][max_k t1] followed by T2 [nkpt][nband][max_k t2]).  Anything in between
+ * is used as far as it goes (more, smaller launches).                                              */
+int dft_plan_workspace_bytes(const dft_plan *p, int32_t nband, int64_t *min_bytes, int64_t *full_bytes);
 
 /* Options: "band_chunk" (bands per FFT pass launch, > 0), "terms" (bit 0 kinetic, bit 1 local,
  * bit 2 non-local, bit 3 meta-GGA term; default 15), "splitk" (GEMM-1 K splits, 0 = automatic), "proj_mode" (0 = default: projector table materialised in
@@ -130,7 +139,8 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value);
 int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);
 
 /* PAW overlap coefficients s^a_ij, HOST [natom][nlmn_max][nlmn_max] real symmetric (zero after
- * dft_plan_create): "the overlap operator S ... has the same structure" as Eq. 26 (PAPER.md :473).  */
+ * dft_plan_create): "the overlap operator S ... has the same structure" as Eq. 26 (PAPER.md :473).
+ * Synchronises the device first, like dft_set_dij.                                                  */
 int dft_set_sij(dft_plan *p, const double *sij);
 
 /* spsi = S psi = psi + sum_a sum_ij |p_a,i> s^a_ij <p_a,j|psi> (PAPER.md :473), same layouts, stream and

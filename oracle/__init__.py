@@ -2,7 +2,9 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference`
 legs may import this package.  It imports nothing from paper_2507_08578_b200 and the
-product never imports it.  All arithmetic is in oracle.c; this file marshals numpy arrays.
+product never imports it.  The arithmetic of the hot path (sphere, FFT tiers, projector table, non-local loops, dense H) is in oracle.c and this
+file marshals numpy arrays for it; the restatements of the NEXT rows (kin_vecpot, density, tau_density, apply_mgga,
+chebyshev_filter, apply_s, cprj, and the Gamma-storage / spinor functions) are plain numpy in this file, each with its own pin in tests/.
 
 `cfg` arguments are the dicts of synth.make_config (input data only).
 """

@@ -31,7 +31,7 @@ DFT_ERR_UNSUPPORTED = -7
 PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather", "gemm1", "dij", "gemm2_kinetic")
 
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
-SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
+SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_workspace_bytes", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_apply_hs", "dft_get_cprj", "dft_chebyshev_filter",
            "dft_set_vector_potential", "dft_accumulate_density", "dft_accumulate_tau",
            "dft_set_vtau",
@@ -73,6 +73,7 @@ def lib():
     L.dft_plan_create.argtypes = [C.POINTER(C.c_void_p), _dp, C.c_int32, _dp, C.c_double, _ip, C.c_int32, _ip, _dp,
                                   C.c_int32, C.POINTER(dft_proj_table), _dp]
     L.dft_plan_get_info.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip, C.POINTER(C.c_int64)]
+    L.dft_plan_workspace_bytes.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.dft_plan_get_kg.argtypes = [C.c_void_p, C.c_int32, _ip, _ip, _dp]
     L.dft_plan_get_projectors.argtypes = [C.c_void_p, C.c_int32, _dp]
     L.dft_set_dij.argtypes = [C.c_void_p, _dp]
@@ -158,6 +159,13 @@ def dft_plan_get_info(plan):
     mpw, nproj, ws = C.c_int32(), C.c_int32(), C.c_int64()
     _check(lib().dft_plan_get_info(plan, C.byref(nk), _i(npw), C.byref(mpw), C.byref(nproj), C.byref(ws)))
     return dict(nkpt=nk.value, npw=npw, mpw=mpw.value, nproj=nproj.value, workspace_bytes_per_band=ws.value)
+
+
+def dft_plan_workspace_bytes(plan, nband):
+    """(min_bytes, full_bytes) of device scratch for dft_set_workspace."""
+    lo, hi = C.c_int64(), C.c_int64()
+    _check(lib().dft_plan_workspace_bytes(plan, nband, C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
 
 
 def dft_plan_get_kg(plan, ik, npw):
@@ -267,6 +275,9 @@ class Plan:
         self.workspace_bytes_per_band = info["workspace_bytes_per_band"]
         self.ngfft = tuple(int(v) for v in cfg["ngfft"])
         self._keep = []
+
+    def workspace_bytes(self, nband):
+        return dft_plan_workspace_bytes(self.h, nband)
 
     def get_kg(self, ik=0):
         return dft_plan_get_kg(self.h, ik, int(self.npw[ik]))

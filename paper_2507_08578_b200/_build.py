@@ -25,7 +25,19 @@ def _stale(target, deps):
 
 
 def build(force=False, verbose=False):
-    """Compile every CUDA source and link the shared library; returns its path."""
+    """Compile every CUDA source and link the shared library; returns its path.  The whole build holds an exclusive
+    file lock, so the ranks of a multi-GPU launch on a fresh box do not compile the same objects at the same time
+    (the first one builds, the others find everything up to date)."""
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            return _build_locked(force, verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(force, verbose):
     objs, jobs = [], []
     for s, o, extra in SOURCES:
         src = os.path.join(CSRC, s)

@@ -296,16 +296,28 @@ int64_t fft_ws_bytes_per_band(const dft_plan *p) {
   return mx;
 }
 
-static bool g_attr_done = false;
+// scratch per band of the all-k-points-per-launch path (fft2_apply_batched): T1 [nkpt][nb][max_k t1] then T2 [nkpt][nb][max_k t2],
+// i.e. the two maxima taken SEPARATELY (the k-point with most columns need not be the one with most planes)
+int64_t fft_ws_bytes_per_band_batched(const dft_plan *p) {
+  int64_t m1 = 0, m2 = 0;
+  for (int ik = 0; ik < p->nkpt; ik++) {
+    const KPoint &kp = p->kp[ik];
+    int64_t t1 = ((int64_t)kp.ncol * p->n[0] * 16 + 255) / 256 * 256;
+    int64_t t2 = ((int64_t)kp.nplane * p->n[1] * p->n[0] * 16 + 255) / 256 * 256;
+    if (t1 > m1) m1 = t1;
+    if (t2 > m2) m2 = t2;
+  }
+  return (m1 + m2) * p->nkpt;
+}
+
 static int set_attrs() {
-  if (g_attr_done) return DFT_OK;
+  // set unconditionally (cheap): a per-process flag would miss a plan on a second device
   int mx = (int)(SMEM_BUDGET + 24 * 1024);
   DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_a_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
   DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_ainv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
   DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_b_kernel<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
   DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_b_kernel<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
   DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_pass_c_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, mx));
-  g_attr_done = true;
   return DFT_OK;
 }
 

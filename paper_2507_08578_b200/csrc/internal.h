@@ -72,6 +72,7 @@ struct KPoint {
 struct PhaseTimer {
   bool on = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[8];
+  std::vector<cudaEvent_t> pool;   // events handed back by dft_plan_phase_ms, reused by later applies
   int64_t launches[8] = {0};
 };
 
@@ -143,6 +144,7 @@ struct dft_plan {
   int sm_count = 148;
   int smem_per_sm = 233472, smem_optin = 232448;   // bytes of shared memory per SM / per CTA (opt-in), from the device
   int64_t last_launches = 0;
+  bool nl_attr_done = false;   // cudaFuncSetAttribute of the GEMM kernels done on this plan's device
   dftb200::PhaseTimer timer;
 };
 
@@ -170,6 +172,7 @@ struct FftExtra {
 };
 // --- fft.cu (K2) --------------------------------------------------------------------------
 int64_t fft_ws_bytes_per_band(const dft_plan *p);
+int64_t fft_ws_bytes_per_band_batched(const dft_plan *p);   // per band, all k-points (fft2_apply_batched's layout)
 // V_loc psi for `nb` bands of k-point ik: psi/hpsi point at the first band ([nb][mpw] complex)
 int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb, void *ws, cudaStream_t st,
                    const FftExtra *extra = nullptr);

@@ -819,7 +819,6 @@ __global__ void kin_only_kernel(const double2 *__restrict__ psi, double2 *__rest
   }
 }
 
-static bool g_nl_attr = false;
 
 // choose the number of K splits of GEMM-1: fill the SMs in whole waves, keep >= 32 slabs per split
 static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
@@ -846,14 +845,14 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   if (cprj_out && p->nproj == 0) return DFT_OK;
   if (p->nproj == 0) with_nl = false;
   if (!with_nl && !with_kin && accumulate && !rec) return DFT_OK;
-  if (!g_nl_attr) {
+  if (!p->nl_attr_done) {   // per plan (= per device), not per process
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_fac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FC_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_fac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FD_SMEM));
-    g_nl_attr = true;
+    p->nl_attr_done = true;
   }
   const int32_t *d_npw = p->d_npw;
   const double *const *d_kin = diag ? diag : p->d_kinptr;

@@ -27,7 +27,9 @@ void set_error(const char *fmt, ...) {
 void phase_begin(dft_plan *p, int phase, cudaStream_t st) {
   if (!p->timer.on) return;
   cudaEvent_t a, b;
-  cudaEventCreate(&a); cudaEventCreate(&b);
+  auto &pool = p->timer.pool;   // events are reused: dft_plan_phase_ms hands them back
+  if (pool.size() >= 2) { a = pool.back(); pool.pop_back(); b = pool.back(); pool.pop_back(); }
+  else { cudaEventCreate(&a); cudaEventCreate(&b); }
   cudaEventRecord(a, st);
   p->timer.ev[phase].push_back({a, b});
 }
@@ -68,6 +70,7 @@ static void destroy_plan(dft_plan *p) {
   if (p->d2h_stream) cudaStreamDestroy(p->d2h_stream);
   for (int ph = 0; ph < 8; ph++)
     for (auto &e : p->timer.ev[ph]) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
+  for (cudaEvent_t e : p->timer.pool) cudaEventDestroy(e);
   cudaGetLastError();
   delete p;
 }
@@ -292,9 +295,9 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
   const size_t band_stride = (size_t)p->mpw * 2;
   if (loc) {
     int chunk; void *ws;
-    if (fft2_batch_ok(p) && (!p->ws_user || p->ws_user_bytes >= fft_ws_bytes_per_band(p) * p->nkpt)) {
+    if (fft2_batch_ok(p) && (!p->ws_user || p->ws_user_bytes >= fft_ws_bytes_per_band_batched(p))) {
       // small boxes, many k-points: every pass is one launch over all k-points (blockIdx.y = k-point)
-      if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p) * p->nkpt, nband, &chunk, &ws, st))) return rc;
+      if ((rc = ensure_workspace(p, fft_ws_bytes_per_band_batched(p), nband, &chunk, &ws, st))) return rc;
       for (int b0 = 0; b0 < nband; b0 += chunk) {
         int nb = nband - b0 < chunk ? nband - b0 : chunk;
         if ((rc = fft2_apply_batched(p, psi + (size_t)b0 * band_stride, hpsi + (size_t)b0 * band_stride, nb, nband, ws, st))) return rc;
@@ -419,6 +422,8 @@ int dft_set_dij(dft_plan *p, const double *dij) {
   size_t n = (size_t)p->natom * p->lmax * p->lmax;
   if (n == 0) return DFT_OK;
   if (!dij) { set_error("dij is NULL"); return DFT_ERR_INVALID_ARG; }
+  // an apply enqueued earlier on a non-blocking stream may still read D_ij: wait for the device before replacing it
+  DFT_CUDA_CHECK(cudaDeviceSynchronize());
   DFT_CUDA_CHECK(cudaMemcpy(p->d_dij, dij, n * sizeof(double), cudaMemcpyHostToDevice));
   return DFT_OK;
 }
@@ -496,6 +501,14 @@ int dft_set_workspace(dft_plan *p, void *dev_ptr, int64_t bytes) {
   if (dev_ptr && (bytes <= 0 || ((uintptr_t)dev_ptr & 255))) { set_error("workspace must be 256-byte aligned with bytes > 0"); return DFT_ERR_INVALID_ARG; }
   if (dev_ptr && bytes < fft_ws_bytes_per_band(p)) { set_error("workspace smaller than one band (%lld bytes needed)", (long long)fft_ws_bytes_per_band(p)); return DFT_ERR_ALLOC; }
   p->ws_user = dev_ptr; p->ws_user_bytes = dev_ptr ? bytes : 0;
+  return DFT_OK;
+}
+
+int dft_plan_workspace_bytes(const dft_plan *p, int32_t nband, int64_t *min_bytes, int64_t *full_bytes) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  if (min_bytes) *min_bytes = fft_ws_bytes_per_band(p);
+  if (full_bytes) *full_bytes = (fft2_batch_ok(p) ? fft_ws_bytes_per_band_batched(p) : fft_ws_bytes_per_band(p)) * (int64_t)nband;
   return DFT_OK;
 }
 
@@ -694,6 +707,7 @@ int dft_set_sij(dft_plan *p, const double *sij) {
   size_t n = (size_t)p->natom * p->lmax * p->lmax;
   if (n == 0) return DFT_OK;
   if (!sij) { set_error("sij is NULL"); return DFT_ERR_INVALID_ARG; }
+  DFT_CUDA_CHECK(cudaDeviceSynchronize());   // see dft_set_dij
   DFT_CUDA_CHECK(cudaMemcpy(p->d_sij, sij, n * sizeof(double), cudaMemcpyHostToDevice));
   return DFT_OK;
 }
@@ -839,7 +853,7 @@ int dft_plan_phase_ms(dft_plan *p, int32_t phase, double *ms, int64_t *launches)
     float t = 0.f;
     DFT_CUDA_CHECK(cudaEventElapsedTime(&t, e.first, e.second));
     tot += t;
-    cudaEventDestroy(e.first); cudaEventDestroy(e.second);
+    p->timer.pool.push_back(e.first); p->timer.pool.push_back(e.second);
   }
   p->timer.ev[phase].clear();
   if (ms) *ms = tot;

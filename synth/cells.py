@@ -23,7 +23,7 @@ BASE_SEED = 20250708
 STREAM_PSI, STREAM_VNOISE, STREAM_DIJ = 1, 2, 3
 
 CONFIG_NAMES = ("c0", "c1", "c2", "c3", "c4",
-                "c1m", "c2m", "c4m", "aniso", "c3k2", "aniso8")
+                "c1m", "c2m", "c4m", "aniso", "c3k2", "aniso8", "anisok3")
 
 _DIAMOND_SITES = np.array([[0, 0, 0], [0, .5, .5], [.5, 0, .5], [.5, .5, 0],
                            [.25, .25, .25], [.25, .75, .75], [.75, .25, .75], [.75, .75, .25]])
@@ -162,13 +162,15 @@ def make_config(name, with_vloc=True, **over):
     elif name in ("c4", "c4m"):
         rprimd = np.diag([4 * a_si] * 3); xred = _si_supercell(4); kpt = [[0, 0, 0]]
         ecut, ngfft, nband = (20.0, (180, 180, 180), 1024) if name == "c4" else (0.5, (36, 36, 36), 7)
-    elif name == "aniso":     # SURVEY.md 8(c) extra case (ii): triclinic, anisotropic box, two types
+    elif name in ("aniso", "anisok3"):     # SURVEY.md 8(c) extra case (ii): triclinic, anisotropic box, two types
         rprimd = np.array([[9.0, 0.4, -0.3], [0.7, 10.5, 0.5], [-0.6, 0.8, 13.0]])
         xred = np.array([[0.0, 0.0, 0.0],                      # exactly on a grid point
                          [0.3183098861837907, 0.7071067811865476, 0.5772156649015329],  # irrational
                          [0.55, 0.25, 0.8]])
         kinds = ["Si", "Al"]; typat = np.array([0, 1, 0], np.int32)
         kpt = [[0.1, -0.2, 0.05]]
+        if name == "anisok3":   # three k-points: most columns at the third, most planes at the second (scratch-size check)
+            kpt = [[0.1, -0.2, 0.05], [0.0, 0.0, 0.5], [0.5, 0.5, 0.0]]
         ecut, ngfft, nband = 2.5, (20, 24, 30), 4
     elif name == "aniso8":    # aniso with two types of at most 8 projectors (8 and 4): rows of one atom are not 8-aligned
         rprimd = np.array([[9.0, 0.4, -0.3], [0.7, 10.5, 0.5], [-0.6, 0.8, 13.0]])

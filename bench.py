@@ -89,17 +89,17 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
 
 
-def read_traffic(config, kernel):
-    """ncu dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed capture summaries."""
-    for name in ("r2_traffic.csv", "r1_traffic.csv"):
-        try:
-            with open(os.path.join(ROOT, "profiles", name)) as f:
-                for row in f.read().splitlines()[1:]:
-                    c_, k_, b_ = row.split(",")[:3]
-                    if c_ == config and k_ == kernel and b_:
-                        return int(b_)
-        except Exception:
-            pass
+def read_traffic(config, kernel, bands_per_launch):
+    """ncu dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed capture summary
+    (profiles/r2_traffic.csv: per launch for the GEMMs, per band for the FFT passes, whose launches are band chunks)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
+            for row in f.read().splitlines()[1:]:
+                c_, k_, b_, per = row.split(",")[:4]
+                if c_ == config and k_ == kernel and b_:
+                    return int(int(b_) * (bands_per_launch if per == "band" else 1))
+    except Exception:
+        pass
     return None
 
 
@@ -392,7 +392,7 @@ def main():
     traffic = None      # ncu dram bytes per launch of that kernel, from the committed capture summary (full-size runs only)
     try:
         if not args.nband and world == 1:
-            traffic = read_traffic(args.config, dom)
+            traffic = read_traffic(args.config, dom, nband / max(1, d["launches_per_step"]))
     except Exception:
         traffic = None
     roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],

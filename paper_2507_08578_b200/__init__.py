@@ -28,7 +28,8 @@ DFT_ERR_CUDA = -5
 DFT_ERR_NOT_READY = -6
 DFT_ERR_UNSUPPORTED = -7
 
-PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather", "gemm1", "dij", "gemm2_kinetic")
+PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather", "gemm1", "dij", "gemm2_kinetic",
+          "fft_small_fused")
 
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_workspace_bytes", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",

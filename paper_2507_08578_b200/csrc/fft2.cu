@@ -828,7 +828,7 @@ static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi
                        int nb, int hb, cudaStream_t st, const FftExtra &X) {
   constexpr int NS = imax(R1, R2);
   int rc;
-  if (pass >= 1 && pass <= 3 && p->fft_path == 0) {
+  if (pass >= 1 && pass <= 3 && (p->fft_path == 0 || p->fft_path == 4)) {
     rc = launch_ring<R1, R2>(p, G, pass, T1, T2, vloc, nb, hb, st);
     if (rc != DFT_ERR_UNSUPPORTED) return rc;
   }

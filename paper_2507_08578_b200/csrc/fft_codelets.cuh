@@ -159,6 +159,7 @@ template <int S> struct Dft<6, S> { static DFT_HD void run(cplx *v) { Pfa<2, 3, 
 template <int S> struct Dft<10, S> { static DFT_HD void run(cplx *v) { Pfa<2, 5, S>::run(v); } };
 template <int S> struct Dft<12, S> { static DFT_HD void run(cplx *v) { Pfa<4, 3, S>::run(v); } };
 template <int S> struct Dft<15, S> { static DFT_HD void run(cplx *v) { Pfa<3, 5, S>::run(v); } };
+template <int S> struct Dft<18, S> { static DFT_HD void run(cplx *v) { Pfa<2, 9, S>::run(v); } };
 template <int S> struct Dft<20, S> { static DFT_HD void run(cplx *v) { Pfa<4, 5, S>::run(v); } };
 
 }  // namespace dftb200

@@ -69,11 +69,13 @@ struct KPoint {
   std::vector<double> h_kin;
 };
 
+// timed kernel groups: 0-4 the five FFT passes, 5 GEMM-1, 6 D_ij, 7 GEMM-2, 8 the fused small-box local term (fft_small.cu)
+constexpr int NPHASE = 9;
 struct PhaseTimer {
   bool on = false;
-  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[8];
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[NPHASE];
   std::vector<cudaEvent_t> pool;   // events handed back by dft_plan_phase_ms, reused by later applies
-  int64_t launches[8] = {0};
+  int64_t launches[NPHASE] = {0};
 };
 
 }  // namespace dftb200
@@ -123,8 +125,10 @@ struct dft_plan {
   // options
   int band_chunk = 0;      // 0 = automatic
   int terms = 15;          // bit 0 kinetic, bit 1 local, bit 2 non-local, bit 3 meta-GGA term (active once dft_set_vtau was called)
-  int fft_path = 0;        // 0 = automatic (register path, TMA ring for the strided passes), 1 = generic Stockham path only,
-                           // 2 = register path without the TMA ring
+  int fft_path = 0;        // 0 = automatic (fused small-box kernel when a band's working set fits one SM's shared memory, else
+                           // the register path with the TMA ring for the strided passes), 1 = generic Stockham path only,
+                           // 2 = register path without the TMA ring, 3 = fused small-box kernel (error if it does not fit),
+                           // 4 = automatic without the small-box kernel
   int splitk = 0;
   int gemm_3m = 1;         // 1 = three real products per complex multiply-add (6 flops), 0 = four (8 flops)
   // workspace
@@ -141,6 +145,8 @@ struct dft_plan {
   void *encode_fn = nullptr;   // cuTensorMapEncodeTiled
   double *d_wgt = nullptr; int64_t wgt_count = 0;    // device copy of the band weights of dft_accumulate_density
   void *d_geom2 = nullptr;    // device array of per-k-point FFT geometry (fft2.cu, built at first batched call)
+  void *d_geom_small = nullptr;   // the same for the fused small-box kernel (fft_small.cu)
+  bool small_attr_done = false;
   int sm_count = 148;
   int smem_per_sm = 233472, smem_optin = 232448;   // bytes of shared memory per SM / per CTA (opt-in), from the device
   int64_t last_launches = 0;
@@ -197,6 +203,11 @@ int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int
 // rho(r) += sum_b wgt[b] |psi_b(r)|^2 (device wgt [nb]); forward passes A, B and the density kernel
 int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st,
                  const double *pre = nullptr);
+
+// --- fft_small.cu (K2s): the whole local term in one kernel, one CTA per (k-point, band), no scratch in device memory
+bool fft_small_ok(const dft_plan *p);
+int fft_small_apply(dft_plan *p, int ik0, int nk, const double *psi, double *hpsi, int nb, int nband_total, cudaStream_t st,
+                    const FftExtra *extra = nullptr);
 
 // --- nonlocal.cu (K3) ---------------------------------------------------------------------
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi

@@ -62,13 +62,13 @@ static void destroy_plan(dft_plan *p) {
   cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
   cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
   cudaFree(p->d_blk_atom); cudaFree(p->d_blk_frow); cudaFree(p->d_blk_first); cudaFree(p->d_blk_nl);
-  cudaFree(p->d_stab); cudaFree(p->d_fytab); cudaFree(p->d_vtau); cudaFree(p->d_qcart); cudaFree(p->d_qhalf); cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  cudaFree(p->d_stab); cudaFree(p->d_fytab); cudaFree(p->d_vtau); cudaFree(p->d_qcart); cudaFree(p->d_qhalf); cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_geom_small); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
   if (p->h2d_stream) cudaStreamDestroy(p->h2d_stream);
   if (p->d2h_stream) cudaStreamDestroy(p->d2h_stream);
-  for (int ph = 0; ph < 8; ph++)
+  for (int ph = 0; ph < NPHASE; ph++)
     for (auto &e : p->timer.ev[ph]) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
   for (cudaEvent_t e : p->timer.pool) cudaEventDestroy(e);
   cudaGetLastError();
@@ -285,6 +285,11 @@ static int ensure_workspace(dft_plan *p, int64_t per_band, int nband, int *chunk
   return DFT_OK;
 }
 
+static int ensure_qcart_ready(dft_plan *p) {
+  if (!p->d_qcart || !p->d_qhalf) { set_error("the k+G arrays of the meta-GGA term are missing"); return DFT_ERR_NOT_READY; }
+  return DFT_OK;
+}
+
 static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nband, cudaStream_t st, const Recurrence *rec = nullptr,
                       double *spsi = nullptr) {
   p->last_launches = 0;
@@ -293,7 +298,11 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
   if (loc && !p->vloc_set) { set_error("dft_apply_h called before dft_set_vloc"); return DFT_ERR_NOT_READY; }
   int rc;
   const size_t band_stride = (size_t)p->mpw * 2;
-  if (loc) {
+  const bool small = (p->fft_path == 0 || p->fft_path == 3) && fft_small_ok(p);
+  if (loc && small) {
+    // the box fits one SM's shared memory: the whole local term of all k-points and bands is ONE launch, no scratch
+    if ((rc = fft_small_apply(p, 0, p->nkpt, psi, hpsi, nband, nband, st))) return rc;
+  } else if (loc) {
     int chunk; void *ws;
     if (fft2_batch_ok(p) && (!p->ws_user || p->ws_user_bytes >= fft_ws_bytes_per_band_batched(p))) {
       // small boxes, many k-points: every pass is one launch over all k-points (blockIdx.y = k-point)
@@ -319,9 +328,19 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
   if ((p->terms & 8) && p->vtau_set) {
     // meta-GGA term (Eq. 8): hpsi += 1/2 sum_d q_d . FFT^-1[ v_tau(r) FFT[ q_d psi ] ], q = k + G Cartesian;
     // three more local applications with diagonal factors fused into the scatter and gather passes
-    int chunk; void *ws;
-    if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
-    for (int ik = 0; ik < p->nkpt; ik++)
+    int chunk = 0; void *ws = nullptr;
+    if (small) {
+      if ((rc = ensure_qcart_ready(p))) return rc;
+      for (int d = 0; d < 3; d++) {
+        FftExtra X;
+        X.vpot = p->d_vtau;
+        X.pre = p->d_qcart + (size_t)d * p->mpw;      // k-point ik: + ik * 3 * mpw (inside the kernel)
+        X.post = p->d_qhalf + (size_t)d * p->mpw;
+        X.accumulate = 1;
+        if ((rc = fft_small_apply(p, 0, p->nkpt, psi, hpsi, nband, nband, st, &X))) return rc;
+      }
+    } else if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
+    for (int ik = 0; ik < p->nkpt && !small; ik++)
       for (int b0 = 0; b0 < nband; b0 += chunk) {
         int nb = nband - b0 < chunk ? nband - b0 : chunk;
         size_t off = ((size_t)ik * nband + b0) * band_stride;
@@ -523,7 +542,8 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     p->terms = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "fft_path")) {
-    if (value < 0 || value > 2) { set_error("fft_path = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if (value < 0 || value > 4) { set_error("fft_path = %lld outside 0..4", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if (value == 3 && !fft_small_ok(p)) { set_error("fft_path = 3: the fused small-box kernel cannot serve this plan (box lengths or shared memory)"); return DFT_ERR_UNSUPPORTED; }
     p->fft_path = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "proj_mode")) {
@@ -846,7 +866,7 @@ int dft_plan_set_timing(dft_plan *p, int32_t on) {
 }
 
 int dft_plan_phase_ms(dft_plan *p, int32_t phase, double *ms, int64_t *launches) {
-  if (!p || phase < 0 || phase >= 8) { set_error("bad phase"); return DFT_ERR_INVALID_ARG; }
+  if (!p || phase < 0 || phase >= NPHASE) { set_error("bad phase"); return DFT_ERR_INVALID_ARG; }
   double tot = 0.0;
   for (auto &e : p->timer.ev[phase]) {
     DFT_CUDA_CHECK(cudaEventSynchronize(e.second));

@@ -53,3 +53,14 @@ def band_rel_err(a, b):
     num = np.linalg.norm(a - b, axis=-1); den = np.linalg.norm(b, axis=-1)
     den = np.where(den == 0, 1.0, den)
     return float(np.max(num / den))
+
+
+def small_box_ok(plan):
+    """True when the fused small-box kernel (fft_path = 3) can serve this plan; the plan's fft_path is left at 0."""
+    try:
+        plan.set_option("fft_path", 3)
+    except dft.DftError as e:
+        assert e.code == dft.DFT_ERR_UNSUPPORTED
+        return False
+    plan.set_option("fft_path", 0)
+    return True

@@ -7,7 +7,7 @@ import torch
 import oracle
 import synth
 from gpu_util import (make_plan, lib_spheres, oracle_spheres, assert_spheres_equal, gpu_apply, oracle_apply,
-                      band_rel_err)
+                      band_rel_err, small_box_ok)
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-10     # north_star: "relative error <= 1e-10 per band in FP64"
@@ -39,11 +39,12 @@ def test_small_cells_all_terms_and_isolations(name):
 @pytest.mark.parametrize("name", ["c0", "c1m", "c4m", "aniso", "c3k2"])
 def test_generic_fft_path_agrees(name):
     """Option fft_path=1 forces the generic shared-memory Stockham kernels (used for box lengths with no
-    two-stage factorisation), 2 the register path without the TMA ring; all paths must match the oracle."""
+    two-stage factorisation), 2 the register path without the TMA ring, 4 the five-pass path where the automatic choice
+    would be the fused small-box kernel, 3 that kernel; all paths must match the oracle."""
     cfg, plan, sph = _setup(name)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     ref = oracle_apply(cfg, sph, psi, method=1 if name in ("c0", "aniso") else 2)
-    for path in (1, 2, 0):
+    for path in (1, 2, 4, 0) + ((3,) if small_box_ok(plan) else ()):
         plan.set_option("fft_path", path)
         err = band_rel_err(gpu_apply(plan, psi), ref)
         assert err <= TOL, "%s fft_path=%d: rel err %.3e" % (name, path, err)
@@ -93,10 +94,12 @@ def test_band_counts_and_chunking(nband):
     cfg, plan, sph = _setup("c1m")
     psi = synth.gen_psi(cfg, [s[2] for s in sph], nband=nband)
     ref = oracle_apply(cfg, sph, psi)
-    for chunk in (0, 1, 7):
-        plan.set_option("band_chunk", chunk)
-        err = band_rel_err(gpu_apply(plan, psi), ref)
-        assert err <= TOL, "nband=%d chunk=%d: %.3e" % (nband, chunk, err)
+    for path, chunks in ((4, (0, 1, 7)), (0, (0,))):     # five-pass path in band chunks; fused small-box kernel (no chunks)
+        plan.set_option("fft_path", path)
+        for chunk in chunks:
+            plan.set_option("band_chunk", chunk)
+            err = band_rel_err(gpu_apply(plan, psi), ref)
+            assert err <= TOL, "nband=%d path=%d chunk=%d: %.3e" % (nband, path, chunk, err)
     plan.destroy()
 
 
@@ -121,11 +124,59 @@ def test_tight_box_wraparound():
     plan.destroy()
 
 
+SMALL_BOX_CASES = [("c0", {}), ("c3k2", {}), ("c1m", {}), ("c2m", {}), ("c4m", {}), ("aniso", {}), ("anisok3", {}),
+                   ("c0", {"ngfft": (9, 9, 9)}), ("c0", {"ngfft": (18, 24, 16)}), ("c0", {"ngfft": (12, 10, 8), "ecut": 3.0})]
+
+
+@pytest.mark.parametrize("name,over", SMALL_BOX_CASES, ids=lambda v: v if isinstance(v, str) else "x".join(map(str, v.get("ngfft", ()))))
+def test_small_box_fused_kernel(name, over):
+    """fft_path = 3: the whole local term in one kernel, one CTA per (k-point, band), the box in shared memory
+    (SURVEY.md 7 step 4(e), 8(d)).  All-terms and local-only results against the oracle, pads zeroed, four launches
+    per application (fused local term, GEMM-1, D_ij, GEMM-2), and the automatic choice picks it."""
+    cfg, plan, sph = _setup(name, **over)
+    assert small_box_ok(plan), "the small-box kernel should serve %s %s" % (name, over)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    method = 1 if name in ("c0", "aniso", "anisok3") else 2
+    for path in (3, 0):
+        plan.set_option("fft_path", path)
+        for terms in (7, 2):
+            plan.set_option("terms", terms)
+            got = gpu_apply(plan, psi)
+            assert plan.last_launches() == (4 if terms == 7 else 1)
+            err = band_rel_err(got, oracle_apply(cfg, sph, psi, terms=terms, method=method))
+            assert err <= TOL, "%s fft_path=%d terms=%d: rel err %.3e" % (name, path, terms, err)
+            for ik in range(plan.nkpt):
+                assert np.all(got[ik][:, plan.npw[ik]:] == 0)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("nband", [1, 3, 64, 65])
+def test_small_box_band_counts(nband):
+    cfg, plan, sph = _setup("c3k2")
+    plan.set_option("fft_path", 3)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph], nband=nband)
+    err = band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi))
+    assert err <= TOL, "nband=%d: %.3e" % (nband, err)
+    plan.destroy()
+
+
+def test_small_box_refused_when_it_does_not_fit():
+    """fft_path = 3 on a plan whose working set exceeds one SM's shared memory is DFT_ERR_UNSUPPORTED (no silent
+    change of path); the automatic choice then keeps the five-pass kernels."""
+    cfg, plan, sph = _setup("c1m", ngfft=(72, 72, 72))
+    assert not small_box_ok(plan)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    assert band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi)) <= TOL
+    assert plan.last_launches() == 8
+    plan.destroy()
+
+
 def test_set_dij_and_user_workspace_and_host_api():
     cfg, plan, sph = _setup("c1m")
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     d2 = cfg["dij"] * 0.5 + 0.1 * np.eye(cfg["nlmn_max"])[None]
     plan.set_dij(d2)
+    plan.set_option("fft_path", 4)           # the five-pass path: the one that uses a workspace
     ws = torch.empty(plan.workspace_bytes_per_band * 2 + 256, dtype=torch.uint8, device="cuda")
     off = (-ws.data_ptr()) % 256
     plan.set_workspace(ws[off:off + plan.workspace_bytes_per_band * 2])
@@ -182,7 +233,7 @@ def test_chebyshev_filter(name):
             t = torch.as_tensor(psi, device="cuda").clone()
             got = plan.chebyshev_filter(t, deg, cen, e).cpu().numpy()
             if plan.nkpt == 1:
-                assert plan.last_launches() == 8 * deg
+                assert plan.last_launches() == (4 if small_box_ok(plan) else 8) * deg
             for ik, (kg, ig, kin) in enumerate(sph):
                 ref = oracle.chebyshev_filter(cfg, ik, kg, ig, kin, psi[ik], deg, cen, e, method=1 if name == "aniso" else 2)
                 npw = len(ig)
@@ -365,6 +416,7 @@ def test_host_api_band_groups():
     cfg, plan, sph = _setup("c1m", nband=200)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     ref = oracle_apply(cfg, sph, psi)
+    plan.set_option("fft_path", 4)
     for groups in (3, 1, 4):
         plan.set_option("host_groups", groups)
         got = plan.apply_h_host(psi)
@@ -379,6 +431,7 @@ def test_multik_host_api_and_small_user_workspace():
     cfg, plan, sph = _setup("c3k2")
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     ref = oracle_apply(cfg, sph, psi)
+    plan.set_option("fft_path", 4)
     assert band_rel_err(gpu_apply(plan, psi), ref) <= TOL
     batched_launches = plan.last_launches()
     assert band_rel_err(plan.apply_h_host(psi), ref) <= TOL
@@ -397,6 +450,7 @@ def test_host_api_uneven_groups():
     cfg, plan, sph = _setup("c1m", nband=520)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     plan.set_option("host_groups", 4)
+    plan.set_option("fft_path", 4)
     got = plan.apply_h_host(psi)
     assert plan.last_launches() == 8 * 4
     ref = gpu_apply(plan, psi)
@@ -495,6 +549,7 @@ def test_multik_scratch_maxima_on_different_kpoints():
     path needs max_k t1 + max_k t2 per band and k-point, more than max_k (t1 + t2).  Run it in an exactly sized caller
     workspace with guard regions on both sides; the guards must stay untouched and the result must match the oracle."""
     cfg, plan, sph = _setup("anisok3")
+    plan.set_option("fft_path", 4)
     geo = []
     n1, n2, n3 = cfg["ngfft"]
     for kg, ig, kin in sph:

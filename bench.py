@@ -77,8 +77,14 @@ class ClockSampler:
 
     def start(self):
         if self.nv:
+            try:    # the first NVML query of a process can take seconds and would stall the first timed launches of a sub-ms cell
+                self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)
+                self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+            except Exception:
+                pass
             self._t = threading.Thread(target=self._run, daemon=True)
             self._t.start()
+            time.sleep(0.25)
 
     def stop(self):
         self._stop.set()

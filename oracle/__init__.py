@@ -294,6 +294,113 @@ def chebyshev_filter(cfg, ik, kg, igfft, kin, psi, degree, center, halfwidth, me
     return t_cur
 
 
+# ---------------------------------------------------------------- NEXT row 4: Gamma-point real-symmetry storage
+# PAPER.md :407 ("time-reversal symmetry ... real-valued wave functions at the Gamma point"), SURVEY.md 8(f) 4.
+# At k = 0 a psi(r) that is real has c(-G) = conj(c(G)), so only one of every pair +-G is stored (reading 26):
+#   kept:  m3 > 0, or m3 = 0 and m2 > 0, or m3 = m2 = 0 and m1 >= 0   (in the order of the full list: ascending box index)
+#   c(0) is real: the imaginary part of the stored c(0) is ignored on input and returned as 0.
+# The operator in this storage is, by definition, the full operator applied to the symmetric vector and restricted again.
+# It maps symmetric vectors to symmetric vectors only if H commutes with time reversal: V real (always) and, with
+# the projector convention of reading 6 (no (-i)^l factor: p(-G) = (-1)^l conj(p(G))), D_ij = 0 whenever l_i + l_j is odd.
+def gamma_half(kg):
+    """(ih, ineg): positions in the full plane-wave list of the kept G and of their partners -G."""
+    kg = np.asarray(kg, np.int64)
+    keep = (kg[:, 2] > 0) | ((kg[:, 2] == 0) & (kg[:, 1] > 0)) | ((kg[:, 2] == 0) & (kg[:, 1] == 0) & (kg[:, 0] >= 0))
+    ih = np.nonzero(keep)[0]
+    pos = {tuple(m): i for i, m in enumerate(kg.tolist())}
+    try:
+        ineg = np.array([pos[(-m[0], -m[1], -m[2])] for m in kg[ih].tolist()], np.int64)
+    except KeyError:
+        raise ValueError("Gamma storage needs a sphere that holds -G for every G (k = 0, no unpaired Nyquist index)")
+    return ih, ineg
+
+
+def gamma_expand(kg, c_half):
+    """c_half [nband][>= nhalf] -> the symmetric full vector [nband][npw]: c(G) = c_half, c(-G) = conj(c_half), c(0) real."""
+    ih, ineg = gamma_half(kg)
+    c_half = np.atleast_2d(np.asarray(c_half, np.complex128))
+    full = np.zeros((c_half.shape[0], len(kg)), np.complex128)
+    full[:, ineg] = np.conj(c_half[:, :len(ih)])
+    full[:, ih] = c_half[:, :len(ih)]
+    self_conj = ih[ih == ineg]                       # G = 0 (its own partner)
+    full[:, self_conj] = full[:, self_conj].real
+    return full
+
+
+def gamma_dot(a_half, b_half, nhalf):
+    """<a|b> of the two symmetric full vectors, from the stored halves: 2 Re sum_{G != 0, kept} conj(a) b + a(0) b(0)
+    with the real parts of the stored a(0), b(0) (G = 0 is stored first: it has the smallest box index)."""
+    a = np.asarray(a_half, np.complex128)[..., :nhalf]; b = np.asarray(b_half, np.complex128)[..., :nhalf]
+    return 2.0 * np.sum((np.conj(a[..., 1:]) * b[..., 1:]).real, axis=-1) + a[..., 0].real * b[..., 0].real
+
+
+def apply_h_gamma(cfg, kg, igfft, kin, psi_half, method=2, terms=ALL, vloc=None, dij=None, sym_tol=1e-12):
+    """H psi in Gamma storage: psi_half [nband][ld >= nhalf] -> [nband][ld] (columns >= nhalf returned as 0).
+    The definition: expand to the symmetric full vector, apply the full-sphere operator (apply_h), check that the
+    result is symmetric (else H does not commute with time reversal and the storage is not closed), restrict."""
+    if np.any(np.asarray(cfg["kpt"][0], float) != 0.0):
+        raise ValueError("Gamma storage needs k = 0")
+    ih, ineg = gamma_half(kg)
+    psi_half = np.atleast_2d(np.asarray(psi_half, np.complex128))
+    full = gamma_expand(kg, psi_half)
+    out = apply_h(cfg, 0, kg, igfft, kin, full, method=method, terms=terms, vloc=vloc, dij=dij)
+    asym = np.max(np.abs(out[:, ineg] - np.conj(out[:, ih]))) if len(ih) else 0.0
+    if asym > sym_tol * max(1.0, np.max(np.abs(out))):
+        raise ValueError("H does not commute with time reversal (D_ij couples projectors of different l-parity?): "
+                         "asymmetry %.3e" % asym)
+    res = np.zeros_like(psi_half)
+    res[:, :len(ih)] = out[:, ih]
+    res[:, 0] = res[:, 0].real          # G = 0: the symmetric result is real there (rounding residue dropped)
+    return res
+
+
+# ---------------------------------------------------------------- NEXT row 4: two-component spinors
+# PAPER.md :448 ("all types of magnetism": non-collinear magnetism, spin-orbit coupling), SURVEY.md 8(f) 4; DESIGN.md
+# reading 27.  psi = (psi_up, psi_dn), each a plane-wave vector on the same sphere.
+#   H = kin (x) 1  +  FFT^-1[ V^{ss'}(r) FFT[psi_s'] ]  +  sum_a sum_ij sum_ss' |p_a,i> D^{a,ss'}_ij <p_a,j|
+# V^{ss'}(r) is a Hermitian 2x2 matrix per grid point, given as four real fields v4 = (V_upup, V_dndn, Re V_updn,
+# Im V_updn), V_dnup = conj(V_updn); D^{a,ss'}_ij is complex, [natom][2][2][lm][lm], Hermitian in ((s,i),(s',j)).
+def apply_h_spinor(cfg, ik, kg, igfft, kin, psi, v4, dspin, method=2, terms=ALL):
+    """psi [nband][2][ld >= npw] -> H psi, same shape; every step is the definition written out with the oracle's own
+    scatter / DFT (g2r, dft3d), the materialised projector table (projector_table) and numpy contractions."""
+    psi = np.ascontiguousarray(psi, np.complex128)
+    nb, two, ld = psi.shape
+    assert two == 2
+    npw = len(kg)
+    n1, n2, n3 = [int(v) for v in cfg["ngfft"]]
+    N = n1 * n2 * n3
+    out = np.zeros_like(psi)
+    v4 = np.asarray(v4, float)
+    vud = v4[2] + 1j * v4[3]
+    if terms & KIN:
+        out[:, :, :npw] += np.asarray(kin, float)[None, None, :] * psi[:, :, :npw]
+    if terms & LOC:
+        ig = np.asarray(igfft, np.int64)
+        for b in range(nb):
+            up = g2r(cfg["ngfft"], igfft, psi[b, 0, :npw], method)
+            dn = g2r(cfg["ngfft"], igfft, psi[b, 1, :npw], method)
+            phi_up = v4[0] * up + vud * dn
+            phi_dn = np.conj(vud) * up + v4[1] * dn
+            out[b, 0, :npw] += dft3d(phi_up, -1, method).reshape(-1)[ig] / N
+            out[b, 1, :npw] += dft3d(phi_dn, -1, method).reshape(-1)[ig] / N
+    if (terms & NL) and cfg["nproj"] > 0:
+        P = projector_table(cfg, ik, kg)                                    # [nproj][npw]
+        dspin = np.asarray(dspin, np.complex128)
+        first = np.concatenate([[0], np.cumsum([cfg["types"][t]["nlmn"] for t in cfg["typat"]])])
+        for b in range(nb):
+            cp = np.stack([P.conj() @ psi[b, s, :npw] for s in range(2)])   # <p|psi_s>, [2][nproj]
+            cq = np.zeros_like(cp)
+            for a in range(cfg["natom"]):
+                lo, hi = first[a], first[a + 1]
+                nl = hi - lo
+                for s in range(2):
+                    for s2 in range(2):
+                        cq[s, lo:hi] += dspin[a, s, s2, :nl, :nl] @ cp[s2, lo:hi]
+            for s in range(2):
+                out[b, s, :npw] += P.T @ cq[s]
+    return out
+
+
 def dense_h(cfg, ik, kg, kin, terms=ALL, vloc=None, dij=None):
     """T0: explicit H[npw][npw] complex128 in the plane-wave basis."""
     P = _Proj(cfg, ik); kg = _i32(kg); kin = _f64(kin)

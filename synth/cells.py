@@ -276,3 +276,51 @@ def gen_psi_torch(cfg, kin_list, device, nband=None):
             n0, n1 = rng.torch_normals_pair(cfg["seed"], STREAM_PSI, idx)
             psi[ik, b0:b1, :npw] = torch.complex(n0 * env, n1 * env)
     return psi
+
+
+# ----------------------------------------------------------------------------
+# inputs of the NEXT row 4 variants: Gamma-point real-symmetry storage, two-component spinors
+# ----------------------------------------------------------------------------
+STREAM_BFIELD, STREAM_DSPIN = 4, 5
+
+
+def projector_l(cfg):
+    """Angular momentum l of every projector row of the table (atoms in order, i = 0 .. nlmn-1)."""
+    return np.concatenate([np.asarray(cfg["types"][t]["l"], np.int64) for t in cfg["typat"]])
+
+
+def gamma_dij(cfg):
+    """D_ij of the cell with the entries that couple projectors of different l-parity set to zero: with the projector
+    convention of DESIGN.md reading 6 (no (-i)^l factor) those are the entries that break time-reversal symmetry, so a
+    real-in-r-space psi stays real under H only without them (reading 26)."""
+    d = np.array(cfg["dij"], float)
+    for a in range(cfg["natom"]):
+        l = np.asarray(cfg["types"][cfg["typat"][a]]["l"], np.int64)
+        nl = len(l)
+        odd = ((l[:, None] + l[None, :]) % 2) == 1
+        d[a, :nl, :nl][odd] = 0.0
+    return d
+
+
+def spinor_inputs(cfg):
+    """(v4, dspin) for the two-component variant (reading 27):
+    v4 [4][n3][n2][n1] = V_upup, V_dndn, Re V_updn, Im V_updn with V = V_loc + B.sigma for a smooth seeded field B(r)
+    (so V_upup = V + Bz, V_dndn = V - Bz, V_updn = Bx - i By); dspin [natom][2][2][lm][lm] complex, Hermitian in the
+    combined index (sigma i), (sigma' j): delta_ss' D_ij plus a seeded Hermitian perturbation of relative size 0.3."""
+    V = np.asarray(cfg["vloc"], float)
+    B = [_vloc_noise(cfg["rprimd"], cfg["ngfft"], 0.5 * cfg["vloc_params"][2], cfg["seed"] + 7919 * (c + 1)) for c in range(3)]
+    v4 = np.ascontiguousarray(np.stack([V + B[2], V - B[2], B[0], -B[1]]))
+    natom, lm = cfg["natom"], cfg["nlmn_max"]
+    n = 2 * lm
+    idx = np.arange(natom * n * n, dtype=np.uint64).reshape(natom, n, n)
+    z = 0.15 * (rng.normals(cfg["seed"], STREAM_DSPIN, idx, 0) + 1j * rng.normals(cfg["seed"], STREAM_DSPIN, idx, 1))
+    dspin = np.zeros((natom, 2, 2, lm, lm), np.complex128)
+    for a in range(natom):
+        nl = cfg["types"][cfg["typat"][a]]["nlmn"]
+        h = z[a] + z[a].conj().T                                 # Hermitian [2 lm][2 lm], index = sigma * lm + i
+        h = h.reshape(2, lm, 2, lm).transpose(0, 2, 1, 3).copy()   # [s][s'][i][j]
+        h[:, :, nl:, :] = 0.0; h[:, :, :, nl:] = 0.0
+        dspin[a] = h
+        for s in range(2):
+            dspin[a, s, s] += cfg["dij"][a]
+    return v4, dspin

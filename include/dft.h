@@ -198,6 +198,33 @@ int dft_set_vector_potential(dft_plan *p, const double *a_cart);
 int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, int32_t degree, double center,
                          double halfwidth, void *stream);
 
+/* Gamma-point real-symmetry storage (PAPER.md :407 "time-reversal symmetry"; reading 26).
+ * Enabled by dft_plan_set_option(p, "gamma_real", 1) on a plan with ONE k-point k = (0,0,0) whose sphere holds -G for
+ * every G; DFT_ERR_UNSUPPORTED otherwise, DFT_ERR_INVALID_ARG if D_ij (now or in a later dft_set_dij) couples
+ * projectors of different l-parity (H would not commute with time reversal).  A band whose psi(r) is real has
+ * c(-G) = conj(c(G)); only the plane waves with m3 > 0, or m3 = 0 and m2 > 0, or m3 = m2 = 0 and m1 >= 0 are stored, in the
+ * order of the full list (ascending box index; G = 0 first), nhalf = (npw + 1)/2 of them.
+ * dft_plan_get_kg_gamma: HOST outputs like dft_plan_get_kg for the stored half (any pointer may be NULL).
+ * dft_apply_h_gamma: psi, hpsi DEVICE [nband][nhalf] complex128, 16-byte aligned, not aliased; hpsi = restriction of
+ * H applied to the symmetric vector (Im psi(0) is ignored, Im hpsi(0) = 0).  Two bands share one complex FFT round
+ * trip and both projector GEMMs are REAL GEMMs on the half sphere.  Honours option "terms" (bits 0-2); enqueues on
+ * `stream` without host synchronisation (scratch is allocated at the first call of a given size).              */
+int dft_plan_get_kg_gamma(const dft_plan *p, int32_t *nhalf, int32_t *kg, int32_t *igfft, double *kin);
+int dft_apply_h_gamma(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);
+
+/* Two-component spinors (PAPER.md :448 "all types of magnetism": non-collinear magnetism, spin-orbit coupling;
+ * SURVEY.md 8(f) row 4; reading 27).  psi = (psi_up, psi_dn): DEVICE [nkpt][nband][2][mpw] complex128.
+ *   H = kin (x) 1 + FFT^-1[ V^{ss'}(r) FFT[psi_s'] ] + sum_a sum_ij sum_ss' |p_a,i> D^{a,ss'}_ij <p_a,j|
+ * dft_set_vloc_spinor: v4 DEVICE [4][n3][n2][n1] doubles = V_upup, V_dndn, Re V_updn, Im V_updn (V_dnup = conj V_updn),
+ * copied on `stream` (as Pauli components V0, Vx, Vy, Vz pre-scaled by 1/N).
+ * dft_set_dij_spinor: dspin HOST [natom][2][2][lmax][lmax] complex128 (re, im interleaved), Hermitian in
+ * ((s,i),(s',j)); NULL returns to the scalar D_ij of dft_set_dij on both components.  Synchronises the device.
+ * dft_apply_h_spinor: rules of dft_apply_h; DFT_ERR_NOT_READY before dft_set_vloc_spinor while the local term is on.
+ * The local term is four scalar local applications (V0 psi + sum_mu V_mu sigma_mu psi), the GEMMs see 2 nband bands. */
+int dft_set_vloc_spinor(dft_plan *p, const double *v4_dev, void *stream);
+int dft_set_dij_spinor(dft_plan *p, const double *dspin_host);
+int dft_apply_h_spinor(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);
+
 /* Same, with HOST psi/hpsi (pageable or pinned): copies psi to the device in band blocks, applies
  * H, copies the result back, and returns after the last copy has completed.                      */
 int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int32_t nband);
@@ -210,7 +237,7 @@ int64_t dft_plan_last_launches(const dft_plan *p);
  * later applies is bracketed by CUDA events on the launching stream; dft_plan_phase_ms then
  * returns (after synchronising) the accumulated milliseconds of phase i and resets it.
  * Phases: 0 fft_A(scatter) 1 fft_B 2 fft_C*V*C^-1 3 fft_B^-1 4 fft_A^-1(gather) 5 gemm1 6 dij
- * 7 gemm2(+kinetic).                                                                             */
+ * 7 gemm2(+kinetic) 8 fused small-box local term 9 pack/unpack (Gamma storage) and sigma products (spinors). */
 int dft_plan_set_timing(dft_plan *p, int32_t on);
 int dft_plan_phase_ms(dft_plan *p, int32_t phase, double *ms, int64_t *launches);
 

@@ -29,13 +29,14 @@ DFT_ERR_NOT_READY = -6
 DFT_ERR_UNSUPPORTED = -7
 
 PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather", "gemm1", "dij", "gemm2_kinetic",
-          "fft_small_fused")
+          "fft_small_fused", "pack_unpack")
 
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_workspace_bytes", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_apply_hs", "dft_get_cprj", "dft_chebyshev_filter",
            "dft_set_vector_potential", "dft_accumulate_density", "dft_accumulate_tau",
-           "dft_set_vtau",
+           "dft_set_vtau", "dft_plan_get_kg_gamma", "dft_apply_h_gamma", "dft_set_vloc_spinor", "dft_set_dij_spinor",
+           "dft_apply_h_spinor",
            "dft_set_vloc", "dft_set_workspace", "dft_plan_set_option", "dft_apply_h", "dft_apply_h_host",
            "dft_plan_last_launches", "dft_plan_set_timing", "dft_plan_phase_ms", "dft_plan_destroy", "dft_last_error")
 
@@ -94,6 +95,11 @@ def lib():
     L.dft_apply_s.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_apply_hs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_get_cprj.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    L.dft_plan_get_kg_gamma.argtypes = [C.c_void_p, _ip, _ip, _ip, _dp]
+    L.dft_apply_h_gamma.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    L.dft_set_vloc_spinor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.dft_set_dij_spinor.argtypes = [C.c_void_p, _dp]
+    L.dft_apply_h_spinor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_plan_set_timing.argtypes = [C.c_void_p, C.c_int32]
     L.dft_plan_phase_ms.argtypes = [C.c_void_p, C.c_int32, _dp, C.POINTER(C.c_int64)]
     L.dft_plan_destroy.argtypes = [C.c_void_p]
@@ -241,6 +247,34 @@ def dft_chebyshev_filter(plan, psi_dev_ptr, work_dev_ptr, nband, degree, center,
     _check(lib().dft_chebyshev_filter(plan, psi_dev_ptr, work_dev_ptr, nband, degree, center, halfwidth, stream))
 
 
+def dft_plan_get_kg_gamma(plan):
+    n = C.c_int32(0)
+    _check(lib().dft_plan_get_kg_gamma(plan, C.byref(n), None, None, None))
+    kg = np.zeros((n.value, 3), np.int32); ig = np.zeros(n.value, np.int32); kin = np.zeros(n.value)
+    _check(lib().dft_plan_get_kg_gamma(plan, C.byref(n), _i(kg), _i(ig), _d(kin)))
+    return kg, ig, kin
+
+
+def dft_apply_h_gamma(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream=0):
+    _check(lib().dft_apply_h_gamma(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream))
+
+
+def dft_set_vloc_spinor(plan, v4_dev_ptr, stream=0):
+    _check(lib().dft_set_vloc_spinor(plan, v4_dev_ptr, stream))
+
+
+def dft_set_dij_spinor(plan, dspin):
+    if dspin is None:
+        _check(lib().dft_set_dij_spinor(plan, None))
+        return
+    d = np.ascontiguousarray(dspin, np.complex128)
+    _check(lib().dft_set_dij_spinor(plan, _d(d.view(np.float64))))
+
+
+def dft_apply_h_spinor(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream=0):
+    _check(lib().dft_apply_h_spinor(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream))
+
+
 def dft_apply_h_host(plan, psi_host_ptr, hpsi_host_ptr, nband):
     _check(lib().dft_apply_h_host(plan, psi_host_ptr, hpsi_host_ptr, nband))
 
@@ -324,6 +358,40 @@ class Plan:
             hpsi = torch.empty_like(psi)
         assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.is_contiguous() and hpsi.shape == psi.shape
         dft_apply_h(self.h, psi.data_ptr(), hpsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
+        return hpsi
+
+    def get_kg_gamma(self):
+        """(kg, igfft, kin) of the stored half sphere (option gamma_real = 1)."""
+        return dft_plan_get_kg_gamma(self.h)
+
+    def apply_h_gamma(self, psi, hpsi=None):
+        """Gamma storage: psi torch complex128 CUDA tensor [nband][nhalf]."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.dim() == 2
+        if hpsi is None:
+            hpsi = torch.empty_like(psi)
+        assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.is_contiguous() and hpsi.shape == psi.shape
+        dft_apply_h_gamma(self.h, psi.data_ptr(), hpsi.data_ptr(), psi.shape[0], torch.cuda.current_stream().cuda_stream)
+        return hpsi
+
+    def set_vloc_spinor(self, v4):
+        """v4: torch float64 CUDA tensor [4][n3][n2][n1] = V_upup, V_dndn, Re V_updn, Im V_updn."""
+        import torch
+        assert v4.is_cuda and v4.dtype == torch.float64 and v4.is_contiguous() and v4.numel() == 4 * int(np.prod(self.ngfft))
+        dft_set_vloc_spinor(self.h, v4.data_ptr(), torch.cuda.current_stream().cuda_stream)
+
+    def set_dij_spinor(self, dspin):
+        dft_set_dij_spinor(self.h, dspin)
+
+    def apply_h_spinor(self, psi, hpsi=None):
+        """psi: torch complex128 CUDA tensor [nkpt][nband][2][mpw] (or [nband][2][mpw] when nkpt = 1)."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.shape[-1] == self.mpw and psi.shape[-2] == 2
+        nband = psi.numel() // (self.nkpt * 2 * self.mpw) if self.mpw else 0
+        if hpsi is None:
+            hpsi = torch.empty_like(psi)
+        assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.is_contiguous() and hpsi.shape == psi.shape
+        dft_apply_h_spinor(self.h, psi.data_ptr(), hpsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
         return hpsi
 
     def set_sij(self, sij):

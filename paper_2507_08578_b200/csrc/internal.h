@@ -69,8 +69,28 @@ struct KPoint {
   std::vector<double> h_kin;
 };
 
-// timed kernel groups: 0-4 the five FFT passes, 5 GEMM-1, 6 D_ij, 7 GEMM-2, 8 the fused small-box local term (fft_small.cu)
-constexpr int NPHASE = 9;
+// Gamma-point real-symmetry storage (gamma.cu; reading 26): the half sphere, its maps to the full sphere and the
+// projector table on it (rows of odd l multiplied by i, so that every projection is real)
+struct GammaData {
+  int nh = 0;                          // stored plane waves = (npw + 1) / 2
+  int32_t *d_kg = nullptr;             // [nh][3]
+  double *d_kin = nullptr;             // [nh]
+  int32_t *d_h2f = nullptr;            // [nh]  position of +G in the full list
+  int32_t *d_h2fneg = nullptr;         // [nh]  position of -G in the full list
+  int32_t *d_f2h = nullptr;            // [npw] +(h + 1): full entry is stored entry h; -(h + 1): its conjugate
+  double *d_ptab = nullptr;            // [nproj][nh] complex
+  double *d_p0 = nullptr;              // [nproj] Re of the table's G = 0 column (the term counted twice by 2 sum_half)
+  int32_t *d_rowpar = nullptr;         // [natom][lmax] l mod 2 of every projector (D_ij couples equal parity only)
+  int32_t *d_npw = nullptr;            // [1] = nh
+  const double **d_kinptr = nullptr;   // [1] -> d_kin
+  double *d_pack = nullptr; int64_t pack_bytes = 0;   // packed band pairs in / out, [2][pairs][mpw] complex
+  std::vector<int32_t> h_kg, h_igfft;
+  std::vector<double> h_kin;
+};
+
+// timed kernel groups: 0-4 the five FFT passes, 5 GEMM-1, 6 D_ij, 7 GEMM-2, 8 the fused small-box local term (fft_small.cu),
+// 9 pack / unpack of band pairs (Gamma storage) and the spin-matrix products of the spinor path
+constexpr int NPHASE = 10;
 struct PhaseTimer {
   bool on = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[NPHASE];
@@ -152,6 +172,12 @@ struct dft_plan {
   int64_t last_launches = 0;
   bool nl_attr_done = false;   // cudaFuncSetAttribute of the GEMM kernels done on this plan's device
   dftb200::PhaseTimer timer;
+  dftb200::GammaData *gam = nullptr;   // built by option gamma_real = 1
+  // two-component spinors (spinor.cu): Pauli components of the local potential, spin-dependent D
+  double *d_vpauli = nullptr;          // [4][n3][n2][n1]: V0, Vx, Vy, Vz, each pre-scaled by 1/N
+  double *d_dspin = nullptr;           // [natom][2][2][lmax][lmax] complex
+  double *d_spin_tmp = nullptr; int64_t spin_tmp_bytes = 0;   // sigma_mu psi, [nband][2][mpw] complex
+  bool vspin_set = false, dspin_set = false, gam_attr_done = false;
 };
 
 namespace dftb200 {
@@ -213,7 +239,27 @@ int fft_small_apply(dft_plan *p, int ik0, int nk, const double *psi, double *hps
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi
 int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin,
                    bool with_nl, cudaStream_t st, const double *dmat = nullptr, const double *const *diag = nullptr,
-                   double *cprj_out = nullptr, const Recurrence *rec = nullptr, double *spsi = nullptr);
+                   double *cprj_out = nullptr, const Recurrence *rec = nullptr, double *spsi = nullptr,
+                   const double *dspin = nullptr);
+
+// Gamma storage: the same three steps as real GEMMs on the half sphere (psi, hpsi: [nband][nh] complex)
+int nonlocal_apply_gamma(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
+                         cudaStream_t st, const Recurrence *rec);
+// spinors: psi [nband][2][mpw]; dspin = null applies the plan's scalar D_ij to both components
+int nonlocal_apply_spinor(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
+                          cudaStream_t st);
+
+// --- plan.cu: the local term of all k-points for [nkpt][nband][mpw] blocks (hpsi = V_loc psi, or += with extra->accumulate)
+int local_term(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStream_t st, const FftExtra *extra = nullptr);
+
+// --- gamma.cu / spinor.cu ------------------------------------------------------------------------
+int gamma_build(dft_plan *p);
+void gamma_free(dft_plan *p);
+int gamma_check_dij(const dft_plan *p, const double *dij_host);
+int gamma_apply(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStream_t st, const Recurrence *rec = nullptr);
+int spinor_apply(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStream_t st);
+int spinor_set_vloc(dft_plan *p, const double *v4, cudaStream_t st);
+int build_projector_table_on(dft_plan *p, const int32_t *d_kg, int npw, int mpw, const double k[3], double *d_out, int rot_odd);
 
 // --- timing hooks ------------------------------------------------------------------------------
 void phase_begin(dft_plan *p, int phase, cudaStream_t st);

@@ -64,7 +64,10 @@ struct Gemm2Params {
 // The MMA main loop shared by both GEMMs.  MODE 1: acc += conj(A) B (GEMM-1); MODE 2: acc += A B.
 // As/Bs: one stage; A rows are addressed as a_row0 + mb*a_mb_stride bytes (+ row-in-block handled
 // by the caller-provided offsets).
-template <int MODE>
+// REAL (Gamma-point storage, gamma.cu): MODE 1 keeps only Re(conj(A) B) = A_r B_r + A_i B_i, a REAL GEMM over the
+// interleaved (re, im) doubles; MODE 2 takes B as real (its imaginary halves are zero): Re += A_r B_r, Im += A_i B_r.
+// Either way two of the four DMMA sets remain.
+template <int MODE, bool REAL = false>
 __device__ __forceinline__ void mma_stage(const unsigned char *As, const unsigned char *Bs, int wm, int wn, int lane,
                                           double (&cre)[4][4][2], double (&cim)[4][4][2]) {
   const int i = lane >> 2, j = lane & 3;
@@ -99,6 +102,16 @@ __device__ __forceinline__ void mma_stage(const unsigned char *As, const unsigne
     for (int mb = 0; mb < 4; mb++)
 #pragma unroll
       for (int nb = 0; nb < 4; nb++) dmma(cre[mb][nb][0], cre[mb][nb][1], ar[mb], br[nb]);
+    if (REAL) {
+#pragma unroll
+      for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+        for (int nb = 0; nb < 4; nb++) {
+          if (MODE == 1) dmma(cre[mb][nb][0], cre[mb][nb][1], ai[mb], bi[nb]);
+          else dmma(cim[mb][nb][0], cim[mb][nb][1], ai[mb], br[nb]);
+        }
+      continue;
+    }
 #pragma unroll
     for (int mb = 0; mb < 4; mb++)
 #pragma unroll
@@ -152,6 +165,7 @@ __device__ __forceinline__ Pipe pipe_setup(unsigned char *smem_raw) {
 
 // ---------------------------------------------------------------- GEMM-1: projection (split-K partials)
 // grid: (tiles_m*tiles_n, nsplit, nkpt)
+template <bool REAL>
 __global__ void __launch_bounds__(NL_THREADS, 1)
 gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapPsi, Gemm1Params Q) {
   extern __shared__ unsigned char smem_raw[];
@@ -184,12 +198,13 @@ gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
     int s = it % NL_STAGES;
     mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
     const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
-    mma_stage<1>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
+    mma_stage<1, REAL>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
     __syncwarp();
     if (lane == 0) mbar_arrive(&P.empty[s]);
   }
-  // partial[ik][split][p][b] complex; thread holds rows p = lane/4, bands 2*(lane%4)+{0,1} of each 8x8 block
+  // partial[ik][split][p][b] complex (REAL: real); thread holds rows p = lane/4, bands 2*(lane%4)+{0,1} of each 8x8 block
   double2 *out = Q.part + ((size_t)(ik * Q.nsplit + split) * Q.nproj) * Q.nband;
+  double *outr = reinterpret_cast<double *>(Q.part) + ((size_t)(ik * Q.nsplit + split) * Q.nproj) * Q.nband;
   const int i = lane >> 2, j = lane & 3;
 #pragma unroll
   for (int mb = 0; mb < 4; mb++) {
@@ -198,9 +213,15 @@ gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
 #pragma unroll
     for (int nb = 0; nb < 4; nb++) {
       int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j;
-      double2 *d = out + (size_t)pr * Q.nband + b;
-      if (b < Q.nband) d[0] = make_double2(cre[mb][nb][0], cim[mb][nb][0]);
-      if (b + 1 < Q.nband) d[1] = make_double2(cre[mb][nb][1], cim[mb][nb][1]);
+      if (REAL) {
+        double *d = outr + (size_t)pr * Q.nband + b;
+        if (b < Q.nband) d[0] = cre[mb][nb][0];
+        if (b + 1 < Q.nband) d[1] = cre[mb][nb][1];
+      } else {
+        double2 *d = out + (size_t)pr * Q.nband + b;
+        if (b < Q.nband) d[0] = make_double2(cre[mb][nb][0], cim[mb][nb][0]);
+        if (b + 1 < Q.nband) d[1] = make_double2(cre[mb][nb][1], cim[mb][nb][1]);
+      }
     }
   }
 }
@@ -236,8 +257,73 @@ __global__ void dij_kernel(const double2 *__restrict__ part, double2 *__restrict
   }
 }
 
+// Gamma storage (reading 26): the real GEMM-1 gives S_j = sum_half (Pt_r psi_r + Pt_i psi_i) with Pt = i^(l odd) p;
+// the projection of the symmetric vector is <p_j|psi> = i^(l_j odd) r_j with r_j = 2 S_j - Pt_r,j(0) Re psi(0) (the G = 0 term
+// is its own partner).  D couples projectors of equal l-parity only, so c'_i = i^(l_i odd) sum_j D_ij r_j, stored as the
+// real number sum_j D_ij r_j (imaginary half 0) for the real GEMM-2 on the same rotated table.
+__global__ void dij_gamma_kernel(const double *__restrict__ part, double2 *__restrict__ cpr, const double *__restrict__ dij,
+                                 const int32_t *__restrict__ typat, const int32_t *__restrict__ nlmn,
+                                 const int32_t *__restrict__ atom_first, const int32_t *__restrict__ rowpar,
+                                 const double *__restrict__ p0, const double2 *__restrict__ psi, int mpw, int lmax, int nproj,
+                                 int nband, int nsplit) {
+  int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+  if (b >= nband) return;
+  int nl = nlmn[typat[a]], first = atom_first[a];
+  const double c0 = psi[(size_t)b * mpw].x;
+  double r[DIJ_MAXL];
+  for (int jj = 0; jj < nl; jj++) {
+    double sr = 0.0;
+    for (int s = 0; s < nsplit; s++) sr += part[((size_t)s * nproj + first + jj) * nband + b];
+    r[jj] = 2.0 * sr - p0[first + jj] * c0;
+  }
+  double2 *dst = cpr + (size_t)b * nproj + first;
+  const double *D = dij + (size_t)a * lmax * lmax;
+  const int32_t *par = rowpar + (size_t)a * lmax;
+  for (int ii = 0; ii < nl; ii++) {
+    double sr = 0.0;
+    for (int jj = 0; jj < nl; jj++)
+      if (par[ii] == par[jj]) sr += D[ii * lmax + jj] * r[jj];
+    dst[ii] = make_double2(sr, 0.0);
+  }
+}
+
+// Spinors (reading 27): rows 2 b + s of the projections are the two components of band b;
+// c'[2b + s][a,i] = sum_s' sum_j D^{a,s s'}_ij <p_a,j|psi_{b,s'}>, D complex [natom][2][2][lmax][lmax]
+__global__ void dij_spinor_kernel(const double2 *__restrict__ part, double2 *__restrict__ cpr, const double2 *__restrict__ dspin,
+                                  const int32_t *__restrict__ typat, const int32_t *__restrict__ nlmn,
+                                  const int32_t *__restrict__ atom_first, int lmax, int nproj, int nband2, int nsplit) {
+  int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y, ik = blockIdx.z;
+  if (2 * b >= nband2) return;
+  int nl = nlmn[typat[a]], first = atom_first[a];
+  double2 c[2][DIJ_MAXL];
+  for (int sp = 0; sp < 2; sp++)
+    for (int jj = 0; jj < nl; jj++) {
+      double sr = 0.0, si = 0.0;
+      for (int s = 0; s < nsplit; s++) {
+        double2 v = part[((size_t)(ik * nsplit + s) * nproj + first + jj) * nband2 + 2 * b + sp];
+        sr += v.x; si += v.y;
+      }
+      c[sp][jj] = make_double2(sr, si);
+    }
+  for (int sp = 0; sp < 2; sp++) {
+    double2 *dst = cpr + ((size_t)ik * nband2 + 2 * b + sp) * nproj + first;
+    for (int ii = 0; ii < nl; ii++) {
+      double sr = 0.0, si = 0.0;
+      for (int s2 = 0; s2 < 2; s2++) {
+        const double2 *D = dspin + (((size_t)a * 2 + sp) * 2 + s2) * lmax * lmax + (size_t)ii * lmax;
+        for (int jj = 0; jj < nl; jj++) {
+          const double2 d = D[jj], v = c[s2][jj];
+          sr += d.x * v.x - d.y * v.y; si += d.x * v.y + d.y * v.x;
+        }
+      }
+      dst[ii] = make_double2(sr, si);
+    }
+  }
+}
+
 // ---------------------------------------------------------------- GEMM-2: back-projection + kinetic epilogue
 // grid: (tiles_n * tiles_m, 1, nkpt), band tiles fastest so that concurrent CTAs share a slab of P in L2
+template <bool REAL>
 __global__ void __launch_bounds__(NL_THREADS, 1)
 gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapC, Gemm2Params Q) {
   extern __shared__ unsigned char smem_raw[];
@@ -269,7 +355,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
     int s = it % NL_STAGES;
     mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
     const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
-    mma_stage<2>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
+    mma_stage<2, REAL>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
     __syncwarp();
     if (lane == 0) mbar_arrive(&P.empty[s]);
   }
@@ -298,6 +384,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
           double2 y = psi[off], xp = Q.sx != 0.0 ? Q.xprev[(size_t)ik * Q.nband * Q.mpw + off] : make_double2(0.0, 0.0);
           r.x = Q.sh * r.x + Q.sy * y.x + Q.sx * xp.x; r.y = Q.sh * r.y + Q.sy * y.y + Q.sx * xp.y;
         }
+        if (REAL && g == 0) r.y = 0.0;     // Gamma storage: c(G = 0) is real (reading 26)
         hpsi[off] = r;
       }
     }
@@ -802,7 +889,7 @@ static int make_map_plain(dft_plan *p, CUtensorMap *m, const void *base, uint64_
 
 __global__ void kin_only_kernel(const double2 *__restrict__ psi, double2 *__restrict__ hpsi, const double *const *kin,
                                 const int32_t *npw, int nband, int mpw, int accumulate, int with_kin, int cheb, double sh,
-                                double sy, double sx, const double2 *__restrict__ xprev) {
+                                double sy, double sx, const double2 *__restrict__ xprev, int gamma = 0) {
   int ik = blockIdx.z, b = blockIdx.y;
   const double *k = kin[ik];
   int n = npw[ik];
@@ -815,6 +902,7 @@ __global__ void kin_only_kernel(const double2 *__restrict__ psi, double2 *__rest
       double2 y = psi[row + g], xp = sx != 0.0 ? xprev[row + g] : make_double2(0.0, 0.0);
       r.x = sh * r.x + sy * y.x + sx * xp.x; r.y = sh * r.y + sy * y.y + sx * xp.y;
     }
+    if (gamma && g == 0) r.y = 0.0;
     hpsi[row + g] = r;
   }
 }
@@ -840,14 +928,14 @@ static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
 // complex): if given, only GEMM-1 and the split-K reduction run and <p|psi> is written there.
 int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
                    cudaStream_t st, const double *dmat, const double *const *diag, double *cprj_out, const Recurrence *rec,
-                   double *spsi) {
+                   double *spsi, const double *dspin) {
   if (p->mpw == 0 || nband == 0) return DFT_OK;
   if (cprj_out && p->nproj == 0) return DFT_OK;
   if (p->nproj == 0) with_nl = false;
   if (!with_nl && !with_kin && accumulate && !rec) return DFT_OK;
   if (!p->nl_attr_done) {   // per plan (= per device), not per process
-    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
-    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_fac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FC_SMEM));
@@ -937,14 +1025,19 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     f1.blk_atom = p->d_blk_atom; f1.blk_frow = p->d_blk_frow; f1.blk_first = p->d_blk_first; f1.blk_nl = p->d_blk_nl; f1.part = q1.part;
     gemm1_fac_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), FC_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1, f1);
   } else if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
-  else gemm1_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  else gemm1_kernel<false><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   phase_end(p, 5, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   // ---- D_ij
   phase_begin(p, 6, st);
-  dij_kernel<<<dim3((nband + 127) / 128, p->natom, nkpt), 128, 0, st>>>(
-      q1.part, reinterpret_cast<double2 *>(cprj_out ? cprj_out : p->d_cprj), cprj_out ? nullptr : dmat, p->d_typat, p->d_nlmn,
-      p->d_atom_first, p->natom, p->lmax, nproj, nband, ns);
+  if (dspin && !cprj_out)
+    dij_spinor_kernel<<<dim3((nband / 2 + 127) / 128, p->natom, nkpt), 128, 0, st>>>(
+        q1.part, reinterpret_cast<double2 *>(p->d_cprj), reinterpret_cast<const double2 *>(dspin), p->d_typat, p->d_nlmn,
+        p->d_atom_first, p->lmax, nproj, nband, ns);
+  else
+    dij_kernel<<<dim3((nband + 127) / 128, p->natom, nkpt), 128, 0, st>>>(
+        q1.part, reinterpret_cast<double2 *>(cprj_out ? cprj_out : p->d_cprj), cprj_out ? nullptr : dmat, p->d_typat, p->d_nlmn,
+        p->d_atom_first, p->natom, p->lmax, nproj, nband, ns);
   phase_end(p, 6, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   if (cprj_out) return DFT_OK;
@@ -962,7 +1055,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_blk_atom,
                                                                                       p->d_blk_frow, p->d_blk_first, p->nfrow);
   } else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
-  else gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  else gemm2_kernel<false><<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   phase_end(p, 7, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   if (spsi) {
@@ -978,11 +1071,102 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     if (fac) gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_blk_atom,
                                                                                                p->d_blk_frow, p->d_blk_first, p->nfrow);
     else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
-    else gemm2_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+    else gemm2_kernel<false><<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
     phase_end(p, 7, st, 1);
     DFT_CUDA_CHECK(cudaGetLastError());
   }
   return DFT_OK;
+}
+
+// ---------------------------------------------------------------- Gamma storage: real GEMMs on the half sphere
+int nonlocal_apply_gamma(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
+                         cudaStream_t st, const Recurrence *rec) {
+  GammaData *G = p->gam;
+  if (!G || G->nh == 0 || nband == 0) return DFT_OK;
+  if (p->nproj == 0) with_nl = false;
+  if (!with_nl && !with_kin && accumulate && !rec) return DFT_OK;
+  if (!p->gam_attr_done) {
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    p->gam_attr_done = true;
+  }
+  const int mpw = G->nh, nproj = p->nproj;
+  const double2 *cpsi = reinterpret_cast<const double2 *>(psi);
+  double2 *chpsi = reinterpret_cast<double2 *>(hpsi);
+  if (!with_nl) {
+    dim3 grid((mpw + 255) / 256 < 64 ? (mpw + 255) / 256 : 64, nband, 1);
+    phase_begin(p, 7, st);
+    kin_only_kernel<<<grid, 256, 0, st>>>(cpsi, chpsi, G->d_kinptr, G->d_npw, nband, mpw, accumulate, with_kin, rec != nullptr,
+                                          rec ? rec->sh : 1.0, rec ? rec->sy : 0.0, rec ? rec->sx : 0.0,
+                                          rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr, 1);
+    phase_end(p, 7, st, 1);
+    DFT_CUDA_CHECK(cudaGetLastError());
+    return DFT_OK;
+  }
+  int rc;
+  Gemm1Params q1;
+  q1.nproj = nproj; q1.nband = nband; q1.nslab = (mpw + 7) / 8;
+  q1.tiles_m = (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
+  int ns = p->splitk > 0 ? p->splitk : choose_splitk(q1.tiles_m * q1.tiles_n, q1.nslab, p->sm_count, 1);
+  if (ns > q1.nslab) ns = q1.nslab;
+  q1.slabs_per_split = (q1.nslab + ns - 1) / ns;
+  ns = (q1.nslab + q1.slabs_per_split - 1) / q1.slabs_per_split;
+  q1.nsplit = ns;
+  int64_t need_part = (int64_t)ns * nproj * nband * 8, need_cprj = (int64_t)nband * nproj * 16;
+  if (need_part > p->part_bytes || !p->d_part) {
+    if (p->d_part) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_part); p->d_part = nullptr; }
+    if (cudaMalloc(&p->d_part, need_part) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes of split-K scratch", (long long)need_part); p->part_bytes = 0; return DFT_ERR_ALLOC; }
+    p->part_bytes = need_part;
+  }
+  if (need_cprj > p->cprj_bytes || !p->d_cprj) {
+    if (p->d_cprj) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_cprj); p->d_cprj = nullptr; }
+    if (cudaMalloc(&p->d_cprj, need_cprj) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes for cprj", (long long)need_cprj); p->cprj_bytes = 0; return DFT_ERR_ALLOC; }
+    p->cprj_bytes = need_cprj;
+  }
+  q1.part = reinterpret_cast<double2 *>(p->d_part);
+  CUtensorMap mapP1, mapPsi, mapP2, mapC;
+  const uint64_t rowb = (uint64_t)mpw * 16;
+  if ((rc = make_map(p, &mapP1, G->d_ptab, 2 * (uint64_t)mpw, nproj, 1, rowb, rowb * nproj, NL_BM))) return rc;
+  if ((rc = make_map(p, &mapPsi, psi, 2 * (uint64_t)mpw, nband, 1, rowb, rowb * nband, NL_BN))) return rc;
+  {
+    cuuint64_t dims[4] = {16, (cuuint64_t)nproj, ((cuuint64_t)mpw + 7) / 8, 1};
+    cuuint64_t strides[3] = {rowb, 128, rowb * nproj};
+    cuuint32_t box[4] = {16, 8, NL_BM / 8, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = ((EncodeFn)p->encode_fn)(&mapP2, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, G->d_ptab, dims, strides, box, estr,
+                                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (Gamma GEMM-2 P map) failed (%d)", (int)r); return DFT_ERR_CUDA; }
+  }
+  if ((rc = make_map(p, &mapC, p->d_cprj, 2 * (uint64_t)nproj, nband, 1, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * nband, NL_BN))) return rc;
+  phase_begin(p, 5, st);
+  gemm1_kernel<true><<<dim3(q1.tiles_m * q1.tiles_n, ns, 1), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  phase_end(p, 5, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  phase_begin(p, 6, st);
+  dij_gamma_kernel<<<dim3((nband + 127) / 128, p->natom, 1), 128, 0, st>>>(
+      p->d_part, reinterpret_cast<double2 *>(p->d_cprj), p->d_dij, p->d_typat, p->d_nlmn, p->d_atom_first, G->d_rowpar, G->d_p0,
+      cpsi, mpw, p->lmax, nproj, nband, ns);
+  phase_end(p, 6, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  Gemm2Params q2;
+  q2.nproj = nproj; q2.nband = nband; q2.mpw = mpw; q2.nslab = (nproj + 7) / 8;
+  q2.tiles_n = q1.tiles_n; q2.accumulate = accumulate; q2.with_kin = with_kin; q2.with_nl = 1;
+  q2.npw = G->d_npw; q2.kin = G->d_kinptr; q2.psi = cpsi; q2.hpsi = chpsi;
+  q2.cheb = rec != nullptr; q2.sh = rec ? rec->sh : 1.0; q2.sy = rec ? rec->sy : 0.0; q2.sx = rec ? rec->sx : 0.0;
+  q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr;
+  const int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
+  phase_begin(p, 7, st);
+  gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  phase_end(p, 7, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+int nonlocal_apply_spinor(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
+                          cudaStream_t st) {
+  return nonlocal_apply(p, psi, hpsi, 2 * nband, accumulate, with_kin, with_nl, st, nullptr, nullptr, nullptr, nullptr, nullptr,
+                        p->dspin_set ? p->d_dspin : nullptr);
 }
 
 }  // namespace dftb200

@@ -65,6 +65,8 @@ static void destroy_plan(dft_plan *p) {
   cudaFree(p->d_stab); cudaFree(p->d_fytab); cudaFree(p->d_vtau); cudaFree(p->d_qcart); cudaFree(p->d_qhalf); cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_geom_small); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
+  gamma_free(p);
+  cudaFree(p->d_vpauli); cudaFree(p->d_dspin); cudaFree(p->d_spin_tmp);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
   if (p->h2d_stream) cudaStreamDestroy(p->h2d_stream);
   if (p->d2h_stream) cudaStreamDestroy(p->d2h_stream);
@@ -290,6 +292,39 @@ static int ensure_qcart_ready(dft_plan *p) {
   return DFT_OK;
 }
 
+// hpsi = V_loc psi (extra: another potential, diagonal factors with k-stride 3 mpw, accumulation) for [nkpt][nband][mpw] blocks
+int local_term(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStream_t st, const FftExtra *extra) {
+  int rc;
+  const size_t band_stride = (size_t)p->mpw * 2;
+  const bool small = (p->fft_path == 0 || p->fft_path == 3) && fft_small_ok(p);
+  if (small)   // the box fits one SM's shared memory: the whole local term of all k-points and bands is ONE launch, no scratch
+    return fft_small_apply(p, 0, p->nkpt, psi, hpsi, nband, nband, st, extra);
+  int chunk; void *ws;
+  if (!extra && fft2_batch_ok(p) && (!p->ws_user || p->ws_user_bytes >= fft_ws_bytes_per_band_batched(p))) {
+    // small boxes, many k-points: every pass is one launch over all k-points (blockIdx.y = k-point)
+    if ((rc = ensure_workspace(p, fft_ws_bytes_per_band_batched(p), nband, &chunk, &ws, st))) return rc;
+    for (int b0 = 0; b0 < nband; b0 += chunk) {
+      int nb = nband - b0 < chunk ? nband - b0 : chunk;
+      if ((rc = fft2_apply_batched(p, psi + (size_t)b0 * band_stride, hpsi + (size_t)b0 * band_stride, nb, nband, ws, st))) return rc;
+    }
+    return DFT_OK;
+  }
+  if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
+  for (int ik = 0; ik < p->nkpt; ik++)
+    for (int b0 = 0; b0 < nband; b0 += chunk) {
+      int nb = nband - b0 < chunk ? nband - b0 : chunk;
+      size_t off = ((size_t)ik * nband + b0) * band_stride;
+      FftExtra X;
+      if (extra) {
+        X = *extra;
+        if (X.pre) X.pre += (size_t)ik * 3 * p->mpw;
+        if (X.post) X.post += (size_t)ik * 3 * p->mpw;
+      }
+      if ((rc = fft_apply_vloc(p, ik, psi + off, hpsi + off, nb, ws, st, extra ? &X : nullptr))) return rc;
+    }
+  return DFT_OK;
+}
+
 static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nband, cudaStream_t st, const Recurrence *rec = nullptr,
                       double *spsi = nullptr) {
   p->last_launches = 0;
@@ -299,27 +334,8 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
   int rc;
   const size_t band_stride = (size_t)p->mpw * 2;
   const bool small = (p->fft_path == 0 || p->fft_path == 3) && fft_small_ok(p);
-  if (loc && small) {
-    // the box fits one SM's shared memory: the whole local term of all k-points and bands is ONE launch, no scratch
-    if ((rc = fft_small_apply(p, 0, p->nkpt, psi, hpsi, nband, nband, st))) return rc;
-  } else if (loc) {
-    int chunk; void *ws;
-    if (fft2_batch_ok(p) && (!p->ws_user || p->ws_user_bytes >= fft_ws_bytes_per_band_batched(p))) {
-      // small boxes, many k-points: every pass is one launch over all k-points (blockIdx.y = k-point)
-      if ((rc = ensure_workspace(p, fft_ws_bytes_per_band_batched(p), nband, &chunk, &ws, st))) return rc;
-      for (int b0 = 0; b0 < nband; b0 += chunk) {
-        int nb = nband - b0 < chunk ? nband - b0 : chunk;
-        if ((rc = fft2_apply_batched(p, psi + (size_t)b0 * band_stride, hpsi + (size_t)b0 * band_stride, nb, nband, ws, st))) return rc;
-      }
-    } else {
-    if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
-    for (int ik = 0; ik < p->nkpt; ik++)
-      for (int b0 = 0; b0 < nband; b0 += chunk) {
-        int nb = nband - b0 < chunk ? nband - b0 : chunk;
-        size_t off = ((size_t)ik * nband + b0) * band_stride;
-        if ((rc = fft_apply_vloc(p, ik, psi + off, hpsi + off, nb, ws, st))) return rc;
-      }
-    }
+  if (loc) {
+    if ((rc = local_term(p, psi, hpsi, nband, st, nullptr))) return rc;
   } else {
     phase_begin(p, 4, st);
     if ((rc = zero_fill(hpsi, (int64_t)p->nkpt * nband * band_stride, st))) return rc;
@@ -441,6 +457,7 @@ int dft_set_dij(dft_plan *p, const double *dij) {
   size_t n = (size_t)p->natom * p->lmax * p->lmax;
   if (n == 0) return DFT_OK;
   if (!dij) { set_error("dij is NULL"); return DFT_ERR_INVALID_ARG; }
+  if (p->gam) { int rcg = gamma_check_dij(p, dij); if (rcg) return rcg; }
   // an apply enqueued earlier on a non-blocking stream may still read D_ij: wait for the device before replacing it
   DFT_CUDA_CHECK(cudaDeviceSynchronize());
   DFT_CUDA_CHECK(cudaMemcpy(p->d_dij, dij, n * sizeof(double), cudaMemcpyHostToDevice));
@@ -569,6 +586,13 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     }
     p->proj_mode = (int)value; return DFT_OK;
   }
+  if (!strcmp(key, "gamma_real")) {
+    if (value < 0 || value > 1) { set_error("gamma_real = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if (value == 1) return gamma_build(p);
+    DFT_CUDA_CHECK(cudaDeviceSynchronize());
+    gamma_free(p);
+    return DFT_OK;
+  }
   if (!strcmp(key, "host_groups")) {
     if (value < 1 || value > 64) { set_error("host_groups = %lld outside 1..64", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->host_groups = (int)value; return DFT_OK;
@@ -592,6 +616,59 @@ int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, voi
   if (nband > 0 && p->mpw > 0 && (!psi || !hpsi)) { set_error("null psi/hpsi"); return DFT_ERR_INVALID_ARG; }
   if (((uintptr_t)psi & 15) || ((uintptr_t)hpsi & 15)) { set_error("psi/hpsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
   return apply_impl(p, psi, hpsi, nband, (cudaStream_t)stream);
+  DFT_GUARD_END
+}
+
+int dft_plan_get_kg_gamma(const dft_plan *p, int32_t *nhalf, int32_t *kg, int32_t *igfft, double *kin) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (!p->gam) { set_error("Gamma storage is not enabled (dft_plan_set_option gamma_real = 1)"); return DFT_ERR_NOT_READY; }
+  const GammaData &G = *p->gam;
+  if (nhalf) *nhalf = G.nh;
+  if (kg && G.nh) memcpy(kg, G.h_kg.data(), sizeof(int32_t) * 3 * (size_t)G.nh);
+  if (igfft && G.nh) memcpy(igfft, G.h_igfft.data(), sizeof(int32_t) * (size_t)G.nh);
+  if (kin && G.nh) memcpy(kin, G.h_kin.data(), sizeof(double) * (size_t)G.nh);
+  return DFT_OK;
+}
+
+int dft_apply_h_gamma(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  if (nband > 0 && p->gam && p->gam->nh > 0 && (!psi || !hpsi)) { set_error("null psi/hpsi"); return DFT_ERR_INVALID_ARG; }
+  if (((uintptr_t)psi & 15) || ((uintptr_t)hpsi & 15)) { set_error("psi/hpsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  return gamma_apply(p, psi, hpsi, nband, (cudaStream_t)stream);
+  DFT_GUARD_END
+}
+
+int dft_set_vloc_spinor(dft_plan *p, const double *v4, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p || !v4) { set_error("null argument"); return DFT_ERR_INVALID_ARG; }
+  return spinor_set_vloc(p, v4, (cudaStream_t)stream);
+  DFT_GUARD_END
+}
+
+int dft_set_dij_spinor(dft_plan *p, const double *dspin) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (!dspin) { p->dspin_set = false; return DFT_OK; }     // back to the scalar D_ij on both components
+  const size_t n = (size_t)p->natom * 4 * p->lmax * p->lmax * 2;
+  if (n == 0) return DFT_OK;
+  DFT_CUDA_CHECK(cudaDeviceSynchronize());                  // an apply enqueued earlier may still read the old matrix
+  if (!p->d_dspin && cudaMalloc(&p->d_dspin, n * sizeof(double)) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the spinor D_ij"); return DFT_ERR_ALLOC; }
+  DFT_CUDA_CHECK(cudaMemcpy(p->d_dspin, dspin, n * sizeof(double), cudaMemcpyHostToDevice));
+  p->dspin_set = true;
+  return DFT_OK;
+  DFT_GUARD_END
+}
+
+int dft_apply_h_spinor(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream) {
+  DFT_GUARD_BEGIN
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0) { set_error("nband = %d is negative", nband); return DFT_ERR_INVALID_ARG; }
+  if (nband > 0 && p->mpw > 0 && (!psi || !hpsi)) { set_error("null psi/hpsi"); return DFT_ERR_INVALID_ARG; }
+  if (((uintptr_t)psi & 15) || ((uintptr_t)hpsi & 15)) { set_error("psi/hpsi must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  if (2 * (int64_t)nband > 65535 * 2) { set_error("nband too large"); return DFT_ERR_INVALID_ARG; }
+  return spinor_apply(p, psi, hpsi, nband, (cudaStream_t)stream);
   DFT_GUARD_END
 }
 

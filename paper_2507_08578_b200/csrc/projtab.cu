@@ -23,6 +23,7 @@ struct ProjParams {
   const int32_t *typat, *nlmn, *lmn_l, *lmn_m, *lmn_irad, *atom_first, *nq;
   const double *dq, *xred, *f, *f2;
   double *ptab;   // this k-point's [nproj][mpw] complex
+  int rot_odd;    // 1: rows of odd l are multiplied by i (Gamma storage, reading 26)
 };
 
 // reading 7
@@ -96,8 +97,9 @@ __global__ void __launch_bounds__(PT_THREADS) projtab_kernel(ProjParams P) {
       F = spline_eval(P.nq[t], P.dq[t], P.f + off, P.f2 + off, qn);
       if (ir < PT_MAXRAD) { frad[ir] = F; have[ir] = true; }
     }
-    double fy = F * real_ylm(P.lmn_l[t * P.lmax + i], P.lmn_m[t * P.lmax + i], qx, qy, qz, qn);
-    dst[(size_t)i * P.mpw] = make_double2(fy * cs, fy * sn);
+    const int l = P.lmn_l[t * P.lmax + i];
+    double fy = F * real_ylm(l, P.lmn_m[t * P.lmax + i], qx, qy, qz, qn);
+    dst[(size_t)i * P.mpw] = (P.rot_odd && (l & 1)) ? make_double2(-(fy * sn), fy * cs) : make_double2(fy * cs, fy * sn);
   }
 }
 
@@ -131,8 +133,25 @@ int build_projector_table(dft_plan *p, int ik, double *maxq_out) {
   P.lmn_irad = p->d_lmn_irad; P.atom_first = p->d_atom_first; P.nq = p->d_nq; P.dq = p->d_dq; P.xred = p->d_xred;
   P.f = p->d_f; P.f2 = p->d_f2;
   P.ptab = p->d_ptab + (size_t)ik * p->nproj * p->mpw * 2;
+  P.rot_odd = 0;
   dim3 grid((p->mpw + PT_THREADS - 1) / PT_THREADS, p->natom);
   projtab_kernel<<<grid, PT_THREADS>>>(P);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+// The same table on another plane-wave list (device kg [npw][3]), rows mpw apart, into d_out [nproj][mpw] complex
+int build_projector_table_on(dft_plan *p, const int32_t *d_kg, int npw, int mpw, const double k[3], double *d_out, int rot_odd) {
+  if (p->natom == 0 || p->nproj == 0 || mpw == 0) return DFT_OK;
+  ProjParams P;
+  for (int i = 0; i < 9; i++) P.bm[i] = p->bm[i];
+  for (int i = 0; i < 3; i++) P.k[i] = k[i];
+  P.npw = npw; P.mpw = mpw; P.natom = p->natom; P.lmax = p->lmax; P.nrad_max = p->nrad_max; P.nq_max = p->nq_max;
+  P.kg = d_kg; P.typat = p->d_typat; P.nlmn = p->d_nlmn; P.lmn_l = p->d_lmn_l; P.lmn_m = p->d_lmn_m;
+  P.lmn_irad = p->d_lmn_irad; P.atom_first = p->d_atom_first; P.nq = p->d_nq; P.dq = p->d_dq; P.xred = p->d_xred;
+  P.f = p->d_f; P.f2 = p->d_f2;
+  P.ptab = d_out; P.rot_odd = rot_odd;
+  projtab_kernel<<<dim3((mpw + PT_THREADS - 1) / PT_THREADS, p->natom), PT_THREADS>>>(P);
   DFT_CUDA_CHECK(cudaGetLastError());
   return DFT_OK;
 }
@@ -236,7 +255,7 @@ int build_factor_tables(dft_plan *p) {
     P.npw = kp.npw; P.mpw = p->mpw; P.natom = p->natom; P.lmax = p->lmax; P.nrad_max = p->nrad_max; P.nq_max = p->nq_max;
     P.kg = kp.kg; P.typat = p->d_typat; P.nlmn = p->d_nlmn; P.lmn_l = p->d_lmn_l; P.lmn_m = p->d_lmn_m;
     P.lmn_irad = p->d_lmn_irad; P.atom_first = p->d_atom_first; P.nq = p->d_nq; P.dq = p->d_dq; P.xred = p->d_xred;
-    P.f = p->d_f; P.f2 = p->d_f2; P.ptab = nullptr;
+    P.f = p->d_f; P.f2 = p->d_f2; P.ptab = nullptr; P.rot_odd = 0;
     stab_kernel<<<dim3((p->mpw + PT_THREADS - 1) / PT_THREADS, p->natom), PT_THREADS>>>(
         P, reinterpret_cast<double2 *>(p->d_stab) + (size_t)ik * p->natom * p->mpw);
     fytab_kernel<<<dim3((p->ldf + PT_THREADS - 1) / PT_THREADS, p->ntypat), PT_THREADS>>>(

@@ -495,6 +495,63 @@ def main():
             line["factorised_projectors"] = {"unavailable": str(e)}
         plan.set_option("proj_mode", 0)
 
+    # ---- context figures: the same cell in Gamma-point real-symmetry storage (half sphere, two bands
+    #      per complex FFT, real GEMMs) and with two-component spinors (nband/2 spinor bands = the same number of rows)
+    if args.cheb_degree > 0 and world == 1 and plan.nkpt == 1 and all(v == 0.0 for v in cfg["kpt"][0]):
+        try:
+            dft.dft_set_dij(plan.h, synth.gamma_dij(cfg))
+            plan.set_option("gamma_real", 1)
+            hkin = plan.get_kg_gamma()[2]
+            gpsi = synth.gen_psi_torch(cfg_r, [hkin], "cuda")[0]
+            ghpsi = torch.empty_like(gpsi)
+            plan.apply_h_gamma(gpsi, ghpsi)
+            torch.cuda.synchronize()
+            g0 = torch.cuda.Event(enable_timing=True); g1 = torch.cuda.Event(enable_timing=True)
+            g0.record()
+            for _ in range(3):
+                plan.apply_h_gamma(gpsi, ghpsi)
+            g1.record()
+            torch.cuda.synchronize()
+            gms = g0.elapsed_time(g1) / 3
+            plan.set_timing(True); plan.phase_ms()
+            plan.apply_h_gamma(gpsi, ghpsi)
+            torch.cuda.synchronize()
+            gph = {k: round(v[0], 3) for k, v in plan.phase_ms().items() if v[0] > 0}
+            plan.set_timing(False)
+            gfl = 2.0 * 2.0 * plan.nproj * len(hkin) * nband          # one real GEMM: 2 flops x nproj x (2 nhalf) x nband
+            line["gamma_real_storage"] = {
+                "value": nband / (gms * 1e-3), "unit": UNIT, "ms_per_step": gms, "nhalf": int(len(hkin)), "phase_ms": gph,
+                "gemm1_tensor_frac": gfl / (gph.get("gemm1", 1e30) * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                "gemm2_tensor_frac": gfl / (gph.get("gemm2_kinetic", 1e30) * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                "api": "dft_apply_h_gamma (option gamma_real = 1; D_ij with the odd-parity couplings removed)"}
+            del gpsi, ghpsi
+            plan.set_option("gamma_real", 0)
+        except dft.DftError as e:
+            line["gamma_real_storage"] = {"unavailable": str(e)}
+        dft.dft_set_dij(plan.h, cfg["dij"])
+        torch.cuda.empty_cache()
+    if args.cheb_degree > 0 and world == 1:
+        try:
+            vl = torch.as_tensor(cfg["vloc"], device="cuda")
+            v4 = torch.stack([vl * 1.05, vl * 0.95, vl * 0.02, vl * -0.01]).contiguous()
+            plan.set_vloc_spinor(v4)
+            snb = nband // 2
+            spsi_ = psi[:, :2 * snb].reshape(plan.nkpt, snb, 2, plan.mpw)
+            shp = torch.empty_like(spsi_)
+            plan.apply_h_spinor(spsi_, shp)
+            torch.cuda.synchronize()
+            s0 = torch.cuda.Event(enable_timing=True); s1 = torch.cuda.Event(enable_timing=True)
+            s0.record(); plan.apply_h_spinor(spsi_, shp); s1.record()
+            torch.cuda.synchronize()
+            sms = s0.elapsed_time(s1)
+            line["spinor"] = {"value": plan.nkpt * snb / (sms * 1e-3), "unit": "spinor bands/s", "ms_per_step": sms,
+                              "spinor_bands": snb, "api": "dft_apply_h_spinor (scalar D_ij on both components; four scalar "
+                              "local applications for the 2x2 potential)"}
+            del v4, shp, spsi_
+        except dft.DftError as e:
+            line["spinor"] = {"unavailable": str(e)}
+        torch.cuda.empty_cache()
+
     # ---- context figure: the vendor-library formulation the paper describes, on the same B200
     if args.vendor and world == 1 and plan.nkpt == 1 and all(t["nlmn"] == cfg["nlmn_max"] for t in cfg["types"]):
         try:

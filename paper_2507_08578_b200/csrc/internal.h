@@ -88,6 +88,9 @@ struct GammaData {
   std::vector<double> h_kin;
 };
 
+struct NlMaps;
+void nl_maps_free(dft_plan *p);
+
 // timed kernel groups: 0-4 the five FFT passes, 5 GEMM-1, 6 D_ij, 7 GEMM-2, 8 the fused small-box local term (fft_small.cu),
 // 9 pack / unpack of band pairs (Gamma storage) and the spin-matrix products of the spinor path
 constexpr int NPHASE = 10;
@@ -167,11 +170,14 @@ struct dft_plan {
   void *d_geom2 = nullptr;    // device array of per-k-point FFT geometry (fft2.cu, built at first batched call)
   void *d_geom_small = nullptr;   // the same for the fused small-box kernel (fft_small.cu)
   bool small_attr_done = false;
+  unsigned small2_attr_mask = 0;  // instantiations of fft_small2.cu whose shared-memory attribute is set on this plan's device
+  int32_t *d_dstmap = nullptr;    // [nkpt][mpw] position of every plane wave in the x-line array of fft_small2.cu
   int sm_count = 148;
   int smem_per_sm = 233472, smem_optin = 232448;   // bytes of shared memory per SM / per CTA (opt-in), from the device
   int64_t last_launches = 0;
   bool nl_attr_done = false;   // cudaFuncSetAttribute of the GEMM kernels done on this plan's device
   dftb200::PhaseTimer timer;
+  dftb200::NlMaps *nl_maps = nullptr;  // tensor maps of the table-mode GEMMs, kept between calls (nonlocal.cu)
   dftb200::GammaData *gam = nullptr;   // built by option gamma_real = 1
   // two-component spinors (spinor.cu): Pauli components of the local potential, spin-dependent D
   double *d_vpauli = nullptr;          // [4][n3][n2][n1]: V0, Vx, Vy, Vz, each pre-scaled by 1/N
@@ -234,6 +240,8 @@ int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, 
 bool fft_small_ok(const dft_plan *p);
 int fft_small_apply(dft_plan *p, int ik0, int nk, const double *psi, double *hpsi, int nb, int nband_total, cudaStream_t st,
                     const FftExtra *extra = nullptr);
+
+int fft_small2_launch(dft_plan *p, void *sb_params, int nk, int nb, cudaStream_t st, bool *handled);   // fft_small2.cu
 
 // --- nonlocal.cu (K3) ---------------------------------------------------------------------
 // hpsi (+)= V_nl psi + kin*psi for all k-points; accumulate = hpsi already holds V_loc psi

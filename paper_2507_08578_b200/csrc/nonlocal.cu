@@ -67,7 +67,9 @@ struct Gemm2Params {
 // REAL (Gamma-point storage, gamma.cu): MODE 1 keeps only Re(conj(A) B) = A_r B_r + A_i B_i, a REAL GEMM over the
 // interleaved (re, im) doubles; MODE 2 takes B as real (its imaginary halves are zero): Re += A_r B_r, Im += A_i B_r.
 // Either way two of the four DMMA sets remain.
-template <int MODE, bool REAL = false>
+// MB: 8-row blocks of the M operand per warp (MODE 1 only: 4 = the 128-row tile, 2 / 1 = skinny tiles of 64 / 32 rows for
+// systems with few projectors).
+template <int MODE, bool REAL = false, int MB = 4>
 __device__ __forceinline__ void mma_stage(const unsigned char *As, const unsigned char *Bs, int wm, int wn, int lane,
                                           double (&cre)[4][4][2], double (&cim)[4][4][2]) {
   const int i = lane >> 2, j = lane & 3;
@@ -76,9 +78,9 @@ __device__ __forceinline__ void mma_stage(const unsigned char *As, const unsigne
     double ar[4], ai[4], br[4], bi[4];
     if (MODE == 1) {
       // A tile [128 rows p][8 complex g]: row = wm*32 + mb*8 + i, chunk (2j+kg) ^ i
-      const unsigned char *a0 = As + (wm * 32 + i) * 128 + (((2 * j + kg) ^ i) << 4);
+      const unsigned char *a0 = As + (wm * 8 * MB + i) * 128 + (((2 * j + kg) ^ i) << 4);
 #pragma unroll
-      for (int mb = 0; mb < 4; mb++) {
+      for (int mb = 0; mb < MB; mb++) {
         double2 v = *reinterpret_cast<const double2 *>(a0 + mb * 8 * 128);
         ar[mb] = v.x; ai[mb] = v.y;
       }
@@ -87,7 +89,7 @@ __device__ __forceinline__ void mma_stage(const unsigned char *As, const unsigne
       const int pr = 2 * j + kg;
       const unsigned char *a0 = As + (wm * 4) * 1024 + pr * 128 + ((i ^ pr) << 4);
 #pragma unroll
-      for (int mb = 0; mb < 4; mb++) {
+      for (int mb = 0; mb < MB; mb++) {
         double2 v = *reinterpret_cast<const double2 *>(a0 + mb * 1024);
         ar[mb] = v.x; ai[mb] = v.y;
       }
@@ -99,12 +101,12 @@ __device__ __forceinline__ void mma_stage(const unsigned char *As, const unsigne
       br[nb] = v.x; bi[nb] = v.y;
     }
 #pragma unroll
-    for (int mb = 0; mb < 4; mb++)
+    for (int mb = 0; mb < MB; mb++)
 #pragma unroll
       for (int nb = 0; nb < 4; nb++) dmma(cre[mb][nb][0], cre[mb][nb][1], ar[mb], br[nb]);
     if (REAL) {
 #pragma unroll
-      for (int mb = 0; mb < 4; mb++)
+      for (int mb = 0; mb < MB; mb++)
 #pragma unroll
         for (int nb = 0; nb < 4; nb++) {
           if (MODE == 1) dmma(cre[mb][nb][0], cre[mb][nb][1], ai[mb], bi[nb]);
@@ -113,31 +115,31 @@ __device__ __forceinline__ void mma_stage(const unsigned char *As, const unsigne
       continue;
     }
 #pragma unroll
-    for (int mb = 0; mb < 4; mb++)
+    for (int mb = 0; mb < MB; mb++)
 #pragma unroll
       for (int nb = 0; nb < 4; nb++) dmma(cim[mb][nb][0], cim[mb][nb][1], ar[mb], bi[nb]);
     if (MODE == 1) {
       // conj(p) psi: re += p_i psi_i, im -= p_i psi_r
 #pragma unroll
-      for (int mb = 0; mb < 4; mb++)
+      for (int mb = 0; mb < MB; mb++)
 #pragma unroll
         for (int nb = 0; nb < 4; nb++) dmma(cre[mb][nb][0], cre[mb][nb][1], ai[mb], bi[nb]);
 #pragma unroll
-      for (int mb = 0; mb < 4; mb++) ai[mb] = -ai[mb];
+      for (int mb = 0; mb < MB; mb++) ai[mb] = -ai[mb];
 #pragma unroll
-      for (int mb = 0; mb < 4; mb++)
+      for (int mb = 0; mb < MB; mb++)
 #pragma unroll
         for (int nb = 0; nb < 4; nb++) dmma(cim[mb][nb][0], cim[mb][nb][1], ai[mb], br[nb]);
     } else {
       // p c: im += p_i c_r, re -= p_i c_i
 #pragma unroll
-      for (int mb = 0; mb < 4; mb++)
+      for (int mb = 0; mb < MB; mb++)
 #pragma unroll
         for (int nb = 0; nb < 4; nb++) dmma(cim[mb][nb][0], cim[mb][nb][1], ai[mb], br[nb]);
 #pragma unroll
       for (int nb = 0; nb < 4; nb++) bi[nb] = -bi[nb];
 #pragma unroll
-      for (int mb = 0; mb < 4; mb++)
+      for (int mb = 0; mb < MB; mb++)
 #pragma unroll
         for (int nb = 0; nb < 4; nb++) dmma(cre[mb][nb][0], cre[mb][nb][1], ai[mb], bi[nb]);
     }
@@ -165,9 +167,10 @@ __device__ __forceinline__ Pipe pipe_setup(unsigned char *smem_raw) {
 
 // ---------------------------------------------------------------- GEMM-1: projection (split-K partials)
 // grid: (tiles_m*tiles_n, nsplit, nkpt)
-template <bool REAL>
+template <bool REAL, int MB = 4>
 __global__ void __launch_bounds__(NL_THREADS, 1)
 gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapPsi, Gemm1Params Q) {
+  constexpr int BM = 32 * MB;            // rows of P per CTA tile (the TMA box of mapP has BM rows)
   extern __shared__ unsigned char smem_raw[];
   Pipe P = pipe_setup(smem_raw);
   const int tile = blockIdx.x, tn = tile % Q.tiles_n, tm = tile / Q.tiles_n;
@@ -179,8 +182,8 @@ gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
     int s = j % NL_STAGES;
     if (j >= NL_STAGES) mbar_wait(&P.empty[s], ((j / NL_STAGES) - 1) & 1);
     unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
-    mbar_expect_tx(&P.full[s], NL_STAGE_BYTES);
-    tma_load_3d(st, &mapP, &P.full[s], (s0 + j) * 16, tm * NL_BM, ik);
+    mbar_expect_tx(&P.full[s], BM * 128 + NL_STAGE_B);
+    tma_load_3d(st, &mapP, &P.full[s], (s0 + j) * 16, tm * BM, ik);
     tma_load_3d(st + NL_STAGE_A, &mapPsi, &P.full[s], (s0 + j) * 16, tn * NL_BN, ik);
   };
   const bool producer = (threadIdx.x == 0);
@@ -198,7 +201,7 @@ gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
     int s = it % NL_STAGES;
     mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
     const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
-    mma_stage<1, REAL>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
+    mma_stage<1, REAL, MB>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
     __syncwarp();
     if (lane == 0) mbar_arrive(&P.empty[s]);
   }
@@ -207,8 +210,8 @@ gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
   double *outr = reinterpret_cast<double *>(Q.part) + ((size_t)(ik * Q.nsplit + split) * Q.nproj) * Q.nband;
   const int i = lane >> 2, j = lane & 3;
 #pragma unroll
-  for (int mb = 0; mb < 4; mb++) {
-    int pr = tm * NL_BM + wm * 32 + mb * 8 + i;
+  for (int mb = 0; mb < MB; mb++) {
+    int pr = tm * BM + wm * 8 * MB + mb * 8 + i;
     if (pr >= Q.nproj) continue;
 #pragma unroll
     for (int nb = 0; nb < 4; nb++) {
@@ -236,13 +239,15 @@ __global__ void dij_kernel(const double2 *__restrict__ part, double2 *__restrict
   if (b >= nband) return;
   int nl = nlmn[typat[a]], first = atom_first[a];
   double2 c[DIJ_MAXL];
-  for (int jj = 0; jj < nl; jj++) {
-    double sr = 0.0, si = 0.0;
-    for (int s = 0; s < nsplit; s++) {
-      double2 v = part[((size_t)(ik * nsplit + s) * nproj + first + jj) * nband + b];
-      sr += v.x; si += v.y;
+  for (int jj = 0; jj < nl; jj++) c[jj] = make_double2(0.0, 0.0);
+  // splits outer, projectors inner: the nl loads of one split are independent (fixed summation order per projector)
+  for (int s = 0; s < nsplit; s++) {
+    const double2 *src = part + ((size_t)(ik * nsplit + s) * nproj + first) * nband + b;
+#pragma unroll 4
+    for (int jj = 0; jj < nl; jj++) {
+      double2 v = src[(size_t)jj * nband];
+      c[jj].x += v.x; c[jj].y += v.y;
     }
-    c[jj] = make_double2(sr, si);
   }
   double2 *dst = cpr + ((size_t)ik * nband + b) * nproj + first;
   if (!dij) {   // no D: the reduced projections <p|psi> themselves (dft_get_cprj)
@@ -850,6 +855,13 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
 }
 
 // ---------------------------------------------------------------- host side
+struct NlMaps {
+  CUtensorMap mapP1, mapP2, mapPsi, mapC;
+  const void *ptab = nullptr, *psi = nullptr, *cprj = nullptr;
+  int bm1 = 0, nband_psi = -1, nband_c = -1;
+};
+void nl_maps_free(dft_plan *p) { delete p->nl_maps; p->nl_maps = nullptr; }
+
 typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                              const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -912,7 +924,7 @@ __global__ void kin_only_kernel(const double2 *__restrict__ psi, double2 *__rest
 static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
   int best = 1; double best_eff = 0.0;
   // at least 32 slabs per split when the tiles alone fill the SMs; small problems (latency-bound) may go down to 8
-  const int min_slabs = (int64_t)tiles * nkpt >= sm_count ? 32 : 8;
+  const int min_slabs = (int64_t)tiles * nkpt >= sm_count ? 32 : (nkpt >= 16 ? 24 : 8);
   for (int s = 1; s <= 64; s++) {
     if (s > 1 && nslab / s < min_slabs) break;
     double units = (double)tiles * s * nkpt;
@@ -936,6 +948,8 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   if (!p->nl_attr_done) {   // per plan (= per device), not per process
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_fac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FC_SMEM));
@@ -970,7 +984,10 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   q1.nproj = nproj; q1.nband = nband;
   q1.nslab = (mpw + 7) / 8;
   const bool fac = p->proj_mode == 1;     // factorised projectors: tiles of 16 atoms instead of 128 table rows
-  q1.tiles_m = fac ? (p->nblk + FC_BA - 1) / FC_BA : (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
+  // few projectors (nproj <= 64): the 4-product GEMM-1 with a 32- or 64-row tile instead of 128 padded rows
+  const int skinny_mb = (!fac && nproj <= 32) ? 1 : ((!fac && nproj <= 64) ? 2 : 0);
+  const int bm1 = skinny_mb ? 32 * skinny_mb : NL_BM;
+  q1.tiles_m = fac ? (p->nblk + FC_BA - 1) / FC_BA : (nproj + bm1 - 1) / bm1; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
   int ns = p->splitk > 0 ? p->splitk : choose_splitk(q1.tiles_m * q1.tiles_n, q1.nslab, p->sm_count, nkpt);
   if (ns > q1.nslab) ns = q1.nslab;
   q1.slabs_per_split = (q1.nslab + ns - 1) / ns;
@@ -988,10 +1005,18 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     p->cprj_bytes = need_cprj;
   }
   q1.part = reinterpret_cast<double2 *>(p->d_part);
-  CUtensorMap mapP1, mapPsi, mapP2, mapC;
+  // the four tensor maps of the table mode are kept between calls (encoding them costs more host time than launching the
+  // kernels of a small cell) and re-encoded only when the pointer or shape they describe changed
+  NlMaps *C = p->nl_maps;
+  if (!C) { C = new NlMaps(); p->nl_maps = C; }
+  CUtensorMap &mapP1 = C->mapP1, &mapPsi = C->mapPsi, &mapP2 = C->mapP2, &mapC = C->mapC;
   uint64_t rowb = (uint64_t)mpw * 16;
-  if (!fac && (rc = make_map(p, &mapP1, p->d_ptab, 2 * (uint64_t)mpw, nproj, nkpt, rowb, rowb * nproj, NL_BM))) return rc;
-  if ((rc = make_map(p, &mapPsi, psi, 2 * (uint64_t)mpw, nband, nkpt, rowb, rowb * nband, NL_BN))) return rc;
+  const bool tab_same = !fac && C->ptab == p->d_ptab && C->bm1 == bm1;
+  if (!fac && !tab_same && (rc = make_map(p, &mapP1, p->d_ptab, 2 * (uint64_t)mpw, nproj, nkpt, rowb, rowb * nproj, bm1))) return rc;
+  if (C->psi != psi || C->nband_psi != nband) {
+    if ((rc = make_map(p, &mapPsi, psi, 2 * (uint64_t)mpw, nband, nkpt, rowb, rowb * nband, NL_BN))) return rc;
+    C->psi = psi; C->nband_psi = nband;
+  }
   CUtensorMap mapS1, mapF1, mapS2, mapF2;
   if (fac) {
     if (!p->d_stab || !p->d_fytab) { set_error("factor tables missing"); return DFT_ERR_NOT_READY; }
@@ -1001,7 +1026,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     if ((rc = make_map_plain(p, &mapS2, p->d_stab, 2 * (uint64_t)mpw, p->natom, nkpt, rowb, rowb * p->natom, 2 * NL_BM, 1))) return rc;
     if ((rc = make_map_plain(p, &mapF2, p->d_fytab, p->ldf, nfr, nkpt, frow, frow * nfr, FD_FLD, (uint32_t)nfr))) return rc;
   }
-  if (!fac) {
+  if (!fac && !tab_same) {
     // GEMM-2 reads P "M-major": view each table row as [g-block][16 doubles] and put the projector
     // index between them, so ONE box {16, 8 rows, 16 g-blocks} brings a 128 g x 8 p tile in the
     // [g-block][p][8 complex] order the fragments want (16 separate 1 KB boxes starved the MMA loop:
@@ -1015,8 +1040,12 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
                                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (GEMM-2 P map) failed (%d)", (int)r); return DFT_ERR_CUDA; }
+    C->ptab = p->d_ptab; C->bm1 = bm1;
   }
-  if ((rc = make_map(p, &mapC, p->d_cprj, 2 * (uint64_t)nproj, nband, nkpt, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * nband, NL_BN))) return rc;
+  if (C->cprj != p->d_cprj || C->nband_c != nband) {
+    if ((rc = make_map(p, &mapC, p->d_cprj, 2 * (uint64_t)nproj, nband, nkpt, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * nband, NL_BN))) return rc;
+    C->cprj = p->d_cprj; C->nband_c = nband;
+  }
   phase_begin(p, 5, st);
   if (fac) {
     Fac1Params f1;
@@ -1024,7 +1053,9 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     f1.slabs_per_split = q1.slabs_per_split; f1.tiles_n = q1.tiles_n;
     f1.blk_atom = p->d_blk_atom; f1.blk_frow = p->d_blk_frow; f1.blk_first = p->d_blk_first; f1.blk_nl = p->d_blk_nl; f1.part = q1.part;
     gemm1_fac_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), FC_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1, f1);
-  } else if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  } else if (skinny_mb == 1) gemm1_kernel<false, 1><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  else if (skinny_mb == 2) gemm1_kernel<false, 2><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  else if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   else gemm1_kernel<false><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   phase_end(p, 5, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());

@@ -62,10 +62,11 @@ static void destroy_plan(dft_plan *p) {
   cudaFree(p->d_f); cudaFree(p->d_f2); cudaFree(p->d_typat); cudaFree(p->d_nlmn); cudaFree(p->d_lmn_l); cudaFree(p->d_lmn_m);
   cudaFree(p->d_lmn_irad); cudaFree(p->d_atom_first); cudaFree(p->d_nq); cudaFree(p->d_dq); cudaFree(p->d_xred);
   cudaFree(p->d_blk_atom); cudaFree(p->d_blk_frow); cudaFree(p->d_blk_first); cudaFree(p->d_blk_nl);
-  cudaFree(p->d_stab); cudaFree(p->d_fytab); cudaFree(p->d_vtau); cudaFree(p->d_qcart); cudaFree(p->d_qhalf); cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_geom_small); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
+  cudaFree(p->d_stab); cudaFree(p->d_fytab); cudaFree(p->d_vtau); cudaFree(p->d_qcart); cudaFree(p->d_qhalf); cudaFree(p->d_wgt); cudaFree(p->d_geom2); cudaFree(p->d_geom_small); cudaFree(p->d_dstmap); cudaFree(p->d_kina); cudaFree((void *)p->d_kinaptr); cudaFree(p->d_dij); cudaFree(p->d_sij); cudaFree(p->d_ones); cudaFree((void *)p->d_oneptr); cudaFree(p->d_ptab); cudaFree(p->d_npw); cudaFree((void *)p->d_kinptr); cudaFree(p->d_vloc);
   for (int c = 0; c < 3; c++) cudaFree(p->d_tw[c]);
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   gamma_free(p);
+  nl_maps_free(p);
   cudaFree(p->d_vpauli); cudaFree(p->d_dspin); cudaFree(p->d_spin_tmp);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
   if (p->h2d_stream) cudaStreamDestroy(p->h2d_stream);
@@ -296,7 +297,7 @@ static int ensure_qcart_ready(dft_plan *p) {
 int local_term(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStream_t st, const FftExtra *extra) {
   int rc;
   const size_t band_stride = (size_t)p->mpw * 2;
-  const bool small = (p->fft_path == 0 || p->fft_path == 3) && fft_small_ok(p);
+  const bool small = (p->fft_path == 0 || p->fft_path == 3 || p->fft_path == 5) && fft_small_ok(p);
   if (small)   // the box fits one SM's shared memory: the whole local term of all k-points and bands is ONE launch, no scratch
     return fft_small_apply(p, 0, p->nkpt, psi, hpsi, nband, nband, st, extra);
   int chunk; void *ws;
@@ -333,7 +334,7 @@ static int apply_impl(dft_plan *p, const double *psi, double *hpsi, int32_t nban
   if (loc && !p->vloc_set) { set_error("dft_apply_h called before dft_set_vloc"); return DFT_ERR_NOT_READY; }
   int rc;
   const size_t band_stride = (size_t)p->mpw * 2;
-  const bool small = (p->fft_path == 0 || p->fft_path == 3) && fft_small_ok(p);
+  const bool small = (p->fft_path == 0 || p->fft_path == 3 || p->fft_path == 5) && fft_small_ok(p);
   if (loc) {
     if ((rc = local_term(p, psi, hpsi, nband, st, nullptr))) return rc;
   } else {
@@ -559,8 +560,8 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     p->terms = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "fft_path")) {
-    if (value < 0 || value > 4) { set_error("fft_path = %lld outside 0..4", (long long)value); return DFT_ERR_INVALID_ARG; }
-    if (value == 3 && !fft_small_ok(p)) { set_error("fft_path = 3: the fused small-box kernel cannot serve this plan (box lengths or shared memory)"); return DFT_ERR_UNSUPPORTED; }
+    if (value < 0 || value > 5) { set_error("fft_path = %lld outside 0..5", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if ((value == 3 || value == 5) && !fft_small_ok(p)) { set_error("fft_path = 3: the fused small-box kernel cannot serve this plan (box lengths or shared memory)"); return DFT_ERR_UNSUPPORTED; }
     p->fft_path = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "proj_mode")) {

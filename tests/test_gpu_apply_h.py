@@ -137,7 +137,7 @@ def test_small_box_fused_kernel(name, over):
     assert small_box_ok(plan), "the small-box kernel should serve %s %s" % (name, over)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     method = 1 if name in ("c0", "aniso", "anisok3") else 2
-    for path in (3, 0):
+    for path in (3, 5, 0):      # 3 / 0: compile-time-size kernel where the box has one; 5: the run-time-dispatched kernel
         plan.set_option("fft_path", path)
         for terms in (7, 2):
             plan.set_option("terms", terms)
@@ -153,10 +153,12 @@ def test_small_box_fused_kernel(name, over):
 @pytest.mark.parametrize("nband", [1, 3, 64, 65])
 def test_small_box_band_counts(nband):
     cfg, plan, sph = _setup("c3k2")
-    plan.set_option("fft_path", 3)
     psi = synth.gen_psi(cfg, [s[2] for s in sph], nband=nband)
-    err = band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi))
-    assert err <= TOL, "nband=%d: %.3e" % (nband, err)
+    ref = oracle_apply(cfg, sph, psi)
+    for path in (3, 5):
+        plan.set_option("fft_path", path)
+        err = band_rel_err(gpu_apply(plan, psi), ref)
+        assert err <= TOL, "nband=%d fft_path=%d: %.3e" % (nband, path, err)
     plan.destroy()
 
 

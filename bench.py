@@ -205,7 +205,9 @@ def measure_config(name, hbm_gbs, steps=20, warmup=3):
     psi = synth.gen_psi_torch(cfg, kin_list, "cuda")
     hpsi = torch.empty_like(psi)
     geo = geometry(plan)
-    fft_bytes, g1, g2 = byte_flop_model(plan, geo, nband, 6.0)
+    sym = plan.nkpt == 1 and not np.any(np.asarray(cfg["kpt"][0]))
+    fpc = 4.0 if sym else 6.0
+    fft_bytes, g1, g2 = byte_flop_model(plan, geo, nband, fpc)
     for _ in range(warmup):
         plan.apply_h(psi, hpsi)
     torch.cuda.synchronize()
@@ -240,7 +242,7 @@ def measure_config(name, hbm_gbs, steps=20, warmup=3):
     dom = max(ph, key=lambda k: ph[k])
     out = {"workload": WORKLOADS[name], "ms_per_step": ms, "ms_per_step_back_to_back": warm, "bands_per_s": units / (ms * 1e-3),
            "launches_per_step": launches, "t_roof_ms": t_roof * 1e3, "frac": t_roof * 1e3 / ms,
-           "frac_vs_F_nl_8flop": (t_roof + gemm_s / 3.0) * 1e3 / ms,
+           "gemm_flops_per_cmac": fpc, "frac_vs_F_nl_8flop": (t_roof + gemm_s * (8.0 / fpc - 1.0)) * 1e3 / ms,
            "t_compulsory_ms": t_comp * 1e3, "frac_compulsory": t_comp * 1e3 / ms,
            "dominant_kernel": dom, "dominant_share": ph[dom] / max(sum(ph.values()), 1e-30),
            "phase_ms": {k: round(v, 5) for k, v in ph.items()}, "l2": "flushed between steps (512 MB write)", "steps": steps}
@@ -280,6 +282,7 @@ def main():
     ap.add_argument("--fft-path", type=int, default=0, help="dft_plan_set_option fft_path (experiments only)")
     ap.add_argument("--proj-mode", type=int, default=0, help="1 = factorised projectors FY.S (experiments only)")
     ap.add_argument("--gemm-3m", type=int, default=1, help="0 = 4-product complex GEMMs (experiments only)")
+    ap.add_argument("--gemm-sym", type=int, default=1, help="0 = complex GEMMs also at k = 0 (experiments only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (experiments only)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the e2e leg (experiments only)")
     ap.add_argument("--ref-bands", type=int, default=0)
@@ -320,6 +323,7 @@ def main():
     if args.fft_path:
         plan.set_option("fft_path", args.fft_path)
     plan.set_option("gemm_3m", args.gemm_3m)
+    plan.set_option("gemm_sym", args.gemm_sym)
     if args.proj_mode:
         plan.set_option("proj_mode", args.proj_mode)
     plan.set_vloc(torch.as_tensor(cfg["vloc"], device="cuda"))
@@ -330,7 +334,10 @@ def main():
     psi = synth.gen_psi_torch(cfg_r, kin_list, "cuda")
     hpsi = torch.empty_like(psi)
     geo = geometry(plan)
-    fpc = 6.0 if args.gemm_3m else 8.0
+    # flops per (projector, plane wave, band) of the GEMM variant that runs: 4 = real GEMMs on the half sphere (k = 0, the
+    # table is symmetric under G -> -G), 6 = Gauss / 3M complex, 8 = four-product complex
+    sym = bool(args.gemm_sym) and not args.proj_mode and plan.nkpt == 1 and not np.any(np.asarray(cfg["kpt"][0]))
+    fpc = 4.0 if sym else (6.0 if args.gemm_3m else 8.0)
     fft_bytes, g1_flops, g2_flops = byte_flop_model(plan, geo, nband, fpc)
     hbm_gbs, hbm_src = measured_peaks()
 
@@ -387,6 +394,10 @@ def main():
                                 "achieved": fl / (ph_ms[name] * 1e-3) / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                                 "flops_per_complex_mac": fpc,
                                 "frac_vs_F_nl_8flop": fl * (8.0 / fpc) / (ph_ms[name] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS}
+    if sym and ph_ms.get("pack_unpack", 0) > 0:     # split into symmetric halves + recombination: 2a and 4a bytes per band
+        sc_bytes = sum(6 * 16.0 * g_["npw"] * nband for g_ in geo)
+        per_kernel["sym_split_combine"] = {"bound": "hbm", "ms_per_step": ph_ms["pack_unpack"], "launches_per_step": ph_n["pack_unpack"],
+                                           "achieved": sc_bytes / (ph_ms["pack_unpack"] * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
     for v in per_kernel.values():
         v["frac"] = v["achieved"] / v["peak"]
     if not per_kernel:      # --cuda-graph: the per-kernel events are not recorded inside a graph replay
@@ -406,13 +417,14 @@ def main():
                 "peak_source": ("FP64 DMMA: 148 SM x 4 x 512 flop / 16 clk x 1.965 GHz (microbenchmark 37.06), "
                                 "DESIGN.md 8" if d["bound"] == "tensor" else hbm_src),
                 "share_of_step": d["ms_per_step"] / ms_step}
-    t_roof = sum(fft_bytes.values()) / (hbm_gbs * 1e9) + (g1_flops + g2_flops) / (FP64_PEAK_TFLOPS * 1e12)
+    sc_s = (sum(6 * 16.0 * g_["npw"] * nband for g_ in geo) / (hbm_gbs * 1e9)) if sym else 0.0
+    t_roof = sum(fft_bytes.values()) / (hbm_gbs * 1e9) + (g1_flops + g2_flops) / (FP64_PEAK_TFLOPS * 1e12) + sc_s
     t_roof8 = sum(fft_bytes.values()) / (hbm_gbs * 1e9) + (g1_flops + g2_flops) * (8.0 / fpc) / (FP64_PEAK_TFLOPS * 1e12)
     path = {"t_roof_ms": t_roof * 1e3, "frac": t_roof * 1e3 / ms_step,
             "frac_vs_F_nl_8flop": t_roof8 * 1e3 / ms_step,
             "definition": "sum_phases max(bytes/HBM_measured, flops/FP64_peak) / measured step time; GEMM flops = %g per "
-                          "complex multiply-add (the variant the kernels run); frac_vs_F_nl_8flop uses SURVEY.md's dense "
-                          "8-flop count F_nl" % fpc,
+                          "(projector, plane wave, band) (the variant the kernels run: 4 = real GEMMs on the half sphere at "
+                          "k = 0, 6 = Gauss, 8 = four products); frac_vs_F_nl_8flop uses SURVEY.md's dense 8-flop count F_nl" % fpc,
             "kernels": per_kernel}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,

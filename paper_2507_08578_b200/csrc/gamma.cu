@@ -89,18 +89,21 @@ int gamma_check_dij(const dft_plan *p, const double *dij) {
   return DFT_OK;
 }
 
-int gamma_build(dft_plan *p) {
-  if (p->gam) return DFT_OK;
-  if (p->nkpt != 1) { set_error("Gamma storage needs a plan with one k-point (has %d)", p->nkpt); return DFT_ERR_UNSUPPORTED; }
-  const KPoint &K = p->kp[0];
-  if (K.k[0] != 0.0 || K.k[1] != 0.0 || K.k[2] != 0.0) { set_error("Gamma storage needs k = 0"); return DFT_ERR_UNSUPPORTED; }
-  const int npw = K.npw, n1 = p->n[0], n2 = p->n[1], n3 = p->n[2];
-  if (p->natom > 0 && p->nproj > 0) {
+// check_dij: the Gamma STORAGE (dft_apply_h_gamma) needs a D_ij without odd-parity couplings; the tables alone (half
+// sphere, maps, rotated projector table) also serve the symmetric-table GEMMs of dft_apply_h at k = 0 (nonlocal.cu), which
+// take any D_ij.
+int gamma_build(dft_plan *p, bool check_dij) {
+  if (check_dij && p->natom > 0 && p->nproj > 0 && p->nkpt == 1) {
     std::vector<double> d((size_t)p->natom * p->lmax * p->lmax);
     DFT_CUDA_CHECK(cudaMemcpy(d.data(), p->d_dij, d.size() * sizeof(double), cudaMemcpyDeviceToHost));
     int rc = gamma_check_dij(p, d.data());
     if (rc) return rc;
   }
+  if (p->gam) return DFT_OK;
+  if (p->nkpt != 1) { set_error("Gamma storage needs a plan with one k-point (has %d)", p->nkpt); return DFT_ERR_UNSUPPORTED; }
+  const KPoint &K = p->kp[0];
+  if (K.k[0] != 0.0 || K.k[1] != 0.0 || K.k[2] != 0.0) { set_error("Gamma storage needs k = 0"); return DFT_ERR_UNSUPPORTED; }
+  const int npw = K.npw, n1 = p->n[0], n2 = p->n[1], n3 = p->n[2];
   GammaData *G = new GammaData();
   std::vector<int32_t> h2f, h2fneg, f2h(npw, 0);
   // position of a box index in the (ascending) full list
@@ -158,7 +161,7 @@ int gamma_build(dft_plan *p) {
 // psi, hpsi: [nband][nh] complex (device)
 int gamma_apply(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStream_t st, const Recurrence *rec) {
   GammaData *G = p->gam;
-  if (!G) { set_error("Gamma storage is not enabled (dft_plan_set_option gamma_real = 1)"); return DFT_ERR_NOT_READY; }
+  if (!G || !p->gamma_on) { set_error("Gamma storage is not enabled (dft_plan_set_option gamma_real = 1)"); return DFT_ERR_NOT_READY; }
   p->last_launches = 0;
   if (nband == 0 || G->nh == 0) return DFT_OK;
   const bool loc = (p->terms & 2) != 0, kin = (p->terms & 1) != 0, nl = (p->terms & 4) != 0 && p->nproj > 0;

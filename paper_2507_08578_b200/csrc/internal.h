@@ -89,6 +89,7 @@ struct GammaData {
 };
 
 struct NlMaps;
+struct SymMaps;
 void nl_maps_free(dft_plan *p);
 
 // timed kernel groups: 0-4 the five FFT passes, 5 GEMM-1, 6 D_ij, 7 GEMM-2, 8 the fused small-box local term (fft_small.cu),
@@ -177,8 +178,13 @@ struct dft_plan {
   int64_t last_launches = 0;
   bool nl_attr_done = false;   // cudaFuncSetAttribute of the GEMM kernels done on this plan's device
   dftb200::PhaseTimer timer;
+  dftb200::SymMaps *sym_maps = nullptr; // the same for the symmetric-table GEMMs at k = 0
   dftb200::NlMaps *nl_maps = nullptr;  // tensor maps of the table-mode GEMMs, kept between calls (nonlocal.cu)
-  dftb200::GammaData *gam = nullptr;   // built by option gamma_real = 1
+  dftb200::GammaData *gam = nullptr;   // half sphere + rotated table: built by option gamma_real = 1 or by the symmetric-table GEMMs
+  bool gamma_on = false;               // option gamma_real = 1 (dft_apply_h_gamma allowed, D_ij parity enforced)
+  int gemm_sym = 1;                    // 1 = at k = 0 run the projector GEMMs of dft_apply_h as real GEMMs on the half sphere (nonlocal.cu)
+  int sym_state = 0;                   // 0 = not tried, 1 = tables ready, -1 = this plan cannot (k != 0, several k-points, unpaired Nyquist index)
+  double *d_symx = nullptr; int64_t symx_bytes = 0;   // time-reversal-even/odd halves of the bands, [2 nband][nhalf] complex
   // two-component spinors (spinor.cu): Pauli components of the local potential, spin-dependent D
   double *d_vpauli = nullptr;          // [4][n3][n2][n1]: V0, Vx, Vy, Vz, each pre-scaled by 1/N
   double *d_dspin = nullptr;           // [natom][2][2][lmax][lmax] complex
@@ -261,7 +267,7 @@ int nonlocal_apply_spinor(dft_plan *p, const double *psi, double *hpsi, int nban
 int local_term(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStream_t st, const FftExtra *extra = nullptr);
 
 // --- gamma.cu / spinor.cu ------------------------------------------------------------------------
-int gamma_build(dft_plan *p);
+int gamma_build(dft_plan *p, bool check_dij);
 void gamma_free(dft_plan *p);
 int gamma_check_dij(const dft_plan *p, const double *dij_host);
 int gamma_apply(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStream_t st, const Recurrence *rec = nullptr);

@@ -860,7 +860,12 @@ struct NlMaps {
   const void *ptab = nullptr, *psi = nullptr, *cprj = nullptr;
   int bm1 = 0, nband_psi = -1, nband_c = -1;
 };
-void nl_maps_free(dft_plan *p) { delete p->nl_maps; p->nl_maps = nullptr; }
+struct SymMaps {
+  CUtensorMap mapP1, mapP2, mapX, mapC;
+  const void *ptab = nullptr, *x = nullptr, *cprj = nullptr;
+  int n2_x = -1, n2_c = -1;
+};
+void nl_maps_free(dft_plan *p) { delete p->nl_maps; p->nl_maps = nullptr; delete p->sym_maps; p->sym_maps = nullptr; }
 
 typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                              const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -935,6 +940,216 @@ static int choose_splitk(int tiles, int nslab, int sm_count, int nkpt) {
   return best;
 }
 
+// ---------------------------------------------------------------- symmetric-table GEMMs at k = 0
+// At k = 0 the projectors obey p(-G) = (-1)^l conj(p(G)) (real F, real Y_lm of parity l, conjugate phases), whatever psi is.
+// Any band is psi = psi_A + i psi_B with psi_A, psi_B time-reversal symmetric (c_A(G) = (c(G) + conj(c(-G)))/2,
+// c_B(G) = (c(G) - conj(c(-G)))/(2i)), and for a symmetric vector every projection is i^(l odd) times a REAL number obtained
+// from the half sphere alone (gamma.cu).  So both GEMMs run as REAL GEMMs over the interleaved (re, im) doubles of the
+// half sphere with 2 nband columns -- 4 flops per (projector, plane wave, band) instead of 8 (four products) or 6
+// (Gauss): gemm1_kernel<true> / gemm2_kernel<true> on the rotated half table of gamma.cu.  Unlike the Gamma STORAGE this
+// needs no symmetry of psi or D_ij: the step between the GEMMs works on the complex z_j = r^A_j + i r^B_j,
+//   <p_j|psi> = i^(l_j odd) z_j,   y_i = (-i)^(l_i odd) sum_j D_ij i^(l_j odd) z_j,   (V_nl psi)(+-G) = sum_i Pt_i(G)^(*) y_i,
+// i.e. h_A = Pt y_r, h_B = Pt y_i on the half sphere and (V_nl psi)(G) = h_A + i h_B, (V_nl psi)(-G) = conj(h_A) + i conj(h_B).
+// Exact up to rounding order, like the Gauss form.
+__global__ void sym_split_kernel(const double2 *__restrict__ psi, double2 *__restrict__ X, const int32_t *__restrict__ h2f,
+                                 const int32_t *__restrict__ h2fneg, int mpw, int nh) {
+  const int h = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+  if (h >= nh) return;
+  const double2 cp = psi[(size_t)b * mpw + h2f[h]], cm = psi[(size_t)b * mpw + h2fneg[h]];
+  X[(size_t)(2 * b) * nh + h] = make_double2(0.5 * (cp.x + cm.x), 0.5 * (cp.y - cm.y));
+  X[(size_t)(2 * b + 1) * nh + h] = make_double2(0.5 * (cp.y + cm.y), -0.5 * (cp.x - cm.x));
+}
+
+// part [nsplit][nproj][2 nband] real (GEMM-1 partial sums S); psi: the bands (for the G = 0 term); cpr: c' [2 nband][nproj]
+// complex with zero imaginary halves (rows 2b, 2b+1 = Re y, Im y), or, when dij is null, cprj_out [nband][nproj] = <p|psi>
+__global__ void dij_sym_kernel(const double *__restrict__ part, double2 *__restrict__ cpr, const double *__restrict__ dij,
+                               const int32_t *__restrict__ typat, const int32_t *__restrict__ nlmn,
+                               const int32_t *__restrict__ atom_first, const int32_t *__restrict__ rowpar,
+                               const double *__restrict__ p0, const double2 *__restrict__ psi, int mpw, int lmax, int nproj,
+                               int nband, int nsplit) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+  if (b >= nband) return;
+  const int nl = nlmn[typat[a]], first = atom_first[a], n2 = 2 * nband;
+  // c_A(0) = Re psi(0), c_B(0) = Im psi(0); G = 0 has the smallest box index, so it is entry 0 of the band
+  const double2 c00 = psi[(size_t)b * mpw];
+  const double ca0 = c00.x, cb0 = c00.y;
+  const int32_t *par = rowpar + (size_t)a * lmax;
+  double2 t[DIJ_MAXL];    // <p_j|psi> = i^(l_j odd) z_j
+  for (int jj = 0; jj < nl; jj++) t[jj] = make_double2(0.0, 0.0);
+  for (int s = 0; s < nsplit; s++) {
+    const double *src = part + ((size_t)s * nproj + first) * n2 + 2 * b;
+#pragma unroll 4
+    for (int jj = 0; jj < nl; jj++) {
+      const double2 v = *reinterpret_cast<const double2 *>(src + (size_t)jj * n2);
+      t[jj].x += v.x; t[jj].y += v.y;
+    }
+  }
+  for (int jj = 0; jj < nl; jj++) {
+    const double za = 2.0 * t[jj].x - p0[first + jj] * ca0, zb = 2.0 * t[jj].y - p0[first + jj] * cb0;
+    t[jj] = par[jj] ? make_double2(-zb, za) : make_double2(za, zb);
+  }
+  if (!dij) {
+    double2 *dst = cpr + (size_t)b * nproj + first;
+    for (int ii = 0; ii < nl; ii++) dst[ii] = t[ii];
+    return;
+  }
+  const double *D = dij + (size_t)a * lmax * lmax;
+  double2 *da = cpr + (size_t)(2 * b) * nproj + first, *db = da + nproj;
+  for (int ii = 0; ii < nl; ii++) {
+    double sr = 0.0, si = 0.0;
+    for (int jj = 0; jj < nl; jj++) { const double d = D[ii * lmax + jj]; sr += d * t[jj].x; si += d * t[jj].y; }
+    const double yr = par[ii] ? si : sr, yi = par[ii] ? -sr : si;     // y = (-i)^(l_i odd) (sr + i si)
+    da[ii] = make_double2(yr, 0.0); db[ii] = make_double2(yi, 0.0);
+  }
+}
+
+// hpsi[b][g] = (accumulate ? hpsi : 0) + diag[g] psi + h_A(+-G) + i h_B(+-G), then the optional recurrence combination
+__global__ void sym_combine_kernel(const double2 *__restrict__ Y, const double2 *__restrict__ psi, double2 *__restrict__ hpsi,
+                                   const double *const *kin, const int32_t *__restrict__ f2h, int npw, int mpw, int nh,
+                                   int accumulate, int with_kin, int cheb, double sh, double sy, double sx,
+                                   const double2 *__restrict__ xprev) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+  if (g >= npw) return;
+  const int t = f2h[g], h = (t > 0 ? t : -t) - 1;
+  double2 a = Y[(size_t)(2 * b) * nh + h], c = Y[(size_t)(2 * b + 1) * nh + h];
+  if (t < 0) { a.y = -a.y; c.y = -c.y; }
+  double2 r = make_double2(a.x - c.y, a.y + c.x);
+  const size_t off = (size_t)b * mpw + g;
+  if (with_kin) { const double2 x = psi[off]; const double kg = kin[0][g]; r.x += kg * x.x; r.y += kg * x.y; }
+  if (accumulate) { const double2 hh = hpsi[off]; r.x += hh.x; r.y += hh.y; }
+  if (cheb) {
+    const double2 y = psi[off], xp = sx != 0.0 ? xprev[off] : make_double2(0.0, 0.0);
+    r.x = sh * r.x + sy * y.x + sx * xp.x; r.y = sh * r.y + sy * y.y + sx * xp.y;
+  }
+  hpsi[off] = r;
+}
+
+// Can this plan run the symmetric-table GEMMs?  Builds the half-sphere tables at the first call.
+static bool sym_ready(dft_plan *p) {
+  if (p->sym_state == 0) {
+    p->sym_state = -1;
+    if (p->nkpt == 1 && p->nproj > 0 && p->mpw > 0 && p->kp[0].k[0] == 0.0 && p->kp[0].k[1] == 0.0 && p->kp[0].k[2] == 0.0) {
+      if (gamma_build(p, false) == DFT_OK && p->gam && p->gam->nh > 0) p->sym_state = 1;
+    }
+  }
+  return p->sym_state == 1;
+}
+
+static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, cudaStream_t st,
+                              const double *dmat, const double *const *diag, double *cprj_out, const Recurrence *rec, double *spsi) {
+  GammaData *G = p->gam;
+  if (!p->gam_attr_done) {
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm1_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, NL_SMEM));
+    p->gam_attr_done = true;
+  }
+  const int nh = G->nh, nproj = p->nproj, mpw = p->mpw, n2 = 2 * nband;
+  const double *const *d_kin = diag ? diag : p->d_kinptr;
+  if (!dmat) dmat = p->d_dij;
+  int rc;
+  const int64_t need_x = (int64_t)n2 * nh * 16;
+  if (need_x > p->symx_bytes || !p->d_symx) {
+    if (p->d_symx) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_symx); p->d_symx = nullptr; p->symx_bytes = 0; }
+    if (cudaMalloc(&p->d_symx, need_x + 256) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes for the symmetric halves of the bands", (long long)need_x); return DFT_ERR_ALLOC; }
+    p->symx_bytes = need_x;
+  }
+  double2 *X = reinterpret_cast<double2 *>(p->d_symx);
+  Gemm1Params q1;
+  q1.nproj = nproj; q1.nband = n2; q1.nslab = (nh + 7) / 8;
+  q1.tiles_m = (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (n2 + NL_BN - 1) / NL_BN;
+  int ns = p->splitk > 0 ? p->splitk : choose_splitk(q1.tiles_m * q1.tiles_n, q1.nslab, p->sm_count, 1);
+  if (ns > q1.nslab) ns = q1.nslab;
+  q1.slabs_per_split = (q1.nslab + ns - 1) / ns;
+  ns = (q1.nslab + q1.slabs_per_split - 1) / q1.slabs_per_split;
+  q1.nsplit = ns;
+  const int64_t need_part = (int64_t)ns * nproj * n2 * 8, need_cprj = (int64_t)n2 * nproj * 16;
+  if (need_part > p->part_bytes || !p->d_part) {
+    if (p->d_part) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_part); p->d_part = nullptr; }
+    if (cudaMalloc(&p->d_part, need_part) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes of split-K scratch", (long long)need_part); p->part_bytes = 0; return DFT_ERR_ALLOC; }
+    p->part_bytes = need_part;
+  }
+  if (need_cprj > p->cprj_bytes || !p->d_cprj) {
+    if (p->d_cprj) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_cprj); p->d_cprj = nullptr; }
+    if (cudaMalloc(&p->d_cprj, need_cprj) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes for cprj", (long long)need_cprj); p->cprj_bytes = 0; return DFT_ERR_ALLOC; }
+    p->cprj_bytes = need_cprj;
+  }
+  q1.part = reinterpret_cast<double2 *>(p->d_part);
+  // tensor maps, kept between calls like those of the complex path
+  SymMaps *C = p->sym_maps;
+  if (!C) { C = new SymMaps(); p->sym_maps = C; }
+  const uint64_t rowb = (uint64_t)nh * 16;
+  if (C->ptab != G->d_ptab) {
+    if ((rc = make_map(p, &C->mapP1, G->d_ptab, 2 * (uint64_t)nh, nproj, 1, rowb, rowb * nproj, NL_BM))) return rc;
+    cuuint64_t dims[4] = {16, (cuuint64_t)nproj, ((cuuint64_t)nh + 7) / 8, 1};
+    cuuint64_t strides[3] = {rowb, 128, rowb * nproj};
+    cuuint32_t box[4] = {16, 8, NL_BM / 8, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = ((EncodeFn)p->encode_fn)(&C->mapP2, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, G->d_ptab, dims, strides, box, estr,
+                                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (symmetric GEMM-2 P map) failed (%d)", (int)r); return DFT_ERR_CUDA; }
+    C->ptab = G->d_ptab;
+  }
+  if (C->x != X || C->n2_x != n2) {
+    if ((rc = make_map(p, &C->mapX, X, 2 * (uint64_t)nh, n2, 1, rowb, rowb * n2, NL_BN))) return rc;
+    C->x = X; C->n2_x = n2;
+  }
+  if (C->cprj != p->d_cprj || C->n2_c != n2) {
+    if ((rc = make_map(p, &C->mapC, p->d_cprj, 2 * (uint64_t)nproj, n2, 1, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * n2, NL_BN))) return rc;
+    C->cprj = p->d_cprj; C->n2_c = n2;
+  }
+  const double2 *cpsi = reinterpret_cast<const double2 *>(psi);
+  // ---- halves, GEMM-1 (real)
+  phase_begin(p, 9, st);
+  sym_split_kernel<<<dim3((nh + 255) / 256, nband), 256, 0, st>>>(cpsi, X, G->d_h2f, G->d_h2fneg, mpw, nh);
+  phase_end(p, 9, st, 1);
+  phase_begin(p, 5, st);
+  gemm1_kernel<true><<<dim3(q1.tiles_m * q1.tiles_n, ns, 1), NL_THREADS, NL_SMEM, st>>>(C->mapP1, C->mapX, q1);
+  phase_end(p, 5, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  // ---- D_ij (complex step on z = r_A + i r_B)
+  phase_begin(p, 6, st);
+  dij_sym_kernel<<<dim3((nband + 127) / 128, p->natom, 1), 128, 0, st>>>(
+      p->d_part, reinterpret_cast<double2 *>(cprj_out ? cprj_out : p->d_cprj), cprj_out ? nullptr : dmat, p->d_typat, p->d_nlmn,
+      p->d_atom_first, G->d_rowpar, G->d_p0, cpsi, mpw, p->lmax, nproj, nband, ns);
+  phase_end(p, 6, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  if (cprj_out) return DFT_OK;
+  // ---- GEMM-2 (real) into the halves buffer, then recombination + diagonal + accumulation
+  Gemm2Params q2;
+  q2.nproj = nproj; q2.nband = n2; q2.mpw = nh; q2.nslab = (nproj + 7) / 8;
+  q2.tiles_n = q1.tiles_n; q2.accumulate = 0; q2.with_kin = 0; q2.with_nl = 1;
+  q2.npw = G->d_npw; q2.kin = G->d_kinptr; q2.psi = X; q2.hpsi = X;
+  q2.cheb = 0; q2.sh = 1.0; q2.sy = 0.0; q2.sx = 0.0; q2.xprev = nullptr;
+  const int tiles_m2 = (nh + NL_BM - 1) / NL_BM;
+  const dim3 cgrid((mpw + 255) / 256, nband);
+  phase_begin(p, 7, st);
+  gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS, NL_SMEM, st>>>(C->mapP2, C->mapC, q2);
+  phase_end(p, 7, st, 1);
+  phase_begin(p, 9, st);
+  sym_combine_kernel<<<cgrid, 256, 0, st>>>(X, cpsi, reinterpret_cast<double2 *>(hpsi), d_kin, G->d_f2h, p->kp[0].npw, mpw, nh, accumulate,
+                                            with_kin, rec != nullptr, rec ? rec->sh : 1.0, rec ? rec->sy : 0.0, rec ? rec->sx : 0.0,
+                                            rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr);
+  phase_end(p, 9, st, 1);
+  DFT_CUDA_CHECK(cudaGetLastError());
+  if (spsi) {   // S psi from the same projections (dft_apply_hs): s_ij step, GEMM-2, recombination with a unit diagonal
+    phase_begin(p, 6, st);
+    dij_sym_kernel<<<dim3((nband + 127) / 128, p->natom, 1), 128, 0, st>>>(
+        p->d_part, reinterpret_cast<double2 *>(p->d_cprj), p->d_sij, p->d_typat, p->d_nlmn, p->d_atom_first, G->d_rowpar, G->d_p0, cpsi,
+        mpw, p->lmax, nproj, nband, ns);
+    phase_end(p, 6, st, 1);
+    phase_begin(p, 7, st);
+    gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS, NL_SMEM, st>>>(C->mapP2, C->mapC, q2);
+    phase_end(p, 7, st, 1);
+    phase_begin(p, 9, st);
+    sym_combine_kernel<<<cgrid, 256, 0, st>>>(X, cpsi, reinterpret_cast<double2 *>(spsi), p->d_oneptr, G->d_f2h, p->kp[0].npw, mpw, nh, 0, 1,
+                                              0, 1.0, 0.0, 0.0, nullptr);
+    phase_end(p, 9, st, 1);
+    DFT_CUDA_CHECK(cudaGetLastError());
+  }
+  return DFT_OK;
+}
+
 // dmat: per-atom matrices applied between the GEMMs (null = the plan's D_ij); diag: per-k-point device pointers to the
 // diagonal multiplying psi in the epilogue (null = the kinetic energies); cprj_out (device, [nkpt][nband][nproj]
 // complex): if given, only GEMM-1 and the split-K reduction run and <p|psi> is written there.
@@ -956,6 +1171,9 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     DFT_CUDA_CHECK(cudaFuncSetAttribute(gemm2_fac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FD_SMEM));
     p->nl_attr_done = true;
   }
+  // k = 0: the projector table is symmetric under G -> -G and both GEMMs run as real GEMMs on the half sphere
+  if (with_nl && p->gemm_sym && p->proj_mode == 0 && !dspin && sym_ready(p))
+    return nonlocal_apply_sym(p, psi, hpsi, nband, accumulate, with_kin, st, dmat, diag, cprj_out, rec, spsi);
   const int32_t *d_npw = p->d_npw;
   const double *const *d_kin = diag ? diag : p->d_kinptr;
   if (!dmat) dmat = p->d_dij;

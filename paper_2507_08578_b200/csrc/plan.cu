@@ -67,6 +67,7 @@ static void destroy_plan(dft_plan *p) {
   cudaFree(p->ws_own); cudaFree(p->d_part); cudaFree(p->d_cprj); cudaFree(p->d_stage_in); cudaFree(p->d_stage_out);
   gamma_free(p);
   nl_maps_free(p);
+  cudaFree(p->d_symx);
   cudaFree(p->d_vpauli); cudaFree(p->d_dspin); cudaFree(p->d_spin_tmp);
   if (p->host_stream) cudaStreamDestroy(p->host_stream);
   if (p->h2d_stream) cudaStreamDestroy(p->h2d_stream);
@@ -458,7 +459,7 @@ int dft_set_dij(dft_plan *p, const double *dij) {
   size_t n = (size_t)p->natom * p->lmax * p->lmax;
   if (n == 0) return DFT_OK;
   if (!dij) { set_error("dij is NULL"); return DFT_ERR_INVALID_ARG; }
-  if (p->gam) { int rcg = gamma_check_dij(p, dij); if (rcg) return rcg; }
+  if (p->gamma_on) { int rcg = gamma_check_dij(p, dij); if (rcg) return rcg; }
   // an apply enqueued earlier on a non-blocking stream may still read D_ij: wait for the device before replacing it
   DFT_CUDA_CHECK(cudaDeviceSynchronize());
   DFT_CUDA_CHECK(cudaMemcpy(p->d_dij, dij, n * sizeof(double), cudaMemcpyHostToDevice));
@@ -589,10 +590,18 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
   }
   if (!strcmp(key, "gamma_real")) {
     if (value < 0 || value > 1) { set_error("gamma_real = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
-    if (value == 1) return gamma_build(p);
-    DFT_CUDA_CHECK(cudaDeviceSynchronize());
-    gamma_free(p);
+    if (value == 1) {
+      int rcg = gamma_build(p, true);
+      if (rcg) return rcg;
+      p->gamma_on = true;
+      return DFT_OK;
+    }
+    p->gamma_on = false;     // the tables stay: the symmetric-table GEMMs of dft_apply_h use them too
     return DFT_OK;
+  }
+  if (!strcmp(key, "gemm_sym")) {
+    if (value < 0 || value > 1) { set_error("gemm_sym = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->gemm_sym = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "host_groups")) {
     if (value < 1 || value > 64) { set_error("host_groups = %lld outside 1..64", (long long)value); return DFT_ERR_INVALID_ARG; }
@@ -622,7 +631,7 @@ int dft_apply_h(dft_plan *p, const double *psi, double *hpsi, int32_t nband, voi
 
 int dft_plan_get_kg_gamma(const dft_plan *p, int32_t *nhalf, int32_t *kg, int32_t *igfft, double *kin) {
   if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
-  if (!p->gam) { set_error("Gamma storage is not enabled (dft_plan_set_option gamma_real = 1)"); return DFT_ERR_NOT_READY; }
+  if (!p->gam || !p->gamma_on) { set_error("Gamma storage is not enabled (dft_plan_set_option gamma_real = 1)"); return DFT_ERR_NOT_READY; }
   const GammaData &G = *p->gam;
   if (nhalf) *nhalf = G.nh;
   if (kg && G.nh) memcpy(kg, G.h_kg.data(), sizeof(int32_t) * 3 * (size_t)G.nh);

@@ -60,10 +60,12 @@ def test_both_gemm_variants_agree(name):
     for terms in (7, 4):
         ref = oracle_apply(cfg, sph, psi, terms=terms, method=1 if name == "aniso" else 2)
         plan.set_option("terms", terms)
-        for g3 in (0, 1):
-            plan.set_option("gemm_3m", g3)
-            err = band_rel_err(gpu_apply(plan, psi), ref)
-            assert err <= TOL, "%s gemm_3m=%d terms=%d: rel err %.3e" % (name, g3, terms, err)
+        for sym in (0, 1):               # gemm_sym = 1 (default): at k = 0 both GEMMs are real GEMMs on the half sphere
+            plan.set_option("gemm_sym", sym)
+            for g3 in (0, 1):
+                plan.set_option("gemm_3m", g3)
+                err = band_rel_err(gpu_apply(plan, psi), ref)
+                assert err <= TOL, "%s gemm_sym=%d gemm_3m=%d terms=%d: rel err %.3e" % (name, sym, g3, terms, err)
     plan.destroy()
 
 
@@ -142,7 +144,8 @@ def test_small_box_fused_kernel(name, over):
         for terms in (7, 2):
             plan.set_option("terms", terms)
             got = gpu_apply(plan, psi)
-            assert plan.last_launches() == (4 if terms == 7 else 1)
+            gamma = cfg["nkpt"] == 1 and not np.any(cfg["kpt"][0])      # symmetric-table GEMMs at k = 0: split + recombination
+            assert plan.last_launches() == ((6 if gamma else 4) if terms == 7 else 1)
             err = band_rel_err(got, oracle_apply(cfg, sph, psi, terms=terms, method=method))
             assert err <= TOL, "%s fft_path=%d terms=%d: rel err %.3e" % (name, path, terms, err)
             for ik in range(plan.nkpt):
@@ -205,8 +208,9 @@ def test_overlap_operator_and_cprj(name):
     for ik, (kg, ig, kin) in enumerate(sph):
         assert np.array_equal(ident[ik][:, :len(ig)], psi[ik][:, :len(ig)]) and np.all(ident[ik][:, len(ig):] == 0)
     plan.set_sij(sij)
-    for g3 in (1, 0):
-        plan.set_option("gemm_3m", g3)
+    for g3 in (1, 0, 2):
+        plan.set_option("gemm_3m", g3 & 1)
+        plan.set_option("gemm_sym", 1 if g3 == 2 else 0)      # last round: the default (real GEMMs at k = 0)
         got = plan.apply_s(tpsi).cpu().numpy()
         cp = plan.get_cprj(tpsi).cpu().numpy()
         for ik, (kg, ig, kin) in enumerate(sph):
@@ -217,11 +221,37 @@ def test_overlap_operator_and_cprj(name):
             cref = oracle.cprj(cfg, ik, kg, psi[ik][:, :len(ig)]).T          # [nband][nproj]
             cerr = float(np.max(np.linalg.norm(cp[ik] - cref, axis=1) / np.linalg.norm(cref, axis=1)))
             assert cerr <= TOL, "%s cprj gemm_3m=%d k=%d: %.3e" % (name, g3, ik, cerr)
-    assert plan.last_launches() == 2
+    assert plan.last_launches() == (3 if name == "c4m" else 2)    # cprj: (split at k = 0,) GEMM-1, reduction
     plan.destroy()
 
 
-@pytest.mark.parametrize("name", ["c1m", "aniso", "c3k2"])
+@pytest.mark.parametrize("name", ["c1m", "c4m", "aniso", "c3k2"])
+def test_apply_hs_one_set_of_projections(name):
+    """dft_apply_hs: H psi and S psi from ONE GEMM-1 (PAPER.md :479-:485) must equal the separate applications' oracle
+    results; at k = 0 (c4m) both with the real symmetric-table GEMMs (default) and with the complex kernels."""
+    cfg, plan, sph = _setup(name)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    rng = np.random.default_rng(5)
+    sij = rng.standard_normal(cfg["dij"].shape) * 0.3
+    sij = 0.5 * (sij + sij.transpose(0, 2, 1))
+    plan.set_sij(sij)
+    tpsi = torch.as_tensor(psi, device="cuda")
+    href = oracle_apply(cfg, sph, psi, method=1 if name == "aniso" else 2)
+    for sym in (1, 0):
+        plan.set_option("gemm_sym", sym)
+        h, s_ = plan.apply_hs(tpsi)
+        torch.cuda.synchronize()
+        assert band_rel_err(h.cpu().numpy(), href) <= TOL
+        got = s_.cpu().numpy()
+        for ik, (kg, ig, kin) in enumerate(sph):
+            ref = oracle.apply_s(cfg, ik, kg, psi[ik], sij)
+            err = float(np.max(np.linalg.norm(got[ik] - ref, axis=1) / np.linalg.norm(ref, axis=1)))
+            assert err <= TOL, "%s S psi of apply_hs gemm_sym=%d k=%d: %.3e" % (name, sym, ik, err)
+            assert np.all(got[ik][:, len(ig):] == 0)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("name", ["c1m", "aniso", "c3k2", "c2m"])
 def test_chebyshev_filter(name):
     """dft_chebyshev_filter (PAPER.md :458, :489) against the oracle's recurrence; T_n grows like cosh(n acosh x) outside
     [-1, 1], so the per-band relative error is what is bounded."""
@@ -234,8 +264,8 @@ def test_chebyshev_filter(name):
         for deg in (0, 1, 4, 7):
             t = torch.as_tensor(psi, device="cuda").clone()
             got = plan.chebyshev_filter(t, deg, cen, e).cpu().numpy()
-            if plan.nkpt == 1:
-                assert plan.last_launches() == (4 if small_box_ok(plan) else 8) * deg
+            if plan.nkpt == 1:      # c2m is at k = 0: its GEMMs are the real ones, with a split and a recombination kernel
+                assert plan.last_launches() == ((4 if small_box_ok(plan) else 8) + (2 if name == "c2m" else 0)) * deg
             for ik, (kg, ig, kin) in enumerate(sph):
                 ref = oracle.chebyshev_filter(cfg, ik, kg, ig, kin, psi[ik], deg, cen, e, method=1 if name == "aniso" else 2)
                 npw = len(ig)
@@ -524,7 +554,8 @@ def _sampled_full_size(name, per_tile, nvariant):
     sub = sample[::max(1, len(sample) // max(nvariant, ntile))]
     pos = [sample.index(b) for b in sub]
     assert len(sub) >= 16 and len({b // 64 for b in sub}) == ntile
-    for key, val in (("gemm_3m", 0), ("proj_mode", 1)):
+    # (the default at k = 0 is the symmetric-table real GEMMs; gemm_sym = 0 gives the complex 3M kernels, then the others)
+    for key, val in (("gemm_sym", 0), ("gemm_3m", 0), ("proj_mode", 1)):
         plan.set_option(key, val)
         out2 = plan.apply_h(psi)
         torch.cuda.synchronize()

@@ -205,7 +205,7 @@ def measure_config(name, hbm_gbs, steps=20, warmup=3):
     psi = synth.gen_psi_torch(cfg, kin_list, "cuda")
     hpsi = torch.empty_like(psi)
     geo = geometry(plan)
-    sym = plan.nkpt == 1 and not np.any(np.asarray(cfg["kpt"][0]))
+    sym = plan.nkpt == 1 and not np.any(np.asarray(cfg["kpt"][0])) and float(plan.nproj) * plan.mpw * nband >= 1e8
     fpc = 4.0 if sym else 6.0
     fft_bytes, g1, g2 = byte_flop_model(plan, geo, nband, fpc)
     for _ in range(warmup):
@@ -282,7 +282,7 @@ def main():
     ap.add_argument("--fft-path", type=int, default=0, help="dft_plan_set_option fft_path (experiments only)")
     ap.add_argument("--proj-mode", type=int, default=0, help="1 = factorised projectors FY.S (experiments only)")
     ap.add_argument("--gemm-3m", type=int, default=1, help="0 = 4-product complex GEMMs (experiments only)")
-    ap.add_argument("--gemm-sym", type=int, default=1, help="0 = complex GEMMs also at k = 0 (experiments only)")
+    ap.add_argument("--gemm-sym", type=int, default=2, help="0 = complex GEMMs also at k = 0, 1 = real GEMMs at k = 0 even for tiny cells (experiments only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (experiments only)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the e2e leg (experiments only)")
     ap.add_argument("--ref-bands", type=int, default=0)
@@ -336,7 +336,8 @@ def main():
     geo = geometry(plan)
     # flops per (projector, plane wave, band) of the GEMM variant that runs: 4 = real GEMMs on the half sphere (k = 0, the
     # table is symmetric under G -> -G), 6 = Gauss / 3M complex, 8 = four-product complex
-    sym = bool(args.gemm_sym) and not args.proj_mode and plan.nkpt == 1 and not np.any(np.asarray(cfg["kpt"][0]))
+    sym = (bool(args.gemm_sym) and not args.proj_mode and plan.nkpt == 1 and not np.any(np.asarray(cfg["kpt"][0]))
+           and (args.gemm_sym == 1 or float(plan.nproj) * plan.mpw * nband >= 1e8))
     fpc = 4.0 if sym else (6.0 if args.gemm_3m else 8.0)
     fft_bytes, g1_flops, g2_flops = byte_flop_model(plan, geo, nband, fpc)
     hbm_gbs, hbm_src = measured_peaks()

@@ -182,7 +182,7 @@ struct dft_plan {
   dftb200::NlMaps *nl_maps = nullptr;  // tensor maps of the table-mode GEMMs, kept between calls (nonlocal.cu)
   dftb200::GammaData *gam = nullptr;   // half sphere + rotated table: built by option gamma_real = 1 or by the symmetric-table GEMMs
   bool gamma_on = false;               // option gamma_real = 1 (dft_apply_h_gamma allowed, D_ij parity enforced)
-  int gemm_sym = 1;                    // 1 = at k = 0 run the projector GEMMs of dft_apply_h as real GEMMs on the half sphere (nonlocal.cu)
+  int gemm_sym = 2;                    // at k = 0 run the projector GEMMs of dft_apply_h as real GEMMs on the half sphere (nonlocal.cu): 0 never, 1 always, 2 = when large enough
   int sym_state = 0;                   // 0 = not tried, 1 = tables ready, -1 = this plan cannot (k != 0, several k-points, unpaired Nyquist index)
   double *d_symx = nullptr; int64_t symx_bytes = 0;   // time-reversal-even/odd halves of the bands, [2 nband][nhalf] complex
   // two-component spinors (spinor.cu): Pauli components of the local potential, spin-dependent D

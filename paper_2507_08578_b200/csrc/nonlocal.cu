@@ -37,6 +37,14 @@ constexpr int NL_CONSUMERS = 8;   // warps: 4 (M) x 2 (N), 32 x 32 complex outpu
 // the kernel at 168.  Lane 0 of warp 0 therefore also issues the TMA loads, NL_PREFETCH slabs ahead,
 // into a stage every warp released two iterations earlier (so it practically never waits).
 constexpr int NL_THREADS = NL_CONSUMERS * 32;
+// The four-product kernels add a producer warpgroup (warps 8-11, lane 0 of warp 8 issues the TMA loads): with the loads
+// issued by a consumer the whole ring was paced by that one warp, and the warps that ran ahead of it starved at the full
+// barrier (ncu: 16 % of the samples of the real GEMM-2 of the symmetric-table path; 91.5 % DMMA).  Twelve warps would cap
+// every thread at 168 registers, so the producer group gives its registers back (setmaxnreg 24) and the two consumer
+// groups take 232 each: 2 x 32 x 232 + 32 x 24 = 15 616 of the 16 384 registers of a sub-partition.
+constexpr int NL_THREADS_P = NL_THREADS + 128;
+__device__ __forceinline__ void reg_dealloc_producer() { asm volatile("setmaxnreg.dec.sync.aligned.u32 24;"); }
+__device__ __forceinline__ void reg_alloc_consumer() { asm volatile("setmaxnreg.inc.sync.aligned.u32 232;"); }
 constexpr int NL_STAGE_A = NL_BM * 128;   // 16 KB
 constexpr int NL_STAGE_B = NL_BN * 128;   // 8 KB
 constexpr int NL_STAGE_BYTES = NL_STAGE_A + NL_STAGE_B;
@@ -168,7 +176,7 @@ __device__ __forceinline__ Pipe pipe_setup(unsigned char *smem_raw) {
 // ---------------------------------------------------------------- GEMM-1: projection (split-K partials)
 // grid: (tiles_m*tiles_n, nsplit, nkpt)
 template <bool REAL, int MB = 4>
-__global__ void __launch_bounds__(NL_THREADS, 1)
+__global__ void __launch_bounds__(NL_THREADS_P, 1)
 gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapPsi, Gemm1Params Q) {
   constexpr int BM = 32 * MB;            // rows of P per CTA tile (the TMA box of mapP has BM rows)
   extern __shared__ unsigned char smem_raw[];
@@ -186,9 +194,13 @@ gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
     tma_load_3d(st, &mapP, &P.full[s], (s0 + j) * 16, tm * BM, ik);
     tma_load_3d(st + NL_STAGE_A, &mapPsi, &P.full[s], (s0 + j) * 16, tn * NL_BN, ik);
   };
-  const bool producer = (threadIdx.x == 0);
-  if (producer)
-    for (int j = 0; j < NL_PREFETCH && j < ns; j++) issue(j);
+  if (warp >= NL_CONSUMERS) {      // the producer group: keeps the whole ring in flight, independent of any consumer's pace
+    reg_dealloc_producer();
+    if (warp == NL_CONSUMERS && lane == 0)
+      for (int j = 0; j < ns; j++) issue(j);
+    return;
+  }
+  reg_alloc_consumer();
   const int wm = warp >> 1, wn = warp & 1;
   double cre[4][4][2], cim[4][4][2];
 #pragma unroll
@@ -196,8 +208,6 @@ gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
 #pragma unroll
     for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
   for (int it = 0; it < ns; it++) {
-    if (producer && it + NL_PREFETCH < ns) issue(it + NL_PREFETCH);
-    __syncwarp();
     int s = it % NL_STAGES;
     mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
     const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
@@ -329,7 +339,7 @@ __global__ void dij_spinor_kernel(const double2 *__restrict__ part, double2 *__r
 // ---------------------------------------------------------------- GEMM-2: back-projection + kinetic epilogue
 // grid: (tiles_n * tiles_m, 1, nkpt), band tiles fastest so that concurrent CTAs share a slab of P in L2
 template <bool REAL>
-__global__ void __launch_bounds__(NL_THREADS, 1)
+__global__ void __launch_bounds__(NL_THREADS_P, 1)
 gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapC, Gemm2Params Q) {
   extern __shared__ unsigned char smem_raw[];
   Pipe P = pipe_setup(smem_raw);
@@ -345,9 +355,13 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
     tma_load_4d(st, &mapP, &P.full[s], 0, j * 8, tm * (NL_BM / 8), ik);
     tma_load_3d(st + NL_STAGE_A, &mapC, &P.full[s], j * 16, tn * NL_BN, ik);
   };
-  const bool producer = (threadIdx.x == 0);
-  if (producer)
-    for (int j = 0; j < NL_PREFETCH && j < ns; j++) issue(j);
+  if (warp >= NL_CONSUMERS) {      // the producer group
+    reg_dealloc_producer();
+    if (warp == NL_CONSUMERS && lane == 0)
+      for (int j = 0; j < ns; j++) issue(j);
+    return;
+  }
+  reg_alloc_consumer();
   const int wm = warp >> 1, wn = warp & 1;
   double cre[4][4][2], cim[4][4][2];
 #pragma unroll
@@ -355,8 +369,6 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
 #pragma unroll
     for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
   for (int it = 0; it < ns; it++) {
-    if (producer && it + NL_PREFETCH < ns) issue(it + NL_PREFETCH);
-    __syncwarp();
     int s = it % NL_STAGES;
     mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
     const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
@@ -966,7 +978,7 @@ __global__ void dij_sym_kernel(const double *__restrict__ part, double2 *__restr
                                const int32_t *__restrict__ typat, const int32_t *__restrict__ nlmn,
                                const int32_t *__restrict__ atom_first, const int32_t *__restrict__ rowpar,
                                const double *__restrict__ p0, const double2 *__restrict__ psi, int mpw, int lmax, int nproj,
-                               int nband, int nsplit) {
+                               int nband, int nsplit, int ldc) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
   if (b >= nband) return;
   const int nl = nlmn[typat[a]], first = atom_first[a], n2 = 2 * nband;
@@ -994,7 +1006,7 @@ __global__ void dij_sym_kernel(const double *__restrict__ part, double2 *__restr
     return;
   }
   const double *D = dij + (size_t)a * lmax * lmax;
-  double2 *da = cpr + (size_t)(2 * b) * nproj + first, *db = da + nproj;
+  double2 *da = cpr + (size_t)(2 * b) * ldc + first, *db = da + ldc;      // ldc: row pitch of c' (complex elements)
   for (int ii = 0; ii < nl; ii++) {
     double sr = 0.0, si = 0.0;
     for (int jj = 0; jj < nl; jj++) { const double d = D[ii * lmax + jj]; sr += d * t[jj].x; si += d * t[jj].y; }
@@ -1062,7 +1074,9 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
   q1.slabs_per_split = (q1.nslab + ns - 1) / ns;
   ns = (q1.nslab + q1.slabs_per_split - 1) / q1.slabs_per_split;
   q1.nsplit = ns;
-  const int64_t need_part = (int64_t)ns * nproj * n2 * 8, need_cprj = (int64_t)n2 * nproj * 16;
+  // row pitch of c': a power-of-two pitch (4096 projectors = 64 KB) makes the 64 rows of a TMA box of GEMM-2 collide in L2
+  const int ldc = (nproj % 256 == 0) ? nproj + 8 : nproj;
+  const int64_t need_part = (int64_t)ns * nproj * n2 * 8, need_cprj = (int64_t)n2 * ldc * 16;
   if (need_part > p->part_bytes || !p->d_part) {
     if (p->d_part) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_part); p->d_part = nullptr; }
     if (cudaMalloc(&p->d_part, need_part) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %lld bytes of split-K scratch", (long long)need_part); p->part_bytes = 0; return DFT_ERR_ALLOC; }
@@ -1095,7 +1109,7 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
     C->x = X; C->n2_x = n2;
   }
   if (C->cprj != p->d_cprj || C->n2_c != n2) {
-    if ((rc = make_map(p, &C->mapC, p->d_cprj, 2 * (uint64_t)nproj, n2, 1, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * n2, NL_BN))) return rc;
+    if ((rc = make_map(p, &C->mapC, p->d_cprj, 2 * (uint64_t)nproj, n2, 1, (uint64_t)ldc * 16, (uint64_t)ldc * 16 * n2, NL_BN))) return rc;
     C->cprj = p->d_cprj; C->n2_c = n2;
   }
   const double2 *cpsi = reinterpret_cast<const double2 *>(psi);
@@ -1104,14 +1118,14 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
   sym_split_kernel<<<dim3((nh + 255) / 256, nband), 256, 0, st>>>(cpsi, X, G->d_h2f, G->d_h2fneg, mpw, nh);
   phase_end(p, 9, st, 1);
   phase_begin(p, 5, st);
-  gemm1_kernel<true><<<dim3(q1.tiles_m * q1.tiles_n, ns, 1), NL_THREADS, NL_SMEM, st>>>(C->mapP1, C->mapX, q1);
+  gemm1_kernel<true><<<dim3(q1.tiles_m * q1.tiles_n, ns, 1), NL_THREADS_P, NL_SMEM, st>>>(C->mapP1, C->mapX, q1);
   phase_end(p, 5, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   // ---- D_ij (complex step on z = r_A + i r_B)
   phase_begin(p, 6, st);
   dij_sym_kernel<<<dim3((nband + 127) / 128, p->natom, 1), 128, 0, st>>>(
       p->d_part, reinterpret_cast<double2 *>(cprj_out ? cprj_out : p->d_cprj), cprj_out ? nullptr : dmat, p->d_typat, p->d_nlmn,
-      p->d_atom_first, G->d_rowpar, G->d_p0, cpsi, mpw, p->lmax, nproj, nband, ns);
+      p->d_atom_first, G->d_rowpar, G->d_p0, cpsi, mpw, p->lmax, nproj, nband, ns, ldc);
   phase_end(p, 6, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   if (cprj_out) return DFT_OK;
@@ -1124,7 +1138,7 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
   const int tiles_m2 = (nh + NL_BM - 1) / NL_BM;
   const dim3 cgrid((mpw + 255) / 256, nband);
   phase_begin(p, 7, st);
-  gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS, NL_SMEM, st>>>(C->mapP2, C->mapC, q2);
+  gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS_P, NL_SMEM, st>>>(C->mapP2, C->mapC, q2);
   phase_end(p, 7, st, 1);
   phase_begin(p, 9, st);
   sym_combine_kernel<<<cgrid, 256, 0, st>>>(X, cpsi, reinterpret_cast<double2 *>(hpsi), d_kin, G->d_f2h, p->kp[0].npw, mpw, nh, accumulate,
@@ -1136,10 +1150,10 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
     phase_begin(p, 6, st);
     dij_sym_kernel<<<dim3((nband + 127) / 128, p->natom, 1), 128, 0, st>>>(
         p->d_part, reinterpret_cast<double2 *>(p->d_cprj), p->d_sij, p->d_typat, p->d_nlmn, p->d_atom_first, G->d_rowpar, G->d_p0, cpsi,
-        mpw, p->lmax, nproj, nband, ns);
+        mpw, p->lmax, nproj, nband, ns, ldc);
     phase_end(p, 6, st, 1);
     phase_begin(p, 7, st);
-    gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS, NL_SMEM, st>>>(C->mapP2, C->mapC, q2);
+    gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS_P, NL_SMEM, st>>>(C->mapP2, C->mapC, q2);
     phase_end(p, 7, st, 1);
     phase_begin(p, 9, st);
     sym_combine_kernel<<<cgrid, 256, 0, st>>>(X, cpsi, reinterpret_cast<double2 *>(spsi), p->d_oneptr, G->d_f2h, p->kp[0].npw, mpw, nh, 0, 1,
@@ -1172,7 +1186,10 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     p->nl_attr_done = true;
   }
   // k = 0: the projector table is symmetric under G -> -G and both GEMMs run as real GEMMs on the half sphere
-  if (with_nl && p->gemm_sym && p->proj_mode == 0 && !dspin && sym_ready(p))
+  // (option gemm_sym: 1 = wherever possible, 2 = automatic: only where the GEMMs are large enough to pay for the two extra
+  // launches, nproj npw nband >= 1e8 complex multiply-adds; tiny cells are launch-bound)
+  if (with_nl && (p->gemm_sym == 1 || (p->gemm_sym == 2 && (double)p->nproj * p->mpw * nband >= 1e8)) && p->proj_mode == 0 && !dspin &&
+      sym_ready(p))
     return nonlocal_apply_sym(p, psi, hpsi, nband, accumulate, with_kin, st, dmat, diag, cprj_out, rec, spsi);
   const int32_t *d_npw = p->d_npw;
   const double *const *d_kin = diag ? diag : p->d_kinptr;
@@ -1271,10 +1288,10 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     f1.slabs_per_split = q1.slabs_per_split; f1.tiles_n = q1.tiles_n;
     f1.blk_atom = p->d_blk_atom; f1.blk_frow = p->d_blk_frow; f1.blk_first = p->d_blk_first; f1.blk_nl = p->d_blk_nl; f1.part = q1.part;
     gemm1_fac_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), FC_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1, f1);
-  } else if (skinny_mb == 1) gemm1_kernel<false, 1><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
-  else if (skinny_mb == 2) gemm1_kernel<false, 2><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  } else if (skinny_mb == 1) gemm1_kernel<false, 1><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  else if (skinny_mb == 2) gemm1_kernel<false, 2><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   else if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
-  else gemm1_kernel<false><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  else gemm1_kernel<false><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   phase_end(p, 5, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   // ---- D_ij
@@ -1304,7 +1321,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_blk_atom,
                                                                                       p->d_blk_frow, p->d_blk_first, p->nfrow);
   } else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
-  else gemm2_kernel<false><<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  else gemm2_kernel<false><<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP2, mapC, q2);
   phase_end(p, 7, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   if (spsi) {
@@ -1320,7 +1337,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     if (fac) gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_blk_atom,
                                                                                                p->d_blk_frow, p->d_blk_first, p->nfrow);
     else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
-    else gemm2_kernel<false><<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+    else gemm2_kernel<false><<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP2, mapC, q2);
     phase_end(p, 7, st, 1);
     DFT_CUDA_CHECK(cudaGetLastError());
   }
@@ -1389,7 +1406,7 @@ int nonlocal_apply_gamma(dft_plan *p, const double *psi, double *hpsi, int nband
   }
   if ((rc = make_map(p, &mapC, p->d_cprj, 2 * (uint64_t)nproj, nband, 1, (uint64_t)nproj * 16, (uint64_t)nproj * 16 * nband, NL_BN))) return rc;
   phase_begin(p, 5, st);
-  gemm1_kernel<true><<<dim3(q1.tiles_m * q1.tiles_n, ns, 1), NL_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
+  gemm1_kernel<true><<<dim3(q1.tiles_m * q1.tiles_n, ns, 1), NL_THREADS_P, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   phase_end(p, 5, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   phase_begin(p, 6, st);
@@ -1406,7 +1423,7 @@ int nonlocal_apply_gamma(dft_plan *p, const double *psi, double *hpsi, int nband
   q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr;
   const int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
   phase_begin(p, 7, st);
-  gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS_P, NL_SMEM, st>>>(mapP2, mapC, q2);
   phase_end(p, 7, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   return DFT_OK;

@@ -600,7 +600,7 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     return DFT_OK;
   }
   if (!strcmp(key, "gemm_sym")) {
-    if (value < 0 || value > 1) { set_error("gemm_sym = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if (value < 0 || value > 2) { set_error("gemm_sym = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->gemm_sym = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "host_groups")) {

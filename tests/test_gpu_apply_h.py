@@ -33,6 +33,11 @@ def test_small_cells_all_terms_and_isolations(name):
         assert err <= TOL, "%s terms=%d: rel err %.3e" % (name, terms, err)
         for ik in range(plan.nkpt):                      # pad entries are written as 0
             assert np.all(got[ik][:, plan.npw[ik]:] == 0)
+        if terms in (7, 4) and plan.nkpt == 1 and not np.any(cfg["kpt"][0]):
+            plan.set_option("gemm_sym", 1)               # k = 0: real GEMMs on the half sphere (automatic only for large cells)
+            err = band_rel_err(gpu_apply(plan, psi), ref)
+            assert err <= TOL, "%s terms=%d gemm_sym=1: rel err %.3e" % (name, terms, err)
+            plan.set_option("gemm_sym", 2)
     plan.destroy()
 
 
@@ -144,8 +149,7 @@ def test_small_box_fused_kernel(name, over):
         for terms in (7, 2):
             plan.set_option("terms", terms)
             got = gpu_apply(plan, psi)
-            gamma = cfg["nkpt"] == 1 and not np.any(cfg["kpt"][0])      # symmetric-table GEMMs at k = 0: split + recombination
-            assert plan.last_launches() == ((6 if gamma else 4) if terms == 7 else 1)
+            assert plan.last_launches() == (4 if terms == 7 else 1)
             err = band_rel_err(got, oracle_apply(cfg, sph, psi, terms=terms, method=method))
             assert err <= TOL, "%s fft_path=%d terms=%d: rel err %.3e" % (name, path, terms, err)
             for ik in range(plan.nkpt):
@@ -210,7 +214,7 @@ def test_overlap_operator_and_cprj(name):
     plan.set_sij(sij)
     for g3 in (1, 0, 2):
         plan.set_option("gemm_3m", g3 & 1)
-        plan.set_option("gemm_sym", 1 if g3 == 2 else 0)      # last round: the default (real GEMMs at k = 0)
+        plan.set_option("gemm_sym", 1 if g3 == 2 else 0)      # last round: the real GEMMs at k = 0 (default for large cells)
         got = plan.apply_s(tpsi).cpu().numpy()
         cp = plan.get_cprj(tpsi).cpu().numpy()
         for ik, (kg, ig, kin) in enumerate(sph):
@@ -259,6 +263,7 @@ def test_chebyshev_filter(name):
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     kmax = max(float(s[2].max()) for s in sph)
     cen, e = 0.5 * kmax + 1.0, 0.5 * kmax + 0.5           # damp roughly [0.5, kmax + 1.5] Ha
+    plan.set_option("gemm_sym", 1)                          # c2m (k = 0): force the real symmetric-table GEMMs (automatic only for large cells)
     for g3 in (1, 0):
         plan.set_option("gemm_3m", g3)
         for deg in (0, 1, 4, 7):

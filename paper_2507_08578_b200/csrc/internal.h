@@ -164,7 +164,7 @@ struct dft_plan {
   // host staging for dft_apply_h_host
   double *d_stage_in = nullptr, *d_stage_out = nullptr; int64_t stage_bytes = 0;
   cudaStream_t host_stream = nullptr, h2d_stream = nullptr, d2h_stream = nullptr;
-  int host_groups = 5;     // dft_apply_h_host: band groups whose copies overlap the kernels of their neighbours
+  int host_groups = 6;     // dft_apply_h_host: band groups whose copies overlap the kernels of their neighbours
   // TMA
   void *encode_fn = nullptr;   // cuTensorMapEncodeTiled
   double *d_wgt = nullptr; int64_t wgt_count = 0;    // device copy of the band weights of dft_accumulate_density

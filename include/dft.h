@@ -120,13 +120,18 @@ int dft_plan_workspace_bytes(const dft_plan *p, int32_t nband, int64_t *min_byte
  * bit 2 non-local, bit 3 meta-GGA term; default 15), "splitk" (GEMM-1 K splits, 0 = automatic), "proj_mode" (0 = default: projector table materialised in
  * device memory; 1 = factorised projectors FY.S evaluated inside both GEMMs; the table is freed (and rebuilt when the option
  * returns to 0; dft_plan_get_projectors gives DFT_ERR_NOT_READY meanwhile); an atom's projectors are taken in blocks of 8 and the form-factor rows of all types (8
- * per block) must not exceed 32, else DFT_ERR_UNSUPPORTED), "host_groups" (dft_apply_h_host only: band groups, default 5,
+ * per block) must not exceed 32, else DFT_ERR_UNSUPPORTED), "host_groups" (dft_apply_h_host only: band groups, default 6,
  * whose host<->device copies overlap the kernels of the neighbouring groups), "gemm_3m" (1 = default: three real
  * products per complex multiply-add in the projector GEMMs, 0 = four; same result up to rounding), "fft_path" (0 = automatic:
  * register-resident two-stage transforms where the box length factorises, their strided passes fed by a
- * TMA shared-memory ring; 1 = generic shared-memory Stockham kernels only; 2 = register-resident
- * transforms without the TMA ring; all compute the same transform).  Unknown key or bad
- * value -> DFT_ERR_INVALID_ARG.                                                                  */
+ * TMA shared-memory ring, or - when one band's pruned working set fits one SM's shared memory - the whole local term
+ * fused in ONE kernel; 1 = generic shared-memory Stockham kernels only; 2 = register-resident transforms without the
+ * TMA ring; 3 = the fused small-box kernel (DFT_ERR_UNSUPPORTED if the plan does not fit); 4 = automatic without it;
+ * 5 = its run-time-dispatched variant; all compute the same transform), "gemm_sym" (k = 0 only: the projector table is
+ * symmetric under G -> -G, so both projector GEMMs of dft_apply_h can run as REAL GEMMs on the half sphere, 4 instead of
+ * 6 flops per projector, plane wave and band, same result up to rounding, any D_ij; 0 = never, 1 = wherever possible,
+ * 2 = default: when nproj * npw * nband >= 1e8; the first such call builds a second table of half the size),
+ * "gamma_real" (1 = enable dft_apply_h_gamma, see there).  Unknown key or bad value -> DFT_ERR_INVALID_ARG.  */
 int dft_plan_set_option(dft_plan *p, const char *key, int64_t value);
 
 /* hpsi = H psi for nband bands per k-point.  psi and hpsi are DEVICE memory, layout

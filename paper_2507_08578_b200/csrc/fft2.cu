@@ -43,6 +43,11 @@ __device__ __forceinline__ cplx cmulc(cplx a, cplx b) {   // a * conj(b)
   return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
 }
 constexpr int F2_THREADS = 256;
+#ifndef F2C_THREADS_N
+#define F2C_THREADS_N 256
+#endif
+constexpr int F2C_THREADS = F2C_THREADS_N;   // pass C ring kernel: threads per CTA (tile = F2C_THREADS / max radix lines, a multiple of 8)
+constexpr int F2C_PER_SM = F2C_THREADS_N <= 128 ? 4 : 2;
 __host__ __device__ constexpr int imax(int a, int b) { return a > b ? a : b; }
 __host__ __device__ constexpr int pad8(int len, int want) { return len + (((want - len) % 8) + 8) % 8; }   // smallest >= len congruent to want mod 8
 
@@ -468,12 +473,12 @@ fft2_b_inv_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cp
 // ---- pass C: box {XT x, one y, all occupied planes} of T2; a CTA owns a contiguous range of tiles with the
 //      band fastest, so its V(r)/N tile [n3][XT] is staged in shared memory once per (y, x-tile) group.
 template <int R1, int R2>
-__global__ void __launch_bounds__(F2_THREADS, 2)
+__global__ void __launch_bounds__(F2C_THREADS, F2C_PER_SM)
 fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *__restrict__ T2,
                    const double *__restrict__ vloc, RingParams Q) {
   constexpr int NS = imax(R1, R2);
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr int XT = (F2_THREADS / NS) & ~7;     // a function of the radices only: all tile addressing is immediate
+  constexpr int XT = (F2C_THREADS / NS) & ~7;     // a function of the radices only: all tile addressing is immediate
   constexpr int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
   constexpr int exn = imax(R1 * KSa, R2 * KSb);
   unsigned char *stages = smem_raw;
@@ -758,7 +763,7 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
   // (128-byte runs, 8 full warps for NS = 15, 16) that fits the block
   int XT = choose_xt2(G.n1, NS), nxt = (G.n1 + XT - 1) / XT;
   if (pass == 2) {
-    XT = (F2_THREADS / NS) & ~7;
+    XT = (F2C_THREADS / NS) & ~7;
     if (XT < 8) return DFT_ERR_UNSUPPORTED;
     int64_t nxy = (int64_t)G.n1 * G.n2;
     if (XT > nxy) return DFT_ERR_UNSUPPORTED;    // tiny planes: the plain kernel
@@ -779,6 +784,9 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
   const size_t fixed = ex + extra + 8 * 8;
   const size_t budget2 = (size_t)(p->smem_per_sm / 2) - 1024, budget1 = (size_t)p->smem_optin;
   int S = 0, per_sm = 2;
+  if (pass == 2 && F2C_PER_SM > 2)        // small pass-C tiles: as many CTAs per SM as shared memory allows (each is its own barrier domain)
+    for (int c = F2C_PER_SM; c > 2 && !S; c--)
+      if (fixed + 2 * (size_t)Q.stage_stride <= (size_t)(p->smem_per_sm / c) - 1024) { S = 2; per_sm = c; }
   for (int s = 4; s >= 2 && !S; s--)
     if (fixed + (size_t)s * Q.stage_stride <= budget2) S = s;
   if (!S) {

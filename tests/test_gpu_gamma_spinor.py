@@ -114,7 +114,7 @@ def _gamma_full_size(name, per_tile):
     for t0 in range(0, nband, 64):
         t1 = min(nband, t0 + 64)
         sample.update((t0, t1 - 1))
-        sample.update(int(v) for v in rng.choice(np.arange(t0 + 1, t1 - 1), size=per_tile - 2, replace=False))
+        sample.update(int(v) for v in rng.choice(np.arange(t0 + 1, t1 - 1), size=min(per_tile - 2, t1 - t0 - 2), replace=False))
     sample = sorted(sample)
     psi = synth.gen_psi_torch(cfg, [hkin], "cuda")[0]
     out = plan.apply_h_gamma(psi)
@@ -130,11 +130,11 @@ def _gamma_full_size(name, per_tile):
 
 
 def test_gamma_c2_full_size_sample():
-    _gamma_full_size("c2", 4)        # 7 tiles x 4 = 28 of 432 bands, nhalf 62 145
+    _gamma_full_size("c2", 10)       # 7 tiles x up to 10 = 66 of 432 bands, nhalf 62 145
 
 
 def test_gamma_c4_full_size_sample():
-    _gamma_full_size("c4", 2)        # 16 tiles x 2 = 32 of 1024 bands, nhalf 147 834
+    _gamma_full_size("c4", 4)        # 16 tiles x 4 = 64 of 1024 bands, nhalf 147 834
 
 
 # ------------------------------------------------------------------------------------------------ spinors

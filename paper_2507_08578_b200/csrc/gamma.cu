@@ -166,6 +166,9 @@ int gamma_apply(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStr
   if (nband == 0 || G->nh == 0) return DFT_OK;
   const bool loc = (p->terms & 2) != 0, kin = (p->terms & 1) != 0, nl = (p->terms & 4) != 0 && p->nproj > 0;
   if (loc && !p->vloc_set) { set_error("dft_apply_h_gamma called before dft_set_vloc"); return DFT_ERR_NOT_READY; }
+  // terms this entry point does not carry (a vector potential also breaks the time-reversal symmetry the storage rests on)
+  if (p->vecpot_on) { set_error("dft_apply_h_gamma: a vector potential is set (H does not commute with time reversal)"); return DFT_ERR_UNSUPPORTED; }
+  if ((p->terms & 8) && p->vtau_set) { set_error("dft_apply_h_gamma: the meta-GGA term is not available in Gamma storage (option terms, bit 3)"); return DFT_ERR_UNSUPPORTED; }
   int rc;
   const int nh = G->nh, mpw = p->mpw, npw = p->kp[0].npw;
   if (loc) {

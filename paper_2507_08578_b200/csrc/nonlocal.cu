@@ -1189,7 +1189,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   // (option gemm_sym: 1 = wherever possible, 2 = automatic: only where the GEMMs are large enough to pay for the two extra
   // launches, nproj npw nband >= 1e8 complex multiply-adds; tiny cells are launch-bound)
   if (with_nl && (p->gemm_sym == 1 || (p->gemm_sym == 2 && (double)p->nproj * p->mpw * nband >= 1e8)) && p->proj_mode == 0 && !dspin &&
-      sym_ready(p))
+      nband <= 32767 && sym_ready(p))
     return nonlocal_apply_sym(p, psi, hpsi, nband, accumulate, with_kin, st, dmat, diag, cprj_out, rec, spsi);
   const int32_t *d_npw = p->d_npw;
   const double *const *d_kin = diag ? diag : p->d_kinptr;
@@ -1431,8 +1431,9 @@ int nonlocal_apply_gamma(dft_plan *p, const double *psi, double *hpsi, int nband
 
 int nonlocal_apply_spinor(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, bool with_nl,
                           cudaStream_t st) {
-  return nonlocal_apply(p, psi, hpsi, 2 * nband, accumulate, with_kin, with_nl, st, nullptr, nullptr, nullptr, nullptr, nullptr,
-                        p->dspin_set ? p->d_dspin : nullptr);
+  // (a vector potential changes the kinetic diagonal of both components alike)
+  return nonlocal_apply(p, psi, hpsi, 2 * nband, accumulate, with_kin, with_nl, st, nullptr, p->vecpot_on ? p->d_kinaptr : nullptr, nullptr,
+                        nullptr, nullptr, p->dspin_set ? p->d_dspin : nullptr);
 }
 
 }  // namespace dftb200

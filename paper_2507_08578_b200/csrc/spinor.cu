@@ -56,6 +56,7 @@ int spinor_apply(dft_plan *p, const double *psi, double *hpsi, int nband, cudaSt
   if (nband == 0 || p->mpw == 0 || p->nkpt == 0) return DFT_OK;
   const bool loc = (p->terms & 2) != 0, kin = (p->terms & 1) != 0, nl = (p->terms & 4) != 0 && p->nproj > 0;
   if (loc && !p->vspin_set) { set_error("dft_apply_h_spinor called before dft_set_vloc_spinor"); return DFT_ERR_NOT_READY; }
+  if ((p->terms & 8) && p->vtau_set) { set_error("dft_apply_h_spinor: the meta-GGA term is not available for spinors (option terms, bit 3)"); return DFT_ERR_UNSUPPORTED; }
   int rc;
   const int rows = 2 * nband;
   const int64_t n = p->nbox;

@@ -93,6 +93,12 @@ def test_gamma_refusals():
     with pytest.raises(dft.DftError) as e:                   # a later D_ij that breaks time reversal
         dft.dft_set_dij(plan.h, cfg["dij"])
     assert e.value.code == dft.DFT_ERR_INVALID_ARG
+    plan.set_vector_potential([0.1, 0.0, -0.2])               # A != 0 breaks time reversal: refused, not ignored
+    with pytest.raises(dft.DftError) as e:
+        plan.apply_h_gamma(torch.zeros((1, 142), dtype=torch.complex128, device="cuda"))
+    assert e.value.code == dft.DFT_ERR_UNSUPPORTED
+    plan.set_vector_potential(None)
+    plan.apply_h_gamma(torch.zeros((1, 142), dtype=torch.complex128, device="cuda"))
     plan.set_option("gamma_real", 0)
     plan.destroy()
     cfg = synth.make_config("c1m")                           # k = (1/4, 1/4, 1/4)
@@ -176,6 +182,23 @@ def test_spinor_all_terms_and_paths(name):
     got = _spinor_gpu(plan, psi)
     ref = plan.apply_h(torch.as_tensor(base, device="cuda")).cpu().numpy().reshape(got.shape)
     assert band_rel_err(got, ref) <= 1e-12
+    plan.destroy()
+
+
+def test_spinor_with_vector_potential():
+    """Velocity gauge (PAPER.md :340): the kinetic diagonal 1/2 |k+G+A|^2 acts on both components."""
+    cfg = synth.make_config("c0")
+    plan = make_plan(cfg)
+    sph = lib_spheres(plan)
+    v4, dspin = synth.spinor_inputs(cfg)
+    plan.set_vloc_spinor(torch.as_tensor(v4, device="cuda"))
+    plan.set_dij_spinor(dspin)
+    a = [0.3, -0.1, 0.2]
+    plan.set_vector_potential(a)
+    kg, ig, kin = sph[0]
+    psi = synth.gen_psi(cfg, [kin], nband=8).reshape(1, 4, 2, plan.mpw)
+    ref = oracle.apply_h_spinor(cfg, 0, kg, ig, oracle.kin_vecpot(cfg["rprimd"], cfg["kpt"][0], kg, a), psi[0], v4, dspin, method=1)
+    assert band_rel_err(_spinor_gpu(plan, psi), ref[None]) <= TOL
     plan.destroy()
 
 

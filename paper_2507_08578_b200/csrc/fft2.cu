@@ -548,11 +548,12 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
     }
     __syncthreads();
     if (s < R1) {
+      // The second exchange is IN PLACE: this thread writes its R2 results exactly where it read its R2 inputs
+      // (row s, slots j2), so no other thread's pending read is overwritten and no barrier is needed before the
+      // writes; the last stage then reads sm[a][s] -- the slots the same thread fills again in the next tile's first
+      // stage -- so the barrier at the end of the tile is not needed either: two CTA barriers per tile instead of four.
 #pragma unroll
       for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KSa + j2 * XT + px];
-    }
-    __syncthreads();
-    if (s < R1) {
       Dft<R2, +1>::run(v);
 #pragma unroll
       for (int k2 = 0; k2 < R2; k2++) v[k2] = cscale(v[k2], vs[(s + R1 * k2) * XT + px]);
@@ -560,12 +561,12 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
 #pragma unroll
       for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], tws[s * cc]);
 #pragma unroll
-      for (int cc = 0; cc < R2; cc++) sm[cc * KSb + s * XT + px] = v[cc];
+      for (int cc = 0; cc < R2; cc++) sm[s * KSa + cc * XT + px] = v[cc];
     }
     __syncthreads();
     if (s < R2) {
 #pragma unroll
-      for (int a = 0; a < R1; a++) v[a] = sm[s * KSb + a * XT + px];
+      for (int a = 0; a < R1; a++) v[a] = sm[a * KSa + s * XT + px];
       Dft<R1, -1>::run(v);
       cplx *base = T2 + (size_t)b * G.t2_band + xy;
 #pragma unroll
@@ -575,7 +576,6 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
       for (int d = 0; d < R1; d++)
         if ((smask >> d) & 1) ((hmask >> d) & 1 ? base2 : base1)[(size_t)(R2 * d) * pstride] = v[d];
     }
-    __syncthreads();
     if (++st == Q.S) { st = 0; ph ^= 1; }
     if (++b == Q.nb) { b = 0; newgroup = true; g++; }
   }

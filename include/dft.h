@@ -216,6 +216,10 @@ int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, 
  * `stream` without host synchronisation (scratch is allocated at the first call of a given size).              */
 int dft_plan_get_kg_gamma(const dft_plan *p, int32_t *nhalf, int32_t *kg, int32_t *igfft, double *kin);
 int dft_apply_h_gamma(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);
+/* dft_chebyshev_filter in Gamma storage: psi DEVICE in/out [nband][nhalf], work DEVICE 2 * nband * nhalf complex128; the
+ * same recurrence with dft_apply_h_gamma as H (for degree >= 1 the result has Im psi(0) = 0).                        */
+int dft_chebyshev_filter_gamma(dft_plan *p, double *psi, double *work, int32_t nband, int32_t degree, double center,
+                               double halfwidth, void *stream);
 
 /* Two-component spinors (PAPER.md :448 "all types of magnetism": non-collinear magnetism, spin-orbit coupling;
  * SURVEY.md 8(f) row 4; reading 27).  psi = (psi_up, psi_dn): DEVICE [nkpt][nband][2][mpw] complex128.

@@ -354,6 +354,23 @@ def apply_h_gamma(cfg, kg, igfft, kin, psi_half, method=2, terms=ALL, vloc=None,
     return res
 
 
+def chebyshev_filter_gamma(cfg, kg, igfft, kin, psi_half, degree, center, halfwidth, method=2, vloc=None, dij=None):
+    """The recurrence of chebyshev_filter (reading 21) with apply_h_gamma as H; Im psi(0) of the input is
+    ignored (reading 26), i.e. T_0 is the symmetric vector itself."""
+    psi = np.array(np.atleast_2d(psi_half), np.complex128)
+    if degree == 0:
+        return psi
+    ih, _ = gamma_half(kg)
+    psi[:, len(ih):] = 0
+    psi[:, 0] = psi[:, 0].real
+    H = lambda x: apply_h_gamma(cfg, kg, igfft, kin, x, method=method, vloc=vloc, dij=dij)
+    t_prev = psi
+    t_cur = (H(t_prev) - center * t_prev) / halfwidth
+    for _ in range(1, degree):
+        t_prev, t_cur = t_cur, 2.0 * (H(t_cur) - center * t_cur) / halfwidth - t_prev
+    return t_cur
+
+
 # ---------------------------------------------------------------- NEXT row 4: two-component spinors
 # PAPER.md :448 ("all types of magnetism": non-collinear magnetism, spin-orbit coupling), SURVEY.md 8(f) 4; DESIGN.md
 # reading 27.  psi = (psi_up, psi_dn), each a plane-wave vector on the same sphere.

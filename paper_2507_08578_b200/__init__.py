@@ -35,7 +35,7 @@ PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather
 SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_workspace_bytes", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_apply_hs", "dft_get_cprj", "dft_chebyshev_filter",
            "dft_set_vector_potential", "dft_accumulate_density", "dft_accumulate_tau",
-           "dft_set_vtau", "dft_plan_get_kg_gamma", "dft_apply_h_gamma", "dft_set_vloc_spinor", "dft_set_dij_spinor",
+           "dft_set_vtau", "dft_plan_get_kg_gamma", "dft_apply_h_gamma", "dft_chebyshev_filter_gamma", "dft_set_vloc_spinor", "dft_set_dij_spinor",
            "dft_apply_h_spinor",
            "dft_set_vloc", "dft_set_workspace", "dft_plan_set_option", "dft_apply_h", "dft_apply_h_host",
            "dft_plan_last_launches", "dft_plan_set_timing", "dft_plan_phase_ms", "dft_plan_destroy", "dft_last_error")
@@ -97,6 +97,8 @@ def lib():
     L.dft_get_cprj.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_plan_get_kg_gamma.argtypes = [C.c_void_p, _ip, _ip, _ip, _dp]
     L.dft_apply_h_gamma.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    L.dft_chebyshev_filter_gamma.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
+                                             C.c_void_p]
     L.dft_set_vloc_spinor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.dft_set_dij_spinor.argtypes = [C.c_void_p, _dp]
     L.dft_apply_h_spinor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
@@ -259,6 +261,10 @@ def dft_apply_h_gamma(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream=0):
     _check(lib().dft_apply_h_gamma(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream))
 
 
+def dft_chebyshev_filter_gamma(plan, psi_dev_ptr, work_dev_ptr, nband, degree, center, halfwidth, stream=0):
+    _check(lib().dft_chebyshev_filter_gamma(plan, psi_dev_ptr, work_dev_ptr, nband, degree, center, halfwidth, stream))
+
+
 def dft_set_vloc_spinor(plan, v4_dev_ptr, stream=0):
     _check(lib().dft_set_vloc_spinor(plan, v4_dev_ptr, stream))
 
@@ -373,6 +379,17 @@ class Plan:
         assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.is_contiguous() and hpsi.shape == psi.shape
         dft_apply_h_gamma(self.h, psi.data_ptr(), hpsi.data_ptr(), psi.shape[0], torch.cuda.current_stream().cuda_stream)
         return hpsi
+
+    def chebyshev_filter_gamma(self, psi, degree, center, halfwidth, work=None):
+        """In place, Gamma storage: psi [nband][nhalf] := T_degree((H - center)/halfwidth) psi."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.dim() == 2
+        if work is None:
+            work = torch.empty(2 * psi.numel(), dtype=torch.complex128, device=psi.device)
+        assert work.is_cuda and work.dtype == torch.complex128 and work.numel() >= 2 * psi.numel()
+        dft_chebyshev_filter_gamma(self.h, psi.data_ptr(), work.data_ptr(), psi.shape[0], degree, center, halfwidth,
+                                   torch.cuda.current_stream().cuda_stream)
+        return psi
 
     def set_vloc_spinor(self, v4):
         """v4: torch float64 CUDA tensor [4][n3][n2][n1] = V_upup, V_dndn, Re V_updn, Im V_updn."""

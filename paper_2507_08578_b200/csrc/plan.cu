@@ -730,18 +730,11 @@ int dft_set_vector_potential(dft_plan *p, const double *a_cart) {
   DFT_GUARD_END
 }
 
-int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, int32_t degree, double center,
-                         double halfwidth, void *stream) {
-  DFT_GUARD_BEGIN
-  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
-  if (nband < 0 || degree < 0) { set_error("nband = %d, degree = %d: negative", nband, degree); return DFT_ERR_INVALID_ARG; }
-  if (!(halfwidth > 0.0) || !(center == center)) { set_error("halfwidth must be > 0 and center finite"); return DFT_ERR_INVALID_ARG; }
-  p->last_launches = 0;
-  const size_t n = (size_t)p->nkpt * nband * p->mpw * 2;   // doubles per psi-sized array
-  if (n == 0 || degree == 0) return DFT_OK;
-  if (!psi || !work) { set_error("null psi/work"); return DFT_ERR_INVALID_ARG; }
-  if (((uintptr_t)psi & 15) || ((uintptr_t)work & 15)) { set_error("psi/work must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
-  cudaStream_t st = (cudaStream_t)stream;
+}  // extern "C"
+// the three-term recurrence around any of the apply functions (full sphere or Gamma storage); n = doubles per psi-sized array
+template <typename Apply>
+static int chebyshev_impl(dft_plan *p, double *psi, double *work, size_t n, int32_t degree, double center, double halfwidth,
+                          cudaStream_t st, Apply apply) {
   // three psi-sized arrays rotate: x = T_{j-1}, y = T_j, w receives T_{j+1} from the GEMM-2 epilogue
   double *buf[3] = {psi, work, work + n};
   int ix = 2, iy = 0, iw = 1;
@@ -751,7 +744,7 @@ int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, 
     if (j == 0) { rec.sh = 1.0 / halfwidth; rec.sy = -center / halfwidth; rec.sx = 0.0; rec.xprev = nullptr; }
     else { rec.sh = 2.0 / halfwidth; rec.sy = -2.0 * center / halfwidth; rec.sx = -1.0; rec.xprev = buf[ix]; }
     // T_{j+1} goes to the third array: the FFT passes store V_loc T_j there before the epilogue reads T_{j-1}
-    int rc = apply_impl(p, buf[iy], buf[iw], nband, st, &rec);
+    int rc = apply(buf[iy], buf[iw], &rec);
     if (rc) return rc;
     launches += p->last_launches;
     int t = ix; ix = iy; iy = iw; iw = t;
@@ -759,6 +752,46 @@ int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, 
   p->last_launches = launches;
   if (buf[iy] != psi) DFT_CUDA_CHECK(cudaMemcpyAsync(psi, buf[iy], n * sizeof(double), cudaMemcpyDeviceToDevice, st));
   return DFT_OK;
+}
+
+static int chebyshev_args(dft_plan *p, const double *psi, const double *work, int32_t nband, int32_t degree, double center, double halfwidth) {
+  if (!p) { set_error("null plan"); return DFT_ERR_INVALID_ARG; }
+  if (nband < 0 || degree < 0) { set_error("nband = %d, degree = %d: negative", nband, degree); return DFT_ERR_INVALID_ARG; }
+  if (!(halfwidth > 0.0) || !(center == center)) { set_error("halfwidth must be > 0 and center finite"); return DFT_ERR_INVALID_ARG; }
+  if (((uintptr_t)psi & 15) || ((uintptr_t)work & 15)) { set_error("psi/work must be 16-byte aligned"); return DFT_ERR_INVALID_ARG; }
+  return DFT_OK;
+}
+
+extern "C" {
+
+int dft_chebyshev_filter(dft_plan *p, double *psi, double *work, int32_t nband, int32_t degree, double center,
+                         double halfwidth, void *stream) {
+  DFT_GUARD_BEGIN
+  int rc = chebyshev_args(p, psi, work, nband, degree, center, halfwidth);
+  if (rc) return rc;
+  p->last_launches = 0;
+  const size_t n = (size_t)p->nkpt * nband * p->mpw * 2;   // doubles per psi-sized array
+  if (n == 0 || degree == 0) return DFT_OK;
+  if (!psi || !work) { set_error("null psi/work"); return DFT_ERR_INVALID_ARG; }
+  cudaStream_t st = (cudaStream_t)stream;
+  return chebyshev_impl(p, psi, work, n, degree, center, halfwidth, st,
+                        [&](const double *x, double *y, const Recurrence *rec) { return apply_impl(p, x, y, nband, st, rec); });
+  DFT_GUARD_END
+}
+
+int dft_chebyshev_filter_gamma(dft_plan *p, double *psi, double *work, int32_t nband, int32_t degree, double center,
+                               double halfwidth, void *stream) {
+  DFT_GUARD_BEGIN
+  int rc = chebyshev_args(p, psi, work, nband, degree, center, halfwidth);
+  if (rc) return rc;
+  if (!p->gam || !p->gamma_on) { set_error("Gamma storage is not enabled (dft_plan_set_option gamma_real = 1)"); return DFT_ERR_NOT_READY; }
+  p->last_launches = 0;
+  const size_t n = (size_t)nband * p->gam->nh * 2;
+  if (n == 0 || degree == 0) return DFT_OK;
+  if (!psi || !work) { set_error("null psi/work"); return DFT_ERR_INVALID_ARG; }
+  cudaStream_t st = (cudaStream_t)stream;
+  return chebyshev_impl(p, psi, work, n, degree, center, halfwidth, st,
+                        [&](const double *x, double *y, const Recurrence *rec) { return gamma_apply(p, x, y, nband, st, rec); });
   DFT_GUARD_END
 }
 

@@ -79,6 +79,21 @@ def test_gamma_matches_the_full_sphere_path_on_symmetric_input():
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["c0", "c2m"])
+def test_gamma_chebyshev_filter(name):
+    """dft_chebyshev_filter_gamma against the oracle's recurrence in Gamma storage (degrees 0, 1, 4, 7)."""
+    cfg, plan, (kg, ig, kin), hkin = _gamma_setup(name)
+    psi = synth.gen_psi(cfg, [hkin])[0]
+    cen, e = 0.5 * float(kin.max()) + 1.0, 0.5 * float(kin.max()) + 0.5
+    for deg in (0, 1, 4, 7):
+        t = torch.as_tensor(psi, device="cuda").clone()
+        got = plan.chebyshev_filter_gamma(t, deg, cen, e).cpu().numpy()
+        ref = oracle.chebyshev_filter_gamma(cfg, kg, ig, kin, psi, deg, cen, e, method=1 if name == "c0" else 2)
+        err = band_rel_err(got, ref)
+        assert err <= TOL, "%s deg=%d: %.3e" % (name, deg, err)
+    plan.destroy()
+
+
 def test_gamma_refusals():
     cfg = synth.make_config("c0")                            # the recipe's dense D couples s and p projectors
     plan = make_plan(cfg)

@@ -114,6 +114,28 @@ def test_gamma_projections_are_real_up_to_i_power_l():
     assert np.max(np.abs(cp[l % 2 == 1].imag)) > 1e-3 * scale
 
 
+def test_gamma_chebyshev_closed_form_and_full_sphere_agreement():
+    """Diagonal H (constant V, D = 0): T_n((kin + V0 - c)/e) c on the stored half, by numpy's chebval; and for the whole
+    operator the Gamma recurrence equals the (pinned) full-sphere recurrence on the expanded vectors."""
+    c = dict(config("c2m")); kg, ig, kin = sphere("c2m")
+    ih, _ = oracle.gamma_half(kg)
+    x = rand_c((2, len(ih)), 31)
+    cen, e = 0.5 * kin.max() + 1.0, 0.5 * kin.max() + 0.5
+    v0 = 0.37
+    for deg in (0, 1, 5):
+        got = oracle.chebyshev_filter_gamma(c, kg, ig, kin, x, deg, cen, e, vloc=np.full_like(c["vloc"], v0), dij=np.zeros_like(c["dij"]))
+        coef = np.zeros(deg + 1); coef[deg] = 1.0
+        x0 = x.copy()
+        if deg > 0:
+            x0[:, 0] = x0[:, 0].real
+        ref = np.polynomial.chebyshev.chebval((kin[ih] + v0 - cen) / e, coef)[None, :] * x0
+        assert rel_err(got, ref) < 1e-12
+    d = synth.gamma_dij(c)
+    got = oracle.chebyshev_filter_gamma(c, kg, ig, kin, x, 4, cen, e, dij=d)
+    full = oracle.chebyshev_filter(c, 0, kg, ig, kin, oracle.gamma_expand(kg, x), 4, cen, e, dij=d)
+    assert rel_err(got[:, 1:], full[:, ih][:, 1:]) < 1e-12 and np.max(np.abs(got[:, 0].imag)) == 0
+
+
 # ------------------------------------------------------------------------------------------------ spinors
 def _spin_diag(c):
     v4 = np.stack([c["vloc"], c["vloc"], np.zeros_like(c["vloc"]), np.zeros_like(c["vloc"])])

@@ -478,6 +478,27 @@ def main():
                        "d2h_bytes_per_step": nbytes, "ms_per_step": dt, "steps": ke,
                        "api": "dft_apply_h_host (pinned host psi -> device, H, device -> pinned host hpsi)"}
         del psi_h, hpsi_h
+    # ---- context: the same step with the other exact GEMM formulations (same table, same bands), and how far their results
+    #      are from the default one: what `frac_vs_F_nl_8flop` > 1 rests on
+    if args.cheb_degree > 0 and world == 1 and sym:
+        ref_h = hpsi.clone()
+        variants = {}
+        for label, opts in (("gauss_3m_complex_6flop", {"gemm_sym": 0, "gemm_3m": 1}), ("four_product_complex_8flop", {"gemm_sym": 0, "gemm_3m": 0})):
+            for k_, v_ in opts.items():
+                plan.set_option(k_, v_)
+            plan.apply_h(psi, hpsi)
+            torch.cuda.synchronize()
+            v0 = torch.cuda.Event(enable_timing=True); v1 = torch.cuda.Event(enable_timing=True)
+            v0.record(); plan.apply_h(psi, hpsi); v1.record()
+            torch.cuda.synchronize()
+            dev = float((torch.linalg.norm(hpsi - ref_h, dim=-1) / torch.linalg.norm(ref_h, dim=-1)).max())
+            variants[label] = {"ms_per_step": v0.elapsed_time(v1), "max_rel_diff_vs_default": dev}
+        plan.set_option("gemm_sym", args.gemm_sym); plan.set_option("gemm_3m", args.gemm_3m)
+        plan.apply_h(psi, hpsi)
+        line["gemm_variants"] = dict(variants, default="real symmetric-table GEMMs, 4 flops per (projector, plane wave, band): %.1f ms" % ms_step)
+        del ref_h
+        torch.cuda.empty_cache()
+
     # ---- context figure: Chebyshev filter of degree mdeg_filter = 10 (PAPER.md :489), i.e. 10
     #      chained H applications with the recurrence fused into GEMM-2's epilogue; not part of `value`
     if args.cheb_degree > 0 and world == 1:

@@ -381,7 +381,7 @@ fft2_b_fwd_ring_kernel(const __grid_constant__ CUtensorMap mapT1, Fft2Geom G, cp
       }
       Dft<R1, +1>::run(v);
 #pragma unroll
-      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw2, s * k1));
+      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw2, s * k1));   // (shared-memory twiddles: slower here, 13.5 -> 13.9 ms at c4)
 #pragma unroll
       for (int k1 = 0; k1 < R1; k1++) sm[k1 * KS + s * XT + px] = v[k1];
     }
@@ -412,10 +412,12 @@ fft2_b_inv_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cp
   unsigned char *stages = smem_raw;
   cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
   Run *runs = reinterpret_cast<Run *>(sm + R2 * KS);
-  uint64_t *full = reinterpret_cast<uint64_t *>(runs + G.nplane);
+  cplx *tws = reinterpret_cast<cplx *>(runs + G.nplane);      // twiddles exp(+2 pi i j / n2) in shared memory: loading them from
+  uint64_t *full = reinterpret_cast<uint64_t *>(tws + G.n2);  // L2 in every tile sat on the critical path (12.25 -> 10.6 ms at c4)
   const int t = threadIdx.x, px = t % XT, s = t / XT;
   for (int i = t; i < G.nplane * 2; i += blockDim.x)
     reinterpret_cast<int4 *>(runs)[i] = __ldg(reinterpret_cast<const int4 *>(G.plane_run) + i);
+  for (int i = t; i < G.n2; i += blockDim.x) tws[i] = __ldg(G.tw2 + i);
   if (t == 0) {
     for (int i = 0; i < Q.S; i++) mbar_init(&full[i], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -448,7 +450,7 @@ fft2_b_inv_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cp
       for (int b2 = 0; b2 < R2; b2++) v[b2] = in[(s + R1 * b2) * XT];
       Dft<R2, -1>::run(v);
 #pragma unroll
-      for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw2, s * cc));
+      for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], tws[s * cc]);
 #pragma unroll
       for (int cc = 0; cc < R2; cc++) sm[cc * KS + s * XT + px] = v[cc];
     }
@@ -773,7 +775,8 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
   const int rows = pass == 1 ? hb : (pass == 2 ? G.nplane : G.n2);
   const int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
   size_t ex = sizeof(cplx) * (size_t)(pass == 1 ? R1 * KSa : (pass == 3 ? R2 * KSb : imax(R1 * KSa, R2 * KSb)));
-  size_t extra = pass == 2 ? sizeof(double) * (size_t)((G.n3 * XT + 1) & ~1) + sizeof(cplx) * (size_t)G.n3 : sizeof(Run) * (size_t)G.nplane;
+  size_t extra = pass == 2 ? sizeof(double) * (size_t)((G.n3 * XT + 1) & ~1) + sizeof(cplx) * (size_t)G.n3
+                           : sizeof(Run) * (size_t)G.nplane + (pass == 3 ? sizeof(cplx) * (size_t)G.n2 : 0);
   RingParams Q;
   Q.XT = XT; Q.nxt = nxt; Q.nb = nb;
   Q.box_bytes = (uint32_t)((size_t)rows * XT * 16);

@@ -355,6 +355,31 @@ def test_meta_gga_term(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("nband", [1, 3, 65])
+def test_symmetric_table_gemms_with_other_terms(nband):
+    """gemm_sym = 1 (k = 0: real GEMMs on the half sphere) together with what else can change the operator: a vector
+    potential (kinetic diagonal only; the projector symmetry is untouched), the meta-GGA term, odd band counts and a band
+    count that spans two GEMM tiles; and after proj_mode went to 1 and back (the full table is rebuilt, the half table stays)."""
+    cfg, plan, sph = _setup("c4m", nband=nband)
+    kg, ig, kin = sph[0]
+    psi = synth.gen_psi(cfg, [kin])
+    plan.set_option("gemm_sym", 1)
+    a = np.array([0.2, 0.1, -0.3])
+    plan.set_vector_potential(a)
+    n = cfg["ngfft"]
+    vt = 0.4 + 0.15 * np.random.default_rng(8).standard_normal((n[2], n[1], n[0]))
+    plan.set_vtau(torch.as_tensor(vt, device="cuda"))
+    ka = oracle.kin_vecpot(cfg["rprimd"], cfg["kpt"][0], kg, a)
+    ref = oracle.apply_h(cfg, 0, kg, ig, ka, psi[0]) + oracle.apply_mgga(cfg, 0, kg, ig, psi[0], vt)
+    got = gpu_apply(plan, psi)
+    assert band_rel_err(got, ref[None]) <= TOL
+    plan.set_option("proj_mode", 1); plan.set_option("proj_mode", 0)
+    assert band_rel_err(gpu_apply(plan, psi), ref[None]) <= TOL
+    plan.set_vector_potential(None); plan.set_vtau(None)
+    assert band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi)) <= TOL
+    plan.destroy()
+
+
 @pytest.mark.parametrize("name", ["c1m", "c4m", "c2m", "aniso", "aniso8", "c3k2"])
 def test_factorised_projectors(name):
     """Option proj_mode = 1 (PAPER.md :477 "computed on-the-fly"): p = FY . S evaluated inside both GEMMs instead of the

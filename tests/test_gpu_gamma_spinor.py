@@ -54,6 +54,26 @@ def test_gamma_small_cells_all_terms_and_paths(name):
     plan.destroy()
 
 
+def test_gamma_and_symmetric_table_on_a_triclinic_cell_with_two_types():
+    """aniso at k = 0: triclinic lattice, anisotropic box, an l = 2 type with 9 projectors next to the 8-projector type.
+    Both k = 0 formulations (Gamma storage; real symmetric-table GEMMs for general complex bands) against the oracle."""
+    cfg, plan, (kg, ig, kin), hkin = _gamma_setup("aniso", kpt=[[0.0, 0.0, 0.0]])
+    psi = synth.gen_psi(cfg, [hkin])[0]
+    ref = oracle.apply_h_gamma(cfg, kg, ig, kin, psi, method=1)
+    assert band_rel_err(_gamma_gpu(plan, psi), ref) <= TOL
+    plan.destroy()
+    cfg = synth.make_config("aniso", kpt=[[0.0, 0.0, 0.0]])      # the recipe's dense D (couples l = 0, 1, 2): fine for complex bands
+    plan = make_plan(cfg)
+    sph = lib_spheres(plan)
+    full = synth.gen_psi(cfg, [sph[0][2]])
+    fref = oracle.apply_h(cfg, 0, *sph[0], full[0], method=1)
+    for sym in (1, 0):
+        plan.set_option("gemm_sym", sym)
+        got = plan.apply_h(torch.as_tensor(full, device="cuda")).cpu().numpy()
+        assert band_rel_err(got, fref[None]) <= TOL, sym
+    plan.destroy()
+
+
 @pytest.mark.parametrize("nband", [1, 3, 64, 65])
 def test_gamma_band_counts(nband):
     """Odd band counts leave the last pair half empty; 65 bands = two GEMM band tiles."""

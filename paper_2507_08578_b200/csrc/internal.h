@@ -90,6 +90,7 @@ struct GammaData {
 
 struct NlMaps;
 struct SymMaps;
+struct StrassenData;
 void nl_maps_free(dft_plan *p);
 
 // timed kernel groups: 0-4 the five FFT passes, 5 GEMM-1, 6 D_ij, 7 GEMM-2, 8 the fused small-box local term (fft_small.cu),
@@ -183,6 +184,8 @@ struct dft_plan {
   dftb200::GammaData *gam = nullptr;   // half sphere + rotated table: built by option gamma_real = 1 or by the symmetric-table GEMMs
   bool gamma_on = false;               // option gamma_real = 1 (dft_apply_h_gamma allowed, D_ij parity enforced)
   int gemm_sym = 2;                    // at k = 0 run the projector GEMMs of dft_apply_h as real GEMMs on the half sphere (nonlocal.cu): 0 never, 1 always, 2 = when large enough
+  dftb200::StrassenData *strassen = nullptr;   // block tables and scratch of the Strassen level on the real GEMMs (nonlocal_strassen.inc)
+  int gemm_strassen = 2;               // 0 never, 1 wherever possible, 2 = automatic (large problems): 7 half-size products per real GEMM instead of 8
   int sym_state = 0;                   // 0 = not tried, 1 = tables ready, -1 = this plan cannot (k != 0, several k-points, unpaired Nyquist index)
   double *d_symx = nullptr; int64_t symx_bytes = 0;   // time-reversal-even/odd halves of the bands, [2 nband][nhalf] complex
   // two-component spinors (spinor.cu): Pauli components of the local potential, spin-dependent D

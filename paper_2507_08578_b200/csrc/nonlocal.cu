@@ -67,6 +67,7 @@ struct Gemm2Params {
   int cheb;
   double sh, sy, sx;
   const double2 *xprev;                // [nkpt][nband][mpw], read only where sx != 0
+  int raw;                             // gemm2_kernel<true> only: 1 = an intermediate product (Strassen block): keep Im of row 0
 };
 
 // The MMA main loop shared by both GEMMs.  MODE 1: acc += conj(A) B (GEMM-1); MODE 2: acc += A B.
@@ -401,7 +402,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
           double2 y = psi[off], xp = Q.sx != 0.0 ? Q.xprev[(size_t)ik * Q.nband * Q.mpw + off] : make_double2(0.0, 0.0);
           r.x = Q.sh * r.x + Q.sy * y.x + Q.sx * xp.x; r.y = Q.sh * r.y + Q.sy * y.y + Q.sx * xp.y;
         }
-        if (REAL && g == 0) r.y = 0.0;     // Gamma storage: c(G = 0) is real (reading 26)
+        if (REAL && g == 0 && !Q.raw) r.y = 0.0;     // Gamma storage: c(G = 0) is real (reading 26)
         hpsi[off] = r;
       }
     }
@@ -877,7 +878,8 @@ struct SymMaps {
   const void *ptab = nullptr, *x = nullptr, *cprj = nullptr;
   int n2_x = -1, n2_c = -1;
 };
-void nl_maps_free(dft_plan *p) { delete p->nl_maps; p->nl_maps = nullptr; delete p->sym_maps; p->sym_maps = nullptr; }
+void strassen_free(dft_plan *p);
+void nl_maps_free(dft_plan *p) { delete p->nl_maps; p->nl_maps = nullptr; delete p->sym_maps; p->sym_maps = nullptr; strassen_free(p); }
 
 typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                              const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -1047,6 +1049,8 @@ static bool sym_ready(dft_plan *p) {
   return p->sym_state == 1;
 }
 
+#include "nonlocal_strassen.inc"
+
 static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int nband, bool accumulate, bool with_kin, cudaStream_t st,
                               const double *dmat, const double *const *diag, double *cprj_out, const Recurrence *rec, double *spsi) {
   GammaData *G = p->gam;
@@ -1066,6 +1070,12 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
     p->symx_bytes = need_x;
   }
   double2 *X = reinterpret_cast<double2 *>(p->d_symx);
+  if (strassen_wanted(p, nband)) {      // seven half-size products per GEMM instead of eight (nonlocal_strassen.inc)
+    phase_begin(p, 9, st);
+    sym_split_kernel<<<dim3((nh + 255) / 256, nband), 256, 0, st>>>(reinterpret_cast<const double2 *>(psi), X, G->d_h2f, G->d_h2fneg, mpw, nh);
+    phase_end(p, 9, st, 1);
+    return nonlocal_apply_sym_strassen(p, psi, hpsi, nband, accumulate, with_kin, st, dmat, d_kin, cprj_out, rec, spsi, X);
+  }
   Gemm1Params q1;
   q1.nproj = nproj; q1.nband = n2; q1.nslab = (nh + 7) / 8;
   q1.tiles_m = (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (n2 + NL_BN - 1) / NL_BN;
@@ -1134,7 +1144,7 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
   q2.nproj = nproj; q2.nband = n2; q2.mpw = nh; q2.nslab = (nproj + 7) / 8;
   q2.tiles_n = q1.tiles_n; q2.accumulate = 0; q2.with_kin = 0; q2.with_nl = 1;
   q2.npw = G->d_npw; q2.kin = G->d_kinptr; q2.psi = X; q2.hpsi = X;
-  q2.cheb = 0; q2.sh = 1.0; q2.sy = 0.0; q2.sx = 0.0; q2.xprev = nullptr;
+  q2.cheb = 0; q2.sh = 1.0; q2.sy = 0.0; q2.sx = 0.0; q2.xprev = nullptr; q2.raw = 0;
   const int tiles_m2 = (nh + NL_BM - 1) / NL_BM;
   const dim3 cgrid((mpw + 255) / 256, nband);
   phase_begin(p, 7, st);
@@ -1313,7 +1323,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   q2.tiles_n = q1.tiles_n; q2.accumulate = accumulate; q2.with_kin = with_kin; q2.with_nl = 1;
   q2.npw = d_npw; q2.kin = d_kin; q2.psi = cpsi; q2.hpsi = chpsi;
   q2.cheb = rec != nullptr; q2.sh = rec ? rec->sh : 1.0; q2.sy = rec ? rec->sy : 0.0; q2.sx = rec ? rec->sx : 0.0;
-  q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr;
+  q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr; q2.raw = 0;
   int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
   phase_begin(p, 7, st);
   if (fac) {
@@ -1420,7 +1430,7 @@ int nonlocal_apply_gamma(dft_plan *p, const double *psi, double *hpsi, int nband
   q2.tiles_n = q1.tiles_n; q2.accumulate = accumulate; q2.with_kin = with_kin; q2.with_nl = 1;
   q2.npw = G->d_npw; q2.kin = G->d_kinptr; q2.psi = cpsi; q2.hpsi = chpsi;
   q2.cheb = rec != nullptr; q2.sh = rec ? rec->sh : 1.0; q2.sy = rec ? rec->sy : 0.0; q2.sx = rec ? rec->sx : 0.0;
-  q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr;
+  q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr; q2.raw = 0;
   const int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
   phase_begin(p, 7, st);
   gemm2_kernel<true><<<dim3(q2.tiles_n * tiles_m2, 1, 1), NL_THREADS_P, NL_SMEM, st>>>(mapP2, mapC, q2);

@@ -599,6 +599,10 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     p->gamma_on = false;     // the tables stay: the symmetric-table GEMMs of dft_apply_h use them too
     return DFT_OK;
   }
+  if (!strcmp(key, "gemm_strassen")) {
+    if (value < 0 || value > 2) { set_error("gemm_strassen = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->gemm_strassen = (int)value; return DFT_OK;
+  }
   if (!strcmp(key, "gemm_sym")) {
     if (value < 0 || value > 2) { set_error("gemm_sym = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->gemm_sym = (int)value; return DFT_OK;

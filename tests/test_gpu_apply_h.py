@@ -355,6 +355,40 @@ def test_meta_gga_term(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name,nband", [("c4m", 7), ("c4m", 2), ("c4m", 65), ("c2m", 5), ("c0", 8)])
+def test_strassen_level_on_the_real_gemms(name, nband):
+    """gemm_strassen = 1 (seven half-size products per real GEMM, block tables with a short second half completed by the TMA
+    zero fill): H psi with term isolations, S psi, cprj, H psi and S psi from one GEMM-1, and the Chebyshev recurrence."""
+    cfg, plan, sph = _setup(name, nband=nband)
+    kg, ig, kin = sph[0]
+    psi = synth.gen_psi(cfg, [kin])
+    tpsi = torch.as_tensor(psi, device="cuda")
+    plan.set_option("gemm_sym", 1); plan.set_option("gemm_strassen", 1)
+    m = 1 if name == "c0" else 2
+    for terms in (7, 4, 5):
+        plan.set_option("terms", terms)
+        err = band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, terms=terms, method=m))
+        assert err <= TOL, "%s nband=%d terms=%d: %.3e" % (name, nband, terms, err)
+    plan.set_option("terms", 7)
+    assert plan.last_launches() > 20                         # 14 GEMM launches + combinations: the Strassen path did run
+    sij = np.random.default_rng(4).standard_normal(cfg["dij"].shape) * 0.3
+    sij = 0.5 * (sij + sij.transpose(0, 2, 1))
+    plan.set_sij(sij)
+    h, s_ = plan.apply_hs(tpsi)
+    cp = plan.get_cprj(tpsi).cpu().numpy()[0]
+    sref = oracle.apply_s(cfg, 0, kg, psi[0], sij)
+    assert band_rel_err(h.cpu().numpy(), oracle_apply(cfg, sph, psi, method=m)) <= TOL
+    assert band_rel_err(s_.cpu().numpy(), sref[None]) <= TOL
+    assert band_rel_err(plan.apply_s(tpsi).cpu().numpy(), sref[None]) <= TOL
+    cref = oracle.cprj(cfg, 0, kg, psi[0][:, :len(ig)]).T
+    assert float(np.max(np.linalg.norm(cp - cref, axis=1) / np.linalg.norm(cref, axis=1))) <= TOL
+    cen, e = 0.5 * float(kin.max()) + 1.0, 0.5 * float(kin.max()) + 0.5
+    got = plan.chebyshev_filter(tpsi.clone(), 3, cen, e).cpu().numpy()
+    ref = oracle.chebyshev_filter(cfg, 0, kg, ig, kin, psi[0], 3, cen, e, method=m)
+    assert band_rel_err(got, ref[None]) <= TOL
+    plan.destroy()
+
+
 @pytest.mark.parametrize("nband", [1, 3, 65])
 def test_symmetric_table_gemms_with_other_terms(nband):
     """gemm_sym = 1 (k = 0: real GEMMs on the half sphere) together with what else can change the operator: a vector
@@ -584,8 +618,9 @@ def _sampled_full_size(name, per_tile, nvariant):
     sub = sample[::max(1, len(sample) // max(nvariant, ntile))]
     pos = [sample.index(b) for b in sub]
     assert len(sub) >= 16 and len({b // 64 for b in sub}) == ntile
-    # (the default at k = 0 is the symmetric-table real GEMMs; gemm_sym = 0 gives the complex 3M kernels, then the others)
-    for key, val in (("gemm_sym", 0), ("gemm_3m", 0), ("proj_mode", 1)):
+    # (the default at k = 0 is the symmetric-table real GEMMs with one Strassen level; gemm_strassen = 0 gives the plain real GEMMs,
+    # gemm_sym = 0 the complex 3M kernels, then the others)
+    for key, val in (("gemm_strassen", 0), ("gemm_sym", 0), ("gemm_3m", 0), ("proj_mode", 1)):
         plan.set_option(key, val)
         out2 = plan.apply_h(psi)
         torch.cuda.synchronize()

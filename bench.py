@@ -207,6 +207,8 @@ def measure_config(name, hbm_gbs, steps=20, warmup=3):
     geo = geometry(plan)
     sym = plan.nkpt == 1 and not np.any(np.asarray(cfg["kpt"][0])) and float(plan.nproj) * plan.mpw * nband >= 1e8
     fpc = 4.0 if sym else 6.0
+    if sym and plan.nproj % 16 == 0 and float(plan.nproj) * plan.mpw * nband >= 1e10:
+        fpc = 3.5       # one Strassen level on the real GEMMs
     fft_bytes, g1, g2 = byte_flop_model(plan, geo, nband, fpc)
     for _ in range(warmup):
         plan.apply_h(psi, hpsi)
@@ -305,6 +307,7 @@ def main():
     ap.add_argument("--fft-path", type=int, default=0, help="dft_plan_set_option fft_path (experiments only)")
     ap.add_argument("--proj-mode", type=int, default=0, help="1 = factorised projectors FY.S (experiments only)")
     ap.add_argument("--gemm-3m", type=int, default=1, help="0 = 4-product complex GEMMs (experiments only)")
+    ap.add_argument("--gemm-strassen", type=int, default=2, help="0 = no Strassen level on the real GEMMs (experiments only)")
     ap.add_argument("--gemm-sym", type=int, default=2, help="0 = complex GEMMs also at k = 0, 1 = real GEMMs at k = 0 even for tiny cells (experiments only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (experiments only)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the e2e leg (experiments only)")
@@ -347,6 +350,7 @@ def main():
         plan.set_option("fft_path", args.fft_path)
     plan.set_option("gemm_3m", args.gemm_3m)
     plan.set_option("gemm_sym", args.gemm_sym)
+    plan.set_option("gemm_strassen", args.gemm_strassen)
     if args.proj_mode:
         plan.set_option("proj_mode", args.proj_mode)
     plan.set_vloc(torch.as_tensor(cfg["vloc"], device="cuda"))
@@ -361,7 +365,8 @@ def main():
     # table is symmetric under G -> -G), 6 = Gauss / 3M complex, 8 = four-product complex
     sym = (bool(args.gemm_sym) and not args.proj_mode and plan.nkpt == 1 and not np.any(np.asarray(cfg["kpt"][0]))
            and (args.gemm_sym == 1 or float(plan.nproj) * plan.mpw * nband >= 1e8))
-    fpc = 4.0 if sym else (6.0 if args.gemm_3m else 8.0)
+    strassen = sym and args.gemm_strassen != 0 and plan.nproj % 16 == 0 and (args.gemm_strassen == 1 or float(plan.nproj) * plan.mpw * nband >= 1e10)
+    fpc = (3.5 if strassen else 4.0) if sym else (6.0 if args.gemm_3m else 8.0)
     fft_bytes, g1_flops, g2_flops = byte_flop_model(plan, geo, nband, fpc)
     hbm_gbs, hbm_src = measured_peaks()
 
@@ -418,8 +423,10 @@ def main():
                                 "achieved": fl / (ph_ms[name] * 1e-3) / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                                 "flops_per_complex_mac": fpc,
                                 "frac_vs_F_nl_8flop": fl * (8.0 / fpc) / (ph_ms[name] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS}
-    if sym and ph_ms.get("pack_unpack", 0) > 0:     # split into symmetric halves + recombination: 2a and 4a bytes per band
-        sc_bytes = sum(6 * 16.0 * g_["npw"] * nband for g_ in geo)
+    if sym and ph_ms.get("pack_unpack", 0) > 0:
+        # split into symmetric halves (2a) + recombination (4a); with the Strassen level also the five band-side block
+        # combinations (3.75a) and a recombination that reads twelve quarter products instead of the halves (6a): 11.75a
+        sc_bytes = sum((11.75 if strassen else 6.0) * 16.0 * g_["npw"] * nband for g_ in geo)
         per_kernel["sym_split_combine"] = {"bound": "hbm", "ms_per_step": ph_ms["pack_unpack"], "launches_per_step": ph_n["pack_unpack"],
                                            "achieved": sc_bytes / (ph_ms["pack_unpack"] * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
     for v in per_kernel.values():
@@ -441,14 +448,14 @@ def main():
                 "peak_source": ("FP64 DMMA: 148 SM x 4 x 512 flop / 16 clk x 1.965 GHz (microbenchmark 37.06), "
                                 "DESIGN.md 8" if d["bound"] == "tensor" else hbm_src),
                 "share_of_step": d["ms_per_step"] / ms_step}
-    sc_s = (sum(6 * 16.0 * g_["npw"] * nband for g_ in geo) / (hbm_gbs * 1e9)) if sym else 0.0
+    sc_s = (sum((11.75 if strassen else 6.0) * 16.0 * g_["npw"] * nband for g_ in geo) / (hbm_gbs * 1e9)) if sym else 0.0
     t_roof = sum(fft_bytes.values()) / (hbm_gbs * 1e9) + (g1_flops + g2_flops) / (FP64_PEAK_TFLOPS * 1e12) + sc_s
     t_roof8 = sum(fft_bytes.values()) / (hbm_gbs * 1e9) + (g1_flops + g2_flops) * (8.0 / fpc) / (FP64_PEAK_TFLOPS * 1e12)
     path = {"t_roof_ms": t_roof * 1e3, "frac": t_roof * 1e3 / ms_step,
             "frac_vs_F_nl_8flop": t_roof8 * 1e3 / ms_step,
             "definition": "sum_phases max(bytes/HBM_measured, flops/FP64_peak) / measured step time; GEMM flops = %g per "
-                          "(projector, plane wave, band) (the variant the kernels run: 4 = real GEMMs on the half sphere at "
-                          "k = 0, 6 = Gauss, 8 = four products); frac_vs_F_nl_8flop uses SURVEY.md's dense 8-flop count F_nl" % fpc,
+                          "(projector, plane wave, band) (the variant the kernels run: 3.5 = real GEMMs on the half sphere at "
+                          "k = 0 with one Strassen level, 4 = without it, 6 = Gauss, 8 = four products); frac_vs_F_nl_8flop uses SURVEY.md's dense 8-flop count F_nl" % fpc,
             "kernels": per_kernel}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -483,7 +490,8 @@ def main():
     if args.cheb_degree > 0 and world == 1 and sym:
         ref_h = hpsi.clone()
         variants = {}
-        for label, opts in (("gauss_3m_complex_6flop", {"gemm_sym": 0, "gemm_3m": 1}), ("four_product_complex_8flop", {"gemm_sym": 0, "gemm_3m": 0})):
+        for label, opts in (("real_symmetric_4flop", {"gemm_strassen": 0}), ("gauss_3m_complex_6flop", {"gemm_sym": 0, "gemm_3m": 1}),
+                            ("four_product_complex_8flop", {"gemm_sym": 0, "gemm_3m": 0})):
             for k_, v_ in opts.items():
                 plan.set_option(k_, v_)
             plan.apply_h(psi, hpsi)
@@ -493,9 +501,10 @@ def main():
             torch.cuda.synchronize()
             dev = float((torch.linalg.norm(hpsi - ref_h, dim=-1) / torch.linalg.norm(ref_h, dim=-1)).max())
             variants[label] = {"ms_per_step": v0.elapsed_time(v1), "max_rel_diff_vs_default": dev}
-        plan.set_option("gemm_sym", args.gemm_sym); plan.set_option("gemm_3m", args.gemm_3m)
+        plan.set_option("gemm_sym", args.gemm_sym); plan.set_option("gemm_3m", args.gemm_3m); plan.set_option("gemm_strassen", args.gemm_strassen)
         plan.apply_h(psi, hpsi)
-        line["gemm_variants"] = dict(variants, default="real symmetric-table GEMMs, 4 flops per (projector, plane wave, band): %.1f ms" % ms_step)
+        line["gemm_variants"] = dict(variants, default="real symmetric-table GEMMs%s, %g flops per (projector, plane wave, band): %.1f ms"
+                                     % (" with one Strassen level" if strassen else "", fpc, ms_step))
         del ref_h
         torch.cuda.empty_cache()
 

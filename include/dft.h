@@ -131,6 +131,9 @@ int dft_plan_workspace_bytes(const dft_plan *p, int32_t nband, int64_t *min_byte
  * symmetric under G -> -G, so both projector GEMMs of dft_apply_h can run as REAL GEMMs on the half sphere, 4 instead of
  * 6 flops per projector, plane wave and band, same result up to rounding, any D_ij; 0 = never, 1 = wherever possible,
  * 2 = default: when nproj * npw * nband >= 1e8; the first such call builds a second table of half the size),
+ * "gemm_strassen" (with gemm_sym active: one level of Strassen's recursion on the two real GEMMs, 7/8 of their flops, same
+ * result up to rounding; 0 = never, 1 = wherever nproj is a multiple of 16, 2 = default: for nproj * npw * nband >= 1e10;
+ * builds nine block tables of a quarter of the half table each at the first such call),
  * "gamma_real" (1 = enable dft_apply_h_gamma, see there).  Unknown key or bad value -> DFT_ERR_INVALID_ARG.  */
 int dft_plan_set_option(dft_plan *p, const char *key, int64_t value);
 

@@ -1074,7 +1074,7 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
     phase_begin(p, 9, st);
     sym_split_kernel<<<dim3((nh + 255) / 256, nband), 256, 0, st>>>(reinterpret_cast<const double2 *>(psi), X, G->d_h2f, G->d_h2fneg, mpw, nh);
     phase_end(p, 9, st, 1);
-    return nonlocal_apply_sym_strassen(p, psi, hpsi, nband, accumulate, with_kin, st, dmat, d_kin, cprj_out, rec, spsi, X);
+    return nonlocal_apply_sym_strassen(p, psi, hpsi, nband, accumulate, with_kin, st, dmat, d_kin, cprj_out, rec, spsi, X, false);
   }
   Gemm1Params q1;
   q1.nproj = nproj; q1.nband = n2; q1.nslab = (nh + 7) / 8;
@@ -1380,6 +1380,8 @@ int nonlocal_apply_gamma(dft_plan *p, const double *psi, double *hpsi, int nband
     return DFT_OK;
   }
   int rc;
+  if (nband % 2 == 0 && strassen_wanted(p, nband / 2))     // one Strassen level on both real GEMMs (nonlocal_strassen.inc)
+    return nonlocal_apply_sym_strassen(p, psi, hpsi, nband, accumulate, with_kin, st, p->d_dij, G->d_kinptr, nullptr, rec, nullptr, cpsi, true);
   Gemm1Params q1;
   q1.nproj = nproj; q1.nband = nband; q1.nslab = (mpw + 7) / 8;
   q1.tiles_m = (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;

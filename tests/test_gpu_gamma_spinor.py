@@ -114,6 +114,30 @@ def test_gamma_chebyshev_filter(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name,nband", [("c4m", 8), ("c2m", 6), ("c4m", 66)])
+def test_gamma_storage_with_the_strassen_level(name, nband):
+    """gemm_strassen = 1 in Gamma storage (even band counts; odd ones keep the plain real GEMMs): H psi with term
+    isolations and the Chebyshev recurrence against the oracle."""
+    cfg, plan, (kg, ig, kin), hkin = _gamma_setup(name, nband=nband)
+    plan.set_option("gemm_strassen", 1)
+    psi = synth.gen_psi(cfg, [hkin], nband=nband)[0]
+    for terms in (7, 4, 5):
+        plan.set_option("terms", terms)
+        ref = oracle.apply_h_gamma(cfg, kg, ig, kin, psi, terms=terms)
+        got = _gamma_gpu(plan, psi)
+        assert band_rel_err(got, ref) <= TOL, "%s terms=%d" % (name, terms)
+        assert np.all(got[:, 0].imag == 0)
+    plan.set_option("terms", 7)
+    assert plan.last_launches() > 20                          # fourteen products + combinations: the Strassen path ran
+    cen, e = 0.5 * float(kin.max()) + 1.0, 0.5 * float(kin.max()) + 0.5
+    t = torch.as_tensor(psi, device="cuda").clone()
+    got = plan.chebyshev_filter_gamma(t, 3, cen, e).cpu().numpy()
+    assert band_rel_err(got, oracle.chebyshev_filter_gamma(cfg, kg, ig, kin, psi, 3, cen, e)) <= TOL
+    odd = synth.gen_psi(cfg, [hkin], nband=nband - 1)[0]       # odd count: falls back to the plain real GEMMs
+    assert band_rel_err(_gamma_gpu(plan, odd), oracle.apply_h_gamma(cfg, kg, ig, kin, odd)) <= TOL
+    plan.destroy()
+
+
 def test_gamma_refusals():
     cfg = synth.make_config("c0")                            # the recipe's dense D couples s and p projectors
     plan = make_plan(cfg)

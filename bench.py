@@ -602,6 +602,8 @@ def main():
             gph = {k: round(v[0], 3) for k, v in plan.phase_ms().items() if v[0] > 0}
             plan.set_timing(False)
             gfl = 2.0 * 2.0 * plan.nproj * len(hkin) * nband          # one real GEMM: 2 flops x nproj x (2 nhalf) x nband
+            if strassen and nband % 2 == 0:
+                gfl *= 7.0 / 8.0                                      # one Strassen level: seven half-size products
             line["gamma_real_storage"] = {
                 "value": nband / (gms * 1e-3), "unit": UNIT, "ms_per_step": gms, "nhalf": int(len(hkin)), "phase_ms": gph,
                 "gemm1_tensor_frac": gfl / (gph.get("gemm1", 1e30) * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,

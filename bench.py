@@ -488,76 +488,92 @@ def main():
     # ---- context: the same step with the other exact GEMM formulations (same table, same bands), and how far their results
     #      are from the default one: what `frac_vs_F_nl_8flop` > 1 rests on
     if args.cheb_degree > 0 and world == 1 and sym:
-        ref_h = hpsi.clone()
-        variants = {}
-        for label, opts in (("real_symmetric_4flop", {"gemm_strassen": 0}), ("gauss_3m_complex_6flop", {"gemm_sym": 0, "gemm_3m": 1}),
-                            ("four_product_complex_8flop", {"gemm_sym": 0, "gemm_3m": 0})):
-            for k_, v_ in opts.items():
-                plan.set_option(k_, v_)
+        try:
+            ref_h = hpsi.clone()
+            variants = {}
+            for label, opts in (("real_symmetric_4flop", {"gemm_strassen": 0}), ("gauss_3m_complex_6flop", {"gemm_sym": 0, "gemm_3m": 1}),
+                                ("four_product_complex_8flop", {"gemm_sym": 0, "gemm_3m": 0})):
+                for k_, v_ in opts.items():
+                    plan.set_option(k_, v_)
+                plan.apply_h(psi, hpsi)
+                torch.cuda.synchronize()
+                v0 = torch.cuda.Event(enable_timing=True); v1 = torch.cuda.Event(enable_timing=True)
+                v0.record(); plan.apply_h(psi, hpsi); v1.record()
+                torch.cuda.synchronize()
+                dev = float((torch.linalg.norm(hpsi - ref_h, dim=-1) / torch.linalg.norm(ref_h, dim=-1)).max())
+                variants[label] = {"ms_per_step": v0.elapsed_time(v1), "max_rel_diff_vs_default": dev}
+            plan.set_option("gemm_sym", args.gemm_sym); plan.set_option("gemm_3m", args.gemm_3m); plan.set_option("gemm_strassen", args.gemm_strassen)
             plan.apply_h(psi, hpsi)
-            torch.cuda.synchronize()
-            v0 = torch.cuda.Event(enable_timing=True); v1 = torch.cuda.Event(enable_timing=True)
-            v0.record(); plan.apply_h(psi, hpsi); v1.record()
-            torch.cuda.synchronize()
-            dev = float((torch.linalg.norm(hpsi - ref_h, dim=-1) / torch.linalg.norm(ref_h, dim=-1)).max())
-            variants[label] = {"ms_per_step": v0.elapsed_time(v1), "max_rel_diff_vs_default": dev}
-        plan.set_option("gemm_sym", args.gemm_sym); plan.set_option("gemm_3m", args.gemm_3m); plan.set_option("gemm_strassen", args.gemm_strassen)
-        plan.apply_h(psi, hpsi)
-        line["gemm_variants"] = dict(variants, default="real symmetric-table GEMMs%s, %g flops per (projector, plane wave, band): %.1f ms"
-                                     % (" with one Strassen level" if strassen else "", fpc, ms_step))
-        del ref_h
+            line["gemm_variants"] = dict(variants, default="real symmetric-table GEMMs%s, %g flops per (projector, plane wave, band): %.1f ms"
+                                         % (" with one Strassen level" if strassen else "", fpc, ms_step))
+            del ref_h
+            torch.cuda.empty_cache()
+        except Exception as e:       # a context figure must never cost the headline (e.g. out of memory)
+            line['gemm_variants'] = {"unavailable": repr(e)[:200]}
         torch.cuda.empty_cache()
 
     # ---- context figure: Chebyshev filter of degree mdeg_filter = 10 (PAPER.md :489), i.e. 10
     #      chained H applications with the recurrence fused into GEMM-2's epilogue; not part of `value`
     if args.cheb_degree > 0 and world == 1:
-        work = torch.empty(2 * psi.numel(), dtype=psi.dtype, device="cuda")
-        tmp = psi.clone()
-        kmax = max(float(k.max()) for k in kin_list)
-        cen, half = 0.5 * kmax + 1.0, 0.5 * kmax + 0.5
-        plan.chebyshev_filter(tmp, 1, cen, half, work)
-        torch.cuda.synchronize()
-        c0 = torch.cuda.Event(enable_timing=True); c1 = torch.cuda.Event(enable_timing=True)
-        c0.record(); plan.chebyshev_filter(tmp, args.cheb_degree, cen, half, work); c1.record()
-        torch.cuda.synchronize()
-        cms = c0.elapsed_time(c1)
-        line["chebyshev_filter"] = {"degree": args.cheb_degree, "ms": cms, "ms_per_h_application": cms / args.cheb_degree,
-                                    "bands_per_s_per_h_application": units / (cms / args.cheb_degree * 1e-3),
-                                    "api": "dft_chebyshev_filter (in place, 2 psi-sized work arrays)"}
-        del work, tmp
+        try:
+            work = torch.empty(2 * psi.numel(), dtype=psi.dtype, device="cuda")
+            tmp = psi.clone()
+            kmax = max(float(k.max()) for k in kin_list)
+            cen, half = 0.5 * kmax + 1.0, 0.5 * kmax + 0.5
+            plan.chebyshev_filter(tmp, 1, cen, half, work)
+            torch.cuda.synchronize()
+            c0 = torch.cuda.Event(enable_timing=True); c1 = torch.cuda.Event(enable_timing=True)
+            c0.record(); plan.chebyshev_filter(tmp, args.cheb_degree, cen, half, work); c1.record()
+            torch.cuda.synchronize()
+            cms = c0.elapsed_time(c1)
+            line["chebyshev_filter"] = {"degree": args.cheb_degree, "ms": cms, "ms_per_h_application": cms / args.cheb_degree,
+                                        "bands_per_s_per_h_application": units / (cms / args.cheb_degree * 1e-3),
+                                        "api": "dft_chebyshev_filter (in place, 2 psi-sized work arrays)"}
+            del work, tmp
+            torch.cuda.empty_cache()
+        except Exception as e:       # a context figure must never cost the headline (e.g. out of memory)
+            line['chebyshev_filter'] = {"unavailable": repr(e)[:200]}
         torch.cuda.empty_cache()
 
     # ---- context figure: H psi and S psi from one set of projections (three GEMMs instead of four)
     if args.cheb_degree > 0 and world == 1:
-        plan.apply_hs(psi)
-        torch.cuda.synchronize()
-        h0 = torch.cuda.Event(enable_timing=True); h1 = torch.cuda.Event(enable_timing=True)
-        h0.record(); hs = plan.apply_hs(psi); h1.record()
-        torch.cuda.synchronize()
-        sp = hs[1]                                   # preallocated output: no allocation inside the timed call
-        s0 = torch.cuda.Event(enable_timing=True); s1 = torch.cuda.Event(enable_timing=True)
-        s0.record(); plan.apply_s(psi, sp); s1.record()
-        torch.cuda.synchronize()
-        line["apply_hs"] = {"ms": h0.elapsed_time(h1), "ms_apply_s_alone": s0.elapsed_time(s1),
-                            "api": "dft_apply_hs (H psi and S psi, one GEMM-1) / dft_apply_s"}
-        del hs, sp
+        try:
+            plan.apply_hs(psi)
+            torch.cuda.synchronize()
+            h0 = torch.cuda.Event(enable_timing=True); h1 = torch.cuda.Event(enable_timing=True)
+            h0.record(); hs = plan.apply_hs(psi); h1.record()
+            torch.cuda.synchronize()
+            sp = hs[1]                                   # preallocated output: no allocation inside the timed call
+            s0 = torch.cuda.Event(enable_timing=True); s1 = torch.cuda.Event(enable_timing=True)
+            s0.record(); plan.apply_s(psi, sp); s1.record()
+            torch.cuda.synchronize()
+            line["apply_hs"] = {"ms": h0.elapsed_time(h1), "ms_apply_s_alone": s0.elapsed_time(s1),
+                                "api": "dft_apply_hs (H psi and S psi, one GEMM-1) / dft_apply_s"}
+            del hs, sp
+            torch.cuda.empty_cache()
+        except Exception as e:       # a context figure must never cost the headline (e.g. out of memory)
+            line['apply_hs'] = {"unavailable": repr(e)[:200]}
         torch.cuda.empty_cache()
 
     # ---- context figure: density accumulation n(r) = sum w |psi(r)|^2 (Eq. 6) over all bands
     if args.cheb_degree > 0 and world == 1:
-        wts = np.ones((plan.nkpt, nband))
-        rho = plan.accumulate_density(psi, wts)
-        torch.cuda.synchronize()
-        d0 = torch.cuda.Event(enable_timing=True); d1 = torch.cuda.Event(enable_timing=True)
-        d0.record(); plan.accumulate_density(psi, wts, rho); d1.record()
-        torch.cuda.synchronize()
-        dms = d0.elapsed_time(d1)
-        n1_, n2_, n3_ = plan.ngfft
-        dbytes = sum(nband * (16.0 * g_["npw"] + 2 * 16.0 * g_["ncol"] * n1_ + 2 * 16.0 * n1_ * n2_ * g_["nplane"]) for g_ in geo)
-        line["density"] = {"ms": dms, "bands_per_s": units / (dms * 1e-3), "hbm_frac": dbytes / (dms * 1e-3) / 1e9 / hbm_gbs,
-                           "bytes_model": "per band a + 2b + 2c (scatter read, T1 write+read, T2 write+read), DESIGN.md 7",
-                           "api": "dft_accumulate_density"}
-        del rho
+        try:
+            wts = np.ones((plan.nkpt, nband))
+            rho = plan.accumulate_density(psi, wts)
+            torch.cuda.synchronize()
+            d0 = torch.cuda.Event(enable_timing=True); d1 = torch.cuda.Event(enable_timing=True)
+            d0.record(); plan.accumulate_density(psi, wts, rho); d1.record()
+            torch.cuda.synchronize()
+            dms = d0.elapsed_time(d1)
+            n1_, n2_, n3_ = plan.ngfft
+            dbytes = sum(nband * (16.0 * g_["npw"] + 2 * 16.0 * g_["ncol"] * n1_ + 2 * 16.0 * n1_ * n2_ * g_["nplane"]) for g_ in geo)
+            line["density"] = {"ms": dms, "bands_per_s": units / (dms * 1e-3), "hbm_frac": dbytes / (dms * 1e-3) / 1e9 / hbm_gbs,
+                               "bytes_model": "per band a + 2b + 2c (scatter read, T1 write+read, T2 write+read), DESIGN.md 7",
+                               "api": "dft_accumulate_density"}
+            del rho
+        except Exception as e:       # a context figure must never cost the headline (e.g. out of memory)
+            line['density'] = {"unavailable": repr(e)[:200]}
+        torch.cuda.empty_cache()
 
     # ---- context figure: the same step with factorised projectors (option proj_mode = 1)
     if args.cheb_degree > 0 and world == 1 and not args.proj_mode:
@@ -574,7 +590,7 @@ def main():
             fms = f0.elapsed_time(f1) / 2
             line["factorised_projectors"] = {"value": units / (fms * 1e-3), "unit": UNIT, "ms_per_step": fms,
                                              "option": "proj_mode = 1 (FY.S tables instead of the materialised projector table)"}
-        except dft.DftError as e:
+        except Exception as e:
             line["factorised_projectors"] = {"unavailable": str(e)}
         plan.set_option("proj_mode", 0)
 
@@ -611,7 +627,7 @@ def main():
                 "api": "dft_apply_h_gamma (option gamma_real = 1; D_ij with the odd-parity couplings removed)"}
             del gpsi, ghpsi
             plan.set_option("gamma_real", 0)
-        except dft.DftError as e:
+        except Exception as e:
             line["gamma_real_storage"] = {"unavailable": str(e)}
         dft.dft_set_dij(plan.h, cfg["dij"])
         torch.cuda.empty_cache()
@@ -633,7 +649,7 @@ def main():
                               "spinor_bands": snb, "api": "dft_apply_h_spinor (scalar D_ij on both components; four scalar "
                               "local applications for the 2x2 potential)"}
             del v4, shp, spsi_
-        except dft.DftError as e:
+        except Exception as e:
             line["spinor"] = {"unavailable": str(e)}
         torch.cuda.empty_cache()
 

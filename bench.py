@@ -25,6 +25,7 @@ sys.path.insert(0, ROOT)
 METRIC = "H|psi> bands/s (FP64)"
 UNIT = "bands/s"
 FP64_PEAK_TFLOPS = 37.2      # 148 SM x 4 sub-partitions x one DMMA.8x8x4 (512 flop) per 16 clk x 1.965 GHz
+FAC_FLOPS_PER_CMAC = 4.75    # factorised projectors: 2 real DMMAs (4 flops) + the complex product conj(S) psi shared by 8 projectors (6/8)
 WORKLOADS = {
     "c0": "c0: Si2 FCC, Gamma, ecut 8 Ha, box 20^3, 8 bands, 16 projectors",
     "c1": "c1: Si64, k=(1/4,1/4,1/4), ecut 15 Ha, box 72^3, 128 bands, 512 projectors",
@@ -367,6 +368,8 @@ def main():
            and (args.gemm_sym == 1 or float(plan.nproj) * plan.mpw * nband >= 1e8))
     strassen = sym and args.gemm_strassen != 0 and plan.nproj % 16 == 0 and (args.gemm_strassen == 1 or float(plan.nproj) * plan.mpw * nband >= 1e10)
     fpc = (3.5 if strassen else 4.0) if sym else (6.0 if args.gemm_3m else 8.0)
+    if args.proj_mode:
+        fpc = FAC_FLOPS_PER_CMAC
     fft_bytes, g1_flops, g2_flops = byte_flop_model(plan, geo, nband, fpc)
     hbm_gbs, hbm_src = measured_peaks()
 
@@ -455,7 +458,7 @@ def main():
             "frac_vs_F_nl_8flop": t_roof8 * 1e3 / ms_step,
             "definition": "sum_phases max(bytes/HBM_measured, flops/FP64_peak) / measured step time; GEMM flops = %g per "
                           "(projector, plane wave, band) (the variant the kernels run: 3.5 = real GEMMs on the half sphere at "
-                          "k = 0 with one Strassen level, 4 = without it, 6 = Gauss, 8 = four products); frac_vs_F_nl_8flop uses SURVEY.md's dense 8-flop count F_nl" % fpc,
+                          "k = 0 with one Strassen level, 4 = without it, 4.75 = factorised projectors, 6 = Gauss, 8 = four products); frac_vs_F_nl_8flop uses SURVEY.md's dense 8-flop count F_nl" % fpc,
             "kernels": per_kernel}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -588,8 +591,26 @@ def main():
             f1.record()
             torch.cuda.synchronize()
             fms = f0.elapsed_time(f1) / 2
-            line["factorised_projectors"] = {"value": units / (fms * 1e-3), "unit": UNIT, "ms_per_step": fms,
-                                             "option": "proj_mode = 1 (FY.S tables instead of the materialised projector table)"}
+            plan.set_timing(True); plan.phase_ms()
+            plan.apply_h(psi, hpsi)
+            torch.cuda.synchronize()
+            fph = {k: round(v[0], 3) for k, v in plan.phase_ms().items() if v[0] > 0}
+            plan.set_timing(False)
+            # the mode's own roofline: per 8 projectors x 8 bands x 4 plane waves two real DMMAs (16 pipe clocks each) and the
+            # four FP64 instructions of z = conj(S) psi (2 clocks each alone; 2.55 measured next to DMMAs)
+            blocks = sum((int(n) + 3) // 4 for n in plan.npw) * (plan.nproj / 8.0) * (nband / 8.0)
+            clk_s = 148 * 4 * 1.965e9
+            ffl = FAC_FLOPS_PER_CMAC * plan.nproj * float(sum(int(n) for n in plan.npw)) * nband
+            line["factorised_projectors"] = {
+                "value": units / (fms * 1e-3), "unit": UNIT, "ms_per_step": fms, "phase_ms": fph,
+                "flops_per_complex_mac": FAC_FLOPS_PER_CMAC,
+                "gemm1_fp64_frac": ffl / (fph.get("gemm1", 1e30) * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                "gemm2_fp64_frac": ffl / (fph.get("gemm2_kinetic", 1e30) * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                "pipe_clock_bound_ms": {"nominal_40_clocks": blocks * 40.0 / clk_s * 1e3, "measured_mix_42.2_clocks": blocks * 42.2 / clk_s * 1e3},
+                "gemm1_frac_of_pipe_bound": blocks * 42.2 / clk_s * 1e3 / fph.get("gemm1", 1e30),
+                "gemm2_frac_of_pipe_bound": blocks * 42.2 / clk_s * 1e3 / fph.get("gemm2_kinetic", 1e30),
+                "option": "proj_mode = 1 (FY.S tables instead of the materialised projector table; 4.75 flops per (projector, "
+                          "plane wave, band): two real products and 6/8 of the complex product conj(S) psi)"}
         except Exception as e:
             line["factorised_projectors"] = {"unavailable": str(e)}
         plan.set_option("proj_mode", 0)

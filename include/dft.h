@@ -74,6 +74,20 @@ int dft_plan_create(dft_plan **out, const double rprimd[9], int32_t nkpt, const 
                     const double *xred, int32_t ntypat, const dft_proj_table *tables,
                     const double *dij);
 
+/* dft_plan_create followed by dft_plan_set_option(keys[i], values[i]) for i = 0 .. nopt-1, in that
+ * order (keys: HOST array of nopt C strings, values: HOST array of nopt integers; nopt may be 0).
+ * One option acts at creation time already: with "proj_mode" = 1 (the paper's "computed
+ * on-the-fly" projectors, PAPER.md :477) the materialised [nproj][mpw] table is never allocated
+ * nor filled, so a cell whose table does not fit in device memory (19.4 GB at c4, growing with
+ * natom^2) can still be planned; the radial-table range check (DFT_ERR_TABLE_RANGE) is done all
+ * the same.  Setting "proj_mode" = 0 later builds the table then.  Errors as dft_plan_create and
+ * dft_plan_set_option; on any error no plan is returned.                                         */
+int dft_plan_create_opts(dft_plan **out, const double rprimd[9], int32_t nkpt, const double *kpt,
+                         double ecut, const int32_t ngfft[3], int32_t natom, const int32_t *typat,
+                         const double *xred, int32_t ntypat, const dft_proj_table *tables,
+                         const double *dij, int32_t nopt, const char *const *keys,
+                         const int64_t *values);
+
 /* Sizes.  Any output pointer may be NULL.  npw: HOST [nkpt].  mpw = max_k npw_k is the leading
  * dimension of psi/hpsi.  workspace_bytes_per_band: device scratch dft_apply_h needs per band of
  * a band chunk (see dft_set_workspace).                                                          */
@@ -119,8 +133,9 @@ int dft_plan_workspace_bytes(const dft_plan *p, int32_t nband, int64_t *min_byte
 /* Options: "band_chunk" (bands per FFT pass launch, > 0), "terms" (bit 0 kinetic, bit 1 local,
  * bit 2 non-local, bit 3 meta-GGA term; default 15), "splitk" (GEMM-1 K splits, 0 = automatic), "proj_mode" (0 = default: projector table materialised in
  * device memory; 1 = factorised projectors FY.S evaluated inside both GEMMs; the table is freed (and rebuilt when the option
- * returns to 0; dft_plan_get_projectors gives DFT_ERR_NOT_READY meanwhile); an atom's projectors are taken in blocks of 8 and the form-factor rows of all types (8
- * per block) must not exceed 32, else DFT_ERR_UNSUPPORTED), "host_groups" (dft_apply_h_host only: band groups, default 6,
+ * returns to 0; dft_plan_get_projectors gives DFT_ERR_NOT_READY meanwhile); an atom's projectors are taken in blocks of 8; when the form-factor rows of all types (8
+ * per block) exceed 32, consecutive types are served in groups of at most 32 rows, both GEMMs once per group; see also
+ * dft_plan_create_opts, which never builds the table), "host_groups" (dft_apply_h_host only: band groups, default 6,
  * whose host<->device copies overlap the kernels of the neighbouring groups), "gemm_3m" (1 = default: three real
  * products per complex multiply-add in the projector GEMMs, 0 = four; same result up to rounding), "fft_path" (0 = automatic:
  * register-resident two-stage transforms where the box length factorises, their strided passes fed by a

@@ -32,7 +32,7 @@ PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather
           "fft_small_fused", "pack_unpack")
 
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
-SYMBOLS = ("dft_plan_create", "dft_plan_get_info", "dft_plan_workspace_bytes", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
+SYMBOLS = ("dft_plan_create", "dft_plan_create_opts", "dft_plan_get_info", "dft_plan_workspace_bytes", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_apply_hs", "dft_get_cprj", "dft_chebyshev_filter",
            "dft_set_vector_potential", "dft_accumulate_density", "dft_accumulate_tau",
            "dft_set_vtau", "dft_plan_get_kg_gamma", "dft_apply_h_gamma", "dft_chebyshev_filter_gamma", "dft_set_vloc_spinor", "dft_set_dij_spinor",
@@ -74,6 +74,7 @@ def lib():
     L.dft_plan_last_launches.argtypes = [C.c_void_p]
     L.dft_plan_create.argtypes = [C.POINTER(C.c_void_p), _dp, C.c_int32, _dp, C.c_double, _ip, C.c_int32, _ip, _dp,
                                   C.c_int32, C.POINTER(dft_proj_table), _dp]
+    L.dft_plan_create_opts.argtypes = L.dft_plan_create.argtypes + [C.c_int32, C.POINTER(C.c_char_p), C.POINTER(C.c_int64)]
     L.dft_plan_get_info.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip, C.POINTER(C.c_int64)]
     L.dft_plan_workspace_bytes.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.dft_plan_get_kg.argtypes = [C.c_void_p, C.c_int32, _ip, _ip, _dp]
@@ -135,9 +136,10 @@ def _i(a):
 
 
 # ------------------------------------------------------------------------------------- C-ABI mirrors
-def dft_plan_create(rprimd, kpt, ecut, ngfft, typat, xred, types, dij):
+def dft_plan_create(rprimd, kpt, ecut, ngfft, typat, xred, types, dij, options=None):
     """types: list of dicts with keys nlmn, l, m, irad, nrad, nq, dq, f[nrad][nq], f2[nrad][nq] (host).
-    Returns the opaque plan handle (int)."""
+    options: None, or a dict / list of (key, value) pairs handed to dft_plan_create_opts (proj_mode = 1 there means the
+    materialised projector table is never built).  Returns the opaque plan handle (int)."""
     rp = _f64(rprimd).reshape(9)
     kp = _f64(kpt).reshape(-1, 3)
     ng = _i32(ngfft).reshape(3)
@@ -155,8 +157,16 @@ def dft_plan_create(rprimd, kpt, ecut, ngfft, typat, xred, types, dij):
         tabs[t].f = _d(f); tabs[t].f2 = _d(f2)
     dj = _f64(dij) if dij is not None else None
     out = C.c_void_p()
-    rc = lib().dft_plan_create(C.byref(out), _d(rp), len(kp), _d(kp), float(ecut), _i(ng), natom,
-                               _i(ty) if natom else None, _d(xr) if natom else None, len(types), tabs, _d(dj))
+    if options is None:
+        rc = lib().dft_plan_create(C.byref(out), _d(rp), len(kp), _d(kp), float(ecut), _i(ng), natom,
+                                   _i(ty) if natom else None, _d(xr) if natom else None, len(types), tabs, _d(dj))
+    else:
+        items = list(options.items()) if isinstance(options, dict) else list(options)
+        keys = (C.c_char_p * max(1, len(items)))(*[str(k).encode() for k, _ in items])
+        vals = (C.c_int64 * max(1, len(items)))(*[int(v) for _, v in items])
+        rc = lib().dft_plan_create_opts(C.byref(out), _d(rp), len(kp), _d(kp), float(ecut), _i(ng), natom,
+                                        _i(ty) if natom else None, _d(xr) if natom else None, len(types), tabs, _d(dj),
+                                        len(items), keys, vals)
     _check(rc)
     return out.value
 
@@ -308,9 +318,9 @@ class Plan:
     """Owns one dft_plan.  `cfg` is a dict with rprimd, kpt, ecut, ngfft, typat, xred, types, dij
     (the layout synth.make_config produces); tensors are torch CUDA tensors."""
 
-    def __init__(self, cfg):
+    def __init__(self, cfg, options=None):
         self.h = dft_plan_create(cfg["rprimd"], cfg["kpt"], cfg["ecut"], cfg["ngfft"], cfg["typat"], cfg["xred"],
-                                 cfg["types"], cfg["dij"])
+                                 cfg["types"], cfg["dij"], options)
         info = dft_plan_get_info(self.h)
         self.nkpt, self.npw, self.mpw, self.nproj = info["nkpt"], info["npw"], info["mpw"], info["nproj"]
         self.workspace_bytes_per_band = info["workspace_bytes_per_band"]

@@ -105,6 +105,8 @@ struct PhaseTimer {
 
 }  // namespace dftb200
 
+struct FacGroup { int frow0, nfrow, blk0, nblk; };   // first FY row / rows, first block / blocks of one group of atom types (projtab.cu)
+
 struct dft_plan {
   // lattice
   double rprimd[9], bm[9], gmet[9];
@@ -133,8 +135,10 @@ struct dft_plan {
   double *d_stab = nullptr, *d_fytab = nullptr;      // factorised projectors: structure factors / form factors (proj_mode = 1)
   int32_t *d_blk_atom = nullptr, *d_blk_frow = nullptr, *d_blk_first = nullptr, *d_blk_nl = nullptr;   // projector blocks (<= 8 rows)
   int nblk = 0, nfrow = 0;                           // number of blocks; FY rows of all types
+  std::vector<FacGroup> fac_groups;                  // consecutive atom types whose FY rows fit the kernels' shared memory
   int ldf = 0;                                       // row length of d_fytab (mpw rounded up to 8)
   int proj_mode = 0;                                 // 0 = materialised table (GEMMs on P), 1 = factorised P = FY . S
+  bool skip_table_at_create = false;                 // dft_plan_create_opts(proj_mode = 1): never allocate the materialised table
   double *d_ptab = nullptr;                          // [nkpt][nproj][mpw] complex, zero padded beyond npw_k
   int32_t *d_npw = nullptr;                          // [nkpt]
   const double **d_kinptr = nullptr;                 // [nkpt] device pointers to kin of each k-point

@@ -640,10 +640,12 @@ constexpr int FC_OFF_S = NL_BN * 128;      // stage layout: psi tile 8 KB | S ti
 constexpr int FC_OFF_F = FC_OFF_S + FC_BA * 128;
 constexpr int FC_STAGE_BYTES = 12 * 1024;      // FY tile: FAC_MAX_FROWS rows x 8 doubles = 2 KB
 constexpr int FC_STAGES = 8;
-constexpr int FC_PREFETCH = FC_STAGES - 2;
 constexpr int FC_SMEM = FC_STAGES * FC_STAGE_BYTES + 1024 + 256;
 constexpr int FC_WARPS = 16;               // 4 (atom groups) x 4 (band groups): four warps per SM sub-partition hide the
-constexpr int FC_THREADS = FC_WARPS * 32;  // DMUL -> DFMA -> DMMA chains of the z = conj(S) psi products
+constexpr int FC_THREADS = FC_WARPS * 32 + 128;  // DMUL -> DFMA -> DMMA chains of the z = conj(S) psi products; warps 16-19 are the
+// producer group (lane 0 of warp 16 issues the TMA loads; a consumer that also issued them paced the ring).  A fifth warp per
+// sub-partition would cap every thread at 96 registers, so the producer warps shrink to 24 and the consumers take 112 (the pool is what the CTA got at launch: 640 x 96).
+__device__ __forceinline__ void reg_alloc_fac_consumer() { asm volatile("setmaxnreg.inc.sync.aligned.u32 112;"); }
 
 struct Fac1Params {
   int nblk, nfrow, nband, nproj, nslab, nsplit, slabs_per_split, tiles_n;
@@ -677,10 +679,14 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
     tma_load_3d(st + FC_OFF_S, &mapS, &full[s], (s0 + j) * 16, atom0, ik);
     tma_load_3d(st + FC_OFF_F, &mapF, &full[s], (s0 + j) * 8, 0, ik);
   };
-  const bool producer = (threadIdx.x == 0);
-  if (producer)
-    for (int j = 0; j < FC_PREFETCH && j < ns; j++) issue(j);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wm = warp >> 2, wn = warp & 3;   // 4 atoms x 16 bands per warp
+  if (warp >= FC_WARPS) {
+    reg_dealloc_producer();
+    if (warp == FC_WARPS && lane == 0)
+      for (int j = 0; j < ns; j++) issue(j);
+    return;
+  }
+  reg_alloc_fac_consumer();
   const int i = lane >> 2, j = lane & 3;
   int frow[4], arow[4];   // this lane's FY row (byte offset in the FY tile) and its block's S row, per block of the warp
 #pragma unroll
@@ -695,8 +701,6 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
 #pragma unroll
     for (int b = 0; b < 2; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
   for (int it = 0; it < ns; it++) {
-    if (producer && it + FC_PREFETCH < ns) issue(it + FC_PREFETCH);
-    __syncwarp();
     int s = it % FC_STAGES;
     mbar_wait(&full[s], (it / FC_STAGES) & 1);
     const unsigned char *Ps = tiles + s * FC_STAGE_BYTES, *Ss = Ps + FC_OFF_S, *Fs = Ps + FC_OFF_F;
@@ -749,7 +753,6 @@ gemm1_fac_kernel(const __grid_constant__ CUtensorMap mapPsi, const __grid_consta
 constexpr int FD_OFF_S = NL_BN * 128;                 // stage: c' tile 8 KB | S_a(G) 2 KB
 constexpr int FD_STAGE_BYTES = 10 * 1024;
 constexpr int FD_STAGES = 8;
-constexpr int FD_PREFETCH = FD_STAGES - 2;
 constexpr int FD_FLD = NL_BM + 4;                     // FY row stride in shared memory (doubles)
 constexpr int FD_FBYTES = FAC_MAX_FROWS * FD_FLD * 8;  // FY rows of every type for the tile's 128 G
 constexpr int FD_SMEM = FD_STAGES * FD_STAGE_BYTES + FD_FBYTES + 1024 + 256;
@@ -781,12 +784,16 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
     tma_load_3d(st, &mapC, &full[s], 2 * __ldg(blk_first + a), tn * NL_BN, ik);
     tma_load_3d(st + FD_OFF_S, &mapS, &full[s], tm * NL_BM * 2, __ldg(blk_atom + a), ik);
   };
-  const bool producer = (threadIdx.x == 0);
-  if (producer && ns > 0) {
-    mbar_expect_tx(fbar, (uint32_t)(nfrow * FD_FLD * 8));
-    tma_load_3d(Fs, &mapF, fbar, tm * NL_BM, 0, ik);
-    for (int a = 0; a < FD_PREFETCH && a < ns; a++) issue(a);
+  if (warp >= FC_WARPS) {
+    reg_dealloc_producer();
+    if (warp == FC_WARPS && lane == 0 && ns > 0) {
+      mbar_expect_tx(fbar, (uint32_t)(nfrow * FD_FLD * 8));
+      tma_load_3d(Fs, &mapF, fbar, tm * NL_BM, 0, ik);
+      for (int a = 0; a < ns; a++) issue(a);
+    }
+    return;
   }
+  reg_alloc_fac_consumer();
   double cre[4][2][2], cim[4][2][2];
 #pragma unroll
   for (int a = 0; a < 4; a++)
@@ -794,8 +801,6 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
     for (int b = 0; b < 2; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
   if (ns > 0) mbar_wait(fbar, 0);
   for (int a = 0; a < ns; a++) {
-    if (producer && a + FD_PREFETCH < ns) issue(a + FD_PREFETCH);
-    __syncwarp();
     int s = a % FD_STAGES;
     const int fr0 = __ldg(blk_frow + a);      // first FY row of this block
     mbar_wait(&full[s], (a / FD_STAGES) & 1);
@@ -1232,7 +1237,9 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   // few projectors (nproj <= 64): the 4-product GEMM-1 with a 32- or 64-row tile instead of 128 padded rows
   const int skinny_mb = (!fac && nproj <= 32) ? 1 : ((!fac && nproj <= 64) ? 2 : 0);
   const int bm1 = skinny_mb ? 32 * skinny_mb : NL_BM;
-  q1.tiles_m = fac ? (p->nblk + FC_BA - 1) / FC_BA : (nproj + bm1 - 1) / bm1; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
+  int fac_tiles = 0;                      // tiles of 16 projector blocks, summed over the groups of atom types
+  if (fac) for (const FacGroup &G : p->fac_groups) fac_tiles += (G.nblk + FC_BA - 1) / FC_BA;
+  q1.tiles_m = fac ? fac_tiles : (nproj + bm1 - 1) / bm1; q1.tiles_n = (nband + NL_BN - 1) / NL_BN;
   int ns = p->splitk > 0 ? p->splitk : choose_splitk(q1.tiles_m * q1.tiles_n, q1.nslab, p->sm_count, nkpt);
   if (ns > q1.nslab) ns = q1.nslab;
   q1.slabs_per_split = (q1.nslab + ns - 1) / ns;
@@ -1262,14 +1269,22 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     if ((rc = make_map(p, &mapPsi, psi, 2 * (uint64_t)mpw, nband, nkpt, rowb, rowb * nband, NL_BN))) return rc;
     C->psi = psi; C->nband_psi = nband;
   }
-  CUtensorMap mapS1, mapF1, mapS2, mapF2;
+  // factorised mode: one S map for all atoms and one pair of FY maps per group of atom types (projtab.cu)
+  CUtensorMap mapS1, mapS2;
+  std::vector<CUtensorMap> mapF1, mapF2;
+  const size_t ngrp = fac ? p->fac_groups.size() : 0;
   if (fac) {
     if (!p->d_stab || !p->d_fytab) { set_error("factor tables missing"); return DFT_ERR_NOT_READY; }
     const uint64_t frow = (uint64_t)p->ldf * 8, nfr = (uint64_t)p->nfrow;
     if ((rc = make_map(p, &mapS1, p->d_stab, 2 * (uint64_t)mpw, p->natom, nkpt, rowb, rowb * p->natom, FC_BA))) return rc;
-    if ((rc = make_map_plain(p, &mapF1, p->d_fytab, p->ldf, nfr, nkpt, frow, frow * nfr, 8, (uint32_t)nfr))) return rc;
     if ((rc = make_map_plain(p, &mapS2, p->d_stab, 2 * (uint64_t)mpw, p->natom, nkpt, rowb, rowb * p->natom, 2 * NL_BM, 1))) return rc;
-    if ((rc = make_map_plain(p, &mapF2, p->d_fytab, p->ldf, nfr, nkpt, frow, frow * nfr, FD_FLD, (uint32_t)nfr))) return rc;
+    mapF1.resize(ngrp); mapF2.resize(ngrp);
+    for (size_t g = 0; g < ngrp; g++) {
+      const FacGroup &G = p->fac_groups[g];
+      const double *base = p->d_fytab + (size_t)G.frow0 * p->ldf;
+      if ((rc = make_map_plain(p, &mapF1[g], base, p->ldf, G.nfrow, nkpt, frow, frow * nfr, 8, (uint32_t)G.nfrow))) return rc;
+      if ((rc = make_map_plain(p, &mapF2[g], base, p->ldf, G.nfrow, nkpt, frow, frow * nfr, FD_FLD, (uint32_t)G.nfrow))) return rc;
+    }
   }
   if (!fac && !tab_same) {
     // GEMM-2 reads P "M-major": view each table row as [g-block][16 doubles] and put the projector
@@ -1293,11 +1308,16 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   }
   phase_begin(p, 5, st);
   if (fac) {
-    Fac1Params f1;
-    f1.nblk = p->nblk; f1.nfrow = p->nfrow; f1.nband = nband; f1.nproj = nproj; f1.nslab = q1.nslab; f1.nsplit = q1.nsplit;
-    f1.slabs_per_split = q1.slabs_per_split; f1.tiles_n = q1.tiles_n;
-    f1.blk_atom = p->d_blk_atom; f1.blk_frow = p->d_blk_frow; f1.blk_first = p->d_blk_first; f1.blk_nl = p->d_blk_nl; f1.part = q1.part;
-    gemm1_fac_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), FC_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1, f1);
+    for (size_t g = 0; g < ngrp; g++) {     // every group writes its own rows of the partial sums
+      const FacGroup &G = p->fac_groups[g];
+      Fac1Params f1;
+      f1.nblk = G.nblk; f1.nfrow = G.nfrow; f1.nband = nband; f1.nproj = nproj; f1.nslab = q1.nslab; f1.nsplit = q1.nsplit;
+      f1.slabs_per_split = q1.slabs_per_split; f1.tiles_n = q1.tiles_n;
+      f1.blk_atom = p->d_blk_atom + G.blk0; f1.blk_frow = p->d_blk_frow + G.blk0; f1.blk_first = p->d_blk_first + G.blk0;
+      f1.blk_nl = p->d_blk_nl + G.blk0; f1.part = q1.part;
+      const int tiles_a = (G.nblk + FC_BA - 1) / FC_BA;
+      gemm1_fac_kernel<<<dim3(tiles_a * q1.tiles_n, ns, nkpt), FC_THREADS, FC_SMEM, st>>>(mapPsi, mapS1, mapF1[g], f1);
+    }
   } else if (skinny_mb == 1) gemm1_kernel<false, 1><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   else if (skinny_mb == 2) gemm1_kernel<false, 2><<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP1, mapPsi, q1);
   else if (p->gemm_3m) gemm1_3m_kernel<<<dim3(q1.tiles_m * q1.tiles_n, ns, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP1, mapPsi, q1);
@@ -1326,11 +1346,21 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   q2.xprev = rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr; q2.raw = 0;
   int tiles_m2 = (mpw + NL_BM - 1) / NL_BM;
   phase_begin(p, 7, st);
-  if (fac) {
-    q2.nslab = p->nblk;
-    gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_blk_atom,
-                                                                                      p->d_blk_frow, p->d_blk_first, p->nfrow);
-  } else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
+  // factorised GEMM-2, once per group of atom types: the first launch carries the caller's accumulate flag and the kinetic
+  // term, the later ones add to its output, and the last one applies the recurrence to the total
+  auto launch_gemm2_fac = [&](Gemm2Params q) {
+    for (size_t g = 0; g < ngrp; g++) {
+      const FacGroup &G = p->fac_groups[g];
+      Gemm2Params qg = q;
+      qg.nslab = G.nblk;
+      if (g > 0) { qg.accumulate = 1; qg.with_kin = 0; }
+      if (g + 1 < ngrp) { qg.cheb = 0; }
+      gemm2_fac_kernel<<<dim3(q.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(
+          mapC, mapS2, mapF2[g], qg, p->d_blk_atom + G.blk0, p->d_blk_frow + G.blk0, p->d_blk_first + G.blk0, G.nfrow);
+    }
+  };
+  if (fac) launch_gemm2_fac(q2);
+  else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
   else gemm2_kernel<false><<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP2, mapC, q2);
   phase_end(p, 7, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
@@ -1344,8 +1374,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     q2.accumulate = 0; q2.with_kin = 1; q2.kin = p->d_oneptr; q2.hpsi = reinterpret_cast<double2 *>(spsi);
     q2.cheb = 0; q2.sh = 1.0; q2.sy = 0.0; q2.sx = 0.0; q2.xprev = nullptr;
     phase_begin(p, 7, st);
-    if (fac) gemm2_fac_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), FC_THREADS, FD_SMEM, st>>>(mapC, mapS2, mapF2, q2, p->d_blk_atom,
-                                                                                               p->d_blk_frow, p->d_blk_first, p->nfrow);
+    if (fac) launch_gemm2_fac(q2);
     else if (p->gemm_3m) gemm2_3m_kernel<<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL3_THREADS, NL_SMEM, st>>>(mapP2, mapC, q2);
     else gemm2_kernel<false><<<dim3(q2.tiles_n * tiles_m2, 1, nkpt), NL_THREADS_P, NL_SMEM, st>>>(mapP2, mapC, q2);
     phase_end(p, 7, st, 1);

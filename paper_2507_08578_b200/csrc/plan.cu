@@ -226,7 +226,7 @@ static int create_impl(dft_plan *p, const double rprimd[9], int32_t nkpt, const 
     if ((rc = to_device((const double ***)&p->d_oneptr, optr.data(), nkpt))) return rc;
   }
   size_t tab = (size_t)nkpt * p->nproj * p->mpw * 16;
-  if (tab) {
+  if (tab && !p->skip_table_at_create) {     // dft_plan_create_opts with proj_mode = 1: the table is never built (19.4 GB at c4)
     if (cudaMalloc(&p->d_ptab, tab + 256) != cudaSuccess) {
       cudaGetLastError();
       set_error("cannot allocate the projector table (%zu bytes)", tab);
@@ -407,6 +407,28 @@ int dft_plan_create(dft_plan **out, const double rprimd[9], int32_t nkpt, const 
   if (natom > 0 && (!typat || !xred || !tables || ntypat < 1)) { set_error("atoms given without typat/xred/tables"); return DFT_ERR_INVALID_ARG; }
   dft_plan *p = new dft_plan();
   int rc = create_impl(p, rprimd, nkpt, kpt, ecut, ngfft, natom, typat, xred, ntypat, tables, dij);
+  if (rc != DFT_OK) { destroy_plan(p); return rc; }
+  *out = p;
+  return DFT_OK;
+  DFT_GUARD_END
+}
+
+int dft_plan_create_opts(dft_plan **out, const double rprimd[9], int32_t nkpt, const double *kpt, double ecut, const int32_t ngfft[3],
+                         int32_t natom, const int32_t *typat, const double *xred, int32_t ntypat, const dft_proj_table *tables,
+                         const double *dij, int32_t nopt, const char *const *keys, const int64_t *values) {
+  DFT_GUARD_BEGIN
+  if (!out || !rprimd || !kpt || !ngfft) { set_error("null argument"); return DFT_ERR_INVALID_ARG; }
+  if (nkpt < 1) { set_error("nkpt = %d must be >= 1", nkpt); return DFT_ERR_INVALID_ARG; }
+  if (!(ecut > 0.0) || !isfinite(ecut)) { set_error("ecut = %g must be positive and finite", ecut); return DFT_ERR_INVALID_ARG; }
+  if (natom < 0 || ntypat < 0) { set_error("negative natom/ntypat"); return DFT_ERR_INVALID_ARG; }
+  if (natom > 0 && (!typat || !xred || !tables || ntypat < 1)) { set_error("atoms given without typat/xred/tables"); return DFT_ERR_INVALID_ARG; }
+  if (nopt < 0 || (nopt > 0 && (!keys || !values))) { set_error("nopt = %d without keys/values", nopt); return DFT_ERR_INVALID_ARG; }
+  for (int i = 0; i < nopt; i++) if (!keys[i]) { set_error("option %d has a null key", i); return DFT_ERR_INVALID_ARG; }
+  dft_plan *p = new dft_plan();
+  // the last value given for proj_mode decides whether the materialised table is built at all
+  for (int i = 0; i < nopt; i++) if (!strcmp(keys[i], "proj_mode")) p->skip_table_at_create = (values[i] == 1);
+  int rc = create_impl(p, rprimd, nkpt, kpt, ecut, ngfft, natom, typat, xred, ntypat, tables, dij);
+  for (int i = 0; i < nopt && rc == DFT_OK; i++) rc = dft_plan_set_option(p, keys[i], values[i]);
   if (rc != DFT_OK) { destroy_plan(p); return rc; }
   *out = p;
   return DFT_OK;

@@ -125,6 +125,7 @@ int build_projector_table(dft_plan *p, int ik, double *maxq_out) {
                 *maxq_out, (p->nq[t] - 1) * p->dq[t], t);
       return DFT_ERR_TABLE_RANGE;
     }
+  if (!p->d_ptab) return DFT_OK;      // plan created in factorised mode: the range check above is all that is needed here
   ProjParams P;
   for (int i = 0; i < 9; i++) P.bm[i] = p->bm[i];
   for (int i = 0; i < 3; i++) P.k[i] = kp.k[i];
@@ -161,10 +162,12 @@ int build_projector_table_on(dft_plan *p, const int32_t *d_kg, int npw, int mpw,
 // Factorised projectors (PAPER.md :477 "computed on-the-fly"): p_{a,i}(m) = FY_{t(a),i}(m) . S_a(m)
 // with FY = F.Y real (one row per projector of an atom TYPE) and S_a(m) = exp(-2 pi i (k+m).x_a) (one row per ATOM).
 // The two small tables replace the [nproj][mpw] complex one: S [natom][mpw] complex, FY [ntypat*8][ldf] real
-// (whole 8-row blocks per type, rows >= nlmn zero), zero for ipw >= npw_k.
+// (whole 8-row blocks per type, rows >= nlmn zero), zero for ipw >= npw_k.  Row r of S belongs to atom srow_atom[r]: the
+// atoms in the order of the block list (by type group, see build_factor_tables), so that the 16 blocks of a GEMM-1 tile
+// read 16 consecutive S rows whatever the order of the types in typat.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(PT_THREADS) stab_kernel(ProjParams P, double2 *__restrict__ stab) {
-  int g = blockIdx.x * PT_THREADS + threadIdx.x, a = blockIdx.y;
+__global__ void __launch_bounds__(PT_THREADS) stab_kernel(ProjParams P, double2 *__restrict__ stab, const int32_t *__restrict__ srow_atom) {
+  int g = blockIdx.x * PT_THREADS + threadIdx.x, a = srow_atom[blockIdx.y];
   if (g >= P.mpw) return;
   double2 v = make_double2(0.0, 0.0);
   if (g < P.npw) {
@@ -176,7 +179,7 @@ __global__ void __launch_bounds__(PT_THREADS) stab_kernel(ProjParams P, double2 
     sincospi(2.0 * arg, &sn, &cs);
     v = make_double2(cs, -sn);
   }
-  stab[(size_t)a * P.mpw + g] = v;
+  stab[(size_t)blockIdx.y * P.mpw + g] = v;
 }
 
 __global__ void __launch_bounds__(PT_THREADS) fytab_kernel(ProjParams P, double *__restrict__ fy, int ldf,
@@ -209,8 +212,10 @@ __global__ void __launch_bounds__(PT_THREADS) fytab_kernel(ProjParams P, double 
 }
 
 // Builds (or rebuilds) both tables for every k-point, and the list of projector BLOCKS the factorised GEMMs walk: an atom
-// with nlmn projectors contributes ceil(nlmn / 8) blocks of up to 8 rows (M = 8 of the DMMA shape).  DFT_ERR_UNSUPPORTED
-// if the FY rows of all types (8 per block) exceed FAC_MAX_FROWS.
+// with nlmn projectors contributes ceil(nlmn / 8) blocks of up to 8 rows (M = 8 of the DMMA shape).  The kernels keep the
+// FY rows they need in shared memory, at most FAC_MAX_FROWS of them, so the atom types are cut into GROUPS of consecutive
+// types whose rows (8 or 16 per type) fit; the block list is ordered by group and both GEMMs run once per group on that
+// group's blocks and FY rows (one group for up to 32 rows, e.g. four types of 8 projectors).
 template <typename T>
 static int upload_vec(T **dst, const std::vector<T> &v) {
   cudaFree(*dst); *dst = nullptr;
@@ -223,26 +228,43 @@ static int upload_vec(T **dst, const std::vector<T> &v) {
 int build_factor_tables(dft_plan *p) {
   if (p->natom == 0 || p->nproj == 0 || p->mpw == 0) return DFT_OK;
   std::vector<int32_t> row0(p->ntypat), rows(p->ntypat);
+  std::vector<int> grp(p->ntypat, 0);
   int nfrow = 0;
-  for (int t = 0; t < p->ntypat; t++) { row0[t] = nfrow; rows[t] = (p->nlmn[t] + 7) / 8 * 8; nfrow += rows[t]; }
-  if (nfrow > FAC_MAX_FROWS) {
-    set_error("factorised projectors: %d form-factor rows (8 per block of projectors, all types) exceed %d", nfrow, FAC_MAX_FROWS);
-    return DFT_ERR_UNSUPPORTED;
-  }
-  std::vector<int32_t> b_atom, b_frow, b_first, b_nl;
-  for (int a = 0; a < p->natom; a++) {
-    int t = p->typat[a], nl = p->nlmn[t];
-    for (int mb = 0; mb * 8 < nl; mb++) {
-      b_atom.push_back(a); b_frow.push_back(row0[t] + 8 * mb); b_first.push_back(p->atom_first[a] + 8 * mb);
-      b_nl.push_back(nl - 8 * mb < 8 ? nl - 8 * mb : 8);
+  p->fac_groups.clear();
+  for (int t = 0; t < p->ntypat; t++) {
+    row0[t] = nfrow; rows[t] = (p->nlmn[t] + 7) / 8 * 8; nfrow += rows[t];
+    if (rows[t] == 0) { grp[t] = -1; continue; }
+    if (p->fac_groups.empty() || p->fac_groups.back().nfrow + rows[t] > FAC_MAX_FROWS) {
+      FacGroup g; g.frow0 = row0[t]; g.nfrow = 0; g.blk0 = 0; g.nblk = 0;
+      p->fac_groups.push_back(g);
     }
+    p->fac_groups.back().nfrow += rows[t];
+    grp[t] = (int)p->fac_groups.size() - 1;
   }
+  std::vector<int32_t> b_atom, b_frow, b_first, b_nl, srow_atom;
+  for (size_t g = 0; g < p->fac_groups.size(); g++) {
+    FacGroup &G = p->fac_groups[g];
+    G.blk0 = (int)b_atom.size();
+    for (int a = 0; a < p->natom; a++) {
+      int t = p->typat[a], nl = p->nlmn[t];
+      if (grp[t] != (int)g) continue;
+      const int srow = (int)srow_atom.size();
+      srow_atom.push_back(a);
+      for (int mb = 0; mb * 8 < nl; mb++) {
+        b_atom.push_back(srow); b_frow.push_back(row0[t] - G.frow0 + 8 * mb); b_first.push_back(p->atom_first[a] + 8 * mb);
+        b_nl.push_back(nl - 8 * mb < 8 ? nl - 8 * mb : 8);
+      }
+    }
+    G.nblk = (int)b_atom.size() - G.blk0;
+  }
+  for (int a = 0; a < p->natom; a++)          // atoms without projectors: rows nobody reads, kept so that the table has natom rows
+    if (p->nlmn[p->typat[a]] == 0) srow_atom.push_back(a);
   p->nblk = (int)b_atom.size(); p->nfrow = nfrow;
   int rc;
-  int32_t *d_row0 = nullptr, *d_rows = nullptr;
+  int32_t *d_row0 = nullptr, *d_rows = nullptr, *d_srow = nullptr;
   if ((rc = upload_vec(&p->d_blk_atom, b_atom)) || (rc = upload_vec(&p->d_blk_frow, b_frow)) ||
       (rc = upload_vec(&p->d_blk_first, b_first)) || (rc = upload_vec(&p->d_blk_nl, b_nl)) ||
-      (rc = upload_vec(&d_row0, row0)) || (rc = upload_vec(&d_rows, rows))) return rc;
+      (rc = upload_vec(&d_row0, row0)) || (rc = upload_vec(&d_rows, rows)) || (rc = upload_vec(&d_srow, srow_atom))) return rc;
   p->ldf = (p->mpw + 7) / 8 * 8;
   size_t sbytes = (size_t)p->nkpt * p->natom * p->mpw * 16 + 256, fbytes = (size_t)p->nkpt * nfrow * p->ldf * 8 + 256;
   if (!p->d_stab && cudaMalloc(&p->d_stab, sbytes) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the structure-factor table (%zu bytes)", sbytes); return DFT_ERR_ALLOC; }
@@ -257,12 +279,12 @@ int build_factor_tables(dft_plan *p) {
     P.lmn_irad = p->d_lmn_irad; P.atom_first = p->d_atom_first; P.nq = p->d_nq; P.dq = p->d_dq; P.xred = p->d_xred;
     P.f = p->d_f; P.f2 = p->d_f2; P.ptab = nullptr; P.rot_odd = 0;
     stab_kernel<<<dim3((p->mpw + PT_THREADS - 1) / PT_THREADS, p->natom), PT_THREADS>>>(
-        P, reinterpret_cast<double2 *>(p->d_stab) + (size_t)ik * p->natom * p->mpw);
+        P, reinterpret_cast<double2 *>(p->d_stab) + (size_t)ik * p->natom * p->mpw, d_srow);
     fytab_kernel<<<dim3((p->ldf + PT_THREADS - 1) / PT_THREADS, p->ntypat), PT_THREADS>>>(
         P, p->d_fytab + (size_t)ik * nfrow * p->ldf, p->ldf, d_row0, d_rows);
   }
   cudaError_t e = cudaDeviceSynchronize();
-  cudaFree(d_row0); cudaFree(d_rows);
+  cudaFree(d_row0); cudaFree(d_rows); cudaFree(d_srow);
   if (e != cudaSuccess) { set_error("factor-table kernels failed: %s", cudaGetErrorString(e)); return DFT_ERR_CUDA; }
   return DFT_OK;
 }

@@ -23,7 +23,7 @@ BASE_SEED = 20250708
 STREAM_PSI, STREAM_VNOISE, STREAM_DIJ = 1, 2, 3
 
 CONFIG_NAMES = ("c0", "c1", "c2", "c3", "c4",
-                "c1m", "c2m", "c4m", "aniso", "c3k2", "aniso8", "anisok3")
+                "c1m", "c2m", "c4m", "aniso", "c3k2", "aniso8", "anisok3", "aniso5t")
 
 _DIAMOND_SITES = np.array([[0, 0, 0], [0, .5, .5], [.5, 0, .5], [.5, .5, 0],
                            [.25, .25, .25], [.25, .75, .75], [.75, .25, .75], [.75, .75, .25]])
@@ -177,6 +177,13 @@ def make_config(name, with_vloc=True, **over):
         xred = np.array([[0.0, 0.0, 0.0], [0.3183098861837907, 0.7071067811865476, 0.5772156649015329],
                          [0.55, 0.25, 0.8], [0.12, 0.61, 0.33]])
         kinds = ["Si", "Sip"]; typat = np.array([1, 0, 1, 0], np.int32)
+        kpt = [[0.1, -0.2, 0.05]]
+        ecut, ngfft, nband = 2.5, (20, 24, 30), 5
+    elif name == "aniso5t":   # five atom types in mixed order (8, 9, 4, 9 and 8 projectors): more form-factor rows than the
+        rprimd = np.array([[9.0, 0.4, -0.3], [0.7, 10.5, 0.5], [-0.6, 0.8, 13.0]])   # factorised kernels hold at once
+        xred = np.array([[0.0, 0.0, 0.0], [0.3183098861837907, 0.7071067811865476, 0.5772156649015329],
+                         [0.55, 0.25, 0.8], [0.12, 0.61, 0.33], [0.81, 0.07, 0.44], [0.37, 0.9, 0.15], [0.66, 0.52, 0.6]])
+        kinds = ["Si", "Al", "Sip", "Al", "Si"]; typat = np.array([4, 1, 0, 3, 2, 1, 0], np.int32)
         kpt = [[0.1, -0.2, 0.05]]
         ecut, ngfft, nband = 2.5, (20, 24, 30), 5
     else:

@@ -7,8 +7,8 @@ import synth
 import paper_2507_08578_b200 as dft
 
 
-def make_plan(cfg):
-    plan = dft.Plan(cfg)
+def make_plan(cfg, options=None):
+    plan = dft.Plan(cfg, options)
     if "vloc" in cfg:
         v = torch.as_tensor(cfg["vloc"], device="cuda")
         plan.set_vloc(v)

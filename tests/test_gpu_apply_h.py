@@ -5,6 +5,7 @@ import pytest
 import torch
 
 import oracle
+import paper_2507_08578_b200 as dft
 import synth
 from gpu_util import (make_plan, lib_spheres, oracle_spheres, assert_spheres_equal, gpu_apply, oracle_apply,
                       band_rel_err, small_box_ok)
@@ -21,14 +22,14 @@ def _setup(name, **over):
     return cfg, plan, sph
 
 
-@pytest.mark.parametrize("name", ["c0", "c1m", "c2m", "c4m", "aniso", "aniso8", "c3k2"])
+@pytest.mark.parametrize("name", ["c0", "c1m", "c2m", "c4m", "aniso", "aniso8", "c3k2", "aniso5t"])
 def test_small_cells_all_terms_and_isolations(name):
     cfg, plan, sph = _setup(name)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     for terms in (7, 1, 2, 4, 3, 6):
         plan.set_option("terms", terms)
         got = gpu_apply(plan, psi)
-        ref = oracle_apply(cfg, sph, psi, terms=terms, method=1 if name in ("c0", "aniso", "aniso8") else 2)
+        ref = oracle_apply(cfg, sph, psi, terms=terms, method=1 if name in ("c0", "aniso", "aniso8", "aniso5t") else 2)
         err = band_rel_err(got, ref)
         assert err <= TOL, "%s terms=%d: rel err %.3e" % (name, terms, err)
         for ik in range(plan.nkpt):                      # pad entries are written as 0
@@ -414,11 +415,12 @@ def test_symmetric_table_gemms_with_other_terms(nband):
     plan.destroy()
 
 
-@pytest.mark.parametrize("name", ["c1m", "c4m", "c2m", "aniso", "aniso8", "c3k2"])
+@pytest.mark.parametrize("name", ["c1m", "c4m", "c2m", "aniso", "aniso8", "c3k2", "aniso5t"])
 def test_factorised_projectors(name):
     """Option proj_mode = 1 (PAPER.md :477 "computed on-the-fly"): p = FY . S evaluated inside both GEMMs instead of the
     materialised table; H psi, S psi and cprj must match the oracle as before.  Atoms with more than 8 projectors (Al: 9)
-    are walked as two blocks of 8 rows."""
+    are walked as two blocks of 8 rows; aniso5t has five atom types in mixed order whose 56 form-factor rows exceed what
+    the kernels hold at once, so both GEMMs run once per group of types."""
     cfg, plan, sph = _setup(name)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     tpsi = torch.as_tensor(psi, device="cuda")
@@ -440,10 +442,48 @@ def test_factorised_projectors(name):
         assert float(np.max(np.linalg.norm(cp[ik] - cref, axis=1) / np.linalg.norm(cref, axis=1))) <= TOL
         sref = oracle.apply_s(cfg, ik, kg, psi[ik], sij)
         assert float(np.max(np.linalg.norm(got[ik] - sref, axis=1) / np.linalg.norm(sref, axis=1))) <= TOL
-    plan.set_option("proj_mode", 0)
     plan.set_option("terms", 15)
+    if name in ("aniso5t", "aniso"):     # the recurrence in the epilogue of the LAST group's GEMM-2 only
+        kmax = max(float(s[2].max()) for s in sph)
+        cen, e = 0.5 * kmax + 1.0, 0.5 * kmax + 0.5
+        got = plan.chebyshev_filter(tpsi.clone(), 3, cen, e).cpu().numpy()
+        for ik, (kg, ig, kin) in enumerate(sph):
+            ref = oracle.chebyshev_filter(cfg, ik, kg, ig, kin, psi[ik], 3, cen, e, method=1)
+            npw = len(ig)
+            assert float(np.max(np.linalg.norm(got[ik][:, :npw] - ref[:, :npw], axis=1) / np.linalg.norm(ref[:, :npw], axis=1))) <= TOL
+    plan.set_option("proj_mode", 0)
     assert band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, method=m)) <= TOL
     plan.destroy()
+
+
+def test_plan_created_in_factorised_mode_never_builds_the_table():
+    """dft_plan_create_opts with proj_mode = 1: the [nproj][mpw] table is neither allocated nor filled (device memory in
+    use grows by less than the table's size), H psi matches the oracle, reading the table back is refused, the radial-table
+    range check still fires, an unknown key is refused without leaking a plan, and proj_mode = 0 later builds the table."""
+    cfg = synth.make_config("c2m", ecut=4.0)
+    torch.cuda.synchronize(); torch.cuda.empty_cache()
+    free0 = torch.cuda.mem_get_info()[0]
+    plan = make_plan(cfg, options=[("proj_mode", 1), ("terms", 15)])
+    torch.cuda.synchronize()
+    used = free0 - torch.cuda.mem_get_info()[0]
+    tab = plan.nproj * plan.mpw * 16
+    assert tab > (64 << 20), "the cell is too small for the memory check to mean anything"
+    assert used < tab // 2, "plan took %d bytes, the table alone would be %d" % (used, tab)
+    sph = lib_spheres(plan)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    assert band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, method=2)) <= TOL
+    with pytest.raises(dft.DftError):
+        plan.get_projectors(0)
+    plan.set_option("proj_mode", 0)
+    assert band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, method=2)) <= TOL
+    assert plan.get_projectors(0).shape == (plan.nproj, plan.npw[0])
+    plan.destroy()
+    with pytest.raises(dft.DftError):
+        make_plan(cfg, options={"proj_mode": 1, "no_such_option": 3})
+    short = dict(cfg, types=[dict(t, nq=t["nq"] // 2, f=t["f"][:, :t["nq"] // 2].copy(), f2=t["f2"][:, :t["nq"] // 2].copy()) for t in cfg["types"]])
+    with pytest.raises(dft.DftError) as ei:
+        make_plan(short, options={"proj_mode": 1})
+    assert ei.value.code == dft.DFT_ERR_TABLE_RANGE
 
 
 def test_apply_h_is_cuda_graph_capturable():

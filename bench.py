@@ -666,9 +666,21 @@ def main():
             s0.record(); plan.apply_h_spinor(spsi_, shp); s1.record()
             torch.cuda.synchronize()
             sms = s0.elapsed_time(s1)
+            plan.set_timing(True); plan.phase_ms()
+            plan.apply_h_spinor(spsi_, shp)
+            torch.cuda.synchronize()
+            sph_ms = {k: round(v[0], 3) for k, v in plan.phase_ms().items() if v[0] > 0}
+            plan.set_timing(False)
+            plan.set_option("spinor_fused", 0)      # the four scalar applications of the Pauli decomposition, for comparison
+            plan.apply_h_spinor(spsi_, shp)
+            s0.record(); plan.apply_h_spinor(spsi_, shp); s1.record()
+            torch.cuda.synchronize()
+            pms = s0.elapsed_time(s1)
+            plan.set_option("spinor_fused", 1)
             line["spinor"] = {"value": plan.nkpt * snb / (sms * 1e-3), "unit": "spinor bands/s", "ms_per_step": sms,
-                              "spinor_bands": snb, "api": "dft_apply_h_spinor (scalar D_ij on both components; four scalar "
-                              "local applications for the 2x2 potential)"}
+                              "spinor_bands": snb, "phase_ms": sph_ms, "ms_per_step_pauli_four_applications": pms,
+                              "api": "dft_apply_h_spinor (scalar D_ij on both components; one local application, the 2x2 "
+                                     "potential multiplied in pass C)"}
             del v4, shp, spsi_
         except Exception as e:
             line["spinor"] = {"unavailable": str(e)}

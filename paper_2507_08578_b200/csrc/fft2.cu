@@ -309,6 +309,81 @@ fft2_c_kernel(Fft2Geom G0, Fft2Batch B, cplx *__restrict__ T2, const double *__r
   }
 }
 
+// ---- pass C for two-component spinors (PAPER.md :448; reading 27): the rows of T2 come in pairs (2 j, 2 j + 1) =
+//      (up, down) component of spinor band j, and the potential is the Hermitian 2 x 2 matrix V^{ss'}(r), given as the four
+//      real fields v4 = (V_upup, V_dndn, Re V_updn, Im V_updn) / N:
+//          out_up = V_upup psi_up + V_updn psi_dn,     out_dn = conj(V_updn) psi_up + V_dndn psi_dn     at every point r.
+//      A tile is 8 consecutive x of BOTH components: lanes px = 0..7 hold the up component, px = 8..15 the down component of
+//      the same points, so after the forward transform the partner value sits in lane ^ 8 of the same warp and one
+//      shuffle per number replaces any second pass over the data: one local application for the whole 2 x 2 matrix
+//      instead of the four of the Pauli decomposition (spinor.cu).  Same exchanges and twiddles as fft2_c_kernel.
+template <int R1, int R2>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+fft2_c_spinor_kernel(Fft2Geom G, cplx *__restrict__ T2, const double *__restrict__ v4, int nxt, int nsb) {
+  constexpr int NS = imax(R1, R2), XT = 16;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  cplx *sm = reinterpret_cast<cplx *>(smem_raw);
+  const int t = threadIdx.x, px = t % XT, s = t / XT, comp = px >> 3;
+  const int sb = blockIdx.x % nsb, tile = blockIdx.x / nsb, xt = tile % nxt, y = tile / nxt;
+  const int x = xt * 8 + (px & 7);
+  const bool xok = x < G.n1;
+  constexpr int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
+  const size_t pstride = (size_t)G.n2 * G.n1;
+  cplx *base = T2 + (size_t)(2 * sb + comp) * G.t2_band + (size_t)y * G.n1 + (xok ? x : 0);
+  cplx v[NS];
+  if (s < R2) {
+#pragma unroll
+    for (int j1 = 0; j1 < R1; j1++) {
+      int p = xok ? run_map(G.zrun, s + R2 * j1) : -1;
+      v[j1] = p >= 0 ? base[(size_t)p * pstride] : make_double2(0.0, 0.0);
+    }
+    Dft<R1, +1>::run(v);
+#pragma unroll
+    for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw3, s * k1));
+#pragma unroll
+    for (int k1 = 0; k1 < R1; k1++) sm[k1 * KSa + s * XT + px] = v[k1];
+  }
+  __syncthreads();
+  if (s < R1) {
+#pragma unroll
+    for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KSa + j2 * XT + px];
+  }
+  __syncthreads();   // every read of the forward exchange is done before the buffer is reused
+  if (s < R1) {
+    Dft<R2, +1>::run(v);
+    // thread s now holds psi_comp(r) at z = s + R1 k2; its partner lane (^ 8) holds the other component at the same points.
+    // The 16 lanes of a half-warp share s, so the branch is uniform per half-warp and the shuffle names that half only.
+    const unsigned half = 0xffffu << (t & 16);
+    const size_t nbox = (size_t)G.n3 * pstride;
+    const double *vp = v4 + (size_t)s * pstride + (size_t)y * G.n1 + (xok ? x : 0);
+    const double *vown = vp + (size_t)comp * nbox, *vre = vp + 2 * nbox, *vim = vp + 3 * nbox;
+    const double sgn = comp ? -1.0 : 1.0;       // the down row of the matrix holds conj(V_updn)
+#pragma unroll
+    for (int k2 = 0; k2 < R2; k2++) {
+      const size_t o = (size_t)(R1 * k2) * pstride;
+      const double a = xok ? __ldg(vown + o) : 0.0, cr = xok ? __ldg(vre + o) : 0.0, ci = xok ? sgn * __ldg(vim + o) : 0.0;
+      const double ox = __shfl_xor_sync(half, v[k2].x, 8), oy = __shfl_xor_sync(half, v[k2].y, 8);
+      v[k2] = make_double2(a * v[k2].x + (cr * ox - ci * oy), a * v[k2].y + (cr * oy + ci * ox));
+    }
+    Dft<R2, -1>::run(v);
+#pragma unroll
+    for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw3, s * cc));
+#pragma unroll
+    for (int cc = 0; cc < R2; cc++) sm[cc * KSb + s * XT + px] = v[cc];
+  }
+  __syncthreads();
+  if (s < R2) {
+#pragma unroll
+    for (int a = 0; a < R1; a++) v[a] = sm[s * KSb + a * XT + px];
+    Dft<R1, -1>::run(v);
+#pragma unroll
+    for (int d = 0; d < R1; d++) {
+      int p = xok ? run_map(G.zrun, s + R2 * d) : -1;
+      if (p >= 0) base[(size_t)p * pstride] = v[d];
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // TMA-ring variants of the three strided passes (B, C, B^-1).  Same arithmetic, same register
 // layout; what changes is how a tile's INPUT reaches the registers.  Above, every thread issues its own
@@ -839,6 +914,17 @@ static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi
                        int nb, int hb, cudaStream_t st, const FftExtra &X) {
   constexpr int NS = imax(R1, R2);
   int rc;
+  if (pass == 2 && X.vspin) {       // two-component spinors: rows in (up, down) pairs, 2 x 2 potential
+    if (nb & 1) { set_error("the spinor local term needs an even number of rows per launch (got %d)", nb); return DFT_ERR_INVALID_ARG; }
+    const int nxt = (G.n1 + 7) / 8;
+    size_t sm = sizeof(cplx) * (size_t)(pad8(R2 * 16, 16) * R1 > pad8(R1 * 16, 16) * R2 ? pad8(R2 * 16, 16) * R1 : pad8(R1 * 16, 16) * R2);
+    int64_t grid = (int64_t)(nb / 2) * nxt * G.n2;
+    if (grid > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
+    if ((rc = set_smem(fft2_c_spinor_kernel<R1, R2>, sm))) return rc;
+    fft2_c_spinor_kernel<R1, R2><<<(unsigned)grid, 16 * NS, sm, st>>>(G, T2, X.vspin, nxt, nb / 2);
+    DFT_CUDA_CHECK(cudaGetLastError());
+    return DFT_OK;
+  }
   if (pass >= 1 && pass <= 3 && (p->fft_path == 0 || p->fft_path == 4)) {
     rc = launch_ring<R1, R2>(p, G, pass, T1, T2, vloc, nb, hb, st);
     if (rc != DFT_ERR_UNSUPPORTED) return rc;

@@ -193,7 +193,8 @@ struct dft_plan {
   int sym_state = 0;                   // 0 = not tried, 1 = tables ready, -1 = this plan cannot (k != 0, several k-points, unpaired Nyquist index)
   double *d_symx = nullptr; int64_t symx_bytes = 0;   // time-reversal-even/odd halves of the bands, [2 nband][nhalf] complex
   // two-component spinors (spinor.cu): Pauli components of the local potential, spin-dependent D
-  double *d_vpauli = nullptr;          // [4][n3][n2][n1]: V0, Vx, Vy, Vz, each pre-scaled by 1/N
+  double *d_vpauli = nullptr;          // [8][n3][n2][n1]: V0, Vx, Vy, Vz, then V_upup, V_dndn, Re V_updn, Im V_updn, each pre-scaled by 1/N
+  int spinor_fused = 1;                // 1: one local application with the 2 x 2 matrix in pass C where the register path serves the box
   double *d_dspin = nullptr;           // [natom][2][2][lmax][lmax] complex
   double *d_spin_tmp = nullptr; int64_t spin_tmp_bytes = 0;   // sigma_mu psi, [nband][2][mpw] complex
   bool vspin_set = false, dspin_set = false, gam_attr_done = false;
@@ -220,6 +221,8 @@ struct FftExtra {
   const double *pre = nullptr;    // device [npw]; null = 1
   const double *post = nullptr;   // device [npw]; null = 1
   int accumulate = 0;             // 1: hpsi += result (pad entries untouched) instead of hpsi = result
+  const double *vspin = nullptr;  // device [4][n3][n2][n1] = (V_upup, V_dndn, Re V_updn, Im V_updn) / N: the rows are (up, down)
+                                  // pairs of two-component spinors and pass C applies the 2 x 2 matrix (register path only)
 };
 // --- fft.cu (K2) --------------------------------------------------------------------------
 int64_t fft_ws_bytes_per_band(const dft_plan *p);

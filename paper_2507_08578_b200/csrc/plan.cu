@@ -312,6 +312,10 @@ int local_term(dft_plan *p, const double *psi, double *hpsi, int nband, cudaStre
     return DFT_OK;
   }
   if ((rc = ensure_workspace(p, fft_ws_bytes_per_band(p), nband, &chunk, &ws, st))) return rc;
+  if (extra && extra->vspin) {      // rows are (up, down) pairs: a chunk holds whole spinor bands
+    chunk &= ~1;
+    if (chunk < 2) { set_error("the workspace holds fewer than the two rows of one spinor band"); return DFT_ERR_ALLOC; }
+  }
   for (int ik = 0; ik < p->nkpt; ik++)
     for (int b0 = 0; b0 < nband; b0 += chunk) {
       int nb = nband - b0 < chunk ? nband - b0 : chunk;
@@ -586,6 +590,10 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     if (value < 0 || value > 5) { set_error("fft_path = %lld outside 0..5", (long long)value); return DFT_ERR_INVALID_ARG; }
     if ((value == 3 || value == 5) && !fft_small_ok(p)) { set_error("fft_path = 3: the fused small-box kernel cannot serve this plan (box lengths or shared memory)"); return DFT_ERR_UNSUPPORTED; }
     p->fft_path = (int)value; return DFT_OK;
+  }
+  if (!strcmp(key, "spinor_fused")) {
+    if (value < 0 || value > 1) { set_error("spinor_fused = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->spinor_fused = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "proj_mode")) {
     if (value < 0 || value > 1) { set_error("proj_mode = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }

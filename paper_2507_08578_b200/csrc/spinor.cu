@@ -10,18 +10,24 @@
 // V0 = (V_upup + V_dndn)/2, Vz = (V_upup - V_dndn)/2, Vx = Re V_updn, Vy = -Im V_updn), and every V_mu is a REAL field, so
 //   V psi = Loc_V0(psi) + sum_mu Loc_Vmu(sigma_mu psi):
 // four applications of the scalar local term (pruned FFT passes of fft2.cu / fft_small.cu, unchanged), the last three
-// on sigma_mu psi (one elementwise kernel each) accumulating onto the first.  Nothing here is shared with the CPU checker.
+// on sigma_mu psi (one elementwise kernel each) accumulating onto the first.  That form serves every box.  Where all three
+// box lengths have a two-radix factorisation and the box is too large for the fused small-box kernel (the five-pass
+// register path of fft2.cu), ONE local application does it all: the rows (band, s) go through passes A and B like 2 nband
+// scalar bands, pass C multiplies the 2 x 2 matrix in real space (fft2_c_spinor_kernel: the two components of a point
+// sit in partner lanes of a warp), and passes B^-1, A^-1 bring both components back -- a quarter of the transforms
+// (option spinor_fused, default 1).  Nothing here is shared with the CPU checker.
 #include "internal.h"
 
 namespace dftb200 {
 
 namespace {
 
-// out[0..3][j] = (V0, Vx, Vy, Vz)(r_j) / N from v4 = (V_upup, V_dndn, Re V_updn, Im V_updn)
+// out[0..3][j] = (V0, Vx, Vy, Vz)(r_j) / N and out[4..7][j] = v4 / N from v4 = (V_upup, V_dndn, Re V_updn, Im V_updn)
 __global__ void pauli_split_kernel(const double *__restrict__ v4, double *__restrict__ out, int64_t n, double s) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     const double uu = v4[i], dd = v4[n + i], re = v4[2 * n + i], im = v4[3 * n + i];
     out[i] = 0.5 * (uu + dd) * s; out[n + i] = re * s; out[2 * n + i] = -im * s; out[3 * n + i] = 0.5 * (uu - dd) * s;
+    out[4 * n + i] = uu * s; out[5 * n + i] = dd * s; out[6 * n + i] = re * s; out[7 * n + i] = im * s;   // the matrix itself / N
   }
 }
 
@@ -42,7 +48,7 @@ __global__ void pauli_apply_kernel(const double2 *__restrict__ psi, double2 *__r
 
 int spinor_set_vloc(dft_plan *p, const double *v4, cudaStream_t st) {
   const int64_t n = p->nbox;
-  if (!p->d_vpauli && cudaMalloc(&p->d_vpauli, sizeof(double) * 4 * n) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the spinor potential"); return DFT_ERR_ALLOC; }
+  if (!p->d_vpauli && cudaMalloc(&p->d_vpauli, sizeof(double) * 8 * n) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the spinor potential"); return DFT_ERR_ALLOC; }
   const int grid = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
   pauli_split_kernel<<<grid, 256, 0, st>>>(v4, p->d_vpauli, n, 1.0 / (double)n);
   DFT_CUDA_CHECK(cudaGetLastError());
@@ -60,7 +66,15 @@ int spinor_apply(dft_plan *p, const double *psi, double *hpsi, int nband, cudaSt
   int rc;
   const int rows = 2 * nband;
   const int64_t n = p->nbox;
-  if (loc) {
+  // one application with the 2 x 2 matrix in pass C where the five-pass register path serves the box
+  bool fused = p->spinor_fused && p->fft_path != 1 && !((p->fft_path == 0 || p->fft_path == 3 || p->fft_path == 5) && fft_small_ok(p));
+  for (int c = 0; c < 3 && fused; c++) fused = fft2_pair(p->n[c], nullptr, nullptr);
+  for (int ik = 0; ik < p->nkpt && fused; ik++) fused = p->kp[ik].runs_ok;
+  if (loc && fused) {
+    FftExtra X;
+    X.vspin = p->d_vpauli + 4 * n;
+    if ((rc = local_term(p, psi, hpsi, rows, st, &X))) return rc;
+  } else if (loc) {
     const int64_t need = (int64_t)p->nkpt * rows * p->mpw * 16;
     if (need > p->spin_tmp_bytes) {
       if (p->d_spin_tmp) { DFT_CUDA_CHECK(cudaStreamSynchronize(st)); cudaFree(p->d_spin_tmp); p->d_spin_tmp = nullptr; p->spin_tmp_bytes = 0; }

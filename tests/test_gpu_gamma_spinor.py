@@ -244,6 +244,41 @@ def test_spinor_all_terms_and_paths(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name,over", [("c1m", {}), ("aniso", {}), ("c3k2", {}), ("c0", {"ngfft": (20, 20, 180)}), ("c0", {"ngfft": (16, 20, 24)})],
+                         ids=lambda v: v if isinstance(v, str) else "x".join(map(str, v.get("ngfft", ()))))
+def test_spinor_local_term_fused_in_pass_c(name, over):
+    """Five-pass register path: ONE local application with the 2 x 2 potential multiplied in pass C (the two components of a
+    point in partner lanes of a warp; option spinor_fused = 1, default) against the four scalar applications of the Pauli
+    decomposition (spinor_fused = 0) and the oracle; band chunks are rounded to whole spinor bands; a quarter of the
+    launches."""
+    cfg = synth.make_config(name, **over)
+    plan = make_plan(cfg)
+    sph = lib_spheres(plan)
+    v4, dspin = synth.spinor_inputs(cfg)
+    plan.set_vloc_spinor(torch.as_tensor(v4, device="cuda"))
+    plan.set_dij_spinor(dspin)
+    nb, mpw = 5, plan.mpw
+    psi = synth.gen_psi(cfg, [s[2] for s in sph], nband=2 * nb).reshape(plan.nkpt, nb, 2, mpw)
+    m = 1 if name in ("c0", "aniso") else 2
+    plan.set_option("fft_path", 4)
+    for terms in (2, 7):
+        plan.set_option("terms", terms)
+        ref = np.stack([oracle.apply_h_spinor(cfg, ik, *sph[ik], psi[ik], v4, dspin, method=m, terms=terms)
+                        for ik in range(plan.nkpt)])
+        for fused in (1, 0):
+            plan.set_option("spinor_fused", fused)
+            for chunk in (0, 2, 3, 7):
+                plan.set_option("band_chunk", chunk)
+                got = _spinor_gpu(plan, psi)
+                err = band_rel_err(got, ref)
+                assert err <= TOL, "%s terms=%d fused=%d chunk=%d: rel err %.3e" % (name, terms, fused, chunk, err)
+                for ik in range(plan.nkpt):
+                    assert np.all(got[ik][:, :, plan.npw[ik]:] == 0)
+                if terms == 2 and chunk == 0:
+                    assert plan.last_launches() == (5 * plan.nkpt if fused else 20 * plan.nkpt + 3)
+    plan.destroy()
+
+
 def test_spinor_with_vector_potential():
     """Velocity gauge (PAPER.md :340): the kinetic diagonal 1/2 |k+G+A|^2 acts on both components."""
     cfg = synth.make_config("c0")

@@ -317,70 +317,87 @@ fft2_c_kernel(Fft2Geom G0, Fft2Batch B, cplx *__restrict__ T2, const double *__r
 //      the same points, so after the forward transform the partner value sits in lane ^ 8 of the same warp and one
 //      shuffle per number replaces any second pass over the data: one local application for the whole 2 x 2 matrix
 //      instead of the four of the Pauli decomposition (spinor.cu).  Same exchanges and twiddles as fft2_c_kernel.
+//      The CTAs are persistent: each walks a contiguous range of (tile, spinor band) pairs with the band fastest and keeps
+//      the four fields of its tile, [4][n3][8] doubles, and the twiddles in shared memory (with the fields read straight
+//      from L2 in the multiply loop, 45 dependent-latency loads per thread, the pass took 109 ms per 1024 rows at c4).
 template <int R1, int R2>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-fft2_c_spinor_kernel(Fft2Geom G, cplx *__restrict__ T2, const double *__restrict__ v4, int nxt, int nsb) {
+fft2_c_spinor_kernel(Fft2Geom G, cplx *__restrict__ T2, const double *__restrict__ v4, int nxt, int nsb, int ntiles) {
   constexpr int NS = imax(R1, R2), XT = 16;
   extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT), exn = imax(R1 * KSa, R2 * KSb);
   cplx *sm = reinterpret_cast<cplx *>(smem_raw);
-  const int t = threadIdx.x, px = t % XT, s = t / XT, comp = px >> 3;
-  const int sb = blockIdx.x % nsb, tile = blockIdx.x / nsb, xt = tile % nxt, y = tile / nxt;
-  const int x = xt * 8 + (px & 7);
-  const bool xok = x < G.n1;
-  constexpr int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
-  const size_t pstride = (size_t)G.n2 * G.n1;
-  cplx *base = T2 + (size_t)(2 * sb + comp) * G.t2_band + (size_t)y * G.n1 + (xok ? x : 0);
-  cplx v[NS];
-  if (s < R2) {
-#pragma unroll
-    for (int j1 = 0; j1 < R1; j1++) {
-      int p = xok ? run_map(G.zrun, s + R2 * j1) : -1;
-      v[j1] = p >= 0 ? base[(size_t)p * pstride] : make_double2(0.0, 0.0);
+  cplx *tws = sm + exn;                                       // exp(+2 pi i j / n3), j < n3
+  double *vs = reinterpret_cast<double *>(tws + G.n3);        // [4][n3][8]
+  const int t = threadIdx.x, px = t % XT, s = t / XT, comp = px >> 3, xq = px & 7;
+  for (int i = t; i < G.n3; i += blockDim.x) tws[i] = __ldg(G.tw3 + i);
+  const int first = (int)(((int64_t)ntiles * blockIdx.x) / gridDim.x);
+  const int nmine = (int)(((int64_t)ntiles * (blockIdx.x + 1)) / gridDim.x) - first;
+  const size_t pstride = (size_t)G.n2 * G.n1, nbox = (size_t)G.n3 * pstride;
+  int sb = first % nsb, g = first / nsb;
+  bool newgroup = true;
+  const unsigned half = 0xffffu << (t & 16);      // the 16 lanes that share this thread's s
+  const double sgn = comp ? -1.0 : 1.0;           // the down row of the matrix holds conj(V_updn)
+  const double *vown = vs + (size_t)comp * G.n3 * 8 + xq, *vre = vs + (size_t)2 * G.n3 * 8 + xq, *vim = vs + (size_t)3 * G.n3 * 8 + xq;
+  for (int it = 0; it < nmine; it++) {
+    const int xt = g % nxt, y = g / nxt, x = xt * 8 + xq;
+    const bool xok = x < G.n1;
+    if (newgroup) {
+      __syncthreads();       // every read of the previous tile's fields (and the twiddle fill, the first time) is done
+      const double *vp = v4 + (size_t)y * G.n1 + xt * 8;
+      for (int i = t; i < 4 * G.n3 * 8; i += blockDim.x) {
+        const int f = i / (G.n3 * 8), r = i - f * (G.n3 * 8), z = r >> 3, xx = r & 7;
+        vs[i] = (xt * 8 + xx < G.n1) ? __ldg(vp + (size_t)f * nbox + (size_t)z * pstride + xx) : 0.0;
+      }
+      newgroup = false;      // the barrier after the first exchange orders these writes before the reads of stage 2
     }
-    Dft<R1, +1>::run(v);
+    cplx *base = T2 + (size_t)(2 * sb + comp) * G.t2_band + (size_t)y * G.n1 + (xok ? x : 0);
+    cplx v[NS];
+    if (s < R2) {
 #pragma unroll
-    for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], ldtw(G.tw3, s * k1));
+      for (int j1 = 0; j1 < R1; j1++) {
+        int p = xok ? run_map(G.zrun, s + R2 * j1) : -1;
+        v[j1] = p >= 0 ? base[(size_t)p * pstride] : make_double2(0.0, 0.0);
+      }
+      Dft<R1, +1>::run(v);
 #pragma unroll
-    for (int k1 = 0; k1 < R1; k1++) sm[k1 * KSa + s * XT + px] = v[k1];
-  }
-  __syncthreads();
-  if (s < R1) {
+      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], tws[s * k1]);
 #pragma unroll
-    for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KSa + j2 * XT + px];
-  }
-  __syncthreads();   // every read of the forward exchange is done before the buffer is reused
-  if (s < R1) {
-    Dft<R2, +1>::run(v);
-    // thread s now holds psi_comp(r) at z = s + R1 k2; its partner lane (^ 8) holds the other component at the same points.
-    // The 16 lanes of a half-warp share s, so the branch is uniform per half-warp and the shuffle names that half only.
-    const unsigned half = 0xffffu << (t & 16);
-    const size_t nbox = (size_t)G.n3 * pstride;
-    const double *vp = v4 + (size_t)s * pstride + (size_t)y * G.n1 + (xok ? x : 0);
-    const double *vown = vp + (size_t)comp * nbox, *vre = vp + 2 * nbox, *vim = vp + 3 * nbox;
-    const double sgn = comp ? -1.0 : 1.0;       // the down row of the matrix holds conj(V_updn)
-#pragma unroll
-    for (int k2 = 0; k2 < R2; k2++) {
-      const size_t o = (size_t)(R1 * k2) * pstride;
-      const double a = xok ? __ldg(vown + o) : 0.0, cr = xok ? __ldg(vre + o) : 0.0, ci = xok ? sgn * __ldg(vim + o) : 0.0;
-      const double ox = __shfl_xor_sync(half, v[k2].x, 8), oy = __shfl_xor_sync(half, v[k2].y, 8);
-      v[k2] = make_double2(a * v[k2].x + (cr * ox - ci * oy), a * v[k2].y + (cr * oy + ci * ox));
+      for (int k1 = 0; k1 < R1; k1++) sm[k1 * KSa + s * XT + px] = v[k1];
     }
-    Dft<R2, -1>::run(v);
+    __syncthreads();
+    if (s < R1) {
+      // in-place second exchange as in fft2_c_ring_kernel: this thread overwrites exactly the slots it read
 #pragma unroll
-    for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], ldtw(G.tw3, s * cc));
+      for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KSa + j2 * XT + px];
+      Dft<R2, +1>::run(v);
+      // thread s now holds psi_comp(r) at z = s + R1 k2; its partner lane (^ 8) holds the other component at the same points.
+      // The 16 lanes of a half-warp share s, so the branch is uniform per half-warp and the shuffle names that half only.
 #pragma unroll
-    for (int cc = 0; cc < R2; cc++) sm[cc * KSb + s * XT + px] = v[cc];
-  }
-  __syncthreads();
-  if (s < R2) {
+      for (int k2 = 0; k2 < R2; k2++) {
+        const int o = (s + R1 * k2) * 8;
+        const double a = vown[o], cr = vre[o], ci = sgn * vim[o];
+        const double ox = __shfl_xor_sync(half, v[k2].x, 8), oy = __shfl_xor_sync(half, v[k2].y, 8);
+        v[k2] = make_double2(a * v[k2].x + (cr * ox - ci * oy), a * v[k2].y + (cr * oy + ci * ox));
+      }
+      Dft<R2, -1>::run(v);
 #pragma unroll
-    for (int a = 0; a < R1; a++) v[a] = sm[s * KSb + a * XT + px];
-    Dft<R1, -1>::run(v);
+      for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], tws[s * cc]);
 #pragma unroll
-    for (int d = 0; d < R1; d++) {
-      int p = xok ? run_map(G.zrun, s + R2 * d) : -1;
-      if (p >= 0) base[(size_t)p * pstride] = v[d];
+      for (int cc = 0; cc < R2; cc++) sm[s * KSa + cc * XT + px] = v[cc];
     }
+    __syncthreads();
+    if (s < R2) {
+#pragma unroll
+      for (int a = 0; a < R1; a++) v[a] = sm[a * KSa + s * XT + px];
+      Dft<R1, -1>::run(v);
+#pragma unroll
+      for (int d = 0; d < R1; d++) {
+        int p = xok ? run_map(G.zrun, s + R2 * d) : -1;
+        if (p >= 0) base[(size_t)p * pstride] = v[d];
+      }
+    }
+    if (++sb == nsb) { sb = 0; newgroup = true; g++; }
   }
 }
 
@@ -917,11 +934,14 @@ static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi
   if (pass == 2 && X.vspin) {       // two-component spinors: rows in (up, down) pairs, 2 x 2 potential
     if (nb & 1) { set_error("the spinor local term needs an even number of rows per launch (got %d)", nb); return DFT_ERR_INVALID_ARG; }
     const int nxt = (G.n1 + 7) / 8;
-    size_t sm = sizeof(cplx) * (size_t)(pad8(R2 * 16, 16) * R1 > pad8(R1 * 16, 16) * R2 ? pad8(R2 * 16, 16) * R1 : pad8(R1 * 16, 16) * R2);
-    int64_t grid = (int64_t)(nb / 2) * nxt * G.n2;
-    if (grid > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
+    const size_t sm = sizeof(cplx) * (size_t)(imax(pad8(R2 * 16, 16) * R1, pad8(R1 * 16, 16) * R2) + G.n3) + sizeof(double) * 4 * (size_t)G.n3 * 8;
+    const int64_t ntiles = (int64_t)(nb / 2) * nxt * G.n2;
+    if (ntiles > 0x7fffffffLL) { set_error("FFT grid too large"); return DFT_ERR_UNSUPPORTED; }
+    if (sm > (size_t)p->smem_optin) { set_error("the spinor pass needs %zu bytes of shared memory", sm); return DFT_ERR_UNSUPPORTED; }
+    int grid = 2 * p->sm_count;
+    if (grid > ntiles) grid = (int)ntiles;
     if ((rc = set_smem(fft2_c_spinor_kernel<R1, R2>, sm))) return rc;
-    fft2_c_spinor_kernel<R1, R2><<<(unsigned)grid, 16 * NS, sm, st>>>(G, T2, X.vspin, nxt, nb / 2);
+    fft2_c_spinor_kernel<R1, R2><<<grid, 16 * NS, sm, st>>>(G, T2, X.vspin, nxt, nb / 2, (int)ntiles);
     DFT_CUDA_CHECK(cudaGetLastError());
     return DFT_OK;
   }

@@ -149,7 +149,9 @@ int dft_plan_workspace_bytes(const dft_plan *p, int32_t nband, int64_t *min_byte
  * "gemm_strassen" (with gemm_sym active: one level of Strassen's recursion on the two real GEMMs, 7/8 of their flops, same
  * result up to rounding; 0 = never, 1 = wherever nproj is a multiple of 16, 2 = default: for nproj * npw * nband >= 1e10;
  * builds nine block tables of a quarter of the half table each at the first such call),
- * "gamma_real" (1 = enable dft_apply_h_gamma, see there).  Unknown key or bad value -> DFT_ERR_INVALID_ARG.  */
+ * "gamma_real" (1 = enable dft_apply_h_gamma, see there), "spinor_fused" (dft_apply_h_spinor: 1 = default, the 2 x 2 potential
+ * multiplied inside the middle FFT pass where the register path serves the box; 0 = four scalar local applications).
+ * Unknown key or bad value -> DFT_ERR_INVALID_ARG.  */
 int dft_plan_set_option(dft_plan *p, const char *key, int64_t value);
 
 /* hpsi = H psi for nband bands per k-point.  psi and hpsi are DEVICE memory, layout
@@ -243,11 +245,14 @@ int dft_chebyshev_filter_gamma(dft_plan *p, double *psi, double *work, int32_t n
  * SURVEY.md 8(f) row 4; reading 27).  psi = (psi_up, psi_dn): DEVICE [nkpt][nband][2][mpw] complex128.
  *   H = kin (x) 1 + FFT^-1[ V^{ss'}(r) FFT[psi_s'] ] + sum_a sum_ij sum_ss' |p_a,i> D^{a,ss'}_ij <p_a,j|
  * dft_set_vloc_spinor: v4 DEVICE [4][n3][n2][n1] doubles = V_upup, V_dndn, Re V_updn, Im V_updn (V_dnup = conj V_updn),
- * copied on `stream` (as Pauli components V0, Vx, Vy, Vz pre-scaled by 1/N).
+ * copied on `stream` (pre-scaled by 1/N, as the four fields and as their Pauli components V0, Vx, Vy, Vz).
  * dft_set_dij_spinor: dspin HOST [natom][2][2][lmax][lmax] complex128 (re, im interleaved), Hermitian in
  * ((s,i),(s',j)); NULL returns to the scalar D_ij of dft_set_dij on both components.  Synchronises the device.
  * dft_apply_h_spinor: rules of dft_apply_h; DFT_ERR_NOT_READY before dft_set_vloc_spinor while the local term is on.
- * The local term is four scalar local applications (V0 psi + sum_mu V_mu sigma_mu psi), the GEMMs see 2 nband bands. */
+ * The GEMMs see 2 nband bands.  The local term is one application with the 2 x 2 matrix multiplied in the middle FFT pass
+ * where the five-pass register path serves the box (option "spinor_fused", default 1), else four scalar local
+ * applications (V0 psi + sum_mu V_mu sigma_mu psi), which need box lengths with a two-radix factorisation or a box small
+ * enough for the fused small-box kernel (otherwise DFT_ERR_UNSUPPORTED). */
 int dft_set_vloc_spinor(dft_plan *p, const double *v4_dev, void *stream);
 int dft_set_dij_spinor(dft_plan *p, const double *dspin_host);
 int dft_apply_h_spinor(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);

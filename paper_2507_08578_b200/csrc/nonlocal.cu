@@ -1075,12 +1075,8 @@ static int nonlocal_apply_sym(dft_plan *p, const double *psi, double *hpsi, int 
     p->symx_bytes = need_x;
   }
   double2 *X = reinterpret_cast<double2 *>(p->d_symx);
-  if (strassen_wanted(p, nband)) {      // seven half-size products per GEMM instead of eight (nonlocal_strassen.inc)
-    phase_begin(p, 9, st);
-    sym_split_kernel<<<dim3((nh + 255) / 256, nband), 256, 0, st>>>(reinterpret_cast<const double2 *>(psi), X, G->d_h2f, G->d_h2fneg, mpw, nh);
-    phase_end(p, 9, st, 1);
+  if (strassen_wanted(p, nband))        // seven half-size products per GEMM instead of eight (nonlocal_strassen.inc)
     return nonlocal_apply_sym_strassen(p, psi, hpsi, nband, accumulate, with_kin, st, dmat, d_kin, cprj_out, rec, spsi, X, false);
-  }
   Gemm1Params q1;
   q1.nproj = nproj; q1.nband = n2; q1.nslab = (nh + 7) / 8;
   q1.tiles_m = (nproj + NL_BM - 1) / NL_BM; q1.tiles_n = (n2 + NL_BN - 1) / NL_BN;

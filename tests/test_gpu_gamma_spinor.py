@@ -279,6 +279,57 @@ def test_spinor_local_term_fused_in_pass_c(name, over):
     plan.destroy()
 
 
+def test_spinor_c4_full_size_local_term_sample():
+    """Full-size c4 box (180^3, radix pair 12 x 15, 295 667 plane waves): 160 spinor bands = 320 rows through the fused
+    2 x 2 pass C in band chunks of whole spinor bands; the oracle checks the local term of a sample that sits on both sides
+    of every chunk boundary (the non-local part of this cell is covered row by row by the scalar full-size test: the GEMMs
+    see the same rows)."""
+    cfg = synth.make_config("c4")
+    plan = make_plan(cfg)
+    (kg, ig, kin), = lib_spheres(plan)
+    v4, dspin = synth.spinor_inputs(cfg)
+    plan.set_vloc_spinor(torch.as_tensor(v4, device="cuda"))
+    nsb = 160
+    psi = synth.gen_psi_torch(cfg, [kin], "cuda", nband=2 * nsb)[0].reshape(1, nsb, 2, plan.mpw)
+    plan.set_option("terms", 2)
+    out = plan.apply_h_spinor(psi)
+    torch.cuda.synchronize()
+    assert plan.last_launches() % 5 == 0 and plan.last_launches() >= 10        # five passes per chunk, several chunks
+    chunk = 2 * nsb // (plan.last_launches() // 5)                              # rows per chunk, roughly
+    sample = sorted({0, nsb - 1, chunk // 2 - 1, chunk // 2, chunk // 2 + 1, nsb // 2})
+    ref = oracle.apply_h_spinor(cfg, 0, kg, ig, kin, psi[0, sample].cpu().numpy(), v4, dspin, method=2, terms=2)
+    err = band_rel_err(out[:, sample].cpu().numpy(), ref[None])
+    print("c4 spinors, local term: %d of %d spinor bands oracle-checked: rel err %.2e" % (len(sample), nsb, err))
+    assert err <= TOL, err
+    plan.destroy()
+    del psi, out
+    torch.cuda.empty_cache()
+
+
+def test_spinor_c2_full_size_sample():
+    """Full-size c2 (128^3, radix pair 8 x 16, 1728 projectors): all 216 spinor bands on the GPU, every term with the spin-
+    dependent D; the oracle checks first, last and two seeded interior spinor bands."""
+    cfg = synth.make_config("c2")
+    plan = make_plan(cfg)
+    (kg, ig, kin), = lib_spheres(plan)
+    v4, dspin = synth.spinor_inputs(cfg)
+    plan.set_vloc_spinor(torch.as_tensor(v4, device="cuda"))
+    plan.set_dij_spinor(dspin)
+    nsb = cfg["nband"] // 2
+    psi = synth.gen_psi_torch(cfg, [kin], "cuda")[0][:2 * nsb].reshape(1, nsb, 2, plan.mpw)
+    out = plan.apply_h_spinor(psi)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(5)
+    sample = sorted({0, nsb - 1} | {int(v) for v in rng.choice(np.arange(1, nsb - 1), size=2, replace=False)})
+    ref = oracle.apply_h_spinor(cfg, 0, kg, ig, kin, psi[0, sample].cpu().numpy(), v4, dspin, method=2)
+    err = band_rel_err(out[:, sample].cpu().numpy(), ref[None])
+    print("c2 spinors, all terms: %d of %d spinor bands oracle-checked: rel err %.2e" % (len(sample), nsb, err))
+    assert err <= TOL, err
+    plan.destroy()
+    del psi, out
+    torch.cuda.empty_cache()
+
+
 def test_spinor_with_vector_potential():
     """Velocity gauge (PAPER.md :340): the kinetic diagonal 1/2 |k+G+A|^2 acts on both components."""
     cfg = synth.make_config("c0")

@@ -148,8 +148,7 @@ int dft_plan_workspace_bytes(const dft_plan *p, int32_t nband, int64_t *min_byte
  * 2 = default: when nproj * npw * nband >= 1e8; the first such call builds a second table of half the size),
  * "gemm_strassen" (with gemm_sym active: one level of Strassen's recursion on the two real GEMMs, 7/8 of their flops, same
  * result up to rounding; 0 = never, 1 = wherever nproj is a multiple of 16, 2 = default: for nproj * npw * nband >= 1e10;
- * builds nine block tables of a quarter of the half table each at the first such call; "gemm2_persistent": 1 = default, the
- * back-projection products of that path run one persistent CTA per SM, 0 = one tile per CTA),
+ * builds nine block tables of a quarter of the half table each at the first such call),
  * "gamma_real" (1 = enable dft_apply_h_gamma, see there), "spinor_fused" (dft_apply_h_spinor: 1 = default, the 2 x 2 potential
  * multiplied inside the middle FFT pass where the register path serves the box; 0 = four scalar local applications).
  * Unknown key or bad value -> DFT_ERR_INVALID_ARG.  */

@@ -68,7 +68,6 @@ struct Gemm2Params {
   double sh, sy, sx;
   const double2 *xprev;                // [nkpt][nband][mpw], read only where sx != 0
   int raw;                             // gemm2_kernel<true> only: 1 = an intermediate product (Strassen block): keep Im of row 0
-  int ntiles = 0;                      // gemm2_kernel: tiles_n * tiles_m when the grid is smaller than that (persistent CTAs), 0 = one tile per CTA
 };
 
 // The MMA main loop shared by both GEMMs.  MODE 1: acc += conj(A) B (GEMM-1); MODE 2: acc += A B.
@@ -345,78 +344,66 @@ __global__ void __launch_bounds__(NL_THREADS_P, 1)
 gemm2_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapC, Gemm2Params Q) {
   extern __shared__ unsigned char smem_raw[];
   Pipe P = pipe_setup(smem_raw);
-  const int ik = blockIdx.z;
+  const int tn = blockIdx.x % Q.tiles_n, tm = blockIdx.x / Q.tiles_n, ik = blockIdx.z;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int ns = Q.with_nl ? Q.nslab : 0;
-  // Q.ntiles > 0: persistent CTAs, tile t of the (band tile fastest) order goes to CTA t mod gridDim.x, so the CTAs that
-  // run together still share a slab of P in L2 and the producer fills the ring with the next tile's slabs while the
-  // consumers are in the epilogue of this one (one tile per CTA leaves the DMMA pipe idle during prologue and epilogue)
-  const int ntiles = Q.ntiles > 0 ? Q.ntiles : (int)gridDim.x;
+  auto issue = [&](int j) {
+    int s = j % NL_STAGES;
+    if (j >= NL_STAGES) mbar_wait(&P.empty[s], ((j / NL_STAGES) - 1) & 1);
+    unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mbar_expect_tx(&P.full[s], NL_STAGE_BYTES);
+    // one box {16 doubles, 8 projector rows, 16 g-blocks}: lands as [g-block][p][8 complex], 128-byte swizzled
+    tma_load_4d(st, &mapP, &P.full[s], 0, j * 8, tm * (NL_BM / 8), ik);
+    tma_load_3d(st + NL_STAGE_A, &mapC, &P.full[s], j * 16, tn * NL_BN, ik);
+  };
   if (warp >= NL_CONSUMERS) {      // the producer group
     reg_dealloc_producer();
-    if (warp == NL_CONSUMERS && lane == 0) {
-      int jg = 0;                  // slabs issued so far by this CTA (ring position)
-      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int tn = tile % Q.tiles_n, tm = tile / Q.tiles_n;
-        for (int j = 0; j < ns; j++, jg++) {
-          const int s = jg % NL_STAGES;
-          if (jg >= NL_STAGES) mbar_wait(&P.empty[s], ((jg / NL_STAGES) - 1) & 1);
-          unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
-          mbar_expect_tx(&P.full[s], NL_STAGE_BYTES);
-          // one box {16 doubles, 8 projector rows, 16 g-blocks}: lands as [g-block][p][8 complex], 128-byte swizzled
-          tma_load_4d(st, &mapP, &P.full[s], 0, j * 8, tm * (NL_BM / 8), ik);
-          tma_load_3d(st + NL_STAGE_A, &mapC, &P.full[s], j * 16, tn * NL_BN, ik);
-        }
-      }
-    }
+    if (warp == NL_CONSUMERS && lane == 0)
+      for (int j = 0; j < ns; j++) issue(j);
     return;
   }
   reg_alloc_consumer();
   const int wm = warp >> 1, wn = warp & 1;
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
+  for (int it = 0; it < ns; it++) {
+    int s = it % NL_STAGES;
+    mbar_wait(&P.full[s], (it / NL_STAGES) & 1);
+    const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
+    mma_stage<2, REAL>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&P.empty[s]);
+  }
+  // epilogue: hpsi[b][g] = (V_loc psi)[b][g] + kin[g] psi[b][g] + acc;  rows g = lane/4, bands 2*(lane%4)+{0,1}
   const int npw = Q.npw[ik];
   const double *kin = Q.kin[ik];
   const double2 *psi = Q.psi + (size_t)ik * Q.nband * Q.mpw;
   double2 *hpsi = Q.hpsi + (size_t)ik * Q.nband * Q.mpw;
   const int i = lane >> 2, j = lane & 3;
-  int itg = 0;                     // slabs consumed so far by this CTA
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const int tn = tile % Q.tiles_n, tm = tile / Q.tiles_n;
-    double cre[4][4][2], cim[4][4][2];
 #pragma unroll
-    for (int a = 0; a < 4; a++)
+  for (int mb = 0; mb < 4; mb++) {
+    int g = tm * NL_BM + wm * 32 + mb * 8 + i;
+    if (g >= npw) continue;
+    double kg = Q.with_kin ? kin[g] : 0.0;
 #pragma unroll
-      for (int b = 0; b < 4; b++) { cre[a][b][0] = cre[a][b][1] = cim[a][b][0] = cim[a][b][1] = 0.0; }
-    for (int it = 0; it < ns; it++, itg++) {
-      int s = itg % NL_STAGES;
-      mbar_wait(&P.full[s], (itg / NL_STAGES) & 1);
-      const unsigned char *st = P.tiles + s * NL_STAGE_BYTES;
-      mma_stage<2, REAL>(st, st + NL_STAGE_A, wm, wn, lane, cre, cim);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&P.empty[s]);
-    }
-    // epilogue: hpsi[b][g] = (V_loc psi)[b][g] + kin[g] psi[b][g] + acc;  rows g = lane/4, bands 2*(lane%4)+{0,1}
+    for (int nb = 0; nb < 4; nb++) {
 #pragma unroll
-    for (int mb = 0; mb < 4; mb++) {
-      int g = tm * NL_BM + wm * 32 + mb * 8 + i;
-      if (g >= npw) continue;
-      double kg = Q.with_kin ? kin[g] : 0.0;
-#pragma unroll
-      for (int nb = 0; nb < 4; nb++) {
-#pragma unroll
-        for (int e = 0; e < 2; e++) {
-          int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j + e;
-          if (b >= Q.nband) continue;
-          size_t off = (size_t)b * Q.mpw + g;
-          double2 r = make_double2(cre[mb][nb][e], cim[mb][nb][e]);
-          if (Q.with_kin) { double2 x = psi[off]; r.x += kg * x.x; r.y += kg * x.y; }
-          if (Q.accumulate) { double2 h = hpsi[off]; r.x += h.x; r.y += h.y; }
-          if (Q.cheb) {
-            double2 y = psi[off], xp = Q.sx != 0.0 ? Q.xprev[(size_t)ik * Q.nband * Q.mpw + off] : make_double2(0.0, 0.0);
-            r.x = Q.sh * r.x + Q.sy * y.x + Q.sx * xp.x; r.y = Q.sh * r.y + Q.sy * y.y + Q.sx * xp.y;
-          }
-          if (REAL && g == 0 && !Q.raw) r.y = 0.0;     // Gamma storage: c(G = 0) is real (reading 26)
-          hpsi[off] = r;
+      for (int e = 0; e < 2; e++) {
+        int b = tn * NL_BN + wn * 32 + nb * 8 + 2 * j + e;
+        if (b >= Q.nband) continue;
+        size_t off = (size_t)b * Q.mpw + g;
+        double2 r = make_double2(cre[mb][nb][e], cim[mb][nb][e]);
+        if (Q.with_kin) { double2 x = psi[off]; r.x += kg * x.x; r.y += kg * x.y; }
+        if (Q.accumulate) { double2 h = hpsi[off]; r.x += h.x; r.y += h.y; }
+        if (Q.cheb) {
+          double2 y = psi[off], xp = Q.sx != 0.0 ? Q.xprev[(size_t)ik * Q.nband * Q.mpw + off] : make_double2(0.0, 0.0);
+          r.x = Q.sh * r.x + Q.sy * y.x + Q.sx * xp.x; r.y = Q.sh * r.y + Q.sy * y.y + Q.sx * xp.y;
         }
+        if (REAL && g == 0 && !Q.raw) r.y = 0.0;     // Gamma storage: c(G = 0) is real (reading 26)
+        hpsi[off] = r;
       }
     }
   }

@@ -257,6 +257,20 @@ int dft_set_vloc_spinor(dft_plan *p, const double *v4_dev, void *stream);
 int dft_set_dij_spinor(dft_plan *p, const double *dspin_host);
 int dft_apply_h_spinor(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);
 
+/* The local term alone, hpsi = FFT^-1[ V_loc(r) FFT[psi] ] (PAPER.md :475; what dft_apply_h computes with option
+ * "terms" = 2), for callers that cannot allocate device memory: code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc.  Arguments, layouts, pad-entry rule and stream semantics of dft_apply_h.  The call
+ * performs no cudaMalloc / cudaFree and calls no allocating library routine, whatever the band count: the pass-to-pass
+ * scratch of the five FFT passes is a static device array of DFT_NOALLOC_SCRATCH_BYTES inside the library (every GPU that
+ * loads the library holds it until the process exits), and the bands go through in chunks that fit it (always the five-pass
+ * path, also for boxes where dft_apply_h would take the fused small-box kernel).  DFT_ERR_ALLOC if the scratch of ONE band,
+ * (ncol*n1 + nplane*n2*n1) * 16 bytes, exceeds the array (boxes above about 190^3; c4 at 180^3 needs 58.5 MB);
+ * DFT_ERR_NOT_READY before dft_set_vloc.  The array is shared by all plans and calls on a GPU and keeps the last call's
+ * contents (nothing in it needs to start at zero): calls that overlap on the GPU -- different streams without an event
+ * between them -- race on it and give wrong results; calls on one stream are safe.                                  */
+#define DFT_NOALLOC_SCRATCH_BYTES (64ll << 20)
+int dft_apply_vloc_noalloc(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);
+
 /* Same, with HOST psi/hpsi (pageable or pinned): copies psi to the device in band blocks, applies
  * H, copies the result back, and returns after the last copy has completed.                      */
 int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int32_t nband);

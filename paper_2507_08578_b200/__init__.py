@@ -23,6 +23,7 @@ DFT_OK = 0
 DFT_ERR_INVALID_ARG = -1
 DFT_ERR_GRID_TOO_SMALL = -2
 DFT_ERR_TABLE_RANGE = -3
+DFT_NOALLOC_SCRATCH_BYTES = 64 << 20     # include/dft.h: static scratch of dft_apply_vloc_noalloc
 DFT_ERR_ALLOC = -4
 DFT_ERR_CUDA = -5
 DFT_ERR_NOT_READY = -6
@@ -32,7 +33,7 @@ PHASES = ("fft_A_scatter", "fft_B", "fft_C_V_Cinv", "fft_Binv", "fft_Ainv_gather
           "fft_small_fused", "pack_unpack")
 
 # every symbol include/dft.h declares (checked by tests/test_abi.py against the header text)
-SYMBOLS = ("dft_plan_create", "dft_plan_create_opts", "dft_plan_get_info", "dft_plan_workspace_bytes", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
+SYMBOLS = ("dft_plan_create", "dft_plan_create_opts", "dft_apply_vloc_noalloc", "dft_plan_get_info", "dft_plan_workspace_bytes", "dft_plan_get_kg", "dft_plan_get_projectors", "dft_plan_copy_projectors_device", "dft_set_dij",
            "dft_set_sij", "dft_apply_s", "dft_apply_hs", "dft_get_cprj", "dft_chebyshev_filter",
            "dft_set_vector_potential", "dft_accumulate_density", "dft_accumulate_tau",
            "dft_set_vtau", "dft_plan_get_kg_gamma", "dft_apply_h_gamma", "dft_chebyshev_filter_gamma", "dft_set_vloc_spinor", "dft_set_dij_spinor",
@@ -85,6 +86,7 @@ def lib():
     L.dft_set_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
     L.dft_plan_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
     L.dft_apply_h.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    L.dft_apply_vloc_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
     L.dft_apply_h_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
     L.dft_set_sij.argtypes = [C.c_void_p, _dp]
     L.dft_set_vector_potential.argtypes = [C.c_void_p, _dp]
@@ -221,6 +223,10 @@ def dft_plan_set_option(plan, key, value):
 
 def dft_apply_h(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream=0):
     _check(lib().dft_apply_h(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream))
+
+
+def dft_apply_vloc_noalloc(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream=0):
+    _check(lib().dft_apply_vloc_noalloc(plan, psi_dev_ptr, hpsi_dev_ptr, nband, stream))
 
 
 def dft_set_sij(plan, sij):
@@ -374,6 +380,17 @@ class Plan:
             hpsi = torch.empty_like(psi)
         assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.is_contiguous() and hpsi.shape == psi.shape
         dft_apply_h(self.h, psi.data_ptr(), hpsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
+        return hpsi
+
+    def apply_vloc_noalloc(self, psi, hpsi):
+        """hpsi = V_loc psi through dft_apply_vloc_noalloc (static scratch inside the library, no allocation): both tensors
+        are the caller's, laid out as for apply_h."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous()
+        assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.is_contiguous() and hpsi.shape == psi.shape
+        assert psi.shape[-1] == self.mpw and (self.mpw == 0 or psi.numel() % (self.nkpt * self.mpw) == 0)
+        nband = psi.numel() // (self.nkpt * self.mpw) if self.mpw else 0
+        dft_apply_vloc_noalloc(self.h, psi.data_ptr(), hpsi.data_ptr(), nband, torch.cuda.current_stream().cuda_stream)
         return hpsi
 
     def get_kg_gamma(self):

@@ -12,7 +12,7 @@ SOURCES = [("plan.cu", "plan.o", []), ("sphere.cu", "sphere.o", []), ("projtab.c
            ("fft_small.cu", "fft_small.o", []), ("fft_small2.cu", "fft_small2.o", []),
            ("fft2.cu", "fft2_p0.o", ["-DFFT2_PART=0"]), ("fft2.cu", "fft2_p1.o", ["-DFFT2_PART=1"]),
            ("fft2.cu", "fft2_p2.o", ["-DFFT2_PART=2"]), ("nonlocal.cu", "nonlocal.o", []),
-           ("gamma.cu", "gamma.o", []), ("spinor.cu", "spinor.o", [])]
+           ("gamma.cu", "gamma.o", []), ("spinor.cu", "spinor.o", []), ("noalloc.cu", "noalloc.o", [])]
 HEADERS = [os.path.join(CSRC, "internal.h"), os.path.join(CSRC, "fft_codelets.cuh"), os.path.join(CSRC, "ptx.cuh"), os.path.join(CSRC, "fft_tw_literals.cuh"), os.path.join(CSRC, "fft_small.cuh"), os.path.join(CSRC, "nonlocal_strassen.inc"), os.path.join(HERE, "..", "include", "dft.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

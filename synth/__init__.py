@@ -10,4 +10,4 @@ Recipe: SURVEY.md section 8(d) "Synthetic inputs" restating BASELINE.json.
 """
 from .rng import normals, uniforms            # noqa: F401
 from .cells import (CONFIG_NAMES, make_config, gen_psi, gen_psi_band, gen_psi_torch,   # noqa: F401
-                    config_seed, projector_l, gamma_dij, spinor_inputs)
+                    config_seed, projector_l, gamma_dij, spinor_inputs, gen_vloc)

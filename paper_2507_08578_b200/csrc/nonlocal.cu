@@ -872,6 +872,70 @@ gemm2_fac_kernel(const __grid_constant__ CUtensorMap mapC, const __grid_constant
   }
 }
 
+// ---------------------------------------------------------------- tiny cells: the whole non-local term in ONE launch
+// For a cell with a few projectors and a few hundred plane waves (c0: 16 x 283 x 8 bands) GEMM-1, the D_ij step and GEMM-2
+// are three dependent launches of 10-17 us that do 36 000 complex multiply-adds: pure launch latency.  Eq. 26 acts on every
+// band by itself, so here one CTA does one band (and k-point) from beginning to end:
+//   1. cprj[p] = sum_G conj(P[p][G]) psi[G]: warp w takes the projectors w, w + 8, ...; its lanes stride over G (coalesced
+//      rows of the table), fixed-order shuffle reduction;
+//   2. c'[i] = sum_j D^a_ij cprj[j] (thread i < nproj, its atom found by a scan of atom_first);
+//   3. hpsi[G] (+)= sum_p P[p][G] c'[p] + kin[G] psi[G] (and the recurrence combination), thread per G.
+// Plain FP64 FMAs (the DMMA tile shapes would be 7/8 padding here); taken when nproj <= 64 and nproj npw nband nkpt <= 1e6
+// (option "nl_tiny" = 0 keeps the GEMM kernels).  Same arithmetic as Eq. 26 in a different summation order.
+constexpr int NLT_MAXP = 64, NLT_THREADS = 256;
+__global__ void __launch_bounds__(NLT_THREADS)
+nl_tiny_kernel(const double2 *__restrict__ ptab, const double2 *__restrict__ psi_all, double2 *__restrict__ hpsi_all,
+               const double *__restrict__ dij, const int32_t *__restrict__ typat, const int32_t *__restrict__ nlmn,
+               const int32_t *__restrict__ atom_first, const int32_t *__restrict__ npw_k, const double *const *kin_k, int natom,
+               int lmax, int nproj, int nband, int mpw, int accumulate, int with_kin, int cheb, double sh, double sy, double sx,
+               const double2 *__restrict__ xprev_all) {
+  __shared__ double2 cp[NLT_MAXP], cq[NLT_MAXP];
+  const int b = blockIdx.x, ik = blockIdx.y, t = threadIdx.x, warp = t >> 5, lane = t & 31;
+  const int npw = npw_k[ik];
+  const double2 *P = ptab + (size_t)ik * nproj * mpw;
+  const size_t row = ((size_t)ik * nband + b) * mpw;
+  const double2 *psi = psi_all + row;
+  double2 *hpsi = hpsi_all + row;
+  for (int p = warp; p < nproj; p += NLT_THREADS / 32) {
+    const double2 *pr = P + (size_t)p * mpw;
+    double sr = 0.0, si = 0.0;
+    for (int g = lane; g < npw; g += 32) {
+      const double2 a = pr[g], x = psi[g];
+      sr += a.x * x.x + a.y * x.y; si += a.x * x.y - a.y * x.x;       // conj(p) psi
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
+    if (lane == 0) cp[p] = make_double2(sr, si);
+  }
+  __syncthreads();
+  if (t < nproj) {
+    int a = 0;
+    while (a + 1 < natom && atom_first[a + 1] <= t) a++;
+    const int first = atom_first[a], nl = nlmn[typat[a]], ii = t - first;
+    const double *D = dij + (size_t)a * lmax * lmax + (size_t)ii * lmax;
+    double sr = 0.0, si = 0.0;
+    for (int jj = 0; jj < nl; jj++) { const double d = D[jj]; sr += d * cp[first + jj].x; si += d * cp[first + jj].y; }
+    cq[t] = make_double2(sr, si);
+  }
+  __syncthreads();
+  const double *kin = kin_k[ik];
+  for (int g = t; g < npw; g += NLT_THREADS) {
+    double rr = 0.0, ri = 0.0;
+    for (int p = 0; p < nproj; p++) {
+      const double2 a = P[(size_t)p * mpw + g], c = cq[p];
+      rr += a.x * c.x - a.y * c.y; ri += a.x * c.y + a.y * c.x;
+    }
+    const double2 x = psi[g];
+    if (with_kin) { const double kg = kin[g]; rr += kg * x.x; ri += kg * x.y; }
+    if (accumulate) { const double2 h = hpsi[g]; rr += h.x; ri += h.y; }
+    if (cheb) {
+      const double2 xp = sx != 0.0 ? xprev_all[row + g] : make_double2(0.0, 0.0);
+      rr = sh * rr + sy * x.x + sx * xp.x; ri = sh * ri + sy * x.y + sx * xp.y;
+    }
+    hpsi[g] = make_double2(rr, ri);
+  }
+}
+
 // ---------------------------------------------------------------- host side
 struct NlMaps {
   CUtensorMap mapP1, mapP2, mapPsi, mapC;
@@ -1208,6 +1272,17 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
   int rc;
   const double2 *cpsi = reinterpret_cast<const double2 *>(psi);
   double2 *chpsi = reinterpret_cast<double2 *>(hpsi);
+  if (with_nl && p->nl_tiny && p->proj_mode == 0 && !cprj_out && !spsi && !dspin && p->nproj <= NLT_MAXP && nband <= 65535 &&
+      p->nkpt <= 65535 && (double)p->nproj * p->mpw * nband * p->nkpt <= 1e6) {
+    phase_begin(p, 7, st);
+    nl_tiny_kernel<<<dim3(nband, p->nkpt), NLT_THREADS, 0, st>>>(
+        reinterpret_cast<const double2 *>(p->d_ptab), cpsi, chpsi, dmat, p->d_typat, p->d_nlmn, p->d_atom_first, d_npw, d_kin, p->natom,
+        p->lmax, p->nproj, nband, p->mpw, accumulate, with_kin, rec != nullptr, rec ? rec->sh : 1.0, rec ? rec->sy : 0.0,
+        rec ? rec->sx : 0.0, rec ? reinterpret_cast<const double2 *>(rec->xprev) : nullptr);
+    phase_end(p, 7, st, 1);
+    DFT_CUDA_CHECK(cudaGetLastError());
+    return DFT_OK;
+  }
   if (!with_nl) {
     dim3 grid((p->mpw + 255) / 256 < 64 ? (p->mpw + 255) / 256 : 64, nband, p->nkpt);
     phase_begin(p, 7, st);

@@ -55,6 +55,13 @@ def band_rel_err(a, b):
     return float(np.max(num / den))
 
 
+def nl_launches(plan, nband):
+    """Launches of the non-local + kinetic part of one dft_apply_h: 1 where the one-launch kernel for tiny cells serves
+    the call (csrc/nonlocal.cu: nproj <= 64 and nproj npw nband nkpt <= 1e6), else GEMM-1, D_ij, GEMM-2."""
+    tiny = 0 < plan.nproj <= 64 and float(plan.nproj) * plan.mpw * nband * plan.nkpt <= 1e6
+    return 1 if tiny else 3
+
+
 def small_box_ok(plan):
     """True when the fused small-box kernel (fft_path = 3) can serve this plan; the plan's fft_path is left at 0."""
     try:

@@ -8,7 +8,7 @@ import oracle
 import paper_2507_08578_b200 as dft
 import synth
 from gpu_util import (make_plan, lib_spheres, oracle_spheres, assert_spheres_equal, gpu_apply, oracle_apply,
-                      band_rel_err, small_box_ok)
+                      band_rel_err, small_box_ok, nl_launches)
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-10     # north_star: "relative error <= 1e-10 per band in FP64"
@@ -39,6 +39,17 @@ def test_small_cells_all_terms_and_isolations(name):
             err = band_rel_err(gpu_apply(plan, psi), ref)
             assert err <= TOL, "%s terms=%d gemm_sym=1: rel err %.3e" % (name, terms, err)
             plan.set_option("gemm_sym", 2)
+    if nl_launches(plan, psi.shape[1]) == 1:
+        # tiny cell: the runs above took the one-launch non-local kernel; the GEMM kernels (skinny GEMM-1 tiles) must agree
+        for terms in (7, 4):
+            plan.set_option("terms", terms)
+            ref = oracle_apply(cfg, sph, psi, terms=terms, method=1 if name in ("c0", "aniso", "aniso8", "aniso5t") else 2)
+            assert plan.apply_h(torch.as_tensor(psi, device="cuda")) is not None and plan.last_launches() == 2     # local term (or zero fill) + one launch
+            plan.set_option("nl_tiny", 0)
+            err = band_rel_err(gpu_apply(plan, psi), ref)
+            assert err <= TOL, "%s terms=%d nl_tiny=0: rel err %.3e" % (name, terms, err)
+            assert plan.last_launches() == 4
+            plan.set_option("nl_tiny", 1)
     plan.destroy()
 
 
@@ -150,7 +161,7 @@ def test_small_box_fused_kernel(name, over):
         for terms in (7, 2):
             plan.set_option("terms", terms)
             got = gpu_apply(plan, psi)
-            assert plan.last_launches() == (4 if terms == 7 else 1)
+            assert plan.last_launches() == (1 + nl_launches(plan, psi.shape[1]) if terms == 7 else 1)
             err = band_rel_err(got, oracle_apply(cfg, sph, psi, terms=terms, method=method))
             assert err <= TOL, "%s fft_path=%d terms=%d: rel err %.3e" % (name, path, terms, err)
             for ik in range(plan.nkpt):
@@ -271,7 +282,7 @@ def test_chebyshev_filter(name):
             t = torch.as_tensor(psi, device="cuda").clone()
             got = plan.chebyshev_filter(t, deg, cen, e).cpu().numpy()
             if plan.nkpt == 1:      # c2m is at k = 0: its GEMMs are the real ones, with a split and a recombination kernel
-                assert plan.last_launches() == ((4 if small_box_ok(plan) else 8) + (2 if name == "c2m" else 0)) * deg
+                assert plan.last_launches() == ((1 if small_box_ok(plan) else 5) + (5 if name == "c2m" else nl_launches(plan, psi.shape[1]))) * deg
             for ik, (kg, ig, kin) in enumerate(sph):
                 ref = oracle.chebyshev_filter(cfg, ik, kg, ig, kin, psi[ik], deg, cen, e, method=1 if name == "aniso" else 2)
                 npw = len(ig)
@@ -706,13 +717,13 @@ def test_multik_scratch_maxima_on_different_kpoints():
     off += (-(buf.data_ptr() + off)) % 256
     plan.set_workspace(buf[off:off + full])
     got = gpu_apply(plan, psi)
-    assert plan.last_launches() == 8                          # one launch per pass over all three k-points
+    assert plan.last_launches() == 5 + nl_launches(plan, nband)   # one launch per pass over all three k-points
     assert band_rel_err(got, ref) <= TOL
     assert bool((buf[:off] == 0xA5).all()) and bool((buf[off + full:] == 0xA5).all()), "scratch written outside the workspace"
     # one byte less than the batched layout needs: the library must fall back to one k-point per launch, not overrun
     plan.set_workspace(buf[off:off + full - 256])
     got = gpu_apply(plan, psi)
-    assert plan.last_launches() > 8 and band_rel_err(got, ref) <= TOL
+    assert plan.last_launches() > 5 + nl_launches(plan, nband) and band_rel_err(got, ref) <= TOL
     assert bool((buf[:off] == 0xA5).all()) and bool((buf[off + full - 256:] == 0xA5).all())
     plan.set_workspace(None)
     plan.destroy()

@@ -675,6 +675,118 @@ fft2_c_ring_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *
   }
 }
 
+// ---- pass C with two barrier domains per CTA (16-line tiles, NS <= 16): warps 0-3 work on the first eight lines of a
+//      tile, warps 4-7 on the other eight, each group with its own named barrier, its own half of the V tile and its own
+//      pace; ring, exchange buffer and twiddles are shared.  The kernel above synchronises all eight warps twice per tile,
+//      so a CTA's shared-memory phases and FP64 phases alternate (ncu: their times ADD UP to the kernel time); with four
+//      barrier domains per SM instead of two, one domain's exchanges can overlap another's transforms.  A ring slot is
+//      written by the TMA for both groups, so it is released by an `empty` mbarrier that both groups arrive on after their
+//      reads; the producer lane (thread 0) waits for it before re-filling the slot.
+template <int R1, int R2>
+__global__ void __launch_bounds__(256, 2)
+fft2_c_ring2_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, cplx *__restrict__ T2,
+                    const double *__restrict__ vloc, RingParams Q) {
+  constexpr int NS = imax(R1, R2);
+  static_assert(NS <= 16, "sixteen slot rows per group");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int XT = 16, HX = 8;
+  constexpr int KSa = pad8(R2 * XT, XT), KSb = pad8(R1 * XT, XT);
+  constexpr int exn = imax(R1 * KSa, R2 * KSb);
+  unsigned char *stages = smem_raw;
+  cplx *sm = reinterpret_cast<cplx *>(stages + (size_t)Q.S * Q.stage_stride);
+  double *vs = reinterpret_cast<double *>(sm + exn);
+  cplx *tws = reinterpret_cast<cplx *>(vs + ((G.n3 * XT + 1) & ~1));   // twiddles exp(+2 pi i j / n3), j < n3
+  uint64_t *full = reinterpret_cast<uint64_t *>(tws + G.n3), *empty = full + Q.S;
+  const int t = threadIdx.x, grp = t >> 7, tl = t & 127, px = grp * HX + (tl & 7), s = tl >> 3;
+  for (int i = t; i < G.n3; i += blockDim.x) tws[i] = __ldg(G.tw3 + i);
+  if (t == 0) {
+    for (int i = 0; i < Q.S; i++) { mbar_init(&full[i], 1); mbar_init(&empty[i], 2); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int first = (int)(((int64_t)Q.ntiles * blockIdx.x) / gridDim.x);
+  const int nmine = (int)(((int64_t)Q.ntiles * (blockIdx.x + 1)) / gridDim.x) - first;
+  const size_t pstride = (size_t)G.n2 * G.n1;
+  int b = first % Q.nb, g = first / Q.nb;
+  int ib = b, ig = g, ist = 0, iround = 0;      // producer's copy (thread 0 only), runs S-1 tiles ahead
+  auto issue = [&]() {
+    if (iround > 0) mbar_wait(&empty[ist], (uint32_t)((iround - 1) & 1));
+    mbar_expect_tx(&full[ist], Q.box_bytes);
+    tma_load_3d(stages + (size_t)ist * Q.stage_stride, &mapT2, &full[ist], 2 * ig * XT, 0, ib);
+    if (++ist == Q.S) { ist = 0; iround++; }
+    if (++ib == Q.nb) { ib = 0; ig++; }
+  };
+  if (t == 0)
+    for (int j = 0; j < Q.S - 1 && j < nmine; j++) issue();
+  int st = 0; uint32_t ph = 0;
+  bool newgroup = true;
+  unsigned vmask = 0, hmask = 0;
+#pragma unroll
+  for (int j1 = 0; j1 < R1; j1++) {
+    const int z = s + R2 * j1;
+    if (run_map(G.zrun, z) >= 0) vmask |= 1u << j1;
+    if ((unsigned)(z - G.zrun.hi) < (unsigned)G.zrun.nhi) hmask |= 1u << j1;
+  }
+  const int off1 = (s - G.zrun.lo) * XT, off2 = (s - G.zrun.hi + G.zrun.nlo) * XT;
+  for (int it = 0; it < nmine; it++) {
+    if (t == 0 && it + Q.S - 1 < nmine) issue();
+    const size_t xy = (size_t)g * XT + px;
+    const bool xok = xy < pstride;
+    if (newgroup) {
+      // this group's half of the V tile; its reads of the previous one ended before its second barrier of the last tile
+      const double *vp = vloc + (size_t)g * XT + grp * HX;
+      for (int i = tl; i < G.n3 * HX; i += 128) {
+        const int z = i >> 3, xx = i & 7;
+        vs[z * XT + grp * HX + xx] = ((size_t)g * XT + grp * HX + xx < pstride) ? __ldg(vp + (size_t)z * pstride + xx) : 0.0;
+      }
+      newgroup = false;
+    }
+    const cplx *in = reinterpret_cast<const cplx *>(stages + (size_t)st * Q.stage_stride) + px;
+    mbar_wait(&full[st], ph);
+    cplx v[NS];
+    if (s < R2) {
+#pragma unroll
+      for (int j1 = 0; j1 < R1; j1++) {
+        const cplx *src = in + ((hmask >> j1) & 1 ? off2 : off1) + R2 * j1 * XT;
+        v[j1] = (vmask >> j1) & 1 ? *src : make_double2(0.0, 0.0);
+      }
+      Dft<R1, +1>::run(v);
+#pragma unroll
+      for (int k1 = 1; k1 < R1; k1++) v[k1] = cmul(v[k1], tws[s * k1]);
+#pragma unroll
+      for (int k1 = 0; k1 < R1; k1++) sm[k1 * KSa + s * XT + px] = v[k1];
+    }
+    if (grp == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
+    if (tl == 0) mbar_arrive(&empty[st]);          // this group has read its half of the ring slot
+    if (s < R1) {
+#pragma unroll
+      for (int j2 = 0; j2 < R2; j2++) v[j2] = sm[s * KSa + j2 * XT + px];
+      Dft<R2, +1>::run(v);
+#pragma unroll
+      for (int k2 = 0; k2 < R2; k2++) v[k2] = cscale(v[k2], vs[(s + R1 * k2) * XT + px]);
+      Dft<R2, -1>::run(v);
+#pragma unroll
+      for (int cc = 1; cc < R2; cc++) v[cc] = cmulc(v[cc], tws[s * cc]);
+#pragma unroll
+      for (int cc = 0; cc < R2; cc++) sm[s * KSa + cc * XT + px] = v[cc];
+    }
+    if (grp == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
+    if (s < R2) {
+#pragma unroll
+      for (int a = 0; a < R1; a++) v[a] = sm[a * KSa + s * XT + px];
+      Dft<R1, -1>::run(v);
+      cplx *base = T2 + (size_t)b * G.t2_band + xy;
+      const unsigned smask = xok ? vmask : 0u;
+      cplx *base1 = base + (ptrdiff_t)(s - G.zrun.lo) * (ptrdiff_t)pstride, *base2 = base + (ptrdiff_t)(s - G.zrun.hi + G.zrun.nlo) * (ptrdiff_t)pstride;
+#pragma unroll
+      for (int d = 0; d < R1; d++)
+        if ((smask >> d) & 1) ((hmask >> d) & 1 ? base2 : base1)[(size_t)(R2 * d) * pstride] = v[d];
+    }
+    if (++st == Q.S) { st = 0; ph ^= 1; }
+    if (++b == Q.nb) { b = 0; newgroup = true; g++; }
+  }
+}
+
 // ---- density (Eq. 6, :140: n(r) = sum_nk w_nk |psi_nk(r)|^2): the forward half of pass C, then
 //      rho(r) += sum_b w_b |psi_b(r)|^2.  A CTA owns WHOLE groups (one flat-xy tile, all bands of the launch), keeps the
 //      running sum over the bands in registers and adds it to rho once per group: no atomics, fixed summation order.
@@ -919,6 +1031,14 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
     if ((rc = set_smem(fft2_b_inv_ring_kernel<R1, R2>, smem))) return rc;
     fft2_b_inv_ring_kernel<R1, R2><<<grid, XT * NS, smem, st>>>(map, G, T1, Q);
   } else {
+    if constexpr (NS <= 16) {
+      if (p->fft_c_split && XT == 16 && F2C_THREADS == 256) {      // two barrier domains per CTA
+        if ((rc = set_smem(fft2_c_ring2_kernel<R1, R2>, smem))) return rc;
+        fft2_c_ring2_kernel<R1, R2><<<grid, 256, smem, st>>>(map, G, T2, vloc, Q);
+        DFT_CUDA_CHECK(cudaGetLastError());
+        return DFT_OK;
+      }
+    }
     if ((rc = set_smem(fft2_c_ring_kernel<R1, R2>, smem))) return rc;
     fft2_c_ring_kernel<R1, R2><<<grid, XT * NS, smem, st>>>(map, G, T2, vloc, Q);
   }

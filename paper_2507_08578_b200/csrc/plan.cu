@@ -591,6 +591,10 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     if ((value == 3 || value == 5) && !fft_small_ok(p)) { set_error("fft_path = 3: the fused small-box kernel cannot serve this plan (box lengths or shared memory)"); return DFT_ERR_UNSUPPORTED; }
     p->fft_path = (int)value; return DFT_OK;
   }
+  if (!strcmp(key, "fft_c_split")) {
+    if (value < 0 || value > 1) { set_error("fft_c_split = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->fft_c_split = (int)value; return DFT_OK;
+  }
   if (!strcmp(key, "nl_tiny")) {
     if (value < 0 || value > 1) { set_error("nl_tiny = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->nl_tiny = (int)value; return DFT_OK;

@@ -149,8 +149,8 @@ int dft_plan_workspace_bytes(const dft_plan *p, int32_t nband, int64_t *min_byte
  * "gemm_strassen" (with gemm_sym active: one level of Strassen's recursion on the two real GEMMs, 7/8 of their flops, same
  * result up to rounding; 0 = never, 1 = wherever nproj is a multiple of 16, 2 = default: for nproj * npw * nband >= 1e10;
  * builds nine block tables of a quarter of the half table each at the first such call),
- * "fft_c_split" (1 = default: the middle FFT pass runs two barrier domains per CTA where its tiles are 16 lines wide, 0 = one;
- * same results), "nl_tiny" (1 = default: cells with nproj <= 64 and nproj * npw * nband * nkpt <= 1e6 take ONE launch for the whole non-local
+ * "fft_c_split" (the middle FFT pass with two barrier domains per CTA where its tiles are 16 lines wide: 0 = never, 1 = wherever
+ * possible, 2 = default: where both radices of the box length are >= 12, e.g. 180, 192, 225, 256; same results), "nl_tiny" (1 = default: cells with nproj <= 64 and nproj * npw * nband * nkpt <= 1e6 take ONE launch for the whole non-local
  * and kinetic part, one CTA per band, instead of GEMM-1, D_ij, GEMM-2; 0 = always the GEMM kernels),
  * "gamma_real" (1 = enable dft_apply_h_gamma, see there), "spinor_fused" (dft_apply_h_spinor: 1 = default, the 2 x 2 potential
  * multiplied inside the middle FFT pass where the register path serves the box; 0 = four scalar local applications).

@@ -1032,7 +1032,9 @@ static int launch_ring(dft_plan *p, const Fft2Geom &G, int pass, cplx *T1, cplx 
     fft2_b_inv_ring_kernel<R1, R2><<<grid, XT * NS, smem, st>>>(map, G, T1, Q);
   } else {
     if constexpr (NS <= 16) {
-      if (p->fft_c_split && XT == 16 && F2C_THREADS == 256) {      // two barrier domains per CTA
+      // two barrier domains per CTA: pays where a tile carries enough arithmetic per exchange (both radices >= 12: 180, 192,
+      // 225, 256: -4 .. -10 %; neutral at 160 / 240; slower at 128 = 8 x 16, +23 %), hence the automatic choice (2)
+      if ((p->fft_c_split == 1 || (p->fft_c_split == 2 && R1 >= 12 && R2 >= 12)) && XT == 16 && F2C_THREADS == 256) {
         if ((rc = set_smem(fft2_c_ring2_kernel<R1, R2>, smem))) return rc;
         fft2_c_ring2_kernel<R1, R2><<<grid, 256, smem, st>>>(map, G, T2, vloc, Q);
         DFT_CUDA_CHECK(cudaGetLastError());

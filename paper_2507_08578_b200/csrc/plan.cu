@@ -592,7 +592,7 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     p->fft_path = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "fft_c_split")) {
-    if (value < 0 || value > 1) { set_error("fft_c_split = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    if (value < 0 || value > 2) { set_error("fft_c_split = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->fft_c_split = (int)value; return DFT_OK;
   }
   if (!strcmp(key, "nl_tiny")) {

@@ -86,6 +86,32 @@ def test_both_gemm_variants_agree(name):
     plan.destroy()
 
 
+@pytest.mark.parametrize("ngfft", [(20, 20, 180), (18, 20, 256), (20, 24, 128), (16, 20, 240), (15, 15, 225)])
+def test_pass_c_barrier_domains(ngfft):
+    """Option fft_c_split: the middle FFT pass (z . V . z^-1) with one barrier domain per CTA (0), two
+    (1: each half of a 16-line tile with its own named barrier, V half-tile and pace) and the automatic choice (2: two where
+    both radices of n3 are >= 12); z lengths 180 = 12 x 15, 256 = 16 x 16, 128 = 8 x 16, 240 = 15 x 16, 225 = 15 x 15, planes
+    whose point count is not a multiple of the tile; against the oracle, and bit-identical to each other."""
+    cfg, plan, sph = _setup("c0", ngfft=ngfft, nband=11)
+    psi = synth.gen_psi(cfg, [sph[0][2]])
+    plan.set_option("fft_path", 4)
+    outs = []
+    for terms in (2, 7):
+        plan.set_option("terms", terms)
+        ref = oracle_apply(cfg, sph, psi, terms=terms, method=2)
+        for split in (0, 1, 2):
+            plan.set_option("fft_c_split", split)
+            for chunk in (0, 3):
+                plan.set_option("band_chunk", chunk)
+                got = gpu_apply(plan, psi)
+                err = band_rel_err(got, ref)
+                assert err <= TOL, "%s terms=%d fft_c_split=%d chunk=%d: %.3e" % (ngfft, terms, split, chunk, err)
+                if terms == 2 and chunk == 0:
+                    outs.append(got)
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+    plan.destroy()
+
+
 def test_box_without_two_stage_factorisation():
     """Box 10 x 20 x 27: 10 and 27 have no two-stage factorisation (generic kernels), 20 = 4 x 5 has, so the
     passes of one transform mix both kernel families."""

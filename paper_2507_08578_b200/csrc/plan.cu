@@ -979,7 +979,16 @@ int dft_apply_h_host(dft_plan *p, const double *psi_host, double *hpsi_host, int
   std::vector<int> sizes;
   {
     const int per = ((nband + ngroup - 1) / ngroup + 63) / 64 * 64;
-    if (ngroup >= 4 && nband >= 64 * 2 * ngroup) {
+    if (ngroup >= 6 && nband >= 128 * ngroup) {
+      // ramp: 64, 128, middle groups in whole pairs of tiles, 128, 64.  A group's host->device copy runs under the kernels
+      // of the group before it and its device->host copy under those of the group after it, and 256 bands take longer to
+      // copy (22 ms at 55 GB/s at c4) than 64 bands take to compute (20 ms): the second and the second-last group are
+      // therefore half as large as the middle ones.
+      const int mid = ngroup - 4, rest = nband - 384, permid = ((rest + mid - 1) / mid + 127) / 128 * 128;
+      sizes.push_back(64); sizes.push_back(128);
+      for (int left = rest; left > 0; left -= permid) sizes.push_back(left < permid ? left : permid);
+      sizes.push_back(128); sizes.push_back(64);
+    } else if (ngroup >= 4 && nband >= 64 * 2 * ngroup) {
       const int mid = ngroup - 2, rest = nband - 128, permid = ((rest + mid - 1) / mid + 63) / 64 * 64;
       sizes.push_back(64);
       for (int left = rest; left > 0; left -= permid) sizes.push_back(left < permid ? left : permid);

@@ -634,6 +634,24 @@ def test_host_api_uneven_groups():
     plan.destroy()
 
 
+def test_host_api_ramped_groups():
+    """Six groups and at least 128 bands per group: 64, 128, middle groups, 128, 64 (a group's copies run under its
+    neighbours' kernels, and large groups next to the small first and last ones would outlast them): 800 bands ->
+    64, 128, 256, 160, 128, 64."""
+    cfg, plan, sph = _setup("c1m", nband=800)
+    psi = synth.gen_psi(cfg, [s[2] for s in sph])
+    plan.set_option("host_groups", 6)
+    plan.set_option("fft_path", 4)
+    got = plan.apply_h_host(psi)
+    assert plan.last_launches() == 8 * 6
+    ref = gpu_apply(plan, psi)
+    assert band_rel_err(got, ref) <= 1e-13
+    sample = [0, 63, 64, 191, 192, 447, 448, 607, 608, 735, 736, 799]       # both sides of every group boundary
+    oref = oracle_apply(cfg, sph, psi[:, sample])
+    assert band_rel_err(got[:, sample], oref) <= TOL
+    plan.destroy()
+
+
 def test_c1_full():
     cfg, plan, sph = _setup("c1")
     psi = synth.gen_psi(cfg, [s[2] for s in sph])

@@ -47,7 +47,7 @@ def test_no_alloc_local_term_matches_existing_path_twice(name, nband):
     assert err1 <= TOL and err2 <= TOL, "%s: %.3e / %.3e" % (name, err1, err2)
     for ik in range(plan.nkpt):                   # pad entries are written as 0, as by dft_apply_h
         assert bool((out[ik][:, int(plan.npw[ik]):] == 0).all())
-    assert free_after == free_before, "device memory in use changed across a call: %d -> %d" % (free_before, free_after)
+    assert free_after >= free_before, "device memory in use grew across a call: free %d -> %d" % (free_before, free_after)
     plan.destroy()
 
 

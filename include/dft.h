@@ -204,8 +204,8 @@ int dft_accumulate_tau(dft_plan *p, const double *psi, const double *weights, do
  * once set, dft_apply_h adds  1/2 sum_{d=x,y,z} (k+G)_d FFT^-1[ v_tau(r) FFT[ (k+G')_d psi ] ]  (three more local
  * applications whose diagonal factors are fused into the scatter and gather passes).  vtau_r: DEVICE
  * [n3][n2][n1] doubles like V_r of dft_set_vloc, copied on `stream`; NULL switches the term off.  Option "terms"
- * bit 3 (value 8) gates it.  Needs box lengths with a two-radix factorisation (else dft_apply_h returns
- * DFT_ERR_UNSUPPORTED while the term is on).                                                       */
+ * bit 3 (value 8) gates it.  Any box the plan accepts is served (the generic FFT passes carry the diagonal factors and
+ * the accumulation too).                                                                            */
 int dft_set_vtau(dft_plan *p, const double *vtau_r, void *stream);
 
 /* Velocity-gauge vector potential (PAPER.md :340: in RT-TDDFT "the velocity gauge changes only the kinetic
@@ -254,8 +254,7 @@ int dft_chebyshev_filter_gamma(dft_plan *p, double *psi, double *work, int32_t n
  * dft_apply_h_spinor: rules of dft_apply_h; DFT_ERR_NOT_READY before dft_set_vloc_spinor while the local term is on.
  * The GEMMs see 2 nband bands.  The local term is one application with the 2 x 2 matrix multiplied in the middle FFT pass
  * where the five-pass register path serves the box (option "spinor_fused", default 1), else four scalar local
- * applications (V0 psi + sum_mu V_mu sigma_mu psi), which need box lengths with a two-radix factorisation or a box small
- * enough for the fused small-box kernel (otherwise DFT_ERR_UNSUPPORTED). */
+ * applications (V0 psi + sum_mu V_mu sigma_mu psi), which every box the plan accepts can take. */
 int dft_set_vloc_spinor(dft_plan *p, const double *v4_dev, void *stream);
 int dft_set_dij_spinor(dft_plan *p, const double *dspin_host);
 int dft_apply_h_spinor(dft_plan *p, const double *psi, double *hpsi, int32_t nband, void *stream);

@@ -120,7 +120,9 @@ struct FftGeom {
 constexpr int FFT_THREADS = 256;
 
 // ---- pass A: scatter + transform along x.  grid (ceil(ncol/CL), nb) -------------------------------
-__global__ void __launch_bounds__(FFT_THREADS) fft_pass_a_kernel(FftGeom G, const cplx *__restrict__ psi, cplx *__restrict__ T1) {
+// pre: optional real diagonal factor in G space ([npw], meta-GGA term), applied while scattering
+__global__ void __launch_bounds__(FFT_THREADS) fft_pass_a_kernel(FftGeom G, const cplx *__restrict__ psi, cplx *__restrict__ T1,
+                                                                 const double *__restrict__ pre) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx *tws = reinterpret_cast<cplx *>(smem_raw);
   cplx *bufa = tws + G.n1, *bufb = bufa + G.CL * G.n1p;
@@ -132,7 +134,11 @@ __global__ void __launch_bounds__(FFT_THREADS) fft_pass_a_kernel(FftGeom G, cons
   int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
   for (int lc = warp; lc < nc; lc += nwarp) {
     int g0 = G.col_start[c0 + lc], g1 = G.col_start[c0 + lc + 1];
-    for (int g = g0 + lane; g < g1; g += 32) bufa[lc * G.n1p + G.pw_i1[g]] = src[g];
+    for (int g = g0 + lane; g < g1; g += 32) {
+      cplx v = src[g];
+      if (pre) { const double f = pre[g]; v.x *= f; v.y *= f; }
+      bufa[lc * G.n1p + G.pw_i1[g]] = v;
+    }
   }
   cplx *res = fft_lines<+1>(bufa, bufb, tws, G.n1, G.f1, G.CL, 1, G.n1p);
   cplx *dst = T1 + (size_t)b * G.t1_band + (size_t)c0 * G.n1;
@@ -140,7 +146,9 @@ __global__ void __launch_bounds__(FFT_THREADS) fft_pass_a_kernel(FftGeom G, cons
 }
 
 // ---- pass A^-1: inverse along x + gather.  grid (ceil(ncol/CL), nb) ---------------------------------
-__global__ void __launch_bounds__(FFT_THREADS) fft_pass_ainv_kernel(FftGeom G, const cplx *__restrict__ T1, cplx *__restrict__ hpsi) {
+// post: optional real diagonal factor applied while gathering; accumulate: hpsi += result (pad entries untouched)
+__global__ void __launch_bounds__(FFT_THREADS) fft_pass_ainv_kernel(FftGeom G, const cplx *__restrict__ T1, cplx *__restrict__ hpsi,
+                                                                    const double *__restrict__ post, int accumulate) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx *tws = reinterpret_cast<cplx *>(smem_raw);
   cplx *bufa = tws + G.n1, *bufb = bufa + G.CL * G.n1p;
@@ -156,10 +164,15 @@ __global__ void __launch_bounds__(FFT_THREADS) fft_pass_ainv_kernel(FftGeom G, c
   int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
   for (int lc = warp; lc < nc; lc += nwarp) {
     int g0 = G.col_start[c0 + lc], g1 = G.col_start[c0 + lc + 1];
-    for (int g = g0 + lane; g < g1; g += 32) dst[g] = res[lc * G.n1p + G.pw_i1[g]];
+    for (int g = g0 + lane; g < g1; g += 32) {
+      cplx v = res[lc * G.n1p + G.pw_i1[g]];
+      if (post) { const double f = post[g]; v.x *= f; v.y *= f; }
+      if (accumulate) { const cplx h = dst[g]; v.x += h.x; v.y += h.y; }
+      dst[g] = v;
+    }
   }
   // entries ipw >= npw of the band are defined to be 0 on output
-  if (blockIdx.x == gridDim.x - 1)
+  if (blockIdx.x == gridDim.x - 1 && !accumulate)
     for (int g = G.npw + threadIdx.x; g < G.mpw; g += blockDim.x) dst[g] = make_double2(0.0, 0.0);
 }
 
@@ -344,8 +357,9 @@ int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb,
   // codelet radices and the sphere's occupied sets are runs; otherwise the generic Stockham kernel
   bool fast[3];
   for (int c = 0; c < 3; c++) fast[c] = p->fft_path != 1 && kp.runs_ok && fft2_pair(p->n[c], nullptr, nullptr);
-  if (extra && !(fast[0] && fast[1] && fast[2])) {
-    set_error("this term needs box lengths with a two-radix factorisation (register FFT path)");
+  const double *vpot = (extra && extra->vpot) ? extra->vpot : p->d_vloc;
+  if (extra && extra->vspin && !(fast[0] && fast[1] && fast[2])) {
+    set_error("the fused spinor pass needs box lengths with a two-radix factorisation (register FFT path)");
     return DFT_ERR_UNSUPPORTED;
   }
   const int axis_of[5] = {0, 1, 2, 1, 0};
@@ -353,11 +367,11 @@ int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb,
     phase_begin(p, pass, st);
     if (fast[axis_of[pass]]) {
       if ((rc = fft2_launch(p, ik, pass, psi, hpsi, T1, T2, G.t1_band, G.t2_band, nb, st, extra))) return rc;
-    } else if (pass == 0) fft_pass_a_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, cpsi, T1);
+    } else if (pass == 0) fft_pass_a_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, cpsi, T1, extra ? extra->pre : nullptr);
     else if (pass == 1) fft_pass_b_kernel<+1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
-    else if (pass == 2) fft_pass_c_kernel<<<gc, FFT_THREADS, sm_c, st>>>(G, T2, p->d_vloc);
+    else if (pass == 2) fft_pass_c_kernel<<<gc, FFT_THREADS, sm_c, st>>>(G, T2, vpot);
     else if (pass == 3) fft_pass_b_kernel<-1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
-    else fft_pass_ainv_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, T1, chpsi);
+    else fft_pass_ainv_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, T1, chpsi, extra ? extra->post : nullptr, extra ? extra->accumulate : 0);
     phase_end(p, pass, st, 1);
   }
   DFT_CUDA_CHECK(cudaGetLastError());

@@ -369,17 +369,22 @@ def test_density_accumulation(name):
     plan.destroy()
 
 
-@pytest.mark.parametrize("name", ["c1m", "aniso", "c3k2"])
-def test_meta_gga_term(name):
-    """dft_set_vtau (Eq. 8): the term alone (terms = 8), with everything else (15), and switched off again."""
-    cfg, plan, sph = _setup(name)
+@pytest.mark.parametrize("name,over,path", [("c1m", {}, 0), ("aniso", {}, 0), ("c3k2", {}, 0), ("c1m", {}, 1),
+                                            ("aniso", {"ngfft": (20, 27, 25)}, 4), ("c0", {"ngfft": (10, 20, 27)}, 4)],
+                         ids=lambda v: v if isinstance(v, str) else ("x".join(map(str, v.get("ngfft", ()))) if isinstance(v, dict) else "path%d" % v))
+def test_meta_gga_term(name, over, path):
+    """dft_set_vtau (Eq. 8): the term alone (terms = 8), with everything else (15), and switched off again; on
+    the automatic path, on the generic kernels (fft_path 1) and on boxes that mix lengths with and without a two-radix
+    factorisation (27 and 10 have none), where the diagonal factors and the accumulation go through the generic passes."""
+    cfg, plan, sph = _setup(name, **over)
+    plan.set_option("fft_path", path)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     n = cfg["ngfft"]
     rng = np.random.default_rng(6)
     vt = 0.4 + 0.15 * rng.standard_normal((n[2], n[1], n[0]))
     plain = gpu_apply(plan, psi)
     plan.set_vtau(torch.as_tensor(vt, device="cuda"))
-    m = 1 if name == "aniso" else 2
+    m = 1 if name in ("aniso", "c0") else 2
     tau = np.zeros_like(psi)
     for ik, (kg, ig, kin) in enumerate(sph):
         tau[ik] = oracle.apply_mgga(cfg, ik, kg, ig, psi[ik], vt, method=m)

@@ -64,3 +64,57 @@ def test_random_cell(seed):
             assert np.all(got[ik][:, plan.npw[ik]:] == 0)
         plan.set_option(key, back)
     plan.destroy()
+
+
+@pytest.mark.parametrize("seed", range(0, 12, 2))
+def test_random_cell_gamma_storage(seed):
+    """The even seeds are Gamma-point cells: the same random cell in real-symmetry storage (DESIGN.md
+    reading 26) with the odd-parity couplings of D_ij removed, on the fused / five-pass / generic local paths, with and
+    without the Strassen level (refused silently where nproj is not a multiple of 16)."""
+    cfg = _random_cfg(seed)
+    cfg["kpt"] = cfg["kpt"][:1]; cfg["nkpt"] = 1
+    cfg["dij"] = synth.gamma_dij(cfg)
+    plan = make_plan(cfg)
+    kg, ig, kin = lib_spheres(plan)[0]
+    plan.set_option("gamma_real", 1)
+    hkin = plan.get_kg_gamma()[2]
+    nb = cfg["nband"] + (cfg["nband"] & 1) + 2                    # even band counts >= 4, and one odd count below
+    for nband in (nb, nb - 1):
+        psi = synth.gen_psi(cfg, [hkin], nband=nband)[0]
+        ref = oracle.apply_h_gamma(cfg, kg, ig, kin, psi, method=1)
+        for path in (0, 4, 1):
+            plan.set_option("fft_path", path)
+            for strassen in (2, 1):
+                plan.set_option("gemm_strassen", strassen)
+                out = plan.apply_h_gamma(torch.as_tensor(psi, device="cuda").contiguous())
+                torch.cuda.synchronize()
+                got = out.cpu().numpy()
+                err = band_rel_err(got, ref)
+                assert err <= TOL, "seed %d nband %d fft_path %d strassen %d: %.3e" % (seed, nband, path, strassen, err)
+                assert np.all(got[:, 0].imag == 0)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("seed", range(1, 12, 2))
+def test_random_cell_spinors(seed):
+    """The odd seeds (general k-points): two-component spinors with a Hermitian 2 x 2 potential and a spin-dependent D
+    (reading 27), fused 2 x 2 pass C where the box allows it, the Pauli form elsewhere (also on the generic kernels: box
+    lengths without a two-radix factorisation)."""
+    cfg = _random_cfg(seed)
+    plan = make_plan(cfg)
+    sph = lib_spheres(plan)
+    v4, dspin = synth.spinor_inputs(cfg)
+    plan.set_vloc_spinor(torch.as_tensor(v4, device="cuda"))
+    plan.set_dij_spinor(dspin)
+    nb = cfg["nband"]
+    psi = synth.gen_psi(cfg, [s[2] for s in sph], nband=2 * nb).reshape(plan.nkpt, nb, 2, plan.mpw)
+    ref = np.stack([oracle.apply_h_spinor(cfg, ik, *sph[ik], psi[ik], v4, dspin, method=1) for ik in range(plan.nkpt)])
+    for path in (0, 4, 1):
+        plan.set_option("fft_path", path)
+        for fused in (1, 0):
+            plan.set_option("spinor_fused", fused)
+            out = plan.apply_h_spinor(torch.as_tensor(psi, device="cuda").contiguous())
+            torch.cuda.synchronize()
+            err = band_rel_err(out.cpu().numpy(), ref)
+            assert err <= TOL, "seed %d fft_path %d spinor_fused %d: %.3e" % (seed, path, fused, err)
+    plan.destroy()

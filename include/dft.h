@@ -192,7 +192,8 @@ int dft_get_cprj(dft_plan *p, const double *psi, double *cprj, int32_t nband, vo
  * and occupations into the weights).  psi: DEVICE [nkpt][nband][mpw]; weights: HOST [nkpt][nband], copied before
  * the call returns (one synchronisation of `stream`); rho: DEVICE [n3][n2][n1] doubles, i1 fastest, ACCUMULATED into (zero it first).  Runs the
  * scatter + x and y passes of dft_apply_h and the forward half of its z pass, summing over bands in registers
- * (no atomics, fixed order).  DFT_ERR_UNSUPPORTED for box lengths without a two-radix factorisation.  */
+ * (no atomics, fixed order).  Any box the plan accepts is served (generic passes where an axis length has no two-radix
+ * factorisation).  */
 int dft_accumulate_density(dft_plan *p, const double *psi, const double *weights, double *rho, int32_t nband, void *stream);
 
 /* Kinetic-energy density of the same equation (Eq. 6: tau(r) = 1/2 sum_nk w_nk |grad psi_nk(r)|^2):

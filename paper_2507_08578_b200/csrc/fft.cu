@@ -244,6 +244,39 @@ __global__ void __launch_bounds__(FFT_THREADS) fft_pass_c_kernel(FftGeom G, cplx
   }
 }
 
+// ---- density on the generic path (Eq. 6, :140): the forward half of pass C, then rho += sum_b w_b |psi_b(r)|^2.
+//      grid (nxt, n2); a CTA owns its (x tile, y) lines for ALL bands of the launch, keeps the running sum in shared memory
+//      and adds it to rho once: no atomics, fixed summation order (the register path has its own kernel in fft2.cu).
+__global__ void __launch_bounds__(FFT_THREADS) fft_density_c_kernel(FftGeom G, const cplx *__restrict__ T2, const double *__restrict__ wgt,
+                                                                    double *__restrict__ rho, int nb) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *tws = reinterpret_cast<cplx *>(smem_raw);
+  cplx *bufa = tws + G.n3, *bufb = bufa + G.n3 * G.XT;
+  double *acc = reinterpret_cast<double *>(bufb + G.n3 * G.XT);
+  int x0 = blockIdx.x * G.XT, nx = min(G.XT, G.n1 - x0), y = blockIdx.y;
+  load_twiddles(tws, G.tw3, G.n3);
+  size_t pstride = (size_t)G.n2 * G.n1;
+  for (int i = threadIdx.x; i < G.n3 * G.XT; i += blockDim.x) acc[i] = 0.0;
+  for (int b = 0; b < nb; b++) {
+    const cplx *t2 = T2 + (size_t)b * G.t2_band + (size_t)y * G.n1 + x0;
+    __syncthreads();
+    for (int i = threadIdx.x; i < G.n3 * G.XT; i += blockDim.x) bufa[i] = make_double2(0.0, 0.0);
+    __syncthreads();
+    for (int i = threadIdx.x; i < G.nplane * G.XT; i += blockDim.x) {
+      int p = i / G.XT, xt = i % G.XT;
+      if (xt < nx) bufa[G.plane_i3[p] * G.XT + xt] = t2[p * pstride + xt];
+    }
+    cplx *res = fft_lines<+1>(bufa, bufb, tws, G.n3, G.f3, G.XT, G.XT, 1);
+    const double w = wgt[b];
+    for (int i = threadIdx.x; i < G.n3 * G.XT; i += blockDim.x) acc[i] += w * (res[i].x * res[i].x + res[i].y * res[i].y);
+  }
+  double *dst = rho + (size_t)y * G.n1 + x0;
+  for (int i = threadIdx.x; i < G.n3 * G.XT; i += blockDim.x) {
+    int z = i / G.XT, xt = i % G.XT;
+    if (xt < nx) dst[z * pstride + xt] += acc[i];
+  }
+}
+
 __global__ void zero_kernel(double *p, int64_t n) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = 0.0;
 }
@@ -374,6 +407,45 @@ int fft_apply_vloc(dft_plan *p, int ik, const double *psi, double *hpsi, int nb,
     else fft_pass_ainv_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, T1, chpsi, extra ? extra->post : nullptr, extra ? extra->accumulate : 0);
     phase_end(p, pass, st, 1);
   }
+  DFT_CUDA_CHECK(cudaGetLastError());
+  return DFT_OK;
+}
+
+// rho(r) += sum_b wgt[b] |psi_b(r)|^2 for nb bands of k-point ik on ANY box the plan accepts: passes A and B as in
+// fft_apply_vloc (register kernels where the axis length has a two-radix factorisation, generic ones elsewhere), then the
+// generic density kernel.  fft2_density (register path, faster) is preferred by the caller where all three axes have it.
+int fft_density_generic(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st,
+                        const double *pre) {
+  int rc = set_attrs();
+  if (rc) return rc;
+  const KPoint &kp = p->kp[ik];
+  if (kp.npw == 0 || nb == 0) return DFT_OK;
+  FftGeom G = make_geom(p, ik);
+  int64_t t1b = ((int64_t)G.t1_band * 16 + 255) / 256 * 256;
+  cplx *T1 = reinterpret_cast<cplx *>(ws);
+  cplx *T2 = reinterpret_cast<cplx *>(reinterpret_cast<char *>(ws) + t1b * nb);
+  G.t1_band = t1b / 16;
+  G.t2_band = (((int64_t)G.t2_band * 16 + 255) / 256 * 256) / 16;
+  const cplx *cpsi = reinterpret_cast<const cplx *>(psi);
+  size_t sm_a = sizeof(cplx) * ((size_t)G.n1 + 2 * (size_t)G.CL * G.n1p);
+  size_t sm_b = sizeof(cplx) * ((size_t)G.n2 + 2 * (size_t)G.n2 * G.XT);
+  size_t sm_d = sizeof(cplx) * ((size_t)G.n3 + 2 * (size_t)G.n3 * G.XT) + sizeof(double) * (size_t)G.n3 * G.XT;
+  dim3 ga((G.ncol + G.CL - 1) / G.CL, nb), gb(G.nxt, G.nplane, nb), gd(G.nxt, G.n2);
+  FftExtra X;
+  X.pre = pre;
+  for (int pass = 0; pass < 2; pass++) {
+    phase_begin(p, pass, st);
+    const bool fast = p->fft_path != 1 && kp.runs_ok && fft2_pair(p->n[pass], nullptr, nullptr);
+    if (fast) {
+      if ((rc = fft2_launch(p, ik, pass, psi, nullptr, T1, T2, G.t1_band, G.t2_band, nb, st, &X))) return rc;
+    } else if (pass == 0) fft_pass_a_kernel<<<ga, FFT_THREADS, sm_a, st>>>(G, cpsi, T1, pre);
+    else fft_pass_b_kernel<+1><<<gb, FFT_THREADS, sm_b, st>>>(G, T1, T2);
+    phase_end(p, pass, st, 1);
+  }
+  if (sm_d > 48 * 1024) DFT_CUDA_CHECK(cudaFuncSetAttribute(fft_density_c_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_d));
+  phase_begin(p, 2, st);
+  fft_density_c_kernel<<<gd, FFT_THREADS, sm_d, st>>>(G, T2, wgt_dev, rho, nb);
+  phase_end(p, 2, st, 1);
   DFT_CUDA_CHECK(cudaGetLastError());
   return DFT_OK;
 }

@@ -251,6 +251,8 @@ bool fft2_batch_ok(const dft_plan *p);
 int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int nband_total, void *ws, cudaStream_t st);
 
 // rho(r) += sum_b wgt[b] |psi_b(r)|^2 (device wgt [nb]); forward passes A, B and the density kernel
+int fft_density_generic(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st,
+                        const double *pre);   // fft.cu: any box (generic passes where an axis has no two-radix factorisation)
 int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, double *rho, int nb, void *ws, cudaStream_t st,
                  const double *pre = nullptr);
 

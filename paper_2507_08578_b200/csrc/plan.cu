@@ -868,9 +868,16 @@ static int accumulate_impl(dft_plan *p, const double *psi, const double *weights
     for (int b0 = 0; b0 < nband; b0 += chunk) {
       int nb = nband - b0 < chunk ? nband - b0 : chunk;
       size_t off = ((size_t)ik * nband + b0) * band_stride;
-      for (int d = 0; d < (tau ? 3 : 1); d++)
-        if ((rc = fft2_density(p, ik, psi + off, p->d_wgt + (size_t)ik * nband + b0, rho, nb, ws, st,
-                               tau ? p->d_qcart + ((size_t)ik * 3 + d) * p->mpw : nullptr))) return rc;
+      bool regpath = p->fft_path != 1 && p->kp[ik].runs_ok;
+      for (int c = 0; c < 3 && regpath; c++) regpath = fft2_pair(p->n[c], nullptr, nullptr);
+      for (int d = 0; d < (tau ? 3 : 1); d++) {
+        const double *pre = tau ? p->d_qcart + ((size_t)ik * 3 + d) * p->mpw : nullptr;
+        rc = regpath ? fft2_density(p, ik, psi + off, p->d_wgt + (size_t)ik * nband + b0, rho, nb, ws, st, pre)
+                     : fft_density_generic(p, ik, psi + off, p->d_wgt + (size_t)ik * nband + b0, rho, nb, ws, st, pre);
+        if (rc == DFT_ERR_UNSUPPORTED && regpath)      // e.g. a tile that does not fit the register kernel: the generic passes
+          rc = fft_density_generic(p, ik, psi + off, p->d_wgt + (size_t)ik * nband + b0, rho, nb, ws, st, pre);
+        if (rc) return rc;
+      }
     }
   return DFT_OK;
   DFT_GUARD_END

@@ -343,11 +343,15 @@ def test_velocity_gauge_kinetic(name):
     plan.destroy()
 
 
-@pytest.mark.parametrize("name", ["c0", "c1m", "aniso", "c3k2"])
-def test_density_accumulation(name):
+@pytest.mark.parametrize("name,over,path", [("c0", {}, 0), ("c1m", {}, 0), ("aniso", {}, 0), ("c3k2", {}, 0), ("c1m", {}, 1),
+                                            ("aniso", {"ngfft": (20, 27, 25)}, 0), ("c0", {"ngfft": (10, 20, 27)}, 0)],
+                         ids=lambda v: v if isinstance(v, str) else ("x".join(map(str, v.get("ngfft", ()))) if isinstance(v, dict) else "path%d" % v))
+def test_density_accumulation(name, over, path):
     """dft_accumulate_density (Eq. 6, :140) against the oracle, accumulating over k-points, in two calls
-    (rho is added to), with a band chunk that leaves a ragged tail."""
-    cfg, plan, sph = _setup(name, nband=7)
+    (rho is added to), with a band chunk that leaves a ragged tail; register kernels, generic kernels (fft_path 1) and
+    boxes that mix axis lengths with and without a two-radix factorisation (the generic density kernel)."""
+    cfg, plan, sph = _setup(name, nband=7, **over)
+    plan.set_option("fft_path", path)
     psi = synth.gen_psi(cfg, [s[2] for s in sph])
     rng = np.random.default_rng(9)
     w = rng.uniform(0.1, 2.0, size=(plan.nkpt, 7))

@@ -877,8 +877,8 @@ fft2_density_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, const
 #define FFT2_PART 0
 #endif
 #define FFT2_PAIRS_0(X) X(3, 3) X(4, 4) X(4, 5) X(4, 6) X(5, 5) X(5, 6) X(4, 8) X(6, 6) X(5, 8) X(12, 15)
-#define FFT2_PAIRS_1(X) X(6, 8) X(5, 10) X(6, 10) X(8, 8) X(8, 9) X(8, 10) X(9, 9) X(9, 10) X(8, 12) X(8, 16)
-#define FFT2_PAIRS_2(X) X(10, 10) X(9, 12) X(10, 12) X(12, 12) X(10, 15) X(10, 16) X(12, 16) X(15, 15) X(15, 16) X(16, 16)
+#define FFT2_PAIRS_1(X) X(6, 8) X(5, 10) X(6, 10) X(8, 8) X(8, 9) X(8, 10) X(9, 9) X(9, 10) X(8, 12) X(8, 16) X(5, 9) X(6, 9)
+#define FFT2_PAIRS_2(X) X(10, 10) X(9, 12) X(10, 12) X(12, 12) X(10, 15) X(10, 16) X(12, 16) X(15, 15) X(15, 16) X(16, 16) X(5, 15) X(9, 15)
 #define FFT2_PAIRS_ALL(X) FFT2_PAIRS_0(X) FFT2_PAIRS_1(X) FFT2_PAIRS_2(X)
 #if FFT2_PART == 0
 #define FFT2_PAIRS(X) FFT2_PAIRS_0(X)

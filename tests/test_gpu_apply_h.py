@@ -112,6 +112,29 @@ def test_pass_c_barrier_domains(ngfft):
     plan.destroy()
 
 
+@pytest.mark.parametrize("ngfft", [(45, 54, 75), (54, 45, 135), (75, 45, 54)])
+def test_box_lengths_45_54_75_135(ngfft):
+    """Register path for the box lengths 45 = 5 x 9, 54 = 6 x 9, 75 = 5 x 15 and 135 = 9 x 15 on every axis in turn
+    (all-terms H psi, local term alone, density) against the oracle."""
+    cfg, plan, sph = _setup("c0", ngfft=ngfft, ecut=20.0, nband=5)
+    psi = synth.gen_psi(cfg, [sph[0][2]])
+    for terms in (7, 2):
+        plan.set_option("terms", terms)
+        ref = oracle_apply(cfg, sph, psi, terms=terms, method=2)
+        for path in (0, 2, 1):
+            plan.set_option("fft_path", path)
+            err = band_rel_err(gpu_apply(plan, psi), ref)
+            assert err <= TOL, "%s terms=%d fft_path=%d: %.3e" % (ngfft, terms, path, err)
+    plan.set_option("fft_path", 0); plan.set_option("terms", 15)
+    gpu_apply(plan, psi)
+    assert plan.last_launches() == 5 + nl_launches(plan, 5)      # five passes
+    w = np.linspace(0.5, 1.5, 5)[None]
+    rho = plan.accumulate_density(torch.as_tensor(psi, device="cuda"), w).cpu().numpy()
+    ref = oracle.density(cfg["ngfft"], sph[0][1], psi[0], w[0], method=2)
+    assert np.max(np.abs(rho - ref)) <= 1e-12 * ref.max()
+    plan.destroy()
+
+
 def test_box_without_two_stage_factorisation():
     """Box 10 x 20 x 27: 10 and 27 have no two-stage factorisation (generic kernels), 20 = 4 x 5 has, so the
     passes of one transform mix both kernel families."""

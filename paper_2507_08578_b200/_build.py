@@ -7,11 +7,11 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdftb200.so")
-# (source, object, extra flags): fft2.cu is compiled in three parts, each instantiating a third of the radix pairs
+# (source, object, extra flags): fft2.cu is compiled in four parts, each instantiating a part of the radix pairs
 SOURCES = [("plan.cu", "plan.o", []), ("sphere.cu", "sphere.o", []), ("projtab.cu", "projtab.o", []), ("fft.cu", "fft.o", []),
            ("fft_small.cu", "fft_small.o", []), ("fft_small2.cu", "fft_small2.o", []),
            ("fft2.cu", "fft2_p0.o", ["-DFFT2_PART=0"]), ("fft2.cu", "fft2_p1.o", ["-DFFT2_PART=1"]),
-           ("fft2.cu", "fft2_p2.o", ["-DFFT2_PART=2"]), ("nonlocal.cu", "nonlocal.o", []),
+           ("fft2.cu", "fft2_p2.o", ["-DFFT2_PART=2"]), ("fft2.cu", "fft2_p3.o", ["-DFFT2_PART=3"]), ("nonlocal.cu", "nonlocal.o", []),
            ("gamma.cu", "gamma.o", []), ("spinor.cu", "spinor.o", []), ("noalloc.cu", "noalloc.o", [])]
 HEADERS = [os.path.join(CSRC, "internal.h"), os.path.join(CSRC, "fft_codelets.cuh"), os.path.join(CSRC, "ptx.cuh"), os.path.join(CSRC, "fft_tw_literals.cuh"), os.path.join(CSRC, "fft_small.cuh"), os.path.join(CSRC, "nonlocal_strassen.inc"), os.path.join(HERE, "..", "include", "dft.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

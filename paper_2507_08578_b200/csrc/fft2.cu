@@ -870,8 +870,8 @@ fft2_density_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, const
 // host side: pair table, launch geometry
 // ------------------------------------------------------------------------------------------
 // (R1, R2) with R1 <= R2, both radices available as register codelets
-// The file is compiled three times (-DFFT2_PART=0,1,2, see _build.py): each translation unit instantiates the kernels of
-// a third of the pairs and exports the three dispatch functions below under a part-specific name; part 0 also holds the
+// The file is compiled four times (-DFFT2_PART=0..3, see _build.py): each translation unit instantiates the kernels of
+// a part of the pairs and exports the three dispatch functions below under a part-specific name; part 0 also holds the
 // entry points, which try the parts in turn.
 #ifndef FFT2_PART
 #define FFT2_PART 0
@@ -879,16 +879,21 @@ fft2_density_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, const
 #define FFT2_PAIRS_0(X) X(3, 3) X(4, 4) X(4, 5) X(4, 6) X(5, 5) X(5, 6) X(4, 8) X(6, 6) X(5, 8) X(12, 15)
 #define FFT2_PAIRS_1(X) X(6, 8) X(5, 10) X(6, 10) X(8, 8) X(8, 9) X(8, 10) X(9, 9) X(9, 10) X(8, 12) X(8, 16) X(5, 9) X(6, 9)
 #define FFT2_PAIRS_2(X) X(10, 10) X(9, 12) X(10, 12) X(12, 12) X(10, 15) X(10, 16) X(12, 16) X(15, 15) X(15, 16) X(16, 16) X(5, 15) X(9, 15)
-#define FFT2_PAIRS_ALL(X) FFT2_PAIRS_0(X) FFT2_PAIRS_1(X) FFT2_PAIRS_2(X)
+// radices 18 = 2 x 9 and 20 = 4 x 5 (prime-factor codelets): 162, 200, 216, 270, 288, 300, 320, 324, 360, 400
+#define FFT2_PAIRS_3(X) X(9, 18) X(10, 20) X(12, 18) X(15, 18) X(16, 18) X(15, 20) X(16, 20) X(18, 18) X(18, 20) X(20, 20)
+#define FFT2_PAIRS_ALL(X) FFT2_PAIRS_0(X) FFT2_PAIRS_1(X) FFT2_PAIRS_2(X) FFT2_PAIRS_3(X)
 #if FFT2_PART == 0
 #define FFT2_PAIRS(X) FFT2_PAIRS_0(X)
 #define FFT2_PARTFN(name) name##_p0
 #elif FFT2_PART == 1
 #define FFT2_PAIRS(X) FFT2_PAIRS_1(X)
 #define FFT2_PARTFN(name) name##_p1
-#else
+#elif FFT2_PART == 2
 #define FFT2_PAIRS(X) FFT2_PAIRS_2(X)
 #define FFT2_PARTFN(name) name##_p2
+#else
+#define FFT2_PAIRS(X) FFT2_PAIRS_3(X)
+#define FFT2_PARTFN(name) name##_p3
 #endif
 constexpr int FFT2_NOT_MINE = 0x7f000001;   // "this pair is instantiated in another part"
 struct Fft2PassArgs {      // arguments of one pass launch, the same for every part
@@ -900,7 +905,7 @@ struct Fft2PassArgs {      // arguments of one pass launch, the same for every p
   int fft2_pass_##part(const Fft2PassArgs &a, int r1, int r2); \
   int fft2_batched_pass_##part(const Fft2PassArgs &a, int r1, int r2); \
   int fft2_density_pass_##part(const Fft2PassArgs &a, int r1, int r2);
-FFT2_DECL(p0) FFT2_DECL(p1) FFT2_DECL(p2)
+FFT2_DECL(p0) FFT2_DECL(p1) FFT2_DECL(p2) FFT2_DECL(p3)
 
 #if FFT2_PART == 0
 bool fft2_pair(int n, int *r1, int *r2) {
@@ -1054,6 +1059,7 @@ static int launch_pass(dft_plan *p, const Fft2Geom &G, int pass, const cplx *psi
   constexpr int NS = imax(R1, R2);
   int rc;
   if (pass == 2 && X.vspin) {       // two-component spinors: rows in (up, down) pairs, 2 x 2 potential
+    if (16 * NS > F2_THREADS) { set_error("the fused spinor pass serves radices up to 16 (box length %d)", G.n3); return DFT_ERR_UNSUPPORTED; }
     if (nb & 1) { set_error("the spinor local term needs an even number of rows per launch (got %d)", nb); return DFT_ERR_INVALID_ARG; }
     const int nxt = (G.n1 + 7) / 8;
     const size_t sm = sizeof(cplx) * (size_t)(imax(pad8(R2 * 16, 16) * R1, pad8(R1 * 16, 16) * R2) + G.n3) + sizeof(double) * 4 * (size_t)G.n3 * 8;
@@ -1166,11 +1172,12 @@ int FFT2_PARTFN(fft2_batched_pass)(const Fft2PassArgs &a, int r1, int r2) {
 }
 
 #if FFT2_PART == 0
-static int try_parts(int (*f0)(const Fft2PassArgs &, int, int), int (*f1)(const Fft2PassArgs &, int, int),
-                     int (*f2)(const Fft2PassArgs &, int, int), const Fft2PassArgs &a, int r1, int r2) {
+typedef int (*PartFn)(const Fft2PassArgs &, int, int);
+static int try_parts(PartFn f0, PartFn f1, PartFn f2, PartFn f3, const Fft2PassArgs &a, int r1, int r2) {
   int rc = f0(a, r1, r2);
   if (rc == FFT2_NOT_MINE) rc = f1(a, r1, r2);
   if (rc == FFT2_NOT_MINE) rc = f2(a, r1, r2);
+  if (rc == FFT2_NOT_MINE) rc = f3(a, r1, r2);
   return rc == FFT2_NOT_MINE ? DFT_ERR_UNSUPPORTED : rc;
 }
 
@@ -1218,7 +1225,7 @@ int fft2_apply_batched(dft_plan *p, const double *psi, double *hpsi, int nb, int
     fft2_pair(p->n[axis_of[pass]], &r1, &r2);
     phase_begin(p, pass, st);
     Fft2PassArgs a = {p, &G, &B, nk, pass, cpsi, chpsi, T1, T2, p->d_vloc, nb, 0, max_ncol, max_nplane, st, nullptr, nullptr, nullptr};
-    rc = try_parts(fft2_batched_pass_p0, fft2_batched_pass_p1, fft2_batched_pass_p2, a, r1, r2);
+    rc = try_parts(fft2_batched_pass_p0, fft2_batched_pass_p1, fft2_batched_pass_p2, fft2_batched_pass_p3, a, r1, r2);
     phase_end(p, pass, st, 1);
     if (rc) { if (rc == DFT_ERR_UNSUPPORTED) set_error("batched FFT pass %d cannot be launched", pass); return rc; }
   }
@@ -1310,7 +1317,7 @@ int fft2_density(dft_plan *p, int ik, const double *psi, const double *wgt_dev, 
   phase_begin(p, 2, st);
   {
     Fft2PassArgs a = {p, &G, nullptr, 1, 2, nullptr, nullptr, T1, T2, nullptr, nb, 0, 0, 0, st, nullptr, wgt_dev, rho};
-    rc = try_parts(fft2_density_pass_p0, fft2_density_pass_p1, fft2_density_pass_p2, a, r1, r2);
+    rc = try_parts(fft2_density_pass_p0, fft2_density_pass_p1, fft2_density_pass_p2, fft2_density_pass_p3, a, r1, r2);
   }
   phase_end(p, 2, st, 1);
   if (rc == DFT_ERR_UNSUPPORTED) set_error("density kernel: tile does not fit (nplane = %d)", kp.nplane);
@@ -1331,7 +1338,7 @@ int fft2_launch(dft_plan *p, int ik, int pass, const double *psi, double *hpsi, 
   cplx *chpsi = reinterpret_cast<cplx *>(hpsi), *t1 = reinterpret_cast<cplx *>(T1), *t2 = reinterpret_cast<cplx *>(T2);
   const int hb = p->kp[ik].max_cols_per_plane;
   Fft2PassArgs a = {p, &G, nullptr, 1, pass, cpsi, chpsi, t1, t2, vpot, nb, hb, 0, 0, st, &X, nullptr, nullptr};
-  return try_parts(fft2_pass_p0, fft2_pass_p1, fft2_pass_p2, a, r1, r2);
+  return try_parts(fft2_pass_p0, fft2_pass_p1, fft2_pass_p2, fft2_pass_p3, a, r1, r2);
 }
 #endif   // FFT2_PART == 0
 

@@ -69,6 +69,7 @@ int spinor_apply(dft_plan *p, const double *psi, double *hpsi, int nband, cudaSt
   // one application with the 2 x 2 matrix in pass C where the five-pass register path serves the box
   bool fused = p->spinor_fused && p->fft_path != 1 && !((p->fft_path == 0 || p->fft_path == 3 || p->fft_path == 5) && fft_small_ok(p));
   for (int c = 0; c < 3 && fused; c++) fused = fft2_pair(p->n[c], nullptr, nullptr);
+  { int r1 = 0, r2 = 0; if (fused && fft2_pair(p->n[2], &r1, &r2) && r2 > 16) fused = false; }   // the 2 x 2 pass holds 16 lanes per slot row
   for (int ik = 0; ik < p->nkpt && fused; ik++) fused = p->kp[ik].runs_ok;
   if (loc && fused) {
     FftExtra X;

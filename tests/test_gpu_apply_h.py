@@ -135,6 +135,39 @@ def test_box_lengths_45_54_75_135(ngfft):
     plan.destroy()
 
 
+@pytest.mark.parametrize("ngfft", [(200, 20, 24), (20, 216, 24), (20, 24, 270), (288, 20, 300), (24, 320, 20), (162, 20, 324),
+                                   (20, 360, 24), (24, 20, 400)])
+def test_box_lengths_with_radices_18_and_20(ngfft):
+    """Register path for 162 = 9 x 18, 200 = 10 x 20, 216 = 12 x 18, 270 = 15 x 18, 288 = 16 x 18, 300 = 15 x 20,
+    320 = 16 x 20, 324 = 18 x 18, 360 = 18 x 20 and 400 = 20 x 20 on each axis (rows of more than 256 points take the plain
+    kernels instead of the TMA ring): all-terms H psi and the local term alone against the oracle, the register path
+    without the ring and the generic kernels too, the density, and two-component spinors (Pauli form where the z length
+    needs a radix above 16)."""
+    cfg, plan, sph = _setup("c0", ngfft=ngfft, nband=3)
+    psi = synth.gen_psi(cfg, [sph[0][2]])
+    for terms in (7, 2):
+        plan.set_option("terms", terms)
+        ref = oracle_apply(cfg, sph, psi, terms=terms, method=2)
+        for path in (0, 2, 1):
+            plan.set_option("fft_path", path)
+            err = band_rel_err(gpu_apply(plan, psi), ref)
+            assert err <= TOL, "%s terms=%d fft_path=%d: %.3e" % (ngfft, terms, path, err)
+    plan.set_option("fft_path", 0); plan.set_option("terms", 15)
+    w = np.linspace(0.5, 1.5, 3)[None]
+    rho = plan.accumulate_density(torch.as_tensor(psi, device="cuda"), w).cpu().numpy()
+    ref = oracle.density(cfg["ngfft"], sph[0][1], psi[0], w[0], method=2)
+    assert np.max(np.abs(rho - ref)) <= 1e-12 * ref.max()
+    v4, dspin = synth.spinor_inputs(cfg)
+    plan.set_vloc_spinor(torch.as_tensor(v4, device="cuda"))
+    plan.set_dij_spinor(dspin)
+    sp = synth.gen_psi(cfg, [sph[0][2]], nband=4).reshape(1, 2, 2, plan.mpw)
+    sref = oracle.apply_h_spinor(cfg, 0, *sph[0], sp[0], v4, dspin, method=2)
+    out = plan.apply_h_spinor(torch.as_tensor(sp, device="cuda").contiguous())
+    torch.cuda.synchronize()
+    assert band_rel_err(out.cpu().numpy(), sref[None]) <= TOL
+    plan.destroy()
+
+
 def test_box_without_two_stage_factorisation():
     """Box 10 x 20 x 27: 10 and 27 have no two-stage factorisation (generic kernels), 20 = 4 x 5 has, so the
     passes of one transform mix both kernel families."""

@@ -161,5 +161,6 @@ template <int S> struct Dft<12, S> { static DFT_HD void run(cplx *v) { Pfa<4, 3,
 template <int S> struct Dft<15, S> { static DFT_HD void run(cplx *v) { Pfa<3, 5, S>::run(v); } };
 template <int S> struct Dft<18, S> { static DFT_HD void run(cplx *v) { Pfa<2, 9, S>::run(v); } };
 template <int S> struct Dft<20, S> { static DFT_HD void run(cplx *v) { Pfa<4, 5, S>::run(v); } };
+template <int S> struct Dft<24, S> { static DFT_HD void run(cplx *v) { Pfa<3, 8, S>::run(v); } };
 
 }  // namespace dftb200

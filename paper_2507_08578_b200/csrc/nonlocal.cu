@@ -243,23 +243,37 @@ gemm1_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ C
 // ---------------------------------------------------------------- D_ij + split-K reduction
 // c'[ik][b][first_a + i] = sum_j D^a_ij sum_s part[ik][s][first_a + j][b];  one thread per (b, a, ik), b fastest
 constexpr int DIJ_MAXL = 16;
-__global__ void dij_kernel(const double2 *__restrict__ part, double2 *__restrict__ cpr, const double *__restrict__ dij,
-                           const int32_t *__restrict__ typat, const int32_t *__restrict__ nlmn,
-                           const int32_t *__restrict__ atom_first, int natom, int lmax, int nproj, int nband, int nsplit) {
-  int b = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y, ik = blockIdx.z;
-  if (b >= nband) return;
+// blockDim = (DIJ_BX bands, DIJ_YS): the split-K partials are summed by DIJ_YS groups of threads, group y taking the splits
+// y, y + DIJ_YS, ... (with a few dozen splits, one thread per band and 128 bands per CTA most of the chip was idle: 73 us at c1),
+// then added up in shared memory in the fixed order y = 0, 1, ...; group 0 applies D.
+constexpr int DIJ_YS = 4, DIJ_BX = 32;
+__global__ void __launch_bounds__(DIJ_BX * DIJ_YS)
+dij_kernel(const double2 *__restrict__ part, double2 *__restrict__ cpr, const double *__restrict__ dij,
+           const int32_t *__restrict__ typat, const int32_t *__restrict__ nlmn,
+           const int32_t *__restrict__ atom_first, int natom, int lmax, int nproj, int nband, int nsplit) {
+  __shared__ double2 red[DIJ_YS - 1][DIJ_MAXL][DIJ_BX];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int b = blockIdx.x * DIJ_BX + tx, a = blockIdx.y, ik = blockIdx.z;
+  const bool live = b < nband;
   int nl = nlmn[typat[a]], first = atom_first[a];
   double2 c[DIJ_MAXL];
   for (int jj = 0; jj < nl; jj++) c[jj] = make_double2(0.0, 0.0);
   // splits outer, projectors inner: the nl loads of one split are independent (fixed summation order per projector)
-  for (int s = 0; s < nsplit; s++) {
-    const double2 *src = part + ((size_t)(ik * nsplit + s) * nproj + first) * nband + b;
+  if (live)
+    for (int s = ty; s < nsplit; s += DIJ_YS) {
+      const double2 *src = part + ((size_t)(ik * nsplit + s) * nproj + first) * nband + b;
 #pragma unroll 4
-    for (int jj = 0; jj < nl; jj++) {
-      double2 v = src[(size_t)jj * nband];
-      c[jj].x += v.x; c[jj].y += v.y;
+      for (int jj = 0; jj < nl; jj++) {
+        double2 v = src[(size_t)jj * nband];
+        c[jj].x += v.x; c[jj].y += v.y;
+      }
     }
-  }
+  if (ty > 0)
+    for (int jj = 0; jj < nl; jj++) red[ty - 1][jj][tx] = c[jj];
+  __syncthreads();
+  if (ty > 0 || !live) return;
+  for (int y = 0; y < DIJ_YS - 1; y++)
+    for (int jj = 0; jj < nl; jj++) { const double2 v = red[y][jj][tx]; c[jj].x += v.x; c[jj].y += v.y; }
   double2 *dst = cpr + ((size_t)ik * nband + b) * nproj + first;
   if (!dij) {   // no D: the reduced projections <p|psi> themselves (dft_get_cprj)
     for (int ii = 0; ii < nl; ii++) dst[ii] = c[ii];
@@ -1402,7 +1416,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
         q1.part, reinterpret_cast<double2 *>(p->d_cprj), reinterpret_cast<const double2 *>(dspin), p->d_typat, p->d_nlmn,
         p->d_atom_first, p->lmax, nproj, nband, ns);
   else
-    dij_kernel<<<dim3((nband + 127) / 128, p->natom, nkpt), 128, 0, st>>>(
+    dij_kernel<<<dim3((nband + DIJ_BX - 1) / DIJ_BX, p->natom, nkpt), dim3(DIJ_BX, DIJ_YS), 0, st>>>(
         q1.part, reinterpret_cast<double2 *>(cprj_out ? cprj_out : p->d_cprj), cprj_out ? nullptr : dmat, p->d_typat, p->d_nlmn,
         p->d_atom_first, p->natom, p->lmax, nproj, nband, ns);
   phase_end(p, 6, st, 1);
@@ -1439,7 +1453,7 @@ int nonlocal_apply(dft_plan *p, const double *psi, double *hpsi, int nband, bool
     // second output from the SAME projections (dft_apply_hs): S psi = psi + sum |p> s <p|psi>.  The split-K partials of
     // GEMM-1 are still there; reduce them again with s_ij into c' and back-project with a unit diagonal.
     phase_begin(p, 6, st);
-    dij_kernel<<<dim3((nband + 127) / 128, p->natom, nkpt), 128, 0, st>>>(q1.part, reinterpret_cast<double2 *>(p->d_cprj), p->d_sij, p->d_typat,
+    dij_kernel<<<dim3((nband + DIJ_BX - 1) / DIJ_BX, p->natom, nkpt), dim3(DIJ_BX, DIJ_YS), 0, st>>>(q1.part, reinterpret_cast<double2 *>(p->d_cprj), p->d_sij, p->d_typat,
                                                                           p->d_nlmn, p->d_atom_first, p->natom, p->lmax, nproj, nband, ns);
     phase_end(p, 6, st, 1);
     q2.accumulate = 0; q2.with_kin = 1; q2.kin = p->d_oneptr; q2.hpsi = reinterpret_cast<double2 *>(spsi);

@@ -139,6 +139,7 @@ struct dft_plan {
   int ldf = 0;                                       // row length of d_fytab (mpw rounded up to 8)
   int proj_mode = 0;                                 // 0 = materialised table (GEMMs on P), 1 = factorised P = FY . S
   int fft_c_split = 2;                               // pass C (16-line tiles): two barrier domains per CTA (fft2_c_ring2_kernel): 0 = never, 1 = wherever possible, 2 = where both radices are >= 12
+  int gemm2_merge = 1;                               // Strassen path: the seven back-projection products in one launch
   int nl_tiny = 1;                                   // tiny cells: the whole non-local term in one launch (nl_tiny_kernel), 0 = always the GEMM kernels
   bool skip_table_at_create = false;                 // dft_plan_create_opts(proj_mode = 1): never allocate the materialised table
   double *d_ptab = nullptr;                          // [nkpt][nproj][mpw] complex, zero padded beyond npw_k

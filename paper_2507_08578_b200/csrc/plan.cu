@@ -595,6 +595,10 @@ int dft_plan_set_option(dft_plan *p, const char *key, int64_t value) {
     if (value < 0 || value > 2) { set_error("fft_c_split = %lld outside 0..2", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->fft_c_split = (int)value; return DFT_OK;
   }
+  if (!strcmp(key, "gemm2_merge")) {
+    if (value < 0 || value > 1) { set_error("gemm2_merge = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
+    p->gemm2_merge = (int)value; return DFT_OK;
+  }
   if (!strcmp(key, "nl_tiny")) {
     if (value < 0 || value > 1) { set_error("nl_tiny = %lld outside 0..1", (long long)value); return DFT_ERR_INVALID_ARG; }
     p->nl_tiny = (int)value; return DFT_OK;

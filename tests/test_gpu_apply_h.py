@@ -473,7 +473,12 @@ def test_strassen_level_on_the_real_gemms(name, nband):
         err = band_rel_err(gpu_apply(plan, psi), oracle_apply(cfg, sph, psi, terms=terms, method=m))
         assert err <= TOL, "%s nband=%d terms=%d: %.3e" % (name, nband, terms, err)
     plan.set_option("terms", 7)
-    assert plan.last_launches() > 20                         # 14 GEMM launches + combinations: the Strassen path did run
+    assert plan.last_launches() > 12                         # 7 + 1 GEMM launches + combinations: the Strassen path did run
+    merged = gpu_apply(plan, psi)
+    plan.set_option("gemm2_merge", 0)                        # the seven back-projection products as seven launches
+    separate = gpu_apply(plan, psi)
+    assert plan.last_launches() > 20 and np.array_equal(merged, separate)
+    plan.set_option("gemm2_merge", 1)
     sij = np.random.default_rng(4).standard_normal(cfg["dij"].shape) * 0.3
     sij = 0.5 * (sij + sij.transpose(0, 2, 1))
     plan.set_sij(sij)

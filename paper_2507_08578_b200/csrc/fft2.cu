@@ -880,7 +880,7 @@ fft2_density_kernel(const __grid_constant__ CUtensorMap mapT2, Fft2Geom G, const
 #define FFT2_PAIRS_1(X) X(6, 8) X(5, 10) X(6, 10) X(8, 8) X(8, 9) X(8, 10) X(9, 9) X(9, 10) X(8, 12) X(8, 16) X(5, 9) X(6, 9)
 #define FFT2_PAIRS_2(X) X(10, 10) X(9, 12) X(10, 12) X(12, 12) X(10, 15) X(10, 16) X(12, 16) X(15, 15) X(15, 16) X(16, 16) X(5, 15) X(9, 15)
 // radices 18 = 2 x 9 and 20 = 4 x 5 (prime-factor codelets): 162, 200, 216, 270, 288, 300, 320, 324, 360, 400
-#define FFT2_PAIRS_3(X) X(9, 18) X(10, 20) X(12, 18) X(15, 18) X(16, 18) X(15, 20) X(16, 20) X(18, 18) X(18, 20) X(20, 20) X(16, 24) X(18, 24) X(20, 24)
+#define FFT2_PAIRS_3(X) X(9, 18) X(10, 20) X(12, 18) X(15, 18) X(16, 18) X(15, 20) X(16, 20) X(18, 18) X(18, 20) X(20, 20) X(16, 24) X(18, 24) X(20, 24) X(24, 24)
 #define FFT2_PAIRS_ALL(X) FFT2_PAIRS_0(X) FFT2_PAIRS_1(X) FFT2_PAIRS_2(X) FFT2_PAIRS_3(X)
 #if FFT2_PART == 0
 #define FFT2_PAIRS(X) FFT2_PAIRS_0(X)

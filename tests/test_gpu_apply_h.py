@@ -136,10 +136,10 @@ def test_box_lengths_45_54_75_135(ngfft):
 
 
 @pytest.mark.parametrize("ngfft", [(200, 20, 24), (20, 216, 24), (20, 24, 270), (288, 20, 300), (24, 320, 20), (162, 20, 324),
-                                   (20, 360, 24), (24, 20, 400), (384, 20, 24), (20, 432, 24), (24, 20, 480)])
+                                   (20, 360, 24), (24, 20, 400), (384, 20, 24), (20, 432, 24), (24, 20, 480), (20, 576, 24)])
 def test_box_lengths_with_radices_18_and_20(ngfft):
     """Register path for 162 = 9 x 18, 200 = 10 x 20, 216 = 12 x 18, 270 = 15 x 18, 288 = 16 x 18, 300 = 15 x 20,
-    320 = 16 x 20, 324 = 18 x 18, 360 = 18 x 20, 400 = 20 x 20 and, with the radix 24 = 3 x 8, 384, 432 and 480 on each axis (rows of more than 256 points take the plain
+    320 = 16 x 20, 324 = 18 x 18, 360 = 18 x 20, 400 = 20 x 20 and, with the radix 24 = 3 x 8, 384, 432, 480 and 576 on each axis (rows of more than 256 points take the plain
     kernels instead of the TMA ring): all-terms H psi and the local term alone against the oracle, the register path
     without the ring and the generic kernels too, the density, and two-component spinors (Pauli form where the z length
     needs a radix above 16)."""
